@@ -1,0 +1,134 @@
+"""Pins for the oracle's KDK leapfrog ("second-order Velocity-Verlet
+integrator with ... fixed time steps"; L43 step 2 backward integration).
+
+Closed forms: two-body circular orbit and Kepler ellipse (period, energy), second-order
+convergence (error ratio 4 when dt halves), energy error ~ dt^2, time reversibility,
+momentum and L_z conservation in the axisymmetric Milky-Way potential.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2511_22468_b200 import workloads as W
+
+
+def _two_body_circular(eps):
+    m1, m2, d, G = 0.7, 0.3, 1.0, 1.0
+    M = m1 + m2
+    w = np.sqrt(G * M / (d * d + eps * eps) ** 1.5)     # softened closed form
+    x1, x2 = -m2 / M * d, m1 / M * d
+    posm = np.array([[x1, 0, 0, m1], [x2, 0, 0, m2]])
+    vel = np.array([[0, w * x1, 0], [0, w * x2, 0]])
+    return posm, vel, G, 2 * np.pi / w
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.3])
+def test_two_body_circular_orbit_closes_with_second_order_error(eps):
+    posm, vel, G, T = _two_body_circular(eps)
+    errs = []
+    for n in (1000, 2000, 4000):
+        p, v, _ = O.leapfrog_kdk(posm, vel, G, eps, T / n, n)
+        sep = np.linalg.norm(p[1, :3] - p[0, :3])
+        # after a whole period the separation returns: to roundoff for the pure 1/r^2 force,
+        # to O(dt^2) once softening changes the force law's radial dependence
+        assert abs(sep - 1.0) <= (1e-12 if eps == 0.0 else 1e-5 * (1000 / n) ** 2)
+        errs.append(np.linalg.norm(p[:, :3] - posm[:, :3], axis=1).max())
+        L0, L1 = O.angular_momentum(posm, vel), O.angular_momentum(p, v)
+        assert abs(L1[2] - L0[2]) <= 1e-14 * abs(L0[2])
+    assert errs[0] < 1e-4
+    assert 3.9 < errs[0] / errs[1] < 4.1 and 3.9 < errs[1] / errs[2] < 4.1
+
+
+def test_kepler_ellipse_period_energy_and_order():
+    G, m1, m2, sma, e = 1.0, 1.0, 1e-3, 1.0, 0.5
+    M = m1 + m2
+    T = 2 * np.pi * np.sqrt(sma ** 3 / (G * M))
+    rp = sma * (1 - e)
+    vp = np.sqrt(G * M * (1 + e) / (sma * (1 - e)))     # vis-viva at pericentre
+    posm = np.array([[-m2 / M * rp, 0, 0, m1], [m1 / M * rp, 0, 0, m2]])
+    vel = np.array([[0, -m2 / M * vp, 0], [0, m1 / M * vp, 0]])
+    E = O.total_energy(posm, vel, G, 0.0)
+    assert abs(E - (-G * m1 * m2 / (2 * sma))) <= 1e-15
+    errs = []
+    for n in (2000, 4000, 8000):
+        p, v, _ = O.leapfrog_kdk(posm, vel, G, 0.0, T / n, n)
+        errs.append(np.linalg.norm(p[1, :3] - posm[1, :3]))
+        assert abs(O.total_energy(p, v, G, 0.0) - E) <= 1e-6 * abs(E)
+    assert errs[0] < 1e-3
+    assert 3.9 < errs[0] / errs[1] < 4.1 and 3.9 < errs[1] / errs[2] < 4.1
+
+
+def test_single_step_matches_hand_expansion():
+    """One KDK step of a particle in a uniform-direction softened two-body field, by hand:
+    v_half = v + a(x) dt/2; x' = x + v_half dt; v' = v_half + a(x') dt/2."""
+    posm = np.array([[0, 0, 0, 1.0], [2.0, 0, 0, 1e-30]])
+    vel = np.array([[0, 0, 0.0], [0, 0.5, 0]])
+    G, eps, dt = 1.0, 0.0, 0.1
+    a0 = np.array([-1.0 / 4.0, 0, 0])
+    vh = vel[1] + a0 * dt / 2
+    x1 = posm[1, :3] + vh * dt
+    a1 = -x1 / np.linalg.norm(x1) ** 3
+    v1 = vh + a1 * dt / 2
+    p, v, acc = O.leapfrog_kdk(posm, vel, G, eps, dt, 1)
+    np.testing.assert_allclose(p[1, :3], x1, rtol=1e-15)
+    np.testing.assert_allclose(v[1], v1, rtol=1e-15)
+    np.testing.assert_allclose(acc[1], a1, rtol=1e-15)
+    assert p[1, 3] == posm[1, 3]
+
+
+def test_energy_error_scales_as_dt_squared_and_momenta_conserved():
+    cfg = W.CONFIGS[0]
+    posm, vel = W.make_state(cfg, n=256)
+    E0 = O.total_energy(posm, vel, cfg.G, cfg.eps)
+    P0, L0 = O.linear_momentum(posm, vel), O.angular_momentum(posm, vel)
+    dE = []
+    for dt in (2e-3, 1e-3, 5e-4):
+        p, v, _ = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, dt, int(round(0.1 / dt)))
+        dE.append(abs(O.total_energy(p, v, cfg.G, cfg.eps) - E0) / abs(E0))
+        assert np.abs(O.linear_momentum(p, v) - P0).max() <= 1e-15
+        assert np.abs(O.angular_momentum(p, v) - L0).max() <= 1e-15
+    assert dE[0] < 1e-6
+    assert 3.0 < dE[0] / dE[1] < 5.0 and 3.0 < dE[1] / dE[2] < 5.0
+
+
+def test_time_reversibility_dt_negation_and_velocity_flip():
+    cfg = W.CONFIGS[0]
+    posm, vel = W.make_state(cfg, n=256)
+    p, v, _ = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, 1e-3, 100)
+    pb, vb, _ = O.leapfrog_kdk(p, v, cfg.G, cfg.eps, -1e-3, 100)
+    assert np.abs(pb[:, :3] - posm[:, :3]).max() <= 1e-13
+    assert np.abs(vb - vel).max() <= 1e-13
+    pf, vf, _ = O.leapfrog_kdk(p, -v, cfg.G, cfg.eps, 1e-3, 100)
+    assert np.abs(pf[:, :3] - posm[:, :3]).max() <= 1e-13
+    assert np.abs(vf + vel).max() <= 1e-13
+
+
+def test_chained_calls_equal_one_long_call_and_zero_steps_is_identity():
+    cfg = W.CONFIGS[0]
+    posm, vel = W.make_state(cfg, n=64)
+    p1, v1, _ = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, 1e-3, 3)
+    p2, v2, _ = O.leapfrog_kdk(p1, v1, cfg.G, cfg.eps, 1e-3, 4)
+    p7, v7, _ = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, 1e-3, 7)
+    assert np.array_equal(p2, p7) and np.array_equal(v2, v7)
+    p0, v0, a0 = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, 1e-3, 0)
+    assert np.array_equal(p0, posm) and np.array_equal(v0, vel)
+    np.testing.assert_array_equal(a0, O.total_accel(posm, cfg.G, cfg.eps, None))
+
+
+def test_milky_way_orbit_conserves_lz_and_energy_order():
+    cfg = W.CONFIGS[1]
+    posm, vel = W.make_state(cfg, n=128)
+    pot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    E0 = O.total_energy(posm, vel, cfg.G, cfg.eps, pot)
+    Lz0 = O.angular_momentum(posm, vel)[2]
+    dE = []
+    for dt in (1.0, 0.5, 0.25):
+        p, v, _ = O.leapfrog_kdk(posm, vel, cfg.G, cfg.eps, dt, int(round(200 / dt)), pot)
+        assert abs(O.angular_momentum(p, v)[2] - Lz0) <= 1e-13 * abs(Lz0)
+        dE.append(abs(O.total_energy(p, v, cfg.G, cfg.eps, pot) - E0) / abs(E0))
+    assert dE[0] < 1e-4 and dE[2] < dE[1] < dE[0]
+    # the cluster's centre of mass follows the single-particle orbit from the same start
+    com = O.centre_of_mass(p)
+    one = np.array([[*cfg.centre, cfg.M]])
+    p1, _, _ = O.leapfrog_kdk(one, np.array([cfg.velocity]), cfg.G, cfg.eps, 0.25, 800, pot)
+    assert np.linalg.norm(com - p1[0, :3]) <= 5e-3

@@ -1,0 +1,126 @@
+"""Pins for the oracle's NFW + Miyamoto-Nagai terms.
+
+The paper names the components but prints no formula; the pins are mathematics:
+acceleration = -grad(potential) by central differences, Poisson's equation against the
+textbook densities (fixes the NFW normalisation, reading R10), circular speed,
+in-plane MN closed form, spherical symmetry / axisymmetry.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2511_22468_b200 import workloads as W
+
+G = W.G_KPC_MSUN_MYR
+NFW = O.Potential.make(nfw=W.NFW_MW)
+MN = O.Potential.make(mn=W.MN_MW)
+BOTH = O.Potential.make(nfw=W.NFW_MW, mn=W.MN_MW)
+POINTS = np.array([[12.4, 0.0, 1.5], [-10.0, -4.0, 6.0], [8.0, 0.0, 0.0], [0.3, -0.2, 0.05], [1.0, 2.0, -3.0]])
+
+
+def _posm(pts):
+    pts = np.atleast_2d(np.asarray(pts, dtype=np.float64))
+    return np.concatenate([pts, np.ones((pts.shape[0], 1))], axis=1)
+
+
+def _fd_grad(pot, x, h):
+    g = np.zeros(3)
+    for k in range(3):
+        p, q = np.array(x, dtype=np.float64), np.array(x, dtype=np.float64)
+        p[k] += h
+        q[k] -= h
+        g[k] = (O.ext_potential(_posm(p), G, pot)[0] - O.ext_potential(_posm(q), G, pot)[0]) / (2 * h)
+    return g
+
+
+@pytest.mark.parametrize("pot", [NFW, MN, BOTH], ids=["nfw", "mn", "both"])
+def test_acceleration_is_minus_gradient_of_potential(pot):
+    for x in POINTS:
+        a = O.ext_accel(_posm(x), G, pot)[0]
+        g = _fd_grad(pot, x, 1e-5 * np.linalg.norm(x))   # truncation ~1e-10, rounding ~1e-11
+        assert np.linalg.norm(a + g) <= 1e-8 * np.linalg.norm(a)
+
+
+def _fd_div(pot, x, h):
+    d = 0.0
+    for k in range(3):
+        p, q = np.array(x, dtype=np.float64), np.array(x, dtype=np.float64)
+        p[k] += h
+        q[k] -= h
+        d += (O.ext_accel(_posm(p), G, pot)[0][k] - O.ext_accel(_posm(q), G, pot)[0][k]) / (2 * h)
+    return d
+
+
+def test_poisson_nfw_fixes_the_normalisation():
+    """div a = -4 pi G rho with rho_NFW = M_s / (4 pi r_s^3) / (c (1+c)^2): M_s = 4 pi rho_0 r_s^3."""
+    Ms, rs = W.NFW_MW
+    for x in POINTS:
+        c = np.linalg.norm(x) / rs
+        rho = Ms / (4 * np.pi * rs ** 3) / (c * (1 + c) ** 2)
+        assert abs(_fd_div(NFW, x, 1e-4 * np.linalg.norm(x)) + 4 * np.pi * G * rho) <= 1e-6 * 4 * np.pi * G * rho
+
+
+def test_poisson_mn():
+    M, a, b = W.MN_MW
+    for x in POINTS:
+        R2, B = x[0] ** 2 + x[1] ** 2, np.sqrt(x[2] ** 2 + b * b)
+        rho = (b * b * M / (4 * np.pi)) * (a * R2 + (a + 3 * B) * (a + B) ** 2) / ((R2 + (a + B) ** 2) ** 2.5 * B ** 3)
+        assert abs(_fd_div(MN, x, 1e-5 * np.linalg.norm(x)) + 4 * np.pi * G * rho) <= 1e-6 * 4 * np.pi * G * rho
+
+
+def test_nfw_circular_speed_and_symmetry():
+    Ms, rs = W.NFW_MW
+    r = 12.49
+    c = r / rs
+    vc2 = G * Ms * (np.log(1 + c) - c / (1 + c)) / r
+    assert abs(np.sqrt(vc2) - 0.223399) <= 2e-6         # kpc/Myr (218.44 km/s), SURVEY 8c
+    rng = np.random.Generator(np.random.PCG64(4))
+    for _ in range(5):
+        u = rng.normal(size=3)
+        u /= np.linalg.norm(u)
+        a = O.ext_accel(_posm(r * u), G, NFW)[0]
+        np.testing.assert_allclose(a, -vc2 / r * u, rtol=1e-13, atol=1e-20)
+
+
+def test_mn_in_plane_closed_form_and_axisymmetry():
+    M, a, b = W.MN_MW
+    for R in (0.5, 3.0, 8.0, 20.0):
+        expect = -G * M * R / (R * R + (a + b) ** 2) ** 1.5
+        for phi in (0.0, 0.7, 2.9):
+            x = np.array([R * np.cos(phi), R * np.sin(phi), 0.0])
+            acc = O.ext_accel(_posm(x), G, MN)[0]
+            np.testing.assert_allclose(acc[:2], expect * x[:2] / R, rtol=1e-13, atol=1e-22)
+            assert acc[2] == 0.0
+    up = O.ext_accel(_posm([3.0, 1.0, 0.4]), G, MN)[0]
+    dn = O.ext_accel(_posm([3.0, 1.0, -0.4]), G, MN)[0]
+    np.testing.assert_allclose(up * [1, 1, -1], dn, rtol=1e-15)
+
+
+def test_far_field_is_keplerian_for_mn():
+    M, a, b = W.MN_MW
+    x = np.array([3.0e4, 4.0e4, 0.0])
+    acc = O.ext_accel(_posm(x), G, MN)[0]
+    r = np.linalg.norm(x)
+    np.testing.assert_allclose(acc, -G * M * x / r ** 3, rtol=1e-7, atol=1e-30)
+
+
+def test_sum_of_terms_and_disabled_terms():
+    p = _posm(POINTS)
+    np.testing.assert_allclose(O.ext_accel(p, G, BOTH), O.ext_accel(p, G, NFW) + O.ext_accel(p, G, MN), rtol=1e-15)
+    assert np.all(O.ext_accel(p, G, None) == 0)
+    assert np.all(O.ext_accel(p, G, O.Potential.make()) == 0)
+    assert np.all(O.ext_accel(_posm([0, 0, 0]), G, NFW) == 0)        # reading R12
+
+
+def test_transcription_crosscheck_against_survey_values():
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "ext_accel_mw.txt"))
+            if l.strip() and not l.startswith("#")]
+    for row in rows:
+        v = np.array([float(t) for t in row])
+        a_nfw = O.ext_accel(_posm(v[:3]), G, NFW)[0]
+        a_mn = O.ext_accel(_posm(v[:3]), G, MN)[0]
+        for got, want in ((a_nfw, v[3:6]), (a_mn, v[6:9])):
+            ok = ~np.isnan(want)
+            np.testing.assert_allclose(got[ok], want[ok], rtol=1e-12, atol=1e-18)
