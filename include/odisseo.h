@@ -1,0 +1,156 @@
+/*
+ * odisseo.h -- C ABI of the B200-native hot path of ODISSEO's direct N-body solver
+ * (arxiv 2511.22468).  PAPER.md = the paper's text; citations are PAPER.md line + section.
+ *
+ * What the library computes
+ *   pair   a_i = G * sum_j m_j (x_j - x_i) / (|x_j - x_i|^2 + eps^2)^{3/2}
+ *          "direct pairwise force computations with softening, without a tree or
+ *          fast-multipole algorithm ... exact forces (up to the softening scale)"
+ *          (section 1; formula: BASELINE.json north_star).
+ *   ext    a_NFW(x) = -G M_s [ln(1+r/r_s) - (r/r_s)/(1+r/r_s)] x / r^3
+ *          a_MN(x)  = -G M (x, y, z (a+B)/B) / D^3,  B = sqrt(z^2+b^2), D^2 = x^2+y^2+(a+B)^2
+ *          NFW halo + Miyamoto-Nagai disk (PAPER.md:L9 Abstract; L45 section 2.2.1; L63 section 2.2.2).
+ *   kdk    a <- a(x); repeat nsteps: v += a dt/2; x += v dt; a <- a(x); v += a dt/2
+ *          "second-order Velocity-Verlet integrator with ... fixed time steps".
+ *
+ * Conventions (all entry points)
+ *   - Every pointer named d_* is a DEVICE pointer, h_* a HOST pointer.  The caller owns
+ *     every buffer; the library allocates no device memory (scratch comes in as
+ *     `d_workspace`; a plan owns only its CUDA graph objects).
+ *   - Particle records are 4 scalars: posm = {x, y, z, m}; vel = {vx, vy, vz, pad};
+ *     acc = {ax, ay, az, pad}.  fp32 records are 16 bytes and must be 16-byte aligned,
+ *     fp64 records are 32 bytes and must be 32-byte aligned.  posm[i].m is read-only and
+ *     is preserved by the integrator.  Pad lanes of outputs are written as 0.
+ *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  No hidden synchronisation, no host-side reads of results.
+ *   - posm and acc (and vel) must not alias or overlap: ODISSEO_ERR_ARG.
+ *   - Errors are return codes, never exceptions or aborts: NULL pointer -> ERR_NULL,
+ *     misaligned pointer -> ERR_ALIGN, n < 0, nsteps < 0, eps <= 0 (the kernels include the
+ *     self term, which is exactly 0 only when eps > 0), non-finite scalar, enabled MN term
+ *     with b <= 0 or enabled NFW term with r_s <= 0 -> ERR_ARG, workspace too small ->
+ *     ERR_WORKSPACE, device is not compute capability 10.x -> ERR_ARCH, CUDA failure ->
+ *     ERR_CUDA (code in odisseo_last_cuda_error()).  n == 0 or nsteps == 0 is an OK no-op
+ *     (nsteps == 0 with acc_valid == 0 still evaluates acc).  Inputs are not screened for
+ *     NaN/Inf particles; they propagate.
+ *   - There is no CPU fallback: without a B200 every compute call fails with ERR_ARCH/ERR_CUDA.
+ *   - Results are bit-reproducible run to run for fixed (n, device SM count): partial sums
+ *     are combined in a fixed order, never with atomics.
+ */
+#ifndef ODISSEO_H
+#define ODISSEO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    ODISSEO_OK = 0,
+    ODISSEO_ERR_NULL = 1,
+    ODISSEO_ERR_ALIGN = 2,
+    ODISSEO_ERR_ARG = 3,
+    ODISSEO_ERR_WORKSPACE = 4,
+    ODISSEO_ERR_ARCH = 5,
+    ODISSEO_ERR_CUDA = 6
+} odisseo_status;
+
+/* NFW: Phi = -G M_s ln(1 + r/r_s) / r, i.e. M_s = 4 pi rho_0 r_s^3 (reading R10).
+ * M_s <= 0 disables the term.  At r = 0 the acceleration is defined as 0. */
+typedef struct { double M_s, r_s; } odisseo_nfw;
+/* Miyamoto-Nagai: Phi = -G M / sqrt(R^2 + (a + sqrt(z^2 + b^2))^2).  M <= 0 disables; b > 0. */
+typedef struct { double M, a, b; } odisseo_mn;
+/* A NULL odisseo_potential pointer means "no external potential" (config 0). HOST struct. */
+typedef struct { odisseo_nfw nfw; odisseo_mn mn; } odisseo_potential;
+
+/* Library version string, e.g. "odisseo-b200 0.1 (sm_100a)". Never NULL. */
+const char *odisseo_version(void);
+const char *odisseo_status_string(odisseo_status s);
+/* cudaError_t value of the most recent ODISSEO_ERR_CUDA on this thread (0 if none). */
+int odisseo_last_cuda_error(void);
+
+/* Upper bound, in bytes, of the device scratch any pair/leapfrog call on n particles
+ * needs (packed source tiles + fixed-order partial sums).  is_f64 != 0 for the fp64 calls.
+ * Returns 0 for n <= 0.  Pure host arithmetic; needs no GPU. */
+size_t odisseo_workspace_bytes(int64_t n, int is_f64);
+
+/* Pair acceleration, fp32.
+ *   d_posm [n][4] float in, d_acc [n][4] float out = G * sum_j ... (pad lane 0).
+ * Sum over ALL j including j == i (exactly 0 for eps > 0).  Per-tile fp32 partial sums are
+ * promoted to fp64 and combined in fixed order, then scaled by G and rounded once. */
+odisseo_status odisseo_pair_accel_f32(const float *d_posm, float *d_acc, int64_t n,
+                                      float G, float eps,
+                                      void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Same in fp64: d_posm [n][4] double (32-byte aligned), d_acc [n][4] double. */
+odisseo_status odisseo_pair_accel_f64(const double *d_posm, double *d_acc, int64_t n,
+                                      double G, double eps,
+                                      void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Structure-of-arrays face of the fp32 pair call: seven length-n float arrays (4-byte
+ * aligned).  Packs into the workspace, runs the same kernel, unpacks.  Workspace must be
+ * odisseo_workspace_bytes(n, 0) + 32 * n + 512 bytes, 256-byte aligned. */
+odisseo_status odisseo_pair_accel_soa_f32(const float *d_x, const float *d_y, const float *d_z,
+                                          const float *d_m, float *d_ax, float *d_ay, float *d_az,
+                                          int64_t n, float G, float eps,
+                                          void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* External acceleration a_NFW + a_MN.
+ * accumulate == 0: d_acc = a_ext (pad 0); accumulate != 0: d_acc.xyz += a_ext.
+ * pot == NULL or both terms disabled: zeros / unchanged.  `pot` is read on the host during
+ * the call (G*M_s, G*M, 1/r_s are combined in double there, then rounded once). */
+odisseo_status odisseo_ext_accel_f32(const float *d_posm, float *d_acc, int64_t n, float G,
+                                     const odisseo_potential *pot, int accumulate, void *stream);
+odisseo_status odisseo_ext_accel_f64(const double *d_posm, double *d_acc, int64_t n, double G,
+                                     const odisseo_potential *pot, int accumulate, void *stream);
+
+/* nsteps kick-drift-kick steps in place.
+ *   d_posm, d_vel in/out; d_acc in/out holds the PAIR-ONLY acceleration a_pair(x):
+ *   acc_valid != 0 promises d_acc == a_pair(d_posm) on entry (as left by a previous call),
+ *   which skips the initial evaluation; on exit d_acc == a_pair(x_final), x and v are
+ *   synchronised at t0 + nsteps*dt.  Chained calls are bit-identical to one long call.
+ * The external acceleration is recomputed from x inside the kick kernels.  dt may be
+ * negative or zero (backward integration, PAPER.md:L43 step 2).  One pair evaluation per
+ * step (+1 at the start unless acc_valid).  The per-step launch sequence is captured
+ * once in a CUDA graph and replayed. */
+odisseo_status odisseo_leapfrog_kdk_f32(float *d_posm, float *d_vel, float *d_acc, int acc_valid,
+                                        int64_t n, float G, float eps, float dt, int64_t nsteps,
+                                        const odisseo_potential *pot,
+                                        void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_f64(double *d_posm, double *d_vel, double *d_acc, int acc_valid,
+                                        int64_t n, double G, double eps, double dt, int64_t nsteps,
+                                        const odisseo_potential *pot,
+                                        void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Host-buffer face of the leapfrog (end-to-end path): copies h_posm, h_vel [n][4] to the
+ * device, runs nsteps KDK steps, copies posm, vel and (if h_acc != NULL) the pair-only
+ * acceleration back.  All copies are cudaMemcpyAsync on `stream`; host buffers should be
+ * pinned for true asynchrony and must stay valid until the stream is synchronised.
+ * d_workspace must hold odisseo_workspace_bytes(n, is_f64) + 3 state arrays
+ * (3 * n * 16 bytes fp32, 3 * n * 32 bytes fp64) + 768 bytes, 256-byte aligned. */
+odisseo_status odisseo_leapfrog_kdk_host_f32(float *h_posm, float *h_vel, float *h_acc,
+                                             int64_t n, float G, float eps, float dt, int64_t nsteps,
+                                             const odisseo_potential *pot,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_host_f64(double *h_posm, double *h_vel, double *h_acc,
+                                             int64_t n, double G, double eps, double dt, int64_t nsteps,
+                                             const odisseo_potential *pot,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Description of the launch plan the library would use for n particles on the current
+ * device (host arithmetic + one device-attribute query): fills out[0..7] with
+ * {i_bodies_per_thread, threads_per_cta, tile_records, persistent_ctas, i_blocks,
+ *  j_tiles, partial_slots, kernels_per_step}.  For tests, bench.py and DESIGN.md. */
+odisseo_status odisseo_describe_plan(int64_t n, int is_f64, int64_t out[8]);
+/* Same for a hypothetical device with num_sms SMs: pure host arithmetic, needs no GPU. */
+odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8]);
+/* Stream-K bookkeeping exactly as the kernels compute it (SURVEY.md 8a row a1'), for host
+ * tests: out = {CTA that owns work unit u, first unit of CTA c, one past the last unit of CTA c}
+ * where units number the (i-block, j-tile) pairs u = b * j_tiles + t.  Pure host arithmetic. */
+odisseo_status odisseo_plan_probe(int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[3]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ODISSEO_H */

@@ -1,0 +1,216 @@
+"""Thin ctypes binding of include/odisseo.h: argument marshalling only.
+
+Every step of the path runs in the CUDA library; PyTorch supplies device memory and
+streams.  There is no CPU fallback: a missing library or a non-zero status raises.
+Function names mirror the C ABI without the ``odisseo_`` prefix and precision suffix
+(the dtype of the tensors selects ``_f32`` / ``_f64``).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libodisseo_b200.so")
+_lib = None
+
+STATUS = {0: "OK", 1: "ERR_NULL", 2: "ERR_ALIGN", 3: "ERR_ARG", 4: "ERR_WORKSPACE", 5: "ERR_ARCH", 6: "ERR_CUDA"}
+
+EXPORTS = [
+    "odisseo_version", "odisseo_status_string", "odisseo_last_cuda_error", "odisseo_workspace_bytes",
+    "odisseo_pair_accel_f32", "odisseo_pair_accel_f64", "odisseo_pair_accel_soa_f32",
+    "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
+    "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
+    "odisseo_describe_plan_for", "odisseo_plan_probe",
+]
+
+
+class OdisseoError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        lib = _lib
+        detail = lib.odisseo_status_string(status).decode() if lib else "?"
+        cuda = lib.odisseo_last_cuda_error() if (lib and status == 6) else 0
+        super().__init__("%s failed: %s (%s)%s" % (where, STATUS.get(status, status), detail,
+                                                    " cudaError=%d" % cuda if cuda else ""))
+
+
+class _NFW(ctypes.Structure):
+    _fields_ = [("M_s", ctypes.c_double), ("r_s", ctypes.c_double)]
+
+
+class _MN(ctypes.Structure):
+    _fields_ = [("M", ctypes.c_double), ("a", ctypes.c_double), ("b", ctypes.c_double)]
+
+
+class Potential(ctypes.Structure):
+    """odisseo_potential: NFW{M_s, r_s} + MN{M, a, b}; a mass <= 0 disables the term."""
+    _fields_ = [("nfw", _NFW), ("mn", _MN)]
+
+    @classmethod
+    def make(cls, nfw: Optional[Sequence[float]] = None, mn: Optional[Sequence[float]] = None):
+        p = cls()
+        p.nfw = _NFW(*(nfw if nfw else (0.0, 1.0)))
+        p.mn = _MN(*(mn if mn else (0.0, 1.0, 1.0)))
+        return p
+
+
+def lib():
+    """Load the C-ABI library; fail loudly when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("CUDA library %s is missing: run `python -m paper_2511_22468_b200.build` "
+                               "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, sz, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
+        f, d = ctypes.c_float, ctypes.c_double
+        L.odisseo_version.restype = ctypes.c_char_p
+        L.odisseo_status_string.restype = ctypes.c_char_p
+        L.odisseo_status_string.argtypes = [ci]
+        L.odisseo_last_cuda_error.restype = ci
+        L.odisseo_workspace_bytes.restype = sz
+        L.odisseo_workspace_bytes.argtypes = [i64, ci]
+        for suffix, sc in (("f32", f), ("f64", d)):
+            getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
+            getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
+            getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+        L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
+        L.odisseo_describe_plan.argtypes = [i64, ci, vp]
+        L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
+        L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        _lib = L
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise OdisseoError(status, where)
+
+
+def _suffix(t: torch.Tensor) -> str:
+    if t.dtype == torch.float32:
+        return "f32"
+    if t.dtype == torch.float64:
+        return "f64"
+    raise TypeError("expected float32 or float64 tensors, got %s" % t.dtype)
+
+
+def _rec(t: torch.Tensor, name: str, n: Optional[int] = None, cuda: bool = True) -> int:
+    if t.dim() != 2 or t.shape[1] != 4 or not t.is_contiguous():
+        raise ValueError("%s must be a contiguous [n, 4] tensor" % name)
+    if cuda and not t.is_cuda:
+        raise ValueError("%s must be a CUDA tensor (no CPU fallback)" % name)
+    if n is not None and t.shape[0] != n:
+        raise ValueError("%s has %d records, expected %d" % (name, t.shape[0], n))
+    return t.shape[0]
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _pot(pot: Optional[Potential]):
+    return ctypes.cast(ctypes.pointer(pot), ctypes.c_void_p) if pot is not None else None
+
+
+def version() -> str:
+    return lib().odisseo_version().decode()
+
+
+def workspace_bytes(n: int, is_f64: bool = False) -> int:
+    return int(lib().odisseo_workspace_bytes(int(n), int(bool(is_f64))))
+
+
+def host_workspace_bytes(n: int, is_f64: bool = False) -> int:
+    """Workspace for leapfrog_kdk_host: scratch + three device state arrays."""
+    return workspace_bytes(n, is_f64) + 3 * n * (32 if is_f64 else 16) + 768
+
+
+def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def describe_plan(n: int, is_f64: bool = False, num_sms: Optional[int] = None) -> dict:
+    out = (ctypes.c_int64 * 8)()
+    if num_sms is None:
+        _check(lib().odisseo_describe_plan(int(n), int(is_f64), out), "describe_plan")
+    else:
+        _check(lib().odisseo_describe_plan_for(int(n), int(is_f64), int(num_sms), out), "describe_plan_for")
+    keys = ["i_bodies_per_thread", "threads_per_cta", "tile_records", "persistent_ctas", "i_blocks", "j_tiles",
+            "partial_slots", "kernels_per_step"]
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def plan_probe(n: int, is_f64: bool, num_sms: int, u: int, c: int):
+    out = (ctypes.c_int64 * 3)()
+    _check(lib().odisseo_plan_probe(int(n), int(is_f64), int(num_sms), int(u), int(c), out), "plan_probe")
+    return int(out[0]), int(out[1]), int(out[2])
+
+
+def pair_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, eps: float, workspace: torch.Tensor, stream=None):
+    """acc[n,4] = pair acceleration of posm[n,4] (odisseo_pair_accel_f32/_f64)."""
+    n = _rec(posm, "posm")
+    _rec(acc, "acc", n)
+    sfx = _suffix(posm)
+    if acc.dtype != posm.dtype:
+        raise TypeError("posm and acc dtypes differ")
+    fn = getattr(lib(), "odisseo_pair_accel_" + sfx)
+    _check(fn(posm.data_ptr(), acc.data_ptr(), n, G, eps, workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "pair_accel_" + sfx)
+    return acc
+
+
+def pair_accel_soa(x, y, z, m, ax, ay, az, G: float, eps: float, workspace: torch.Tensor, stream=None):
+    n = x.numel()
+    for t in (x, y, z, m, ax, ay, az):
+        if t.dtype != torch.float32 or not t.is_cuda or not t.is_contiguous() or t.numel() != n:
+            raise ValueError("SoA arguments must be contiguous float32 CUDA vectors of equal length")
+    _check(lib().odisseo_pair_accel_soa_f32(x.data_ptr(), y.data_ptr(), z.data_ptr(), m.data_ptr(), ax.data_ptr(),
+                                            ay.data_ptr(), az.data_ptr(), n, G, eps, workspace.data_ptr(),
+                                            workspace.numel(), _stream(stream)), "pair_accel_soa_f32")
+
+
+def ext_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, pot: Optional[Potential], accumulate: bool = False,
+              stream=None):
+    n = _rec(posm, "posm")
+    _rec(acc, "acc", n)
+    sfx = _suffix(posm)
+    fn = getattr(lib(), "odisseo_ext_accel_" + sfx)
+    _check(fn(posm.data_ptr(), acc.data_ptr(), n, G, _pot(pot), int(bool(accumulate)), _stream(stream)),
+           "ext_accel_" + sfx)
+    return acc
+
+
+def leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, eps: float, dt: float,
+                 nsteps: int, pot: Optional[Potential], workspace: torch.Tensor, acc_valid: bool = False, stream=None):
+    """nsteps KDK steps in place on device tensors (odisseo_leapfrog_kdk_f32/_f64)."""
+    n = _rec(posm, "posm")
+    _rec(vel, "vel", n)
+    _rec(acc, "acc", n)
+    sfx = _suffix(posm)
+    fn = getattr(lib(), "odisseo_leapfrog_kdk_" + sfx)
+    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr(), int(bool(acc_valid)), n, G, eps, dt, int(nsteps),
+              _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)), "leapfrog_kdk_" + sfx)
+
+
+def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch.Tensor], G: float, eps: float,
+                      dt: float, nsteps: int, pot: Optional[Potential], workspace: torch.Tensor, stream=None):
+    """Host-buffer face: posm/vel/acc are (pinned) CPU tensors updated in place after a stream sync."""
+    n = _rec(posm, "posm", cuda=False)
+    _rec(vel, "vel", n, cuda=False)
+    if posm.is_cuda or vel.is_cuda:
+        raise ValueError("leapfrog_kdk_host takes host tensors")
+    if acc is not None:
+        _rec(acc, "acc", n, cuda=False)
+    sfx = _suffix(posm)
+    fn = getattr(lib(), "odisseo_leapfrog_kdk_host_" + sfx)
+    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr() if acc is not None else None, n, G, eps, dt,
+              int(nsteps), _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "leapfrog_kdk_host_" + sfx)

@@ -1,0 +1,488 @@
+// C ABI of the ODISSEO B200 library (include/odisseo.h): argument validation, launch plan,
+// workspace carving, per-step launch sequence and its CUDA-graph capture.
+#include <math.h>
+#include <string.h>
+
+#include <mutex>
+#include <vector>
+
+#include "odisseo_common.cuh"
+
+namespace odisseo {
+
+// ------------------------------- launch plan ------------------------------------------
+PairPlan make_plan(int64_t n, int is_f64, int num_sms)
+{
+    PairPlan p;
+    memset(&p, 0, sizeof(p));
+    p.n = n;
+    p.variant = (n <= 4096) ? 1 : 0;
+    int minb;
+    if (p.variant == 0) {
+        p.ipt = is_f64 ? 4 : 8;
+        p.cthreads = 256;
+        minb = 2;
+    } else {
+        p.ipt = 2;
+        p.cthreads = 64;
+        minb = 8;
+    }
+    p.rec_bytes = 32;
+    p.IB = p.ipt * p.cthreads;
+    p.nb = (int32_t)((n + p.IB - 1) / p.IB);
+    int64_t P = (int64_t)num_sms * minb;
+    int32_t T = 256;
+    for (; T > 32; T >>= 1) {
+        const int64_t U = (int64_t)p.nb * ((n + T - 1) / T);
+        if (U >= 8 * P) break;
+    }
+    p.T = T;
+    p.J = (int32_t)((n + T - 1) / T);
+    p.U = (int64_t)p.nb * p.J;
+    if (P > p.U) P = p.U;
+    if (P < 1) P = 1;
+    p.P = (int32_t)P;
+    p.slots = p.P + p.nb;
+    return p;
+}
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+odisseo_status cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    (void)cudaGetLastError();
+    return ODISSEO_ERR_CUDA;
+}
+
+struct DeviceInfo { int device; int sms; int major; bool configured; };
+std::mutex g_mutex;
+std::vector<DeviceInfo> g_devices;
+
+odisseo_status device_info(DeviceInfo& out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    for (const DeviceInfo& d : g_devices)
+        if (d.device == dev) { out = d; return d.major == 10 ? ODISSEO_OK : ODISSEO_ERR_ARCH; }
+    DeviceInfo d{dev, 0, 0, false};
+    e = cudaDeviceGetAttribute(&d.major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (d.major != 10) { g_devices.push_back(d); out = d; return ODISSEO_ERR_ARCH; }
+    e = configure_pair_f32();
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = configure_pair_f64();
+    if (e != cudaSuccess) return cuda_fail(e);
+    d.configured = true;
+    g_devices.push_back(d);
+    out = d;
+    return ODISSEO_OK;
+}
+
+inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+inline bool overlap(const void* a, size_t na, const void* b, size_t nb)
+{
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + nb && y < x + na;
+}
+
+template <typename T> odisseo_status check_pair_scalars(T G, T eps)
+{
+    if (!isfinite((double)G) || !isfinite((double)eps) || !(eps > (T)0)) return ODISSEO_ERR_ARG;
+    const double e2 = (double)eps * (double)eps;
+    if (e2 < 1e-30 || e2 > 1e30) return ODISSEO_ERR_ARG;   // fp32 rsqrt seed range (pair_f64.cu)
+    return ODISSEO_OK;
+}
+
+template <typename T> odisseo_status make_pot(T G, const odisseo_potential* pot, PotParams<T>& out)
+{
+    memset(&out, 0, sizeof(out));
+    if (!pot) return ODISSEO_OK;
+    if (pot->nfw.M_s > 0.0) {
+        if (!(pot->nfw.r_s > 0.0) || !isfinite(pot->nfw.M_s) || !isfinite(pot->nfw.r_s)) return ODISSEO_ERR_ARG;
+        out.GMs = (T)((double)G * pot->nfw.M_s);
+        out.inv_rs = (T)(1.0 / pot->nfw.r_s);
+    }
+    if (pot->mn.M > 0.0) {
+        if (!(pot->mn.b > 0.0) || !(pot->mn.a >= 0.0) || !isfinite(pot->mn.M) || !isfinite(pot->mn.a) ||
+            !isfinite(pot->mn.b))
+            return ODISSEO_ERR_ARG;
+        out.GMd = (T)((double)G * pot->mn.M);
+        out.a = (T)pot->mn.a;
+        out.b2 = (T)(pot->mn.b * pot->mn.b);
+    }
+    return ODISSEO_OK;
+}
+
+// ---- typed launch shims ----------------------------------------------------------------
+inline cudaError_t launch_pair(const PairPlan& p, const float* x, const void* j, double* part, float eps, cudaStream_t s)
+{ return launch_pair_f32(p, x, j, part, eps, s); }
+inline cudaError_t launch_pair(const PairPlan& p, const double* x, const void* j, double* part, double eps, cudaStream_t s)
+{ return launch_pair_f64(p, x, j, part, eps, s); }
+inline cudaError_t launch_step(const PairPlan& p, float* x, float* v, float* a, void* j, const double* part, float G,
+                               const PotParams<float>& pot, float dt, int flags, cudaStream_t s)
+{ return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, s); }
+inline cudaError_t launch_step(const PairPlan& p, double* x, double* v, double* a, void* j, const double* part, double G,
+                               const PotParams<double>& pot, double dt, int flags, cudaStream_t s)
+{ return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, s); }
+
+inline cudaError_t launch_ext(const float* x, float* a, int64_t n, const PotParams<float>& pot, int accumulate, cudaStream_t s)
+{ return launch_ext_f32(x, a, n, pot, accumulate, s); }
+inline cudaError_t launch_ext(const double* x, double* a, int64_t n, const PotParams<double>& pot, int accumulate, cudaStream_t s)
+{ return launch_ext_f64(x, a, n, pot, accumulate, s); }
+
+struct Carve { void* jsrc; double* partials; };
+
+odisseo_status carve(const PairPlan& plan, void* ws, size_t ws_bytes, Carve& out)
+{
+    if (!ws) return ODISSEO_ERR_NULL;
+    if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
+    const size_t need = plan_jsrc_bytes(plan) + plan_partial_bytes(plan);
+    if (ws_bytes < need) return ODISSEO_ERR_WORKSPACE;
+    out.jsrc = ws;
+    out.partials = reinterpret_cast<double*>(static_cast<unsigned char*>(ws) + plan_jsrc_bytes(plan));
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!posm || !acc) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+    if (overlap(posm, n * rec, acc, n * rec)) return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    Carve cv;
+    st = carve(plan, ws, ws_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    PotParams<T> nopot;
+    memset(&nopot, 0, sizeof(nopot));
+    cudaError_t e = launch_step(plan, const_cast<T*>(posm), (T*)nullptr, acc, cv.jsrc, cv.partials, G, nopot, (T)0,
+                                STEP_PACK_ONLY, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_step(plan, const_cast<T*>(posm), (T*)nullptr, acc, cv.jsrc, cv.partials, G, nopot, (T)0,
+                    STEP_FROM_PARTIALS, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status ext_accel_impl(const T* posm, T* acc, int64_t n, T G, const odisseo_potential* pot, int accumulate,
+                              void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!posm || !acc) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+    if (overlap(posm, n * rec, acc, n * rec)) return ODISSEO_ERR_ARG;
+    if (!isfinite((double)G)) return ODISSEO_ERR_ARG;
+    PotParams<T> pp;
+    odisseo_status st = make_pot<T>(G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e = launch_ext(posm, acc, n, pp, accumulate, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+// ---- CUDA-graph cache for the per-step launch sequence -----------------------------------
+struct GraphKey {
+    int is_f64;
+    const void *posm, *vel, *acc, *ws;
+    int64_t n;
+    double G, eps, dt;
+    odisseo_potential pot;
+    int has_pot;
+    int block;   // steps per graph
+    int device;
+    bool operator==(const GraphKey& o) const { return memcmp(this, &o, sizeof(GraphKey)) == 0; }
+};
+struct GraphEntry { GraphKey key; cudaGraphExec_t exec; uint64_t stamp; };
+std::vector<GraphEntry> g_graphs;
+uint64_t g_stamp = 0;
+constexpr size_t GRAPH_CACHE = 8;
+
+template <typename T>
+odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
+                             const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!posm || !vel || !acc) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(vel, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+    if (overlap(posm, n * rec, acc, n * rec) || overlap(posm, n * rec, vel, n * rec) ||
+        overlap(vel, n * rec, acc, n * rec))
+        return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
+    PotParams<T> pp;
+    st = make_pot<T>(G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    if (nsteps == 0 && acc_valid) return ODISSEO_OK;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    Carve cv;
+    st = carve(plan, ws, ws_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+
+#define ODISSEO_TRY(call) do { e = (call); if (e != cudaSuccess) return cuda_fail(e); } while (0)
+    int first = 0;
+    if (!acc_valid) {
+        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_PACK_ONLY, s));
+        ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+        first = STEP_FROM_PARTIALS;
+    }
+    if (nsteps == 0) {
+        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first, s));
+        return ODISSEO_OK;
+    }
+    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN, s));
+
+    int64_t mid = nsteps - 1;     // full steps: pair + (close, open)
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
+    const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2;
+    if (use_graph) {
+        const int block = (int)(mid < 16 ? mid : 16);
+        GraphKey key;
+        memset(&key, 0, sizeof(key));
+        key.is_f64 = sizeof(T) == 8; key.posm = posm; key.vel = vel; key.acc = acc; key.ws = ws; key.n = n;
+        key.G = (double)G; key.eps = (double)eps; key.dt = (double)dt; key.has_pot = pot != nullptr;
+        if (pot) key.pot = *pot;
+        key.block = block; key.device = dev.device;
+        cudaGraphExec_t exec = nullptr;
+        {
+            std::lock_guard<std::mutex> lock(g_mutex);
+            for (GraphEntry& ge : g_graphs)
+                if (ge.key == key) { exec = ge.exec; ge.stamp = ++g_stamp; break; }
+        }
+        if (!exec) {
+            cudaGraph_t graph = nullptr;
+            ODISSEO_TRY(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+            cudaError_t ce = cudaSuccess;
+            for (int k = 0; k < block && ce == cudaSuccess; ++k) {
+                ce = launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s);
+                if (ce == cudaSuccess)
+                    ce = launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
+                                     STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s);
+            }
+            e = cudaStreamEndCapture(s, &graph);
+            if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return cuda_fail(ce); }
+            if (e != cudaSuccess) return cuda_fail(e);
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return cuda_fail(e);
+            std::lock_guard<std::mutex> lock(g_mutex);
+            if (g_graphs.size() >= GRAPH_CACHE) {
+                size_t victim = 0;
+                for (size_t k = 1; k < g_graphs.size(); ++k)
+                    if (g_graphs[k].stamp < g_graphs[victim].stamp) victim = k;
+                cudaGraphExecDestroy(g_graphs[victim].exec);
+                g_graphs.erase(g_graphs.begin() + victim);
+            }
+            g_graphs.push_back(GraphEntry{key, exec, ++g_stamp});
+        }
+        while (mid >= block) {
+            ODISSEO_TRY(cudaGraphLaunch(exec, s));
+            mid -= block;
+        }
+    }
+    for (; mid > 0; --mid) {
+        ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
+                                STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s));
+    }
+    ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE, s));
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int64_t n, T G, T eps, T dt, int64_t nsteps,
+                                  const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!h_posm || !h_vel || !ws) return ODISSEO_ERR_NULL;
+    if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
+    const size_t arr = ((size_t)n * 4 * sizeof(T) + 255) & ~(size_t)255;
+    if (ws_bytes < 3 * arr) return ODISSEO_ERR_WORKSPACE;
+    unsigned char* base = static_cast<unsigned char*>(ws);
+    T* d_posm = reinterpret_cast<T*>(base);
+    T* d_vel = reinterpret_cast<T*>(base + arr);
+    T* d_acc = reinterpret_cast<T*>(base + 2 * arr);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    ODISSEO_TRY(cudaMemcpyAsync(d_posm, h_posm, (size_t)n * 4 * sizeof(T), cudaMemcpyHostToDevice, s));
+    ODISSEO_TRY(cudaMemcpyAsync(d_vel, h_vel, (size_t)n * 4 * sizeof(T), cudaMemcpyHostToDevice, s));
+    odisseo_status st = leapfrog_impl<T>(d_posm, d_vel, d_acc, 0, n, G, eps, dt, nsteps, pot, base + 3 * arr,
+                                         ws_bytes - 3 * arr, stream);
+    if (st != ODISSEO_OK) return st;
+    ODISSEO_TRY(cudaMemcpyAsync(h_posm, d_posm, (size_t)n * 4 * sizeof(T), cudaMemcpyDeviceToHost, s));
+    ODISSEO_TRY(cudaMemcpyAsync(h_vel, d_vel, (size_t)n * 4 * sizeof(T), cudaMemcpyDeviceToHost, s));
+    if (h_acc) ODISSEO_TRY(cudaMemcpyAsync(h_acc, d_acc, (size_t)n * 4 * sizeof(T), cudaMemcpyDeviceToHost, s));
+    return ODISSEO_OK;
+}
+#undef ODISSEO_TRY
+
+}  // namespace
+}  // namespace odisseo
+
+using namespace odisseo;
+
+extern "C" {
+
+const char* odisseo_version(void) { return "odisseo-b200 0.1 (sm_100a)"; }
+
+const char* odisseo_status_string(odisseo_status s)
+{
+    switch (s) {
+        case ODISSEO_OK: return "ok";
+        case ODISSEO_ERR_NULL: return "null pointer";
+        case ODISSEO_ERR_ALIGN: return "misaligned pointer";
+        case ODISSEO_ERR_ARG: return "invalid argument";
+        case ODISSEO_ERR_WORKSPACE: return "workspace too small";
+        case ODISSEO_ERR_ARCH: return "device is not compute capability 10.x (B200)";
+        case ODISSEO_ERR_CUDA: return "CUDA error (see odisseo_last_cuda_error)";
+    }
+    return "unknown status";
+}
+
+int odisseo_last_cuda_error(void) { return g_last_cuda_error; }
+
+size_t odisseo_workspace_bytes(int64_t n, int is_f64)
+{
+    if (n <= 0) return 0;
+    // bound over devices with up to 192 SMs: more CTAs -> more partial rows, smaller tiles -> same padding bound
+    const PairPlan p = make_plan(n, is_f64, 192);
+    const size_t jsrc = (((size_t)(n + 256) * p.rec_bytes) + 255) & ~(size_t)255;
+    return jsrc + (size_t)p.slots * 3 * p.IB * sizeof(double);
+}
+
+odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8])
+{
+    if (!out) return ODISSEO_ERR_NULL;
+    if (n <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
+    const PairPlan p = make_plan(n, is_f64, num_sms);
+    out[0] = p.ipt; out[1] = p.cthreads + 32; out[2] = p.T; out[3] = p.P;
+    out[4] = p.nb; out[5] = p.J; out[6] = p.slots; out[7] = 2;
+    return ODISSEO_OK;
+}
+
+odisseo_status odisseo_describe_plan(int64_t n, int is_f64, int64_t out[8])
+{
+    if (!out) return ODISSEO_ERR_NULL;
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    return odisseo_describe_plan_for(n, is_f64, dev.sms, out);
+}
+
+// Host-side check of the stream-K bookkeeping for tests: for unit u returns the owning CTA,
+// and for CTA c its [start, end) range, exactly as the kernels compute them.
+odisseo_status odisseo_plan_probe(int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[3])
+{
+    if (!out) return ODISSEO_ERR_NULL;
+    if (n <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
+    const PairPlan p = make_plan(n, is_f64, num_sms);
+    if (u < 0 || u >= p.U || c < 0 || c >= p.P) return ODISSEO_ERR_ARG;
+    out[0] = plan_owner(p, u);
+    out[1] = plan_start(p, c);
+    out[2] = plan_start(p, c + 1);
+    return ODISSEO_OK;
+}
+
+odisseo_status odisseo_pair_accel_f32(const float* d_posm, float* d_acc, int64_t n, float G, float eps,
+                                      void* d_workspace, size_t workspace_bytes, void* stream)
+{ return pair_accel_impl<float>(d_posm, d_acc, n, G, eps, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_pair_accel_f64(const double* d_posm, double* d_acc, int64_t n, double G, double eps,
+                                      void* d_workspace, size_t workspace_bytes, void* stream)
+{ return pair_accel_impl<double>(d_posm, d_acc, n, G, eps, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_pair_accel_soa_f32(const float* d_x, const float* d_y, const float* d_z, const float* d_m,
+                                          float* d_ax, float* d_ay, float* d_az, int64_t n, float G, float eps,
+                                          void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!d_x || !d_y || !d_z || !d_m || !d_ax || !d_ay || !d_az || !d_workspace) return ODISSEO_ERR_NULL;
+    if (misaligned(d_x, 4) || misaligned(d_y, 4) || misaligned(d_z, 4) || misaligned(d_m, 4) || misaligned(d_ax, 4) ||
+        misaligned(d_ay, 4) || misaligned(d_az, 4))
+        return ODISSEO_ERR_ALIGN;
+    if (misaligned(d_workspace, 256)) return ODISSEO_ERR_ALIGN;
+    const size_t arr = ((size_t)n * 16 + 255) & ~(size_t)255;
+    if (workspace_bytes < 2 * arr) return ODISSEO_ERR_WORKSPACE;
+    odisseo_status st = check_pair_scalars<float>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    unsigned char* base = static_cast<unsigned char*>(d_workspace);
+    float* posm = reinterpret_cast<float*>(base);
+    float* acc = reinterpret_cast<float*>(base + arr);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e = launch_soa_pack_f32(d_x, d_y, d_z, d_m, posm, n, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    st = pair_accel_impl<float>(posm, acc, n, G, eps, base + 2 * arr, workspace_bytes - 2 * arr, stream);
+    if (st != ODISSEO_OK) return st;
+    e = launch_soa_unpack_f32(acc, d_ax, d_ay, d_az, n, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+odisseo_status odisseo_ext_accel_f32(const float* d_posm, float* d_acc, int64_t n, float G,
+                                     const odisseo_potential* pot, int accumulate, void* stream)
+{ return ext_accel_impl<float>(d_posm, d_acc, n, G, pot, accumulate, stream); }
+
+odisseo_status odisseo_ext_accel_f64(const double* d_posm, double* d_acc, int64_t n, double G,
+                                     const odisseo_potential* pot, int accumulate, void* stream)
+{ return ext_accel_impl<double>(d_posm, d_acc, n, G, pot, accumulate, stream); }
+
+odisseo_status odisseo_leapfrog_kdk_f32(float* d_posm, float* d_vel, float* d_acc, int acc_valid, int64_t n, float G,
+                                        float eps, float dt, int64_t nsteps, const odisseo_potential* pot,
+                                        void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_impl<float>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d_acc, int acc_valid, int64_t n,
+                                        double G, double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
+                                        void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_leapfrog_kdk_host_f32(float* h_posm, float* h_vel, float* h_acc, int64_t n, float G, float eps,
+                                             float dt, int64_t nsteps, const odisseo_potential* pot,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_host_impl<float>(h_posm, h_vel, h_acc, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_leapfrog_kdk_host_f64(double* h_posm, double* h_vel, double* h_acc, int64_t n, double G,
+                                             double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_host_impl<double>(h_posm, h_vel, h_acc, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+}  // extern "C"

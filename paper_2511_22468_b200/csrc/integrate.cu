@@ -1,0 +1,242 @@
+// O(N) kernels of the hot path: fixed-order reduction of the pair partial sums, external
+// NFW + Miyamoto-Nagai acceleration, kick / drift, and (re)staging of the source array the
+// pair kernels read by TMA.  One fused launch per KDK step:
+//
+//   a_pair = G * sum_{rows of this i-block, increasing j} partial      [STEP_FROM_PARTIALS] -> acc
+//   a      = a_pair + a_NFW(x) + a_MN(x)
+//   v     += a dt/2          [STEP_CLOSE: second half kick of the step that just ended]
+//   v     += a dt/2 ; x += v dt   [STEP_OPEN: first half kick + drift of the next step]
+//   stage x for the next pair evaluation
+//
+// The two half kicks are two separate FMAs, so a step split across two calls is bit-identical to
+// the fused one (PAPER.md:L47 Velocity-Verlet; chaining contract in include/odisseo.h).
+// Memory-bound: one 16 B (32 B) record load per array, coalesced 128-bit accesses.
+#include "odisseo_common.cuh"
+
+namespace odisseo {
+
+namespace {
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { typedef float4 type; };
+template <> struct Vec4<double> { typedef double4 type; };
+
+__device__ __forceinline__ float rsqrt_acc(float x) { return 1.0f / sqrtf(x); }
+__device__ __forceinline__ double rsqrt_acc(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ float sqrt_acc(float x) { return sqrtf(x); }
+__device__ __forceinline__ double sqrt_acc(double x) { return sqrt(x); }
+__device__ __forceinline__ float log1p_acc(float x) { return log1pf(x); }
+__device__ __forceinline__ double log1p_acc(double x) { return log1p(x); }
+
+// NFW enclosed-mass function m(c) = ln(1+c) - c/(1+c).  For small c the two terms cancel
+// (m ~ c^2/2), so below c = 0.1 use the alternating series sum_{k>=2} (-1)^k (k-1)/k c^k
+// (reading R12); the truncation c^(K+1) is < 1 ulp for the K used.
+template <typename T> __device__ __forceinline__ T nfw_menc(T c)
+{
+    if (c < (T)0.1) {
+        constexpr int K = sizeof(T) == 4 ? 9 : 18;
+        T s = (T)0;
+#pragma unroll
+        for (int k = K; k >= 2; --k) {
+            const T coef = (T)((k & 1) ? -1.0 : 1.0) * (T)(k - 1) / (T)k;
+            s = fma(s, c, coef);
+        }
+        return s * c * c;
+    }
+    return log1p_acc(c) - c / ((T)1 + c);
+}
+
+template <typename T>
+__device__ __forceinline__ void ext_accel(const PotParams<T>& pot, T x, T y, T z, T& ax, T& ay, T& az)
+{
+    ax = ay = az = (T)0;
+    if (pot.GMs != (T)0) {
+        const T r2 = fma(x, x, fma(y, y, z * z));
+        if (r2 > (T)0) {
+            const T rinv = rsqrt_acc(r2);
+            const T c = (r2 * rinv) * pot.inv_rs;
+            const T f = -pot.GMs * nfw_menc(c) * (rinv * rinv * rinv);
+            ax = f * x; ay = f * y; az = f * z;
+        }
+    }
+    if (pot.GMd != (T)0) {
+        const T B = sqrt_acc(fma(z, z, pot.b2));
+        const T sB = pot.a + B;
+        const T D2 = fma(x, x, fma(y, y, sB * sB));
+        const T dinv = rsqrt_acc(D2);
+        const T f = -pot.GMd * (dinv * dinv * dinv);
+        ax = fma(f, x, ax);
+        ay = fma(f, y, ay);
+        az = fma(f * z, sB / B, az);
+    }
+}
+
+// Staged source record writers.  fp32: {x,x,y,y},{z,z,m,m} (pre-duplicated packed operands);
+// fp64: plain {x,y,z,m}.  Records [n, n_pad) are zero-mass padding.
+__device__ __forceinline__ void stage_record(void* jsrc, int64_t i, float x, float y, float z, float m)
+{
+    float4* out = reinterpret_cast<float4*>(jsrc) + 2 * i;
+    out[0] = make_float4(x, x, y, y);
+    out[1] = make_float4(z, z, m, m);
+}
+__device__ __forceinline__ void stage_record(void* jsrc, int64_t i, double x, double y, double z, double m)
+{
+    reinterpret_cast<double4*>(jsrc)[i] = make_double4(x, y, z, m);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
+            typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
+            const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags)
+{
+    typedef typename Vec4<T>::type V4;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t npad = plan_npad(plan);
+    if (i >= npad) return;
+    if (i >= plan.n) {
+        if (flags & (STEP_OPEN | STEP_PACK_ONLY)) stage_record(jsrc, i, (T)0, (T)0, (T)0, (T)0);
+        return;
+    }
+    V4 p = posm[i];
+    if (flags & STEP_PACK_ONLY) {
+        stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+        return;
+    }
+
+    T apx, apy, apz;
+    if (flags & STEP_FROM_PARTIALS) {
+        const int32_t b = (int32_t)(i / plan.IB);
+        const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
+        const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
+        const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        for (int32_t c = c0; c <= c1; ++c) {               // fixed order: increasing j
+            const double* row = partials + (size_t)(c + b) * 3 * plan.IB;
+            sx += row[r];
+            sy += row[plan.IB + r];
+            sz += row[2 * plan.IB + r];
+        }
+        apx = (T)((double)G * sx);
+        apy = (T)((double)G * sy);
+        apz = (T)((double)G * sz);
+        V4 a; a.x = apx; a.y = apy; a.z = apz; a.w = (T)0;
+        acc[i] = a;
+    } else {
+        const V4 a = acc[i];
+        apx = a.x; apy = a.y; apz = a.z;
+    }
+    if (!(flags & (STEP_CLOSE | STEP_OPEN))) return;
+
+    T ex, ey, ez;
+    ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
+    const T tx = apx + ex, ty = apy + ey, tz = apz + ez;
+    const T h = (T)0.5 * dt;
+    V4 v = vel[i];
+    if (flags & STEP_CLOSE) {
+        v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+    }
+    if (flags & STEP_OPEN) {
+        v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+        p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
+        posm[i] = p;
+        stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+    }
+    v.w = (T)0;
+    vel[i] = v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+ext_kernel(const typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ acc, const int64_t n,
+           const PotParams<T> pot, const int accumulate)
+{
+    typedef typename Vec4<T>::type V4;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const V4 p = posm[i];
+    T ex, ey, ez;
+    ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
+    V4 a;
+    if (accumulate) {
+        a = acc[i];
+        a.x += ex; a.y += ey; a.z += ez;
+    } else {
+        a.x = ex; a.y = ey; a.z = ez; a.w = (T)0;
+    }
+    acc[i] = a;
+}
+
+__global__ void __launch_bounds__(256)
+soa_pack_kernel(const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
+                const float* __restrict__ m, float4* __restrict__ posm, const int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) posm[i] = make_float4(x[i], y[i], z[i], m[i]);
+}
+
+__global__ void __launch_bounds__(256)
+soa_unpack_kernel(const float4* __restrict__ acc, float* __restrict__ ax, float* __restrict__ ay,
+                  float* __restrict__ az, const int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        const float4 a = acc[i];
+        ax[i] = a.x; ay[i] = a.y; az[i] = a.z;
+    }
+}
+
+inline unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
+
+}  // namespace
+
+cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
+                            const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
+                            cudaStream_t stream)
+{
+    step_kernel<float><<<grid_for(plan_npad(plan)), 256, 0, stream>>>(
+        reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
+        partials, plan, G, pot, dt, flags);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
+                            const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
+                            cudaStream_t stream)
+{
+    step_kernel<double><<<grid_for(plan_npad(plan)), 256, 0, stream>>>(
+        reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
+        partials, plan, G, pot, dt, flags);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,
+                           cudaStream_t stream)
+{
+    ext_kernel<float><<<grid_for(n), 256, 0, stream>>>(reinterpret_cast<const float4*>(posm),
+                                                       reinterpret_cast<float4*>(acc), n, pot, accumulate);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const PotParams<double>& pot, int accumulate,
+                           cudaStream_t stream)
+{
+    ext_kernel<double><<<grid_for(n), 256, 0, stream>>>(reinterpret_cast<const double4*>(posm),
+                                                        reinterpret_cast<double4*>(acc), n, pot, accumulate);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
+                                int64_t n, cudaStream_t stream)
+{
+    soa_pack_kernel<<<grid_for(n), 256, 0, stream>>>(x, y, z, m, reinterpret_cast<float4*>(posm), n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream)
+{
+    soa_unpack_kernel<<<grid_for(n), 256, 0, stream>>>(reinterpret_cast<const float4*>(acc), ax, ay, az, n);
+    return cudaGetLastError();
+}
+
+}  // namespace odisseo

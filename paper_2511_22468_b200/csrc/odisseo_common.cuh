@@ -1,0 +1,164 @@
+// Shared device/host definitions of the ODISSEO B200 library: the launch plan (stream-K
+// decomposition of the (i-block x j-tile) interaction space), PTX wrappers for mbarrier /
+// 1-D TMA bulk copies / packed fp32 arithmetic.  sm_100a only.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/odisseo.h"
+
+namespace odisseo {
+
+// ---------------------------------------------------------------------------------------
+// Launch plan.  The N x N interaction matrix is cut into
+// nb = ceil(n / IB) i-blocks (IB targets held in registers by one CTA) times
+// J = ceil(n / T) j-tiles (T source records staged through shared memory per TMA copy).
+// The U = nb * J units are numbered u = b * J + t and dealt to P persistent CTAs in
+// contiguous, equal (+-1) ranges: CTA c owns [start(c), start(c+1)), start(c) = floor(c*U/P).
+// A CTA therefore walks a few consecutive i-blocks ("segments"); each segment writes one
+// row of partial sums into slot (c + b), and the reduce step adds the rows of an i-block in
+// increasing c (= increasing j) order: fixed order, no atomics, bit-reproducible.
+// ---------------------------------------------------------------------------------------
+struct PairPlan {
+    int64_t n;        // particles
+    int64_t U;        // work units = nb * J
+    int32_t IB;       // targets per i-block = ipt * cthreads
+    int32_t T;        // source records per j-tile
+    int32_t J;        // j-tiles
+    int32_t nb;       // i-blocks
+    int32_t P;        // persistent CTAs (grid size)
+    int32_t ipt;      // i-bodies per thread
+    int32_t cthreads; // compute threads per CTA (one extra producer warp is added at launch)
+    int32_t variant;  // 0 = large (8 compute warps), 1 = small (2 compute warps)
+    int32_t slots;    // rows in the partial buffer = P + nb
+    int32_t rec_bytes;// bytes per staged source record
+};
+
+__host__ __device__ __forceinline__ int64_t plan_start(const PairPlan& p, int64_t c) {
+    return (c * p.U) / p.P;
+}
+// CTA that owns unit u: the largest c with start(c) <= u.
+__host__ __device__ __forceinline__ int32_t plan_owner(const PairPlan& p, int64_t u) {
+    int64_t c = ((u + 1) * p.P + p.U - 1) / p.U - 1;
+    return (int32_t)(c < p.P - 1 ? c : p.P - 1);
+}
+__host__ __device__ __forceinline__ int64_t plan_npad(const PairPlan& p) { return (int64_t)p.J * p.T; }
+__host__ __device__ __forceinline__ size_t plan_jsrc_bytes(const PairPlan& p) {
+    size_t b = (size_t)plan_npad(p) * p.rec_bytes;
+    return (b + 255) & ~(size_t)255;
+}
+__host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p) {
+    return (size_t)p.slots * 3 * p.IB * sizeof(double);
+}
+
+PairPlan make_plan(int64_t n, int is_f64, int num_sms);
+
+// External potential with the host-side pre-combined products (reading R4).
+template <typename T> struct PotParams {
+    T GMs, inv_rs;   // NFW: G*M_s, 1/r_s   (GMs == 0 disables)
+    T GMd, a, b2;    // MN:  G*M, a, b^2    (GMd == 0 disables)
+};
+
+// Step-kernel flags.
+enum : int {
+    STEP_FROM_PARTIALS = 1,   // a_pair = G * fixed-order sum of partial rows (else read acc)
+    STEP_CLOSE = 2,           // closing half kick  v += a dt/2  (end of a step)
+    STEP_OPEN = 4,            // opening half kick + drift: v += a dt/2; x += v dt (start of next step)
+    STEP_PACK_ONLY = 8        // only (re)write the staged source array from posm
+};
+
+// ---------------------------------------------------------------------------------------
+// PTX wrappers
+// ---------------------------------------------------------------------------------------
+#if defined(__CUDACC__)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier.  dst, src and
+// bytes must be multiples of 16.  SASS: UBLKCP.
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// Packed fp32 pairs in 64-bit registers (FFMA2 / FADD2 / FMUL2 on sm_100a).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpk(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+#endif  // __CUDACC__
+
+// launchers (defined in pair_f32.cu / pair_f64.cu / integrate.cu)
+cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials,
+                            float eps, cudaStream_t stream);
+cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials,
+                            double eps, cudaStream_t stream);
+cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
+                            const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
+                            cudaStream_t stream);
+cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
+                            const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
+                            cudaStream_t stream);
+cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,
+                           cudaStream_t stream);
+cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const PotParams<double>& pot, int accumulate,
+                           cudaStream_t stream);
+cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
+                                int64_t n, cudaStream_t stream);
+cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
+cudaError_t configure_pair_f32();
+cudaError_t configure_pair_f64();
+
+}  // namespace odisseo

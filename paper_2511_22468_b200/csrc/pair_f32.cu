@@ -1,0 +1,191 @@
+// fp32 all-pairs Plummer-softened acceleration (section 1; SURVEY.md 8a rows a1, a1').
+//
+//   partial_i = sum_{j in segment} m_j (x_j - x_i) (|x_j - x_i|^2 + eps^2)^{-3/2}      (G applied in the reduce step)
+//
+// Design (B200-first, not the paper's XLA broadcast):
+//   * persistent grid, P = SMs x resident CTAs, stream-K split of the (i-block x j-tile) space
+//     (odisseo_common.cuh) -> every SM busy for any N, no wave-quantisation tail;
+//   * source tiles arrive by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx) issued by
+//     a dedicated producer warp into a STAGES-deep ring; consumers release a stage with one
+//     mbarrier arrive per warp -- no __syncthreads in the main loop;
+//   * each compute thread keeps 2*NPAIR targets in registers as packed f32x2 pairs; sources are
+//     staged pre-duplicated {x,x,y,y},{z,z,m,m} so that one LDS.128 yields two ready packed
+//     operands and the body is 3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per TWO interactions
+//     (half the issue slots of the scalar form, no register-pair MOVs);
+//   * two-level summation: fp32 inside one tile (<= 256 terms), promoted to fp64 between tiles
+//     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18);
+//   * the self term and the zero-mass padding records contribute exactly 0 because eps > 0.
+#include "odisseo_common.cuh"
+
+namespace odisseo {
+
+namespace {
+
+constexpr int STAGES = 4;
+
+template <int NPAIR, int CWARPS, int MINB>
+__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
+pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsrc, double* __restrict__ partials,
+                  const PairPlan plan, const float eps2)
+{
+    constexpr int CTHREADS = CWARPS * 32;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[STAGES];
+
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5;
+    const int lane = tid & 31;
+    const int64_t c = blockIdx.x;
+    const int64_t u0 = plan_start(plan, c);
+    const int64_t u1 = plan_start(plan, c + 1);
+    if (u0 >= u1) return;
+
+    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], CWARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (warp == CWARPS) {
+        // ---- producer warp: one elected lane streams the CTA's tile sequence --------------
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            int32_t t = (int32_t)(u0 % plan.J);
+            for (int64_t u = u0; u < u1; ++u) {
+                mbar_wait(&empty_bar[s], ph ^ 1u);   // passes at once during the first round
+                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
+                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
+                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
+                            &full_bar[s]);
+                if (++t == plan.J) t = 0;
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+        return;
+    }
+
+    // ---- compute warps ----------------------------------------------------------------------
+    const f32x2 e2 = pk(eps2, eps2);
+    f32x2 xi[NPAIR], yi[NPAIR], zi[NPAIR];
+    f32x2 ax[NPAIR], ay[NPAIR], az[NPAIR];
+    // fp64 outer sums live in shared memory (48 registers otherwise): osum[k][tid], k = 3*(2p+h)+comp
+    double* __restrict__ osum = reinterpret_cast<double*>(smem_raw + (size_t)STAGES * tile_bytes) + tid;
+
+    int32_t b = (int32_t)(u0 / plan.J);
+    int32_t t = (int32_t)(u0 - (int64_t)b * plan.J);
+    bool seg_start = true;
+    int s = 0;
+    uint32_t ph = 0;
+
+    for (int64_t u = u0; u < u1; ++u) {
+        if (seg_start) {
+            const int64_t base = (int64_t)b * plan.IB + tid;
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) {
+                int64_t i0 = base + (int64_t)(2 * p) * CTHREADS;
+                int64_t i1 = i0 + CTHREADS;
+                i0 = i0 < plan.n ? i0 : plan.n - 1;     // clamped rows are computed and never read back
+                i1 = i1 < plan.n ? i1 : plan.n - 1;
+                const float4 p0 = __ldg(posm + i0);
+                const float4 p1 = __ldg(posm + i1);
+                xi[p] = pk(p0.x, p1.x);
+                yi[p] = pk(p0.y, p1.y);
+                zi[p] = pk(p0.z, p1.z);
+                ax[p] = ay[p] = az[p] = 0ull;
+            }
+#pragma unroll
+            for (int k = 0; k < 6 * NPAIR; ++k) osum[k * CTHREADS] = 0.0;
+            seg_start = false;
+        }
+
+        mbar_wait(&full_bar[s], ph);
+        const ulonglong2* __restrict__ tile = reinterpret_cast<const ulonglong2*>(smem_raw + (size_t)s * tile_bytes);
+#pragma unroll 4
+        for (int j = 0; j < plan.T; ++j) {
+            const ulonglong2 A = tile[2 * j];        // {x,x},{y,y}
+            const ulonglong2 B = tile[2 * j + 1];    // {z,z},{m,m}
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) {
+                const f32x2 dx = sub2(A.x, xi[p]);
+                const f32x2 dy = sub2(A.y, yi[p]);
+                const f32x2 dz = sub2(B.x, zi[p]);
+                f32x2 r2 = fma2(dx, dx, e2);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dz, dz, r2);
+                float r2l, r2h;
+                unpk(r2, r2l, r2h);
+                const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
+                const f32x2 ri2 = mul2(ri, ri);
+                const f32x2 mri = mul2(B.y, ri);
+                const f32x2 w = mul2(ri2, mri);
+                ax[p] = fma2(w, dx, ax[p]);
+                ay[p] = fma2(w, dy, ay[p]);
+                az[p] = fma2(w, dz, az[p]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[s]);
+        if (++s == STAGES) { s = 0; ph ^= 1u; }
+
+        // second summation level: promote the tile sums to fp64
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            float lo, hi;
+            unpk(ax[p], lo, hi); osum[(6 * p + 0) * CTHREADS] += (double)lo; osum[(6 * p + 3) * CTHREADS] += (double)hi;
+            unpk(ay[p], lo, hi); osum[(6 * p + 1) * CTHREADS] += (double)lo; osum[(6 * p + 4) * CTHREADS] += (double)hi;
+            unpk(az[p], lo, hi); osum[(6 * p + 2) * CTHREADS] += (double)lo; osum[(6 * p + 5) * CTHREADS] += (double)hi;
+            ax[p] = ay[p] = az[p] = 0ull;
+        }
+
+        const bool seg_end = (t == plan.J - 1) || (u == u1 - 1);
+        if (seg_end) {
+            double* row = partials + (size_t)(c + b) * 3 * plan.IB;
+#pragma unroll
+            for (int k = 0; k < 2 * NPAIR; ++k) {
+                const int r = k * CTHREADS + tid;
+                row[r] = osum[(3 * k + 0) * CTHREADS];
+                row[plan.IB + r] = osum[(3 * k + 1) * CTHREADS];
+                row[2 * plan.IB + r] = osum[(3 * k + 2) * CTHREADS];
+            }
+            seg_start = true;
+        }
+        if (++t == plan.J) { t = 0; ++b; }
+    }
+}
+
+template <int NPAIR, int CWARPS, int MINB>
+cudaError_t launch_variant(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
+                           cudaStream_t stream)
+{
+    const size_t smem = (size_t)STAGES * plan.T * 32 + (size_t)6 * NPAIR * CWARPS * 32 * sizeof(double);
+    pair_f32x2_kernel<NPAIR, CWARPS, MINB><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
+        reinterpret_cast<const float4*>(posm), reinterpret_cast<const uint4*>(jsrc), partials, plan, eps * eps);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t configure_pair_f32()
+{
+    cudaError_t e = cudaFuncSetAttribute(pair_f32x2_kernel<4, 8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         STAGES * 256 * 32 + 6 * 4 * 8 * 32 * 8);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pair_f32x2_kernel<1, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                STAGES * 256 * 32 + 6 * 1 * 2 * 32 * 8);
+}
+
+cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
+                            cudaStream_t stream)
+{
+    if (plan.variant == 0) return launch_variant<4, 8, 2>(plan, posm, jsrc, partials, eps, stream);
+    return launch_variant<1, 2, 8>(plan, posm, jsrc, partials, eps, stream);
+}
+
+}  // namespace odisseo

@@ -1,0 +1,121 @@
+"""CPU-side checks of the C-ABI boundary: the library builds and loads, exports every symbol
+include/odisseo.h declares, validates arguments before touching a device, and its stream-K
+bookkeeping (SURVEY.md 8a row a1': fixed-order partial sums) is consistent by brute force.
+No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2511_22468_b200 import binding as B
+from paper_2511_22468_b200 import build as build_mod
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build_mod.build()
+    return B.lib()
+
+
+def test_exports_every_declared_symbol(lib):
+    header = open(os.path.join(ROOT, "include", "odisseo.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(odisseo_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations parsed"
+    assert declared == set(B.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.odisseo_version()
+
+
+def test_status_strings(lib):
+    for code in range(7):
+        assert lib.odisseo_status_string(code)
+    assert lib.odisseo_last_cuda_error() == 0
+
+
+def test_workspace_bytes_is_monotone_and_bounds_every_plan(lib):
+    assert B.workspace_bytes(0) == 0 and B.workspace_bytes(-5) == 0
+    prev = 0
+    for n in (1, 2, 127, 1024, 4096, 4097, 16384, 65536, 262144, 1048576):
+        for f64 in (False, True):
+            w = B.workspace_bytes(n, f64)
+            for sms in (1, 8, 132, 148, 160, 192):
+                p = B.describe_plan(n, f64, sms)
+                ib = p["i_bodies_per_thread"] * (p["threads_per_cta"] - 32)
+                need = ((p["j_tiles"] * p["tile_records"] * 32 + 255) // 256) * 256 + p["partial_slots"] * 3 * ib * 8
+                assert need <= w, (n, f64, sms)
+        assert B.workspace_bytes(n) >= prev
+        prev = B.workspace_bytes(n)
+    assert B.workspace_bytes(1048576) < 256 << 20
+
+
+@pytest.mark.parametrize("n,sms", [(1, 148), (33, 148), (1000, 148), (1024, 148), (4097, 148), (16384, 148),
+                                   (65536, 148), (100003, 7), (262144, 148)])
+@pytest.mark.parametrize("f64", [False, True])
+def test_streamk_ranges_partition_units_and_owner_matches(n, sms, f64):
+    p = B.describe_plan(n, f64, sms)
+    P, nb, J = p["persistent_ctas"], p["i_blocks"], p["j_tiles"]
+    U = nb * J
+    ib = p["i_bodies_per_thread"] * (p["threads_per_cta"] - 32)
+    assert nb == -(-n // ib) and J == -(-n // p["tile_records"]) and 1 <= P <= U
+    assert p["partial_slots"] == P + nb
+    # ranges tile [0, U) in order, sizes differ by at most one
+    prev_end, sizes = 0, []
+    step = max(1, P // 97)
+    cs = sorted(set(list(range(0, P, step)) + [0, P - 1]))
+    for c in range(P) if P <= 600 else cs:
+        _, s, e = B.plan_probe(n, f64, sms, 0, c)
+        assert s <= e
+        if P <= 600:
+            assert s == prev_end
+            prev_end = e
+        sizes.append(e - s)
+    if P <= 600:
+        assert prev_end == U
+    assert max(sizes) - min(sizes) <= 1 and min(sizes) >= 1
+    # owner(u) is the CTA whose range holds u; slots c + b are distinct for distinct segments
+    us = range(U) if U <= 3000 else list(range(0, U, max(1, U // 1500))) + [U - 1]
+    seen = {}
+    for u in us:
+        c, _, _ = B.plan_probe(n, f64, sms, u, 0)
+        _, s, e = B.plan_probe(n, f64, sms, u, c)
+        assert s <= u < e
+        slot = c + u // J
+        assert seen.setdefault(slot, (c, u // J)) == (c, u // J)
+        assert slot < p["partial_slots"]
+
+
+def test_argument_validation_happens_before_any_device_work(lib):
+    buf = (ctypes.c_float * 64)()
+    addr = ctypes.addressof(buf)
+    addr16 = (addr + 15) & ~15
+    ws = ctypes.c_void_p(256)
+    f = lib.odisseo_pair_accel_f32
+    assert f(None, None, 0, 1.0, 0.1, None, 0, None) == 0                       # n == 0: no-op
+    assert f(None, None, -1, 1.0, 0.1, None, 0, None) == 3                      # n < 0
+    assert f(None, addr16, 4, 1.0, 0.1, ws, 1 << 20, None) == 1                 # NULL
+    assert f(addr16 + 4, addr16 + 128, 4, 1.0, 0.1, ws, 1 << 20, None) == 2     # misaligned
+    assert f(addr16, addr16 + 16, 4, 1.0, 0.1, ws, 1 << 20, None) == 3          # overlap
+    assert f(addr16, addr16 + 128, 4, 1.0, 0.0, ws, 1 << 20, None) == 3         # eps <= 0
+    assert f(addr16, addr16 + 128, 4, float("nan"), 0.1, ws, 1 << 20, None) == 3
+    g = lib.odisseo_leapfrog_kdk_f32
+    assert g(addr16, addr16 + 64, addr16 + 128, 0, 4, 1.0, 0.1, 0.1, -1, None, ws, 1 << 20, None) == 3
+    assert g(addr16, addr16 + 64, addr16 + 128, 1, 4, 1.0, 0.1, 0.1, 0, None, ws, 1 << 20, None) == 0
+    bad = B.Potential.make(mn=(1.0, 1.0, 0.0))                                   # MN with b = 0
+    e = lib.odisseo_ext_accel_f32
+    assert e(addr16, addr16 + 128, 4, 1.0, ctypes.cast(ctypes.pointer(bad), ctypes.c_void_p), 0, None) == 3
+
+
+def test_product_path_fails_loudly_without_gpu_or_library(monkeypatch):
+    import torch
+    if not torch.cuda.is_available():
+        with pytest.raises(ValueError, match="CUDA tensor"):
+            B.pair_accel(torch.zeros(4, 4), torch.zeros(4, 4), 1.0, 0.1, torch.zeros(256, dtype=torch.uint8))
+    monkeypatch.setattr(B, "_lib", None)
+    monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/libodisseo_b200.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        B.lib()

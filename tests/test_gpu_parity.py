@@ -1,0 +1,326 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  fp32 pair:  |a_gpu,i - a_ref,i| / sum_j |a_ij| <= 1e-5 for every particle
+  fp64 pair:  the same ratio <= 1e-12
+  config 0, fp64, 10 steps: positions agree to <= 1e-10 relative
+fp32 trajectory tolerances are SURVEY.md 8c (iii)/(iv), derived in DESIGN.md.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2511_22468_b200 import binding as B
+from paper_2511_22468_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_F32 = 1e-5
+TOL_F64 = 1e-12
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "gpu tests need a B200"
+    B.lib()
+
+
+def dev(a, dtype):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def gpu_pair(posm_np, G, eps, dtype):
+    posm = dev(posm_np, dtype)
+    acc = torch.full_like(posm, float("nan"))
+    ws = B.alloc_workspace(B.workspace_bytes(posm.shape[0], dtype == np.float64))
+    B.pair_accel(posm, acc, G, eps, ws)
+    torch.cuda.synchronize()
+    return acc.cpu().numpy()
+
+
+def pair_ratio(acc_gpu, posm64, G, eps, targets=None):
+    ref, S = O.pair_accel(posm64, G, eps, targets=targets)
+    got = acc_gpu[:, :3].astype(np.float64)
+    if targets is not None:
+        got = got[targets]
+    num = np.linalg.norm(got - ref, axis=1)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        ratio = np.where(S > 0, num / S, np.where(num == 0, 0.0, np.inf))
+    return float(ratio.max()) if ratio.size else 0.0
+
+
+def f32_inputs(posm64, G, eps):
+    """Same seeded inputs for both sides: fp32-rounded state and scalars, promoted to double."""
+    p32 = W.to_f32(posm64)
+    return p32, p32.astype(np.float64), float(np.float32(G)), float(np.float32(eps))
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 127, 129, 1000, 1025, 4096, 4097, 5000, 9001])
+def test_pair_f32_ragged_sizes_unequal_masses(n):
+    posm64, _ = W.random_cloud(n, seed=100 + n)
+    p32, p64, G, eps = f32_inputs(posm64, 1.0, 0.05)
+    acc = gpu_pair(p32, G, eps, np.float32)
+    assert np.all(acc[:, 3] == 0)
+    assert pair_ratio(acc, p64, G, eps) <= TOL_F32
+
+
+@pytest.mark.parametrize("n", [1, 2, 127, 1000, 1025, 4097, 6000])
+def test_pair_f64_ragged_sizes_unequal_masses(n):
+    posm64, _ = W.random_cloud(n, seed=200 + n)
+    acc = gpu_pair(posm64, 1.0, 0.05, np.float64)
+    assert pair_ratio(acc, posm64, 1.0, 0.05) <= TOL_F64
+
+
+@pytest.mark.parametrize("ci", [0, 1])
+def test_pair_f32_configs_full(ci):
+    cfg = W.CONFIGS[ci]
+    posm64, _ = W.make_state(cfg)
+    p32, p64, G, eps = f32_inputs(posm64, cfg.G, cfg.eps)
+    acc = gpu_pair(p32, G, eps, np.float32)
+    assert pair_ratio(acc, p64, G, eps) <= TOL_F32
+
+
+def test_pair_f64_config0_full():
+    cfg = W.CONFIGS[0]
+    posm64, _ = W.make_state(cfg)
+    acc = gpu_pair(posm64, cfg.G, cfg.eps, np.float64)
+    assert pair_ratio(acc, posm64, cfg.G, cfg.eps) <= TOL_F64
+
+
+@pytest.mark.parametrize("ci,dtype", [(2, np.float32), (3, np.float32), (3, np.float64), (4, np.float32)])
+def test_pair_full_size_on_seeded_target_subset(ci, dtype):
+    """BASELINE.json full sizes in the launch configuration bench.py times; the oracle
+    evaluates the seeded 4,096-target subset against all sources."""
+    cfg = W.CONFIGS[ci]
+    posm64, _ = W.make_state(cfg)
+    idx = W.target_subset(cfg.n)
+    if dtype == np.float32:
+        p, p64, G, eps = f32_inputs(posm64, cfg.G, cfg.eps)
+        tol = TOL_F32
+    else:
+        p, p64, G, eps, tol = posm64, posm64, cfg.G, cfg.eps, TOL_F64
+    acc = gpu_pair(p, G, eps, dtype)
+    assert np.all(np.isfinite(acc))
+    assert pair_ratio(acc, p64, G, eps, targets=idx) <= tol
+
+
+def test_pair_is_bit_reproducible_and_obeys_newtons_third_law():
+    cfg = W.CONFIGS[1]
+    posm64, _ = W.make_state(cfg)
+    p32, p64, G, eps = f32_inputs(posm64, cfg.G, cfg.eps)
+    a1 = gpu_pair(p32, G, eps, np.float32)
+    a2 = gpu_pair(p32, G, eps, np.float32)
+    assert a1.tobytes() == a2.tobytes()
+    m = p64[:, 3:4]
+    a = a1[:, :3].astype(np.float64)
+    assert np.linalg.norm(np.sum(m * a, axis=0)) / np.sum(m[:, 0] * np.linalg.norm(a, axis=1)) <= 1e-5
+
+
+def test_pair_coincident_particles_and_self_term_contribute_zero():
+    posm = np.array([[1, 2, 3, 1.0], [1, 2, 3, 5.0], [2, 2, 3, 2.0]])
+    acc = gpu_pair(posm.astype(np.float32), 1.0, 0.5, np.float32)
+    assert pair_ratio(acc, posm, 1.0, 0.5) <= TOL_F32
+    one = gpu_pair(np.array([[4.0, 5.0, 6.0, 7.0]], dtype=np.float32), 1.0, 0.5, np.float32)
+    assert np.all(one == 0)
+
+
+def test_pair_soa_matches_aos_bitwise():
+    posm64, _ = W.random_cloud(3001, seed=5)
+    p32 = W.to_f32(posm64)
+    ref = gpu_pair(p32, 1.0, 0.05, np.float32)
+    cols = [dev(p32[:, k].copy(), np.float32) for k in range(4)]
+    outs = [torch.empty(3001, device="cuda") for _ in range(3)]
+    ws = B.alloc_workspace(B.workspace_bytes(3001) + 32 * 3001 + 512)
+    B.pair_accel_soa(*cols, *outs, 1.0, 0.05, ws)
+    torch.cuda.synchronize()
+    for k in range(3):
+        assert outs[k].cpu().numpy().tobytes() == np.ascontiguousarray(ref[:, k]).tobytes()
+
+
+# ---------------------------------------------------------------------------------------------
+# external potential
+# ---------------------------------------------------------------------------------------------
+def _mw(cfg=W.CONFIGS[1]):
+    return B.Potential.make(nfw=cfg.nfw, mn=cfg.mn), O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 2e-6), (np.float64, 1e-13)])
+def test_ext_accel_workload_radii(dtype, tol):
+    cfg = W.CONFIGS[2]
+    posm64, _ = W.make_state(cfg, n=5000)
+    posm64[:2000, :3] = np.random.Generator(np.random.PCG64(3)).uniform(-25, 25, (2000, 3))   # whole galaxy
+    bpot, opot = _mw(cfg)
+    if dtype == np.float32:
+        p = W.to_f32(posm64)
+        p64, G = p.astype(np.float64), float(np.float32(cfg.G))
+    else:
+        p, p64, G = posm64, posm64, cfg.G
+    posm = dev(p, dtype)
+    acc = torch.full_like(posm, float("nan"))
+    B.ext_accel(posm, acc, G, bpot)
+    ref = O.ext_accel(p64, G, opot)
+    got = acc.cpu().numpy()[:, :3].astype(np.float64)
+    rel = np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert rel.max() <= tol
+    B.ext_accel(posm, acc, G, bpot, accumulate=True)                # acc.xyz += a_ext
+    got2 = acc.cpu().numpy()[:, :3].astype(np.float64)
+    assert np.abs(got2 - 2 * got).max() <= 1e-6 * np.abs(got).max()
+    B.ext_accel(posm, acc, G, None)
+    assert np.all(acc.cpu().numpy() == 0)
+
+
+def _nfw_accel_mpmath(pts, G, Ms, rs):
+    """40-digit evaluation of the NFW formula (include/odisseo.h): the fp64 oracle itself loses
+    ~eps * 2 r_s / r to cancellation at r << r_s, so small radii are checked against this."""
+    import mpmath
+    mpmath.mp.dps = 40
+    out = np.zeros((len(pts), 3))
+    for k, p in enumerate(pts):
+        x = [mpmath.mpf(float(t)) for t in p]
+        r = mpmath.sqrt(x[0] ** 2 + x[1] ** 2 + x[2] ** 2)
+        c = r / mpmath.mpf(rs)
+        f = -mpmath.mpf(G) * mpmath.mpf(Ms) * (mpmath.log(1 + c) - c / (1 + c)) / r ** 3
+        out[k] = [float(f * t) for t in x]
+    return out
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 3e-6), (np.float64, 1e-13)])
+def test_ext_accel_small_radii_series_branch_and_origin(dtype, tol):
+    r = np.geomspace(1e-4, 5.0, 400)
+    dirs = np.random.Generator(np.random.PCG64(8)).normal(size=(400, 3))
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    posm64 = np.concatenate([r[:, None] * dirs, np.ones((400, 1))], axis=1)
+    posm64 = np.concatenate([posm64, [[0, 0, 0, 1.0]]])
+    p = posm64.astype(dtype)
+    nfw_b = B.Potential.make(nfw=W.NFW_MW)
+    G = float(np.float32(W.G_KPC_MSUN_MYR)) if dtype == np.float32 else W.G_KPC_MSUN_MYR
+    posm = dev(p, dtype)
+    acc = torch.empty_like(posm)
+    B.ext_accel(posm, acc, G, nfw_b)
+    got = acc.cpu().numpy()[:, :3].astype(np.float64)
+    ref = _nfw_accel_mpmath(p[:-1, :3].astype(np.float64), G, *W.NFW_MW)
+    assert np.all(got[-1] == 0)
+    rel = np.linalg.norm(got[:-1] - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    assert rel.max() <= tol
+    # where the oracle is well conditioned (r >= 1 kpc) the two references agree
+    far = r >= 1.0
+    oref = O.ext_accel(p[:-1].astype(np.float64), G, O.Potential.make(nfw=W.NFW_MW))
+    assert (np.linalg.norm(oref[far] - ref[far], axis=1) / np.linalg.norm(ref[far], axis=1)).max() <= 1e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# leapfrog
+# ---------------------------------------------------------------------------------------------
+def gpu_leapfrog(posm_np, vel_np, G, eps, dt, nsteps, pot, dtype, acc_valid=False, acc_np=None, chunks=None):
+    posm = dev(posm_np, dtype)
+    vel = dev(W.vel4(vel_np, dtype) if vel_np.shape[1] == 3 else vel_np, dtype)
+    acc = dev(acc_np, dtype) if acc_np is not None else torch.full_like(posm, float("nan"))
+    ws = B.alloc_workspace(B.workspace_bytes(posm.shape[0], dtype == np.float64))
+    valid = acc_valid
+    for k in (chunks or [nsteps]):
+        B.leapfrog_kdk(posm, vel, acc, G, eps, dt, k, pot, ws, acc_valid=valid)
+        valid = True
+    torch.cuda.synchronize()
+    return posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy()
+
+
+def test_leapfrog_f64_config0_ten_steps_matches_oracle_to_1e10():
+    cfg = W.CONFIGS[0]
+    posm64, vel64 = W.make_state(cfg)
+    p, v, a = gpu_leapfrog(posm64, vel64, cfg.G, cfg.eps, cfg.dt, cfg.nsteps, None, np.float64)
+    pr, vr, _ = O.leapfrog_kdk(posm64, vel64, cfg.G, cfg.eps, cfg.dt, cfg.nsteps)
+    dx = np.linalg.norm(p[:, :3] - pr[:, :3], axis=1) / np.maximum(np.linalg.norm(pr[:, :3], axis=1), cfg.a)
+    dv = np.linalg.norm(v[:, :3] - vr, axis=1) / np.maximum(np.linalg.norm(vr, axis=1), np.sqrt(cfg.G * cfg.M / cfg.a))
+    assert dx.max() <= 1e-10 and dv.max() <= 1e-10
+    assert np.array_equal(p[:, 3], posm64[:, 3])                       # masses preserved
+    assert pair_ratio(a, p, cfg.G, cfg.eps) <= TOL_F64                 # acc == a_pair(x_final)
+
+
+@pytest.mark.parametrize("ci,n", [(0, None), (1, 4096), (1, None)])
+def test_leapfrog_f32_ten_steps_short_horizon_parity(ci, n):
+    """10 fp32 steps against the fp64 oracle from the same fp32-rounded state:
+    |dx| <= 1e-5 max(|x|, a),  |dv| <= 1e-5 |v| + 1.5e-4 |dt| (S_i + |a_ext,i|)."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg, n=n)
+    p32, v32 = W.to_f32(posm64), W.to_f32(vel64)
+    G, eps, dt = (float(np.float32(t)) for t in (cfg.G, cfg.eps, cfg.dt))
+    bpot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    opot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    p, v, a = gpu_leapfrog(p32, v32, G, eps, dt, 10, bpot, np.float32)
+    pr, vr, _ = O.leapfrog_kdk(p32.astype(np.float64), v32.astype(np.float64), G, eps, dt, 10, opot)
+    _, S = O.pair_accel(pr, G, eps)
+    aext = np.linalg.norm(O.ext_accel(pr, G, opot), axis=1)
+    dx = np.linalg.norm(p[:, :3] - pr[:, :3], axis=1)
+    dv = np.linalg.norm(v[:, :3] - vr, axis=1)
+    assert np.all(dx <= 1e-5 * np.maximum(np.linalg.norm(pr[:, :3], axis=1), cfg.a))
+    assert np.all(dv <= 1e-5 * np.linalg.norm(vr, axis=1) + 1.5e-4 * abs(dt) * (S + aext))
+    # re-synchronised parity (8c ii): acc left by the call is a_pair of the GPU's own final state
+    assert pair_ratio(a, p.astype(np.float64), G, eps) <= TOL_F32
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_leapfrog_chained_calls_are_bit_identical_to_one_call(dtype):
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.make_state(cfg, n=3000)
+    p0, v0 = posm64.astype(dtype), vel64.astype(dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    one = gpu_leapfrog(p0, v0, cfg.G, cfg.eps, cfg.dt, 23, pot, dtype)
+    chained = gpu_leapfrog(p0, v0, cfg.G, cfg.eps, cfg.dt, 23, pot, dtype, chunks=[1, 0, 2, 19, 1])
+    again = gpu_leapfrog(p0, v0, cfg.G, cfg.eps, cfg.dt, 23, pot, dtype)
+    for x, y, z in zip(one, chained, again):
+        assert x.tobytes() == y.tobytes() == z.tobytes()
+
+
+def test_leapfrog_zero_steps_evaluates_acc_only_and_negative_dt_reverses():
+    cfg = W.CONFIGS[0]
+    posm64, vel64 = W.make_state(cfg)
+    p, v, a = gpu_leapfrog(posm64, vel64, cfg.G, cfg.eps, cfg.dt, 0, None, np.float64)
+    assert np.array_equal(p, posm64) and np.array_equal(v[:, :3], vel64)
+    assert pair_ratio(a, posm64, cfg.G, cfg.eps) <= TOL_F64
+    pf, vf, af = gpu_leapfrog(posm64, vel64, cfg.G, cfg.eps, cfg.dt, 20, None, np.float64)
+    pb, vb, _ = gpu_leapfrog(pf, vf, cfg.G, cfg.eps, -cfg.dt, 20, None, np.float64, acc_valid=True, acc_np=af)
+    assert np.abs(pb[:, :3] - posm64[:, :3]).max() <= 1e-12 and np.abs(vb[:, :3] - vel64).max() <= 1e-12
+
+
+def test_leapfrog_host_face_matches_device_face_bitwise():
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.make_state(cfg, n=5000)
+    p32, v32 = W.to_f32(posm64), W.vel4(W.to_f32(vel64), np.float32)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    ref = gpu_leapfrog(p32, v32, cfg.G, cfg.eps, cfg.dt, 7, pot, np.float32)
+    hp = torch.from_numpy(p32.copy()).pin_memory()
+    hv = torch.from_numpy(v32.copy()).pin_memory()
+    ha = torch.empty_like(hp).pin_memory()
+    ws = B.alloc_workspace(B.host_workspace_bytes(5000))
+    B.leapfrog_kdk_host(hp, hv, ha, cfg.G, cfg.eps, cfg.dt, 7, pot, ws)
+    torch.cuda.synchronize()
+    assert hp.numpy().tobytes() == ref[0].tobytes()
+    assert hv.numpy().tobytes() == ref[1].tobytes()
+    assert ha.numpy().tobytes() == ref[2].tobytes()
+
+
+def test_leapfrog_conserves_lz_and_tracks_single_particle_orbit_f32():
+    """invariants of a GPU trajectory measured with the oracle's diagnostics."""
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.make_state(cfg, n=4096)
+    p32, v32 = W.to_f32(posm64), W.to_f32(vel64)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    p, v, _ = gpu_leapfrog(p32, v32, cfg.G, cfg.eps, cfg.dt, 400, pot, np.float32)
+    L0 = O.angular_momentum(p32, v32)[2]
+    L1 = O.angular_momentum(p, v[:, :3])[2]
+    assert abs(L1 - L0) <= 2e-5 * abs(L0)
+    opot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    one, _, _ = O.leapfrog_kdk(np.array([[*cfg.centre, cfg.M]]), np.array([cfg.velocity]), cfg.G, cfg.eps, cfg.dt, 400, opot)
+    assert np.linalg.norm(O.centre_of_mass(p) - one[0, :3]) <= 5e-3
+
+
+def test_workspace_too_small_and_bad_alignment_are_reported():
+    posm = torch.zeros(5000, 4, device="cuda")
+    acc = torch.zeros_like(posm)
+    with pytest.raises(B.OdisseoError, match="ERR_WORKSPACE"):
+        B.pair_accel(posm, acc, 1.0, 0.1, B.alloc_workspace(1024))
+    ws = B.alloc_workspace(B.workspace_bytes(5000) + 64)
+    with pytest.raises(B.OdisseoError, match="ERR_ALIGN"):
+        B.pair_accel(posm, acc, 1.0, 0.1, ws[16:])
+    with pytest.raises(B.OdisseoError, match="ERR_ARG"):
+        B.pair_accel(posm, posm, 1.0, 0.1, ws)

@@ -124,3 +124,20 @@ def test_transcription_crosscheck_against_survey_values():
         for got, want in ((a_nfw, v[3:6]), (a_mn, v[6:9])):
             ok = ~np.isnan(want)
             np.testing.assert_allclose(got[ok], want[ok], rtol=1e-12, atol=1e-18)
+
+
+def test_nfw_against_40_digit_evaluation_and_conditioning_at_small_radius():
+    """The oracle evaluates ln(1+c) - c/(1+c) as written; at c << 1 the two terms cancel and
+    the relative error grows like eps * 2/c.  Pin: exact (mpmath) within that bound everywhere,
+    and to 1e-14 at workload radii (r >= 1 kpc)."""
+    import mpmath
+    mpmath.mp.dps = 40
+    Ms, rs = W.NFW_MW
+    for r in (1e-4, 1e-2, 0.5, 1.0, 8.0, 12.4, 40.0):
+        x = np.array([r * 0.6, 0.0, r * 0.8])
+        a = O.ext_accel(_posm(x), G, NFW)[0]
+        c = mpmath.mpf(r) / rs
+        f = -mpmath.mpf(G) * Ms * (mpmath.log(1 + c) - c / (1 + c)) / mpmath.mpf(r) ** 3
+        exact = np.array([float(f * t) for t in x])
+        tol = max(1e-14, 4 * 2.2e-16 * 2 * rs / r)
+        assert np.linalg.norm(a - exact) <= tol * np.linalg.norm(exact)
