@@ -1,0 +1,330 @@
+"""Benchmark of the ODISSEO hot path on B200 (contract: task prompt section 4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config I]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one kick-drift-kick
+step of BASELINE.json configs[3] (Plummer progenitor, N = 262,144, NFW + Miyamoto-Nagai potential,
+fp32) = one O(N^2) pair evaluation + fixed-order reduce + external acceleration + kick/drift/kick,
+called through the C ABI (odisseo_leapfrog_kdk_f32, nsteps = 1, acc_valid = 1).
+metric = pairwise interactions/s (N^2 per step); steps/s is reported beside it.
+Multi-GPU: the path does not shard in this build: every rank
+advances its own seeded replica, no data-path collective, scaling = "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star convention
+SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
+FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
+# dram bytes per pair-kernel launch at N = 262,144 from profiles/ (ncu --set full); None until captured
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = None
+
+
+def _peaks():
+    here = os.path.dirname(os.path.abspath(__file__))
+    try:
+        with open(os.path.join(here, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except OSError:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, torch_device_index: int, period_s: float = 0.05):
+        super().__init__(daemon=True)
+        self.period = period_s
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._halt = threading.Event()
+        self.handle = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            self.handle = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            self.nvml = pynvml
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+        except Exception as exc:  # noqa: BLE001 - NVML is optional evidence, never the product path
+            self.error = repr(exc)
+
+    def run(self):
+        if self.handle is None:
+            return
+        n = self.nvml
+        names = {
+            getattr(n, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(n, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(n, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(n, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(n, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+            getattr(n, "nvmlClocksThrottleReasonApplicationsClocksSetting", 0x2): "applications_clocks_setting",
+        }
+        while not self._halt.is_set():
+            try:
+                self.samples.append(int(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)))
+                mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            self._halt.wait(self.period)
+
+    def stop(self) -> dict:
+        self._halt.set()
+        if self.is_alive():
+            self.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def _dist_setup(n_gpus: int):
+    """One process per GPU under torchrun; returns (rank, world, dist-or-None)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world == 1:
+        return 0, 1, None
+    import torch
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    dist.init_process_group(backend="nccl")
+    return rank, world, dist
+
+
+def _max_over_ranks(x: float, dist) -> float:
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def _barrier(dist):
+    import torch
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def _oracle_sample_rate(cfg, seconds_target: float):
+    """CPU baseline: the oracle as it stands, timed on this host's cores on a bounded sample of the
+    workload: the pair + external acceleration of a seeded subset of targets against all N sources."""
+    from oracle import oracle as O
+    from paper_2511_22468_b200 import workloads as W
+    posm64, _ = W.make_state(cfg)
+    p64 = W.to_f32(posm64).astype(np.float64)            # the same fp32-rounded inputs the GPU sees
+    G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
+    opot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    probe = W.target_subset(cfg.n, size=min(cfg.n, 128), seed=7)
+    t0 = time.perf_counter()
+    O.pair_accel(p64, G, eps, targets=probe)
+    t_probe = max(time.perf_counter() - t0, 1e-6)
+    nt = int(min(cfg.n, max(128, seconds_target / t_probe * probe.size)))
+    targets = W.target_subset(cfg.n, size=nt)
+    t0 = time.perf_counter()
+    O.pair_accel(p64, G, eps, targets=targets)
+    O.ext_accel(p64[targets], G, opot)
+    dt = time.perf_counter() - t0
+    return {"value": nt * cfg.n / dt / 1e9, "unit": "G-int/s", "cores": O.num_threads(), "kind": "oracle",
+            "sample": "%d seeded targets x all %d sources of %s, one pair+ext evaluation, %.1f s"
+                      % (nt, cfg.n, cfg.name, dt)}, (p64, G, eps, opot)
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the fp64 CPU oracle on the host cores, same config/metric/unit (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    from paper_2511_22468_b200 import workloads as W
+    cfg = W.CONFIGS[args.config]
+    base, (p64, G, eps, opot) = _oracle_sample_rate(cfg, seconds_target=2.0)
+    # each step: a bounded sample (a seeded target subset) sized for ~4 s of CPU work
+    nt = int(min(cfg.n, max(128, base["value"] * 1e9 * 4.0 / cfg.n)))
+    targets = W.target_subset(cfg.n, size=nt)
+    times = []
+    for k in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        O.pair_accel(p64, G, eps, targets=targets)
+        O.ext_accel(p64[targets], G, opot)
+        if k >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = float(np.sum(times))
+    value = nt * cfg.n * args.steps / total / 1e9
+    sample = "%d seeded targets x all %d sources per step (of N^2 = %.3g)" % (nt, cfg.n, float(cfg.n) ** 2)
+    line = {
+        "impl": "reference", "metric": "pairwise interactions/s", "value": value, "unit": "G-int/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n": cfg.n, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "G-int/s", "cores": O.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "G-int/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def _steps_per_s(B, W, torch, ci: int, nsteps: int, dtype=np.float32):
+    """KDK steps/s of another config through one odisseo_leapfrog_kdk call (whole-step CUDA graph)."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg)
+    posm = torch.from_numpy(np.ascontiguousarray(posm64, dtype=dtype)).cuda()
+    vel = torch.from_numpy(W.vel4(vel64.astype(dtype), dtype)).cuda()
+    acc = torch.empty_like(posm)
+    ws = B.alloc_workspace(B.workspace_bytes(cfg.n, dtype == np.float64))
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, min(nsteps, 20), pot, ws)          # warm-up + graph build
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, ws, acc_valid=True)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    return {"workload": cfg.name, "dtype": "f32" if dtype == np.float32 else "f64", "steps": nsteps,
+            "steps_per_s": nsteps / (ms * 1e-3), "G_int_per_s": nsteps * float(cfg.n) ** 2 / (ms * 1e-3) / 1e9}
+
+
+def run_ours(args, rank: int, world: int, dist):
+    import torch
+    from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
+    from paper_2511_22468_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a B200: the hot path has no CPU fallback")
+    dev = torch.cuda.current_device()
+    cfg = W.CONFIGS[args.config]
+    n = cfg.n
+    posm64, vel64 = W.make_state(cfg, seed=cfg.seed + rank)               # one seeded replica per rank
+    p32, v32 = W.to_f32(posm64), W.vel4(W.to_f32(vel64), np.float32)
+    G, eps, dt = float(np.float32(cfg.G)), float(np.float32(cfg.eps)), float(np.float32(cfg.dt))
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    posm, vel = torch.from_numpy(p32).cuda(), torch.from_numpy(v32).cuda()
+    acc = torch.empty_like(posm)
+    ws = B.alloc_workspace(B.host_workspace_bytes(n))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+    K, Wm = args.steps, args.warmup
+
+    # ---- device-resident arm ----------------------------------------------------------------
+    B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 0, pot, ws)                 # initial a_pair(x0), untimed
+    for _ in range(Wm):
+        B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 1, pot, ws, acc_valid=True)
+        flush.zero_()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    _barrier(dist)
+    sampler = ClockSampler(dev)
+    sampler.start()
+    launches0 = B.launch_count()
+    B.profile_begin()
+    for k in range(K):
+        ev[k][0].record()
+        B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 1, pot, ws, acc_valid=True)
+        ev[k][1].record()
+        flush.zero_()                                                      # L2 flush between timed steps
+    torch.cuda.synchronize()
+    pair_ms, pair_launches, dropped = B.profile_end()
+    launches = B.launch_count() - launches0
+    clocks = sampler.stop()
+    _barrier(dist)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = _max_over_ranks(float(np.sum(step_ms)), dist)
+    value = world * K * float(n) ** 2 / (total_ms * 1e-3) / 1e9
+
+    # ---- end-to-end arm: host buffers through odisseo_leapfrog_kdk_host_f32 -------------------
+    hp, hv = torch.from_numpy(p32.copy()).pin_memory(), torch.from_numpy(v32.copy()).pin_memory()
+    ha = torch.empty_like(hp).pin_memory()
+    B.leapfrog_kdk_host(hp, hv, ha, G, eps, dt, 0, pot, ws)
+    torch.cuda.synchronize()
+    for _ in range(Wm):
+        B.leapfrog_kdk_host(hp, hv, ha, G, eps, dt, 1, pot, ws, acc_valid=True)
+        torch.cuda.synchronize()
+    _barrier(dist)
+    e2e_ms = 0.0
+    for k in range(K):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        B.leapfrog_kdk_host(hp, hv, ha, G, eps, dt, 1, pot, ws, acc_valid=True)   # H2D x,v,a + step + D2H x,v,a
+        b.record()
+        torch.cuda.synchronize()                                                     # host reads the result
+        e2e_ms += a.elapsed_time(b)
+        flush.zero_()
+    _barrier(dist)
+    e2e_ms = _max_over_ranks(e2e_ms, dist)
+    if rank != 0:
+        return
+
+    peaks, peak_kind = _peaks()
+    pair_avg_ms = pair_ms / max(pair_launches, 1)
+    achieved = FLOPS_PER_INTERACTION * float(n) ** 2 / (pair_avg_ms * 1e-3) / 1e12
+    line = {
+        "metric": "pairwise interactions/s", "value": value, "unit": "G-int/s", "n_gpus": world, "steps": K,
+        "warmup": Wm, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "n": n, "eps": cfg.eps, "dt": cfg.dt, "potential": "NFW+MN",
+                   "interactions_per_step": float(n) ** 2, "parallelism": "replicas x%d" % world,
+                   "l2": "256 MiB buffer rewritten between timed steps (outside the per-step events)",
+                   "plan": B.describe_plan(n)},
+        "kdk_steps_per_s": world * K / (total_ms * 1e-3),
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "e2e": {"value": world * K * float(n) ** 2 / (e2e_ms * 1e-3) / 1e9, "unit": "G-int/s",
+                "h2d_bytes_per_step": 3 * 16 * n, "d2h_bytes_per_step": 3 * 16 * n,
+                "ms_per_step": e2e_ms / K},
+        "roofline": {"bound": "alu", "kernel": "pair_f32x2_kernel", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
+                     "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                     "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz %s)"
+                                  % (SM_MAX_HZ / 1e6, peak_kind),
+                     "flops_per_interaction": FLOPS_PER_INTERACTION, "launch_ms": pair_avg_ms,
+                     "launches_timed": pair_launches, "launches_dropped": dropped,
+                     "share_of_step": pair_ms / float(np.sum(step_ms)),
+                     "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES},
+    }
+    if world == 1 and not args.no_extras:
+        line["cpu_baseline"] = _oracle_sample_rate(cfg, seconds_target=15.0)[0]
+        extras = [_steps_per_s(B, W, torch, 0, 1000, np.float64), _steps_per_s(B, W, torch, 0, 1000),
+                  _steps_per_s(B, W, torch, 1, 1000), _steps_per_s(B, W, torch, 2, 60)]
+        if args.config != 3:
+            extras.append(_steps_per_s(B, W, torch, 3, 5))
+        extras.append(_steps_per_s(B, W, torch, 3, 3, np.float64))
+        extras.append(_steps_per_s(B, W, torch, 4, 2))
+        line["other_configs"] = extras
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default: the headline)")
+    ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args, int(os.environ.get("RANK", "0")))
+        return 0
+    rank, world, dist = _dist_setup(args.gpus)
+    try:
+        run_ours(args, rank, world, dist)
+    finally:
+        if dist is not None:
+            dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -123,20 +123,35 @@ odisseo_status odisseo_leapfrog_kdk_f64(double *d_posm, double *d_vel, double *d
                                         const odisseo_potential *pot,
                                         void *d_workspace, size_t workspace_bytes, void *stream);
 
-/* Host-buffer face of the leapfrog (end-to-end path): copies h_posm, h_vel [n][4] to the
- * device, runs nsteps KDK steps, copies posm, vel and (if h_acc != NULL) the pair-only
- * acceleration back.  All copies are cudaMemcpyAsync on `stream`; host buffers should be
+/* Host-buffer face of the leapfrog (end-to-end path): copies h_posm, h_vel [n][4] (and, when
+ * acc_valid != 0, h_acc, which must then be non-NULL and hold a_pair(h_posm) as left by a
+ * previous call) to the device, runs nsteps KDK steps, copies posm, vel and (if h_acc != NULL)
+ * the pair-only acceleration back.  All copies are cudaMemcpyAsync on `stream`; host buffers should be
  * pinned for true asynchrony and must stay valid until the stream is synchronised.
  * d_workspace must hold odisseo_workspace_bytes(n, is_f64) + 3 state arrays
  * (3 * n * 16 bytes fp32, 3 * n * 32 bytes fp64) + 768 bytes, 256-byte aligned. */
-odisseo_status odisseo_leapfrog_kdk_host_f32(float *h_posm, float *h_vel, float *h_acc,
+odisseo_status odisseo_leapfrog_kdk_host_f32(float *h_posm, float *h_vel, float *h_acc, int acc_valid,
                                              int64_t n, float G, float eps, float dt, int64_t nsteps,
                                              const odisseo_potential *pot,
                                              void *d_workspace, size_t workspace_bytes, void *stream);
-odisseo_status odisseo_leapfrog_kdk_host_f64(double *h_posm, double *h_vel, double *h_acc,
+odisseo_status odisseo_leapfrog_kdk_host_f64(double *h_posm, double *h_vel, double *h_acc, int acc_valid,
                                              int64_t n, double G, double eps, double dt, int64_t nsteps,
                                              const odisseo_potential *pot,
                                              void *d_workspace, size_t workspace_bytes, void *stream);
+
+/* Instrumentation (bench.py's gpu_launches and roofline legs).
+ *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA
+ *     graph replay counts its kernel nodes).  Host counter, no GPU work.
+ *   odisseo_profile_begin / _end: between the two calls every pair-kernel launch (the O(N^2)
+ *     kernel only, not the O(N) kernels around it) is bracketed by a pair of CUDA events on
+ *     the stream it is launched on, and the leapfrog calls replay no graph (graph nodes
+ *     cannot be timed individually).  _end waits for the recorded launches and returns the
+ *     sum of their durations in milliseconds, how many were timed, and how many were not
+ *     because the pool of 4,096 event pairs ran out.  One profile at a time per process;
+ *     _end without _begin -> ERR_ARG.  Output pointers are HOST pointers and may be NULL. */
+int64_t odisseo_launch_count(void);
+odisseo_status odisseo_profile_begin(void);
+odisseo_status odisseo_profile_end(double *h_ms_total, int64_t *h_launches, int64_t *h_dropped);
 
 /* Description of the launch plan the library would use for n particles on the current
  * device (host arithmetic + one device-attribute query): fills out[0..7] with

@@ -24,7 +24,8 @@ EXPORTS = [
     "odisseo_pair_accel_f32", "odisseo_pair_accel_f64", "odisseo_pair_accel_soa_f32",
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
-    "odisseo_describe_plan_for", "odisseo_plan_probe",
+    "odisseo_describe_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
+    "odisseo_profile_end",
 ]
 
 
@@ -78,11 +79,15 @@ def lib():
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
-            getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
         L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        L.odisseo_launch_count.restype = i64
+        L.odisseo_launch_count.argtypes = []
+        L.odisseo_profile_begin.argtypes = []
+        L.odisseo_profile_end.argtypes = [vp, vp, vp]
         _lib = L
     return _lib
 
@@ -201,7 +206,8 @@ def leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: fl
 
 
 def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch.Tensor], G: float, eps: float,
-                      dt: float, nsteps: int, pot: Optional[Potential], workspace: torch.Tensor, stream=None):
+                      dt: float, nsteps: int, pot: Optional[Potential], workspace: torch.Tensor,
+                      acc_valid: bool = False, stream=None):
     """Host-buffer face: posm/vel/acc are (pinned) CPU tensors updated in place after a stream sync."""
     n = _rec(posm, "posm", cuda=False)
     _rec(vel, "vel", n, cuda=False)
@@ -211,6 +217,24 @@ def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch
         _rec(acc, "acc", n, cuda=False)
     sfx = _suffix(posm)
     fn = getattr(lib(), "odisseo_leapfrog_kdk_host_" + sfx)
-    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr() if acc is not None else None, n, G, eps, dt,
+    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr() if acc is not None else None, int(bool(acc_valid)),
+              n, G, eps, dt,
               int(nsteps), _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "leapfrog_kdk_host_" + sfx)
+
+
+def launch_count() -> int:
+    """Kernels launched by the library in this process so far (odisseo_launch_count)."""
+    return int(lib().odisseo_launch_count())
+
+
+def profile_begin():
+    """Start bracketing every pair-kernel launch with CUDA events (odisseo_profile_begin)."""
+    _check(lib().odisseo_profile_begin(), "profile_begin")
+
+
+def profile_end():
+    """(total ms of the timed pair-kernel launches, launches timed, launches dropped)."""
+    ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
+    return float(ms.value), int(nl.value), int(nd.value)

@@ -3,6 +3,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -49,6 +50,17 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
 namespace {
 
 thread_local int g_last_cuda_error = 0;
+
+// ---- instrumentation (include/odisseo.h "Instrumentation") --------------------------------
+std::atomic<int64_t> g_launches{0};
+struct Profile {
+    bool active = false;
+    std::vector<cudaEvent_t> ev;     // pairs (start, stop) around pair-kernel launches
+    size_t used = 0;                 // events used so far
+    int64_t dropped = 0;             // launches seen after the pool ran out
+};
+Profile g_prof;
+constexpr size_t PROFILE_MAX_LAUNCHES = 4096;
 
 odisseo_status cuda_fail(cudaError_t e)
 {
@@ -121,21 +133,41 @@ template <typename T> odisseo_status make_pot(T G, const odisseo_potential* pot,
 }
 
 // ---- typed launch shims ----------------------------------------------------------------
-inline cudaError_t launch_pair(const PairPlan& p, const float* x, const void* j, double* part, float eps, cudaStream_t s)
+inline cudaError_t launch_pair_raw(const PairPlan& p, const float* x, const void* j, double* part, float eps, cudaStream_t s)
 { return launch_pair_f32(p, x, j, part, eps, s); }
-inline cudaError_t launch_pair(const PairPlan& p, const double* x, const void* j, double* part, double eps, cudaStream_t s)
+inline cudaError_t launch_pair_raw(const PairPlan& p, const double* x, const void* j, double* part, double eps, cudaStream_t s)
 { return launch_pair_f64(p, x, j, part, eps, s); }
+// Pair-kernel launch; while a profile is open (and the stream is not capturing) it is bracketed
+// by a pair of CUDA events on the launching stream.
+template <typename T>
+cudaError_t launch_pair(const PairPlan& p, const T* x, const void* j, double* part, T eps, cudaStream_t s, bool capturing = false)
+{
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (!g_prof.active || capturing) return launch_pair_raw(p, x, j, part, eps, s);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (g_prof.used + 2 > g_prof.ev.size()) {
+        ++g_prof.dropped;
+        return launch_pair_raw(p, x, j, part, eps, s);
+    }
+    cudaError_t e = cudaEventRecord(g_prof.ev[g_prof.used], s);
+    if (e != cudaSuccess) return e;
+    e = launch_pair_raw(p, x, j, part, eps, s);
+    if (e != cudaSuccess) return e;
+    e = cudaEventRecord(g_prof.ev[g_prof.used + 1], s);
+    g_prof.used += 2;
+    return e;
+}
 inline cudaError_t launch_step(const PairPlan& p, float* x, float* v, float* a, void* j, const double* part, float G,
                                const PotParams<float>& pot, float dt, int flags, cudaStream_t s)
-{ return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, s); }
 inline cudaError_t launch_step(const PairPlan& p, double* x, double* v, double* a, void* j, const double* part, double G,
                                const PotParams<double>& pot, double dt, int flags, cudaStream_t s)
-{ return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, s); }
 
 inline cudaError_t launch_ext(const float* x, float* a, int64_t n, const PotParams<float>& pot, int accumulate, cudaStream_t s)
-{ return launch_ext_f32(x, a, n, pot, accumulate, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_ext_f32(x, a, n, pot, accumulate, s); }
 inline cudaError_t launch_ext(const double* x, double* a, int64_t n, const PotParams<double>& pot, int accumulate, cudaStream_t s)
-{ return launch_ext_f64(x, a, n, pot, accumulate, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_ext_f64(x, a, n, pot, accumulate, s); }
 
 struct Carve { void* jsrc; double* partials; };
 
@@ -255,7 +287,7 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     int first = 0;
     if (!acc_valid) {
         ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_PACK_ONLY, s));
-        ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+        ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
         first = STEP_FROM_PARTIALS;
     }
     if (nsteps == 0) {
@@ -267,7 +299,9 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     int64_t mid = nsteps - 1;     // full steps: pair + (close, open)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
-    const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2;
+    // no graph on the legacy stream, inside a caller's capture, or while a profile is open
+    // (event pairs around the pair kernels cannot be read back from graph nodes)
+    const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2 && !g_prof.active;
     if (use_graph) {
         const int block = (int)(mid < 16 ? mid : 16);
         GraphKey key;
@@ -285,14 +319,16 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
         if (!exec) {
             cudaGraph_t graph = nullptr;
             ODISSEO_TRY(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+            const int64_t counted = g_launches.load();   // captured launches run at replay, not now
             cudaError_t ce = cudaSuccess;
             for (int k = 0; k < block && ce == cudaSuccess; ++k) {
-                ce = launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s);
+                ce = launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s, true);
                 if (ce == cudaSuccess)
                     ce = launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
                                      STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s);
             }
             e = cudaStreamEndCapture(s, &graph);
+            g_launches.store(counted);
             if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return cuda_fail(ce); }
             if (e != cudaSuccess) return cuda_fail(e);
             e = cudaGraphInstantiate(&exec, graph, 0);
@@ -310,26 +346,27 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
         }
         while (mid >= block) {
             ODISSEO_TRY(cudaGraphLaunch(exec, s));
+            g_launches.fetch_add(2 * block, std::memory_order_relaxed);
             mid -= block;
         }
     }
     for (; mid > 0; --mid) {
-        ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+        ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
         ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
                                 STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s));
     }
-    ODISSEO_TRY(launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s));
+    ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
     ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE, s));
     return ODISSEO_OK;
 }
 
 template <typename T>
-odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int64_t n, T G, T eps, T dt, int64_t nsteps,
+odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
                                   const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
 {
     if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
     if (n == 0) return ODISSEO_OK;
-    if (!h_posm || !h_vel || !ws) return ODISSEO_ERR_NULL;
+    if (!h_posm || !h_vel || !ws || (acc_valid && !h_acc)) return ODISSEO_ERR_NULL;
     if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
     const size_t arr = ((size_t)n * 4 * sizeof(T) + 255) & ~(size_t)255;
     if (ws_bytes < 3 * arr) return ODISSEO_ERR_WORKSPACE;
@@ -341,7 +378,8 @@ odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int64_t n, T G,
     cudaError_t e;
     ODISSEO_TRY(cudaMemcpyAsync(d_posm, h_posm, (size_t)n * 4 * sizeof(T), cudaMemcpyHostToDevice, s));
     ODISSEO_TRY(cudaMemcpyAsync(d_vel, h_vel, (size_t)n * 4 * sizeof(T), cudaMemcpyHostToDevice, s));
-    odisseo_status st = leapfrog_impl<T>(d_posm, d_vel, d_acc, 0, n, G, eps, dt, nsteps, pot, base + 3 * arr,
+    if (acc_valid) ODISSEO_TRY(cudaMemcpyAsync(d_acc, h_acc, (size_t)n * 4 * sizeof(T), cudaMemcpyHostToDevice, s));
+    odisseo_status st = leapfrog_impl<T>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, base + 3 * arr,
                                          ws_bytes - 3 * arr, stream);
     if (st != ODISSEO_OK) return st;
     ODISSEO_TRY(cudaMemcpyAsync(h_posm, d_posm, (size_t)n * 4 * sizeof(T), cudaMemcpyDeviceToHost, s));
@@ -375,6 +413,46 @@ const char* odisseo_status_string(odisseo_status s)
 }
 
 int odisseo_last_cuda_error(void) { return g_last_cuda_error; }
+
+int64_t odisseo_launch_count(void) { return g_launches.load(); }
+
+odisseo_status odisseo_profile_begin(void)
+{
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    while (g_prof.ev.size() < 2 * PROFILE_MAX_LAUNCHES) {
+        cudaEvent_t ev;
+        cudaError_t e = cudaEventCreate(&ev);
+        if (e != cudaSuccess) return cuda_fail(e);
+        g_prof.ev.push_back(ev);
+    }
+    g_prof.used = 0;
+    g_prof.dropped = 0;
+    g_prof.active = true;
+    return ODISSEO_OK;
+}
+
+odisseo_status odisseo_profile_end(double* h_ms_total, int64_t* h_launches, int64_t* h_dropped)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (!g_prof.active) return ODISSEO_ERR_ARG;
+    g_prof.active = false;
+    double total = 0.0;
+    for (size_t k = 0; k + 1 < g_prof.used; k += 2) {
+        cudaError_t e = cudaEventSynchronize(g_prof.ev[k + 1]);
+        if (e != cudaSuccess) return cuda_fail(e);
+        float ms = 0.f;
+        e = cudaEventElapsedTime(&ms, g_prof.ev[k], g_prof.ev[k + 1]);
+        if (e != cudaSuccess) return cuda_fail(e);
+        total += (double)ms;
+    }
+    if (h_ms_total) *h_ms_total = total;
+    if (h_launches) *h_launches = (int64_t)(g_prof.used / 2);
+    if (h_dropped) *h_dropped = g_prof.dropped;
+    return ODISSEO_OK;
+}
 
 size_t odisseo_workspace_bytes(int64_t n, int is_f64)
 {
@@ -448,6 +526,7 @@ odisseo_status odisseo_pair_accel_soa_f32(const float* d_x, const float* d_y, co
     float* posm = reinterpret_cast<float*>(base);
     float* acc = reinterpret_cast<float*>(base + arr);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
+    g_launches.fetch_add(2, std::memory_order_relaxed);
     cudaError_t e = launch_soa_pack_f32(d_x, d_y, d_z, d_m, posm, n, s);
     if (e != cudaSuccess) return cuda_fail(e);
     st = pair_accel_impl<float>(posm, acc, n, G, eps, base + 2 * arr, workspace_bytes - 2 * arr, stream);
@@ -475,14 +554,14 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
                                         void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
 
-odisseo_status odisseo_leapfrog_kdk_host_f32(float* h_posm, float* h_vel, float* h_acc, int64_t n, float G, float eps,
+odisseo_status odisseo_leapfrog_kdk_host_f32(float* h_posm, float* h_vel, float* h_acc, int acc_valid, int64_t n, float G, float eps,
                                              float dt, int64_t nsteps, const odisseo_potential* pot,
                                              void* d_workspace, size_t workspace_bytes, void* stream)
-{ return leapfrog_host_impl<float>(h_posm, h_vel, h_acc, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+{ return leapfrog_host_impl<float>(h_posm, h_vel, h_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
 
-odisseo_status odisseo_leapfrog_kdk_host_f64(double* h_posm, double* h_vel, double* h_acc, int64_t n, double G,
+odisseo_status odisseo_leapfrog_kdk_host_f64(double* h_posm, double* h_vel, double* h_acc, int acc_valid, int64_t n, double G,
                                              double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
                                              void* d_workspace, size_t workspace_bytes, void* stream)
-{ return leapfrog_host_impl<double>(h_posm, h_vel, h_acc, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+{ return leapfrog_host_impl<double>(h_posm, h_vel, h_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
 
 }  // extern "C"

@@ -297,6 +297,40 @@ def test_leapfrog_host_face_matches_device_face_bitwise():
     assert hp.numpy().tobytes() == ref[0].tobytes()
     assert hv.numpy().tobytes() == ref[1].tobytes()
     assert ha.numpy().tobytes() == ref[2].tobytes()
+    # chained host calls re-upload the pair-only acceleration (acc_valid) and stay bit-identical
+    hp2 = torch.from_numpy(p32.copy()).pin_memory()
+    hv2 = torch.from_numpy(v32.copy()).pin_memory()
+    ha2 = torch.empty_like(hp2).pin_memory()
+    B.leapfrog_kdk_host(hp2, hv2, ha2, cfg.G, cfg.eps, cfg.dt, 3, pot, ws)
+    torch.cuda.synchronize()
+    B.leapfrog_kdk_host(hp2, hv2, ha2, cfg.G, cfg.eps, cfg.dt, 4, pot, ws, acc_valid=True)
+    torch.cuda.synchronize()
+    assert hp2.numpy().tobytes() == ref[0].tobytes()
+    assert hv2.numpy().tobytes() == ref[1].tobytes()
+    assert ha2.numpy().tobytes() == ref[2].tobytes()
+
+
+def test_launch_count_and_pair_kernel_profile():
+    """Instrumentation used by bench.py: the launch counter counts graph-replayed kernels, and a
+    profile brackets exactly the pair-kernel launches without changing results."""
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.make_state(cfg, n=2048)
+    p32, v32 = W.to_f32(posm64), W.to_f32(vel64)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    c0 = B.launch_count()
+    ref = gpu_leapfrog(p32, v32, cfg.G, cfg.eps, cfg.dt, 40, pot, np.float32)     # graph replay inside
+    c1 = B.launch_count()
+    # pack + pair + open, then 40 x (pair + step)
+    assert c1 - c0 == 3 + 2 * 40
+    B.profile_begin()
+    got = gpu_leapfrog(p32, v32, cfg.G, cfg.eps, cfg.dt, 40, pot, np.float32)     # no graph while profiling
+    ms, timed, dropped = B.profile_end()
+    assert B.launch_count() - c1 == 3 + 2 * 40
+    assert timed == 41 and dropped == 0 and ms > 0
+    for x, y in zip(ref, got):
+        assert x.tobytes() == y.tobytes()
+    with pytest.raises(B.OdisseoError):
+        B.profile_end()
 
 
 def test_leapfrog_conserves_lz_and_tracks_single_particle_orbit_f32():
