@@ -20,9 +20,12 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     p.variant = (n <= 4096) ? 1 : 0;
     int minb;
     if (p.variant == 0) {
+        // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
+        // packed interaction chains of a thread (2 warps per scheduler x ILP 4 beats 4.5 warps x ILP 1:
+        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144, profiles/r01_pair_f32_variants.txt)
         p.ipt = is_f64 ? 4 : 8;
         p.cthreads = 256;
-        minb = 2;
+        minb = is_f64 ? 2 : 1;
     } else {
         p.ipt = 2;
         p.cthreads = 64;
@@ -32,7 +35,7 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     p.IB = p.ipt * p.cthreads;
     p.nb = (int32_t)((n + p.IB - 1) / p.IB);
     int64_t P = (int64_t)num_sms * minb;
-    int32_t T = 256;
+    int32_t T = (p.variant == 0 && !is_f64) ? 512 : 256;
     for (; T > 32; T >>= 1) {
         const int64_t U = (int64_t)p.nb * ((n + T - 1) / T);
         if (U >= 8 * P) break;
@@ -459,7 +462,7 @@ size_t odisseo_workspace_bytes(int64_t n, int is_f64)
     if (n <= 0) return 0;
     // bound over devices with up to 192 SMs: more CTAs -> more partial rows, smaller tiles -> same padding bound
     const PairPlan p = make_plan(n, is_f64, 192);
-    const size_t jsrc = (((size_t)(n + 256) * p.rec_bytes) + 255) & ~(size_t)255;
+    const size_t jsrc = (((size_t)(n + 512) * p.rec_bytes) + 255) & ~(size_t)255;
     return jsrc + (size_t)p.slots * 3 * p.IB * sizeof(double);
 }
 

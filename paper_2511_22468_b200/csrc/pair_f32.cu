@@ -23,7 +23,7 @@ namespace {
 
 constexpr int STAGES = 4;
 
-template <int NPAIR, int CWARPS, int MINB>
+template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
 __global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
 pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsrc, double* __restrict__ partials,
                   const PairPlan plan, const float eps2)
@@ -95,9 +95,12 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
                 i1 = i1 < plan.n ? i1 : plan.n - 1;
                 const float4 p0 = __ldg(posm + i0);
                 const float4 p1 = __ldg(posm + i1);
-                xi[p] = pk(p0.x, p1.x);
-                yi[p] = pk(p0.y, p1.y);
-                zi[p] = pk(p0.z, p1.z);
+                // x + (-0) == x exactly; routing the pack through FADD2 makes the pair a native 64-bit
+                // register value, so ptxas does not re-assemble it with MOVs inside the j loop
+                const f32x2 nz = pk(-0.0f, -0.0f);
+                xi[p] = add2(pk(p0.x, p1.x), nz);
+                yi[p] = add2(pk(p0.y, p1.y), nz);
+                zi[p] = add2(pk(p0.z, p1.z), nz);
                 ax[p] = ay[p] = az[p] = 0ull;
             }
 #pragma unroll
@@ -107,7 +110,7 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
 
         mbar_wait(&full_bar[s], ph);
         const ulonglong2* __restrict__ tile = reinterpret_cast<const ulonglong2*>(smem_raw + (size_t)s * tile_bytes);
-#pragma unroll 4
+#pragma unroll JUNROLL
         for (int j = 0; j < plan.T; ++j) {
             const ulonglong2 A = tile[2 * j];        // {x,x},{y,y}
             const ulonglong2 B = tile[2 * j + 1];    // {z,z},{m,m}
@@ -160,12 +163,12 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
     }
 }
 
-template <int NPAIR, int CWARPS, int MINB>
+template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
 cudaError_t launch_variant(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
                            cudaStream_t stream)
 {
     const size_t smem = (size_t)STAGES * plan.T * 32 + (size_t)6 * NPAIR * CWARPS * 32 * sizeof(double);
-    pair_f32x2_kernel<NPAIR, CWARPS, MINB><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
+    pair_f32x2_kernel<NPAIR, CWARPS, MINB, JUNROLL><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
         reinterpret_cast<const float4*>(posm), reinterpret_cast<const uint4*>(jsrc), partials, plan, eps * eps);
     return cudaGetLastError();
 }
@@ -174,8 +177,8 @@ cudaError_t launch_variant(const PairPlan& plan, const float* posm, const void* 
 
 cudaError_t configure_pair_f32()
 {
-    cudaError_t e = cudaFuncSetAttribute(pair_f32x2_kernel<4, 8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         STAGES * 256 * 32 + 6 * 4 * 8 * 32 * 8);
+    cudaError_t e = cudaFuncSetAttribute(pair_f32x2_kernel<4, 8, 1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         STAGES * 512 * 32 + 6 * 4 * 8 * 32 * 8);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(pair_f32x2_kernel<1, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 STAGES * 256 * 32 + 6 * 1 * 2 * 32 * 8);
@@ -184,7 +187,7 @@ cudaError_t configure_pair_f32()
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
                             cudaStream_t stream)
 {
-    if (plan.variant == 0) return launch_variant<4, 8, 2>(plan, posm, jsrc, partials, eps, stream);
+    if (plan.variant == 0) return launch_variant<4, 8, 1, 8>(plan, posm, jsrc, partials, eps, stream);
     return launch_variant<1, 2, 8>(plan, posm, jsrc, partials, eps, stream);
 }
 
