@@ -24,8 +24,8 @@ import numpy as np
 FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star convention
 SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
-# dram bytes per pair-kernel launch at N = 262,144 from profiles/ (ncu --set full); None until captured
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144 (ncu --set full)
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 13152768    # profiles/r01_pair_f32_ncu_full.txt: 13.15 MB read + 0 written
 
 
 def _peaks():
@@ -291,7 +291,7 @@ def run_ours(args, rank: int, world: int, dist):
                      "flops_per_interaction": FLOPS_PER_INTERACTION, "launch_ms": pair_avg_ms,
                      "launches_timed": pair_launches, "launches_dropped": dropped,
                      "share_of_step": pair_ms / float(np.sum(step_ms)),
-                     "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES},
+                     "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES if args.config == 3 else None},
     }
     if world == 1 and not args.no_extras:
         line["cpu_baseline"] = _oracle_sample_rate(cfg, seconds_target=15.0)[0]
