@@ -25,7 +25,7 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
         // 68.9 % vs 60.2 % of FP32 peak at N = 262,144, profiles/r01_pair_f32_variants.txt)
         p.ipt = is_f64 ? 4 : 8;
         p.cthreads = 256;
-        minb = is_f64 ? 2 : 1;
+        minb = 1;
     } else {
         p.ipt = 2;
         p.cthreads = 64;
@@ -111,7 +111,7 @@ template <typename T> odisseo_status check_pair_scalars(T G, T eps)
 {
     if (!isfinite((double)G) || !isfinite((double)eps) || !(eps > (T)0)) return ODISSEO_ERR_ARG;
     const double e2 = (double)eps * (double)eps;
-    if (e2 < 1e-30 || e2 > 1e30) return ODISSEO_ERR_ARG;   // fp32 rsqrt seed range (pair_f64.cu)
+    if (e2 < 1e-30 || e2 > 1e30) return ODISSEO_ERR_ARG;   // keeps eps^2 and r2 inside the fp32 normal range
     return ODISSEO_OK;
 }
 

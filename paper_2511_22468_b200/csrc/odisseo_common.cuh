@@ -143,6 +143,12 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+// Double-precision reciprocal-square-root seed (MUFU.RSQ64H): ~22 good bits, low word zero.
+__device__ __forceinline__ double rsqrt_approx_f64(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    return r;
+}
 #endif  // __CUDACC__
 
 // launchers (defined in pair_f32.cu / pair_f64.cu / integrate.cu)

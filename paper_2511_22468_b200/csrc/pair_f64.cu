@@ -2,11 +2,13 @@
 //
 // Same persistent stream-K / TMA-ring structure as pair_f32.cu; sources are plain
 // {x, y, z, m} double records (32 B) copied into a zero-mass-padded staging array.
-// r^-1 = (r2)^-1/2 is an fp32 MUFU.RSQ seed (relative error ~2^-22 plus the fp32 rounding of
-// r2) refined by ONE third-order step  y' = y + y e (1/2 + 3/8 e),  e = 1 - r2 y^2,
-// whose remainder (5/16) e^3 ~ 1e-21 is far below fp64 rounding: 5 FP64 ops instead of the
-// ~20 of the library rsqrt().  The seed needs r2 inside the fp32 normal range; api.cu rejects
-// eps^2 outside [1e-30, 1e30] and larger r2 saturates to a zero contribution.
+// (r2)^-3/2 comes from the double-precision seed y0 = rsqrt.approx.ftz.f64(r2) (MUFU.RSQ64H on the
+// high word: relative error ~2^-22, low word zero, no F2F conversions) and ONE correction of the
+// cube:  t = y0^2,  e = 1 - r2 t,  (r2)^-3/2 = y0^3 (1-e)^-3/2 = y0^3 (1 + e (3/2 + 15/8 e)) + O(e^3),
+// remainder (35/16) e^3 ~ 2e-19: 7 FP64 ops for m (r2)^-3/2 instead of ~20 with the library rsqrt().
+// 16 FP64-pipe ops + 1 MUFU per interaction (3 DADD, 9 DFMA, 4 DMUL).  A DFMA holds a scheduler's
+// dispatch port 2 cycles and every other instruction 1, so F2F or integer conversions around an fp32
+// seed cost as much as the arithmetic they feed.
 // Sums are kept in fp64 registers for the whole segment (no tile flush needed).
 #include "odisseo_common.cuh"
 
@@ -16,7 +18,7 @@ namespace {
 
 constexpr int STAGES = 4;
 
-template <int IPT, int CWARPS, int MINB>
+template <int IPT, int CWARPS, int MINB, int JUNROLL>
 __global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
 pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ jsrc, double* __restrict__ partials,
                 const PairPlan plan, const double eps2)
@@ -85,7 +87,7 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
 
         mbar_wait(&full_bar[s], ph);
         const double4* __restrict__ tile = reinterpret_cast<const double4*>(smem_raw + (size_t)s * tile_bytes);
-#pragma unroll 2
+#pragma unroll JUNROLL
         for (int j = 0; j < plan.T; ++j) {
             const double4 q = tile[j];
 #pragma unroll
@@ -96,10 +98,11 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
                 double r2 = fma(dx, dx, eps2);
                 r2 = fma(dy, dy, r2);
                 r2 = fma(dz, dz, r2);
-                const double y0 = (double)rsqrt_approx((float)r2);
-                const double e = fma(-r2 * y0, y0, 1.0);
-                const double y = fma(y0 * e, fma(0.375, e, 0.5), y0);
-                const double w = (y * y) * (q.w * y);
+                const double y0 = rsqrt_approx_f64(r2);
+                const double t = y0 * y0;
+                const double e = fma(-r2, t, 1.0);
+                const double c = fma(e, fma(1.875, e, 1.5), 1.0);
+                const double w = ((t * y0) * q.w) * c;
                 ax[k] = fma(w, dx, ax[k]);
                 ay[k] = fma(w, dy, ay[k]);
                 az[k] = fma(w, dz, az[k]);
@@ -125,12 +128,12 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
     }
 }
 
-template <int IPT, int CWARPS, int MINB>
+template <int IPT, int CWARPS, int MINB, int JUNROLL>
 cudaError_t launch_variant(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
                            cudaStream_t stream)
 {
     const size_t smem = (size_t)STAGES * plan.T * 32;
-    pair_f64_kernel<IPT, CWARPS, MINB><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
+    pair_f64_kernel<IPT, CWARPS, MINB, JUNROLL><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
         reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(jsrc), partials, plan, eps * eps);
     return cudaGetLastError();
 }
@@ -139,18 +142,18 @@ cudaError_t launch_variant(const PairPlan& plan, const double* posm, const void*
 
 cudaError_t configure_pair_f64()
 {
-    cudaError_t e = cudaFuncSetAttribute(pair_f64_kernel<4, 8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(pair_f64_kernel<4, 8, 1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          STAGES * 256 * 32);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_f64_kernel<2, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(pair_f64_kernel<2, 2, 8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 STAGES * 256 * 32);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
                             cudaStream_t stream)
 {
-    if (plan.variant == 0) return launch_variant<4, 8, 2>(plan, posm, jsrc, partials, eps, stream);
-    return launch_variant<2, 2, 8>(plan, posm, jsrc, partials, eps, stream);
+    if (plan.variant == 0) return launch_variant<4, 8, 1, 4>(plan, posm, jsrc, partials, eps, stream);
+    return launch_variant<2, 2, 8, 2>(plan, posm, jsrc, partials, eps, stream);
 }
 
 }  // namespace odisseo
