@@ -358,3 +358,51 @@ def test_workspace_too_small_and_bad_alignment_are_reported():
         B.pair_accel(posm, acc, 1.0, 0.1, ws[16:])
     with pytest.raises(B.OdisseoError, match="ERR_ARG"):
         B.pair_accel(posm, posm, 1.0, 0.1, ws)
+
+
+@pytest.mark.parametrize("ci,dtype", [(3, np.float32), (4, np.float32), (3, np.float64)])
+def test_full_size_step_resynchronised_parity_and_one_step_shadowing(ci, dtype):
+    """SURVEY.md 8c (ii)+(iii) at BASELINE.json's full sizes, in the launch configuration bench.py times
+    (one odisseo_leapfrog_kdk call per step, acc_valid = 1).  From the GPU's own state at step k the
+    oracle advances the seeded 4,096 targets one KDK step in fp64 (all sources); the GPU state at k+1
+    must agree to |dx| <= 1e-6 |x| and |dv| <= 1e-6 |v| + 1.5e-5 |dt| (S_i + |a_ext,i|) in fp32
+    (1e-12 / 1e-12 + 1e-11 in fp64), and the acc the call leaves is a_pair of its own final state."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg)
+    f32 = dtype == np.float32
+    p0, v0 = posm64.astype(dtype), vel64.astype(dtype)
+    G, eps, dt = ((float(np.float32(t)) for t in (cfg.G, cfg.eps, cfg.dt)) if f32 else (cfg.G, cfg.eps, cfg.dt))
+    bpot, opot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn), O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    posm, vel = dev(p0, dtype), dev(W.vel4(v0, dtype), dtype)
+    acc = torch.full_like(posm, float("nan"))
+    ws = B.alloc_workspace(B.workspace_bytes(cfg.n, not f32))
+    B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 0, bpot, ws)                      # a_pair(x0)
+    B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 1, bpot, ws, acc_valid=True)      # step 1
+    torch.cuda.synchronize()
+    pk, vk, ak = (t.cpu().numpy().astype(np.float64) for t in (posm, vel, acc))
+    B.leapfrog_kdk(posm, vel, acc, G, eps, dt, 1, bpot, ws, acc_valid=True)      # step 2 = k -> k+1
+    torch.cuda.synchronize()
+    p1, v1, a1 = (t.cpu().numpy().astype(np.float64) for t in (posm, vel, acc))
+    assert np.array_equal(p1[:, 3], p0[:, 3].astype(np.float64))                 # masses preserved
+
+    idx = W.target_subset(cfg.n)
+    tol_a = TOL_F32 if f32 else TOL_F64
+    # (ii) re-synchronised: acc == a_pair(own state), at k and at k+1
+    assert pair_ratio(ak, pk, G, eps, targets=idx) <= tol_a
+    assert pair_ratio(a1, p1, G, eps, targets=idx) <= tol_a
+    # (iii) one oracle KDK step for the targets, from the GPU state at k
+    a_pair_k, S_k = O.pair_accel(pk, G, eps, targets=idx)
+    a_k = a_pair_k + O.ext_accel(pk[idx], G, opot)
+    v_half = vk[idx, :3] + 0.5 * dt * a_k
+    x_new = pk[idx, :3] + dt * v_half
+    src = p1.copy()
+    src[idx, :3] = x_new                                                          # targets at the oracle's x(k+1)
+    a_pair_1, S_1 = O.pair_accel(src, G, eps, targets=idx)
+    a_1 = a_pair_1 + O.ext_accel(src[idx], G, opot)
+    v_new = v_half + 0.5 * dt * a_1
+    dx = np.linalg.norm(p1[idx, :3] - x_new, axis=1)
+    dv = np.linalg.norm(v1[idx, :3] - v_new, axis=1)
+    aext = np.linalg.norm(a_1 - a_pair_1, axis=1)
+    rx, rv, ra = (1e-6, 1e-6, 1.5e-5) if f32 else (1e-12, 1e-12, 1e-11)
+    assert np.all(dx <= rx * np.linalg.norm(x_new, axis=1))
+    assert np.all(dv <= rv * np.linalg.norm(v_new, axis=1) + ra * abs(dt) * (np.maximum(S_k, S_1) + aext))
