@@ -462,7 +462,7 @@ size_t odisseo_workspace_bytes(int64_t n, int is_f64)
     if (n <= 0) return 0;
     // bound over devices with up to 192 SMs: more CTAs -> more partial rows, smaller tiles -> same padding bound
     const PairPlan p = make_plan(n, is_f64, 192);
-    const size_t jsrc = (((size_t)(n + 512) * p.rec_bytes) + 255) & ~(size_t)255;
+    const size_t jsrc = (((size_t)(n + 512) * p.rec_bytes + ((size_t)(n + 512) / STEP_THREADS + 1) * sizeof(int)) + 255) & ~(size_t)255;
     return jsrc + (size_t)p.slots * 3 * p.IB * sizeof(double);
 }
 

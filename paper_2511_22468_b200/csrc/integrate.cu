@@ -72,7 +72,8 @@ __device__ __forceinline__ void ext_accel(const PotParams<T>& pot, T x, T y, T z
 }
 
 // Staged source record writers.  fp32: {x,x,y,y},{z,z,m,m} (pre-duplicated packed operands);
-// fp64: plain {x,y,z,m}.  Records [n, n_pad) are zero-mass padding.
+// fp64: plain {x,y,z,m}.  Records [n, n_pad) are massless padding parked far away
+// (odisseo_common.cuh PAD_POS_*).
 __device__ __forceinline__ void stage_record(void* jsrc, int64_t i, float x, float y, float z, float m)
 {
     float4* out = reinterpret_cast<float4*>(jsrc) + 2 * i;
@@ -84,77 +85,85 @@ __device__ __forceinline__ void stage_record(void* jsrc, int64_t i, double x, do
     reinterpret_cast<double4*>(jsrc)[i] = make_double4(x, y, z, m);
 }
 
+__device__ __forceinline__ float pad_pos(float) { return PAD_POS_F32; }
+__device__ __forceinline__ double pad_pos(double) { return PAD_POS_F64; }
+
 template <typename T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(STEP_THREADS)
 step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
             typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
             const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags)
 {
     typedef typename Vec4<T>::type V4;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t npad = plan_npad(plan);
-    if (i >= npad) return;
-    if (i >= plan.n) {
-        if (flags & (STEP_OPEN | STEP_PACK_ONLY)) stage_record(jsrc, i, (T)0, (T)0, (T)0, (T)0);
-        return;
-    }
-    V4 p = posm[i];
-    if (flags & STEP_PACK_ONLY) {
-        stage_record(jsrc, i, p.x, p.y, p.z, p.w);
-        return;
-    }
-
-    T apx, apy, apz;
-    if (flags & STEP_FROM_PARTIALS) {
-        const int32_t b = (int32_t)(i / plan.IB);
-        const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
-        const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
-        const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
-        double sx = 0.0, sy = 0.0, sz = 0.0;
-        // fixed order: increasing j.  Rows are fetched REDUCE_BATCH at a time so the L2 latencies of a
-        // batch overlap (a plain loop serialises one ~1 us round trip per row: 32 rows at N = 1,024);
-        // absent rows add +0.0, which leaves the sum unchanged.
-        constexpr int REDUCE_BATCH = 8;
-        for (int32_t c = c0; c <= c1; c += REDUCE_BATCH) {
-            double vx[REDUCE_BATCH], vy[REDUCE_BATCH], vz[REDUCE_BATCH];
+    const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
+    int mass_differs = 0;
+    if (i < plan.n) {
+        V4 p = posm[i];
+        if (flags & STEP_PACK_ONLY) {
+            stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+        } else {
+            T apx, apy, apz;
+            if (flags & STEP_FROM_PARTIALS) {
+                const int32_t b = (int32_t)(i / plan.IB);
+                const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
+                const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
+                const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
+                double sx = 0.0, sy = 0.0, sz = 0.0;
+                // fixed order: increasing j.  Rows are fetched REDUCE_BATCH at a time so the L2 latencies
+                // of a batch overlap (a plain loop serialises one ~1 us round trip per row: 32 rows at
+                // N = 1,024); absent rows add +0.0, which leaves the sum unchanged.
+                constexpr int REDUCE_BATCH = 8;
+                for (int32_t c = c0; c <= c1; c += REDUCE_BATCH) {
+                    double vx[REDUCE_BATCH], vy[REDUCE_BATCH], vz[REDUCE_BATCH];
 #pragma unroll
-            for (int k = 0; k < REDUCE_BATCH; ++k) {
-                const bool live = c + k <= c1;
-                const double* row = partials + (size_t)(c + (live ? k : 0) + b) * 3 * plan.IB;
-                vx[k] = live ? __ldcg(row + r) : 0.0;
-                vy[k] = live ? __ldcg(row + plan.IB + r) : 0.0;
-                vz[k] = live ? __ldcg(row + 2 * plan.IB + r) : 0.0;
+                    for (int k = 0; k < REDUCE_BATCH; ++k) {
+                        const bool live = c + k <= c1;
+                        const double* row = partials + (size_t)(c + (live ? k : 0) + b) * 3 * plan.IB;
+                        vx[k] = live ? __ldcg(row + r) : 0.0;
+                        vy[k] = live ? __ldcg(row + plan.IB + r) : 0.0;
+                        vz[k] = live ? __ldcg(row + 2 * plan.IB + r) : 0.0;
+                    }
+#pragma unroll
+                    for (int k = 0; k < REDUCE_BATCH; ++k) { sx += vx[k]; sy += vy[k]; sz += vz[k]; }
+                }
+                apx = (T)((double)G * sx);
+                apy = (T)((double)G * sy);
+                apz = (T)((double)G * sz);
+                V4 a; a.x = apx; a.y = apy; a.z = apz; a.w = (T)0;
+                acc[i] = a;
+            } else {
+                const V4 a = acc[i];
+                apx = a.x; apy = a.y; apz = a.z;
             }
-#pragma unroll
-            for (int k = 0; k < REDUCE_BATCH; ++k) { sx += vx[k]; sy += vy[k]; sz += vz[k]; }
+            if (flags & (STEP_CLOSE | STEP_OPEN)) {
+                T ex, ey, ez;
+                ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
+                const T tx = apx + ex, ty = apy + ey, tz = apz + ez;
+                const T h = (T)0.5 * dt;
+                V4 v = vel[i];
+                if (flags & STEP_CLOSE) {
+                    v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+                }
+                if (flags & STEP_OPEN) {
+                    v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+                    p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
+                    posm[i] = p;
+                    stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+                }
+                v.w = (T)0;
+                vel[i] = v;
+            }
         }
-        apx = (T)((double)G * sx);
-        apy = (T)((double)G * sy);
-        apz = (T)((double)G * sz);
-        V4 a; a.x = apx; a.y = apy; a.z = apz; a.w = (T)0;
-        acc[i] = a;
-    } else {
-        const V4 a = acc[i];
-        apx = a.x; apy = a.y; apz = a.z;
+        if (staging) mass_differs = !(p.w == *(const volatile T*)&posm[0].w);   // masses never change; NaN counts as different
+    } else if (staging && i < plan_npad(plan)) {
+        const T far = pad_pos((T)0);
+        stage_record(jsrc, i, far, far, far, (T)0);
     }
-    if (!(flags & (STEP_CLOSE | STEP_OPEN))) return;
-
-    T ex, ey, ez;
-    ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
-    const T tx = apx + ex, ty = apy + ey, tz = apz + ez;
-    const T h = (T)0.5 * dt;
-    V4 v = vel[i];
-    if (flags & STEP_CLOSE) {
-        v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+    if (staging) {                                                     // uniform branch: flags is a kernel argument
+        const int any = __syncthreads_or(mass_differs);
+        if (threadIdx.x == 0) const_cast<int*>(plan_flags(jsrc, plan))[blockIdx.x] = any;
     }
-    if (flags & STEP_OPEN) {
-        v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
-        p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
-        posm[i] = p;
-        stage_record(jsrc, i, p.x, p.y, p.z, p.w);
-    }
-    v.w = (T)0;
-    vel[i] = v;
 }
 
 template <typename T>
@@ -205,7 +214,7 @@ cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
                             cudaStream_t stream)
 {
-    step_kernel<float><<<grid_for(plan_npad(plan)), 256, 0, stream>>>(
+    step_kernel<float><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
         reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
         partials, plan, G, pot, dt, flags);
     return cudaGetLastError();
@@ -215,7 +224,7 @@ cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, dou
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
                             cudaStream_t stream)
 {
-    step_kernel<double><<<grid_for(plan_npad(plan)), 256, 0, stream>>>(
+    step_kernel<double><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
         reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
         partials, plan, G, pot, dt, flags);
     return cudaGetLastError();

@@ -44,10 +44,24 @@ __host__ __device__ __forceinline__ int32_t plan_owner(const PairPlan& p, int64_
     return (int32_t)(c < p.P - 1 ? c : p.P - 1);
 }
 __host__ __device__ __forceinline__ int64_t plan_npad(const PairPlan& p) { return (int64_t)p.J * p.T; }
+// Equal-mass detection: the kernel that stages the sources also writes one
+// int per block of STEP_THREADS particles, non-zero when some mass in the block differs from
+// posm[0].m.  The flags sit behind the staged records; the pair kernels OR them at start-up.
+constexpr int STEP_THREADS = 256;
+__host__ __device__ __forceinline__ int32_t plan_nflags(const PairPlan& p) {
+    return (int32_t)((plan_npad(p) + STEP_THREADS - 1) / STEP_THREADS);
+}
 __host__ __device__ __forceinline__ size_t plan_jsrc_bytes(const PairPlan& p) {
-    size_t b = (size_t)plan_npad(p) * p.rec_bytes;
+    size_t b = (size_t)plan_npad(p) * p.rec_bytes + (size_t)plan_nflags(p) * sizeof(int);
     return (b + 255) & ~(size_t)255;
 }
+__host__ __device__ __forceinline__ const int* plan_flags(const void* jsrc, const PairPlan& p) {
+    return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) + (size_t)plan_npad(p) * p.rec_bytes);
+}
+// Padding records of the staged source array: zero mass, parked so far away that the softened
+// inverse cube underflows to exactly 0 (ftz) -- they contribute 0 with or without the mass factor.
+constexpr float PAD_POS_F32 = 3.0e18f;
+constexpr double PAD_POS_F64 = 1.0e150;
 __host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p) {
     return (size_t)p.slots * 3 * p.IB * sizeof(double);
 }

@@ -14,7 +14,10 @@
 //     (half the issue slots of the scalar form, no register-pair MOVs);
 //   * two-level summation: fp32 inside one tile (<= 256 terms), promoted to fp64 between tiles
 //     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18);
-//   * the self term and the zero-mass padding records contribute exactly 0 because eps > 0.
+//   * the self term contributes exactly 0 because eps > 0; padding records are massless and parked at
+//     3e18, where the inverse cube underflows to exactly 0 (ftz), so they vanish on both paths;
+//   * equal masses (the paper's Plummer progenitors, PAPER.md:L43 step 3) are detected on the device by
+//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2.
 #include "odisseo_common.cuh"
 
 namespace odisseo {
@@ -23,55 +26,19 @@ namespace {
 
 constexpr int STAGES = 4;
 
-template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
-__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
-pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsrc, double* __restrict__ partials,
-                  const PairPlan plan, const float eps2)
+// Consumer side of the pair kernel for one CTA.  EQM = all masses equal (detected on the device by
+// the staging kernel): the per-source mass factor leaves the inner loop (11 instead of 12 packed FP32
+// ops per two interactions) and multiplies the fp64 sums once per segment.
+template <int NPAIR, int CWARPS, int JUNROLL, bool EQM>
+__device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, double* __restrict__ partials,
+                                              const PairPlan& plan, const float eps2, unsigned char* smem_raw,
+                                              uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
+                                              const int64_t u0, const int64_t u1, const uint32_t tile_bytes)
 {
     constexpr int CTHREADS = CWARPS * 32;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[STAGES];
-    __shared__ __align__(8) uint64_t empty_bar[STAGES];
-
     const int tid = threadIdx.x;
-    const int warp = tid >> 5;
     const int lane = tid & 31;
-    const int64_t c = blockIdx.x;
-    const int64_t u0 = plan_start(plan, c);
-    const int64_t u1 = plan_start(plan, c + 1);
-    if (u0 >= u1) return;
-
-    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], CWARPS);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    if (warp == CWARPS) {
-        // ---- producer warp: one elected lane streams the CTA's tile sequence --------------
-        if (lane == 0) {
-            int s = 0;
-            uint32_t ph = 0;
-            int32_t t = (int32_t)(u0 % plan.J);
-            for (int64_t u = u0; u < u1; ++u) {
-                mbar_wait(&empty_bar[s], ph ^ 1u);   // passes at once during the first round
-                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
-                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
-                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
-                            &full_bar[s]);
-                if (++t == plan.J) t = 0;
-                if (++s == STAGES) { s = 0; ph ^= 1u; }
-            }
-        }
-        return;
-    }
-
-    // ---- compute warps ----------------------------------------------------------------------
+    const double m0 = EQM ? (double)__ldg(&posm[0].w) : 1.0;
     const f32x2 e2 = pk(eps2, eps2);
     f32x2 xi[NPAIR], yi[NPAIR], zi[NPAIR];
     f32x2 ax[NPAIR], ay[NPAIR], az[NPAIR];
@@ -126,8 +93,7 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
                 unpk(r2, r2l, r2h);
                 const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
                 const f32x2 ri2 = mul2(ri, ri);
-                const f32x2 mri = mul2(B.y, ri);
-                const f32x2 w = mul2(ri2, mri);
+                const f32x2 w = mul2(ri2, EQM ? ri : mul2(B.y, ri));
                 ax[p] = fma2(w, dx, ax[p]);
                 ay[p] = fma2(w, dy, ay[p]);
                 az[p] = fma2(w, dz, az[p]);
@@ -153,14 +119,74 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
 #pragma unroll
             for (int k = 0; k < 2 * NPAIR; ++k) {
                 const int r = k * CTHREADS + tid;
-                row[r] = osum[(3 * k + 0) * CTHREADS];
-                row[plan.IB + r] = osum[(3 * k + 1) * CTHREADS];
-                row[2 * plan.IB + r] = osum[(3 * k + 2) * CTHREADS];
+                row[r] = m0 * osum[(3 * k + 0) * CTHREADS];
+                row[plan.IB + r] = m0 * osum[(3 * k + 1) * CTHREADS];
+                row[2 * plan.IB + r] = m0 * osum[(3 * k + 2) * CTHREADS];
             }
             seg_start = true;
         }
         if (++t == plan.J) { t = 0; ++b; }
     }
+}
+
+template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
+__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
+pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsrc, double* __restrict__ partials,
+                  const PairPlan plan, const float eps2)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[STAGES];
+
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5;
+    const int lane = tid & 31;
+    const int64_t c = blockIdx.x;
+    const int64_t u0 = plan_start(plan, c);
+    const int64_t u1 = plan_start(plan, c + 1);
+    if (u0 >= u1) return;
+
+    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], CWARPS);
+        }
+        mbar_fence_init();
+    }
+    // equal-mass flags written by the staging kernel (odisseo_common.cuh): one uniform decision per grid
+    int differs = 0;
+    {
+        const int* __restrict__ mflags = plan_flags(jsrc, plan);
+        const int nflags = plan_nflags(plan);
+        for (int k = tid; k < nflags; k += (CWARPS + 1) * 32) differs |= __ldg(mflags + k);
+    }
+    const bool eqm = __syncthreads_or(differs) == 0;        // also publishes the mbarrier inits
+
+    if (warp == CWARPS) {
+        // ---- producer warp: one elected lane streams the CTA's tile sequence --------------
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            int32_t t = (int32_t)(u0 % plan.J);
+            for (int64_t u = u0; u < u1; ++u) {
+                mbar_wait(&empty_bar[s], ph ^ 1u);   // passes at once during the first round
+                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
+                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
+                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
+                            &full_bar[s]);
+                if (++t == plan.J) t = 0;
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+        return;
+    }
+
+    if (eqm)
+        consume_tiles<NPAIR, CWARPS, JUNROLL, true>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+    else
+        consume_tiles<NPAIR, CWARPS, JUNROLL, false>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
 }
 
 template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>

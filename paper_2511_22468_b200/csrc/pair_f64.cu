@@ -18,53 +18,18 @@ namespace {
 
 constexpr int STAGES = 4;
 
-template <int IPT, int CWARPS, int MINB, int JUNROLL>
-__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
-pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ jsrc, double* __restrict__ partials,
-                const PairPlan plan, const double eps2)
+// Consumer side for one CTA.  EQM = all masses equal (flags from the staging kernel): the mass
+// factor leaves the inner loop (15 instead of 16 FP64 ops) and multiplies the sums once per segment.
+template <int IPT, int CWARPS, int JUNROLL, bool EQM>
+__device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, double* __restrict__ partials,
+                                              const PairPlan& plan, const double eps2, unsigned char* smem_raw,
+                                              uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
+                                              const int64_t u0, const int64_t u1, const uint32_t tile_bytes)
 {
     constexpr int CTHREADS = CWARPS * 32;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[STAGES];
-    __shared__ __align__(8) uint64_t empty_bar[STAGES];
-
     const int tid = threadIdx.x;
-    const int warp = tid >> 5;
     const int lane = tid & 31;
-    const int64_t c = blockIdx.x;
-    const int64_t u0 = plan_start(plan, c);
-    const int64_t u1 = plan_start(plan, c + 1);
-    if (u0 >= u1) return;
-
-    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], CWARPS);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    if (warp == CWARPS) {
-        if (lane == 0) {
-            int s = 0;
-            uint32_t ph = 0;
-            int32_t t = (int32_t)(u0 % plan.J);
-            for (int64_t u = u0; u < u1; ++u) {
-                mbar_wait(&empty_bar[s], ph ^ 1u);
-                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
-                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
-                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
-                            &full_bar[s]);
-                if (++t == plan.J) t = 0;
-                if (++s == STAGES) { s = 0; ph ^= 1u; }
-            }
-        }
-        return;
-    }
-
+    const double m0 = EQM ? posm[0].w : 1.0;
     double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
     int32_t b = (int32_t)(u0 / plan.J);
     int32_t t = (int32_t)(u0 - (int64_t)b * plan.J);
@@ -102,7 +67,7 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
                 const double t = y0 * y0;
                 const double e = fma(-r2, t, 1.0);
                 const double c = fma(e, fma(1.875, e, 1.5), 1.0);
-                const double w = ((t * y0) * q.w) * c;
+                const double w = EQM ? (t * y0) * c : ((t * y0) * q.w) * c;
                 ax[k] = fma(w, dx, ax[k]);
                 ay[k] = fma(w, dy, ay[k]);
                 az[k] = fma(w, dz, az[k]);
@@ -118,14 +83,72 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
 #pragma unroll
             for (int k = 0; k < IPT; ++k) {
                 const int r = k * CTHREADS + tid;
-                row[r] = ax[k];
-                row[plan.IB + r] = ay[k];
-                row[2 * plan.IB + r] = az[k];
+                row[r] = m0 * ax[k];
+                row[plan.IB + r] = m0 * ay[k];
+                row[2 * plan.IB + r] = m0 * az[k];
             }
             seg_start = true;
         }
         if (++t == plan.J) { t = 0; ++b; }
     }
+}
+
+template <int IPT, int CWARPS, int MINB, int JUNROLL>
+__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
+pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ jsrc, double* __restrict__ partials,
+                const PairPlan plan, const double eps2)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[STAGES];
+
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5;
+    const int lane = tid & 31;
+    const int64_t c = blockIdx.x;
+    const int64_t u0 = plan_start(plan, c);
+    const int64_t u1 = plan_start(plan, c + 1);
+    if (u0 >= u1) return;
+
+    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], CWARPS);
+        }
+        mbar_fence_init();
+    }
+    int differs = 0;
+    {
+        const int* __restrict__ mflags = plan_flags(jsrc, plan);
+        const int nflags = plan_nflags(plan);
+        for (int k = tid; k < nflags; k += (CWARPS + 1) * 32) differs |= __ldg(mflags + k);
+    }
+    const bool eqm = __syncthreads_or(differs) == 0;        // also publishes the mbarrier inits
+
+    if (warp == CWARPS) {
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            int32_t t = (int32_t)(u0 % plan.J);
+            for (int64_t u = u0; u < u1; ++u) {
+                mbar_wait(&empty_bar[s], ph ^ 1u);
+                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
+                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
+                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
+                            &full_bar[s]);
+                if (++t == plan.J) t = 0;
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+        return;
+    }
+
+    if (eqm)
+        consume_tiles<IPT, CWARPS, JUNROLL, true>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+    else
+        consume_tiles<IPT, CWARPS, JUNROLL, false>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
 }
 
 template <int IPT, int CWARPS, int MINB, int JUNROLL>

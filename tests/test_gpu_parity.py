@@ -71,6 +71,50 @@ def test_pair_f64_ragged_sizes_unequal_masses(n):
     assert pair_ratio(acc, posm64, 1.0, 0.05) <= TOL_F64
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n", [1, 2, 3, 127, 129, 1000, 1025, 4097, 5000])
+def test_pair_equal_masses_ragged_sizes_take_the_equal_mass_path(n, dtype):
+    """All masses equal: the kernels drop the per-source mass factor from the inner loop (the staging
+    kernel's flags decide on the device); ragged tails are padded with far-away zero-mass records."""
+    posm64, _ = W.random_cloud(n, seed=300 + n, unequal_mass=False)
+    posm64[:, 3] = 0.37
+    if dtype == np.float32:
+        p, p64, G, eps = f32_inputs(posm64, 1.0, 0.05)
+        tol = TOL_F32
+    else:
+        p, p64, G, eps, tol = posm64, posm64, 1.0, 0.05, TOL_F64
+    acc = gpu_pair(p, G, eps, dtype)
+    assert np.all(np.isfinite(acc))
+    assert pair_ratio(acc, p64, G, eps) <= tol
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n,odd", [(1025, 1024), (5000, 0), (5000, 4999), (9001, 4500)])
+def test_pair_one_different_mass_anywhere_selects_the_general_path(n, odd, dtype):
+    """A single particle whose mass differs (first, middle or last record, incl. the ragged tail block) must
+    switch every CTA to the general kernel; using the equal-mass path would miss a factor 5."""
+    posm64, _ = W.random_cloud(n, seed=400 + n, unequal_mass=False)
+    posm64[odd, 3] = 5.0
+    if dtype == np.float32:
+        p, p64, G, eps = f32_inputs(posm64, 1.0, 0.05)
+        tol = TOL_F32
+    else:
+        p, p64, G, eps, tol = posm64, posm64, 1.0, 0.05, TOL_F64
+    acc = gpu_pair(p, G, eps, dtype)
+    assert pair_ratio(acc, p64, G, eps) <= tol
+    # and the decision is re-taken on every call with the same workspace
+    posm = dev(p, dtype)
+    out = torch.empty_like(posm)
+    ws = B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64))
+    B.pair_accel(posm, out, G, eps, ws)
+    posm[odd, 3] = 1.0
+    B.pair_accel(posm, out, G, eps, ws)
+    torch.cuda.synchronize()
+    p64b = p64.copy()
+    p64b[odd, 3] = 1.0
+    assert pair_ratio(out.cpu().numpy(), p64b, G, eps) <= tol
+
+
 @pytest.mark.parametrize("ci", [0, 1])
 def test_pair_f32_configs_full(ci):
     cfg = W.CONFIGS[ci]
