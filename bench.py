@@ -25,7 +25,7 @@ FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star con
 SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144 (ncu --set full)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 13152768    # profiles/r01_pair_f32_ncu_full.txt: 13.15 MB read + 0 written
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 12645888    # profiles/r01_pair_f32_ncu_full.txt: 12.64 MB read + 4 KB written
 
 
 def _peaks():
@@ -200,6 +200,41 @@ def _steps_per_s(B, W, torch, ci: int, nsteps: int, dtype=np.float32):
             "steps_per_s": nsteps / (ms * 1e-3), "G_int_per_s": nsteps * float(cfg.n) ** 2 / (ms * 1e-3) / 1e9}
 
 
+def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: int = 10):
+    """HBM roofline of the O(N) integrator kernel (reduce-free form: reads posm, vel, acc; writes posm, vel and
+    the staged sources = 112 B per particle in fp32) through odisseo_kick_drift_f32 at N = 2^24: 1.9 GB per
+    launch, far larger than the 126 MB L2."""
+    cfg = W.CONFIGS[3]
+    g = torch.Generator(device="cuda").manual_seed(1234)
+    posm = torch.randn(n, 4, device="cuda", generator=g) * 0.02
+    posm[:, 0] -= 10.0
+    posm[:, 1] -= 4.0
+    posm[:, 2] += 6.0
+    posm[:, 3] = cfg.M / n
+    vel = torch.randn(n, 4, device="cuda", generator=g) * 0.002
+    acc = torch.randn(n, 4, device="cuda", generator=g) * 1e-6
+    ws = B.alloc_workspace(B.workspace_bytes(n))
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    G, dt = float(np.float32(cfg.G)), float(np.float32(cfg.dt))
+    for _ in range(3):
+        B.kick_drift(posm, vel, acc, G, dt, pot, 3, ws)
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        B.kick_drift(posm, vel, acc, G, dt, pot, 3, ws)
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    ms = float(np.mean(ts))
+    nbytes = 112.0 * n
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"kernel": "step_kernel<float> (kick + drift + NFW/MN + staging)", "n": n, "bound": "hbm",
+            "bytes_per_particle": 112, "launch_ms": ms, "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": gbs / peaks["hbm_gbs"], "peak_kind": peak_kind + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)"}
+
+
 def run_ours(args, rank: int, world: int, dist):
     import torch
     from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
@@ -316,6 +351,8 @@ def run_ours(args, rank: int, world: int, dist):
         extras.append(_steps_per_s(B, W, torch, 3, 3, np.float64))
         extras.append(_steps_per_s(B, W, torch, 4, 2))
         line["other_configs"] = extras
+        del posm_g, acc_g
+        line["integrator_roofline"] = _integrator_roofline(B, W, torch, peaks, peak_kind)
     print(json.dumps(line), flush=True)
 
 
@@ -327,9 +364,18 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
+    ap.add_argument("--integrator-only", action="store_true",
+                    help="run only the O(N) integrator kernel's HBM roofline leg (N = 2^24) and print it")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args, int(os.environ.get("RANK", "0")))
+        return 0
+    if args.integrator_only:
+        import torch
+        from paper_2511_22468_b200 import binding as B
+        from paper_2511_22468_b200 import workloads as W
+        peaks, peak_kind = _peaks()
+        print(json.dumps({"integrator_roofline": _integrator_roofline(B, W, torch, peaks, peak_kind)}), flush=True)
         return 0
     rank, world, dist = _dist_setup(args.gpus)
     try:

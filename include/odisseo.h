@@ -123,6 +123,22 @@ odisseo_status odisseo_leapfrog_kdk_f64(double *d_posm, double *d_vel, double *d
                                         const odisseo_potential *pot,
                                         void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* The O(N) integrator kernel on its own (SURVEY.md 8a rows a2 + a3): given the
+ * pair-only acceleration in d_acc (input, unchanged), with a = d_acc + a_NFW(x) + a_MN(x):
+ *   mode & 1: closing half kick          v += a dt/2
+ *   mode & 2: opening half kick + drift  v += a dt/2 ; x += v dt   (a evaluated BEFORE the drift),
+ *             and the moved sources are staged into the workspace for the next pair evaluation.
+ * mode 3 = the kernel a full leapfrog step launches between two pair evaluations.  This is the launch
+ * bench.py times for the integrator's HBM roofline; it is also the building block for callers that
+ * obtain pair accelerations elsewhere.  Workspace as for odisseo_pair_accel_*.  mode outside 1..3 ->
+ * ERR_ARG. */
+odisseo_status odisseo_kick_drift_f32(float *d_posm, float *d_vel, const float *d_acc, int64_t n, float G,
+                                      float dt, const odisseo_potential *pot, int mode,
+                                      void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_kick_drift_f64(double *d_posm, double *d_vel, const double *d_acc, int64_t n, double G,
+                                      double dt, const odisseo_potential *pot, int mode,
+                                      void *d_workspace, size_t workspace_bytes, void *stream);
+
 /* Host-buffer face of the leapfrog (end-to-end path): copies h_posm, h_vel [n][4] (and, when
  * acc_valid != 0, h_acc, which must then be non-NULL and hold a_pair(h_posm) as left by a
  * previous call) to the device, runs nsteps KDK steps, copies posm, vel and (if h_acc != NULL)

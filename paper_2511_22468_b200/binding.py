@@ -25,7 +25,7 @@ EXPORTS = [
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
     "odisseo_describe_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
-    "odisseo_profile_end",
+    "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
 ]
 
 
@@ -79,6 +79,7 @@ def lib():
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
@@ -203,6 +204,19 @@ def leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: fl
     fn = getattr(lib(), "odisseo_leapfrog_kdk_" + sfx)
     _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr(), int(bool(acc_valid)), n, G, eps, dt, int(nsteps),
               _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)), "leapfrog_kdk_" + sfx)
+
+
+def kick_drift(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, dt: float,
+               pot: Optional[Potential], mode: int, workspace: torch.Tensor, stream=None):
+    """The O(N) integrator kernel alone (odisseo_kick_drift_f32/_f64): mode 1 = closing half kick,
+    2 = opening half kick + drift (+ staging of the moved sources), 3 = both."""
+    n = _rec(posm, "posm")
+    _rec(vel, "vel", n)
+    _rec(acc, "acc", n)
+    sfx = _suffix(posm)
+    fn = getattr(lib(), "odisseo_kick_drift_" + sfx)
+    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr(), n, G, dt, _pot(pot), int(mode), workspace.data_ptr(),
+              workspace.numel(), _stream(stream)), "kick_drift_" + sfx)
 
 
 def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch.Tensor], G: float, eps: float,

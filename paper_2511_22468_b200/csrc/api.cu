@@ -364,6 +364,36 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
 }
 
 template <typename T>
+odisseo_status kick_drift_impl(T* posm, T* vel, const T* acc, int64_t n, T G, T dt, const odisseo_potential* pot,
+                               int mode, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0 || mode < 1 || mode > 3) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!posm || !vel || !acc) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(vel, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+    if (overlap(posm, n * rec, acc, n * rec) || overlap(posm, n * rec, vel, n * rec) ||
+        overlap(vel, n * rec, acc, n * rec))
+        return ODISSEO_ERR_ARG;
+    if (!isfinite((double)G) || !isfinite((double)dt)) return ODISSEO_ERR_ARG;
+    PotParams<T> pp;
+    odisseo_status st = make_pot<T>(G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    Carve cv;
+    st = carve(plan, ws, ws_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    const int flags = ((mode & 1) ? STEP_CLOSE : 0) | ((mode & 2) ? STEP_OPEN : 0);
+    cudaError_t e = launch_step(plan, posm, vel, const_cast<T*>(acc), cv.jsrc, cv.partials, G, pp, dt, flags,
+                                static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+template <typename T>
 odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
                                   const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
 {
@@ -556,6 +586,16 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
                                         double G, double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
                                         void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_kick_drift_f32(float* d_posm, float* d_vel, const float* d_acc, int64_t n, float G, float dt,
+                                      const odisseo_potential* pot, int mode, void* d_workspace,
+                                      size_t workspace_bytes, void* stream)
+{ return kick_drift_impl<float>(d_posm, d_vel, d_acc, n, G, dt, pot, mode, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_kick_drift_f64(double* d_posm, double* d_vel, const double* d_acc, int64_t n, double G, double dt,
+                                      const odisseo_potential* pot, int mode, void* d_workspace,
+                                      size_t workspace_bytes, void* stream)
+{ return kick_drift_impl<double>(d_posm, d_vel, d_acc, n, G, dt, pot, mode, d_workspace, workspace_bytes, stream); }
 
 odisseo_status odisseo_leapfrog_kdk_host_f32(float* h_posm, float* h_vel, float* h_acc, int acc_valid, int64_t n, float G, float eps,
                                              float dt, int64_t nsteps, const odisseo_potential* pot,

@@ -88,8 +88,11 @@ __device__ __forceinline__ void stage_record(void* jsrc, int64_t i, double x, do
 __device__ __forceinline__ float pad_pos(float) { return PAD_POS_F32; }
 __device__ __forceinline__ double pad_pos(double) { return PAD_POS_F64; }
 
-template <typename T>
-__global__ void __launch_bounds__(STEP_THREADS)
+// REDUCE = the launch starts from the pair kernel's partial rows (flags & STEP_FROM_PARTIALS); a
+// compile-time switch so that the plain kick/drift instantiation does not carry the reduce batch in
+// registers (occupancy is what hides HBM latency here).
+template <typename T, bool REDUCE>
+__global__ void __launch_bounds__(STEP_THREADS, REDUCE ? 2 : (sizeof(T) == 4 ? 5 : 3))
 step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
             typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
             const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags)
@@ -98,13 +101,19 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
     int mass_differs = 0;
+    int* const block_flag = const_cast<int*>(plan_flags(jsrc, plan)) + blockIdx.x;
+    if (staging) {                                   // uniform branch: flags is a kernel argument
+        if (threadIdx.x == 0) *block_flag = 0;
+        __syncthreads();                             // before any load is in flight: costs nothing
+    }
     if (i < plan.n) {
+        const T mass0 = reinterpret_cast<const T*>(posm)[3];            // masses are never modified
         V4 p = posm[i];
         if (flags & STEP_PACK_ONLY) {
             stage_record(jsrc, i, p.x, p.y, p.z, p.w);
         } else {
             T apx, apy, apz;
-            if (flags & STEP_FROM_PARTIALS) {
+            if (REDUCE) {
                 const int32_t b = (int32_t)(i / plan.IB);
                 const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
                 const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
@@ -155,14 +164,15 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
                 vel[i] = v;
             }
         }
-        if (staging) mass_differs = !(p.w == *(const volatile T*)&posm[0].w);   // masses never change; NaN counts as different
+        if (staging) mass_differs = !(p.w == mass0);                // NaN counts as different
     } else if (staging && i < plan_npad(plan)) {
         const T far = pad_pos((T)0);
         stage_record(jsrc, i, far, far, far, (T)0);
     }
-    if (staging) {                                                     // uniform branch: flags is a kernel argument
-        const int any = __syncthreads_or(mass_differs);
-        if (threadIdx.x == 0) const_cast<int*>(plan_flags(jsrc, plan))[blockIdx.x] = any;
+    if (staging) {
+        // same-value plain stores after the block's own zeroing: no atomics, no closing barrier
+        const unsigned any = __ballot_sync(0xffffffffu, mass_differs);
+        if (any != 0u && (threadIdx.x & 31) == 0) *block_flag = 1;
     }
 }
 
@@ -214,9 +224,14 @@ cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
                             cudaStream_t stream)
 {
-    step_kernel<float><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-        reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
-        partials, plan, G, pot, dt, flags);
+    if (flags & STEP_FROM_PARTIALS)
+        step_kernel<float, true><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
+            reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
+            partials, plan, G, pot, dt, flags);
+    else
+        step_kernel<float, false><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
+            reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
+            partials, plan, G, pot, dt, flags);
     return cudaGetLastError();
 }
 
@@ -224,9 +239,14 @@ cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, dou
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
                             cudaStream_t stream)
 {
-    step_kernel<double><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-        reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
-        partials, plan, G, pot, dt, flags);
+    if (flags & STEP_FROM_PARTIALS)
+        step_kernel<double, true><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
+            reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
+            partials, plan, G, pot, dt, flags);
+    else
+        step_kernel<double, false><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
+            reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
+            partials, plan, G, pot, dt, flags);
     return cudaGetLastError();
 }
 

@@ -450,3 +450,28 @@ def test_full_size_step_resynchronised_parity_and_one_step_shadowing(ci, dtype):
     rx, rv, ra = (1e-6, 1e-6, 1.5e-5) if f32 else (1e-12, 1e-12, 1e-11)
     assert np.all(dx <= rx * np.linalg.norm(x_new, axis=1))
     assert np.all(dv <= rv * np.linalg.norm(v_new, axis=1) + ra * abs(dt) * (np.maximum(S_k, S_1) + aext))
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_kick_drift_composes_to_the_leapfrog_bitwise(dtype):
+    """odisseo_kick_drift (the integrator kernel alone) + odisseo_pair_accel reproduce
+    odisseo_leapfrog_kdk bit for bit: a0 = pair(x0); [open]; a1 = pair(x1); [close+open]; a2; [close]."""
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.make_state(cfg, n=3001)
+    p0, v0 = posm64.astype(dtype), vel64.astype(dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    ref = gpu_leapfrog(p0, v0, cfg.G, cfg.eps, cfg.dt, 2, pot, dtype)
+    posm, vel = dev(p0, dtype), dev(W.vel4(v0, dtype), dtype)
+    acc = torch.empty_like(posm)
+    ws = B.alloc_workspace(B.workspace_bytes(3001, dtype == np.float64))
+    B.pair_accel(posm, acc, cfg.G, cfg.eps, ws)
+    B.kick_drift(posm, vel, acc, cfg.G, cfg.dt, pot, 2, ws)
+    B.pair_accel(posm, acc, cfg.G, cfg.eps, ws)
+    B.kick_drift(posm, vel, acc, cfg.G, cfg.dt, pot, 3, ws)
+    B.pair_accel(posm, acc, cfg.G, cfg.eps, ws)
+    B.kick_drift(posm, vel, acc, cfg.G, cfg.dt, pot, 1, ws)
+    torch.cuda.synchronize()
+    for got, want in zip((posm, vel, acc), ref):
+        assert got.cpu().numpy().tobytes() == want.tobytes()
+    with pytest.raises(B.OdisseoError, match="ERR_ARG"):
+        B.kick_drift(posm, vel, acc, cfg.G, cfg.dt, pot, 0, ws)
