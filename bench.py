@@ -235,6 +235,33 @@ def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: 
             "frac": gbs / peaks["hbm_gbs"], "peak_kind": peak_kind + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)"}
 
 
+def _ensemble_rate(B, W, torch, n: int = 1000, nsim: int = 2960, nsteps: int = 50):
+    """Batched small-N ensembles (the paper's inference workload shape: N = 1,000 particles per
+    simulation): nsim simulations x nsteps KDK steps in ONE odisseo_ensemble_leapfrog_kdk_f32 launch."""
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg, n=n)
+    posm = torch.from_numpy(np.repeat(W.to_f32(p64)[None], nsim, axis=0)).cuda()
+    vel = torch.from_numpy(np.repeat(W.vel4(W.to_f32(v64), np.float32)[None], nsim, axis=0)).cuda()
+    ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
+    rng = np.random.Generator(np.random.PCG64(5))
+    prm = [(cfg.G, cfg.eps, cfg.dt * rng.uniform(0.5, 1.5),
+            B.Potential.make(nfw=(cfg.nfw[0] * rng.uniform(0.5, 2.0), cfg.nfw[1]),
+                             mn=(cfg.mn[0] * rng.uniform(0.5, 2.0), cfg.mn[1], cfg.mn[2]))) for _ in range(nsim)]
+    B.ensemble_leapfrog_kdk(posm, vel, prm, 2, ws)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    B.ensemble_leapfrog_kdk(posm, vel, prm, nsteps, ws)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    ints = nsim * (nsteps + 1) * float(n) ** 2
+    tf = ints * FLOPS_PER_INTERACTION / (ms * 1e-3) / 1e12
+    return {"workload": "ensemble of %d simulations, N = %d each, per-simulation dt / M_NFW / M_MN" % (nsim, n),
+            "steps": nsteps, "ms": ms, "sim_steps_per_s": nsim * nsteps / (ms * 1e-3),
+            "G_int_per_s": ints / (ms * 1e-3) / 1e9, "frac_fp32_peak": tf / FP32_PEAK_TFLOPS, "gpu_launches": 1}
+
+
 def run_ours(args, rank: int, world: int, dist):
     import torch
     from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
@@ -353,6 +380,7 @@ def run_ours(args, rank: int, world: int, dist):
         line["other_configs"] = extras
         del posm_g, acc_g
         line["integrator_roofline"] = _integrator_roofline(B, W, torch, peaks, peak_kind)
+        line["ensemble"] = _ensemble_rate(B, W, torch)
     print(json.dumps(line), flush=True)
 
 

@@ -155,6 +155,25 @@ odisseo_status odisseo_leapfrog_kdk_host_f64(double *h_posm, double *h_vel, doub
                                              const odisseo_potential *pot,
                                              void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* Batched small-N ensembles (the paper's inference workload: 10^4 grid points and
+ * bootstrap resamples, each an N = 1,000, 1,000-step simulation with its own potential masses,
+ * progenitor mass and integration time, Fig. 2, L47, L53).  nsim independent simulations
+ * of n particles each (1 <= n <= 2,048) are advanced nsteps KDK steps by one kernel launch, one CTA per
+ * simulation, state resident on the SM for the whole time loop.
+ *   d_posm, d_vel  [nsim][n][4] float, in/out (device, 16-byte aligned); masses preserved, vel pad lane 0.
+ *   h_params       HOST array of nparams records; nparams == 1: all simulations share it, else
+ *                  nparams must equal nsim.  eps > 0 per record; pot terms with mass <= 0 are disabled.
+ *   d_workspace    odisseo_ensemble_workspace_bytes(nsim) bytes, 256-byte aligned (device copy of the
+ *                  parameter records; h_params may be reused as soon as the call returns).
+ * Each simulation computes exactly what odisseo_leapfrog_kdk_f32 computes (acc_valid = 0), with fp32
+ * two-level summation in 512-source tiles; results agree with it to rounding, not bit for bit. */
+typedef struct { double G, eps, dt; odisseo_potential pot; } odisseo_sim_params;
+size_t odisseo_ensemble_workspace_bytes(int64_t nsim);
+odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float *d_posm, float *d_vel, int64_t n, int64_t nsim,
+                                                 const odisseo_sim_params *h_params, int64_t nparams,
+                                                 int64_t nsteps, void *d_workspace, size_t workspace_bytes,
+                                                 void *stream);
+
 /* Instrumentation (bench.py's gpu_launches and roofline legs).
  *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA
  *     graph replay counts its kernel nodes).  Host counter, no GPU work.

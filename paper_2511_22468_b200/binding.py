@@ -26,6 +26,7 @@ EXPORTS = [
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
     "odisseo_describe_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
     "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
+    "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
 ]
 
 
@@ -59,6 +60,11 @@ class Potential(ctypes.Structure):
         return p
 
 
+class SimParams(ctypes.Structure):
+    """odisseo_sim_params: per-simulation G, eps, dt and potential of the ensemble call."""
+    _fields_ = [("G", ctypes.c_double), ("eps", ctypes.c_double), ("dt", ctypes.c_double), ("pot", Potential)]
+
+
 def lib():
     """Load the C-ABI library; fail loudly when it has not been built."""
     global _lib
@@ -85,6 +91,9 @@ def lib():
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
         L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        L.odisseo_ensemble_workspace_bytes.restype = sz
+        L.odisseo_ensemble_workspace_bytes.argtypes = [i64]
+        L.odisseo_ensemble_leapfrog_kdk_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp]
         L.odisseo_launch_count.restype = i64
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
@@ -235,6 +244,32 @@ def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch
               n, G, eps, dt,
               int(nsteps), _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "leapfrog_kdk_host_" + sfx)
+
+
+def ensemble_workspace_bytes(nsim: int) -> int:
+    return int(lib().odisseo_ensemble_workspace_bytes(int(nsim)))
+
+
+def ensemble_leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, params, nsteps: int, workspace: torch.Tensor,
+                          stream=None):
+    """nsim independent small-N simulations in one launch (odisseo_ensemble_leapfrog_kdk_f32).
+
+    posm, vel: contiguous float32 CUDA tensors [nsim, n, 4]; params: a list of (G, eps, dt, Potential-or-None)
+    tuples, one per simulation or a single one shared by all."""
+    if posm.dim() != 3 or posm.shape[2] != 4 or posm.shape != vel.shape or not posm.is_contiguous() \
+            or not vel.is_contiguous() or posm.dtype != torch.float32 or vel.dtype != torch.float32:
+        raise ValueError("posm and vel must be contiguous float32 [nsim, n, 4] tensors")
+    if not (posm.is_cuda and vel.is_cuda):
+        raise ValueError("posm and vel must be CUDA tensors (no CPU fallback)")
+    nsim, n = int(posm.shape[0]), int(posm.shape[1])
+    arr = (SimParams * len(params))()
+    for k, (G, eps, dt, pot) in enumerate(params):
+        arr[k].G, arr[k].eps, arr[k].dt = float(G), float(eps), float(dt)
+        arr[k].pot = pot if pot is not None else Potential.make()
+    _check(lib().odisseo_ensemble_leapfrog_kdk_f32(posm.data_ptr(), vel.data_ptr(), n, nsim,
+                                                   ctypes.cast(arr, ctypes.c_void_p), len(params), int(nsteps),
+                                                   workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "ensemble_leapfrog_kdk_f32")
 
 
 def launch_count() -> int:

@@ -587,6 +587,51 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
                                         void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
 
+size_t odisseo_ensemble_workspace_bytes(int64_t nsim)
+{
+    if (nsim <= 0) return 0;
+    return (((size_t)nsim * sizeof(EnsembleParams)) + 255) & ~(size_t)255;
+}
+
+odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float* d_posm, float* d_vel, int64_t n, int64_t nsim,
+                                                 const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
+                                                 void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
+    if (n == 0 || nsim == 0) return ODISSEO_OK;
+    if (!d_posm || !d_vel || !h_params || !d_workspace) return ODISSEO_ERR_NULL;
+    if (misaligned(d_posm, 16) || misaligned(d_vel, 16) || misaligned(d_workspace, 256)) return ODISSEO_ERR_ALIGN;
+    const size_t bytes = (size_t)nsim * n * 16;
+    if (overlap(d_posm, bytes, d_vel, bytes)) return ODISSEO_ERR_ARG;
+    if (nparams != 1 && nparams != nsim) return ODISSEO_ERR_ARG;
+    if (workspace_bytes < (size_t)nparams * sizeof(EnsembleParams)) return ODISSEO_ERR_WORKSPACE;
+    std::vector<EnsembleParams> dev_params((size_t)nparams);
+    for (int64_t k = 0; k < nparams; ++k) {
+        const odisseo_sim_params& hp = h_params[k];
+        const float G = (float)hp.G, eps = (float)hp.eps, dt = (float)hp.dt;
+        odisseo_status st = check_pair_scalars<float>(G, eps);
+        if (st != ODISSEO_OK) return st;
+        if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
+        EnsembleParams& d = dev_params[(size_t)k];
+        st = make_pot<float>(G, &hp.pot, d.pot);
+        if (st != ODISSEO_OK) return st;
+        d.G = G; d.eps2 = eps * eps; d.dt = dt;
+    }
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    // pageable source: the runtime stages it before returning, so dev_params may die with this frame
+    cudaError_t e = cudaMemcpyAsync(d_workspace, dev_params.data(), (size_t)nparams * sizeof(EnsembleParams),
+                                    cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    e = launch_ensemble_f32(d_posm, d_vel, static_cast<const EnsembleParams*>(d_workspace), nparams == 1 ? 1 : 0,
+                            (int)n, nsim, nsteps, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
 odisseo_status odisseo_kick_drift_f32(float* d_posm, float* d_vel, const float* d_acc, int64_t n, float G, float dt,
                                       const odisseo_potential* pot, int mode, void* d_workspace,
                                       size_t workspace_bytes, void* stream)

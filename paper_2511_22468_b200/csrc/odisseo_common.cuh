@@ -74,6 +74,13 @@ template <typename T> struct PotParams {
     T GMd, a, b2;    // MN:  G*M, a, b^2    (GMd == 0 disables)
 };
 
+// Per-simulation parameters of the ensemble kernel (ensemble.cu), device layout, 32 bytes.
+struct EnsembleParams {
+    float G, eps2, dt;
+    PotParams<float> pot;
+};
+constexpr int ENSEMBLE_MAX_N = 2048;
+
 // Step-kernel flags.
 enum : int {
     STEP_FROM_PARTIALS = 1,   // a_pair = G * fixed-order sum of partial rows (else read acc)
@@ -183,6 +190,8 @@ cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const Pot
 cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
                                 int64_t n, cudaStream_t stream);
 cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
+cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
+                                int64_t nsim, int64_t nsteps, cudaStream_t stream);
 cudaError_t configure_pair_f32();
 cudaError_t configure_pair_f64();
 

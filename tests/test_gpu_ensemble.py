@@ -1,0 +1,127 @@
+"""GPU parity of the batched small-N ensemble call against the fp64 CPU oracle:
+every simulation of a batch must match oracle.leapfrog_kdk run on its own inputs and parameters."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2511_22468_b200 import binding as B
+from paper_2511_22468_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _f32(x):
+    return float(np.float32(x))
+
+
+def _make_batch(n, sims):
+    """sims: list of dicts(seed, M, dt_scale, nfw_scale, mn_scale, unequal, isolated)."""
+    cfg = W.CONFIGS[1]
+    posm = np.zeros((len(sims), n, 4), dtype=np.float32)
+    vel = np.zeros((len(sims), n, 4), dtype=np.float32)
+    bparams, oparams = [], []
+    for k, s in enumerate(sims):
+        if s.get("isolated"):
+            c0 = W.CONFIGS[0]
+            p64, v64 = W.plummer_sphere(n, c0.G, c0.M, c0.a, s["seed"])
+            G, eps, dt, bpot, opot = c0.G, c0.eps, c0.dt, None, None
+        else:
+            p64, v64 = W.plummer_sphere(n, cfg.G, s["M"], cfg.a, s["seed"])
+            p64[:, :3] += np.asarray(cfg.centre)
+            v64 += np.asarray(cfg.velocity)
+            nfw = (cfg.nfw[0] * s["nfw_scale"], cfg.nfw[1])
+            mn = (cfg.mn[0] * s["mn_scale"], cfg.mn[1], cfg.mn[2])
+            G, eps, dt = cfg.G, cfg.eps, cfg.dt * s["dt_scale"]
+            bpot, opot = B.Potential.make(nfw=nfw, mn=mn), O.Potential.make(nfw=nfw, mn=mn)
+        if s.get("unequal"):
+            p64[:, 3] *= np.random.Generator(np.random.PCG64(s["seed"])).uniform(0.5, 1.5, n)
+        posm[k] = W.to_f32(p64)
+        vel[k, :, :3] = W.to_f32(v64)
+        bparams.append((G, eps, dt, bpot))
+        oparams.append((_f32(G), _f32(eps), _f32(dt), opot))
+    return posm, vel, bparams, oparams
+
+
+def _check_against_oracle(posm0, vel0, posm1, vel1, oparams, nsteps, a_scale):
+    for k, (G, eps, dt, opot) in enumerate(oparams):
+        pr, vr, _ = O.leapfrog_kdk(posm0[k].astype(np.float64), vel0[k, :, :3].astype(np.float64), G, eps, dt, nsteps, opot)
+        _, S = O.pair_accel(pr, G, eps)
+        aext = np.linalg.norm(O.ext_accel(pr, G, opot), axis=1) if opot is not None else 0.0
+        dx = np.linalg.norm(posm1[k, :, :3] - pr[:, :3], axis=1)
+        dv = np.linalg.norm(vel1[k, :, :3] - vr, axis=1)
+        # 10-step short-horizon tolerances
+        assert np.all(dx <= 1e-5 * np.maximum(np.linalg.norm(pr[:, :3], axis=1), a_scale[k])), "sim %d dx" % k
+        assert np.all(dv <= 1e-5 * np.linalg.norm(vr, axis=1) + 1.5e-4 * abs(dt) * (S + aext)), "sim %d dv" % k
+        assert np.array_equal(posm1[k, :, 3], posm0[k, :, 3])
+        assert np.all(vel1[k, :, 3] == 0)
+
+
+def _run(posm, vel, bparams, nsteps):
+    dp, dv = torch.from_numpy(posm.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    ws = B.alloc_workspace(B.ensemble_workspace_bytes(posm.shape[0]))
+    B.ensemble_leapfrog_kdk(dp, dv, bparams, nsteps, ws)
+    torch.cuda.synchronize()
+    return dp.cpu().numpy(), dv.cpu().numpy()
+
+
+def test_ensemble_per_simulation_parameters_match_the_oracle():
+    n = 1000                                                    # the paper's N; ragged vs 1,024
+    sims = [dict(seed=11, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0),
+            dict(seed=12, M=2.0e4, dt_scale=0.5, nfw_scale=0.7, mn_scale=1.3),
+            dict(seed=13, M=0.5e4, dt_scale=-1.0, nfw_scale=1.2, mn_scale=0.0),       # backward, no disk
+            dict(seed=14, M=1.0e4, dt_scale=1.0, nfw_scale=0.0, mn_scale=1.0),        # no halo
+            dict(seed=15, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0, unequal=True),
+            dict(seed=16, isolated=True)]
+    posm, vel, bparams, oparams = _make_batch(n, sims)
+    p1, v1 = _run(posm, vel, bparams, 10)
+    a_scale = [W.CONFIGS[1].a] * 5 + [W.CONFIGS[0].a]
+    _check_against_oracle(posm, vel, p1, v1, oparams, 10, a_scale)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 255, 257, 512, 513, 1024, 1025, 1536, 2000, 2048])
+def test_ensemble_sizes_and_shared_parameters(n):
+    sims = [dict(seed=100 + n + k, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0, unequal=(k == 1)) for k in range(3)]
+    posm, vel, bparams, oparams = _make_batch(n, sims)
+    p1, v1 = _run(posm, vel, bparams[:1], 4)                    # one shared parameter record
+    _check_against_oracle(posm, vel, p1, v1, oparams, 4, [W.CONFIGS[1].a] * 3)
+
+
+def test_ensemble_agrees_with_the_single_simulation_path_and_is_reproducible():
+    n = 1000
+    sims = [dict(seed=21 + k, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0) for k in range(4)]
+    posm, vel, bparams, _ = _make_batch(n, sims)
+    p1, v1 = _run(posm, vel, bparams, 20)
+    p2, v2 = _run(posm, vel, bparams, 20)
+    assert p1.tobytes() == p2.tobytes() and v1.tobytes() == v2.tobytes()
+    cfg = W.CONFIGS[1]
+    for k in range(4):
+        dp, dv = torch.from_numpy(posm[k].copy()).cuda(), torch.from_numpy(vel[k].copy()).cuda()
+        acc = torch.empty_like(dp)
+        ws = B.alloc_workspace(B.workspace_bytes(n))
+        B.leapfrog_kdk(dp, dv, acc, cfg.G, cfg.eps, cfg.dt, 20, bparams[k][3], ws)
+        torch.cuda.synchronize()
+        rel = np.abs(dp.cpu().numpy()[:, :3] - p1[k, :, :3]).max() / 12.4
+        assert rel <= 2e-6
+
+
+def test_ensemble_zero_steps_many_simulations_and_argument_errors():
+    n, nsim = 300, 700                                          # more CTAs than one wave
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg, n=n)
+    posm = np.repeat(W.to_f32(p64)[None], nsim, axis=0)
+    vel = np.repeat(W.vel4(W.to_f32(v64), np.float32)[None], nsim, axis=0)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    p0, v0 = _run(posm, vel, [(cfg.G, cfg.eps, cfg.dt, pot)], 0)
+    assert p0.tobytes() == posm.tobytes() and v0.tobytes() == vel.tobytes()
+    p1, v1 = _run(posm, vel, [(cfg.G, cfg.eps, cfg.dt, pot)], 3)
+    assert all(p1[k].tobytes() == p1[0].tobytes() for k in range(nsim))      # identical inputs, identical outputs
+    dp, dv = torch.from_numpy(posm).cuda(), torch.from_numpy(vel).cuda()
+    ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
+    with pytest.raises(B.OdisseoError, match="ERR_ARG"):
+        B.ensemble_leapfrog_kdk(dp, dv, [(cfg.G, cfg.eps, cfg.dt, pot)] * 2, 1, ws)       # 2 records for 700 sims
+    with pytest.raises(B.OdisseoError, match="ERR_ARG"):
+        B.ensemble_leapfrog_kdk(dp, dv, [(cfg.G, 0.0, cfg.dt, pot)], 1, ws)               # eps must be > 0
+    big = torch.zeros(1, 2049, 4, device="cuda")
+    with pytest.raises(B.OdisseoError, match="ERR_ARG"):
+        B.ensemble_leapfrog_kdk(big, big.clone(), [(cfg.G, cfg.eps, cfg.dt, pot)], 1, ws)
