@@ -22,7 +22,7 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     if (p.variant == 0) {
         // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
         // packed interaction chains of a thread (2 warps per scheduler x ILP 4 beats 4.5 warps x ILP 1:
-        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144, profiles/r01_pair_f32_variants.txt)
+        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144)
         p.ipt = is_f64 ? 4 : 8;
         p.cthreads = 256;
         minb = 1;
@@ -35,10 +35,17 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     p.IB = p.ipt * p.cthreads;
     p.nb = (int32_t)((n + p.IB - 1) / p.IB);
     int64_t P = (int64_t)num_sms * minb;
-    int32_t T = (p.variant == 0 && !is_f64) ? 512 : 256;
-    for (; T > 32; T >>= 1) {
-        const int64_t U = (int64_t)p.nb * ((n + T - 1) / T);
-        if (U >= 8 * P) break;
+    // Tile length: the busiest CTA walks ceil(U / P) units of (T + overhead) source records each
+    // (overhead = barrier hand-over + fp64 flush of the tile sums, ~16 records' worth); take the T that
+    // minimises that product.  Long tiles amortise the overhead, short ones even out the stream-K split.
+    const int32_t Tmax = (p.variant == 0 && !is_f64) ? 512 : 256;
+    int32_t T = Tmax;
+    int64_t best = -1;
+    for (int32_t t = Tmax; t >= 32; t >>= 1) {
+        const int64_t U = (int64_t)p.nb * ((n + t - 1) / t);
+        const int64_t ctas = U < P ? U : P;
+        const int64_t cost = ((U + ctas - 1) / ctas) * (t + 16);
+        if (best < 0 || cost < best) { best = cost; T = t; }
     }
     p.T = T;
     p.J = (int32_t)((n + T - 1) / T);
