@@ -91,8 +91,9 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
-def _dist_setup(n_gpus: int):
-    """One process per GPU under torchrun; returns (rank, world, dist-or-None)."""
+def _dist_setup(n_gpus: int, backend: str = "nccl"):
+    """One process per GPU under torchrun; returns (rank, world, dist-or-None).  backend = "gloo" is the
+    CPU stand-in the tests use for the rank logic (no kernels run there)."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     if world == 1:
@@ -100,25 +101,39 @@ def _dist_setup(n_gpus: int):
     import torch
     import torch.distributed as dist
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    dist.init_process_group(backend="nccl")
+    if backend == "nccl":
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    dist.init_process_group(backend=backend)
     return rank, world, dist
 
 
+def replica_seed(cfg_seed: int, rank: int) -> int:
+    """Replicas only: every rank advances its own seeded copy of the workload."""
+    return int(cfg_seed) + int(rank)
+
+
 def _max_over_ranks(x: float, dist) -> float:
+    """The job is as slow as its slowest rank: MAX all-reduce of a device-measured duration."""
     if dist is None:
         return x
     import torch
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    device = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def whole_job_rate(n: int, steps: int, world: int, total_ms: float) -> float:
+    """G-int/s of the whole job: every rank processed steps * n^2 interactions in total_ms (max over ranks)."""
+    return world * steps * float(n) ** 2 / (total_ms * 1e-3) / 1e9
 
 
 def _barrier(dist):
     import torch
     if dist is not None:
         dist.barrier()
-    torch.cuda.synchronize()
+    if torch.cuda.is_available():
+        torch.cuda.synchronize()
 
 
 def _oracle_sample_rate(cfg, seconds_target: float):
@@ -271,7 +286,7 @@ def run_ours(args, rank: int, world: int, dist):
     dev = torch.cuda.current_device()
     cfg = W.CONFIGS[args.config]
     n = cfg.n
-    posm64, vel64 = W.make_state(cfg, seed=cfg.seed + rank)               # one seeded replica per rank
+    posm64, vel64 = W.make_state(cfg, seed=replica_seed(cfg.seed, rank))     # one seeded replica per rank
     p32, v32 = W.to_f32(posm64), W.vel4(W.to_f32(vel64), np.float32)
     G, eps, dt = float(np.float32(cfg.G)), float(np.float32(cfg.eps)), float(np.float32(cfg.dt))
     pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
@@ -304,7 +319,7 @@ def run_ours(args, rank: int, world: int, dist):
     _barrier(dist)
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = _max_over_ranks(float(np.sum(step_ms)), dist)
-    value = world * K * float(n) ** 2 / (total_ms * 1e-3) / 1e9
+    value = whole_job_rate(n, K, world, total_ms)
 
     # ---- end-to-end arm: host buffers through odisseo_leapfrog_kdk_host_f32 -------------------
     hp, hv = torch.from_numpy(p32.copy()).pin_memory(), torch.from_numpy(v32.copy()).pin_memory()
@@ -343,7 +358,7 @@ def run_ours(args, rank: int, world: int, dist):
         "kdk_steps_per_s": world * K / (total_ms * 1e-3),
         "gpu_launches": launches,
         "clocks": clocks,
-        "e2e": {"value": world * K * float(n) ** 2 / (e2e_ms * 1e-3) / 1e9, "unit": "G-int/s",
+        "e2e": {"value": whole_job_rate(n, K, world, e2e_ms), "unit": "G-int/s",
                 "h2d_bytes_per_step": 3 * 16 * n, "d2h_bytes_per_step": 3 * 16 * n,
                 "ms_per_step": e2e_ms / K},
         "roofline": {"bound": "alu", "kernel": "pair_f32x2_kernel", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
