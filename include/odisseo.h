@@ -155,6 +155,26 @@ odisseo_status odisseo_leapfrog_kdk_host_f64(double *h_posm, double *h_vel, doub
                                              const odisseo_potential *pot,
                                              void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* Conservation diagnostics: everything is evaluated in fp64 from the
+ * given state, whatever its precision, with fixed-order reductions (bit-reproducible).
+ *   d_out [16] double, DEVICE:  [0] kinetic energy 1/2 sum m v^2
+ *                               [1] pair potential energy -1/2 G sum_i sum_{j!=i} m_i m_j (r_ij^2+eps^2)^-1/2
+ *                               [2] external potential energy sum m_i (Phi_NFW + Phi_MN)(x_i)  (0 if pot NULL)
+ *                               [3..5] linear momentum  [6..8] angular momentum about the origin
+ *                               [9..11] centre of mass  [12] total mass  [13] = [0]+[1]+[2]  [14..15] 0
+ *   d_phi  optional DEVICE array of n doubles: per-particle pair potential phi_i (W = 1/2 sum m_i phi_i); may be NULL.
+ *   d_workspace  odisseo_diagnostics_workspace_bytes(n) bytes, 256-byte aligned.
+ * One O(N^2) fp64 pass (the fp64 pair kernel in potential mode) plus three O(N) kernels.  The pass sums
+ * the self term m_i / eps with the others and removes it afterwards, so [1] carries a rounding of a few
+ * ulp of the self energy 1/2 G sum m_i^2 / eps (invisible unless n is tiny). */
+size_t odisseo_diagnostics_workspace_bytes(int64_t n);
+odisseo_status odisseo_diagnostics_f32(const float *d_posm, const float *d_vel, int64_t n, float G, float eps,
+                                       const odisseo_potential *pot, double *d_out, double *d_phi,
+                                       void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_diagnostics_f64(const double *d_posm, const double *d_vel, int64_t n, double G, double eps,
+                                       const odisseo_potential *pot, double *d_out, double *d_phi,
+                                       void *d_workspace, size_t workspace_bytes, void *stream);
+
 /* Batched small-N ensembles (the paper's inference workload: 10^4 grid points and
  * bootstrap resamples, each an N = 1,000, 1,000-step simulation with its own potential masses,
  * progenitor mass and integration time, Fig. 2, L47, L53).  nsim independent simulations

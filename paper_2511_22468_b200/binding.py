@@ -27,6 +27,7 @@ EXPORTS = [
     "odisseo_describe_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
     "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
+    "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
 ]
 
 
@@ -85,12 +86,15 @@ def lib():
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_diagnostics_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
         L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        L.odisseo_diagnostics_workspace_bytes.restype = sz
+        L.odisseo_diagnostics_workspace_bytes.argtypes = [i64]
         L.odisseo_ensemble_workspace_bytes.restype = sz
         L.odisseo_ensemble_workspace_bytes.argtypes = [i64]
         L.odisseo_ensemble_leapfrog_kdk_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp]
@@ -244,6 +248,32 @@ def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch
               n, G, eps, dt,
               int(nsteps), _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "leapfrog_kdk_host_" + sfx)
+
+
+DIAGNOSTIC_FIELDS = ("kinetic", "pair_potential", "ext_potential", "px", "py", "pz", "lx", "ly", "lz",
+                     "com_x", "com_y", "com_z", "mass", "energy")
+
+
+def diagnostics_workspace_bytes(n: int) -> int:
+    return int(lib().odisseo_diagnostics_workspace_bytes(int(n)))
+
+
+def diagnostics(posm: torch.Tensor, vel: torch.Tensor, G: float, eps: float, pot: Optional[Potential],
+                out: torch.Tensor, workspace: torch.Tensor, phi: Optional[torch.Tensor] = None, stream=None):
+    """Energies, momenta and centre of mass of a state in fp64 (odisseo_diagnostics_f32/_f64).
+    out: float64 CUDA tensor of 16 values (DIAGNOSTIC_FIELDS name the first 14); phi: optional float64 [n]."""
+    n = _rec(posm, "posm")
+    _rec(vel, "vel", n)
+    sfx = _suffix(posm)
+    if out.dtype != torch.float64 or out.numel() < 16 or not out.is_cuda or not out.is_contiguous():
+        raise ValueError("out must be a contiguous float64 CUDA tensor of at least 16 values")
+    if phi is not None and (phi.dtype != torch.float64 or phi.numel() != n or not phi.is_cuda or not phi.is_contiguous()):
+        raise ValueError("phi must be a contiguous float64 CUDA tensor of n values")
+    fn = getattr(lib(), "odisseo_diagnostics_" + sfx)
+    _check(fn(posm.data_ptr(), vel.data_ptr(), n, G, eps, _pot(pot), out.data_ptr(),
+              phi.data_ptr() if phi is not None else None, workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "diagnostics_" + sfx)
+    return out
 
 
 def ensemble_workspace_bytes(nsim: int) -> int:

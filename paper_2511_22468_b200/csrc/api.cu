@@ -400,6 +400,63 @@ odisseo_status kick_drift_impl(T* posm, T* vel, const T* acc, int64_t n, T G, T 
     return ODISSEO_OK;
 }
 
+inline cudaError_t launch_diag_stage(const PairPlan& p, const float* x, void* j, cudaStream_t s) { return launch_diag_stage_f32(p, x, j, s); }
+inline cudaError_t launch_diag_stage(const PairPlan& p, const double* x, void* j, cudaStream_t s) { return launch_diag_stage_f64(p, x, j, s); }
+inline cudaError_t launch_diag_terms(const PairPlan& p, const float* x, const float* v, const double* part, double G, double eps,
+                                     const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
+{ return launch_diag_terms_f32(p, x, v, part, G, eps, pot, bs, phi, s); }
+inline cudaError_t launch_diag_terms(const PairPlan& p, const double* x, const double* v, const double* part, double G, double eps,
+                                     const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
+{ return launch_diag_terms_f64(p, x, v, part, G, eps, pot, bs, phi, s); }
+
+inline size_t diag_block_sum_bytes(int64_t n)
+{ return ((size_t)((n + STEP_THREADS - 1) / STEP_THREADS) * DIAG_VALUES * sizeof(double) + 255) & ~(size_t)255; }
+
+template <typename T>
+odisseo_status diagnostics_impl(const T* posm, const T* vel, int64_t n, T G, T eps, const odisseo_potential* pot,
+                                double* out, double* phi, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (!out) return ODISSEO_ERR_NULL;
+    if (misaligned(out, 8) || (phi && misaligned(phi, 8))) return ODISSEO_ERR_ALIGN;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (n == 0) {
+        e = cudaMemsetAsync(out, 0, DIAG_VALUES * sizeof(double), s);
+        return e == cudaSuccess ? ODISSEO_OK : cuda_fail(e);
+    }
+    if (!posm || !vel) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(vel, rec)) return ODISSEO_ERR_ALIGN;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    PotParams<double> pp;
+    st = make_pot<double>((double)G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, 1, dev.sms);        // the O(N^2) pass is always the fp64 kernel
+    if (!ws) return ODISSEO_ERR_NULL;
+    if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
+    const size_t bs_bytes = diag_block_sum_bytes(n);
+    if (ws_bytes < bs_bytes) return ODISSEO_ERR_WORKSPACE;
+    Carve cv;
+    st = carve(plan, static_cast<unsigned char*>(ws) + bs_bytes, ws_bytes - bs_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    double* block_sums = static_cast<double*>(ws);
+    g_launches.fetch_add(4, std::memory_order_relaxed);
+    e = launch_diag_stage(plan, posm, cv.jsrc, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_potential_f64(plan, cv.jsrc, cv.partials, (double)eps, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_diag_terms(plan, posm, vel, cv.partials, (double)G, (double)eps, pp, block_sums, phi, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_diag_final(block_sums, (int)((n + STEP_THREADS - 1) / STEP_THREADS), out, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
 template <typename T>
 odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
                                   const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
@@ -593,6 +650,22 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
                                         double G, double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
                                         void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+size_t odisseo_diagnostics_workspace_bytes(int64_t n)
+{
+    if (n <= 0) return 0;
+    return diag_block_sum_bytes(n) + odisseo_workspace_bytes(n, 1);
+}
+
+odisseo_status odisseo_diagnostics_f32(const float* d_posm, const float* d_vel, int64_t n, float G, float eps,
+                                       const odisseo_potential* pot, double* d_out, double* d_phi, void* d_workspace,
+                                       size_t workspace_bytes, void* stream)
+{ return diagnostics_impl<float>(d_posm, d_vel, n, G, eps, pot, d_out, d_phi, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_diagnostics_f64(const double* d_posm, const double* d_vel, int64_t n, double G, double eps,
+                                       const odisseo_potential* pot, double* d_out, double* d_phi, void* d_workspace,
+                                       size_t workspace_bytes, void* stream)
+{ return diagnostics_impl<double>(d_posm, d_vel, n, G, eps, pot, d_out, d_phi, d_workspace, workspace_bytes, stream); }
 
 size_t odisseo_ensemble_workspace_bytes(int64_t nsim)
 {

@@ -190,6 +190,19 @@ cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const Pot
 cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
                                 int64_t n, cudaStream_t stream);
 cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
+cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double* partials, double eps,
+                                 cudaStream_t stream);
+// diagnostics.cu: stage (promote to double) / per-particle terms + block sums / final fixed-order sum
+constexpr int DIAG_VALUES = 16;
+cudaError_t launch_diag_stage_f32(const PairPlan& plan, const float* posm, void* jsrc, cudaStream_t stream);
+cudaError_t launch_diag_stage_f64(const PairPlan& plan, const double* posm, void* jsrc, cudaStream_t stream);
+cudaError_t launch_diag_terms_f32(const PairPlan& plan, const float* posm, const float* vel, const double* partials,
+                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  double* phi_out, cudaStream_t stream);
+cudaError_t launch_diag_terms_f64(const PairPlan& plan, const double* posm, const double* vel, const double* partials,
+                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  double* phi_out, cudaStream_t stream);
+cudaError_t launch_diag_final(const double* block_sums, int nblocks, double* out, cudaStream_t stream);
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
                                 int64_t nsim, int64_t nsteps, cudaStream_t stream);
 cudaError_t configure_pair_f32();

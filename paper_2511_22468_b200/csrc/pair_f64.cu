@@ -20,7 +20,9 @@ constexpr int STAGES = 4;
 
 // Consumer side for one CTA.  EQM = all masses equal (flags from the staging kernel): the mass
 // factor leaves the inner loop (15 instead of 16 FP64 ops) and multiplies the sums once per segment.
-template <int IPT, int CWARPS, int JUNROLL, bool EQM>
+// POT = accumulate the softened potential sum_j m_j (r2)^-1/2 (x-plane of the partial rows only)
+// instead of the acceleration: the O(N^2) part of odisseo_diagnostics_* (diagnostics.cu).
+template <int IPT, int CWARPS, int JUNROLL, bool EQM, bool POT>
 __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, double* __restrict__ partials,
                                               const PairPlan& plan, const double eps2, unsigned char* smem_raw,
                                               uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
@@ -66,11 +68,17 @@ __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, 
                 const double y0 = rsqrt_approx_f64(r2);
                 const double t = y0 * y0;
                 const double e = fma(-r2, t, 1.0);
-                const double c = fma(e, fma(1.875, e, 1.5), 1.0);
-                const double w = EQM ? (t * y0) * c : ((t * y0) * q.w) * c;
-                ax[k] = fma(w, dx, ax[k]);
-                ay[k] = fma(w, dy, ay[k]);
-                az[k] = fma(w, dz, az[k]);
+                if (POT) {
+                    // (r2)^-1/2 = y0 (1-e)^-1/2 = y0 (1 + e (1/2 + 3/8 e)) + O(e^3)
+                    const double y = y0 * fma(e, fma(0.375, e, 0.5), 1.0);
+                    ax[k] = EQM ? ax[k] + y : fma(q.w, y, ax[k]);
+                } else {
+                    const double c = fma(e, fma(1.875, e, 1.5), 1.0);
+                    const double w = EQM ? (t * y0) * c : ((t * y0) * q.w) * c;
+                    ax[k] = fma(w, dx, ax[k]);
+                    ay[k] = fma(w, dy, ay[k]);
+                    az[k] = fma(w, dz, az[k]);
+                }
             }
         }
         __syncwarp();
@@ -84,8 +92,10 @@ __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, 
             for (int k = 0; k < IPT; ++k) {
                 const int r = k * CTHREADS + tid;
                 row[r] = m0 * ax[k];
-                row[plan.IB + r] = m0 * ay[k];
-                row[2 * plan.IB + r] = m0 * az[k];
+                if (!POT) {
+                    row[plan.IB + r] = m0 * ay[k];
+                    row[2 * plan.IB + r] = m0 * az[k];
+                }
             }
             seg_start = true;
         }
@@ -93,7 +103,7 @@ __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, 
     }
 }
 
-template <int IPT, int CWARPS, int MINB, int JUNROLL>
+template <int IPT, int CWARPS, int MINB, int JUNROLL, bool POT>
 __global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
 pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ jsrc, double* __restrict__ partials,
                 const PairPlan plan, const double eps2)
@@ -146,17 +156,17 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
     }
 
     if (eqm)
-        consume_tiles<IPT, CWARPS, JUNROLL, true>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<IPT, CWARPS, JUNROLL, true, POT>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
     else
-        consume_tiles<IPT, CWARPS, JUNROLL, false>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<IPT, CWARPS, JUNROLL, false, POT>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
 }
 
-template <int IPT, int CWARPS, int MINB, int JUNROLL>
+template <int IPT, int CWARPS, int MINB, int JUNROLL, bool POT>
 cudaError_t launch_variant(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
                            cudaStream_t stream)
 {
     const size_t smem = (size_t)STAGES * plan.T * 32;
-    pair_f64_kernel<IPT, CWARPS, MINB, JUNROLL><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
+    pair_f64_kernel<IPT, CWARPS, MINB, JUNROLL, POT><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
         reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(jsrc), partials, plan, eps * eps);
     return cudaGetLastError();
 }
@@ -165,18 +175,31 @@ cudaError_t launch_variant(const PairPlan& plan, const double* posm, const void*
 
 cudaError_t configure_pair_f64()
 {
-    cudaError_t e = cudaFuncSetAttribute(pair_f64_kernel<4, 8, 1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         STAGES * 256 * 32);
+    const int smem = STAGES * 256 * 32;
+    cudaError_t e = cudaFuncSetAttribute(pair_f64_kernel<4, 8, 1, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_f64_kernel<2, 2, 8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                STAGES * 256 * 32);
+    e = cudaFuncSetAttribute(pair_f64_kernel<2, 2, 8, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pair_f64_kernel<4, 8, 1, 4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pair_f64_kernel<2, 2, 8, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
                             cudaStream_t stream)
 {
-    if (plan.variant == 0) return launch_variant<4, 8, 1, 4>(plan, posm, jsrc, partials, eps, stream);
-    return launch_variant<2, 2, 8, 2>(plan, posm, jsrc, partials, eps, stream);
+    if (plan.variant == 0) return launch_variant<4, 8, 1, 4, false>(plan, posm, jsrc, partials, eps, stream);
+    return launch_variant<2, 2, 8, 2, false>(plan, posm, jsrc, partials, eps, stream);
+}
+
+// Softened potential sums phi'_i = sum_j m_j (r_ij^2 + eps^2)^-1/2 (self term included) into the x-plane of
+// the partial rows; targets are read from the staged double records themselves.
+cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double* partials, double eps,
+                                 cudaStream_t stream)
+{
+    const double* targets = static_cast<const double*>(jsrc);
+    if (plan.variant == 0) return launch_variant<4, 8, 1, 4, true>(plan, targets, jsrc, partials, eps, stream);
+    return launch_variant<2, 2, 8, 2, true>(plan, targets, jsrc, partials, eps, stream);
 }
 
 }  // namespace odisseo
