@@ -175,6 +175,47 @@ odisseo_status odisseo_diagnostics_f64(const double *d_posm, const double *d_vel
                                        const odisseo_potential *pot, double *d_out, double *d_phi,
                                        void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* Reverse-mode derivative.  The paper's simulator is "end-to-end differentiable" with
+ * respect to initial conditions, integration time, particle masses and potential parameters (PAPER.md:L15,
+ * L21; used for Theta = (t_end, M_Plummer, M_NFW, M_MN) in L43 and for (M_vir, r_s, M, a, b) in L63).
+ *
+ * odisseo_accel_vjp_*: cotangent d_cot [n][4] (lanes x, y, z; pad ignored) pulled back through
+ *   a(x) = a_pair(x; m, G, eps) + a_NFW(x) + a_MN(x):
+ *     d_gx [n][4]      (da/dx)^T c                      (pad lane 0)
+ *     d_gm [n] double  d(c.a)/dm_i
+ *     d_gparams [8] double, DEVICE: d(c.a)/d(M_s, r_s, M_d, a, b, G, eps), slot 7 = 0
+ * odisseo_leapfrog_kdk_tape_*: odisseo_leapfrog_kdk_* (acc_valid = 0) that also records the nsteps + 1
+ *   snapshots {posm, vel, pair-only acc} k = 0..nsteps into d_tape (odisseo_tape_bytes(n, nsteps, is_f64)
+ *   bytes: snapshot k at byte offset k * 3 * n * record size).  Final state bit-identical to the plain call.
+ * odisseo_leapfrog_kdk_vjp_*: given the tape and the cotangents of the final state, d_lx = dL/dx_N and
+ *   d_lv = dL/dv_N ([n][4], in/out), returns in place dL/dx_0 and dL/dv_0, and
+ *     d_gm [n] double  dL/dm_i        d_gparams [8] double: dL/d(M_s, r_s, M_d, a, b, G, eps, dt)
+ *   (dt at fixed nsteps, i.e. t_end / nsteps; M_s, r_s, M_d, a, b as in odisseo_potential, disabled terms give 0).
+ * O(N^2) pull-back per recorded step (~35 flops per pair), fixed-order sums (bit-reproducible), O(N) parts in
+ * fp64.  Workspace: odisseo_vjp_workspace_bytes(n, is_f64), 256-byte aligned. */
+size_t odisseo_vjp_workspace_bytes(int64_t n, int is_f64);
+size_t odisseo_tape_bytes(int64_t n, int64_t nsteps, int is_f64);
+odisseo_status odisseo_accel_vjp_f32(const float *d_posm, const float *d_cot, int64_t n, float G, float eps,
+                                     const odisseo_potential *pot, float *d_gx, double *d_gm, double *d_gparams,
+                                     void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_accel_vjp_f64(const double *d_posm, const double *d_cot, int64_t n, double G, double eps,
+                                     const odisseo_potential *pot, double *d_gx, double *d_gm, double *d_gparams,
+                                     void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_tape_f32(float *d_posm, float *d_vel, float *d_acc, int64_t n, float G, float eps,
+                                             float dt, int64_t nsteps, const odisseo_potential *pot,
+                                             float *d_tape, size_t tape_bytes,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_tape_f64(double *d_posm, double *d_vel, double *d_acc, int64_t n, double G, double eps,
+                                             double dt, int64_t nsteps, const odisseo_potential *pot,
+                                             double *d_tape, size_t tape_bytes,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_vjp_f32(const float *d_tape, int64_t n, float G, float eps, float dt, int64_t nsteps,
+                                            const odisseo_potential *pot, float *d_lx, float *d_lv, double *d_gm,
+                                            double *d_gparams, void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_leapfrog_kdk_vjp_f64(const double *d_tape, int64_t n, double G, double eps, double dt, int64_t nsteps,
+                                            const odisseo_potential *pot, double *d_lx, double *d_lv, double *d_gm,
+                                            double *d_gparams, void *d_workspace, size_t workspace_bytes, void *stream);
+
 /* Batched small-N ensembles (the paper's inference workload: 10^4 grid points and
  * bootstrap resamples, each an N = 1,000, 1,000-step simulation with its own potential masses,
  * progenitor mass and integration time, Fig. 2, L47, L53).  nsim independent simulations

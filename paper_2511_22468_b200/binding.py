@@ -28,6 +28,9 @@ EXPORTS = [
     "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
+    "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
+    "odisseo_leapfrog_kdk_tape_f32", "odisseo_leapfrog_kdk_tape_f64", "odisseo_leapfrog_kdk_vjp_f32",
+    "odisseo_leapfrog_kdk_vjp_f64",
 ]
 
 
@@ -86,6 +89,9 @@ def lib():
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_accel_vjp_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, vp, sz, vp]
+            getattr(L, "odisseo_leapfrog_kdk_tape_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, sc, i64, vp, vp, sz, vp, sz, vp]
+            getattr(L, "odisseo_leapfrog_kdk_vjp_" + suffix).argtypes = [vp, i64, sc, sc, sc, i64, vp, vp, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_diagnostics_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
@@ -93,6 +99,10 @@ def lib():
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
         L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        L.odisseo_vjp_workspace_bytes.restype = sz
+        L.odisseo_vjp_workspace_bytes.argtypes = [i64, ci]
+        L.odisseo_tape_bytes.restype = sz
+        L.odisseo_tape_bytes.argtypes = [i64, i64, ci]
         L.odisseo_diagnostics_workspace_bytes.restype = sz
         L.odisseo_diagnostics_workspace_bytes.argtypes = [i64]
         L.odisseo_ensemble_workspace_bytes.restype = sz
@@ -248,6 +258,69 @@ def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch
               n, G, eps, dt,
               int(nsteps), _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "leapfrog_kdk_host_" + sfx)
+
+
+GRADIENT_FIELDS = ("M_s", "r_s", "M_d", "a", "b", "G", "eps", "dt")
+
+
+def vjp_workspace_bytes(n: int, is_f64: bool = False) -> int:
+    return int(lib().odisseo_vjp_workspace_bytes(int(n), int(bool(is_f64))))
+
+
+def tape_bytes(n: int, nsteps: int, is_f64: bool = False) -> int:
+    return int(lib().odisseo_tape_bytes(int(n), int(nsteps), int(bool(is_f64))))
+
+
+def _f64vec(t: torch.Tensor, name: str, numel: int):
+    if t.dtype != torch.float64 or t.numel() < numel or not t.is_cuda or not t.is_contiguous():
+        raise ValueError("%s must be a contiguous float64 CUDA tensor of %d values" % (name, numel))
+
+
+def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: Optional[Potential], gx: torch.Tensor,
+              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, stream=None):
+    """Cotangent cot [n,4] pulled back through a = a_pair + a_ext (odisseo_accel_vjp_f32/_f64)."""
+    n = _rec(posm, "posm")
+    _rec(cot, "cot", n)
+    _rec(gx, "gx", n)
+    _f64vec(gm, "gm", n)
+    _f64vec(gparams, "gparams", 8)
+    sfx = _suffix(posm)
+    fn = getattr(lib(), "odisseo_accel_vjp_" + sfx)
+    _check(fn(posm.data_ptr(), cot.data_ptr(), n, G, eps, _pot(pot), gx.data_ptr(), gm.data_ptr(), gparams.data_ptr(),
+              workspace.data_ptr(), workspace.numel(), _stream(stream)), "accel_vjp_" + sfx)
+
+
+def leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, eps: float, dt: float,
+                      nsteps: int, pot: Optional[Potential], tape: torch.Tensor, workspace: torch.Tensor, stream=None):
+    """leapfrog_kdk that also records the nsteps + 1 snapshots {posm, vel, pair-only acc} into tape
+    (same dtype, at least 3 * (nsteps + 1) * n * 4 scalars)."""
+    n = _rec(posm, "posm")
+    _rec(vel, "vel", n)
+    _rec(acc, "acc", n)
+    sfx = _suffix(posm)
+    if tape.dtype != posm.dtype or not tape.is_cuda or not tape.is_contiguous():
+        raise ValueError("tape must be a contiguous CUDA tensor of the state's dtype")
+    fn = getattr(lib(), "odisseo_leapfrog_kdk_tape_" + sfx)
+    _check(fn(posm.data_ptr(), vel.data_ptr(), acc.data_ptr(), n, G, eps, dt, int(nsteps), _pot(pot), tape.data_ptr(),
+              tape.numel() * tape.element_size(), workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "leapfrog_kdk_tape_" + sfx)
+
+
+def leapfrog_kdk_vjp(tape: torch.Tensor, n: int, G: float, eps: float, dt: float, nsteps: int, pot: Optional[Potential],
+                     lx: torch.Tensor, lv: torch.Tensor, gm: torch.Tensor, gparams: torch.Tensor,
+                     workspace: torch.Tensor, stream=None):
+    """Reverse-mode derivative of nsteps KDK steps from the tape: lx, lv [n,4] hold dL/dx_N, dL/dv_N on entry and
+    dL/dx_0, dL/dv_0 on exit; gm [n] and gparams [8] (GRADIENT_FIELDS) are float64 outputs."""
+    _rec(lx, "lx", n)
+    _rec(lv, "lv", n)
+    _f64vec(gm, "gm", n)
+    _f64vec(gparams, "gparams", 8)
+    sfx = _suffix(lx)
+    if tape.dtype != lx.dtype or not tape.is_cuda or tape.numel() < 12 * n * (nsteps + 1):
+        raise ValueError("tape does not hold nsteps + 1 snapshots of the state's dtype")
+    fn = getattr(lib(), "odisseo_leapfrog_kdk_vjp_" + sfx)
+    _check(fn(tape.data_ptr(), n, G, eps, dt, int(nsteps), _pot(pot), lx.data_ptr(), lv.data_ptr(), gm.data_ptr(),
+              gparams.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream(stream)), "leapfrog_kdk_vjp_" + sfx)
 
 
 DIAGNOSTIC_FIELDS = ("kinetic", "pair_potential", "ext_potential", "px", "py", "pz", "lx", "ly", "lz",

@@ -457,6 +457,127 @@ odisseo_status diagnostics_impl(const T* posm, const T* vel, int64_t n, T G, T e
     return ODISSEO_OK;
 }
 
+inline cudaError_t launch_accel_vjp(const float* x, const float* c, int64_t n, double G, double eps, const PotParams<double>& pot, float* gx,
+                                    double* gm, double* gp, const double* dts, int accum, void* ws, int sms, cudaStream_t s)
+{ return launch_accel_vjp_f32(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, ws, sms, s); }
+inline cudaError_t launch_accel_vjp(const double* x, const double* c, int64_t n, double G, double eps, const PotParams<double>& pot, double* gx,
+                                    double* gm, double* gp, const double* dts, int accum, void* ws, int sms, cudaStream_t s)
+{ return launch_accel_vjp_f64(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, ws, sms, s); }
+inline cudaError_t launch_vjp_pre(const float* tk, const float* tk1, int64_t n, const PotParams<float>& pot, float dt, float w, int first,
+                                  const float* lx, float* lv, float* cot, double* dts, cudaStream_t s)
+{ return launch_vjp_pre_f32(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
+inline cudaError_t launch_vjp_pre(const double* tk, const double* tk1, int64_t n, const PotParams<double>& pot, double dt, double w, int first,
+                                  const double* lx, double* lv, double* cot, double* dts, cudaStream_t s)
+{ return launch_vjp_pre_f64(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
+
+template <typename T>
+odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps, const odisseo_potential* pot, T* gx,
+                              double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (!gparams) return ODISSEO_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (n == 0) {
+        cudaError_t e0 = cudaMemsetAsync(gparams, 0, 8 * sizeof(double), s);
+        return e0 == cudaSuccess ? ODISSEO_OK : cuda_fail(e0);
+    }
+    if (!posm || !cot || !gx || !gm || !ws) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(posm, rec) || misaligned(cot, rec) || misaligned(gx, rec) || misaligned(gm, 8) || misaligned(gparams, 8) ||
+        misaligned(ws, 256))
+        return ODISSEO_ERR_ALIGN;
+    if (overlap(posm, n * rec, gx, n * rec) || overlap(cot, n * rec, gx, n * rec)) return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    PotParams<double> pp;
+    st = make_pot<double>((double)G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    if (ws_bytes < vjp_workspace_bytes(n, sizeof(T) == 8, dev.sms)) return ODISSEO_ERR_WORKSPACE;
+    g_launches.fetch_add(3, std::memory_order_relaxed);
+    cudaError_t e = launch_accel_vjp(posm, cot, n, (double)G, (double)eps, pp, gx, gm, gparams, nullptr, 0, ws, dev.sms, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status leapfrog_tape_impl(T* posm, T* vel, T* acc, int64_t n, T G, T eps, T dt, int64_t nsteps,
+                                  const odisseo_potential* pot, T* tape, size_t tape_bytes, void* ws, size_t ws_bytes,
+                                  void* stream)
+{
+    if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!tape) return ODISSEO_ERR_NULL;
+    const size_t arr = (size_t)n * 4 * sizeof(T);
+    if (misaligned(tape, 4 * sizeof(T))) return ODISSEO_ERR_ALIGN;
+    if (tape_bytes < (size_t)(nsteps + 1) * 3 * arr) return ODISSEO_ERR_WORKSPACE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    unsigned char* t = reinterpret_cast<unsigned char*>(tape);
+    for (int64_t k = 0; k <= nsteps; ++k) {
+        odisseo_status st = leapfrog_impl<T>(posm, vel, acc, k > 0, n, G, eps, dt, k > 0 ? 1 : 0, pot, ws, ws_bytes, stream);
+        if (st != ODISSEO_OK) return st;
+        cudaError_t e = cudaMemcpyAsync(t, posm, arr, cudaMemcpyDeviceToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(t + arr, vel, arr, cudaMemcpyDeviceToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(t + 2 * arr, acc, arr, cudaMemcpyDeviceToDevice, s);
+        if (e != cudaSuccess) return cuda_fail(e);
+        t += 3 * arr;
+    }
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int64_t nsteps, const odisseo_potential* pot,
+                                 T* lx, T* lv, double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
+    if (!gparams) return ODISSEO_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemsetAsync(gparams, 0, 8 * sizeof(double), s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (n == 0) return ODISSEO_OK;
+    if (!tape || !lx || !lv || !gm || !ws) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(tape, rec) || misaligned(lx, rec) || misaligned(lv, rec) || misaligned(gm, 8) || misaligned(gparams, 8) ||
+        misaligned(ws, 256))
+        return ODISSEO_ERR_ALIGN;
+    if (overlap(lx, n * rec, lv, n * rec)) return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
+    PotParams<double> pd;
+    st = make_pot<double>((double)G, pot, pd);
+    if (st != ODISSEO_OK) return st;
+    PotParams<T> pt;
+    st = make_pot<T>(G, pot, pt);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    if (ws_bytes < vjp_workspace_bytes(n, sizeof(T) == 8, dev.sms)) return ODISSEO_ERR_WORKSPACE;
+    e = cudaMemsetAsync(gm, 0, (size_t)n * sizeof(double), s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (nsteps == 0) return ODISSEO_OK;                    // the final state is the initial state
+    double* dt_sums;
+    void* cotv;
+    vjp_carve(ws, n, dev.sms, &dt_sums, &cotv);
+    T* cot = static_cast<T*>(cotv);
+    const size_t snap = (size_t)n * 12;                    // scalars per snapshot
+    const T half = (T)0.5 * dt;
+    for (int64_t k = nsteps; k >= 0; --k) {
+        const T* tk = tape + (size_t)k * snap;
+        const int first = k == nsteps;
+        const T w = (first || k == 0) ? half : dt;
+        g_launches.fetch_add(4, std::memory_order_relaxed);
+        e = launch_vjp_pre(tk, first ? (const T*)nullptr : tk + snap, n, pt, dt, w, first, lx, lv, cot, dt_sums, s);
+        if (e != cudaSuccess) return cuda_fail(e);
+        e = launch_accel_vjp(tk, cot, n, (double)G, (double)eps, pd, lx, gm, gparams, dt_sums, 1, ws, dev.sms, s);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return ODISSEO_OK;
+}
+
 template <typename T>
 odisseo_status leapfrog_host_impl(T* h_posm, T* h_vel, T* h_acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
                                   const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
@@ -650,6 +771,48 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
                                         double G, double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
                                         void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_impl<double>(d_posm, d_vel, d_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+size_t odisseo_vjp_workspace_bytes(int64_t n, int is_f64)
+{
+    if (n <= 0) return 0;
+    size_t b = 0;
+    for (int sms = 64; sms <= 192; sms += 4) {            // bound over devices with up to 192 SMs
+        const size_t c = vjp_workspace_bytes(n, is_f64, sms);
+        if (c > b) b = c;
+    }
+    return b;
+}
+
+size_t odisseo_tape_bytes(int64_t n, int64_t nsteps, int is_f64)
+{
+    if (n <= 0 || nsteps < 0) return 0;
+    return (size_t)(nsteps + 1) * 3 * (size_t)n * 4 * (is_f64 ? 8 : 4);
+}
+
+odisseo_status odisseo_accel_vjp_f32(const float* d_posm, const float* d_cot, int64_t n, float G, float eps,
+                                     const odisseo_potential* pot, float* d_gx, double* d_gm, double* d_gparams,
+                                     void* d_workspace, size_t workspace_bytes, void* stream)
+{ return accel_vjp_impl<float>(d_posm, d_cot, n, G, eps, pot, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_accel_vjp_f64(const double* d_posm, const double* d_cot, int64_t n, double G, double eps,
+                                     const odisseo_potential* pot, double* d_gx, double* d_gm, double* d_gparams,
+                                     void* d_workspace, size_t workspace_bytes, void* stream)
+{ return accel_vjp_impl<double>(d_posm, d_cot, n, G, eps, pot, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_leapfrog_kdk_tape_f32(float* d_posm, float* d_vel, float* d_acc, int64_t n, float G, float eps, float dt,
+                                             int64_t nsteps, const odisseo_potential* pot, float* d_tape, size_t tape_bytes,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_tape_impl<float>(d_posm, d_vel, d_acc, n, G, eps, dt, nsteps, pot, d_tape, tape_bytes, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_leapfrog_kdk_tape_f64(double* d_posm, double* d_vel, double* d_acc, int64_t n, double G, double eps, double dt,
+                                             int64_t nsteps, const odisseo_potential* pot, double* d_tape, size_t tape_bytes,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_tape_impl<double>(d_posm, d_vel, d_acc, n, G, eps, dt, nsteps, pot, d_tape, tape_bytes, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_leapfrog_kdk_vjp_f32(const float* d_tape, int64_t n, float G, float eps, float dt, int64_t nsteps,
+                                            const odisseo_potential* pot, float* d_lx, float* d_lv, double* d_gm,
+                                            double* d_gparams, void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_vjp_impl<float>(d_tape, n, G, eps, dt, nsteps, pot, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_leapfrog_kdk_vjp_f64(const double* d_tape, int64_t n, double G, double eps, double dt, int64_t nsteps,
+                                            const odisseo_potential* pot, double* d_lx, double* d_lv, double* d_gm,
+                                            double* d_gparams, void* d_workspace, size_t workspace_bytes, void* stream)
+{ return leapfrog_vjp_impl<double>(d_tape, n, G, eps, dt, nsteps, pot, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
 
 size_t odisseo_diagnostics_workspace_bytes(int64_t n)
 {

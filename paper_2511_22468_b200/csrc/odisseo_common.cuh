@@ -203,6 +203,20 @@ cudaError_t launch_diag_terms_f64(const PairPlan& plan, const double* posm, cons
                                   double G, double eps, const PotParams<double>& pot, double* block_sums,
                                   double* phi_out, cudaStream_t stream);
 cudaError_t launch_diag_final(const double* block_sums, int nblocks, double* out, cudaStream_t stream);
+// adjoint.cu
+void vjp_plan(int64_t n, int num_sms, int* nsplit, int64_t* chunk);
+size_t vjp_workspace_bytes(int64_t n, int is_f64, int num_sms);
+void vjp_carve(void* ws, int64_t n, int num_sms, double** dt_sums, void** cot);
+cudaError_t launch_accel_vjp_f32(const float* posm, const float* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
+                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
+                                 int num_sms, cudaStream_t stream);
+cudaError_t launch_accel_vjp_f64(const double* posm, const double* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
+                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
+                                 int num_sms, cudaStream_t stream);
+cudaError_t launch_vjp_pre_f32(const float* tape_k, const float* tape_k1, int64_t n, const PotParams<float>& pot, float dt, float w,
+                               int first, const float* lx, float* lv, float* cot, double* dt_sums, cudaStream_t stream);
+cudaError_t launch_vjp_pre_f64(const double* tape_k, const double* tape_k1, int64_t n, const PotParams<double>& pot, double dt,
+                               double w, int first, const double* lx, double* lv, double* cot, double* dt_sums, cudaStream_t stream);
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
                                 int64_t nsim, int64_t nsteps, cudaStream_t stream);
 cudaError_t configure_pair_f32();
