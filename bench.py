@@ -277,6 +277,38 @@ def _ensemble_rate(B, W, torch, n: int = 1000, nsim: int = 2960, nsteps: int = 5
             "G_int_per_s": ints / (ms * 1e-3) / 1e9, "frac_fp32_peak": tf / FP32_PEAK_TFLOPS, "gpu_launches": 1}
 
 
+def _adjoint_rate(B, W, torch, n: int = 16384, nsteps: int = 20):
+    """Reverse-mode derivative: forward with tape + backward through nsteps KDK steps of a
+    config-1-shaped progenitor, fp32; the O(N^2) pull-back kernel dominates (37 flops per pair)."""
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg, n=n)
+    posm0 = torch.from_numpy(W.to_f32(p64)).cuda()
+    vel0 = torch.from_numpy(W.vel4(W.to_f32(v64), np.float32)).cuda()
+    acc = torch.empty_like(posm0)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    ws = B.alloc_workspace(max(B.workspace_bytes(n), B.vjp_workspace_bytes(n)))
+    tape = torch.empty(B.tape_bytes(n, nsteps) // 4, dtype=torch.float32, device="cuda")
+    gm = torch.empty(n, dtype=torch.float64, device="cuda")
+    gp = torch.empty(8, dtype=torch.float64, device="cuda")
+    times = []
+    for rep in range(3):
+        posm, vel = posm0.clone(), vel0.clone()
+        lx, lv = torch.ones_like(posm), torch.zeros_like(posm)           # loss = sum of final coordinates
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record()
+        B.leapfrog_kdk_tape(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, tape, ws)
+        e1.record()
+        B.leapfrog_kdk_vjp(tape, n, cfg.G, cfg.eps, cfg.dt, nsteps, pot, lx, lv, gm, gp, ws)
+        e2.record()
+        torch.cuda.synchronize()
+        times.append((e0.elapsed_time(e1), e1.elapsed_time(e2)))
+    fwd, bwd = min(t[0] for t in times), min(t[1] for t in times)
+    pairs = (nsteps + 1) * float(n) ** 2
+    return {"workload": "%s shape, N = %d, %d KDK steps, fp32" % (cfg.name, n, nsteps), "forward_tape_ms": fwd,
+            "backward_ms": bwd, "backward_G_pairs_per_s": pairs / (bwd * 1e-3) / 1e9,
+            "backward_over_forward": bwd / fwd, "dL_d(M_s,r_s,M_d,a,b,G,eps,dt)": [float(x) for x in gp.cpu()]}
+
+
 def run_ours(args, rank: int, world: int, dist):
     import torch
     from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
@@ -396,6 +428,7 @@ def run_ours(args, rank: int, world: int, dist):
         del posm_g, acc_g
         line["integrator_roofline"] = _integrator_roofline(B, W, torch, peaks, peak_kind)
         line["ensemble"] = _ensemble_rate(B, W, torch)
+        line["adjoint"] = _adjoint_rate(B, W, torch)
     print(json.dumps(line), flush=True)
 
 
