@@ -309,6 +309,42 @@ def _adjoint_rate(B, W, torch, n: int = 16384, nsteps: int = 20):
             "backward_over_forward": bwd / fwd, "dL_d(M_s,r_s,M_d,a,b,G,eps,dt)": [float(x) for x in gp.cpu()]}
 
 
+def _ensemble_adjoint_rate(B, W, torch, n: int = 1000, nsim: int = 296, nsteps: int = 100):
+    """Gradient of every simulation of a batch (the paper's gradient-descent stage shape, PAPER.md:L43 steps 5-6):
+    ensemble forward with tape + ensemble backward, one launch each."""
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg, n=n)
+    posm = torch.from_numpy(np.repeat(W.to_f32(p64)[None], nsim, axis=0)).cuda()
+    vel = torch.from_numpy(np.repeat(W.vel4(W.to_f32(v64), np.float32)[None], nsim, axis=0)).cuda()
+    ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
+    rng = np.random.Generator(np.random.PCG64(6))
+    prm = [(cfg.G, cfg.eps, cfg.dt * rng.uniform(0.5, 1.5),
+            B.Potential.make(nfw=(cfg.nfw[0] * rng.uniform(0.5, 2.0), cfg.nfw[1]),
+                             mn=(cfg.mn[0] * rng.uniform(0.5, 2.0), cfg.mn[1], cfg.mn[2]))) for _ in range(nsim)]
+    tape = torch.empty(B.ensemble_tape_bytes(n, nsim, nsteps) // 4, dtype=torch.float32, device="cuda")
+    gm = torch.empty(nsim, n, dtype=torch.float64, device="cuda")
+    gp = torch.empty(nsim, 8, dtype=torch.float64, device="cuda")
+    best = None
+    for _ in range(2):
+        p, v = posm.clone(), vel.clone()
+        lx, lv = torch.ones_like(p), torch.zeros_like(p)
+        lx[:, :, 3] = 0
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record()
+        B.ensemble_leapfrog_kdk_tape(p, v, prm, nsteps, tape, ws)
+        e1.record()
+        B.ensemble_leapfrog_kdk_vjp(tape, prm, nsteps, lx, lv, gm, gp, ws)
+        e2.record()
+        torch.cuda.synchronize()
+        best = (e0.elapsed_time(e1), e1.elapsed_time(e2))
+    pairs = nsim * (nsteps + 1) * float(n) ** 2
+    return {"workload": "gradients of %d simulations, N = %d each, %d KDK steps, per-simulation parameters" % (nsim, n, nsteps),
+            "tape_GB": tape.numel() * 4 / 1e9, "forward_tape_ms": best[0], "backward_ms": best[1],
+            "backward_G_pairs_per_s": pairs / (best[1] * 1e-3) / 1e9,
+            "backward_frac_fp32_peak_at_37_flops": 37.0 * pairs / (best[1] * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+            "sim_grad_steps_per_s": nsim * nsteps / ((best[0] + best[1]) * 1e-3), "gpu_launches": 2}
+
+
 def run_ours(args, rank: int, world: int, dist):
     import torch
     from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
@@ -429,6 +465,7 @@ def run_ours(args, rank: int, world: int, dist):
         line["integrator_roofline"] = _integrator_roofline(B, W, torch, peaks, peak_kind)
         line["ensemble"] = _ensemble_rate(B, W, torch)
         line["adjoint"] = _adjoint_rate(B, W, torch)
+        line["ensemble_adjoint"] = _ensemble_adjoint_rate(B, W, torch)
     print(json.dumps(line), flush=True)
 
 

@@ -224,7 +224,7 @@ odisseo_status odisseo_leapfrog_kdk_vjp_f64(const double *d_tape, int64_t n, dou
  *   d_posm, d_vel  [nsim][n][4] float, in/out (device, 16-byte aligned); masses preserved, vel pad lane 0.
  *   h_params       HOST array of nparams records; nparams == 1: all simulations share it, else
  *                  nparams must equal nsim.  eps > 0 per record; pot terms with mass <= 0 are disabled.
- *   d_workspace    odisseo_ensemble_workspace_bytes(nsim) bytes, 256-byte aligned (device copy of the
+ *   d_workspace    odisseo_ensemble_workspace_bytes(nsim) bytes, 256-byte aligned (device copies of the
  *                  parameter records; h_params may be reused as soon as the call returns).
  * Each simulation computes exactly what odisseo_leapfrog_kdk_f32 computes (acc_valid = 0), with fp32
  * two-level summation in 512-source tiles; results agree with it to rounding, not bit for bit. */
@@ -234,6 +234,26 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float *d_posm, float *d_vel, in
                                                  const odisseo_sim_params *h_params, int64_t nparams,
                                                  int64_t nsteps, void *d_workspace, size_t workspace_bytes,
                                                  void *stream);
+
+/* Reverse-mode derivative of the ensembles (the paper's gradient-descent stage: 10 gradient steps for each of
+ * 1,000 bootstrap resamples of an N = 1,000, 1,000-step simulation, PAPER.md:L43 steps 5-6, L47, L53).
+ *   odisseo_ensemble_leapfrog_kdk_tape_f32: the ensemble call that also records, per simulation and per step
+ *     k = 0..nsteps, {posm, vel, TOTAL acceleration} ([nsim][nsteps+1][3][n][4] float,
+ *     odisseo_ensemble_tape_bytes(n, nsim, nsteps) bytes).  Final state identical to the plain call.
+ *   odisseo_ensemble_leapfrog_kdk_vjp_f32: d_lx, d_lv [nsim][n][4] hold dL/dx_N, dL/dv_N of every simulation on
+ *     entry and dL/dx_0, dL/dv_0 on exit; d_gm [nsim][n] double = dL/dm_i; d_gparams [nsim][8] double =
+ *     dL/d(M_s, r_s, M_d, a, b, G, eps, dt) of each simulation.  h_params as in the forward call (the same
+ *     records).  One CTA per simulation, the whole backward time loop in one kernel. */
+size_t odisseo_ensemble_tape_bytes(int64_t n, int64_t nsim, int64_t nsteps);
+odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float *d_posm, float *d_vel, int64_t n, int64_t nsim,
+                                                      const odisseo_sim_params *h_params, int64_t nparams,
+                                                      int64_t nsteps, float *d_tape, size_t tape_bytes,
+                                                      void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float *d_tape, int64_t n, int64_t nsim,
+                                                     const odisseo_sim_params *h_params, int64_t nparams,
+                                                     int64_t nsteps, float *d_lx, float *d_lv, double *d_gm,
+                                                     double *d_gparams, void *d_workspace, size_t workspace_bytes,
+                                                     void *stream);
 
 /* Instrumentation (bench.py's gpu_launches and roofline legs).
  *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA

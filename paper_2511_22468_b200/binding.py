@@ -30,7 +30,8 @@ EXPORTS = [
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
     "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
     "odisseo_leapfrog_kdk_tape_f32", "odisseo_leapfrog_kdk_tape_f64", "odisseo_leapfrog_kdk_vjp_f32",
-    "odisseo_leapfrog_kdk_vjp_f64",
+    "odisseo_leapfrog_kdk_vjp_f64", "odisseo_ensemble_tape_bytes", "odisseo_ensemble_leapfrog_kdk_tape_f32",
+    "odisseo_ensemble_leapfrog_kdk_vjp_f32",
 ]
 
 
@@ -108,6 +109,10 @@ def lib():
         L.odisseo_ensemble_workspace_bytes.restype = sz
         L.odisseo_ensemble_workspace_bytes.argtypes = [i64]
         L.odisseo_ensemble_leapfrog_kdk_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp]
+        L.odisseo_ensemble_tape_bytes.restype = sz
+        L.odisseo_ensemble_tape_bytes.argtypes = [i64, i64, i64]
+        L.odisseo_ensemble_leapfrog_kdk_tape_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp, sz, vp]
+        L.odisseo_ensemble_leapfrog_kdk_vjp_f32.argtypes = [vp, i64, i64, vp, i64, i64, vp, vp, vp, vp, vp, sz, vp]
         L.odisseo_launch_count.restype = i64
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
@@ -351,6 +356,58 @@ def diagnostics(posm: torch.Tensor, vel: torch.Tensor, G: float, eps: float, pot
 
 def ensemble_workspace_bytes(nsim: int) -> int:
     return int(lib().odisseo_ensemble_workspace_bytes(int(nsim)))
+
+
+def _sim_params(params):
+    arr = (SimParams * len(params))()
+    for k, (G, eps, dt, pot) in enumerate(params):
+        arr[k].G, arr[k].eps, arr[k].dt = float(G), float(eps), float(dt)
+        arr[k].pot = pot if pot is not None else Potential.make()
+    return arr
+
+
+def _ens_state(posm, vel, names="posm and vel"):
+    if posm.dim() != 3 or posm.shape[2] != 4 or posm.shape != vel.shape or not posm.is_contiguous() \
+            or not vel.is_contiguous() or posm.dtype != torch.float32 or vel.dtype != torch.float32:
+        raise ValueError("%s must be contiguous float32 [nsim, n, 4] tensors" % names)
+    if not (posm.is_cuda and vel.is_cuda):
+        raise ValueError("%s must be CUDA tensors (no CPU fallback)" % names)
+    return int(posm.shape[0]), int(posm.shape[1])
+
+
+def ensemble_tape_bytes(n: int, nsim: int, nsteps: int) -> int:
+    return int(lib().odisseo_ensemble_tape_bytes(int(n), int(nsim), int(nsteps)))
+
+
+def ensemble_leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, params, nsteps: int, tape: torch.Tensor,
+                               workspace: torch.Tensor, stream=None):
+    """ensemble_leapfrog_kdk that also records {posm, vel, total acc} per simulation and step into tape (float32)."""
+    nsim, n = _ens_state(posm, vel)
+    if tape.dtype != torch.float32 or not tape.is_cuda or not tape.is_contiguous():
+        raise ValueError("tape must be a contiguous float32 CUDA tensor")
+    arr = _sim_params(params)
+    _check(lib().odisseo_ensemble_leapfrog_kdk_tape_f32(posm.data_ptr(), vel.data_ptr(), n, nsim,
+                                                        ctypes.cast(arr, ctypes.c_void_p), len(params), int(nsteps),
+                                                        tape.data_ptr(), tape.numel() * 4, workspace.data_ptr(),
+                                                        workspace.numel(), _stream(stream)),
+           "ensemble_leapfrog_kdk_tape_f32")
+
+
+def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch.Tensor, lv: torch.Tensor,
+                              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, stream=None):
+    """Gradients of every simulation of a batch from its tape: lx, lv [nsim, n, 4] in/out; gm float64 [nsim, n];
+    gparams float64 [nsim, 8] (GRADIENT_FIELDS)."""
+    nsim, n = _ens_state(lx, lv, "lx and lv")
+    _f64vec(gm, "gm", nsim * n)
+    _f64vec(gparams, "gparams", nsim * 8)
+    if tape.dtype != torch.float32 or not tape.is_cuda or tape.numel() * 4 < ensemble_tape_bytes(n, nsim, nsteps):
+        raise ValueError("tape does not hold nsteps + 1 snapshots of every simulation")
+    arr = _sim_params(params)
+    _check(lib().odisseo_ensemble_leapfrog_kdk_vjp_f32(tape.data_ptr(), n, nsim, ctypes.cast(arr, ctypes.c_void_p),
+                                                       len(params), int(nsteps), lx.data_ptr(), lv.data_ptr(),
+                                                       gm.data_ptr(), gparams.data_ptr(), workspace.data_ptr(),
+                                                       workspace.numel(), _stream(stream)),
+           "ensemble_leapfrog_kdk_vjp_f32")
 
 
 def ensemble_leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, params, nsteps: int, workspace: torch.Tensor,

@@ -16,37 +16,17 @@
 // grid = (target blocks, source splits); per-tile sums in the state's precision, promoted to fp64 between
 // tiles; split rows and every block sum are combined in a fixed order (bit-reproducible, no atomics).
 // The O(N) parts (external potential, parameter sums) are evaluated in fp64 whatever the state precision.
-#include "odisseo_common.cuh"
-#include "ext_potential.cuh"
+#include "adjoint_terms.cuh"
 
 namespace odisseo {
 
 namespace {
 
-constexpr int VJP_THREADS = 256;
 constexpr int VJP_TILE = 128;
-constexpr int VJP_COMPS = 6;
 
 template <typename T> struct AVec4;
 template <> struct AVec4<float> { typedef float4 type; };
 template <> struct AVec4<double> { typedef double4 type; };
-
-__device__ __forceinline__ void inv_powers(float s, float& f, float& g)
-{
-    const float y = rsqrt_approx(s);
-    const float y2 = y * y;
-    f = y2 * y;
-    g = -3.0f * f * y2;
-}
-__device__ __forceinline__ void inv_powers(double s, double& f, double& g)
-{
-    const double y0 = rsqrt_approx_f64(s);
-    const double e = fma(-s, y0 * y0, 1.0);
-    const double y = y0 * fma(e, fma(0.375, e, 0.5), 1.0);       // s^-1/2 to fp64 rounding
-    const double y2 = y * y;
-    f = y2 * y;
-    g = -3.0 * f * y2;
-}
 
 // partial rows: partials[((split * VJP_COMPS + comp) * n_rows) + i], comp = gx, gy, gz, mass term, eps term, G term
 template <typename T, int IPT>
@@ -93,26 +73,8 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
             const V4 p = sp[j], c = sc[j];
 #pragma unroll
             for (int k = 0; k < IPT; ++k) {
-                const T dx = p.x - xi[k], dy = p.y - yi[k], dz = p.z - zi[k];
-                const T s = fma(dz, dz, fma(dy, dy, fma(dx, dx, eps2)));
-                T f, g;
-                inv_powers(s, f, g);
-                const T pj = fma(dz, c.z, fma(dy, c.y, dx * c.x));              // d . c_j
-                const T qi = fma(dz, czi[k], fma(dy, cyi[k], dx * cxi[k]));     // d . c_i
-                // u = m_i c_j - m_j c_i written as m_i (c_j - c_i) + (m_i - m_j) c_i: the difference of
-                // cotangents is taken first (exact for close values), and the self term is exactly 0
-                const T dm = mi[k] - p.w;
-                const T ux = fma(dm, cxi[k], mi[k] * (c.x - cxi[k]));
-                const T uy = fma(dm, cyi[k], mi[k] * (c.y - cyi[k]));
-                const T uz = fma(dm, czi[k], mi[k] * (c.z - czi[k]));
-                const T gdu = g * fma(dz, uz, fma(dy, uy, dx * ux));            // g (d . u)
-                ax[k] = fma(f, ux, fma(gdu, dx, ax[k]));
-                ay[k] = fma(f, uy, fma(gdu, dy, ay[k]));
-                az[k] = fma(f, uz, fma(gdu, dz, az[k]));
-                am[k] = fma(f, pj, am[k]);
-                const T mq = p.w * qi;                                           // m_j (d . c_i)
-                ae[k] = fma(g, mq, ae[k]);
-                ag[k] = fma(f, mq, ag[k]);
+                vjp_pair_term<T>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xi[k], yi[k], zi[k], mi[k], cxi[k], cyi[k], czi[k], eps2,
+                                 ax[k], ay[k], az[k], am[k], ae[k], ag[k]);
             }
         }
 #pragma unroll
@@ -128,71 +90,6 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
             double* row = partials + (size_t)blockIdx.y * VJP_COMPS * n_rows + i;
             row[0] = ox[k]; row[n_rows] = oy[k]; row[2 * n_rows] = oz[k]; row[3 * n_rows] = om[k]; row[4 * n_rows] = oe[k]; row[5 * n_rows] = og[k];
         }
-    }
-}
-
-// Fixed-shape sum over the block (xor-shuffle tree, then warp sums in order); valid in thread 0.
-__device__ __forceinline__ double vjp_block_sum(double v, double* warp_scratch)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) warp_scratch[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double s = 0.0;
-    if (threadIdx.x == 0)
-        for (int w = 0; w < VJP_THREADS / 32; ++w) s += warp_scratch[w];
-    return s;
-}
-
-// Cotangent c pulled back through a_NFW + a_MN at x, in fp64: h = (da/dx)^T c, and the terms of the
-// parameter sums t[0..5] = d(c.a)/d(M_s, r_s, M_d, a, b, G).
-__device__ __forceinline__ void ext_vjp(const PotParams<double>& pot, const double G, const double x, const double y,
-                                        const double z, const double cx, const double cy, const double cz,
-                                        double (&h)[3], double (&t)[6])
-{
-    h[0] = h[1] = h[2] = 0.0;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) t[k] = 0.0;
-    const double invG = G != 0.0 ? 1.0 / G : 0.0;
-    if (pot.GMs != 0.0) {
-        const double r2 = fma(x, x, fma(y, y, z * z));
-        if (r2 > 0.0) {
-            const double r = sqrt(r2), ir = 1.0 / r, ir3 = ir * ir * ir;
-            const double cc = r * pot.inv_rs, opc = 1.0 + cc;
-            const double mu = nfw_menc(cc);
-            const double dmu_dr = pot.inv_rs * cc / (opc * opc);
-            const double F = mu * ir3;
-            const double dF_over_r = (dmu_dr * ir3 - 3.0 * mu * ir3 * ir) * ir;
-            const double xc = fma(x, cx, fma(y, cy, z * cz));
-            const double k1 = -pot.GMs * F, k2 = -pot.GMs * dF_over_r * xc;
-            h[0] = fma(k1, cx, k2 * x); h[1] = fma(k1, cy, k2 * y); h[2] = fma(k1, cz, k2 * z);
-            const double ca = k1 * xc;                                   // c . a_NFW
-            t[0] += ca * (G * (1.0 / pot.GMs));                          // / M_s
-            t[5] += ca * invG;
-            const double dmu_drs = -cc * cc * pot.inv_rs / (opc * opc);
-            t[1] += -pot.GMs * dmu_drs * ir3 * xc;
-        }
-    }
-    if (pot.GMd != 0.0) {
-        const double b = sqrt(pot.b2);
-        const double B = sqrt(fma(z, z, pot.b2)), iB = 1.0 / B;
-        const double s = pot.a + B;
-        const double D2 = fma(x, x, fma(y, y, s * s));
-        const double iD = 1.0 / sqrt(D2), iD3 = iD * iD * iD, iD5 = iD3 * iD * iD;
-        const double kz = s * iB;                                        // a_z numerator is z kz
-        const double wz = z * kz;
-        const double dzk_dz = kz - pot.a * z * z * iB * iB * iB;         // d(z kz)/dz
-        const double cw = fma(cx, x, fma(cy, y, cz * wz));
-        const double q = -3.0 * cw * iD5;
-        h[0] += -pot.GMd * fma(q, x, cx * iD3);
-        h[1] += -pot.GMd * fma(q, y, cy * iD3);
-        h[2] += -pot.GMd * fma(q, wz, cz * dzk_dz * iD3);
-        const double ca = -pot.GMd * cw * iD3;                           // c . a_MN
-        t[2] += ca * (G * (1.0 / pot.GMd));
-        t[5] += ca * invG;
-        t[3] += -pot.GMd * fma(q, s, cz * z * iB * iD3);
-        t[4] += -pot.GMd * fma(q, s * b * iB, cz * z * (-pot.a * b * iB * iB * iB) * iD3);
     }
 }
 

@@ -1,0 +1,125 @@
+// Device building blocks of the reverse-mode derivative shared by adjoint.cu (one simulation, O(N^2) grid
+// kernel) and ensemble_adjoint.cu (one CTA per simulation).  Formulas: header of adjoint.cu.
+#pragma once
+
+#include "odisseo_common.cuh"
+#include "ext_potential.cuh"
+
+namespace odisseo {
+
+constexpr int VJP_THREADS = 256;
+constexpr int VJP_COMPS = 6;       // gx, gy, gz, mass term, eps term, G term
+
+__device__ __forceinline__ void inv_powers(float s, float& f, float& g)
+{
+    const float y = rsqrt_approx(s);
+    const float y2 = y * y;
+    f = y2 * y;
+    g = -3.0f * f * y2;
+}
+__device__ __forceinline__ void inv_powers(double s, double& f, double& g)
+{
+    const double y0 = rsqrt_approx_f64(s);
+    const double e = fma(-s, y0 * y0, 1.0);
+    const double y = y0 * fma(e, fma(0.375, e, 0.5), 1.0);       // s^-1/2 to fp64 rounding
+    const double y2 = y * y;
+    f = y2 * y;
+    g = -3.0 * f * y2;
+}
+
+// One source j against one target i: accumulates (J^T c)_i / G (ax, ay, az), -dL/dm_i / G (am),
+// dL/deps / (eps G) (ae) and dL/dG of the pair part (ag).
+template <typename T>
+__device__ __forceinline__ void vjp_pair_term(const T px, const T py, const T pz, const T pm, const T cjx, const T cjy,
+                                              const T cjz, const T xi, const T yi, const T zi, const T mi, const T cxi,
+                                              const T cyi, const T czi, const T eps2, T& ax, T& ay, T& az, T& am, T& ae,
+                                              T& ag)
+{
+    const T dx = px - xi, dy = py - yi, dz = pz - zi;
+    const T s = fma(dz, dz, fma(dy, dy, fma(dx, dx, eps2)));
+    T f, g;
+    inv_powers(s, f, g);
+    const T pj = fma(dz, cjz, fma(dy, cjy, dx * cjx));              // d . c_j
+    const T qi = fma(dz, czi, fma(dy, cyi, dx * cxi));     // d . c_i
+    // u = m_i c_j - m_j c_i written as m_i (c_j - c_i) + (m_i - m_j) c_i: the difference of
+    // cotangents is taken first (exact for close values), and the self term is exactly 0
+    const T dm = mi - pm;
+    const T ux = fma(dm, cxi, mi * (cjx - cxi));
+    const T uy = fma(dm, cyi, mi * (cjy - cyi));
+    const T uz = fma(dm, czi, mi * (cjz - czi));
+    const T gdu = g * fma(dz, uz, fma(dy, uy, dx * ux));            // g (d . u)
+    ax = fma(f, ux, fma(gdu, dx, ax));
+    ay = fma(f, uy, fma(gdu, dy, ay));
+    az = fma(f, uz, fma(gdu, dz, az));
+    am = fma(f, pj, am);
+    const T mq = pm * qi;                                           // m_j (d . c_i)
+    ae = fma(g, mq, ae);
+    ag = fma(f, mq, ag);
+}
+
+// Fixed-shape sum over the block (xor-shuffle tree, then warp sums in order); valid in thread 0.
+__device__ __forceinline__ double vjp_block_sum(double v, double* warp_scratch)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) warp_scratch[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < VJP_THREADS / 32; ++w) s += warp_scratch[w];
+    return s;
+}
+
+// Cotangent c pulled back through a_NFW + a_MN at x, in fp64: h = (da/dx)^T c, and the terms of the
+// parameter sums t[0..5] = d(c.a)/d(M_s, r_s, M_d, a, b, G).
+__device__ __forceinline__ void ext_vjp(const PotParams<double>& pot, const double G, const double x, const double y,
+                                        const double z, const double cx, const double cy, const double cz,
+                                        double (&h)[3], double (&t)[6])
+{
+    h[0] = h[1] = h[2] = 0.0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) t[k] = 0.0;
+    const double invG = G != 0.0 ? 1.0 / G : 0.0;
+    if (pot.GMs != 0.0) {
+        const double r2 = fma(x, x, fma(y, y, z * z));
+        if (r2 > 0.0) {
+            const double r = sqrt(r2), ir = 1.0 / r, ir3 = ir * ir * ir;
+            const double cc = r * pot.inv_rs, opc = 1.0 + cc;
+            const double mu = nfw_menc(cc);
+            const double dmu_dr = pot.inv_rs * cc / (opc * opc);
+            const double F = mu * ir3;
+            const double dF_over_r = (dmu_dr * ir3 - 3.0 * mu * ir3 * ir) * ir;
+            const double xc = fma(x, cx, fma(y, cy, z * cz));
+            const double k1 = -pot.GMs * F, k2 = -pot.GMs * dF_over_r * xc;
+            h[0] = fma(k1, cx, k2 * x); h[1] = fma(k1, cy, k2 * y); h[2] = fma(k1, cz, k2 * z);
+            const double ca = k1 * xc;                                   // c . a_NFW
+            t[0] += ca * (G * (1.0 / pot.GMs));                          // / M_s
+            t[5] += ca * invG;
+            const double dmu_drs = -cc * cc * pot.inv_rs / (opc * opc);
+            t[1] += -pot.GMs * dmu_drs * ir3 * xc;
+        }
+    }
+    if (pot.GMd != 0.0) {
+        const double b = sqrt(pot.b2);
+        const double B = sqrt(fma(z, z, pot.b2)), iB = 1.0 / B;
+        const double s = pot.a + B;
+        const double D2 = fma(x, x, fma(y, y, s * s));
+        const double iD = 1.0 / sqrt(D2), iD3 = iD * iD * iD, iD5 = iD3 * iD * iD;
+        const double kz = s * iB;                                        // a_z numerator is z kz
+        const double wz = z * kz;
+        const double dzk_dz = kz - pot.a * z * z * iB * iB * iB;         // d(z kz)/dz
+        const double cw = fma(cx, x, fma(cy, y, cz * wz));
+        const double q = -3.0 * cw * iD5;
+        h[0] += -pot.GMd * fma(q, x, cx * iD3);
+        h[1] += -pot.GMd * fma(q, y, cy * iD3);
+        h[2] += -pot.GMd * fma(q, wz, cz * dzk_dz * iD3);
+        const double ca = -pot.GMd * cw * iD3;                           // c . a_MN
+        t[2] += ca * (G * (1.0 / pot.GMd));
+        t[5] += ca * invG;
+        t[3] += -pot.GMd * fma(q, s, cz * z * iB * iD3);
+        t[4] += -pot.GMd * fma(q, s * b * iB, cz * z * (-pot.a * b * iB * iB * iB) * iD3);
+    }
+}
+
+}  // namespace odisseo

@@ -833,44 +833,117 @@ odisseo_status odisseo_diagnostics_f64(const double* d_posm, const double* d_vel
 size_t odisseo_ensemble_workspace_bytes(int64_t nsim)
 {
     if (nsim <= 0) return 0;
-    return (((size_t)nsim * sizeof(EnsembleParams)) + 255) & ~(size_t)255;
+    return (((size_t)nsim * (sizeof(EnsembleParams) + sizeof(EnsembleParams64))) + 511) & ~(size_t)255;
 }
 
-odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float* d_posm, float* d_vel, int64_t n, int64_t nsim,
-                                                 const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
-                                                 void* d_workspace, size_t workspace_bytes, void* stream)
+size_t odisseo_ensemble_tape_bytes(int64_t n, int64_t nsim, int64_t nsteps)
 {
-    if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
-    if (n == 0 || nsim == 0) return ODISSEO_OK;
-    if (!d_posm || !d_vel || !h_params || !d_workspace) return ODISSEO_ERR_NULL;
-    if (misaligned(d_posm, 16) || misaligned(d_vel, 16) || misaligned(d_workspace, 256)) return ODISSEO_ERR_ALIGN;
-    const size_t bytes = (size_t)nsim * n * 16;
-    if (overlap(d_posm, bytes, d_vel, bytes)) return ODISSEO_ERR_ARG;
-    if (nparams != 1 && nparams != nsim) return ODISSEO_ERR_ARG;
-    if (workspace_bytes < (size_t)nparams * sizeof(EnsembleParams)) return ODISSEO_ERR_WORKSPACE;
-    std::vector<EnsembleParams> dev_params((size_t)nparams);
+    if (n <= 0 || nsim <= 0 || nsteps < 0) return 0;
+    return (size_t)nsim * (size_t)(nsteps + 1) * 3 * (size_t)n * 16;
+}
+
+namespace {
+
+// Validates the host records and uploads them: float records at ws, double records behind them.
+odisseo_status ensemble_upload_params(const odisseo_sim_params* h_params, int64_t nparams, void* ws, size_t ws_bytes,
+                                      cudaStream_t s, const EnsembleParams** d32, const EnsembleParams64** d64)
+{
+    const size_t off64 = (((size_t)nparams * sizeof(EnsembleParams)) + 255) & ~(size_t)255;
+    if (ws_bytes < off64 + (size_t)nparams * sizeof(EnsembleParams64)) return ODISSEO_ERR_WORKSPACE;
+    std::vector<EnsembleParams> p32((size_t)nparams);
+    std::vector<EnsembleParams64> p64((size_t)nparams);
     for (int64_t k = 0; k < nparams; ++k) {
         const odisseo_sim_params& hp = h_params[k];
         const float G = (float)hp.G, eps = (float)hp.eps, dt = (float)hp.dt;
         odisseo_status st = check_pair_scalars<float>(G, eps);
         if (st != ODISSEO_OK) return st;
         if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
-        EnsembleParams& d = dev_params[(size_t)k];
+        EnsembleParams& d = p32[(size_t)k];
         st = make_pot<float>(G, &hp.pot, d.pot);
         if (st != ODISSEO_OK) return st;
         d.G = G; d.eps2 = eps * eps; d.dt = dt;
+        EnsembleParams64& q = p64[(size_t)k];            // the fp32-rounded scalars, as the forward kernel used them
+        st = make_pot<double>((double)G, &hp.pot, q.pot);
+        if (st != ODISSEO_OK) return st;
+        q.G = (double)G; q.eps = (double)eps; q.dt = (double)dt;
     }
+    unsigned char* base = static_cast<unsigned char*>(ws);
+    // pageable sources: the runtime stages them before returning, so the vectors may die with this frame
+    cudaError_t e = cudaMemcpyAsync(base, p32.data(), (size_t)nparams * sizeof(EnsembleParams), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(base + off64, p64.data(), (size_t)nparams * sizeof(EnsembleParams64), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *d32 = reinterpret_cast<const EnsembleParams*>(base);
+    *d64 = reinterpret_cast<const EnsembleParams64*>(base + off64);
+    return ODISSEO_OK;
+}
+
+odisseo_status ensemble_forward(float* d_posm, float* d_vel, int64_t n, int64_t nsim, const odisseo_sim_params* h_params,
+                                int64_t nparams, int64_t nsteps, float* d_tape, size_t tape_bytes, bool want_tape,
+                                void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
+    if (n == 0 || nsim == 0) return ODISSEO_OK;
+    if (!d_posm || !d_vel || !h_params || !d_workspace || (want_tape && !d_tape)) return ODISSEO_ERR_NULL;
+    if (misaligned(d_posm, 16) || misaligned(d_vel, 16) || misaligned(d_workspace, 256) || (want_tape && misaligned(d_tape, 16)))
+        return ODISSEO_ERR_ALIGN;
+    const size_t bytes = (size_t)nsim * n * 16;
+    if (overlap(d_posm, bytes, d_vel, bytes)) return ODISSEO_ERR_ARG;
+    if (nparams != 1 && nparams != nsim) return ODISSEO_ERR_ARG;
+    if (want_tape && tape_bytes < odisseo_ensemble_tape_bytes(n, nsim, nsteps)) return ODISSEO_ERR_WORKSPACE;
     DeviceInfo dev;
     odisseo_status st = device_info(dev);
     if (st != ODISSEO_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    // pageable source: the runtime stages it before returning, so dev_params may die with this frame
-    cudaError_t e = cudaMemcpyAsync(d_workspace, dev_params.data(), (size_t)nparams * sizeof(EnsembleParams),
-                                    cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(e);
+    const EnsembleParams* d32;
+    const EnsembleParams64* d64;
+    st = ensemble_upload_params(h_params, nparams, d_workspace, workspace_bytes, s, &d32, &d64);
+    if (st != ODISSEO_OK) return st;
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    e = launch_ensemble_f32(d_posm, d_vel, static_cast<const EnsembleParams*>(d_workspace), nparams == 1 ? 1 : 0,
-                            (int)n, nsim, nsteps, s);
+    cudaError_t e = launch_ensemble_f32(d_posm, d_vel, d32, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps,
+                                        want_tape ? d_tape : nullptr, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+}  // namespace
+
+odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float* d_posm, float* d_vel, int64_t n, int64_t nsim,
+                                                 const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
+                                                 void* d_workspace, size_t workspace_bytes, void* stream)
+{ return ensemble_forward(d_posm, d_vel, n, nsim, h_params, nparams, nsteps, nullptr, 0, false, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float* d_posm, float* d_vel, int64_t n, int64_t nsim,
+                                                      const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
+                                                      float* d_tape, size_t tape_bytes, void* d_workspace,
+                                                      size_t workspace_bytes, void* stream)
+{ return ensemble_forward(d_posm, d_vel, n, nsim, h_params, nparams, nsteps, d_tape, tape_bytes, true, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_t n, int64_t nsim,
+                                                     const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
+                                                     float* d_lx, float* d_lv, double* d_gm, double* d_gparams,
+                                                     void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
+    if (n == 0 || nsim == 0) return ODISSEO_OK;
+    if (!d_tape || !d_lx || !d_lv || !d_gm || !d_gparams || !h_params || !d_workspace) return ODISSEO_ERR_NULL;
+    if (misaligned(d_tape, 16) || misaligned(d_lx, 16) || misaligned(d_lv, 16) || misaligned(d_gm, 8) ||
+        misaligned(d_gparams, 8) || misaligned(d_workspace, 256))
+        return ODISSEO_ERR_ALIGN;
+    const size_t bytes = (size_t)nsim * n * 16;
+    if (overlap(d_lx, bytes, d_lv, bytes)) return ODISSEO_ERR_ARG;
+    if (nparams != 1 && nparams != nsim) return ODISSEO_ERR_ARG;
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const EnsembleParams* d32;
+    const EnsembleParams64* d64;
+    st = ensemble_upload_params(h_params, nparams, d_workspace, workspace_bytes, s, &d32, &d64);
+    if (st != ODISSEO_OK) return st;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = launch_ensemble_vjp_f32(d_tape, d64, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps, d_lx, d_lv, d_gm,
+                                            d_gparams, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }

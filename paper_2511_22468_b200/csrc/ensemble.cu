@@ -92,7 +92,7 @@ __device__ __forceinline__ void ens_pair(const ulonglong2* __restrict__ src, con
 template <int NPAIR>
 __global__ void __launch_bounds__(ENS_THREADS, NPAIR <= 2 ? 2 : 1)
 ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const EnsembleParams* __restrict__ params,
-                    const int shared_params, const int n, const int64_t nsteps)
+                    const int shared_params, const int n, const int64_t nsteps, float4* __restrict__ tape)
 {
     extern __shared__ __align__(16) unsigned char ens_smem[];
     float4* const stage4 = reinterpret_cast<float4*>(ens_smem);
@@ -171,10 +171,35 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
         }
     };
 
+    // optional tape for the reverse-mode derivative (ensemble_adjoint.cu): snapshot k of this simulation =
+    // {posm, vel, TOTAL acceleration} at the synchronised time t0 + k dt, (nsteps + 1) x 3 x n records
+    float4* const T0 = tape ? tape + (size_t)sim * (size_t)(nsteps + 1) * 3 * n : nullptr;
+    auto record = [&](const int64_t k) {
+        if (!T0) return;
+        float4* const S = T0 + (size_t)k * 3 * n;
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            float x[2], y[2], z[2], m[2], a[2], b[2], c[2], ga[2], gb[2], gc[2];
+            unpk(xi[p], x[0], x[1]); unpk(yi[p], y[0], y[1]); unpk(zi[p], z[0], z[1]); unpk(mi[p], m[0], m[1]);
+            unpk(vx[p], a[0], a[1]); unpk(vy[p], b[0], b[1]); unpk(vz[p], c[0], c[1]);
+            unpk(gx[p], ga[0], ga[1]); unpk(gy[p], gb[0], gb[1]); unpk(gz[p], gc[0], gc[1]);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int i = (2 * p + h) * ENS_THREADS + tid;
+                if (i < n) {
+                    S[i] = make_float4(x[h], y[h], z[h], m[h]);
+                    S[n + i] = make_float4(a[h], b[h], c[h], 0.0f);
+                    S[2 * n + i] = make_float4(ga[h], gb[h], gc[h], 0.0f);
+                }
+            }
+        }
+    };
+
     // ---- KDK: a <- a(x); repeat { v += a dt/2; x += v dt; a <- a(x); v += a dt/2 } ----
     const float hdt = 0.5f * prm.dt;
     const f32x2 h2 = pk(hdt, hdt), d2 = pk(prm.dt, prm.dt);
     accel();
+    record(0);
     for (int64_t s = 0; s < nsteps; ++s) {
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
@@ -186,6 +211,7 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
         for (int p = 0; p < NPAIR; ++p) {
             vx[p] = fma2(gx[p], h2, vx[p]); vy[p] = fma2(gy[p], h2, vy[p]); vz[p] = fma2(gz[p], h2, vz[p]);
         }
+        record(s + 1);
     }
 
 #pragma unroll
@@ -206,25 +232,26 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
 
 template <int NPAIR>
 cudaError_t launch_ens(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n, int64_t nsim,
-                       int64_t nsteps, cudaStream_t stream)
+                       int64_t nsteps, float* tape, cudaStream_t stream)
 {
     const size_t smem = (size_t)NPAIR * ENS_TILE * 32;
     cudaError_t e = cudaFuncSetAttribute(ensemble_kdk_kernel<NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     ensemble_kdk_kernel<NPAIR><<<(unsigned)nsim, ENS_THREADS, smem, stream>>>(
-        reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), params, shared_params, n, nsteps);
+        reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), params, shared_params, n, nsteps,
+        reinterpret_cast<float4*>(tape));
     return cudaGetLastError();
 }
 
 }  // namespace
 
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
-                                int64_t nsim, int64_t nsteps, cudaStream_t stream)
+                                int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream)
 {
-    if (n <= 1 * ENS_TILE) return launch_ens<1>(posm, vel, params, shared_params, n, nsim, nsteps, stream);
-    if (n <= 2 * ENS_TILE) return launch_ens<2>(posm, vel, params, shared_params, n, nsim, nsteps, stream);
-    if (n <= 3 * ENS_TILE) return launch_ens<3>(posm, vel, params, shared_params, n, nsim, nsteps, stream);
-    return launch_ens<4>(posm, vel, params, shared_params, n, nsim, nsteps, stream);
+    if (n <= 1 * ENS_TILE) return launch_ens<1>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    if (n <= 2 * ENS_TILE) return launch_ens<2>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    if (n <= 3 * ENS_TILE) return launch_ens<3>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    return launch_ens<4>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
 }
 
 }  // namespace odisseo

@@ -79,6 +79,11 @@ struct EnsembleParams {
     float G, eps2, dt;
     PotParams<float> pot;
 };
+// The same in double for the O(N) parts of the ensemble pull-back (ensemble_adjoint.cu), 64 bytes.
+struct EnsembleParams64 {
+    double G, eps, dt;
+    PotParams<double> pot;
+};
 constexpr int ENSEMBLE_MAX_N = 2048;
 
 // Step-kernel flags.
@@ -218,7 +223,10 @@ cudaError_t launch_vjp_pre_f32(const float* tape_k, const float* tape_k1, int64_
 cudaError_t launch_vjp_pre_f64(const double* tape_k, const double* tape_k1, int64_t n, const PotParams<double>& pot, double dt,
                                double w, int first, const double* lx, double* lv, double* cot, double* dt_sums, cudaStream_t stream);
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
-                                int64_t nsim, int64_t nsteps, cudaStream_t stream);
+                                int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream);
+cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
+                                    int64_t nsim, int64_t nsteps, float* lx, float* lv, double* gm, double* gparams,
+                                    cudaStream_t stream);
 cudaError_t configure_pair_f32();
 cudaError_t configure_pair_f64();
 

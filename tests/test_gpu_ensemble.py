@@ -125,3 +125,68 @@ def test_ensemble_zero_steps_many_simulations_and_argument_errors():
     big = torch.zeros(1, 2049, 4, device="cuda")
     with pytest.raises(B.OdisseoError, match="ERR_ARG"):
         B.ensemble_leapfrog_kdk(big, big.clone(), [(cfg.G, cfg.eps, cfg.dt, pot)], 1, ws)
+
+
+# ---------------------------------------------------------------------------------------------
+# reverse-mode derivative of the ensembles (oracle/adjoint.py, pinned by finite differences)
+# ---------------------------------------------------------------------------------------------
+def _run_vjp(posm, vel, bparams, nsteps, lx, lv):
+    nsim, n = posm.shape[:2]
+    dp, dv = torch.from_numpy(posm.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
+    tape = torch.empty(B.ensemble_tape_bytes(n, nsim, nsteps) // 4, dtype=torch.float32, device="cuda")
+    B.ensemble_leapfrog_kdk_tape(dp, dv, bparams, nsteps, tape, ws)
+    dlx, dlv = torch.from_numpy(lx.copy()).cuda(), torch.from_numpy(lv.copy()).cuda()
+    gm = torch.full((nsim, n), float("nan"), dtype=torch.float64, device="cuda")
+    gp = torch.full((nsim, 8), float("nan"), dtype=torch.float64, device="cuda")
+    B.ensemble_leapfrog_kdk_vjp(tape, bparams, nsteps, dlx, dlv, gm, gp, ws)
+    torch.cuda.synchronize()
+    return dp.cpu().numpy(), dv.cpu().numpy(), dlx.cpu().numpy(), dlv.cpu().numpy(), gm.cpu().numpy(), gp.cpu().numpy()
+
+
+@pytest.mark.parametrize("n,nsteps", [(1000, 5), (300, 3), (1, 2), (1300, 2), (2048, 1)])
+def test_ensemble_vjp_matches_the_oracle_adjoint_per_simulation(n, nsteps):
+    from oracle import adjoint as A
+    sims = [dict(seed=31, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0),
+            dict(seed=32, M=2.0e4, dt_scale=0.5, nfw_scale=0.7, mn_scale=1.3),
+            dict(seed=33, M=1.0e4, dt_scale=-1.0, nfw_scale=1.2, mn_scale=1.0, unequal=True)]
+    posm, vel, bparams, oparams = _make_batch(n, sims)
+    rng = np.random.Generator(np.random.PCG64(34))
+    lx = np.zeros((3, n, 4), dtype=np.float32)
+    lv = np.zeros((3, n, 4), dtype=np.float32)
+    lx[:, :, :3] = rng.normal(size=(3, n, 3))
+    lv[:, :, :3] = rng.normal(size=(3, n, 3)) * 10.0
+    pf, vf, gx0, gv0, gm, gp = _run_vjp(posm, vel, bparams, nsteps, lx, lv)
+    # the tape call leaves the same final state as the plain call
+    p_plain, v_plain = _run(posm, vel, bparams, nsteps)
+    assert pf.tobytes() == p_plain.tobytes() and vf.tobytes() == v_plain.tobytes()
+    cfg = W.CONFIGS[1]
+    for k, (G, eps, dt, _) in enumerate(oparams):
+        s = sims[k]
+        nfw = (cfg.nfw[0] * s["nfw_scale"], cfg.nfw[1])
+        mn = (cfg.mn[0] * s["mn_scale"], cfg.mn[1], cfg.mn[2])
+        ref = A.leapfrog_kdk_vjp(posm[k].astype(np.float64), vel[k, :, :3].astype(np.float64), G, eps, dt, nsteps,
+                                 lx[k, :, :3].astype(np.float64), lv[k, :, :3].astype(np.float64), nfw, mn)
+        # fp32 pull-back: 1e-3 of the largest component (measured ~3e-4 after 5 steps)
+        assert np.abs(gx0[k, :, :3] - ref["x0"]).max() <= 1e-3 * np.abs(ref["x0"]).max(), "sim %d x0" % k
+        assert np.abs(gv0[k, :, :3] - ref["v0"]).max() <= 1e-3 * np.abs(ref["v0"]).max(), "sim %d v0" % k
+        assert np.abs(gm[k] - ref["m"]).max() <= 1e-3 * max(np.abs(ref["m"]).max(), 1e-300), "sim %d m" % k
+        for name in ("M_s", "r_s", "M_d", "a", "b", "dt"):
+            kk = B.GRADIENT_FIELDS.index(name)
+            assert abs(gp[k, kk] - ref[name]) <= 1e-3 * abs(ref[name]), "sim %d %s" % (k, name)
+        assert np.all(gx0[k, :, 3] == 0) and np.all(gv0[k, :, 3] == 0)
+
+
+def test_ensemble_vjp_zero_steps_is_the_identity_and_is_reproducible():
+    sims = [dict(seed=41 + k, M=1.0e4, dt_scale=1.0, nfw_scale=1.0, mn_scale=1.0) for k in range(2)]
+    posm, vel, bparams, _ = _make_batch(500, sims)
+    lx = np.random.Generator(np.random.PCG64(1)).normal(size=(2, 500, 4)).astype(np.float32)
+    lv = np.random.Generator(np.random.PCG64(2)).normal(size=(2, 500, 4)).astype(np.float32)
+    lx[:, :, 3] = 0
+    lv[:, :, 3] = 0
+    _, _, gx0, gv0, gm, gp = _run_vjp(posm, vel, bparams, 0, lx, lv)
+    assert gx0.tobytes() == lx.tobytes() and gv0.tobytes() == lv.tobytes() and np.all(gm == 0) and np.all(gp == 0)
+    a = _run_vjp(posm, vel, bparams, 6, lx, lv)
+    b = _run_vjp(posm, vel, bparams, 6, lx, lv)
+    for x, y in zip(a, b):
+        assert x.tobytes() == y.tobytes()
