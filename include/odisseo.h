@@ -191,15 +191,19 @@ odisseo_status odisseo_diagnostics_f64(const double *d_posm, const double *d_vel
  *   d_lv = dL/dv_N ([n][4], in/out), returns in place dL/dx_0 and dL/dv_0, and
  *     d_gm [n] double  dL/dm_i        d_gparams [8] double: dL/d(M_s, r_s, M_d, a, b, G, eps, dt)
  *   (dt at fixed nsteps, i.e. t_end / nsteps; M_s, r_s, M_d, a, b as in odisseo_potential, disabled terms give 0).
- * O(N^2) pull-back per recorded step (~35 flops per pair), fixed-order sums (bit-reproducible), O(N) parts in
- * fp64.  Workspace: odisseo_vjp_workspace_bytes(n, is_f64), 256-byte aligned. */
+ * with_eps_G == 0 leaves the G and eps slots 0 and skips their terms in the O(N^2) loop (neither is in the
+ * paper's parameter vectors; ~15 % of the pull-back's instructions).
+ * O(N^2) pull-back per recorded step (29-41 instructions per pair), fixed-order sums (bit-reproducible), O(N)
+ * parts in fp64.  Workspace: odisseo_vjp_workspace_bytes(n, is_f64), 256-byte aligned. */
 size_t odisseo_vjp_workspace_bytes(int64_t n, int is_f64);
 size_t odisseo_tape_bytes(int64_t n, int64_t nsteps, int is_f64);
 odisseo_status odisseo_accel_vjp_f32(const float *d_posm, const float *d_cot, int64_t n, float G, float eps,
-                                     const odisseo_potential *pot, float *d_gx, double *d_gm, double *d_gparams,
+                                     const odisseo_potential *pot, int with_eps_G, float *d_gx, double *d_gm,
+                                     double *d_gparams,
                                      void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_accel_vjp_f64(const double *d_posm, const double *d_cot, int64_t n, double G, double eps,
-                                     const odisseo_potential *pot, double *d_gx, double *d_gm, double *d_gparams,
+                                     const odisseo_potential *pot, int with_eps_G, double *d_gx, double *d_gm,
+                                     double *d_gparams,
                                      void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_leapfrog_kdk_tape_f32(float *d_posm, float *d_vel, float *d_acc, int64_t n, float G, float eps,
                                              float dt, int64_t nsteps, const odisseo_potential *pot,
@@ -210,10 +214,10 @@ odisseo_status odisseo_leapfrog_kdk_tape_f64(double *d_posm, double *d_vel, doub
                                              double *d_tape, size_t tape_bytes,
                                              void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_leapfrog_kdk_vjp_f32(const float *d_tape, int64_t n, float G, float eps, float dt, int64_t nsteps,
-                                            const odisseo_potential *pot, float *d_lx, float *d_lv, double *d_gm,
+                                            const odisseo_potential *pot, int with_eps_G, float *d_lx, float *d_lv, double *d_gm,
                                             double *d_gparams, void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_leapfrog_kdk_vjp_f64(const double *d_tape, int64_t n, double G, double eps, double dt, int64_t nsteps,
-                                            const odisseo_potential *pot, double *d_lx, double *d_lv, double *d_gm,
+                                            const odisseo_potential *pot, int with_eps_G, double *d_lx, double *d_lv, double *d_gm,
                                             double *d_gparams, void *d_workspace, size_t workspace_bytes, void *stream);
 
 /* Batched small-N ensembles (the paper's inference workload: 10^4 grid points and
@@ -251,7 +255,7 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float *d_posm, float *d_ve
                                                       void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float *d_tape, int64_t n, int64_t nsim,
                                                      const odisseo_sim_params *h_params, int64_t nparams,
-                                                     int64_t nsteps, float *d_lx, float *d_lv, double *d_gm,
+                                                     int64_t nsteps, int with_eps_G, float *d_lx, float *d_lv, double *d_gm,
                                                      double *d_gparams, void *d_workspace, size_t workspace_bytes,
                                                      void *stream);
 

@@ -90,9 +90,9 @@ def lib():
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
-            getattr(L, "odisseo_accel_vjp_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, vp, sz, vp]
+            getattr(L, "odisseo_accel_vjp_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, ci, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_tape_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, sc, i64, vp, vp, sz, vp, sz, vp]
-            getattr(L, "odisseo_leapfrog_kdk_vjp_" + suffix).argtypes = [vp, i64, sc, sc, sc, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+            getattr(L, "odisseo_leapfrog_kdk_vjp_" + suffix).argtypes = [vp, i64, sc, sc, sc, i64, vp, ci, vp, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_diagnostics_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
@@ -112,7 +112,7 @@ def lib():
         L.odisseo_ensemble_tape_bytes.restype = sz
         L.odisseo_ensemble_tape_bytes.argtypes = [i64, i64, i64]
         L.odisseo_ensemble_leapfrog_kdk_tape_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp, sz, vp]
-        L.odisseo_ensemble_leapfrog_kdk_vjp_f32.argtypes = [vp, i64, i64, vp, i64, i64, vp, vp, vp, vp, vp, sz, vp]
+        L.odisseo_ensemble_leapfrog_kdk_vjp_f32.argtypes = [vp, i64, i64, vp, i64, i64, ci, vp, vp, vp, vp, vp, sz, vp]
         L.odisseo_launch_count.restype = i64
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
@@ -282,7 +282,7 @@ def _f64vec(t: torch.Tensor, name: str, numel: int):
 
 
 def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: Optional[Potential], gx: torch.Tensor,
-              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, stream=None):
+              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, with_eps_G: bool = False, stream=None):
     """Cotangent cot [n,4] pulled back through a = a_pair + a_ext (odisseo_accel_vjp_f32/_f64)."""
     n = _rec(posm, "posm")
     _rec(cot, "cot", n)
@@ -291,7 +291,8 @@ def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: 
     _f64vec(gparams, "gparams", 8)
     sfx = _suffix(posm)
     fn = getattr(lib(), "odisseo_accel_vjp_" + sfx)
-    _check(fn(posm.data_ptr(), cot.data_ptr(), n, G, eps, _pot(pot), gx.data_ptr(), gm.data_ptr(), gparams.data_ptr(),
+    _check(fn(posm.data_ptr(), cot.data_ptr(), n, G, eps, _pot(pot), int(bool(with_eps_G)), gx.data_ptr(), gm.data_ptr(),
+              gparams.data_ptr(),
               workspace.data_ptr(), workspace.numel(), _stream(stream)), "accel_vjp_" + sfx)
 
 
@@ -313,7 +314,7 @@ def leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, 
 
 def leapfrog_kdk_vjp(tape: torch.Tensor, n: int, G: float, eps: float, dt: float, nsteps: int, pot: Optional[Potential],
                      lx: torch.Tensor, lv: torch.Tensor, gm: torch.Tensor, gparams: torch.Tensor,
-                     workspace: torch.Tensor, stream=None):
+                     workspace: torch.Tensor, with_eps_G: bool = False, stream=None):
     """Reverse-mode derivative of nsteps KDK steps from the tape: lx, lv [n,4] hold dL/dx_N, dL/dv_N on entry and
     dL/dx_0, dL/dv_0 on exit; gm [n] and gparams [8] (GRADIENT_FIELDS) are float64 outputs."""
     _rec(lx, "lx", n)
@@ -324,7 +325,8 @@ def leapfrog_kdk_vjp(tape: torch.Tensor, n: int, G: float, eps: float, dt: float
     if tape.dtype != lx.dtype or not tape.is_cuda or tape.numel() < 12 * n * (nsteps + 1):
         raise ValueError("tape does not hold nsteps + 1 snapshots of the state's dtype")
     fn = getattr(lib(), "odisseo_leapfrog_kdk_vjp_" + sfx)
-    _check(fn(tape.data_ptr(), n, G, eps, dt, int(nsteps), _pot(pot), lx.data_ptr(), lv.data_ptr(), gm.data_ptr(),
+    _check(fn(tape.data_ptr(), n, G, eps, dt, int(nsteps), _pot(pot), int(bool(with_eps_G)), lx.data_ptr(), lv.data_ptr(),
+              gm.data_ptr(),
               gparams.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream(stream)), "leapfrog_kdk_vjp_" + sfx)
 
 
@@ -394,7 +396,8 @@ def ensemble_leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, params, ns
 
 
 def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch.Tensor, lv: torch.Tensor,
-                              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, stream=None):
+                              gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor,
+                              with_eps_G: bool = False, stream=None):
     """Gradients of every simulation of a batch from its tape: lx, lv [nsim, n, 4] in/out; gm float64 [nsim, n];
     gparams float64 [nsim, 8] (GRADIENT_FIELDS)."""
     nsim, n = _ens_state(lx, lv, "lx and lv")
@@ -404,8 +407,8 @@ def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch
         raise ValueError("tape does not hold nsteps + 1 snapshots of every simulation")
     arr = _sim_params(params)
     _check(lib().odisseo_ensemble_leapfrog_kdk_vjp_f32(tape.data_ptr(), n, nsim, ctypes.cast(arr, ctypes.c_void_p),
-                                                       len(params), int(nsteps), lx.data_ptr(), lv.data_ptr(),
-                                                       gm.data_ptr(), gparams.data_ptr(), workspace.data_ptr(),
+                                                       len(params), int(nsteps), int(bool(with_eps_G)), lx.data_ptr(),
+                                                       lv.data_ptr(), gm.data_ptr(), gparams.data_ptr(), workspace.data_ptr(),
                                                        workspace.numel(), _stream(stream)),
            "ensemble_leapfrog_kdk_vjp_f32")
 

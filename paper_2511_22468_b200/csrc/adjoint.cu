@@ -29,7 +29,7 @@ template <> struct AVec4<float> { typedef float4 type; };
 template <> struct AVec4<double> { typedef double4 type; };
 
 // partial rows: partials[((split * VJP_COMPS + comp) * n_rows) + i], comp = gx, gy, gz, mass term, eps term, G term
-template <typename T, int IPT>
+template <typename T, int IPT, bool EG>
 __global__ void __launch_bounds__(VJP_THREADS)
 pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename AVec4<T>::type* __restrict__ cot,
                 const int64_t n, const int64_t n_rows, const int64_t chunk, const T eps2, double* __restrict__ partials)
@@ -73,7 +73,7 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
             const V4 p = sp[j], c = sc[j];
 #pragma unroll
             for (int k = 0; k < IPT; ++k) {
-                vjp_pair_term<T>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xi[k], yi[k], zi[k], mi[k], cxi[k], cyi[k], czi[k], eps2,
+                vjp_pair_term<T, false, EG>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xi[k], yi[k], zi[k], mi[k], cxi[k], cyi[k], czi[k], eps2,
                                  ax[k], ay[k], az[k], am[k], ae[k], ag[k]);
             }
         }
@@ -101,7 +101,7 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
                   const double* __restrict__ partials, const int64_t n, const int64_t n_rows, const int nsplit,
                   const double G, const double eps, const PotParams<double> pot,
                   typename AVec4<T>::type* __restrict__ gx_out, double* __restrict__ gm_out, const int accumulate,
-                  double* __restrict__ block_sums)
+                  const int with_eps_G, double* __restrict__ block_sums)
 {
     typedef typename AVec4<T>::type V4;
     __shared__ double warp_scratch[VJP_THREADS / 32];
@@ -133,8 +133,10 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
         gm_out[i] = gm;
 #pragma unroll
         for (int k = 0; k < 5; ++k) term[k] = t[k];
-        term[5] = t[5] + r[5];                                          // d/dG: external + pair (sum_j m_j f d.c_i)
-        term[6] = eps * G * r[4];
+        if (with_eps_G) {
+            term[5] = t[5] + r[5];                                      // d/dG: external + pair (sum_j m_j f d.c_i)
+            term[6] = eps * G * r[4];
+        }
     }
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
@@ -237,7 +239,7 @@ size_t vjp_workspace_bytes(int64_t n, int is_f64, int num_sms)
 template <typename T>
 static cudaError_t accel_vjp_launch(const T* posm, const T* cot, int64_t n, double G, double eps,
                                     const PotParams<double>& pot, T* gx, double* gm, double* gparams, const double* dt_sums,
-                                    int accumulate, void* ws, int num_sms, cudaStream_t stream)
+                                    int accumulate, int with_eps_G, void* ws, int num_sms, cudaStream_t stream)
 {
     typedef typename AVec4<T>::type V4;
     int nsplit; int64_t chunk;
@@ -247,13 +249,17 @@ static cudaError_t accel_vjp_launch(const T* posm, const T* cot, int64_t n, doub
     double* block_sums = reinterpret_cast<double*>(static_cast<unsigned char*>(ws) + off);
     const unsigned blocks = vjp_grid(n);
     dim3 grid((unsigned)((n + VJP_THREADS * 2 - 1) / (VJP_THREADS * 2)), (unsigned)nsplit);
-    pair_vjp_kernel<T, 2><<<grid, VJP_THREADS, 0, stream>>>(reinterpret_cast<const V4*>(posm), reinterpret_cast<const V4*>(cot),
-                                                            n, n, chunk, (T)(eps * eps), partials);
+    if (with_eps_G)
+        pair_vjp_kernel<T, 2, true><<<grid, VJP_THREADS, 0, stream>>>(reinterpret_cast<const V4*>(posm), reinterpret_cast<const V4*>(cot),
+                                                                      n, n, chunk, (T)(eps * eps), partials);
+    else
+        pair_vjp_kernel<T, 2, false><<<grid, VJP_THREADS, 0, stream>>>(reinterpret_cast<const V4*>(posm), reinterpret_cast<const V4*>(cot),
+                                                                       n, n, chunk, (T)(eps * eps), partials);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     vjp_finish_kernel<T><<<blocks, VJP_THREADS, 0, stream>>>(reinterpret_cast<const V4*>(posm), reinterpret_cast<const V4*>(cot),
                                                              partials, n, n, nsplit, G, eps, pot, reinterpret_cast<V4*>(gx), gm,
-                                                             accumulate, block_sums);
+                                                             accumulate, with_eps_G, block_sums);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     vjp_final_kernel<<<1, VJP_THREADS, 0, stream>>>(block_sums, dt_sums, (int)blocks, gparams, accumulate);
@@ -261,13 +267,13 @@ static cudaError_t accel_vjp_launch(const T* posm, const T* cot, int64_t n, doub
 }
 
 cudaError_t launch_accel_vjp_f32(const float* posm, const float* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
-                                 int num_sms, cudaStream_t stream)
-{ return accel_vjp_launch<float>(posm, cot, n, G, eps, pot, gx, gm, gparams, dt_sums, accumulate, ws, num_sms, stream); }
+                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
+                                 void* ws, int num_sms, cudaStream_t stream)
+{ return accel_vjp_launch<float>(posm, cot, n, G, eps, pot, gx, gm, gparams, dt_sums, accumulate, with_eps_G, ws, num_sms, stream); }
 cudaError_t launch_accel_vjp_f64(const double* posm, const double* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
-                                 int num_sms, cudaStream_t stream)
-{ return accel_vjp_launch<double>(posm, cot, n, G, eps, pot, gx, gm, gparams, dt_sums, accumulate, ws, num_sms, stream); }
+                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
+                                 void* ws, int num_sms, cudaStream_t stream)
+{ return accel_vjp_launch<double>(posm, cot, n, G, eps, pot, gx, gm, gparams, dt_sums, accumulate, with_eps_G, ws, num_sms, stream); }
 
 // dt sums and cotangent array live behind the block sums in the workspace (vjp_workspace_bytes).
 void vjp_carve(void* ws, int64_t n, int num_sms, double** dt_sums, void** cot)

@@ -458,11 +458,11 @@ odisseo_status diagnostics_impl(const T* posm, const T* vel, int64_t n, T G, T e
 }
 
 inline cudaError_t launch_accel_vjp(const float* x, const float* c, int64_t n, double G, double eps, const PotParams<double>& pot, float* gx,
-                                    double* gm, double* gp, const double* dts, int accum, void* ws, int sms, cudaStream_t s)
-{ return launch_accel_vjp_f32(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, ws, sms, s); }
+                                    double* gm, double* gp, const double* dts, int accum, int eg, void* ws, int sms, cudaStream_t s)
+{ return launch_accel_vjp_f32(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, eg, ws, sms, s); }
 inline cudaError_t launch_accel_vjp(const double* x, const double* c, int64_t n, double G, double eps, const PotParams<double>& pot, double* gx,
-                                    double* gm, double* gp, const double* dts, int accum, void* ws, int sms, cudaStream_t s)
-{ return launch_accel_vjp_f64(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, ws, sms, s); }
+                                    double* gm, double* gp, const double* dts, int accum, int eg, void* ws, int sms, cudaStream_t s)
+{ return launch_accel_vjp_f64(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, eg, ws, sms, s); }
 inline cudaError_t launch_vjp_pre(const float* tk, const float* tk1, int64_t n, const PotParams<float>& pot, float dt, float w, int first,
                                   const float* lx, float* lv, float* cot, double* dts, cudaStream_t s)
 { return launch_vjp_pre_f32(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
@@ -471,8 +471,8 @@ inline cudaError_t launch_vjp_pre(const double* tk, const double* tk1, int64_t n
 { return launch_vjp_pre_f64(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
 
 template <typename T>
-odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps, const odisseo_potential* pot, T* gx,
-                              double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
+odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps, const odisseo_potential* pot, int with_eps_G,
+                              T* gx, double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
 {
     if (n < 0) return ODISSEO_ERR_ARG;
     if (!gparams) return ODISSEO_ERR_NULL;
@@ -497,7 +497,7 @@ odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps
     if (st != ODISSEO_OK) return st;
     if (ws_bytes < vjp_workspace_bytes(n, sizeof(T) == 8, dev.sms)) return ODISSEO_ERR_WORKSPACE;
     g_launches.fetch_add(3, std::memory_order_relaxed);
-    cudaError_t e = launch_accel_vjp(posm, cot, n, (double)G, (double)eps, pp, gx, gm, gparams, nullptr, 0, ws, dev.sms, s);
+    cudaError_t e = launch_accel_vjp(posm, cot, n, (double)G, (double)eps, pp, gx, gm, gparams, nullptr, 0, with_eps_G != 0, ws, dev.sms, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -529,7 +529,7 @@ odisseo_status leapfrog_tape_impl(T* posm, T* vel, T* acc, int64_t n, T G, T eps
 
 template <typename T>
 odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int64_t nsteps, const odisseo_potential* pot,
-                                 T* lx, T* lv, double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
+                                 int with_eps_G, T* lx, T* lv, double* gm, double* gparams, void* ws, size_t ws_bytes, void* stream)
 {
     if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
     if (!gparams) return ODISSEO_ERR_NULL;
@@ -572,7 +572,7 @@ odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int
         g_launches.fetch_add(4, std::memory_order_relaxed);
         e = launch_vjp_pre(tk, first ? (const T*)nullptr : tk + snap, n, pt, dt, w, first, lx, lv, cot, dt_sums, s);
         if (e != cudaSuccess) return cuda_fail(e);
-        e = launch_accel_vjp(tk, cot, n, (double)G, (double)eps, pd, lx, gm, gparams, dt_sums, 1, ws, dev.sms, s);
+        e = launch_accel_vjp(tk, cot, n, (double)G, (double)eps, pd, lx, gm, gparams, dt_sums, 1, with_eps_G != 0, ws, dev.sms, s);
         if (e != cudaSuccess) return cuda_fail(e);
     }
     return ODISSEO_OK;
@@ -790,13 +790,13 @@ size_t odisseo_tape_bytes(int64_t n, int64_t nsteps, int is_f64)
 }
 
 odisseo_status odisseo_accel_vjp_f32(const float* d_posm, const float* d_cot, int64_t n, float G, float eps,
-                                     const odisseo_potential* pot, float* d_gx, double* d_gm, double* d_gparams,
+                                     const odisseo_potential* pot, int with_eps_G, float* d_gx, double* d_gm, double* d_gparams,
                                      void* d_workspace, size_t workspace_bytes, void* stream)
-{ return accel_vjp_impl<float>(d_posm, d_cot, n, G, eps, pot, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+{ return accel_vjp_impl<float>(d_posm, d_cot, n, G, eps, pot, with_eps_G, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
 odisseo_status odisseo_accel_vjp_f64(const double* d_posm, const double* d_cot, int64_t n, double G, double eps,
-                                     const odisseo_potential* pot, double* d_gx, double* d_gm, double* d_gparams,
+                                     const odisseo_potential* pot, int with_eps_G, double* d_gx, double* d_gm, double* d_gparams,
                                      void* d_workspace, size_t workspace_bytes, void* stream)
-{ return accel_vjp_impl<double>(d_posm, d_cot, n, G, eps, pot, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+{ return accel_vjp_impl<double>(d_posm, d_cot, n, G, eps, pot, with_eps_G, d_gx, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
 odisseo_status odisseo_leapfrog_kdk_tape_f32(float* d_posm, float* d_vel, float* d_acc, int64_t n, float G, float eps, float dt,
                                              int64_t nsteps, const odisseo_potential* pot, float* d_tape, size_t tape_bytes,
                                              void* d_workspace, size_t workspace_bytes, void* stream)
@@ -806,13 +806,13 @@ odisseo_status odisseo_leapfrog_kdk_tape_f64(double* d_posm, double* d_vel, doub
                                              void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_tape_impl<double>(d_posm, d_vel, d_acc, n, G, eps, dt, nsteps, pot, d_tape, tape_bytes, d_workspace, workspace_bytes, stream); }
 odisseo_status odisseo_leapfrog_kdk_vjp_f32(const float* d_tape, int64_t n, float G, float eps, float dt, int64_t nsteps,
-                                            const odisseo_potential* pot, float* d_lx, float* d_lv, double* d_gm,
+                                            const odisseo_potential* pot, int with_eps_G, float* d_lx, float* d_lv, double* d_gm,
                                             double* d_gparams, void* d_workspace, size_t workspace_bytes, void* stream)
-{ return leapfrog_vjp_impl<float>(d_tape, n, G, eps, dt, nsteps, pot, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+{ return leapfrog_vjp_impl<float>(d_tape, n, G, eps, dt, nsteps, pot, with_eps_G, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
 odisseo_status odisseo_leapfrog_kdk_vjp_f64(const double* d_tape, int64_t n, double G, double eps, double dt, int64_t nsteps,
-                                            const odisseo_potential* pot, double* d_lx, double* d_lv, double* d_gm,
+                                            const odisseo_potential* pot, int with_eps_G, double* d_lx, double* d_lv, double* d_gm,
                                             double* d_gparams, void* d_workspace, size_t workspace_bytes, void* stream)
-{ return leapfrog_vjp_impl<double>(d_tape, n, G, eps, dt, nsteps, pot, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
+{ return leapfrog_vjp_impl<double>(d_tape, n, G, eps, dt, nsteps, pot, with_eps_G, d_lx, d_lv, d_gm, d_gparams, d_workspace, workspace_bytes, stream); }
 
 size_t odisseo_diagnostics_workspace_bytes(int64_t n)
 {
@@ -921,7 +921,7 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float* d_posm, float* d_ve
 
 odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_t n, int64_t nsim,
                                                      const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
-                                                     float* d_lx, float* d_lv, double* d_gm, double* d_gparams,
+                                                     int with_eps_G, float* d_lx, float* d_lv, double* d_gm, double* d_gparams,
                                                      void* d_workspace, size_t workspace_bytes, void* stream)
 {
     if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
@@ -942,7 +942,7 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_
     st = ensemble_upload_params(h_params, nparams, d_workspace, workspace_bytes, s, &d32, &d64);
     if (st != ODISSEO_OK) return st;
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    cudaError_t e = launch_ensemble_vjp_f32(d_tape, d64, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps, d_lx, d_lv, d_gm,
+    cudaError_t e = launch_ensemble_vjp_f32(d_tape, d64, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps, with_eps_G != 0, d_lx, d_lv, d_gm,
                                             d_gparams, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;

@@ -19,7 +19,7 @@ namespace {
 
 constexpr int EVJP_TILE = 512;
 
-template <int NQ>
+template <int NQ, bool EG>
 __global__ void __launch_bounds__(VJP_THREADS, NQ <= 2 ? 2 : 1)
 ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __restrict__ params, const int shared_params,
                     const int n, const int64_t nsteps, float4* __restrict__ lx, float4* __restrict__ lv,
@@ -54,6 +54,16 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
 #pragma unroll
     for (int k = 0; k < 8; ++k) gp[k] = 0.0;
 
+    // equal masses (checked once on snapshot 0; masses never change): the mass leaves the pair loop
+    int differs = 0;
+    const float mass0 = T0[0].w;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int i = q * VJP_THREADS + tid;
+        if (i < n) differs |= !(T0[i].w == mass0);
+    }
+    const bool eqm = __syncthreads_or(differs) == 0;
+
     for (int64_t k = nsteps; k >= 0 && nsteps > 0; --k) {
         const float4* const S = T0 + (size_t)k * 3 * n;
         const bool first = k == nsteps;
@@ -62,7 +72,9 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             const int i = q * VJP_THREADS + tid;
-            float4 p = make_float4(0.f, 0.f, 0.f, 0.f), v = p, a = p;     // slots beyond n: m = 0, c = 0
+            // slots beyond n: massless, zero cotangent, parked so far away that f and g underflow to exactly 0
+            // (the equal-mass loop does not multiply by m_j)
+            float4 p = make_float4(PAD_POS_F32, PAD_POS_F32, PAD_POS_F32, 0.f), v = make_float4(0.f, 0.f, 0.f, 0.f), a = v;
             if (i < n) { p = __ldcs(S + i); v = __ldcs(S + n + i); a = __ldcs(S + 2 * n + i); }
             if (!first) {
                 // dL/ddt terms and Lv_k = Lv_{k+1} + dt Lx_{k+1}   (vh_k = v_k + dt/2 a_k as in the forward kernel)
@@ -92,13 +104,26 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
 #pragma unroll
                 for (int c = 0; c < VJP_COMPS; ++c) t[q][c] = 0.f;
             const int j1 = j0 + EVJP_TILE < n_pad ? j0 + EVJP_TILE : n_pad;
+            if (eqm && !EG) {
 #pragma unroll 4
-            for (int j = j0; j < j1; ++j) {
-                const float4 p = sp[j], c = sc[j];
+                for (int j = j0; j < j1; ++j) {
+                    const float4 p = sp[j], c = sc[j];
 #pragma unroll
-                for (int q = 0; q < NQ; ++q)
-                    vjp_pair_term<float>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xs[q][0], xs[q][1], xs[q][2], xs[q][3], cs[q][0],
-                                         cs[q][1], cs[q][2], eps2, t[q][0], t[q][1], t[q][2], t[q][3], t[q][4], t[q][5]);
+                    for (int q = 0; q < NQ; ++q)
+                        vjp_pair_term<float, true, false>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xs[q][0], xs[q][1], xs[q][2], xs[q][3],
+                                                          cs[q][0], cs[q][1], cs[q][2], eps2, t[q][0], t[q][1], t[q][2], t[q][3],
+                                                          t[q][4], t[q][5]);
+                }
+            } else {
+#pragma unroll 4
+                for (int j = j0; j < j1; ++j) {
+                    const float4 p = sp[j], c = sc[j];
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q)
+                        vjp_pair_term<float, false, EG>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xs[q][0], xs[q][1], xs[q][2], xs[q][3],
+                                                        cs[q][0], cs[q][1], cs[q][2], eps2, t[q][0], t[q][1], t[q][2], t[q][3],
+                                                        t[q][4], t[q][5]);
+                }
             }
 #pragma unroll
             for (int q = 0; q < NQ; ++q)
@@ -112,14 +137,17 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
                 double h[3], t6[6];
                 ext_vjp(prm.pot, prm.G, (double)xs[q][0], (double)xs[q][1], (double)xs[q][2], (double)cs[q][0], (double)cs[q][1],
                         (double)cs[q][2], h, t6);
-                Lx[q][0] = (float)((double)Lx[q][0] + fma(prm.G, (double)o[q][0], h[0]));
-                Lx[q][1] = (float)((double)Lx[q][1] + fma(prm.G, (double)o[q][1], h[1]));
-                Lx[q][2] = (float)((double)Lx[q][2] + fma(prm.G, (double)o[q][2], h[2]));
+                const double gscale = (eqm && !EG) ? prm.G * (double)mass0 : prm.G;   // the equal-mass loop left m out
+                Lx[q][0] = (float)((double)Lx[q][0] + fma(gscale, (double)o[q][0], h[0]));
+                Lx[q][1] = (float)((double)Lx[q][1] + fma(gscale, (double)o[q][1], h[1]));
+                Lx[q][2] = (float)((double)Lx[q][2] + fma(gscale, (double)o[q][2], h[2]));
                 gm[q] += -prm.G * (double)o[q][3];
 #pragma unroll
                 for (int c = 0; c < 5; ++c) gp[c] += t6[c];
-                gp[5] += t6[5] + (double)o[q][5];
-                gp[6] += prm.eps * prm.G * (double)o[q][4];
+                if (EG) {
+                    gp[5] += t6[5] + (double)o[q][5];
+                    gp[6] += prm.eps * prm.G * (double)o[q][4];
+                }
             }
         }
     }
@@ -140,14 +168,14 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
     }
 }
 
-template <int NQ>
+template <int NQ, bool EG>
 cudaError_t launch_evjp(const float* tape, const EnsembleParams64* params, int shared_params, int n, int64_t nsim,
                         int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, cudaStream_t stream)
 {
     const size_t smem = (size_t)NQ * VJP_THREADS * 32;
-    cudaError_t e = cudaFuncSetAttribute(ensemble_vjp_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(ensemble_vjp_kernel<NQ, EG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ensemble_vjp_kernel<NQ><<<(unsigned)nsim, VJP_THREADS, smem, stream>>>(
+    ensemble_vjp_kernel<NQ, EG><<<(unsigned)nsim, VJP_THREADS, smem, stream>>>(
         reinterpret_cast<const float4*>(tape), params, shared_params, n, nsteps, reinterpret_cast<float4*>(lx),
         reinterpret_cast<float4*>(lv), gm, gparams);
     return cudaGetLastError();
@@ -155,20 +183,28 @@ cudaError_t launch_evjp(const float* tape, const EnsembleParams64* params, int s
 
 }  // namespace
 
-cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
-                                    int64_t nsim, int64_t nsteps, float* lx, float* lv, double* gm, double* gparams,
-                                    cudaStream_t stream)
+template <bool EG>
+static cudaError_t dispatch_evjp(const float* tape, const EnsembleParams64* params, int shared_params, int n, int64_t nsim,
+                                 int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, cudaStream_t stream)
 {
     switch ((n + VJP_THREADS - 1) / VJP_THREADS) {
-        case 1: return launch_evjp<1>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 2: return launch_evjp<2>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 3: return launch_evjp<3>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 4: return launch_evjp<4>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 5: return launch_evjp<5>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 6: return launch_evjp<6>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 7: return launch_evjp<7>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        default: return launch_evjp<8>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 1: return launch_evjp<1, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 2: return launch_evjp<2, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 3: return launch_evjp<3, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 4: return launch_evjp<4, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 5: return launch_evjp<5, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 6: return launch_evjp<6, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 7: return launch_evjp<7, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        default: return launch_evjp<8, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
     }
+}
+
+cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
+                                    int64_t nsim, int64_t nsteps, int with_eps_G, float* lx, float* lv, double* gm,
+                                    double* gparams, cudaStream_t stream)
+{
+    if (with_eps_G) return dispatch_evjp<true>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+    return dispatch_evjp<false>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
 }
 
 }  // namespace odisseo

@@ -213,11 +213,11 @@ void vjp_plan(int64_t n, int num_sms, int* nsplit, int64_t* chunk);
 size_t vjp_workspace_bytes(int64_t n, int is_f64, int num_sms);
 void vjp_carve(void* ws, int64_t n, int num_sms, double** dt_sums, void** cot);
 cudaError_t launch_accel_vjp_f32(const float* posm, const float* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
-                                 int num_sms, cudaStream_t stream);
+                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
+                                 void* ws, int num_sms, cudaStream_t stream);
 cudaError_t launch_accel_vjp_f64(const double* posm, const double* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, void* ws,
-                                 int num_sms, cudaStream_t stream);
+                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
+                                 void* ws, int num_sms, cudaStream_t stream);
 cudaError_t launch_vjp_pre_f32(const float* tape_k, const float* tape_k1, int64_t n, const PotParams<float>& pot, float dt, float w,
                                int first, const float* lx, float* lv, float* cot, double* dt_sums, cudaStream_t stream);
 cudaError_t launch_vjp_pre_f64(const double* tape_k, const double* tape_k1, int64_t n, const PotParams<double>& pot, double dt,
@@ -225,8 +225,8 @@ cudaError_t launch_vjp_pre_f64(const double* tape_k, const double* tape_k1, int6
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
                                 int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream);
 cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
-                                    int64_t nsim, int64_t nsteps, float* lx, float* lv, double* gm, double* gparams,
-                                    cudaStream_t stream);
+                                    int64_t nsim, int64_t nsteps, int with_eps_G, float* lx, float* lv, double* gm,
+                                    double* gparams, cudaStream_t stream);
 cudaError_t configure_pair_f32();
 cudaError_t configure_pair_f64();
 

@@ -24,13 +24,13 @@ def pad4(a, dtype):
     return out
 
 
-def gpu_accel_vjp(posm, c, G, eps, pot, dtype):
+def gpu_accel_vjp(posm, c, G, eps, pot, dtype, with_eps_G=True):
     n = posm.shape[0]
     gx = torch.full((n, 4), float("nan"), dtype=torch.float32 if dtype == np.float32 else torch.float64, device="cuda")
     gm = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
     gp = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
     ws = B.alloc_workspace(B.vjp_workspace_bytes(n, dtype == np.float64))
-    B.accel_vjp(dev(posm, dtype), dev(pad4(c, dtype), dtype), G, eps, pot, gx, gm, gp, ws)
+    B.accel_vjp(dev(posm, dtype), dev(pad4(c, dtype), dtype), G, eps, pot, gx, gm, gp, ws, with_eps_G=with_eps_G)
     torch.cuda.synchronize()
     return gx.cpu().numpy().astype(np.float64), gm.cpu().numpy(), gp.cpu().numpy()
 
@@ -65,6 +65,10 @@ def test_accel_vjp_matches_the_oracle(n, dtype, tol):
             scale = max(scale, abs(pG) if k == 5 else abs(peps))
         assert abs(gp[k] - r) <= 10 * tol * scale, NAMES[k]
     assert gp[7] == 0
+    # without the eps / G terms: same gradients, slots 5 and 6 left 0
+    gx2, gm2, gp2 = gpu_accel_vjp(p, c, G, eps, B.Potential.make(nfw=cfg.nfw, mn=cfg.mn), dtype, with_eps_G=False)
+    assert gx2.tobytes() == gx.tobytes() and gm2.tobytes() == gm.tobytes()
+    assert np.array_equal(gp2[:5], gp[:5]) and gp2[5] == 0 and gp2[6] == 0
 
 
 def test_accel_vjp_without_potential_and_reproducible():
@@ -88,7 +92,7 @@ def gpu_leapfrog_vjp(p, v, G, eps, dt, nsteps, pot, lx, lv, dtype):
     dlx, dlv = dev(pad4(lx, dtype), dtype), dev(pad4(lv, dtype), dtype)
     gm = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
     gp = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
-    B.leapfrog_kdk_vjp(tape, n, G, eps, dt, nsteps, pot, dlx, dlv, gm, gp, ws)
+    B.leapfrog_kdk_vjp(tape, n, G, eps, dt, nsteps, pot, dlx, dlv, gm, gp, ws, with_eps_G=True)
     torch.cuda.synchronize()
     final = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
     return dlx.cpu().numpy().astype(np.float64), dlv.cpu().numpy().astype(np.float64), gm.cpu().numpy(), gp.cpu().numpy(), final

@@ -130,7 +130,7 @@ def test_ensemble_zero_steps_many_simulations_and_argument_errors():
 # ---------------------------------------------------------------------------------------------
 # reverse-mode derivative of the ensembles (oracle/adjoint.py, pinned by finite differences)
 # ---------------------------------------------------------------------------------------------
-def _run_vjp(posm, vel, bparams, nsteps, lx, lv):
+def _run_vjp(posm, vel, bparams, nsteps, lx, lv, with_eps_G=False):
     nsim, n = posm.shape[:2]
     dp, dv = torch.from_numpy(posm.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
     ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
@@ -139,7 +139,7 @@ def _run_vjp(posm, vel, bparams, nsteps, lx, lv):
     dlx, dlv = torch.from_numpy(lx.copy()).cuda(), torch.from_numpy(lv.copy()).cuda()
     gm = torch.full((nsim, n), float("nan"), dtype=torch.float64, device="cuda")
     gp = torch.full((nsim, 8), float("nan"), dtype=torch.float64, device="cuda")
-    B.ensemble_leapfrog_kdk_vjp(tape, bparams, nsteps, dlx, dlv, gm, gp, ws)
+    B.ensemble_leapfrog_kdk_vjp(tape, bparams, nsteps, dlx, dlv, gm, gp, ws, with_eps_G=with_eps_G)
     torch.cuda.synchronize()
     return dp.cpu().numpy(), dv.cpu().numpy(), dlx.cpu().numpy(), dlv.cpu().numpy(), gm.cpu().numpy(), gp.cpu().numpy()
 
@@ -175,6 +175,17 @@ def test_ensemble_vjp_matches_the_oracle_adjoint_per_simulation(n, nsteps):
             kk = B.GRADIENT_FIELDS.index(name)
             assert abs(gp[k, kk] - ref[name]) <= 1e-3 * abs(ref[name]), "sim %d %s" % (k, name)
         assert np.all(gx0[k, :, 3] == 0) and np.all(gv0[k, :, 3] == 0)
+        assert gp[k, 5] == 0 and gp[k, 6] == 0                       # eps / G terms not requested
+    # with the eps and G terms (general loop for every simulation): same gradients to rounding, slots 5, 6 filled
+    _, _, gx1, gv1, gm1, gp1 = _run_vjp(posm, vel, bparams, nsteps, lx, lv, with_eps_G=True)
+    for k, (G, eps, dt, _) in enumerate(oparams):
+        s = sims[k]
+        ref = A.leapfrog_kdk_vjp(posm[k].astype(np.float64), vel[k, :, :3].astype(np.float64), G, eps, dt, nsteps,
+                                 lx[k, :, :3].astype(np.float64), lv[k, :, :3].astype(np.float64),
+                                 (cfg.nfw[0] * s["nfw_scale"], cfg.nfw[1]), (cfg.mn[0] * s["mn_scale"], cfg.mn[1], cfg.mn[2]))
+        assert np.abs(gx1[k, :, :3] - ref["x0"]).max() <= 1e-3 * np.abs(ref["x0"]).max()
+        assert abs(gp1[k, 5] - ref["G"]) <= 2e-3 * abs(ref["G"])
+        assert abs(gp1[k, 6] - ref["eps"]) <= 2e-2 * abs(ref["eps"]) + 1e-6 * abs(ref["dt"])
 
 
 def test_ensemble_vjp_zero_steps_is_the_identity_and_is_reproducible():
