@@ -22,7 +22,7 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     if (p.variant == 0) {
         // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
         // packed interaction chains of a thread (2 warps per scheduler x ILP 4 beats 4.5 warps x ILP 1:
-        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144, DESIGN.md section 10)
+        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144, DESIGN.md section 11)
         p.ipt = is_f64 ? 4 : 8;
         p.cthreads = 256;
         minb = 1;

@@ -8,7 +8,7 @@
 // remainder (35/16) e^3 ~ 2e-19: 7 FP64 ops for m (r2)^-3/2 instead of ~20 with the library rsqrt().
 // 16 FP64-pipe ops + 1 MUFU per interaction (3 DADD, 9 DFMA, 4 DMUL).  A DFMA holds a scheduler's
 // dispatch port 2 cycles and every other instruction 1, so F2F or integer conversions around an fp32
-// seed cost as much as the arithmetic they feed (DESIGN.md section 10).
+// seed cost as much as the arithmetic they feed (DESIGN.md section 11).
 // Sums are kept in fp64 registers for the whole segment (no tile flush needed).
 #include "odisseo_common.cuh"
 
