@@ -49,6 +49,8 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
             const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags)
 {
     typedef typename Vec4<T>::type V4;
+    pdl_launch_dependents();
+    pdl_wait();                                      // the pair kernel's rows (or the caller's state) are complete
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
     int mass_differs = 0;
@@ -175,30 +177,26 @@ cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
                             cudaStream_t stream)
 {
+    const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
+    typedef float4 V4;
     if (flags & STEP_FROM_PARTIALS)
-        step_kernel<float, true><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-            reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
-            partials, plan, G, pot, dt, flags);
-    else
-        step_kernel<float, false><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-            reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), reinterpret_cast<float4*>(acc), jsrc,
-            partials, plan, G, pot, dt, flags);
-    return cudaGetLastError();
+        return launch_pdl(step_kernel<float, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+    return launch_pdl(step_kernel<float, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
 }
 
 cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
                             cudaStream_t stream)
 {
+    const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
+    typedef double4 V4;
     if (flags & STEP_FROM_PARTIALS)
-        step_kernel<double, true><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-            reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
-            partials, plan, G, pot, dt, flags);
-    else
-        step_kernel<double, false><<<grid_for(plan_npad(plan)), STEP_THREADS, 0, stream>>>(
-            reinterpret_cast<double4*>(posm), reinterpret_cast<double4*>(vel), reinterpret_cast<double4*>(acc), jsrc,
-            partials, plan, G, pot, dt, flags);
-    return cudaGetLastError();
+        return launch_pdl(step_kernel<double, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+    return launch_pdl(step_kernel<double, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
 }
 
 cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,

@@ -169,6 +169,15 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+// Programmatic dependent launch (sm_90+): a kernel launched with launch_pdl() may become resident while
+// its predecessor in the stream is still running; pdl_wait() blocks until the predecessor has completed
+// and its writes are visible, so everything before it (barrier init, plan arithmetic) overlaps the
+// predecessor's tail and the launch latency.  pdl_launch_dependents() lets the NEXT kernel start that
+// early; it is issued first thing, which is safe because the dependent's pdl_wait() still waits for full
+// completion.  Both are no-ops when the kernel was launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Double-precision reciprocal-square-root seed (MUFU.RSQ64H): ~22 good bits, low word zero.
 __device__ __forceinline__ double rsqrt_approx_f64(double x) {
     double r;
@@ -176,6 +185,24 @@ __device__ __forceinline__ double rsqrt_approx_f64(double x) {
     return r;
 }
 #endif  // __CUDACC__
+
+#if defined(__CUDACC__)
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
 
 // launchers (defined in pair_f32.cu / pair_f64.cu / integrate.cu)
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials,

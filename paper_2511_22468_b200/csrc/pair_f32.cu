@@ -138,6 +138,7 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
     __shared__ __align__(8) uint64_t full_bar[STAGES];
     __shared__ __align__(8) uint64_t empty_bar[STAGES];
 
+    pdl_launch_dependents();
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
@@ -156,6 +157,7 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
         mbar_fence_init();
     }
     // equal-mass flags written by the staging kernel (odisseo_common.cuh): one uniform decision per grid
+    pdl_wait();                                             // the staging kernel's records and flags are complete
     int differs = 0;
     {
         const int* __restrict__ mflags = plan_flags(jsrc, plan);
@@ -194,9 +196,8 @@ cudaError_t launch_variant(const PairPlan& plan, const float* posm, const void* 
                            cudaStream_t stream)
 {
     const size_t smem = (size_t)STAGES * plan.T * 32 + (size_t)6 * NPAIR * CWARPS * 32 * sizeof(double);
-    pair_f32x2_kernel<NPAIR, CWARPS, MINB, JUNROLL><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
-        reinterpret_cast<const float4*>(posm), reinterpret_cast<const uint4*>(jsrc), partials, plan, eps * eps);
-    return cudaGetLastError();
+    return launch_pdl(pair_f32x2_kernel<NPAIR, CWARPS, MINB, JUNROLL>, dim3(plan.P), dim3((CWARPS + 1) * 32), smem, stream,
+                      reinterpret_cast<const float4*>(posm), reinterpret_cast<const uint4*>(jsrc), partials, plan, eps * eps);
 }
 
 }  // namespace

@@ -112,6 +112,7 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
     __shared__ __align__(8) uint64_t full_bar[STAGES];
     __shared__ __align__(8) uint64_t empty_bar[STAGES];
 
+    pdl_launch_dependents();
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
@@ -129,6 +130,7 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
         }
         mbar_fence_init();
     }
+    pdl_wait();                                             // the staging kernel's records and flags are complete
     int differs = 0;
     {
         const int* __restrict__ mflags = plan_flags(jsrc, plan);
@@ -166,9 +168,8 @@ cudaError_t launch_variant(const PairPlan& plan, const double* posm, const void*
                            cudaStream_t stream)
 {
     const size_t smem = (size_t)STAGES * plan.T * 32;
-    pair_f64_kernel<IPT, CWARPS, MINB, JUNROLL, POT><<<plan.P, (CWARPS + 1) * 32, smem, stream>>>(
-        reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(jsrc), partials, plan, eps * eps);
-    return cudaGetLastError();
+    return launch_pdl(pair_f64_kernel<IPT, CWARPS, MINB, JUNROLL, POT>, dim3(plan.P), dim3((CWARPS + 1) * 32), smem, stream,
+                      reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(jsrc), partials, plan, eps * eps);
 }
 
 }  // namespace
