@@ -122,7 +122,7 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
     if (u0 >= u1) return;
 
     const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
-    if (tid == 0) {
+    if (tid == CWARPS * 32) {                               // the producer lane owns init and the first loads
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(&full_bar[s], 1);
@@ -131,6 +131,18 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
         mbar_fence_init();
     }
     pdl_wait();                                             // the staging kernel's records and flags are complete
+    // the first STAGES tiles need no hand-over: issue them before anything else so that their latency
+    // overlaps the flag reduction and the target loads
+    const int prefetch = (int)((u1 - u0) < STAGES ? (u1 - u0) : STAGES);
+    if (tid == CWARPS * 32) {
+        int32_t t = (int32_t)(u0 % plan.J);
+        for (int s = 0; s < prefetch; ++s) {
+            mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
+            tma_load_1d(smem_raw + (size_t)s * tile_bytes,
+                        reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes, &full_bar[s]);
+            if (++t == plan.J) t = 0;
+        }
+    }
     int differs = 0;
     {
         const int* __restrict__ mflags = plan_flags(jsrc, plan);
@@ -141,10 +153,10 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
 
     if (warp == CWARPS) {
         if (lane == 0) {
-            int s = 0;
-            uint32_t ph = 0;
-            int32_t t = (int32_t)(u0 % plan.J);
-            for (int64_t u = u0; u < u1; ++u) {
+            int s = prefetch % STAGES;
+            uint32_t ph = prefetch == STAGES ? 1u : 0u;
+            int32_t t = (int32_t)((u0 + prefetch) % plan.J);
+            for (int64_t u = u0 + prefetch; u < u1; ++u) {
                 mbar_wait(&empty_bar[s], ph ^ 1u);
                 mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
                 tma_load_1d(smem_raw + (size_t)s * tile_bytes,
