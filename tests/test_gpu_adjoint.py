@@ -71,6 +71,25 @@ def test_accel_vjp_matches_the_oracle(n, dtype, tol):
     assert np.array_equal(gp2[:5], gp[:5]) and gp2[5] == 0 and gp2[6] == 0
 
 
+@pytest.mark.parametrize("n", [2, 128, 513, 3001])
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-10), (np.float32, 2e-5)])
+def test_accel_vjp_equal_masses_take_the_tile_wise_equal_mass_loop(n, dtype, tol):
+    """All masses equal: full tiles run the loop without the mass (decided per tile on the device); the padded
+    last tile and any tile with a different mass fall back to the general loop.  Same oracle, same tolerance."""
+    cfg, p, _, c, G, eps = _inputs(n, 650 + n, dtype, unequal=False)
+    gx, gm, gp = gpu_accel_vjp(p, c, G, eps, None, dtype, with_eps_G=False)
+    rx, rm, _, _ = A.pair_accel_vjp(p.astype(np.float64), c.astype(np.float64), G, eps)
+    assert np.abs(gx[:, :3] - rx).max() <= tol * np.abs(rx).max()
+    assert np.abs(gm - rm).max() <= tol * max(np.abs(rm).max(), 1e-300)
+    if n > 200:                                          # one odd mass in the middle: its tile goes general
+        p2 = p.copy()
+        p2[n // 2, 3] *= 3
+        gx2, gm2, _ = gpu_accel_vjp(p2, c, G, eps, None, dtype, with_eps_G=False)
+        rx2, rm2, _, _ = A.pair_accel_vjp(p2.astype(np.float64), c.astype(np.float64), G, eps)
+        assert np.abs(gx2[:, :3] - rx2).max() <= tol * np.abs(rx2).max()
+        assert np.abs(gm2 - rm2).max() <= tol * np.abs(rm2).max()
+
+
 def test_accel_vjp_without_potential_and_reproducible():
     cfg, p, _, c, G, eps = _inputs(2000, 77, np.float64)
     a = gpu_accel_vjp(p, c, G, eps, None, np.float64)
