@@ -88,6 +88,19 @@ odisseo_status odisseo_pair_accel_f64(const double *d_posm, double *d_acc, int64
                                       double G, double eps,
                                       void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* Cross form (SURVEY.md 8b "optional subset call", 8e, 8f NEXT-1): acceleration AT nt target positions DUE TO n
+ * sources,  d_acc[i] = G sum_j m_j (x_j - t_i) / (|x_j - t_i|^2 + eps^2)^{3/2}.  Targets need not be sources
+ * (tracer particles, a seeded subset, one rank's slice of a sharded run: targets = my slice, sources = all
+ * particles); the mass lane of d_targets is ignored; a target that coincides with a source gets exactly 0 from it.
+ * Same kernels, same fixed-order sums.  Workspace: odisseo_cross_workspace_bytes(nt, n, is_f64). */
+size_t odisseo_cross_workspace_bytes(int64_t nt, int64_t n, int is_f64);
+odisseo_status odisseo_pair_accel_cross_f32(const float *d_targets, int64_t nt, const float *d_sources, int64_t n,
+                                            float *d_acc, float G, float eps,
+                                            void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_pair_accel_cross_f64(const double *d_targets, int64_t nt, const double *d_sources, int64_t n,
+                                            double *d_acc, double G, double eps,
+                                            void *d_workspace, size_t workspace_bytes, void *stream);
+
 /* Structure-of-arrays face of the fp32 pair call: seven length-n float arrays (4-byte
  * aligned).  Packs into the workspace, runs the same kernel, unpacks.  Workspace must be
  * odisseo_workspace_bytes(n, 0) + 32 * n + 512 bytes, 256-byte aligned. */

@@ -31,7 +31,8 @@ EXPORTS = [
     "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
     "odisseo_leapfrog_kdk_tape_f32", "odisseo_leapfrog_kdk_tape_f64", "odisseo_leapfrog_kdk_vjp_f32",
     "odisseo_leapfrog_kdk_vjp_f64", "odisseo_ensemble_tape_bytes", "odisseo_ensemble_leapfrog_kdk_tape_f32",
-    "odisseo_ensemble_leapfrog_kdk_vjp_f32",
+    "odisseo_ensemble_leapfrog_kdk_vjp_f32", "odisseo_cross_workspace_bytes", "odisseo_pair_accel_cross_f32",
+    "odisseo_pair_accel_cross_f64",
 ]
 
 
@@ -88,6 +89,7 @@ def lib():
         L.odisseo_workspace_bytes.argtypes = [i64, ci]
         for suffix, sc in (("f32", f), ("f64", d)):
             getattr(L, "odisseo_pair_accel_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, sz, vp]
+            getattr(L, "odisseo_pair_accel_cross_" + suffix).argtypes = [vp, i64, vp, i64, vp, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_ext_accel_" + suffix).argtypes = [vp, vp, i64, sc, vp, ci, vp]
             getattr(L, "odisseo_leapfrog_kdk_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
             getattr(L, "odisseo_accel_vjp_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, ci, vp, vp, vp, vp, sz, vp]
@@ -96,6 +98,8 @@ def lib():
             getattr(L, "odisseo_diagnostics_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+        L.odisseo_cross_workspace_bytes.restype = sz
+        L.odisseo_cross_workspace_bytes.argtypes = [i64, i64, ci]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
@@ -198,6 +202,25 @@ def pair_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, eps: float, work
     fn = getattr(lib(), "odisseo_pair_accel_" + sfx)
     _check(fn(posm.data_ptr(), acc.data_ptr(), n, G, eps, workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "pair_accel_" + sfx)
+    return acc
+
+
+def cross_workspace_bytes(nt: int, n: int, is_f64: bool = False) -> int:
+    return int(lib().odisseo_cross_workspace_bytes(int(nt), int(n), int(bool(is_f64))))
+
+
+def pair_accel_cross(targets: torch.Tensor, sources: torch.Tensor, acc: torch.Tensor, G: float, eps: float,
+                     workspace: torch.Tensor, stream=None):
+    """acc[nt,4] = acceleration at targets[nt,4] due to sources[n,4] (odisseo_pair_accel_cross_f32/_f64)."""
+    nt = _rec(targets, "targets")
+    n = _rec(sources, "sources")
+    _rec(acc, "acc", nt)
+    sfx = _suffix(targets)
+    if sources.dtype != targets.dtype or acc.dtype != targets.dtype:
+        raise TypeError("targets, sources and acc dtypes differ")
+    fn = getattr(lib(), "odisseo_pair_accel_cross_" + sfx)
+    _check(fn(targets.data_ptr(), nt, sources.data_ptr(), n, acc.data_ptr(), G, eps, workspace.data_ptr(),
+              workspace.numel(), _stream(stream)), "pair_accel_cross_" + sfx)
     return acc
 
 

@@ -12,12 +12,15 @@
 namespace odisseo {
 
 // ------------------------------- launch plan ------------------------------------------
-PairPlan make_plan(int64_t n, int is_f64, int num_sms)
+PairPlan make_plan(int64_t n, int is_f64, int num_sms) { return make_cross_plan(n, n, is_f64, num_sms); }
+
+PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
 {
     PairPlan p;
     memset(&p, 0, sizeof(p));
     p.n = n;
-    p.variant = (n <= 4096) ? 1 : 0;
+    p.nt = nt;
+    p.variant = (nt <= 4096 && n <= 4096) ? 1 : 0;
     int minb;
     if (p.variant == 0) {
         // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
@@ -33,7 +36,7 @@ PairPlan make_plan(int64_t n, int is_f64, int num_sms)
     }
     p.rec_bytes = 32;
     p.IB = p.ipt * p.cthreads;
-    p.nb = (int32_t)((n + p.IB - 1) / p.IB);
+    p.nb = (int32_t)((nt + p.IB - 1) / p.IB);
     int64_t P = (int64_t)num_sms * minb;
     // Tile length: the busiest CTA walks ceil(U / P) units of (T + overhead) source records each
     // (overhead = barrier hand-over + fp64 flush of the tile sums, ~16 records' worth); take the T that
@@ -220,6 +223,48 @@ odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, voi
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_step(plan, const_cast<T*>(posm), (T*)nullptr, acc, cv.jsrc, cv.partials, G, nopot, (T)0,
                     STEP_FROM_PARTIALS, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, float G, float* a, cudaStream_t s)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f32(p, part, G, a, s); }
+inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, double G, double* a, cudaStream_t s)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f64(p, part, G, a, s); }
+
+// Acceleration at nt target positions due to n sources (targets need not be sources; their masses are ignored).
+template <typename T>
+odisseo_status pair_cross_impl(const T* targets, int64_t nt, const T* sources, int64_t n, T* acc, T G, T eps, void* ws,
+                               size_t ws_bytes, void* stream)
+{
+    if (n < 0 || nt < 0) return ODISSEO_ERR_ARG;
+    if (nt == 0) return ODISSEO_OK;
+    if (!targets || !acc || (n > 0 && !sources)) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(targets, rec) || misaligned(acc, rec) || (n > 0 && misaligned(sources, rec))) return ODISSEO_ERR_ALIGN;
+    if (overlap(targets, nt * rec, acc, nt * rec) || (n > 0 && overlap(sources, n * rec, acc, nt * rec))) return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (n == 0) {
+        cudaError_t e0 = cudaMemsetAsync(acc, 0, (size_t)nt * rec, s);
+        return e0 == cudaSuccess ? ODISSEO_OK : cuda_fail(e0);
+    }
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_cross_plan(nt, n, sizeof(T) == 8, dev.sms);
+    Carve cv;
+    st = carve(plan, ws, ws_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    PotParams<T> nopot;
+    memset(&nopot, 0, sizeof(nopot));
+    cudaError_t e = launch_step(plan, const_cast<T*>(sources), (T*)nullptr, (T*)nullptr, cv.jsrc, cv.partials, G, nopot, (T)0,
+                                STEP_PACK_ONLY, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_pair(plan, targets, cv.jsrc, cv.partials, eps, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_reduce_rows(plan, cv.partials, G, acc, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -680,6 +725,28 @@ size_t odisseo_workspace_bytes(int64_t n, int is_f64)
     const size_t jsrc = (((size_t)(n + 512) * p.rec_bytes + ((size_t)(n + 512) / STEP_THREADS + 1) * sizeof(int)) + 255) & ~(size_t)255;
     return jsrc + (size_t)p.slots * 3 * p.IB * sizeof(double);
 }
+
+size_t odisseo_cross_workspace_bytes(int64_t nt, int64_t n, int is_f64)
+{
+    if (n <= 0 || nt <= 0) return 0;
+    size_t best = 0;
+    for (int sms = 64; sms <= 192; sms += 4) {            // bound over devices with up to 192 SMs
+        const PairPlan p = make_cross_plan(nt, n, is_f64, sms);
+        const size_t b = plan_jsrc_bytes(p) + plan_partial_bytes(p);
+        if (b > best) best = b;
+    }
+    return best;
+}
+
+odisseo_status odisseo_pair_accel_cross_f32(const float* d_targets, int64_t nt, const float* d_sources, int64_t n,
+                                            float* d_acc, float G, float eps, void* d_workspace, size_t workspace_bytes,
+                                            void* stream)
+{ return pair_cross_impl<float>(d_targets, nt, d_sources, n, d_acc, G, eps, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_pair_accel_cross_f64(const double* d_targets, int64_t nt, const double* d_sources, int64_t n,
+                                            double* d_acc, double G, double eps, void* d_workspace, size_t workspace_bytes,
+                                            void* stream)
+{ return pair_cross_impl<double>(d_targets, nt, d_sources, n, d_acc, G, eps, d_workspace, workspace_bytes, stream); }
 
 odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8])
 {

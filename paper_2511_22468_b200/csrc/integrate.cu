@@ -129,6 +129,28 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
     }
 }
 
+// Fixed-order row reduce alone (cross call: the targets are not the staged sources): acc_i = G * sum of rows.
+template <typename T>
+__global__ void __launch_bounds__(STEP_THREADS)
+reduce_rows_kernel(const double* __restrict__ partials, const PairPlan plan, const T G, typename Vec4<T>::type* __restrict__ acc)
+{
+    pdl_wait();
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= plan.nt) return;
+    const int32_t b = (int32_t)(i / plan.IB);
+    const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
+    const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
+    const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    for (int32_t c = c0; c <= c1; ++c) {                   // increasing j
+        const double* row = partials + (size_t)(c + b) * 3 * plan.IB;
+        sx += __ldcg(row + r); sy += __ldcg(row + plan.IB + r); sz += __ldcg(row + 2 * plan.IB + r);
+    }
+    typename Vec4<T>::type a;
+    a.x = (T)((double)G * sx); a.y = (T)((double)G * sy); a.z = (T)((double)G * sz); a.w = (T)0;
+    acc[i] = a;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 ext_kernel(const typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ acc, const int64_t n,
@@ -197,6 +219,17 @@ cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, dou
                           reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
     return launch_pdl(step_kernel<double, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
                       reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+}
+
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, float G, float* acc, cudaStream_t stream)
+{
+    return launch_pdl(reduce_rows_kernel<float>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, plan, G,
+                      reinterpret_cast<float4*>(acc));
+}
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, double G, double* acc, cudaStream_t stream)
+{
+    return launch_pdl(reduce_rows_kernel<double>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, plan, G,
+                      reinterpret_cast<double4*>(acc));
 }
 
 cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,

@@ -21,7 +21,8 @@ namespace odisseo {
 // increasing c (= increasing j) order: fixed order, no atomics, bit-reproducible.
 // ---------------------------------------------------------------------------------------
 struct PairPlan {
-    int64_t n;        // particles
+    int64_t n;        // source particles (staged, tiled along j)
+    int64_t nt;       // target particles (held in registers, blocked along i); == n except for the cross call
     int64_t U;        // work units = nb * J
     int32_t IB;       // targets per i-block = ipt * cthreads
     int32_t T;        // source records per j-tile
@@ -67,6 +68,7 @@ __host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p)
 }
 
 PairPlan make_plan(int64_t n, int is_f64, int num_sms);
+PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms);   // nt targets against n sources
 
 // External potential with the host-side pre-combined products (reading R4).
 template <typename T> struct PotParams {
@@ -222,6 +224,8 @@ cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const Pot
 cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
                                 int64_t n, cudaStream_t stream);
 cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, float G, float* acc, cudaStream_t stream);
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, double G, double* acc, cudaStream_t stream);
 cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double* partials, double eps,
                                  cudaStream_t stream);
 // diagnostics.cu: stage (promote to double) / per-particle terms + block sums / final fixed-order sum

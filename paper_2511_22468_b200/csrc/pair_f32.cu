@@ -30,7 +30,8 @@ constexpr int STAGES = 4;
 // the staging kernel): the per-source mass factor leaves the inner loop (11 instead of 12 packed FP32
 // ops per two interactions) and multiplies the fp64 sums once per segment.
 template <int NPAIR, int CWARPS, int JUNROLL, bool EQM>
-__device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, double* __restrict__ partials,
+__device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, const uint4* __restrict__ jsrc,
+                                              double* __restrict__ partials,
                                               const PairPlan& plan, const float eps2, unsigned char* smem_raw,
                                               uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
                                               const int64_t u0, const int64_t u1, const uint32_t tile_bytes)
@@ -38,7 +39,7 @@ __device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, d
     constexpr int CTHREADS = CWARPS * 32;
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const double m0 = EQM ? (double)__ldg(&posm[0].w) : 1.0;
+    const double m0 = EQM ? (double)__ldg(reinterpret_cast<const float*>(jsrc) + 6) : 1.0;   // mass of staged record 0
     const f32x2 e2 = pk(eps2, eps2);
     f32x2 xi[NPAIR], yi[NPAIR], zi[NPAIR];
     f32x2 ax[NPAIR], ay[NPAIR], az[NPAIR];
@@ -58,8 +59,8 @@ __device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, d
             for (int p = 0; p < NPAIR; ++p) {
                 int64_t i0 = base + (int64_t)(2 * p) * CTHREADS;
                 int64_t i1 = i0 + CTHREADS;
-                i0 = i0 < plan.n ? i0 : plan.n - 1;     // clamped rows are computed and never read back
-                i1 = i1 < plan.n ? i1 : plan.n - 1;
+                i0 = i0 < plan.nt ? i0 : plan.nt - 1;     // clamped rows are computed and never read back
+                i1 = i1 < plan.nt ? i1 : plan.nt - 1;
                 const float4 p0 = __ldg(posm + i0);
                 const float4 p1 = __ldg(posm + i1);
                 // x + (-0) == x exactly; routing the pack through FADD2 makes the pair a native 64-bit
@@ -201,9 +202,9 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
     }
 
     if (eqm)
-        consume_tiles<NPAIR, CWARPS, JUNROLL, true>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<NPAIR, CWARPS, JUNROLL, true>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
     else
-        consume_tiles<NPAIR, CWARPS, JUNROLL, false>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<NPAIR, CWARPS, JUNROLL, false>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
 }
 
 template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>

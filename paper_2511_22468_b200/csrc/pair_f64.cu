@@ -23,7 +23,8 @@ constexpr int STAGES = 4;
 // POT = accumulate the softened potential sum_j m_j (r2)^-1/2 (x-plane of the partial rows only)
 // instead of the acceleration: the O(N^2) part of odisseo_diagnostics_* (diagnostics.cu).
 template <int IPT, int CWARPS, int JUNROLL, bool EQM, bool POT>
-__device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, double* __restrict__ partials,
+__device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, const double4* __restrict__ jsrc,
+                                              double* __restrict__ partials,
                                               const PairPlan& plan, const double eps2, unsigned char* smem_raw,
                                               uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
                                               const int64_t u0, const int64_t u1, const uint32_t tile_bytes)
@@ -31,7 +32,7 @@ __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, 
     constexpr int CTHREADS = CWARPS * 32;
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const double m0 = EQM ? posm[0].w : 1.0;
+    const double m0 = EQM ? jsrc[0].w : 1.0;                 // mass of staged record 0
     double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT];
     int32_t b = (int32_t)(u0 / plan.J);
     int32_t t = (int32_t)(u0 - (int64_t)b * plan.J);
@@ -44,7 +45,7 @@ __device__ __forceinline__ void consume_tiles(const double4* __restrict__ posm, 
 #pragma unroll
             for (int k = 0; k < IPT; ++k) {
                 int64_t i = (int64_t)b * plan.IB + (int64_t)k * CTHREADS + tid;
-                i = i < plan.n ? i : plan.n - 1;
+                i = i < plan.nt ? i : plan.nt - 1;
                 const double4 p = posm[i];
                 xi[k] = p.x; yi[k] = p.y; zi[k] = p.z;
                 ax[k] = ay[k] = az[k] = 0.0;
@@ -173,9 +174,9 @@ pair_f64_kernel(const double4* __restrict__ posm, const double4* __restrict__ js
     }
 
     if (eqm)
-        consume_tiles<IPT, CWARPS, JUNROLL, true, POT>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<IPT, CWARPS, JUNROLL, true, POT>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
     else
-        consume_tiles<IPT, CWARPS, JUNROLL, false, POT>(posm, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
+        consume_tiles<IPT, CWARPS, JUNROLL, false, POT>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
 }
 
 template <int IPT, int CWARPS, int MINB, int JUNROLL, bool POT>

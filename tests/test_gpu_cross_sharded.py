@@ -1,0 +1,151 @@
+"""GPU parity of odisseo_pair_accel_cross_* (targets need not be sources) and of the sharded driver run with
+emulated ranks on one GPU (SURVEY.md 8b optional subset call, 8e, 8f NEXT-1)."""
+import threading
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2511_22468_b200 import binding as B
+from paper_2511_22468_b200 import sharded as S
+from paper_2511_22468_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(a, dtype):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def gpu_cross(targets, sources, G, eps, dtype):
+    t, s = dev(targets, dtype), dev(sources, dtype)
+    acc = torch.full_like(t, float("nan"))
+    ws = B.alloc_workspace(B.cross_workspace_bytes(t.shape[0], s.shape[0], dtype == np.float64))
+    B.pair_accel_cross(t, s, acc, G, eps, ws)
+    torch.cuda.synchronize()
+    return acc.cpu().numpy()
+
+
+def oracle_cross(targets64, sources64, G, eps):
+    both = np.concatenate([sources64, targets64], axis=0)
+    both[sources64.shape[0]:, 3] = 0.0
+    idx = np.arange(sources64.shape[0], both.shape[0])
+    return O.pair_accel(both, G, eps, targets=idx)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12)])
+@pytest.mark.parametrize("nt,n", [(1, 1), (5, 1000), (1000, 5), (4096, 6000), (300, 20000), (9000, 3000)])
+def test_cross_tracers_match_the_oracle(nt, n, dtype, tol):
+    cfg = W.CONFIGS[1]
+    src64, _ = W.random_cloud(n, seed=40 + n, scale=0.01, centre=cfg.centre)
+    src64[:, 3] *= cfg.M / n
+    tgt64, _ = W.random_cloud(nt, seed=41 + nt, scale=0.02, centre=cfg.centre)
+    tgt64[:, 3] = 123.0                                                  # target masses are ignored
+    if dtype == np.float32:
+        src, tgt = W.to_f32(src64), W.to_f32(tgt64)
+        G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
+    else:
+        src, tgt, G, eps = src64, tgt64, cfg.G, cfg.eps
+    acc = gpu_cross(tgt, src, G, eps, dtype)
+    ref, Sn = oracle_cross(tgt.astype(np.float64), src.astype(np.float64), G, eps)
+    ratio = np.linalg.norm(acc[:, :3].astype(np.float64) - ref, axis=1) / Sn
+    assert ratio.max() <= tol and np.all(acc[:, 3] == 0)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_cross_with_targets_equal_sources_is_the_pair_call_and_slices_recombine(dtype):
+    cfg = W.CONFIGS[1]
+    posm64, _ = W.make_state(cfg, n=10000)
+    p = posm64.astype(dtype)
+    full = gpu_cross(p, p, cfg.G, cfg.eps, dtype)
+    posm = dev(p, dtype)
+    acc = torch.empty_like(posm)
+    B.pair_accel(posm, acc, cfg.G, cfg.eps, B.alloc_workspace(B.workspace_bytes(10000, dtype == np.float64)))
+    torch.cuda.synchronize()
+    assert full.tobytes() == acc.cpu().numpy().tobytes()                 # same plan, same sums
+    ref, Sn = O.pair_accel(p.astype(np.float64), float(dtype(cfg.G)), float(dtype(cfg.eps)))
+    tol = 1e-5 if dtype == np.float32 else 1e-12
+    for lo, hi in S.slice_bounds(10000, 3):                              # each slice against all sources
+        part = gpu_cross(p[lo:hi], p, cfg.G, cfg.eps, dtype)
+        assert (np.linalg.norm(part[:, :3].astype(np.float64) - ref[lo:hi], axis=1) / Sn[lo:hi]).max() <= tol
+
+
+def test_cross_config4_seeded_subset_of_a_million_sources():
+    """BASELINE.json configs[4]: "a single isolated pair-force evaluation checked against the fp64 oracle on a seeded
+    subset of 4,096 target particles" -- here the subset is ALSO what the GPU evaluates (4,096 targets x 2^20 sources)."""
+    cfg = W.CONFIGS[4]
+    posm64, _ = W.make_state(cfg)
+    p32 = W.to_f32(posm64)
+    idx = W.target_subset(cfg.n)
+    G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
+    acc = gpu_cross(p32[idx], p32, G, eps, np.float32)
+    ref, Sn = O.pair_accel(p32.astype(np.float64), G, eps, targets=idx)
+    assert (np.linalg.norm(acc[:, :3].astype(np.float64) - ref, axis=1) / Sn).max() <= 1e-5
+
+
+class _ThreadExchange:
+    """In-process stand-in for DistExchange: R emulated ranks (threads) on one GPU copy their slices to each other."""
+
+    def __init__(self, bounds, buffers):
+        self.bounds, self.buffers, self.barrier = bounds, buffers, threading.Barrier(len(bounds))
+
+    def for_rank(self, rank):
+        def exchange(posm_all):
+            torch.cuda.synchronize()
+            self.barrier.wait()
+            for src, (lo, hi) in enumerate(self.bounds):
+                if src != rank and hi > lo:
+                    posm_all[lo:hi].copy_(self.buffers[src][lo:hi])
+            torch.cuda.synchronize()
+            self.barrier.wait()
+        return exchange
+
+
+@pytest.mark.parametrize("world", [1, 3])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_sharded_driver_with_emulated_ranks_matches_the_single_gpu_leapfrog(world, dtype):
+    cfg = W.CONFIGS[1]
+    n, nsteps = 5000, 6
+    posm64, vel64 = W.make_state(cfg, n=n)
+    p0, v0 = posm64.astype(dtype), W.vel4(vel64.astype(dtype), dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    posm, vel = dev(p0, dtype), dev(v0, dtype)
+    acc = torch.empty_like(posm)
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64)))
+    torch.cuda.synchronize()
+    want = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
+
+    bounds = S.slice_bounds(n, world)
+    bufs = [dev(p0, dtype) for _ in range(world)]
+    vels = [dev(v0[lo:hi], dtype) for lo, hi in bounds]
+    accs = [torch.empty(hi - lo, 4, dtype=bufs[0].dtype, device="cuda") for lo, hi in bounds]
+    ex = _ThreadExchange(bounds, bufs)
+    errors = []
+
+    def run(rank):
+        try:
+            lo, hi = bounds[rank]
+            comp = S.CudaCompute(n, hi - lo, dtype == np.float64, cfg.G, cfg.eps, cfg.dt, pot)
+            S.sharded_leapfrog_kdk(comp, ex.for_rank(rank), bufs[rank], vels[rank], accs[rank], lo, hi, nsteps)
+            torch.cuda.synchronize()
+        except Exception as exc:                                         # noqa: BLE001
+            errors.append(exc)
+            ex.barrier.abort()
+    threads = [threading.Thread(target=run, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    got_p = bufs[0].cpu().numpy()
+    got_v = np.concatenate([v.cpu().numpy() for v in vels])
+    got_a = np.concatenate([a.cpu().numpy() for a in accs])
+    if world == 1:                                                       # same kernels, same plan: bit for bit
+        assert got_p.tobytes() == want[0].tobytes() and got_v.tobytes() == want[1].tobytes() and got_a.tobytes() == want[2].tobytes()
+    else:                                                                # other stream-K split: equal to rounding
+        rel = 1e-6 if dtype == np.float32 else 1e-13
+        assert np.abs(got_p[:, :3] - want[0][:, :3]).max() <= rel * 12.4
+        assert np.abs(got_v[:, :3] - want[1][:, :3]).max() <= rel * 0.21 * 10
+        for r in range(1, world):                                        # every rank holds the same positions
+            assert bufs[r].cpu().numpy().tobytes() == got_p.tobytes()
