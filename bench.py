@@ -348,6 +348,38 @@ def _ensemble_adjoint_rate(B, W, torch, n: int = 1000, nsim: int = 296, nsteps: 
             "sim_grad_steps_per_s": nsim * nsteps / ((best[0] + best[1]) * 1e-3), "gpu_launches": 2}
 
 
+def _sharded_projection(B, W, torch, ci: int = 3):
+    """Per-rank pair time of the target-sharded form (sharded.py) for R = 1, 2, 4, 8 ranks, measured on ONE GPU as
+    cross(slice of N/R targets, all N sources): what each of R GPUs would compute per KDK step.  The exchange (16 N
+    bytes per step over NVLink) is not included; nothing here ran on more than one GPU."""
+    from paper_2511_22468_b200 import sharded as S
+    cfg = W.CONFIGS[ci]
+    posm64, _ = W.make_state(cfg)
+    posm = torch.from_numpy(W.to_f32(posm64)).cuda()
+    G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
+    out = []
+    for R in (1, 2, 4, 8):
+        lo, hi = S.slice_bounds(cfg.n, R)[R - 1]
+        tgt = posm[lo:hi].contiguous()
+        acc = torch.empty_like(tgt)
+        ws = B.alloc_workspace(B.cross_workspace_bytes(hi - lo, cfg.n))
+        for _ in range(2):
+            B.pair_accel_cross(tgt, posm, acc, G, eps, ws)
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            B.pair_accel_cross(tgt, posm, acc, G, eps, ws)
+            b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        out.append({"ranks": R, "targets_per_rank": hi - lo, "pair_ms_per_rank": min(ts)})
+    for o in out:
+        o["compute_speedup_vs_1"] = out[0]["pair_ms_per_rank"] / o["pair_ms_per_rank"]
+    return {"workload": cfg.name, "exchange_bytes_per_step": 16 * cfg.n, "measured_on_gpus": 1, "ranks": out}
+
+
 def run_ours(args, rank: int, world: int, dist):
     import torch
     from paper_2511_22468_b200 import binding as B        # raises when the CUDA library is missing
@@ -469,6 +501,7 @@ def run_ours(args, rank: int, world: int, dist):
         line["ensemble"] = _ensemble_rate(B, W, torch)
         line["adjoint"] = _adjoint_rate(B, W, torch)
         line["ensemble_adjoint"] = _ensemble_adjoint_rate(B, W, torch)
+        line["sharded_projection"] = _sharded_projection(B, W, torch)
     print(json.dumps(line), flush=True)
 
 
