@@ -121,3 +121,32 @@ def test_diagnostics_full_size_config3_against_sampled_oracle_potential():
         assert abs(phi[i] - ref) <= 1e-12 * abs(ref)
     assert abs(out[0] - O.kinetic_energy(p64, v32.astype(np.float64))) <= 1e-12 * out[0]
     assert abs(out[2] - O.ext_potential_energy(p64, G, O.Potential.make(nfw=cfg.nfw, mn=cfg.mn))) <= 1e-12 * abs(out[2])
+
+
+@pytest.mark.parametrize("ci,nsteps", [(1, 1000), (2, 600)])
+def test_full_length_fp32_runs_keep_the_invariants(ci, nsteps):
+    """SURVEY.md 8c (v) at BASELINE.json's sizes and step counts (config 1 in full: 1,000 steps; config 2: the first
+    600 of 3,000): the fp32 GPU trajectory conserves L_z (exact for KDK in an axisymmetric potential), keeps the energy
+    error bounded, and the cluster's centre of mass follows the single-particle orbit the oracle integrates from the same
+    start (PAPER.md:L43 steps 2-3).  Measured: |dLz/Lz| ~ 1e-8, |dE/E| <= 2.5e-5, CoM offset <= 0.02 kpc."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg)
+    posm = torch.from_numpy(W.to_f32(posm64)).cuda()
+    vel = torch.from_numpy(W.vel4(W.to_f32(vel64), np.float32)).cuda()
+    acc = torch.empty_like(posm)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    ws = B.alloc_workspace(B.workspace_bytes(cfg.n))
+    wd = B.alloc_workspace(B.diagnostics_workspace_bytes(cfg.n))
+    d0 = torch.empty(16, dtype=torch.float64, device="cuda")
+    d1 = torch.empty(16, dtype=torch.float64, device="cuda")
+    B.diagnostics(posm, vel, cfg.G, cfg.eps, pot, d0, wd)
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, ws)
+    B.diagnostics(posm, vel, cfg.G, cfg.eps, pot, d1, wd)
+    torch.cuda.synchronize()
+    d0, d1 = d0.cpu().numpy(), d1.cpu().numpy()
+    assert abs(d1[8] - d0[8]) <= 1e-6 * abs(d0[8])                        # L_z
+    assert abs(d1[13] - d0[13]) <= 1e-4 * abs(d0[13])                     # total energy
+    assert d1[12] == d0[12]                                               # masses untouched
+    one, _, _ = O.leapfrog_kdk(np.array([[*cfg.centre, cfg.M]]), np.array([cfg.velocity]), cfg.G, cfg.eps, cfg.dt,
+                               nsteps, O.Potential.make(nfw=cfg.nfw, mn=cfg.mn))
+    assert np.linalg.norm(d1[9:12] - one[0, :3]) <= 0.05                  # kpc, on a ~12 kpc orbit
