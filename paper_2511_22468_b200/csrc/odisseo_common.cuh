@@ -11,8 +11,8 @@
 namespace odisseo {
 
 // ---------------------------------------------------------------------------------------
-// Launch plan.  The N x N interaction matrix is cut into
-// nb = ceil(n / IB) i-blocks (IB targets held in registers by one CTA) times
+// Launch plan.  The nt x n interaction matrix (nt = n except for the cross
+// call) is cut into nb = ceil(nt / IB) i-blocks (IB targets held in registers by one CTA) times
 // J = ceil(n / T) j-tiles (T source records staged through shared memory per TMA copy).
 // The U = nb * J units are numbered u = b * J + t and dealt to P persistent CTAs in
 // contiguous, equal (+-1) ranges: CTA c owns [start(c), start(c+1)), start(c) = floor(c*U/P).

@@ -3,7 +3,9 @@
 //   partial_i = sum_{j in segment} m_j (x_j - x_i) (|x_j - x_i|^2 + eps^2)^{-3/2}      (G applied in the reduce step)
 //
 // Design (B200-first, not the paper's XLA broadcast):
-//   * persistent grid, P = SMs x resident CTAs, stream-K split of the (i-block x j-tile) space
+//   * persistent grid, one 9-warp CTA per SM (8 compute warps + 1 producer warp, ~160 registers per
+//     thread so that ptxas interleaves a thread's four interaction chains), stream-K split of the
+//     (i-block x j-tile) space
 //     (odisseo_common.cuh) -> every SM busy for any N, no wave-quantisation tail;
 //   * source tiles arrive by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx) issued by
 //     a dedicated producer warp into a STAGES-deep ring; consumers release a stage with one
@@ -12,12 +14,13 @@
 //     staged pre-duplicated {x,x,y,y},{z,z,m,m} so that one LDS.128 yields two ready packed
 //     operands and the body is 3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per TWO interactions
 //     (half the issue slots of the scalar form, no register-pair MOVs);
-//   * two-level summation: fp32 inside one tile (<= 256 terms), promoted to fp64 between tiles
+//   * two-level summation: fp32 inside one tile (<= 512 terms), promoted to fp64 between tiles
 //     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18);
 //   * the self term contributes exactly 0 because eps > 0; padding records are massless and parked at
 //     3e18, where the inverse cube underflows to exactly 0 (ftz), so they vanish on both paths;
 //   * equal masses (the paper's Plummer progenitors, PAPER.md:L43 step 3) are detected on the device by
-//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2.
+//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2;
+//   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
 #include "odisseo_common.cuh"
 
 namespace odisseo {
