@@ -3,4 +3,4 @@
 ``workloads`` (seeded input generators) imports no native code; the CUDA library is
 loaded on first use of ``binding`` and fails loudly when it is missing.
 """
-__all__ = ["workloads", "binding"]
+__all__ = ["workloads", "binding", "sharded", "autograd"]

@@ -1,0 +1,104 @@
+"""torch.autograd faces of the differentiable leapfrog: plumbing around the C ABI, no arithmetic of the method.
+
+The paper's users write a loss of the final particle state and ask JAX for its gradient with respect to the
+potential parameters, the integration time, the masses and the initial conditions (PAPER.md:L15, L21, L43
+step 5, L63).  With these two Functions the same workflow runs on the CUDA library:
+
+    xf, vf = leapfrog_kdk(posm0, vel0, theta, dt, G, eps, nsteps)      # theta = (M_s, r_s, M_d, a, b)
+    loss(xf, vf).backward()                                           # posm0.grad[:, 3] is dL/dm_i, theta.grad, dt.grad
+
+forward  = odisseo_leapfrog_kdk_tape_*           (records the state tape)
+backward = odisseo_leapfrog_kdk_vjp_*            (walks it backwards; csrc/adjoint.cu)
+and the ensemble pair odisseo_ensemble_leapfrog_kdk_tape_f32 / _vjp_f32 for batches of small simulations.
+Inputs are never modified; the tape lives until backward has run (or the graph is freed).
+"""
+from __future__ import annotations
+
+import torch
+
+from . import binding as B
+
+
+def _potential(theta) -> B.Potential:
+    t = [float(x) for x in theta.detach().cpu().tolist()]
+    return B.Potential.make(nfw=(t[0], t[1]), mn=(t[2], t[3], t[4]))
+
+
+class _LeapfrogKDK(torch.autograd.Function):
+    @staticmethod
+    def forward(ctx, posm0, vel0, theta, dt, G, eps, nsteps):
+        n = posm0.shape[0]
+        f64 = posm0.dtype == torch.float64
+        posm, vel = posm0.detach().clone().contiguous(), vel0.detach().clone().contiguous()
+        acc = torch.empty_like(posm)
+        ws = B.alloc_workspace(max(B.workspace_bytes(n, f64), B.vjp_workspace_bytes(n, f64)))
+        tape = torch.empty(B.tape_bytes(n, nsteps, f64) // posm.element_size(), dtype=posm.dtype, device=posm.device)
+        pot = _potential(theta)
+        B.leapfrog_kdk_tape(posm, vel, acc, float(G), float(eps), float(dt), int(nsteps), pot, tape, ws)
+        ctx.save_for_backward(tape, theta, dt)
+        ctx.meta = (n, float(G), float(eps), int(nsteps), ws)
+        return posm, vel
+
+    @staticmethod
+    def backward(ctx, g_posm, g_vel):
+        tape, theta, dt = ctx.saved_tensors
+        n, G, eps, nsteps, ws = ctx.meta
+        lx = g_posm.detach().clone().contiguous()
+        lv = g_vel.detach().clone().contiguous()
+        g_mass_final = lx[:, 3].clone()                    # the final mass lane IS the initial mass lane
+        lx[:, 3] = 0
+        lv[:, 3] = 0
+        gm = torch.empty(n, dtype=torch.float64, device=lx.device)
+        gp = torch.empty(8, dtype=torch.float64, device=lx.device)
+        B.leapfrog_kdk_vjp(tape, n, G, eps, float(dt), nsteps, _potential(theta), lx, lv, gm, gp, ws)
+        g_posm0 = lx
+        g_posm0[:, 3] = gm.to(lx.dtype) + g_mass_final
+        g_theta = gp[:5].to(theta.dtype).to(theta.device)
+        g_dt = gp[7].to(dt.dtype).to(dt.device).reshape(dt.shape)
+        return g_posm0, lv, g_theta, g_dt, None, None, None
+
+
+def leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.Tensor, dt: torch.Tensor, G: float, eps: float,
+                 nsteps: int):
+    """Differentiable nsteps KDK steps.  posm0, vel0: CUDA [n, 4] (float32 or float64); theta: 5 values
+    (M_s, r_s, M_d, a, b), a mass <= 0 disables that term; dt: 0-d tensor.  Returns (posm_final, vel_final);
+    gradients flow to posm0 (lane 3 = masses), vel0, theta and dt."""
+    dt = torch.as_tensor(dt)
+    return _LeapfrogKDK.apply(posm0, vel0, theta, dt, G, eps, nsteps)
+
+
+class _EnsembleLeapfrogKDK(torch.autograd.Function):
+    @staticmethod
+    def forward(ctx, posm0, vel0, theta, dt, G, eps, nsteps):
+        nsim, n = posm0.shape[:2]
+        posm, vel = posm0.detach().clone().contiguous(), vel0.detach().clone().contiguous()
+        ws = B.alloc_workspace(B.ensemble_workspace_bytes(nsim))
+        tape = torch.empty(B.ensemble_tape_bytes(n, nsim, nsteps) // 4, dtype=torch.float32, device=posm.device)
+        th, dts = theta.detach().cpu().tolist(), dt.detach().cpu().tolist()
+        params = [(float(G), float(eps), float(dts[k]), B.Potential.make(nfw=(th[k][0], th[k][1]), mn=(th[k][2], th[k][3], th[k][4])))
+                  for k in range(nsim)]
+        B.ensemble_leapfrog_kdk_tape(posm, vel, params, int(nsteps), tape, ws)
+        ctx.save_for_backward(tape, theta, dt)
+        ctx.meta = (nsim, n, params, int(nsteps), ws)
+        return posm, vel
+
+    @staticmethod
+    def backward(ctx, g_posm, g_vel):
+        tape, theta, dt = ctx.saved_tensors
+        nsim, n, params, nsteps, ws = ctx.meta
+        lx, lv = g_posm.detach().clone().contiguous(), g_vel.detach().clone().contiguous()
+        g_mass_final = lx[:, :, 3].clone()
+        lx[:, :, 3] = 0
+        lv[:, :, 3] = 0
+        gm = torch.empty(nsim, n, dtype=torch.float64, device=lx.device)
+        gp = torch.empty(nsim, 8, dtype=torch.float64, device=lx.device)
+        B.ensemble_leapfrog_kdk_vjp(tape, params, nsteps, lx, lv, gm, gp, ws)
+        lx[:, :, 3] = gm.to(lx.dtype) + g_mass_final
+        return lx, lv, gp[:, :5].to(theta.dtype).to(theta.device), gp[:, 7].to(dt.dtype).to(dt.device), None, None, None
+
+
+def ensemble_leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.Tensor, dt: torch.Tensor, G: float,
+                          eps: float, nsteps: int):
+    """Differentiable batch of small simulations: posm0, vel0 float32 CUDA [nsim, n, 4] (n <= 2,048); theta [nsim, 5];
+    dt [nsim].  Returns (posm_final, vel_final); gradients flow to posm0 (lane 3 = masses), vel0, theta and dt."""
+    return _EnsembleLeapfrogKDK.apply(posm0, vel0, theta, dt, G, eps, nsteps)

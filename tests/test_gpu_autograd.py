@@ -1,0 +1,70 @@
+"""torch.autograd faces (paper_2511_22468_b200/autograd.py) against the oracle adjoint: a loss of the final state,
+`.backward()`, and the gradients land on the initial state (mass lane included), the potential parameters and dt."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import adjoint as A
+from paper_2511_22468_b200 import autograd as AG
+from paper_2511_22468_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _state(n, seed, dtype):
+    cfg = W.CONFIGS[1]
+    posm64, vel64 = W.random_cloud(n, seed=seed, scale=0.01, centre=cfg.centre)
+    posm64[:, 3] *= cfg.M / n
+    vel64 = vel64 * 0.02 + np.asarray(cfg.velocity)
+    return cfg, posm64.astype(dtype), W.vel4(vel64.astype(dtype), dtype)
+
+
+def test_single_simulation_f64_backward_matches_the_oracle_adjoint():
+    n, nsteps = 300, 5
+    cfg, p, v = _state(n, 21, np.float64)
+    rng = np.random.Generator(np.random.PCG64(22))
+    wx, wv = rng.normal(size=(n, 3)), rng.normal(size=(n, 3)) * 10.0
+    posm0 = torch.from_numpy(p).cuda().requires_grad_()
+    vel0 = torch.from_numpy(v).cuda().requires_grad_()
+    theta = torch.tensor([cfg.nfw[0], cfg.nfw[1], cfg.mn[0], cfg.mn[1], cfg.mn[2]], dtype=torch.float64, requires_grad=True)
+    dt = torch.tensor(cfg.dt, dtype=torch.float64, requires_grad=True)
+    xf, vf = AG.leapfrog_kdk(posm0, vel0, theta, dt, cfg.G, cfg.eps, nsteps)
+    loss = (torch.from_numpy(wx).cuda() * xf[:, :3]).sum() + (torch.from_numpy(wv).cuda() * vf[:, :3]).sum()
+    loss.backward()
+    ref = A.leapfrog_kdk_vjp(p, v[:, :3], cfg.G, cfg.eps, cfg.dt, nsteps, wx, wv, cfg.nfw, cfg.mn)
+    g = posm0.grad.cpu().numpy()
+    assert np.abs(g[:, :3] - ref["x0"]).max() <= 1e-9 * np.abs(ref["x0"]).max()
+    assert np.abs(g[:, 3] - ref["m"]).max() <= 1e-9 * np.abs(ref["m"]).max()
+    assert np.abs(vel0.grad.cpu().numpy()[:, :3] - ref["v0"]).max() <= 1e-9 * np.abs(ref["v0"]).max()
+    for k, name in enumerate(A.PARAM_NAMES):
+        assert abs(theta.grad[k].item() - ref[name]) <= 1e-8 * abs(ref[name]), name
+    assert abs(dt.grad.item() - ref["dt"]) <= 1e-8 * abs(ref["dt"])
+    assert np.array_equal(posm0.detach().cpu().numpy(), p)               # inputs untouched
+
+
+def test_ensemble_f32_backward_matches_the_oracle_adjoint_per_simulation():
+    nsim, n, nsteps = 3, 500, 4
+    cfg, p, v = _state(n, 31, np.float32)
+    posm = np.repeat(p[None], nsim, axis=0)
+    vel = np.repeat(v[None], nsim, axis=0)
+    rng = np.random.Generator(np.random.PCG64(32))
+    wx = rng.normal(size=(nsim, n, 3)).astype(np.float32)
+    scale = np.array([[1.0, 1.0, 1.0, 1.0, 1.0], [0.7, 1.0, 1.3, 1.0, 1.0], [1.2, 1.1, 0.9, 1.0, 1.2]])
+    th = scale * np.array([cfg.nfw[0], cfg.nfw[1], cfg.mn[0], cfg.mn[1], cfg.mn[2]])
+    dts = np.array([cfg.dt, 0.5 * cfg.dt, -cfg.dt])
+    posm0 = torch.from_numpy(posm).cuda().requires_grad_()
+    vel0 = torch.from_numpy(vel).cuda().requires_grad_()
+    theta = torch.tensor(th, dtype=torch.float64, requires_grad=True)
+    dt = torch.tensor(dts, dtype=torch.float64, requires_grad=True)
+    xf, vf = AG.ensemble_leapfrog_kdk(posm0, vel0, theta, dt, cfg.G, cfg.eps, nsteps)
+    (torch.from_numpy(wx).cuda() * xf[:, :, :3]).sum().backward()
+    G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
+    for k in range(nsim):
+        ref = A.leapfrog_kdk_vjp(posm[k].astype(np.float64), vel[k, :, :3].astype(np.float64), G, eps, float(np.float32(dts[k])),
+                                 nsteps, wx[k].astype(np.float64), np.zeros((n, 3)), (th[k, 0], th[k, 1]), (th[k, 2], th[k, 3], th[k, 4]))
+        g = posm0.grad[k].cpu().numpy().astype(np.float64)
+        assert np.abs(g[:, :3] - ref["x0"]).max() <= 1e-3 * np.abs(ref["x0"]).max()
+        assert np.abs(g[:, 3] - ref["m"]).max() <= 1e-3 * np.abs(ref["m"]).max()
+        for j, name in enumerate(A.PARAM_NAMES):
+            assert abs(theta.grad[k, j].item() - ref[name]) <= 1e-3 * abs(ref[name]), (k, name)
+        assert abs(dt.grad[k].item() - ref["dt"]) <= 1e-3 * abs(ref["dt"])
