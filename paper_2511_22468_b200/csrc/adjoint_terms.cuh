@@ -65,6 +65,31 @@ __device__ __forceinline__ void vjp_pair_term(const T px, const T py, const T pz
     }
 }
 
+// The equal-mass, no-eps/G term on packed fp32 pairs: TWO sources (j, j+1) against one target whose coordinates and
+// cotangent are duplicated in both halves.  27 FFMA2/FADD2/FMUL2 + 2 MUFU per two pairs; the halves of the
+// accumulators are the even-j and odd-j partial sums.  Same formulas as vjp_pair_term<float, true, false>.
+__device__ __forceinline__ void vjp_pair_term_x2(const f32x2 px, const f32x2 py, const f32x2 pz, const f32x2 cjx, const f32x2 cjy,
+                                                 const f32x2 cjz, const f32x2 xi, const f32x2 yi, const f32x2 zi,
+                                                 const f32x2 cxi, const f32x2 cyi, const f32x2 czi, const f32x2 e2,
+                                                 const f32x2 minus3, f32x2& ax, f32x2& ay, f32x2& az, f32x2& am)
+{
+    const f32x2 dx = sub2(px, xi), dy = sub2(py, yi), dz = sub2(pz, zi);
+    const f32x2 s = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, e2)));
+    float sl, sh;
+    unpk(s, sl, sh);
+    const f32x2 y = pk(rsqrt_approx(sl), rsqrt_approx(sh));
+    const f32x2 y2 = mul2(y, y);
+    const f32x2 f = mul2(y2, y);
+    const f32x2 g = mul2(mul2(f, y2), minus3);
+    const f32x2 pj = fma2(dz, cjz, fma2(dy, cjy, mul2(dx, cjx)));          // d . c_j
+    const f32x2 ux = sub2(cjx, cxi), uy = sub2(cjy, cyi), uz = sub2(cjz, czi);
+    const f32x2 gdu = mul2(g, fma2(dz, uz, fma2(dy, uy, mul2(dx, ux))));     // g (d . u)
+    ax = fma2(f, ux, fma2(gdu, dx, ax));
+    ay = fma2(f, uy, fma2(gdu, dy, ay));
+    az = fma2(f, uz, fma2(gdu, dz, az));
+    am = fma2(f, pj, am);
+}
+
 // Fixed-shape sum over the block (xor-shuffle tree, then warp sums in order); valid in thread 0.
 __device__ __forceinline__ double vjp_block_sum(double v, double* warp_scratch)
 {

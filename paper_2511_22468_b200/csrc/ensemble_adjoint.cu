@@ -29,6 +29,7 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
     constexpr int n_pad = NQ * VJP_THREADS;
     float4* const sp = reinterpret_cast<float4*>(evjp_smem);            // {x, y, z, m}
     float4* const sc = sp + n_pad;                                      // {cx, cy, cz, 0}
+    float* const soa = reinterpret_cast<float*>(sc + n_pad);            // x[], y[], z[], cx[], cy[], cz[] (packed loop)
     __shared__ double warp_scratch[VJP_THREADS / 32];
     const int tid = threadIdx.x;
     const int64_t sim = blockIdx.x;
@@ -88,8 +89,13 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
             an[q][0] = a.x; an[q][1] = a.y; an[q][2] = a.z;
             xs[q][0] = p.x; xs[q][1] = p.y; xs[q][2] = p.z; xs[q][3] = p.w;
             cs[q][0] = w * Lv[q][0]; cs[q][1] = w * Lv[q][1]; cs[q][2] = w * Lv[q][2];
-            sp[i] = p;
-            sc[i] = make_float4(cs[q][0], cs[q][1], cs[q][2], 0.f);
+            if (eqm && !EG) {                                          // structure of arrays: LDS.64 = two sources
+                soa[i] = p.x; soa[n_pad + i] = p.y; soa[2 * n_pad + i] = p.z;
+                soa[3 * n_pad + i] = cs[q][0]; soa[4 * n_pad + i] = cs[q][1]; soa[5 * n_pad + i] = cs[q][2];
+            } else {
+                sp[i] = p;
+                sc[i] = make_float4(cs[q][0], cs[q][1], cs[q][2], 0.f);
+            }
         }
         __syncthreads();                                               // sources staged
         float o[NQ][VJP_COMPS];                                        // n <= 2,048: two-level fp32 sums suffice
@@ -105,15 +111,34 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
                 for (int c = 0; c < VJP_COMPS; ++c) t[q][c] = 0.f;
             const int j1 = j0 + EVJP_TILE < n_pad ? j0 + EVJP_TILE : n_pad;
             if (eqm && !EG) {
-#pragma unroll 4
-                for (int j = j0; j < j1; ++j) {
-                    const float4 p = sp[j], c = sc[j];
+                // packed loop: two sources per instruction, the target duplicated in both halves
+                const f32x2 e2 = pk(eps2, eps2), m3 = pk(-3.0f, -3.0f);
+                f32x2 X[NQ], Y[NQ], Z[NQ], CX[NQ], CY[NQ], CZ[NQ], a2[NQ][4];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    X[q] = pk(xs[q][0], xs[q][0]); Y[q] = pk(xs[q][1], xs[q][1]); Z[q] = pk(xs[q][2], xs[q][2]);
+                    CX[q] = pk(cs[q][0], cs[q][0]); CY[q] = pk(cs[q][1], cs[q][1]); CZ[q] = pk(cs[q][2], cs[q][2]);
+                    a2[q][0] = a2[q][1] = a2[q][2] = a2[q][3] = 0ull;
+                }
+                const f32x2* const s2 = reinterpret_cast<const f32x2*>(soa);
+                constexpr int H = n_pad / 2;                            // f32x2 elements per array
+#pragma unroll 2
+                for (int j = j0 / 2; j < j1 / 2; ++j) {
+                    const f32x2 px = s2[j], py = s2[H + j], pz = s2[2 * H + j];
+                    const f32x2 qx = s2[3 * H + j], qy = s2[4 * H + j], qz = s2[5 * H + j];
 #pragma unroll
                     for (int q = 0; q < NQ; ++q)
-                        vjp_pair_term<float, true, false>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xs[q][0], xs[q][1], xs[q][2], xs[q][3],
-                                                          cs[q][0], cs[q][1], cs[q][2], eps2, t[q][0], t[q][1], t[q][2], t[q][3],
-                                                          t[q][4], t[q][5]);
+                        vjp_pair_term_x2(px, py, pz, qx, qy, qz, X[q], Y[q], Z[q], CX[q], CY[q], CZ[q], e2, m3, a2[q][0], a2[q][1],
+                                         a2[q][2], a2[q][3]);
                 }
+#pragma unroll
+                for (int q = 0; q < NQ; ++q)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        float lo, hi;
+                        unpk(a2[q][c], lo, hi);
+                        t[q][c] = lo + hi;
+                    }
             } else {
 #pragma unroll 4
                 for (int j = j0; j < j1; ++j) {
@@ -172,7 +197,7 @@ template <int NQ, bool EG>
 cudaError_t launch_evjp(const float* tape, const EnsembleParams64* params, int shared_params, int n, int64_t nsim,
                         int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, cudaStream_t stream)
 {
-    const size_t smem = (size_t)NQ * VJP_THREADS * 32;
+    const size_t smem = (size_t)NQ * VJP_THREADS * (32 + 24);
     cudaError_t e = cudaFuncSetAttribute(ensemble_vjp_kernel<NQ, EG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     ensemble_vjp_kernel<NQ, EG><<<(unsigned)nsim, VJP_THREADS, smem, stream>>>(
