@@ -37,6 +37,7 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
     typedef typename AVec4<T>::type V4;
     __shared__ V4 sp[VJP_TILE];
     __shared__ V4 sc[VJP_TILE];
+    __shared__ __align__(8) float soa[sizeof(T) == 4 ? 6 * VJP_TILE : 2];   // x[], y[], z[], cx[], cy[], cz[] (packed fp32 loop)
     const int tid = threadIdx.x;
     const int64_t i_base = (int64_t)blockIdx.x * (VJP_THREADS * IPT) + tid;
     const int64_t j_begin = (int64_t)blockIdx.y * chunk;
@@ -72,6 +73,10 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
             else { p.x = p.y = p.z = p.w = (T)0; c.x = c.y = c.z = c.w = (T)0; }   // m = 0, c = 0: contributes 0
             sp[tid] = p;
             sc[tid] = c;
+            if constexpr (sizeof(T) == 4) {
+                soa[tid] = p.x; soa[VJP_TILE + tid] = p.y; soa[2 * VJP_TILE + tid] = p.z;
+                soa[3 * VJP_TILE + tid] = c.x; soa[4 * VJP_TILE + tid] = c.y; soa[5 * VJP_TILE + tid] = c.z;
+            }
             src_equal = (p.w == mu);                        // padding (m = 0) makes the tile general
         }
         const bool eqm = __syncthreads_and(src_equal) != 0 && targets_equal;      // also: tile staged
@@ -79,13 +84,44 @@ pair_vjp_kernel(const typename AVec4<T>::type* __restrict__ posm, const typename
 #pragma unroll
         for (int k = 0; k < IPT; ++k) ax[k] = ay[k] = az[k] = am[k] = ae[k] = ag[k] = (T)0;
         if (eqm) {
-#pragma unroll 4
-            for (int j = 0; j < VJP_TILE; ++j) {
-                const V4 p = sp[j], c = sc[j];
+            if constexpr (sizeof(T) == 4) {
+                // packed fp32 loop: two sources per instruction, the target duplicated in both halves
+                const f32x2 e2 = pk(eps2, eps2), m3 = pk(-3.0f, -3.0f);
+                f32x2 X[IPT], Y[IPT], Z[IPT], CX[IPT], CY[IPT], CZ[IPT], a2[IPT][4];
 #pragma unroll
-                for (int k = 0; k < IPT; ++k)
-                    vjp_pair_term<T, true, false>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xi[k], yi[k], zi[k], mi[k], cxi[k], cyi[k],
-                                                  czi[k], eps2, ax[k], ay[k], az[k], am[k], ae[k], ag[k]);
+                for (int k = 0; k < IPT; ++k) {
+                    X[k] = pk(xi[k], xi[k]); Y[k] = pk(yi[k], yi[k]); Z[k] = pk(zi[k], zi[k]);
+                    CX[k] = pk(cxi[k], cxi[k]); CY[k] = pk(cyi[k], cyi[k]); CZ[k] = pk(czi[k], czi[k]);
+                    a2[k][0] = a2[k][1] = a2[k][2] = a2[k][3] = 0ull;
+                }
+                const f32x2* const s2 = reinterpret_cast<const f32x2*>(soa);
+                constexpr int H = VJP_TILE / 2;
+#pragma unroll 2
+                for (int j = 0; j < H; ++j) {
+                    const f32x2 px = s2[j], py = s2[H + j], pz = s2[2 * H + j];
+                    const f32x2 qx = s2[3 * H + j], qy = s2[4 * H + j], qz = s2[5 * H + j];
+#pragma unroll
+                    for (int k = 0; k < IPT; ++k)
+                        vjp_pair_term_x2(px, py, pz, qx, qy, qz, X[k], Y[k], Z[k], CX[k], CY[k], CZ[k], e2, m3, a2[k][0], a2[k][1],
+                                         a2[k][2], a2[k][3]);
+                }
+#pragma unroll
+                for (int k = 0; k < IPT; ++k) {
+                    float lo, hi;
+                    unpk(a2[k][0], lo, hi); ax[k] = lo + hi;
+                    unpk(a2[k][1], lo, hi); ay[k] = lo + hi;
+                    unpk(a2[k][2], lo, hi); az[k] = lo + hi;
+                    unpk(a2[k][3], lo, hi); am[k] = lo + hi;
+                }
+            } else {
+#pragma unroll 4
+                for (int j = 0; j < VJP_TILE; ++j) {
+                    const V4 p = sp[j], c = sc[j];
+#pragma unroll
+                    for (int k = 0; k < IPT; ++k)
+                        vjp_pair_term<T, true, false>(p.x, p.y, p.z, p.w, c.x, c.y, c.z, xi[k], yi[k], zi[k], mi[k], cxi[k], cyi[k],
+                                                      czi[k], eps2, ax[k], ay[k], az[k], am[k], ae[k], ag[k]);
+                }
             }
         } else {
 #pragma unroll 4
