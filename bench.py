@@ -163,6 +163,42 @@ def _oracle_sample_rate(cfg, seconds_target: float):
                       % (nt, cfg.n, cfg.name, dt)}, (p64, G, eps, opot)
 
 
+def run_cpu_pieces():
+    """the oracle timed on this host's cores on the listed pieces (minutes of CPU; not part of
+    the default run).  Prints one JSON object."""
+    from oracle import oracle as O
+    from paper_2511_22468_b200 import workloads as W
+    out = {"cores": O.num_threads(), "kind": "oracle", "pieces": []}
+
+    def timed(label, interactions, fn):
+        t0 = time.perf_counter()
+        fn()
+        dt = time.perf_counter() - t0
+        out["pieces"].append({"piece": label, "seconds": dt, "interactions": interactions, "G_int_per_s": interactions / dt / 1e9})
+
+    for ci in (1, 2):
+        cfg = W.CONFIGS[ci]
+        p64 = W.to_f32(W.make_state(cfg)[0]).astype(np.float64)
+        timed("full pair evaluation, N = %d" % cfg.n, float(cfg.n) ** 2, lambda: O.pair_accel(p64, cfg.G, cfg.eps))
+    for ci in (3, 4):
+        cfg = W.CONFIGS[ci]
+        p64 = W.to_f32(W.make_state(cfg)[0]).astype(np.float64)
+        idx = W.target_subset(cfg.n)
+        timed("4,096-target subset, N = %d" % cfg.n, 4096.0 * cfg.n, lambda: O.pair_accel(p64, cfg.G, cfg.eps, targets=idx))
+    cfg = W.CONFIGS[0]
+    p64, v64 = W.make_state(cfg)
+    timed("config 0 end to end (N = 1,024, 10 KDK steps, fp64)", 11.0 * cfg.n ** 2,
+          lambda: O.leapfrog_kdk(p64, v64, cfg.G, cfg.eps, cfg.dt, cfg.nsteps))
+    out["pieces"][-1]["steps_per_s"] = cfg.nsteps / out["pieces"][-1]["seconds"]
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg)
+    opot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    timed("config 1, 100 of its 1,000 KDK steps (N = 16,384)", 101.0 * cfg.n ** 2,
+          lambda: O.leapfrog_kdk(p64, v64, cfg.G, cfg.eps, cfg.dt, 100, opot))
+    out["pieces"][-1]["steps_per_s"] = 100 / out["pieces"][-1]["seconds"]
+    print(json.dumps(out), flush=True)
+
+
 def run_reference(args, rank: int):
     """--impl reference: the fp64 CPU oracle on the host cores, same config/metric/unit (rank 0 only)."""
     if rank != 0:
@@ -515,7 +551,12 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
     ap.add_argument("--integrator-only", action="store_true",
                     help="run only the O(N) integrator kernel's HBM roofline leg (N = 2^24) and print it")
+    ap.add_argument("--cpu-pieces", action="store_true",
+                    help="time the oracle on the pieces BASELINE.md section 3 lists (minutes of CPU) and print them")
     args = ap.parse_args()
+    if args.cpu_pieces:
+        run_cpu_pieces()
+        return 0
     if args.impl == "reference":
         run_reference(args, int(os.environ.get("RANK", "0")))
         return 0
