@@ -148,8 +148,14 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
             stage4[2 * i1 + 1] = make_float4(z1, z1, m1, m1);
         }
         __syncthreads();                                   // sources staged
-        if (eqm) ens_pair<NPAIR, true>(src, n_pad, prm.eps2, prm.G * mass0, xi, yi, zi, gx, gy, gz);
-        else     ens_pair<NPAIR, false>(src, n_pad, prm.eps2, prm.G, xi, yi, zi, gx, gy, gz);
+        if (n == 1) {
+            // a single particle feels only the external potential (its softened self term is exactly 0): the orbit
+            // mode of the paper's pipeline (backward integration of the centre of mass, PAPER.md:L43 step 2; orbit
+            // fitting, L57) skips the pair loop
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) gx[p] = gy[p] = gz[p] = 0ull;
+        } else if (eqm) ens_pair<NPAIR, true>(src, n_pad, prm.eps2, prm.G * mass0, xi, yi, zi, gx, gy, gz);
+        else            ens_pair<NPAIR, false>(src, n_pad, prm.eps2, prm.G, xi, yi, zi, gx, gy, gz);
         __syncthreads();                                   // sources consumed: the next drift may overwrite them
         if (prm.pot.GMs != 0.0f || prm.pot.GMd != 0.0f) {
 #pragma unroll

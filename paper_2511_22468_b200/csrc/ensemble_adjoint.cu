@@ -103,7 +103,7 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
         for (int q = 0; q < NQ; ++q)
 #pragma unroll
             for (int c = 0; c < VJP_COMPS; ++c) o[q][c] = 0.f;
-        for (int j0 = 0; j0 < n_pad; j0 += EVJP_TILE) {
+        for (int j0 = 0; j0 < n_pad && n > 1; j0 += EVJP_TILE) {          // n == 1: no pairs (orbit mode)
             float t[NQ][VJP_COMPS];
 #pragma unroll
             for (int q = 0; q < NQ; ++q)
