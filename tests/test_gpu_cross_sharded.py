@@ -149,3 +149,32 @@ def test_sharded_driver_with_emulated_ranks_matches_the_single_gpu_leapfrog(worl
         assert np.abs(got_v[:, :3] - want[1][:, :3]).max() <= rel * 0.21 * 10
         for r in range(1, world):                                        # every rank holds the same positions
             assert bufs[r].cpu().numpy().tobytes() == got_p.tobytes()
+
+
+def test_degenerate_sizes_are_ok_noops_or_zeros():
+    """n == 0 / nt == 0 / nsim == 0 / nsteps == 0 through every newer entry point: status OK, outputs untouched or zero."""
+    cfg = W.CONFIGS[1]
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    ws = B.alloc_workspace(1 << 20)
+    e4 = torch.zeros(0, 4, device="cuda")
+    s4 = torch.randn(50, 4, device="cuda")
+    t4 = torch.randn(7, 4, device="cuda")
+    acc = torch.full((7, 4), 5.0, device="cuda")
+    B.pair_accel_cross(t4, e4, acc, 1.0, 0.1, ws)                        # no sources: zero acceleration
+    torch.cuda.synchronize()
+    assert torch.all(acc == 0)
+    B.pair_accel_cross(e4, s4, torch.zeros(0, 4, device="cuda"), 1.0, 0.1, ws)   # no targets: no-op
+    B.pair_accel(e4, e4.clone(), 1.0, 0.1, ws)
+    B.leapfrog_kdk(e4, e4.clone(), e4.clone(), 1.0, 0.1, 0.1, 5, pot, ws)
+    B.kick_drift(e4, e4.clone(), e4.clone(), 1.0, 0.1, pot, 3, ws)
+    out = torch.full((16,), 7.0, dtype=torch.float64, device="cuda")
+    B.diagnostics(e4, e4.clone(), 1.0, 0.1, pot, out, ws)
+    gp = torch.full((8,), 7.0, dtype=torch.float64, device="cuda")
+    B.accel_vjp(e4, e4.clone(), 1.0, 0.1, pot, e4.clone(), torch.zeros(0, dtype=torch.float64, device="cuda"), gp, ws)
+    torch.cuda.synchronize()
+    assert torch.all(out == 0) and torch.all(gp == 0)
+    e34 = torch.zeros(0, 10, 4, device="cuda")
+    B.ensemble_leapfrog_kdk(e34, e34.clone(), [(cfg.G, cfg.eps, cfg.dt, pot)], 3, ws)       # no simulations
+    e30 = torch.zeros(4, 0, 4, device="cuda")
+    B.ensemble_leapfrog_kdk(e30, e30.clone(), [(cfg.G, cfg.eps, cfg.dt, pot)], 3, ws)       # no particles
+    torch.cuda.synchronize()
