@@ -127,6 +127,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "WAIT_DONE:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// The producer lane's wait: it has a whole tile time (microseconds) of slack, so it backs off between polls instead
+// of competing with the two compute warps of its scheduler for issue slots (the plain loop retired ~7 % of the
+// kernel's warp instructions, all on one of the four schedulers).
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
+    uint32_t done = 0;
+    while (true) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(256);
+    }
+}
 // 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier.  dst, src and
 // bytes must be multiples of 16.  SASS: UBLKCP.
 __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {

@@ -192,7 +192,7 @@ pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsr
             uint32_t ph = prefetch == STAGES ? 1u : 0u;
             int32_t t = (int32_t)((u0 + prefetch) % plan.J);
             for (int64_t u = u0 + prefetch; u < u1; ++u) {
-                mbar_wait(&empty_bar[s], ph ^ 1u);
+                mbar_wait_backoff(&empty_bar[s], ph ^ 1u);
                 mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
                 tma_load_1d(smem_raw + (size_t)s * tile_bytes,
                             reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
