@@ -92,3 +92,33 @@ def test_ensemble_checkpointed_backward_equals_the_full_tape_backward():
         assert g[0].tobytes() == grads[0][0].tobytes()                   # same forward, bit for bit
         for a, b in zip(g[1:], grads[0][1:]):
             assert np.abs(a - b).max() <= 2e-5 * np.abs(b).max()
+
+
+def test_gradient_descent_on_the_halo_mass_recovers_the_mock_value():
+    """The paper's use of the gradients in miniature (PAPER.md:L43 steps 4-5): a mock stream is simulated with the true
+    halo mass, the same progenitor is re-simulated with a wrong halo mass, and gradient steps on a point-wise loss of the
+    final positions (obtained through ensemble autograd) drive the halo mass back to the true value."""
+    cfg = W.CONFIGS[1]
+    n, nsteps = 500, 60
+    _, p, v = _state(n, 51, np.float32)
+    posm0 = torch.from_numpy(p[None]).cuda()
+    vel0 = torch.from_numpy(v[None]).cuda()
+    dt = torch.tensor([cfg.dt], dtype=torch.float64)
+    true = torch.tensor([[cfg.nfw[0], cfg.nfw[1], cfg.mn[0], cfg.mn[1], cfg.mn[2]]], dtype=torch.float64)
+    with torch.no_grad():
+        x_obs, _ = AG.ensemble_leapfrog_kdk(posm0, vel0, true, dt, cfg.G, cfg.eps, nsteps)
+    log_m = torch.tensor(np.log(1.3 * cfg.nfw[0]), dtype=torch.float64, requires_grad=True)      # 30 % too heavy
+    losses = []
+    for _ in range(12):
+        theta = torch.stack([torch.exp(log_m), true[0, 1], true[0, 2], true[0, 3], true[0, 4]]).reshape(1, 5)
+        xf, _ = AG.ensemble_leapfrog_kdk(posm0, vel0, theta, dt, cfg.G, cfg.eps, nsteps, checkpoint_every=20)
+        loss = ((xf[:, :, :3] - x_obs[:, :, :3]).double() ** 2).mean()
+        (g,) = torch.autograd.grad(loss, log_m)
+        losses.append(loss.item())
+        # Gauss-Newton-like step for a one-parameter least-squares problem: loss ~ c (log m - log m*)^2
+        with torch.no_grad():
+            log_m -= (2.0 * loss.item() / g.item()) if g.item() != 0.0 else 0.0
+            log_m.clamp_(np.log(0.5 * cfg.nfw[0]), np.log(2.0 * cfg.nfw[0]))
+    m = float(torch.exp(log_m.detach()))
+    assert losses[-1] <= 1e-3 * losses[0]
+    assert abs(m / cfg.nfw[0] - 1.0) <= 1e-2
