@@ -25,7 +25,7 @@ FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star con
 SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144 (ncu --set full)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 12645888    # profiles/r01_pair_f32_ncu_full.txt: 12.64 MB read + 4 KB written
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 12669440    # profiles/r01_pair_f32_ncu_full.txt: 12.67 MB read + 0 written
 
 
 def _peaks():
