@@ -9,7 +9,11 @@ CUDA package ``paper_2511_22468_b200`` and shares no code with it.
 Citations: PAPER.md:L15-17 (direct softened pair force), L9/L45/L63 (NFW + MN),
 L47 (Velocity-Verlet, fixed steps); formulas from BASELINE.json north_star and
 DESIGN.md readings R1-R14.  No function is "parity unpinned": see the pin list
-in the header of odisseo_oracle.c.
+in the header of odisseo_oracle.c; the O(N) diagnostics below (kinetic energy, momenta, centre of
+mass) are pinned by hand values in tests/test_oracle_leapfrog.py (single particle on each axis,
+hand-expanded cross product, unequal-mass binary L_z = mu omega d^2) and the zero point of the
+potentials by closed forms in tests/test_oracle_potential.py (Phi_NFW(0) = -G M_s/r_s,
+r Phi_NFW / ln(1+r/r_s) = -G M_s, Phi_MN(0) = -G M/(a+b)).
 
 Layouts: ``posm`` float64 [n, 4] = {x, y, z, m}; ``vel`` / ``acc`` float64 [n, 3].
 """

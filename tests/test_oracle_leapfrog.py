@@ -132,3 +132,51 @@ def test_milky_way_orbit_conserves_lz_and_energy_order():
     one = np.array([[*cfg.centre, cfg.M]])
     p1, _, _ = O.leapfrog_kdk(one, np.array([cfg.velocity]), cfg.G, cfg.eps, 0.25, 800, pot)
     assert np.linalg.norm(com - p1[0, :3]) <= 5e-3
+
+
+# ---- hand-value pins of the O(N) diagnostics (VERDICT r1 "parity unpinned") ---------
+# Conservation tests alone cannot see a sign flip (cross(v, x)), a permuted axis or a dropped mass
+# weight; these values are computed by hand from the definitions L = sum m x cross v, P = sum m v,
+# K = 1/2 sum m |v|^2, x_com = sum m x / sum m.
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_angular_momentum_single_particle_hand_values(axis):
+    """m = 2 at e_a with v = 3 e_b (a, b, c cyclic) -> L = +6 e_c: fixes sign, axis order and mass weight."""
+    a, b, c = axis, (axis + 1) % 3, (axis + 2) % 3
+    posm = np.zeros((1, 4)); vel = np.zeros((1, 3))
+    posm[0, a], posm[0, 3], vel[0, b] = 1.0, 2.0, 3.0
+    L = O.angular_momentum(posm, vel)
+    expect = np.zeros(3); expect[c] = 6.0
+    assert np.array_equal(L, expect)
+    # and the anti-cyclic arrangement gives -6
+    posm2 = np.zeros((1, 4)); vel2 = np.zeros((1, 3))
+    posm2[0, b], posm2[0, 3], vel2[0, a] = 1.0, 2.0, 3.0
+    assert np.array_equal(O.angular_momentum(posm2, vel2), -expect)
+
+
+def test_angular_momentum_general_vector_hand_expansion():
+    """x = (1,2,3), v = (4,5,6), m = 0.5: x cross v = (2*6-3*5, 3*4-1*6, 1*5-2*4) = (-3, 6, -3)."""
+    L = O.angular_momentum(np.array([[1.0, 2.0, 3.0, 0.5]]), np.array([[4.0, 5.0, 6.0]]))
+    assert np.array_equal(L, np.array([-1.5, 3.0, -1.5]))
+
+
+def test_angular_momentum_unequal_mass_binary_closed_form():
+    """Circular binary about its centre of mass: L_z = mu omega d^2, mu = m1 m2/(m1+m2) (mass weight)."""
+    posm, vel, G, T = _two_body_circular(0.3)
+    m1, m2, d = 0.7, 0.3, 1.0
+    w = 2 * np.pi / T
+    L = O.angular_momentum(posm, vel)
+    assert L[0] == 0.0 and L[1] == 0.0
+    assert abs(L[2] - m1 * m2 / (m1 + m2) * w * d * d) <= 1e-15
+    # dropping the mass weight would give omega (x1^2 + x2^2) = 0.58 omega instead of 0.21 omega
+    assert abs(L[2] - w * 0.58) > 0.1
+
+
+def test_linear_momentum_kinetic_energy_centre_of_mass_hand_values():
+    posm = np.array([[1.0, 0.0, 0.0, 2.0], [0.0, 4.0, 0.0, 6.0]])
+    vel = np.array([[0.0, 3.0, 0.0], [1.0, 0.0, -2.0]])
+    assert np.array_equal(O.linear_momentum(posm, vel), np.array([6.0, 6.0, -12.0]))
+    assert O.kinetic_energy(posm, vel) == 0.5 * 2.0 * 9.0 + 0.5 * 6.0 * 5.0      # 9 + 15 = 24
+    assert np.array_equal(O.centre_of_mass(posm), np.array([0.25, 3.0, 0.0]))    # (2*1/8, 6*4/8, 0)
+    # L = 2 (1,0,0)x(0,3,0) + 6 (0,4,0)x(1,0,-2) = (0,0,6) + 6 (-8, 0, -4) = (-48, 0, -18)
+    assert np.array_equal(O.angular_momentum(posm, vel), np.array([-48.0, 0.0, -18.0]))

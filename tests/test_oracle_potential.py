@@ -141,3 +141,40 @@ def test_nfw_against_40_digit_evaluation_and_conditioning_at_small_radius():
         exact = np.array([float(f * t) for t in x])
         tol = max(1e-14, 4 * 2.2e-16 * 2 * rs / r)
         assert np.linalg.norm(a - exact) <= tol * np.linalg.norm(exact)
+
+
+# ---- zero point of the potentials (finite differences and Poisson pin only grad Phi) ----------------
+# Closed forms: Phi_NFW(r -> 0) = -G M_s / r_s; r Phi_NFW(r) / ln(1 + r/r_s) = -G M_s for every r
+# (so Phi -> 0 like ln(r)/r at infinity, no additive constant); Phi_MN(0,0,0) = -G M / (a + b);
+# Phi_MN(R,0,z) r -> -G M as r -> infinity.
+
+def test_potential_zero_points_closed_forms():
+    G, Ms, rs, Md, a, b = 4.4985e-12, 1e12, 16.0, 6.8e10, 3.0, 0.28
+    nfw = O.Potential.make(nfw=(Ms, rs))
+    mn = O.Potential.make(mn=(Md, a, b))
+    # NFW centre: exact limit at r = 0 and the first-order expansion -G M_s/r_s (1 - c/2) next to it
+    assert O.ext_potential(np.array([[0.0, 0.0, 0.0, 1.0]]), G, nfw)[0] == -G * Ms / rs
+    r = 1e-6 * rs
+    phi = O.ext_potential(np.array([[r, 0.0, 0.0, 1.0]]), G, nfw)[0]
+    assert abs(phi / (-G * Ms / rs) - (1 - 0.5e-6)) <= 1e-11
+    # NFW far field: r Phi / ln(1 + r/r_s) = -G M_s (an additive constant C would add C r / ln(1+c))
+    for c in (1.0, 1e3, 1e6):
+        r = c * rs
+        phi = O.ext_potential(np.array([[0.0, r / np.sqrt(2), -r / np.sqrt(2), 1.0]]), G, nfw)[0]
+        assert abs(phi * r / np.log1p(c) / (-G * Ms) - 1.0) <= 1e-14
+    # hand value: c = 1 -> Phi = -G M_s ln 2 / r_s
+    phi = O.ext_potential(np.array([[rs, 0.0, 0.0, 1.0]]), G, nfw)[0]
+    assert abs(phi - (-G * Ms * 0.6931471805599453 / rs)) <= 1e-15 * abs(phi)
+    # MN centre and far field
+    assert abs(O.ext_potential(np.array([[0.0, 0.0, 0.0, 1.0]]), G, mn)[0] - (-G * Md / (a + b))) <= 1e-16
+    r = 1e9
+    phi = O.ext_potential(np.array([[0.6 * r, 0.0, 0.8 * r, 1.0]]), G, mn)[0]
+    assert abs(phi * r / (-G * Md) - 1.0) <= 1e-8
+    # off-centre value from the definition written out: B = sqrt(z^2 + b^2), D = sqrt(R^2 + (a + B)^2)
+    B = np.sqrt(1.0 + b * b); D = np.sqrt(16.0 + (a + B) ** 2)
+    phi = O.ext_potential(np.array([[4.0, 0.0, 1.0, 1.0]]), G, mn)[0]
+    assert abs(phi - (-G * Md / D)) <= 1e-16
+    # the two terms add, and the energy weights by mass: sum m Phi
+    both = O.Potential.make(nfw=(Ms, rs), mn=(Md, a, b))
+    p = np.array([[8.0, 1.0, -2.0, 3.0]])
+    assert abs(O.ext_potential_energy(p, G, both) - 3.0 * (O.ext_potential(p, G, nfw)[0] + O.ext_potential(p, G, mn)[0])) <= 1e-18
