@@ -286,6 +286,23 @@ int64_t odisseo_launch_count(void);
 odisseo_status odisseo_profile_begin(void);
 odisseo_status odisseo_profile_end(double *h_ms_total, int64_t *h_launches, int64_t *h_dropped);
 
+/* Pipe-rate micro-benchmarks ("verify with step-0
+ * micro-benchmarks"): the measured FP32 / FP64 / MUFU rates the roofline fractions are quoted
+ * against, next to the nominal ones.  Instrumentation, not part of the hot path.
+ *   odisseo_ubench_kinds: number of kinds; odisseo_ubench_name(kind): static string, NULL if out of
+ *     range ("ffma", "ffma2_3src", "ffma2_shared", "ffma2_square", "fadd2", "fmul2", "mufu_rsq",
+ *     "dfma", and interleaved mixes with the pair kernel's instruction proportions).
+ *   odisseo_ubench_run: launches kind on ctas_per_sm * SMs CTAs of `threads` threads (multiple of 32,
+ *     <= 1024), `iters` (even, >= 2) loop iterations per thread, one warm-up launch + 3 timed with
+ *     CUDA events on `stream`; SYNCHRONISES the stream and allocates 256 B of device memory for
+ *     the duration of the call.  h_out (HOST, 6 doubles) = {best time in ms, FP32-pipe lane
+ *     operations executed (a packed instruction counts 2 per thread), MUFU results, FP64
+ *     operations, shared-memory loads (per thread), SM count}.
+ *   Errors: ERR_NULL, ERR_ARG (range), ERR_ARCH, ERR_CUDA. */
+int odisseo_ubench_kinds(void);
+const char *odisseo_ubench_name(int kind);
+odisseo_status odisseo_ubench_run(int kind, int ctas_per_sm, int threads, int64_t iters, double h_out[6], void *stream);
+
 /* Description of the launch plan the library would use for n particles on the current
  * device (host arithmetic + one device-attribute query): fills out[0..7] with
  * {i_bodies_per_thread, threads_per_cta, tile_records, persistent_ctas, i_blocks,

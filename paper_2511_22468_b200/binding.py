@@ -32,7 +32,7 @@ EXPORTS = [
     "odisseo_leapfrog_kdk_tape_f32", "odisseo_leapfrog_kdk_tape_f64", "odisseo_leapfrog_kdk_vjp_f32",
     "odisseo_leapfrog_kdk_vjp_f64", "odisseo_ensemble_tape_bytes", "odisseo_ensemble_leapfrog_kdk_tape_f32",
     "odisseo_ensemble_leapfrog_kdk_vjp_f32", "odisseo_cross_workspace_bytes", "odisseo_pair_accel_cross_f32",
-    "odisseo_pair_accel_cross_f64",
+    "odisseo_pair_accel_cross_f64", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
 ]
 
 
@@ -121,6 +121,10 @@ def lib():
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
         L.odisseo_profile_end.argtypes = [vp, vp, vp]
+        L.odisseo_ubench_kinds.argtypes = []
+        L.odisseo_ubench_name.restype = ctypes.c_char_p
+        L.odisseo_ubench_name.argtypes = [ci]
+        L.odisseo_ubench_run.argtypes = [ci, ci, ci, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -473,3 +477,16 @@ def profile_end():
     ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
     _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
     return float(ms.value), int(nl.value), int(nd.value)
+
+
+def ubench_kinds():
+    """Names of the pipe-rate micro-benchmarks, indexed by kind."""
+    L = lib()
+    return [L.odisseo_ubench_name(k).decode() for k in range(L.odisseo_ubench_kinds())]
+
+
+def ubench_run(kind: int, ctas_per_sm: int = 2, threads: int = 1024, iters: int = 1 << 14, stream=None):
+    """One micro-benchmark: dict(ms, fp32_lane_ops, mufu, fp64_ops, lds, sms) as counted by the library."""
+    out = (ctypes.c_double * 6)()
+    _check(lib().odisseo_ubench_run(int(kind), int(ctas_per_sm), int(threads), int(iters), out, _stream(stream)), "ubench_run")
+    return {"ms": out[0], "fp32_lane_ops": out[1], "mufu": out[2], "fp64_ops": out[3], "lds": out[4], "sms": int(out[5])}

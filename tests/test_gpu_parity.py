@@ -115,8 +115,10 @@ def test_pair_one_different_mass_anywhere_selects_the_general_path(n, odd, dtype
     assert pair_ratio(out.cpu().numpy(), p64b, G, eps) <= tol
 
 
-@pytest.mark.parametrize("ci", [0, 1])
+@pytest.mark.parametrize("ci", [0, 1, 2])
 def test_pair_f32_configs_full(ci):
+    """step-0 acceleration parity at FULL N for configs 0-2 (config 2: 4.3e9 oracle
+    interactions, ~1 s on the box's cores)."""
     cfg = W.CONFIGS[ci]
     posm64, _ = W.make_state(cfg)
     p32, p64, G, eps = f32_inputs(posm64, cfg.G, cfg.eps)
