@@ -142,13 +142,20 @@ def test_full_length_fp32_runs_keep_the_invariants(ci):
     d0 = torch.empty(16, dtype=torch.float64, device="cuda")
     d1 = torch.empty(16, dtype=torch.float64, device="cuda")
     B.diagnostics(posm, vel, cfg.G, cfg.eps, pot, d0, wd)
-    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, ws)
+    # the centre of mass is compared after at most 600 steps: once the stream wraps a good part of the orbit (config 2
+    # covers ~10 orbits) the centre of mass of a curved stream is no longer a point of the orbit (measured 1.2 kpc off)
+    ncom = min(nsteps, 600)
+    dc = torch.empty(16, dtype=torch.float64, device="cuda")
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, ncom, pot, ws)
+    B.diagnostics(posm, vel, cfg.G, cfg.eps, pot, dc, wd)
+    if nsteps > ncom:
+        B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps - ncom, pot, ws, acc_valid=True)
     B.diagnostics(posm, vel, cfg.G, cfg.eps, pot, d1, wd)
     torch.cuda.synchronize()
-    d0, d1 = d0.cpu().numpy(), d1.cpu().numpy()
+    d0, d1, dc = d0.cpu().numpy(), d1.cpu().numpy(), dc.cpu().numpy()
     one, _, _ = O.leapfrog_kdk(np.array([[*cfg.centre, cfg.M]]), np.array([cfg.velocity]), cfg.G, cfg.eps, cfg.dt,
-                               nsteps, O.Potential.make(nfw=cfg.nfw, mn=cfg.mn))
-    com_off = float(np.linalg.norm(d1[9:12] - one[0, :3]))
+                               ncom, O.Potential.make(nfw=cfg.nfw, mn=cfg.mn))
+    com_off = float(np.linalg.norm(dc[9:12] - one[0, :3]))
     print("cfg%d %d steps: dLz/Lz %.2e dE/E %.2e CoM offset %.4f kpc" % (
         ci, nsteps, abs(d1[8] - d0[8]) / abs(d0[8]), abs(d1[13] - d0[13]) / abs(d0[13]), com_off))
     assert abs(d1[8] - d0[8]) <= 1e-6 * abs(d0[8])                        # L_z
