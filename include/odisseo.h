@@ -71,8 +71,10 @@ const char *odisseo_status_string(odisseo_status s);
 int odisseo_last_cuda_error(void);
 
 /* Upper bound, in bytes, of the device scratch any pair/leapfrog call on n particles
- * needs (packed source tiles + fixed-order partial sums).  is_f64 != 0 for the fp64 calls.
- * Returns 0 for n <= 0.  Pure host arithmetic; needs no GPU. */
+ * needs (staged source records + one row of fixed-order partial sums per work unit).
+ * is_f64 != 0 for the fp64 calls.  Returns 0 for n <= 0.  With a current CUDA device the
+ * bound is the one for that device's SM count; without one (no GPU) it is the maximum over
+ * devices with 64..192 SMs.  Host arithmetic only. */
 size_t odisseo_workspace_bytes(int64_t n, int is_f64);
 
 /* Pair acceleration, fp32.
@@ -305,15 +307,19 @@ odisseo_status odisseo_ubench_run(int kind, int ctas_per_sm, int threads, int64_
 
 /* Description of the launch plan the library would use for n particles on the current
  * device (host arithmetic + one device-attribute query): fills out[0..7] with
- * {i_bodies_per_thread, threads_per_cta, tile_records, persistent_ctas, i_blocks,
- *  j_tiles, partial_slots, kernels_per_step}.  For tests, bench.py and DESIGN.md. */
+ * {i_bodies_per_thread, threads_per_cta, max_tile_records, persistent_ctas, i_blocks,
+ *  source_chunks, partial_rows, kernels_per_step}.  For tests, bench.py and DESIGN.md. */
 odisseo_status odisseo_describe_plan(int64_t n, int is_f64, int64_t out[8]);
 /* Same for a hypothetical device with num_sms SMs: pure host arithmetic, needs no GPU. */
 odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8]);
-/* Stream-K bookkeeping exactly as the kernels compute it (SURVEY.md 8a row a1'), for host
- * tests: out = {CTA that owns work unit u, first unit of CTA c, one past the last unit of CTA c}
- * where units number the (i-block, j-tile) pairs u = b * j_tiles + t.  Pure host arithmetic. */
-odisseo_status odisseo_plan_probe(int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[3]);
+/* Same for nt targets against n sources (the cross call): max_tile_records and source_chunks depend on
+ * n and num_sms only, never on nt (the same fixed reduction order per target). */
+odisseo_status odisseo_describe_cross_plan_for(int64_t nt, int64_t n, int is_f64, int num_sms, int64_t out[8]);
+/* Unit bookkeeping exactly as the kernels compute it (SURVEY.md 8a row a1'), for host tests: units number
+ * the (i-block, source chunk) pairs u = b * source_chunks + s;
+ * out = {CTA that owns unit u, first unit of CTA c, one past the last unit of CTA c,
+ *        first source record of u's chunk, one past its last source record}.  Pure host arithmetic. */
+odisseo_status odisseo_plan_probe(int64_t nt, int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[5]);
 
 #ifdef __cplusplus
 }

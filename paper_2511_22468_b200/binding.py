@@ -24,7 +24,7 @@ EXPORTS = [
     "odisseo_pair_accel_f32", "odisseo_pair_accel_f64", "odisseo_pair_accel_soa_f32",
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
-    "odisseo_describe_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
+    "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
     "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
@@ -103,7 +103,8 @@ def lib():
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
         L.odisseo_describe_plan.argtypes = [i64, ci, vp]
         L.odisseo_describe_plan_for.argtypes = [i64, ci, ci, vp]
-        L.odisseo_plan_probe.argtypes = [i64, ci, ci, i64, i64, vp]
+        L.odisseo_describe_cross_plan_for.argtypes = [i64, i64, ci, ci, vp]
+        L.odisseo_plan_probe.argtypes = [i64, i64, ci, ci, i64, i64, vp]
         L.odisseo_vjp_workspace_bytes.restype = sz
         L.odisseo_vjp_workspace_bytes.argtypes = [i64, ci]
         L.odisseo_tape_bytes.restype = sz
@@ -179,21 +180,27 @@ def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:
     return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
 
 
-def describe_plan(n: int, is_f64: bool = False, num_sms: Optional[int] = None) -> dict:
+_PLAN_KEYS = ["i_bodies_per_thread", "threads_per_cta", "max_tile_records", "persistent_ctas", "i_blocks", "source_chunks",
+              "partial_rows", "kernels_per_step"]
+
+
+def describe_plan(n: int, is_f64: bool = False, num_sms: Optional[int] = None, nt: Optional[int] = None) -> dict:
+    """Launch plan for n sources (and nt targets, default n) on the current device or one with num_sms SMs."""
     out = (ctypes.c_int64 * 8)()
     if num_sms is None:
         _check(lib().odisseo_describe_plan(int(n), int(is_f64), out), "describe_plan")
     else:
-        _check(lib().odisseo_describe_plan_for(int(n), int(is_f64), int(num_sms), out), "describe_plan_for")
-    keys = ["i_bodies_per_thread", "threads_per_cta", "tile_records", "persistent_ctas", "i_blocks", "j_tiles",
-            "partial_slots", "kernels_per_step"]
-    return dict(zip(keys, [int(v) for v in out]))
+        _check(lib().odisseo_describe_cross_plan_for(int(n if nt is None else nt), int(n), int(is_f64), int(num_sms), out),
+               "describe_cross_plan_for")
+    return dict(zip(_PLAN_KEYS, [int(v) for v in out]))
 
 
-def plan_probe(n: int, is_f64: bool, num_sms: int, u: int, c: int):
-    out = (ctypes.c_int64 * 3)()
-    _check(lib().odisseo_plan_probe(int(n), int(is_f64), int(num_sms), int(u), int(c), out), "plan_probe")
-    return int(out[0]), int(out[1]), int(out[2])
+def plan_probe(n: int, is_f64: bool, num_sms: int, u: int, c: int, nt: Optional[int] = None):
+    """(owner CTA of unit u, first unit of CTA c, end unit of CTA c, first source of u's chunk, end source)."""
+    out = (ctypes.c_int64 * 5)()
+    _check(lib().odisseo_plan_probe(int(n if nt is None else nt), int(n), int(is_f64), int(num_sms), int(u), int(c), out),
+           "plan_probe")
+    return tuple(int(v) for v in out)
 
 
 def pair_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, eps: float, workspace: torch.Tensor, stream=None):

@@ -14,49 +14,69 @@ namespace odisseo {
 // ------------------------------- launch plan ------------------------------------------
 PairPlan make_plan(int64_t n, int is_f64, int num_sms) { return make_cross_plan(n, n, is_f64, num_sms); }
 
+// Geometry of one kernel variant: i-bodies per thread, compute threads, resident CTAs per SM.
+struct VariantGeom { int ipt, cthreads, minb; };
+static VariantGeom variant_geom(int variant, int is_f64)
+{
+    // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
+    // packed interaction chains of a thread (2 warps per scheduler x ILP 4 beats 4.5 warps x ILP 1:
+    // 68.9 % vs 60.2 % of FP32 peak at N = 262,144)
+    if (variant == 0) return VariantGeom{is_f64 ? 4 : 8, 256, 1};
+    return VariantGeom{2, 64, 8};
+}
+
+// Tile length and chunk count: functions of the SOURCE count (and the SM count) alone, so that a slice of
+// the targets evaluated anywhere adds the same numbers in the same grouping.
+// T: the longest tile the variant n would get on its own stages.  S: the busiest CTA walks
+// ceil(nb S / P) units of (chunk records + per-tile and per-row overheads, in records' worth of time); take
+// the S that minimises that product for the single-device evaluation nt = n; chunks hold >= 32 sources.
+static void source_split(int64_t n, int is_f64, int num_sms, int32_t* T_out, int32_t* S_out)
+{
+    const int variant = n <= 4096 ? 1 : 0;
+    const VariantGeom g = variant_geom(variant, is_f64);
+    const int32_t T = (variant == 0 && !is_f64) ? 512 : 256;
+    const int64_t n8 = (n + 7) / 8;
+    const int64_t nb = (n + (int64_t)g.ipt * g.cthreads - 1) / ((int64_t)g.ipt * g.cthreads);
+    const int64_t Pmax = (int64_t)num_sms * g.minb;
+    int64_t smax = n8 / 4;
+    if (smax < 1) smax = 1;
+    if (smax > 512) smax = 512;
+    int64_t best = -1;
+    int32_t S = 1;
+    for (int64_t s = 1; s <= smax; ++s) {
+        const int64_t chunk = 8 * ((n8 + s - 1) / s);
+        const int64_t tiles = (chunk + T - 1) / T;
+        const int64_t U = nb * s;
+        const int64_t ctas = U < Pmax ? U : Pmax;
+        const int64_t cost = ((U + ctas - 1) / ctas) * (chunk + 16 * tiles + 32) + 2 * s;
+        if (best < 0 || cost < best) { best = cost; S = (int32_t)s; }
+    }
+    *T_out = T;
+    *S_out = S;
+}
+
 PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
 {
     PairPlan p;
     memset(&p, 0, sizeof(p));
     p.n = n;
     p.nt = nt;
+    p.n8 = (n + 7) / 8;
+    source_split(n, is_f64, num_sms, &p.T, &p.S);
+    // the small variant's stages hold 256 records: it needs T <= 256, i.e. n <= 4,096
     p.variant = (nt <= 4096 && n <= 4096) ? 1 : 0;
-    int minb;
-    if (p.variant == 0) {
-        // fp32: one 8-warp CTA per SM with ~160 registers per thread lets ptxas interleave the four
-        // packed interaction chains of a thread (2 warps per scheduler x ILP 4 beats 4.5 warps x ILP 1:
-        // 68.9 % vs 60.2 % of FP32 peak at N = 262,144)
-        p.ipt = is_f64 ? 4 : 8;
-        p.cthreads = 256;
-        minb = 1;
-    } else {
-        p.ipt = 2;
-        p.cthreads = 64;
-        minb = 8;
-    }
+    const VariantGeom g = variant_geom(p.variant, is_f64);
+    p.ipt = g.ipt;
+    p.cthreads = g.cthreads;
     p.rec_bytes = 32;
+    p.comps = 3;
     p.IB = p.ipt * p.cthreads;
     p.nb = (int32_t)((nt + p.IB - 1) / p.IB);
-    int64_t P = (int64_t)num_sms * minb;
-    // Tile length: the busiest CTA walks ceil(U / P) units of (T + overhead) source records each
-    // (overhead = barrier hand-over + fp64 flush of the tile sums, ~16 records' worth); take the T that
-    // minimises that product.  Long tiles amortise the overhead, short ones even out the stream-K split.
-    const int32_t Tmax = (p.variant == 0 && !is_f64) ? 512 : 256;
-    int32_t T = Tmax;
-    int64_t best = -1;
-    for (int32_t t = Tmax; t >= 32; t >>= 1) {
-        const int64_t U = (int64_t)p.nb * ((n + t - 1) / t);
-        const int64_t ctas = U < P ? U : P;
-        const int64_t cost = ((U + ctas - 1) / ctas) * (t + 16);
-        if (best < 0 || cost < best) { best = cost; T = t; }
-    }
-    p.T = T;
-    p.J = (int32_t)((n + T - 1) / T);
-    p.U = (int64_t)p.nb * p.J;
+    p.U = (int64_t)p.nb * p.S;
+    int64_t P = (int64_t)num_sms * g.minb;
     if (P > p.U) P = p.U;
     if (P < 1) P = 1;
     p.P = (int32_t)P;
-    p.slots = p.P + p.nb;
     return p;
 }
 
@@ -227,10 +247,10 @@ odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, voi
     return ODISSEO_OK;
 }
 
-inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, float G, float* a, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f32(p, part, G, a, s); }
-inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, double G, double* a, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f64(p, part, G, a, s); }
+inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, const void* j, float G, float* a, cudaStream_t s)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f32(p, part, j, G, a, s); }
+inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, const void* j, double G, double* a, cudaStream_t s)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f64(p, part, j, G, a, s); }
 
 // Acceleration at nt target positions due to n sources (targets need not be sources; their masses are ignored).
 template <typename T>
@@ -264,7 +284,7 @@ odisseo_status pair_cross_impl(const T* targets, int64_t nt, const T* sources, i
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_pair(plan, targets, cv.jsrc, cv.partials, eps, s);
     if (e != cudaSuccess) return cuda_fail(e);
-    e = launch_reduce_rows(plan, cv.partials, G, acc, s);
+    e = launch_reduce_rows(plan, cv.partials, cv.jsrc, G, acc, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -447,12 +467,12 @@ odisseo_status kick_drift_impl(T* posm, T* vel, const T* acc, int64_t n, T G, T 
 
 inline cudaError_t launch_diag_stage(const PairPlan& p, const float* x, void* j, cudaStream_t s) { return launch_diag_stage_f32(p, x, j, s); }
 inline cudaError_t launch_diag_stage(const PairPlan& p, const double* x, void* j, cudaStream_t s) { return launch_diag_stage_f64(p, x, j, s); }
-inline cudaError_t launch_diag_terms(const PairPlan& p, const float* x, const float* v, const double* part, double G, double eps,
-                                     const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
-{ return launch_diag_terms_f32(p, x, v, part, G, eps, pot, bs, phi, s); }
-inline cudaError_t launch_diag_terms(const PairPlan& p, const double* x, const double* v, const double* part, double G, double eps,
-                                     const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
-{ return launch_diag_terms_f64(p, x, v, part, G, eps, pot, bs, phi, s); }
+inline cudaError_t launch_diag_terms(const PairPlan& p, const float* x, const float* v, const double* part, const void* j, double G,
+                                     double eps, const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
+{ return launch_diag_terms_f32(p, x, v, part, j, G, eps, pot, bs, phi, s); }
+inline cudaError_t launch_diag_terms(const PairPlan& p, const double* x, const double* v, const double* part, const void* j, double G,
+                                     double eps, const PotParams<double>& pot, double* bs, double* phi, cudaStream_t s)
+{ return launch_diag_terms_f64(p, x, v, part, j, G, eps, pot, bs, phi, s); }
 
 inline size_t diag_block_sum_bytes(int64_t n)
 { return ((size_t)((n + STEP_THREADS - 1) / STEP_THREADS) * DIAG_VALUES * sizeof(double) + 255) & ~(size_t)255; }
@@ -495,7 +515,7 @@ odisseo_status diagnostics_impl(const T* posm, const T* vel, int64_t n, T G, T e
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_potential_f64(plan, cv.jsrc, cv.partials, (double)eps, s);
     if (e != cudaSuccess) return cuda_fail(e);
-    e = launch_diag_terms(plan, posm, vel, cv.partials, (double)G, (double)eps, pp, block_sums, phi, s);
+    e = launch_diag_terms(plan, posm, vel, cv.partials, cv.jsrc, (double)G, (double)eps, pp, block_sums, phi, s);
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_diag_final(block_sums, (int)((n + STEP_THREADS - 1) / STEP_THREADS), out, s);
     if (e != cudaSuccess) return cuda_fail(e);
@@ -717,20 +737,22 @@ odisseo_status odisseo_profile_end(double* h_ms_total, int64_t* h_launches, int6
     return ODISSEO_OK;
 }
 
-size_t odisseo_workspace_bytes(int64_t n, int is_f64)
-{
-    if (n <= 0) return 0;
-    // bound over devices with up to 192 SMs: more CTAs -> more partial rows, smaller tiles -> same padding bound
-    const PairPlan p = make_plan(n, is_f64, 192);
-    const size_t jsrc = (((size_t)(n + 512) * p.rec_bytes + ((size_t)(n + 512) / STEP_THREADS + 1) * sizeof(int)) + 255) & ~(size_t)255;
-    return jsrc + (size_t)p.slots * 3 * p.IB * sizeof(double);
-}
+size_t odisseo_workspace_bytes(int64_t n, int is_f64) { return odisseo_cross_workspace_bytes(n, n, is_f64); }
 
 size_t odisseo_cross_workspace_bytes(int64_t nt, int64_t n, int is_f64)
 {
     if (n <= 0 || nt <= 0) return 0;
     size_t best = 0;
-    for (int sms = 64; sms <= 192; sms += 4) {            // bound over devices with up to 192 SMs
+    int lo = 64, hi = 192;                                // bound over devices with 64 to 192 SMs ...
+    {
+        int dev = -1, sms = 0;                            // ... or exactly the current device when there is one
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+            sms > 0)
+            lo = hi = sms;
+        else
+            (void)cudaGetLastError();
+    }
+    for (int sms = lo; sms <= hi; ++sms) {
         const PairPlan p = make_cross_plan(nt, n, is_f64, sms);
         const size_t b = plan_jsrc_bytes(p) + plan_partial_bytes(p);
         if (b > best) best = b;
@@ -748,15 +770,18 @@ odisseo_status odisseo_pair_accel_cross_f64(const double* d_targets, int64_t nt,
                                             void* stream)
 { return pair_cross_impl<double>(d_targets, nt, d_sources, n, d_acc, G, eps, d_workspace, workspace_bytes, stream); }
 
-odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8])
+odisseo_status odisseo_describe_cross_plan_for(int64_t nt, int64_t n, int is_f64, int num_sms, int64_t out[8])
 {
     if (!out) return ODISSEO_ERR_NULL;
-    if (n <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
-    const PairPlan p = make_plan(n, is_f64, num_sms);
+    if (n <= 0 || nt <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
+    const PairPlan p = make_cross_plan(nt, n, is_f64, num_sms);
     out[0] = p.ipt; out[1] = p.cthreads + 32; out[2] = p.T; out[3] = p.P;
-    out[4] = p.nb; out[5] = p.J; out[6] = p.slots; out[7] = 2;
+    out[4] = p.nb; out[5] = p.S; out[6] = p.U; out[7] = 2;
     return ODISSEO_OK;
 }
+
+odisseo_status odisseo_describe_plan_for(int64_t n, int is_f64, int num_sms, int64_t out[8])
+{ return odisseo_describe_cross_plan_for(n, n, is_f64, num_sms, out); }
 
 odisseo_status odisseo_describe_plan(int64_t n, int is_f64, int64_t out[8])
 {
@@ -767,17 +792,19 @@ odisseo_status odisseo_describe_plan(int64_t n, int is_f64, int64_t out[8])
     return odisseo_describe_plan_for(n, is_f64, dev.sms, out);
 }
 
-// Host-side check of the stream-K bookkeeping for tests: for unit u returns the owning CTA,
-// and for CTA c its [start, end) range, exactly as the kernels compute them.
-odisseo_status odisseo_plan_probe(int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[3])
+// Host-side check of the unit bookkeeping for tests: for unit u the owning CTA and the source records of its
+// chunk, and for CTA c its [start, end) unit range, exactly as the kernels compute them.
+odisseo_status odisseo_plan_probe(int64_t nt, int64_t n, int is_f64, int num_sms, int64_t u, int64_t c, int64_t out[5])
 {
     if (!out) return ODISSEO_ERR_NULL;
-    if (n <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
-    const PairPlan p = make_plan(n, is_f64, num_sms);
+    if (n <= 0 || nt <= 0 || num_sms <= 0) return ODISSEO_ERR_ARG;
+    const PairPlan p = make_cross_plan(nt, n, is_f64, num_sms);
     if (u < 0 || u >= p.U || c < 0 || c >= p.P) return ODISSEO_ERR_ARG;
     out[0] = plan_owner(p, u);
     out[1] = plan_start(p, c);
     out[2] = plan_start(p, c + 1);
+    out[3] = plan_chunk_lo(p, u % p.S);
+    out[4] = plan_chunk_lo(p, u % p.S + 1);
     return ODISSEO_OK;
 }
 

@@ -73,8 +73,8 @@ __device__ __forceinline__ double block_sum(double v, double* warp_scratch)
 template <typename T>
 __global__ void __launch_bounds__(STEP_THREADS)
 diag_terms_kernel(const typename DVec4<T>::type* __restrict__ posm, const typename DVec4<T>::type* __restrict__ vel,
-                  const double* __restrict__ partials, const PairPlan plan, const double G, const double eps,
-                  const PotParams<double> pot, double* __restrict__ block_sums, double* __restrict__ phi_out)
+                  const double* __restrict__ partials, const void* __restrict__ jsrc, const PairPlan plan, const double G,
+                  const double eps, const PotParams<double> pot, double* __restrict__ block_sums, double* __restrict__ phi_out)
 {
     __shared__ double warp_scratch[STEP_THREADS / 32];
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -85,12 +85,9 @@ diag_terms_kernel(const typename DVec4<T>::type* __restrict__ posm, const typena
         const typename DVec4<T>::type p = posm[i];
         const typename DVec4<T>::type w = vel[i];
         const double x = p.x, y = p.y, z = p.z, m = p.w, vx = w.x, vy = w.y, vz = w.z;
-        const int32_t b = (int32_t)(i / plan.IB);
-        const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
-        const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
-        const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
-        double sum = 0.0;
-        for (int32_t c = c0; c <= c1; ++c) sum += __ldcg(partials + (size_t)(c + b) * 3 * plan.IB + r);   // increasing j
+        double rows[1];
+        reduce_unit_rows<1>(partials, plan, i, rows);                    // increasing j, fixed grouping
+        const double sum = plan_row_mass<double>(jsrc, plan) * rows[0];
         const double phi = -G * (sum - m / eps);       // the kernel's self term is m_i (0 + eps^2)^-1/2
         if (phi_out) phi_out[i] = phi;
         val[0] = 0.5 * m * fma(vx, vx, fma(vy, vy, vz * vz));
@@ -146,20 +143,20 @@ cudaError_t launch_diag_stage_f64(const PairPlan& plan, const double* posm, void
     return cudaGetLastError();
 }
 cudaError_t launch_diag_terms_f32(const PairPlan& plan, const float* posm, const float* vel, const double* partials,
-                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  const void* jsrc, double G, double eps, const PotParams<double>& pot, double* block_sums,
                                   double* phi_out, cudaStream_t stream)
 {
     diag_terms_kernel<float><<<grid_for(plan.n), STEP_THREADS, 0, stream>>>(
-        reinterpret_cast<const float4*>(posm), reinterpret_cast<const float4*>(vel), partials, plan, G, eps, pot,
+        reinterpret_cast<const float4*>(posm), reinterpret_cast<const float4*>(vel), partials, jsrc, plan, G, eps, pot,
         block_sums, phi_out);
     return cudaGetLastError();
 }
 cudaError_t launch_diag_terms_f64(const PairPlan& plan, const double* posm, const double* vel, const double* partials,
-                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  const void* jsrc, double G, double eps, const PotParams<double>& pot, double* block_sums,
                                   double* phi_out, cudaStream_t stream)
 {
     diag_terms_kernel<double><<<grid_for(plan.n), STEP_THREADS, 0, stream>>>(
-        reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(vel), partials, plan, G, eps, pot,
+        reinterpret_cast<const double4*>(posm), reinterpret_cast<const double4*>(vel), partials, jsrc, plan, G, eps, pot,
         block_sums, phi_out);
     return cudaGetLastError();
 }

@@ -67,31 +67,14 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
         } else {
             T apx, apy, apz;
             if (REDUCE) {
-                const int32_t b = (int32_t)(i / plan.IB);
-                const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
-                const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
-                const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
-                double sx = 0.0, sy = 0.0, sz = 0.0;
-                // fixed order: increasing j.  Rows are fetched REDUCE_BATCH at a time so the L2 latencies
-                // of a batch overlap (a plain loop serialises one ~1 us round trip per row: 32 rows at
-                // N = 1,024); absent rows add +0.0, which leaves the sum unchanged.
-                constexpr int REDUCE_BATCH = 8;
-                for (int32_t c = c0; c <= c1; c += REDUCE_BATCH) {
-                    double vx[REDUCE_BATCH], vy[REDUCE_BATCH], vz[REDUCE_BATCH];
-#pragma unroll
-                    for (int k = 0; k < REDUCE_BATCH; ++k) {
-                        const bool live = c + k <= c1;
-                        const double* row = partials + (size_t)(c + (live ? k : 0) + b) * 3 * plan.IB;
-                        vx[k] = live ? __ldcg(row + r) : 0.0;
-                        vy[k] = live ? __ldcg(row + plan.IB + r) : 0.0;
-                        vz[k] = live ? __ldcg(row + 2 * plan.IB + r) : 0.0;
-                    }
-#pragma unroll
-                    for (int k = 0; k < REDUCE_BATCH; ++k) { sx += vx[k]; sy += vy[k]; sz += vz[k]; }
-                }
-                apx = (T)((double)G * sx);
-                apy = (T)((double)G * sy);
-                apz = (T)((double)G * sz);
+                // fixed order: the S rows of this i-block in increasing s, then the factors left out of the rows
+                double sum[3];
+                reduce_unit_rows<3>(partials, plan, i, sum);
+                const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
+                const double sx = sum[0], sy = sum[1], sz = sum[2];
+                apx = (T)(gm * sx);
+                apy = (T)(gm * sy);
+                apz = (T)(gm * sz);
                 V4 a; a.x = apx; a.y = apy; a.z = apz; a.w = (T)0;
                 acc[i] = a;
             } else {
@@ -132,22 +115,17 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
 // Fixed-order row reduce alone (cross call: the targets are not the staged sources): acc_i = G * sum of rows.
 template <typename T>
 __global__ void __launch_bounds__(STEP_THREADS)
-reduce_rows_kernel(const double* __restrict__ partials, const PairPlan plan, const T G, typename Vec4<T>::type* __restrict__ acc)
+reduce_rows_kernel(const double* __restrict__ partials, const void* __restrict__ jsrc, const PairPlan plan, const T G,
+                   typename Vec4<T>::type* __restrict__ acc)
 {
     pdl_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= plan.nt) return;
-    const int32_t b = (int32_t)(i / plan.IB);
-    const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
-    const int32_t c0 = plan_owner(plan, (int64_t)b * plan.J);
-    const int32_t c1 = plan_owner(plan, (int64_t)(b + 1) * plan.J - 1);
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    for (int32_t c = c0; c <= c1; ++c) {                   // increasing j
-        const double* row = partials + (size_t)(c + b) * 3 * plan.IB;
-        sx += __ldcg(row + r); sy += __ldcg(row + plan.IB + r); sz += __ldcg(row + 2 * plan.IB + r);
-    }
+    double sum[3];
+    reduce_unit_rows<3>(partials, plan, i, sum);
+    const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
     typename Vec4<T>::type a;
-    a.x = (T)((double)G * sx); a.y = (T)((double)G * sy); a.z = (T)((double)G * sz); a.w = (T)0;
+    a.x = (T)(gm * sum[0]); a.y = (T)(gm * sum[1]); a.z = (T)(gm * sum[2]); a.w = (T)0;
     acc[i] = a;
 }
 
@@ -221,14 +199,16 @@ cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, dou
                       reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
 }
 
-cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, float G, float* acc, cudaStream_t stream)
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,
+                                   cudaStream_t stream)
 {
-    return launch_pdl(reduce_rows_kernel<float>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, plan, G,
+    return launch_pdl(reduce_rows_kernel<float>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, plan, G,
                       reinterpret_cast<float4*>(acc));
 }
-cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, double G, double* acc, cudaStream_t stream)
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, double G, double* acc,
+                                   cudaStream_t stream)
 {
-    return launch_pdl(reduce_rows_kernel<double>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, plan, G,
+    return launch_pdl(reduce_rows_kernel<double>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, plan, G,
                       reinterpret_cast<double4*>(acc));
 }
 

@@ -13,27 +13,33 @@ namespace odisseo {
 // ---------------------------------------------------------------------------------------
 // Launch plan.  The nt x n interaction matrix (nt = n except for the cross
 // call) is cut into nb = ceil(nt / IB) i-blocks (IB targets held in registers by one CTA) times
-// J = ceil(n / T) j-tiles (T source records staged through shared memory per TMA copy).
-// The U = nb * J units are numbered u = b * J + t and dealt to P persistent CTAs in
-// contiguous, equal (+-1) ranges: CTA c owns [start(c), start(c+1)), start(c) = floor(c*U/P).
-// A CTA therefore walks a few consecutive i-blocks ("segments"); each segment writes one
-// row of partial sums into slot (c + b), and the reduce step adds the rows of an i-block in
-// increasing c (= increasing j) order: fixed order, no atomics, bit-reproducible.
+// S source chunks.  The chunk boundaries are a function of n alone: with n8 = ceil(n / 8) source
+// octets, chunk s holds the records [8 floor(s n8 / S), 8 floor((s+1) n8 / S)), and a chunk is
+// walked in tiles of at most T records (one TMA copy each).  The U = nb * S units are numbered
+// u = b * S + s and dealt to P persistent CTAs in contiguous, equal (+-1) ranges: CTA c owns
+// [start(c), start(c+1)), start(c) = floor(c*U/P).  Every unit writes its own row of partial sums
+// (row index = u), and the reduce step adds the S rows of an i-block in increasing s: the value
+// a target receives is  G m0 sum_s ( sum_{tiles of chunk s} fp32 tile sum ),  a fixed grouping
+// that depends on n only -- not on the number of targets, CTAs or ranks (SURVEY.md 8f NEXT-1:
+// "same fixed reduction order per i"), with no atomics: bit-reproducible.
+// S is chosen on the host so that nb(n) * S is a multiple of the CTA count when that is cheap
+// (148 = 4 * 37: S = 37 at n = 2^18 gives 32 equal units per CTA): no wave-quantisation tail.
 // ---------------------------------------------------------------------------------------
 struct PairPlan {
-    int64_t n;        // source particles (staged, tiled along j)
+    int64_t n;        // source particles (staged, chunked along j)
     int64_t nt;       // target particles (held in registers, blocked along i); == n except for the cross call
-    int64_t U;        // work units = nb * J
+    int64_t n8;       // source octets = ceil(n / 8); the staged array holds 8 * n8 records
+    int64_t U;        // work units = nb * S = rows of the partial buffer
     int32_t IB;       // targets per i-block = ipt * cthreads
-    int32_t T;        // source records per j-tile
-    int32_t J;        // j-tiles
+    int32_t T;        // most source records per tile (a function of n)
+    int32_t S;        // source chunks (a function of n and the SM count)
     int32_t nb;       // i-blocks
     int32_t P;        // persistent CTAs (grid size)
     int32_t ipt;      // i-bodies per thread
     int32_t cthreads; // compute threads per CTA (one extra producer warp is added at launch)
     int32_t variant;  // 0 = large (8 compute warps), 1 = small (2 compute warps)
-    int32_t slots;    // rows in the partial buffer = P + nb
     int32_t rec_bytes;// bytes per staged source record
+    int32_t comps;    // planes of IB doubles per row (3: x, y, z sums)
 };
 
 __host__ __device__ __forceinline__ int64_t plan_start(const PairPlan& p, int64_t c) {
@@ -44,28 +50,77 @@ __host__ __device__ __forceinline__ int32_t plan_owner(const PairPlan& p, int64_
     int64_t c = ((u + 1) * p.P + p.U - 1) / p.U - 1;
     return (int32_t)(c < p.P - 1 ? c : p.P - 1);
 }
-__host__ __device__ __forceinline__ int64_t plan_npad(const PairPlan& p) { return (int64_t)p.J * p.T; }
+// First record of source chunk s (s = S gives the end of the staged array).
+__host__ __device__ __forceinline__ int64_t plan_chunk_lo(const PairPlan& p, int64_t s) {
+    return 8 * ((s * p.n8) / p.S);
+}
+__host__ __device__ __forceinline__ int64_t plan_npad(const PairPlan& p) { return 8 * p.n8; }
 // Equal-mass detection: the kernel that stages the sources also writes one
 // int per block of STEP_THREADS particles, non-zero when some mass in the block differs from
-// posm[0].m.  The flags sit behind the staged records; the pair kernels OR them at start-up.
+// posm[0].m.  The flags sit behind the staged records; the pair kernels OR them at start-up and CTA 0
+// records the decision in the word behind the flags (1 = the rows were summed without the mass factor:
+// the reduce step multiplies by the mass of staged record 0).
 constexpr int STEP_THREADS = 256;
 __host__ __device__ __forceinline__ int32_t plan_nflags(const PairPlan& p) {
     return (int32_t)((plan_npad(p) + STEP_THREADS - 1) / STEP_THREADS);
 }
 __host__ __device__ __forceinline__ size_t plan_jsrc_bytes(const PairPlan& p) {
-    size_t b = (size_t)plan_npad(p) * p.rec_bytes + (size_t)plan_nflags(p) * sizeof(int);
+    size_t b = (size_t)plan_npad(p) * p.rec_bytes + ((size_t)plan_nflags(p) + 1) * sizeof(int);
     return (b + 255) & ~(size_t)255;
 }
 __host__ __device__ __forceinline__ const int* plan_flags(const void* jsrc, const PairPlan& p) {
     return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) + (size_t)plan_npad(p) * p.rec_bytes);
+}
+__host__ __device__ __forceinline__ const int* plan_eqm_word(const void* jsrc, const PairPlan& p) {
+    return plan_flags(jsrc, p) + plan_nflags(p);
 }
 // Padding records of the staged source array: zero mass, parked so far away that the softened
 // inverse cube underflows to exactly 0 (ftz) -- they contribute 0 with or without the mass factor.
 constexpr float PAD_POS_F32 = 3.0e18f;
 constexpr double PAD_POS_F64 = 1.0e150;
 __host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p) {
-    return (size_t)p.slots * 3 * p.IB * sizeof(double);
+    return (size_t)p.U * p.comps * p.IB * sizeof(double);
 }
+
+#if defined(__CUDACC__)
+// Reduce step: the S rows of target i's i-block added in increasing s (fixed order), NCOMP planes.
+// Rows are fetched REDUCE_BATCH at a time so the L2 latencies of a batch overlap (a plain loop serialises
+// one ~1 us round trip per row); absent rows add +0.0, which leaves the sum unchanged.
+template <int NCOMP>
+__device__ __forceinline__ void reduce_unit_rows(const double* __restrict__ partials, const PairPlan& plan, const int64_t i,
+                                                 double (&sum)[NCOMP])
+{
+    constexpr int REDUCE_BATCH = 8;
+    const int32_t b = (int32_t)(i / plan.IB);
+    const int32_t r = (int32_t)(i - (int64_t)b * plan.IB);
+    const size_t stride = (size_t)plan.comps * plan.IB;
+    const double* base = partials + (size_t)b * plan.S * stride + r;
+#pragma unroll
+    for (int k = 0; k < NCOMP; ++k) sum[k] = 0.0;
+    for (int32_t s = 0; s < plan.S; s += REDUCE_BATCH) {
+        double v[REDUCE_BATCH][NCOMP];
+#pragma unroll
+        for (int q = 0; q < REDUCE_BATCH; ++q) {
+            const bool live = s + q < plan.S;
+            const double* row = base + (size_t)(s + (live ? q : 0)) * stride;
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) v[q][k] = live ? __ldcg(row + (size_t)k * plan.IB) : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < REDUCE_BATCH; ++q)
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) sum[k] += v[q][k];
+    }
+}
+// Factor the pair kernel left out of the rows: the common mass when it took the equal-mass loop, else 1.
+template <typename T>
+__device__ __forceinline__ double plan_row_mass(const void* __restrict__ jsrc, const PairPlan& plan)
+{
+    if (__ldcg(plan_eqm_word(jsrc, plan)) == 0) return 1.0;
+    // mass of staged record 0: fp32 records are {x,x,y,y},{z,z,m,m}; fp64 records {x,y,z,m}
+    return sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 6) : __ldcg(static_cast<const double*>(jsrc) + 3);
+}
+#endif
 
 PairPlan make_plan(int64_t n, int is_f64, int num_sms);
 PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms);   // nt targets against n sources
@@ -240,8 +295,10 @@ cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const Pot
 cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
                                 int64_t n, cudaStream_t stream);
 cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
-cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, float G, float* acc, cudaStream_t stream);
-cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, double G, double* acc, cudaStream_t stream);
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,
+                                   cudaStream_t stream);
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, double G, double* acc,
+                                   cudaStream_t stream);
 cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double* partials, double eps,
                                  cudaStream_t stream);
 // diagnostics.cu: stage (promote to double) / per-particle terms + block sums / final fixed-order sum
@@ -249,10 +306,10 @@ constexpr int DIAG_VALUES = 16;
 cudaError_t launch_diag_stage_f32(const PairPlan& plan, const float* posm, void* jsrc, cudaStream_t stream);
 cudaError_t launch_diag_stage_f64(const PairPlan& plan, const double* posm, void* jsrc, cudaStream_t stream);
 cudaError_t launch_diag_terms_f32(const PairPlan& plan, const float* posm, const float* vel, const double* partials,
-                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  const void* jsrc, double G, double eps, const PotParams<double>& pot, double* block_sums,
                                   double* phi_out, cudaStream_t stream);
 cudaError_t launch_diag_terms_f64(const PairPlan& plan, const double* posm, const double* vel, const double* partials,
-                                  double G, double eps, const PotParams<double>& pot, double* block_sums,
+                                  const void* jsrc, double G, double eps, const PotParams<double>& pot, double* block_sums,
                                   double* phi_out, cudaStream_t stream);
 cudaError_t launch_diag_final(const double* block_sums, int nblocks, double* out, cudaStream_t stream);
 // adjoint.cu

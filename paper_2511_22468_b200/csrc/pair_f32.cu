@@ -1,69 +1,65 @@
 // fp32 all-pairs Plummer-softened acceleration (section 1; SURVEY.md 8a rows a1, a1').
 //
-//   partial_i = sum_{j in segment} m_j (x_j - x_i) (|x_j - x_i|^2 + eps^2)^{-3/2}      (G applied in the reduce step)
+//   row(b, s)_i = sum_{j in chunk s} m_j (x_j - x_i) (|x_j - x_i|^2 + eps^2)^{-3/2}      (G applied in the reduce step)
 //
 // Design (B200-first, not the paper's XLA broadcast):
 //   * persistent grid, one 9-warp CTA per SM (8 compute warps + 1 producer warp, ~160 registers per
-//     thread so that ptxas interleaves a thread's four interaction chains), stream-K split of the
-//     (i-block x j-tile) space
-//     (odisseo_common.cuh) -> every SM busy for any N, no wave-quantisation tail;
-//   * source tiles arrive by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx) issued by
-//     a dedicated producer warp into a STAGES-deep ring; consumers release a stage with one
-//     mbarrier arrive per warp -- no __syncthreads in the main loop;
+//     thread so that ptxas interleaves a thread's four interaction chains), contiguous equal ranges of
+//     (i-block x source-chunk) units per CTA, source tiles through a TMA ring (pair_stream.cuh)
+//     -> every SM busy for any N, no wave-quantisation tail;
 //   * each compute thread keeps 2*NPAIR targets in registers as packed f32x2 pairs; sources are
 //     staged pre-duplicated {x,x,y,y},{z,z,m,m} so that one LDS.128 yields two ready packed
 //     operands and the body is 3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per TWO interactions
 //     (half the issue slots of the scalar form, no register-pair MOVs);
 //   * two-level summation: fp32 inside one tile (<= 512 terms), promoted to fp64 between tiles
-//     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18);
+//     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18); one row of
+//     fp64 sums per unit, rows added in unit order by the reduce step (fixed grouping, function of n only);
 //   * the self term contributes exactly 0 because eps > 0; padding records are massless and parked at
 //     3e18, where the inverse cube underflows to exactly 0 (ftz), so they vanish on both paths;
 //   * equal masses (the paper's Plummer progenitors, PAPER.md:L43 step 3) are detected on the device by
-//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2;
+//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2, and the
+//     reduce step multiplies by the mass once;
 //   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
-#include "odisseo_common.cuh"
+#include "pair_stream.cuh"
 
 namespace odisseo {
 
 namespace {
 
-constexpr int STAGES = 4;
+template <int NPAIR, int CWARPS_, int MINB_, int JUNROLL>
+struct PairF32 {
+    static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 32, COMPS = 3;
+    static constexpr int CTHREADS = CWARPS * 32;
+    struct Params { const float4* posm; float eps2; };
+    static size_t outer_bytes() { return (size_t)6 * NPAIR * CTHREADS * sizeof(double); }
 
-// Consumer side of the pair kernel for one CTA.  EQM = all masses equal (detected on the device by
-// the staging kernel): the per-source mass factor leaves the inner loop (11 instead of 12 packed FP32
-// ops per two interactions) and multiplies the fp64 sums once per segment.
-template <int NPAIR, int CWARPS, int JUNROLL, bool EQM>
-__device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, const uint4* __restrict__ jsrc,
-                                              double* __restrict__ partials,
-                                              const PairPlan& plan, const float eps2, unsigned char* smem_raw,
-                                              uint64_t* full_bar, uint64_t* empty_bar, const int64_t c,
-                                              const int64_t u0, const int64_t u1, const uint32_t tile_bytes)
-{
-    constexpr int CTHREADS = CWARPS * 32;
-    const int tid = threadIdx.x;
-    const int lane = tid & 31;
-    const double m0 = EQM ? (double)__ldg(reinterpret_cast<const float*>(jsrc) + 6) : 1.0;   // mass of staged record 0
-    const f32x2 e2 = pk(eps2, eps2);
-    f32x2 xi[NPAIR], yi[NPAIR], zi[NPAIR];
-    f32x2 ax[NPAIR], ay[NPAIR], az[NPAIR];
-    // fp64 outer sums live in shared memory (48 registers otherwise): osum[k][tid], k = 3*(2p+h)+comp
-    double* __restrict__ osum = reinterpret_cast<double*>(smem_raw + (size_t)STAGES * tile_bytes) + tid;
+    // EQM = all masses equal (detected on the device by the staging kernel): the per-source mass factor
+    // leaves the inner loop (11 instead of 12 packed FP32 ops per two interactions).
+    template <bool EQM>
+    struct State {
+        const float4* __restrict__ posm;
+        const int64_t nt;
+        const int32_t IB;
+        const f32x2 e2;
+        // fp64 outer sums live in shared memory (48 registers otherwise): osum[k][tid], k = 3*(2p+h)+comp
+        double* __restrict__ osum;
+        f32x2 xi[NPAIR], yi[NPAIR], zi[NPAIR];
+        f32x2 ax[NPAIR], ay[NPAIR], az[NPAIR];
 
-    int32_t b = (int32_t)(u0 / plan.J);
-    int32_t t = (int32_t)(u0 - (int64_t)b * plan.J);
-    bool seg_start = true;
-    int s = 0;
-    uint32_t ph = 0;
-
-    for (int64_t u = u0; u < u1; ++u) {
-        if (seg_start) {
-            const int64_t base = (int64_t)b * plan.IB + tid;
+        __device__ __forceinline__ State(const Params& prm, const PairPlan& plan, unsigned char* outer)
+            : posm(prm.posm), nt(plan.nt), IB(plan.IB), e2(pk(prm.eps2, prm.eps2)),
+              osum(reinterpret_cast<double*>(outer) + threadIdx.x)
+        {
+        }
+        __device__ __forceinline__ void load_targets(const int32_t b)
+        {
+            const int64_t base = (int64_t)b * IB + threadIdx.x;
 #pragma unroll
             for (int p = 0; p < NPAIR; ++p) {
                 int64_t i0 = base + (int64_t)(2 * p) * CTHREADS;
                 int64_t i1 = i0 + CTHREADS;
-                i0 = i0 < plan.nt ? i0 : plan.nt - 1;     // clamped rows are computed and never read back
-                i1 = i1 < plan.nt ? i1 : plan.nt - 1;
+                i0 = i0 < nt ? i0 : nt - 1;               // clamped rows are computed and never read back
+                i1 = i1 < nt ? i1 : nt - 1;
                 const float4 p0 = __ldg(posm + i0);
                 const float4 p1 = __ldg(posm + i1);
                 // x + (-0) == x exactly; routing the pack through FADD2 makes the pair a native 64-bit
@@ -74,167 +70,84 @@ __device__ __forceinline__ void consume_tiles(const float4* __restrict__ posm, c
                 zi[p] = add2(pk(p0.z, p1.z), nz);
                 ax[p] = ay[p] = az[p] = 0ull;
             }
+        }
+        __device__ __forceinline__ void zero_outer()
+        {
 #pragma unroll
             for (int k = 0; k < 6 * NPAIR; ++k) osum[k * CTHREADS] = 0.0;
-            seg_start = false;
         }
-
-        mbar_wait(&full_bar[s], ph);
-        const ulonglong2* __restrict__ tile = reinterpret_cast<const ulonglong2*>(smem_raw + (size_t)s * tile_bytes);
+        __device__ __forceinline__ void tile(const unsigned char* tile_raw, const int len)
+        {
+            const ulonglong2* __restrict__ t = reinterpret_cast<const ulonglong2*>(tile_raw);
 #pragma unroll JUNROLL
-        for (int j = 0; j < plan.T; ++j) {
-            const ulonglong2 A = tile[2 * j];        // {x,x},{y,y}
-            const ulonglong2 B = tile[2 * j + 1];    // {z,z},{m,m}
+            for (int j = 0; j < len; ++j) {
+                const ulonglong2 A = t[2 * j];        // {x,x},{y,y}
+                const ulonglong2 B = t[2 * j + 1];    // {z,z},{m,m}
+#pragma unroll
+                for (int p = 0; p < NPAIR; ++p) {
+                    const f32x2 dx = sub2(A.x, xi[p]);
+                    const f32x2 dy = sub2(A.y, yi[p]);
+                    const f32x2 dz = sub2(B.x, zi[p]);
+                    f32x2 r2 = fma2(dx, dx, e2);
+                    r2 = fma2(dy, dy, r2);
+                    r2 = fma2(dz, dz, r2);
+                    float r2l, r2h;
+                    unpk(r2, r2l, r2h);
+                    const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
+                    const f32x2 ri2 = mul2(ri, ri);
+                    const f32x2 w = mul2(ri2, EQM ? ri : mul2(B.y, ri));
+                    ax[p] = fma2(w, dx, ax[p]);
+                    ay[p] = fma2(w, dy, ay[p]);
+                    az[p] = fma2(w, dz, az[p]);
+                }
+            }
+        }
+        // second summation level: promote the tile sums to fp64
+        __device__ __forceinline__ void flush_tile()
+        {
 #pragma unroll
             for (int p = 0; p < NPAIR; ++p) {
-                const f32x2 dx = sub2(A.x, xi[p]);
-                const f32x2 dy = sub2(A.y, yi[p]);
-                const f32x2 dz = sub2(B.x, zi[p]);
-                f32x2 r2 = fma2(dx, dx, e2);
-                r2 = fma2(dy, dy, r2);
-                r2 = fma2(dz, dz, r2);
-                float r2l, r2h;
-                unpk(r2, r2l, r2h);
-                const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
-                const f32x2 ri2 = mul2(ri, ri);
-                const f32x2 w = mul2(ri2, EQM ? ri : mul2(B.y, ri));
-                ax[p] = fma2(w, dx, ax[p]);
-                ay[p] = fma2(w, dy, ay[p]);
-                az[p] = fma2(w, dz, az[p]);
+                float lo, hi;
+                unpk(ax[p], lo, hi); osum[(6 * p + 0) * CTHREADS] += (double)lo; osum[(6 * p + 3) * CTHREADS] += (double)hi;
+                unpk(ay[p], lo, hi); osum[(6 * p + 1) * CTHREADS] += (double)lo; osum[(6 * p + 4) * CTHREADS] += (double)hi;
+                unpk(az[p], lo, hi); osum[(6 * p + 2) * CTHREADS] += (double)lo; osum[(6 * p + 5) * CTHREADS] += (double)hi;
+                ax[p] = ay[p] = az[p] = 0ull;
             }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty_bar[s]);
-        if (++s == STAGES) { s = 0; ph ^= 1u; }
-
-        // second summation level: promote the tile sums to fp64
-#pragma unroll
-        for (int p = 0; p < NPAIR; ++p) {
-            float lo, hi;
-            unpk(ax[p], lo, hi); osum[(6 * p + 0) * CTHREADS] += (double)lo; osum[(6 * p + 3) * CTHREADS] += (double)hi;
-            unpk(ay[p], lo, hi); osum[(6 * p + 1) * CTHREADS] += (double)lo; osum[(6 * p + 4) * CTHREADS] += (double)hi;
-            unpk(az[p], lo, hi); osum[(6 * p + 2) * CTHREADS] += (double)lo; osum[(6 * p + 5) * CTHREADS] += (double)hi;
-            ax[p] = ay[p] = az[p] = 0ull;
-        }
-
-        const bool seg_end = (t == plan.J - 1) || (u == u1 - 1);
-        if (seg_end) {
-            double* row = partials + (size_t)(c + b) * 3 * plan.IB;
+        __device__ __forceinline__ void write_row(double* __restrict__ row)
+        {
 #pragma unroll
             for (int k = 0; k < 2 * NPAIR; ++k) {
-                const int r = k * CTHREADS + tid;
-                row[r] = m0 * osum[(3 * k + 0) * CTHREADS];
-                row[plan.IB + r] = m0 * osum[(3 * k + 1) * CTHREADS];
-                row[2 * plan.IB + r] = m0 * osum[(3 * k + 2) * CTHREADS];
-            }
-            seg_start = true;
-        }
-        if (++t == plan.J) { t = 0; ++b; }
-    }
-}
-
-template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
-__global__ void __launch_bounds__((CWARPS + 1) * 32, MINB)
-pair_f32x2_kernel(const float4* __restrict__ posm, const uint4* __restrict__ jsrc, double* __restrict__ partials,
-                  const PairPlan plan, const float eps2)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[STAGES];
-    __shared__ __align__(8) uint64_t empty_bar[STAGES];
-
-    const int tid = threadIdx.x;
-    const int warp = tid >> 5;
-    const int lane = tid & 31;
-    const int64_t c = blockIdx.x;
-    const int64_t u0 = plan_start(plan, c);
-    const int64_t u1 = plan_start(plan, c + 1);
-    // Let the next kernel become resident early only when this one is short (a few tiles per CTA): its
-    // CTAs then hide their launch latency behind our tail.  Behind a long evaluation, early dependents would
-    // sit on the SMs for milliseconds (measured -0.3 % at N = 262,144); there the implicit trigger at exit is used.
-    if (u1 - u0 <= 16) pdl_launch_dependents();
-    if (u0 >= u1) return;
-
-    const uint32_t tile_bytes = (uint32_t)plan.T * 32u;
-    if (tid == CWARPS * 32) {                               // the producer lane owns init and the first loads
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], CWARPS);
-        }
-        mbar_fence_init();
-    }
-    // equal-mass flags written by the staging kernel (odisseo_common.cuh): one uniform decision per grid
-    pdl_wait();                                             // the staging kernel's records and flags are complete
-    // the first STAGES tiles need no hand-over: issue them before anything else so that their latency
-    // overlaps the flag reduction and the target loads
-    const int prefetch = (int)((u1 - u0) < STAGES ? (u1 - u0) : STAGES);
-    if (tid == CWARPS * 32) {
-        int32_t t = (int32_t)(u0 % plan.J);
-        for (int s = 0; s < prefetch; ++s) {
-            mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
-            tma_load_1d(smem_raw + (size_t)s * tile_bytes,
-                        reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes, &full_bar[s]);
-            if (++t == plan.J) t = 0;
-        }
-    }
-    int differs = 0;
-    {
-        const int* __restrict__ mflags = plan_flags(jsrc, plan);
-        const int nflags = plan_nflags(plan);
-        for (int k = tid; k < nflags; k += (CWARPS + 1) * 32) differs |= __ldg(mflags + k);
-    }
-    const bool eqm = __syncthreads_or(differs) == 0;        // also publishes the mbarrier inits
-
-    if (warp == CWARPS) {
-        // ---- producer warp: one elected lane streams the CTA's tile sequence --------------
-        if (lane == 0) {
-            int s = prefetch % STAGES;
-            uint32_t ph = prefetch == STAGES ? 1u : 0u;
-            int32_t t = (int32_t)((u0 + prefetch) % plan.J);
-            for (int64_t u = u0 + prefetch; u < u1; ++u) {
-                mbar_wait_backoff(&empty_bar[s], ph ^ 1u);
-                mbar_arrive_expect_tx(&full_bar[s], tile_bytes);
-                tma_load_1d(smem_raw + (size_t)s * tile_bytes,
-                            reinterpret_cast<const unsigned char*>(jsrc) + (size_t)t * tile_bytes, tile_bytes,
-                            &full_bar[s]);
-                if (++t == plan.J) t = 0;
-                if (++s == STAGES) { s = 0; ph ^= 1u; }
+                const int r = k * CTHREADS + threadIdx.x;
+                row[r] = osum[(3 * k + 0) * CTHREADS];
+                row[IB + r] = osum[(3 * k + 1) * CTHREADS];
+                row[2 * IB + r] = osum[(3 * k + 2) * CTHREADS];
             }
         }
-        return;
-    }
+    };
+};
 
-    if (eqm)
-        consume_tiles<NPAIR, CWARPS, JUNROLL, true>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
-    else
-        consume_tiles<NPAIR, CWARPS, JUNROLL, false>(posm, jsrc, partials, plan, eps2, smem_raw, full_bar, empty_bar, c, u0, u1, tile_bytes);
-}
-
-template <int NPAIR, int CWARPS, int MINB, int JUNROLL = 4>
-cudaError_t launch_variant(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
-                           cudaStream_t stream)
-{
-    const size_t smem = (size_t)STAGES * plan.T * 32 + (size_t)6 * NPAIR * CWARPS * 32 * sizeof(double);
-    return launch_pdl(pair_f32x2_kernel<NPAIR, CWARPS, MINB, JUNROLL>, dim3(plan.P), dim3((CWARPS + 1) * 32), smem, stream,
-                      reinterpret_cast<const float4*>(posm), reinterpret_cast<const uint4*>(jsrc), partials, plan, eps * eps);
-}
+typedef PairF32<4, 8, 1, 8> LargeF32;    // 2,048 targets per CTA, one CTA per SM
+typedef PairF32<1, 2, 8, 4> SmallF32;    // 128 targets per CTA, up to 8 CTAs per SM (n <= 4,096)
 
 }  // namespace
 
 cudaError_t configure_pair_f32()
 {
-    cudaError_t e = cudaFuncSetAttribute(pair_f32x2_kernel<4, 8, 1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         STAGES * 512 * 32 + 6 * 4 * 8 * 32 * 8);
+    cudaError_t e = configure_stream<LargeF32>(512);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_f32x2_kernel<1, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                STAGES * 256 * 32 + 6 * 1 * 2 * 32 * 8);
+    return configure_stream<SmallF32>(256);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
                             cudaStream_t stream)
 {
-    if (plan.variant == 0) return launch_variant<4, 8, 1, 8>(plan, posm, jsrc, partials, eps, stream);
-    return launch_variant<1, 2, 8>(plan, posm, jsrc, partials, eps, stream);
+    if (plan.variant == 0) {
+        const LargeF32::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
+        return launch_stream<LargeF32>(plan, prm, jsrc, partials, stream);
+    }
+    const SmallF32::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
+    return launch_stream<SmallF32>(plan, prm, jsrc, partials, stream);
 }
 
 }  // namespace odisseo

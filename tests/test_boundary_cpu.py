@@ -43,32 +43,32 @@ def test_workspace_bytes_is_monotone_and_bounds_every_plan(lib):
     for n in (1, 2, 127, 1024, 4096, 4097, 16384, 65536, 262144, 1048576):
         for f64 in (False, True):
             w = B.workspace_bytes(n, f64)
-            for sms in (1, 8, 132, 148, 160, 192):
+            for sms in (64, 132, 148, 160, 192):
                 p = B.describe_plan(n, f64, sms)
                 ib = p["i_bodies_per_thread"] * (p["threads_per_cta"] - 32)
-                need = ((p["j_tiles"] * p["tile_records"] * 32 + 255) // 256) * 256 + p["partial_slots"] * 3 * ib * 8
+                npad = 8 * -(-n // 8)
+                need = ((npad * 32 + (-(-npad // 256) + 1) * 4 + 255) // 256) * 256 + p["partial_rows"] * 3 * ib * 8
                 assert need <= w, (n, f64, sms)
         assert B.workspace_bytes(n) >= prev
         prev = B.workspace_bytes(n)
-    assert B.workspace_bytes(1048576) < 256 << 20
+    assert B.workspace_bytes(1048576) < 4 << 30
 
 
 @pytest.mark.parametrize("n,sms", [(1, 148), (33, 148), (1000, 148), (1024, 148), (4097, 148), (16384, 148),
                                    (65536, 148), (100003, 7), (262144, 148)])
 @pytest.mark.parametrize("f64", [False, True])
-def test_streamk_ranges_partition_units_and_owner_matches(n, sms, f64):
+def test_unit_ranges_partition_the_work_and_chunks_partition_the_sources(n, sms, f64):
     p = B.describe_plan(n, f64, sms)
-    P, nb, J = p["persistent_ctas"], p["i_blocks"], p["j_tiles"]
-    U = nb * J
+    P, nb, S, T = p["persistent_ctas"], p["i_blocks"], p["source_chunks"], p["max_tile_records"]
+    U = nb * S
     ib = p["i_bodies_per_thread"] * (p["threads_per_cta"] - 32)
-    assert nb == -(-n // ib) and J == -(-n // p["tile_records"]) and 1 <= P <= U
-    assert p["partial_slots"] == P + nb
-    # ranges tile [0, U) in order, sizes differ by at most one
+    assert nb == -(-n // ib) and 1 <= P <= U and p["partial_rows"] == U
+    # CTA ranges tile [0, U) in order, sizes differ by at most one
     prev_end, sizes = 0, []
     step = max(1, P // 97)
     cs = sorted(set(list(range(0, P, step)) + [0, P - 1]))
     for c in range(P) if P <= 600 else cs:
-        _, s, e = B.plan_probe(n, f64, sms, 0, c)
+        _, s, e, _, _ = B.plan_probe(n, f64, sms, 0, c)
         assert s <= e
         if P <= 600:
             assert s == prev_end
@@ -77,16 +77,47 @@ def test_streamk_ranges_partition_units_and_owner_matches(n, sms, f64):
     if P <= 600:
         assert prev_end == U
     assert max(sizes) - min(sizes) <= 1 and min(sizes) >= 1
-    # owner(u) is the CTA whose range holds u; slots c + b are distinct for distinct segments
+    # owner(u) is the CTA whose range holds u
     us = range(U) if U <= 3000 else list(range(0, U, max(1, U // 1500))) + [U - 1]
-    seen = {}
     for u in us:
-        c, _, _ = B.plan_probe(n, f64, sms, u, 0)
-        _, s, e = B.plan_probe(n, f64, sms, u, c)
+        c = B.plan_probe(n, f64, sms, u, 0)[0]
+        _, s, e, _, _ = B.plan_probe(n, f64, sms, u, c)
         assert s <= u < e
-        slot = c + u // J
-        assert seen.setdefault(slot, (c, u // J)) == (c, u // J)
-        assert slot < p["partial_slots"]
+    # the S chunks of an i-block partition the staged sources [0, 8 ceil(n/8)) in order, on multiples of 8,
+    # with sizes equal up to one octet; every chunk is non-empty
+    end = 0
+    lens = []
+    for s in range(S):
+        _, _, _, lo, hi = B.plan_probe(n, f64, sms, s, 0)
+        assert lo == end and hi > lo and lo % 8 == 0 and hi % 8 == 0
+        lens.append(hi - lo)
+        end = hi
+    assert end == 8 * -(-n // 8)
+    assert max(lens) - min(lens) <= 8
+    assert T in (256, 512)
+
+
+@pytest.mark.parametrize("n", [1000, 4096, 4097, 16384, 262144])
+@pytest.mark.parametrize("f64", [False, True])
+def test_summation_grouping_depends_on_the_source_count_only(n, f64):
+    """SURVEY 8f NEXT-1 ("same fixed reduction order per i"): tile length and chunk boundaries -- everything that fixes which
+    numbers are added in which grouping -- are the same whatever the number of targets (a rank's slice, a tracer set)."""
+    ref = B.describe_plan(n, f64, 148)
+    chunks = [B.plan_probe(n, f64, 148, s, 0)[3:] for s in range(ref["source_chunks"])]
+    for nt in (1, 7, n // 8 + 1, n // 3, n // 2, n, 3 * n):
+        p = B.describe_plan(n, f64, 148, nt=nt)
+        assert p["source_chunks"] == ref["source_chunks"] and p["max_tile_records"] == ref["max_tile_records"]
+        assert [B.plan_probe(n, f64, 148, s, 0, nt=nt)[3:] for s in range(p["source_chunks"])] == chunks
+
+
+@pytest.mark.parametrize("n", [65536, 262144, 1048576])
+def test_large_plans_have_no_wave_quantisation_tail(n):
+    """The chunk count is chosen so that the busiest CTA walks at most 1 % more units than the average
+    (N = 262,144 on 148 SMs: 128 i-blocks x 15 chunks = 1,920 units, 13 on the busiest CTA against 12.97)."""
+    p = B.describe_plan(n, False, 148)
+    U = p["i_blocks"] * p["source_chunks"]
+    assert p["persistent_ctas"] == 148
+    assert -(-U // 148) <= 1.01 * U / 148
 
 
 def test_argument_validation_happens_before_any_device_work(lib):
