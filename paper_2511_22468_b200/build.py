@@ -17,7 +17,7 @@ SOURCES = ["api.cu", "pair_f32.cu", "pair_f64.cu", "integrate.cu", "ensemble.cu"
 HEADERS = [os.path.join(CSRC, "odisseo_common.cuh"), os.path.join(CSRC, "ext_potential.cuh"), os.path.join(CSRC, "adjoint_terms.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "odisseo.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC"]
+              "-Xcompiler", "-fPIC"] + os.environ.get("ODISSEO_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

@@ -30,14 +30,10 @@ static VariantGeom variant_geom(int variant, int is_f64)
 // T: the longest tile the variant n would get on its own stages.  S: the busiest CTA walks
 // ceil(nb S / P) units of (chunk records + per-tile and per-row overheads, in records' worth of time); take
 // the S that minimises that product for the single-device evaluation nt = n; chunks hold >= 32 sources.
-static void source_split(int64_t n, int is_f64, int num_sms, int32_t* T_out, int32_t* S_out)
+static int32_t source_split(int64_t n, int32_t T, int64_t targets_per_cta, int64_t Pmax)
 {
-    const int variant = n <= 4096 ? 1 : 0;
-    const VariantGeom g = variant_geom(variant, is_f64);
-    const int32_t T = (variant == 0 && !is_f64) ? 512 : 256;
     const int64_t n8 = (n + 7) / 8;
-    const int64_t nb = (n + (int64_t)g.ipt * g.cthreads - 1) / ((int64_t)g.ipt * g.cthreads);
-    const int64_t Pmax = (int64_t)num_sms * g.minb;
+    const int64_t nb = (n + targets_per_cta - 1) / targets_per_cta;
     int64_t smax = n8 / 4;
     if (smax < 1) smax = 1;
     if (smax > 512) smax = 512;
@@ -51,8 +47,7 @@ static void source_split(int64_t n, int is_f64, int num_sms, int32_t* T_out, int
         const int64_t cost = ((U + ctas - 1) / ctas) * (chunk + 16 * tiles + 32) + 2 * s;
         if (best < 0 || cost < best) { best = cost; S = (int32_t)s; }
     }
-    *T_out = T;
-    *S_out = S;
+    return S;
 }
 
 PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
@@ -62,8 +57,12 @@ PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
     p.n = n;
     p.nt = nt;
     p.n8 = (n + 7) / 8;
-    source_split(n, is_f64, num_sms, &p.T, &p.S);
-    // the small variant's stages hold 256 records: it needs T <= 256, i.e. n <= 4,096
+    {
+        // T: the longest tile the variant n would get on its own stages (the small variant's hold 256 records)
+        const VariantGeom gn = variant_geom(n <= 4096 ? 1 : 0, is_f64);
+        p.T = (n > 4096 && !is_f64) ? 512 : 256;
+        p.S = source_split(n, p.T, (int64_t)gn.ipt * gn.cthreads, (int64_t)num_sms * gn.minb);
+    }
     p.variant = (nt <= 4096 && n <= 4096) ? 1 : 0;
     const VariantGeom g = variant_geom(p.variant, is_f64);
     p.ipt = g.ipt;
@@ -74,6 +73,32 @@ PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
     p.nb = (int32_t)((nt + p.IB - 1) / p.IB);
     p.U = (int64_t)p.nb * p.S;
     int64_t P = (int64_t)num_sms * g.minb;
+    if (P > p.U) P = p.U;
+    if (P < 1) P = 1;
+    p.P = (int32_t)P;
+    return p;
+}
+
+// Plan of the O(N^2) pull-back kernels (adjoint.cu): targets = sources = the n particles, one CTA per SM.
+PairPlan make_vjp_plan(int64_t n, int is_f64, int num_sms)
+{
+    PairPlan p;
+    memset(&p, 0, sizeof(p));
+    int ipt, cthreads, tile, minb;
+    vjp_geometry(is_f64, &ipt, &cthreads, &tile, &minb);
+    p.n = p.nt = n;
+    p.n8 = (n + 7) / 8;
+    p.T = tile;
+    p.ipt = ipt;
+    p.cthreads = cthreads;
+    p.IB = ipt * cthreads;
+    p.S = source_split(n, p.T, p.IB, (int64_t)num_sms * minb);
+    p.variant = 0;
+    p.rec_bytes = 64;
+    p.comps = 6;
+    p.nb = (int32_t)((n + p.IB - 1) / p.IB);
+    p.U = (int64_t)p.nb * p.S;
+    int64_t P = (int64_t)num_sms * minb;
     if (P > p.U) P = p.U;
     if (P < 1) P = 1;
     p.P = (int32_t)P;
@@ -123,6 +148,8 @@ odisseo_status device_info(DeviceInfo& out)
     e = configure_pair_f32();
     if (e != cudaSuccess) return cuda_fail(e);
     e = configure_pair_f64();
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = configure_vjp();
     if (e != cudaSuccess) return cuda_fail(e);
     d.configured = true;
     g_devices.push_back(d);
@@ -191,11 +218,11 @@ cudaError_t launch_pair(const PairPlan& p, const T* x, const void* j, double* pa
     return e;
 }
 inline cudaError_t launch_step(const PairPlan& p, float* x, float* v, float* a, void* j, const double* part, float G,
-                               const PotParams<float>& pot, float dt, int flags, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, s); }
+                               const PotParams<float>& pot, float dt, int flags, cudaStream_t s, float* snap = nullptr)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, snap, s); }
 inline cudaError_t launch_step(const PairPlan& p, double* x, double* v, double* a, void* j, const double* part, double G,
-                               const PotParams<double>& pot, double dt, int flags, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, s); }
+                               const PotParams<double>& pot, double dt, int flags, cudaStream_t s, double* snap = nullptr)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, snap, s); }
 
 inline cudaError_t launch_ext(const float* x, float* a, int64_t n, const PotParams<float>& pot, int accumulate, cudaStream_t s)
 { g_launches.fetch_add(1, std::memory_order_relaxed); return launch_ext_f32(x, a, n, pot, accumulate, s); }
@@ -331,7 +358,7 @@ constexpr size_t GRAPH_CACHE = 8;
 
 template <typename T>
 odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, T G, T eps, T dt, int64_t nsteps,
-                             const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream)
+                             const odisseo_potential* pot, void* ws, size_t ws_bytes, void* stream, T* tape = nullptr)
 {
     if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
     if (n == 0) return ODISSEO_OK;
@@ -359,6 +386,9 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     cudaError_t e;
 
 #define ODISSEO_TRY(call) do { e = (call); if (e != cudaSuccess) return cuda_fail(e); } while (0)
+    // tape != nullptr (odisseo_leapfrog_kdk_tape_*): every step kernel also stores the synchronised snapshot
+    // {x_k, v_k, pair-only a_k} it holds in registers at the moment between two steps -- no copies, no extra launch
+    const size_t snap = (size_t)n * 12;
     int first = 0;
     if (!acc_valid) {
         ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_PACK_ONLY, s));
@@ -366,17 +396,17 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
         first = STEP_FROM_PARTIALS;
     }
     if (nsteps == 0) {
-        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first, s));
+        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | (tape ? STEP_SNAPSHOT : 0), s, tape));
         return ODISSEO_OK;
     }
-    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN, s));
+    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN, s, tape));
 
     int64_t mid = nsteps - 1;     // full steps: pair + (close, open)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
     // no graph on the legacy stream, inside a caller's capture, or while a profile is open
     // (event pairs around the pair kernels cannot be read back from graph nodes)
-    const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2 && !g_prof.active;
+    const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2 && !g_prof.active && !tape;
     if (use_graph) {
         const int block = (int)(mid < 16 ? mid : 16);
         GraphKey key;
@@ -428,10 +458,11 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     for (; mid > 0; --mid) {
         ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
         ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
-                                STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s));
+                                STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s, tape ? tape + (size_t)(nsteps - mid) * snap : nullptr));
     }
     ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
-    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE, s));
+    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE, s,
+                            tape ? tape + (size_t)nsteps * snap : nullptr));
     return ODISSEO_OK;
 }
 
@@ -522,18 +553,20 @@ odisseo_status diagnostics_impl(const T* posm, const T* vel, int64_t n, T G, T e
     return ODISSEO_OK;
 }
 
-inline cudaError_t launch_accel_vjp(const float* x, const float* c, int64_t n, double G, double eps, const PotParams<double>& pot, float* gx,
-                                    double* gm, double* gp, const double* dts, int accum, int eg, void* ws, int sms, cudaStream_t s)
-{ return launch_accel_vjp_f32(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, eg, ws, sms, s); }
-inline cudaError_t launch_accel_vjp(const double* x, const double* c, int64_t n, double G, double eps, const PotParams<double>& pot, double* gx,
-                                    double* gm, double* gp, const double* dts, int accum, int eg, void* ws, int sms, cudaStream_t s)
-{ return launch_accel_vjp_f64(x, c, n, G, eps, pot, gx, gm, gp, dts, accum, eg, ws, sms, s); }
-inline cudaError_t launch_vjp_pre(const float* tk, const float* tk1, int64_t n, const PotParams<float>& pot, float dt, float w, int first,
-                                  const float* lx, float* lv, float* cot, double* dts, cudaStream_t s)
-{ return launch_vjp_pre_f32(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
-inline cudaError_t launch_vjp_pre(const double* tk, const double* tk1, int64_t n, const PotParams<double>& pot, double dt, double w, int first,
-                                  const double* lx, double* lv, double* cot, double* dts, cudaStream_t s)
-{ return launch_vjp_pre_f64(tk, tk1, n, pot, dt, w, first, lx, lv, cot, dts, s); }
+inline cudaError_t launch_accel_vjp(const PairPlan& p, const float* x, const float* c, double G, double eps, const PotParams<double>& pot,
+                                    float* gx, double* gm, double* gp, int eg, void* ws, cudaStream_t s)
+{ return launch_accel_vjp_f32(p, x, c, G, eps, pot, gx, gm, gp, eg, ws, s); }
+inline cudaError_t launch_accel_vjp(const PairPlan& p, const double* x, const double* c, double G, double eps, const PotParams<double>& pot,
+                                    double* gx, double* gm, double* gp, int eg, void* ws, cudaStream_t s)
+{ return launch_accel_vjp_f64(p, x, c, G, eps, pot, gx, gm, gp, eg, ws, s); }
+inline cudaError_t launch_leapfrog_vjp(const PairPlan& p, const float* tape, int64_t nsteps, double G, double eps, float dt,
+                                       const PotParams<double>& pd, const PotParams<float>& pt, int eg, float* lx, float* lv, double* gm,
+                                       double* gp, void* ws, int64_t* nl, cudaStream_t s)
+{ return launch_leapfrog_vjp_f32(p, tape, nsteps, G, eps, dt, pd, pt, eg, lx, lv, gm, gp, ws, nl, s); }
+inline cudaError_t launch_leapfrog_vjp(const PairPlan& p, const double* tape, int64_t nsteps, double G, double eps, double dt,
+                                       const PotParams<double>& pd, const PotParams<double>& pt, int eg, double* lx, double* lv, double* gm,
+                                       double* gp, void* ws, int64_t* nl, cudaStream_t s)
+{ return launch_leapfrog_vjp_f64(p, tape, nsteps, G, eps, dt, pd, pt, eg, lx, lv, gm, gp, ws, nl, s); }
 
 template <typename T>
 odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps, const odisseo_potential* pot, int with_eps_G,
@@ -560,9 +593,10 @@ odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps
     DeviceInfo dev;
     st = device_info(dev);
     if (st != ODISSEO_OK) return st;
-    if (ws_bytes < vjp_workspace_bytes(n, sizeof(T) == 8, dev.sms)) return ODISSEO_ERR_WORKSPACE;
-    g_launches.fetch_add(3, std::memory_order_relaxed);
-    cudaError_t e = launch_accel_vjp(posm, cot, n, (double)G, (double)eps, pp, gx, gm, gparams, nullptr, 0, with_eps_G != 0, ws, dev.sms, s);
+    const PairPlan plan = make_vjp_plan(n, sizeof(T) == 8, dev.sms);
+    if (ws_bytes < vjp_workspace_bytes(plan, sizeof(T) == 8)) return ODISSEO_ERR_WORKSPACE;
+    g_launches.fetch_add(4, std::memory_order_relaxed);
+    cudaError_t e = launch_accel_vjp(plan, posm, cot, (double)G, (double)eps, pp, gx, gm, gparams, with_eps_G != 0, ws, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -578,18 +612,7 @@ odisseo_status leapfrog_tape_impl(T* posm, T* vel, T* acc, int64_t n, T G, T eps
     const size_t arr = (size_t)n * 4 * sizeof(T);
     if (misaligned(tape, 4 * sizeof(T))) return ODISSEO_ERR_ALIGN;
     if (tape_bytes < (size_t)(nsteps + 1) * 3 * arr) return ODISSEO_ERR_WORKSPACE;
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
-    unsigned char* t = reinterpret_cast<unsigned char*>(tape);
-    for (int64_t k = 0; k <= nsteps; ++k) {
-        odisseo_status st = leapfrog_impl<T>(posm, vel, acc, k > 0, n, G, eps, dt, k > 0 ? 1 : 0, pot, ws, ws_bytes, stream);
-        if (st != ODISSEO_OK) return st;
-        cudaError_t e = cudaMemcpyAsync(t, posm, arr, cudaMemcpyDeviceToDevice, s);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(t + arr, vel, arr, cudaMemcpyDeviceToDevice, s);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(t + 2 * arr, acc, arr, cudaMemcpyDeviceToDevice, s);
-        if (e != cudaSuccess) return cuda_fail(e);
-        t += 3 * arr;
-    }
-    return ODISSEO_OK;
+    return leapfrog_impl<T>(posm, vel, acc, 0, n, G, eps, dt, nsteps, pot, ws, ws_bytes, stream, tape);
 }
 
 template <typename T>
@@ -620,26 +643,15 @@ odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int
     DeviceInfo dev;
     st = device_info(dev);
     if (st != ODISSEO_OK) return st;
-    if (ws_bytes < vjp_workspace_bytes(n, sizeof(T) == 8, dev.sms)) return ODISSEO_ERR_WORKSPACE;
+    const PairPlan plan = make_vjp_plan(n, sizeof(T) == 8, dev.sms);
+    if (ws_bytes < vjp_workspace_bytes(plan, sizeof(T) == 8)) return ODISSEO_ERR_WORKSPACE;
     e = cudaMemsetAsync(gm, 0, (size_t)n * sizeof(double), s);
     if (e != cudaSuccess) return cuda_fail(e);
     if (nsteps == 0) return ODISSEO_OK;                    // the final state is the initial state
-    double* dt_sums;
-    void* cotv;
-    vjp_carve(ws, n, dev.sms, &dt_sums, &cotv);
-    T* cot = static_cast<T*>(cotv);
-    const size_t snap = (size_t)n * 12;                    // scalars per snapshot
-    const T half = (T)0.5 * dt;
-    for (int64_t k = nsteps; k >= 0; --k) {
-        const T* tk = tape + (size_t)k * snap;
-        const int first = k == nsteps;
-        const T w = (first || k == 0) ? half : dt;
-        g_launches.fetch_add(4, std::memory_order_relaxed);
-        e = launch_vjp_pre(tk, first ? (const T*)nullptr : tk + snap, n, pt, dt, w, first, lx, lv, cot, dt_sums, s);
-        if (e != cudaSuccess) return cuda_fail(e);
-        e = launch_accel_vjp(tk, cot, n, (double)G, (double)eps, pd, lx, gm, gparams, dt_sums, 1, with_eps_G != 0, ws, dev.sms, s);
-        if (e != cudaSuccess) return cuda_fail(e);
-    }
+    int64_t launches = 0;
+    e = launch_leapfrog_vjp(plan, tape, nsteps, (double)G, (double)eps, dt, pd, pt, with_eps_G != 0, lx, lv, gm, gparams, ws, &launches, s);
+    g_launches.fetch_add(launches, std::memory_order_relaxed);
+    if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
 
@@ -869,9 +881,18 @@ odisseo_status odisseo_leapfrog_kdk_f64(double* d_posm, double* d_vel, double* d
 size_t odisseo_vjp_workspace_bytes(int64_t n, int is_f64)
 {
     if (n <= 0) return 0;
+    int lo = 64, hi = 192;                                // as odisseo_workspace_bytes: the current device, else a bound
+    {
+        int dev = -1, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+            sms > 0)
+            lo = hi = sms;
+        else
+            (void)cudaGetLastError();
+    }
     size_t b = 0;
-    for (int sms = 64; sms <= 192; sms += 4) {            // bound over devices with up to 192 SMs
-        const size_t c = vjp_workspace_bytes(n, is_f64, sms);
+    for (int sms = lo; sms <= hi; ++sms) {
+        const size_t c = vjp_workspace_bytes(make_vjp_plan(n, is_f64, sms), is_f64);
         if (c > b) b = c;
     }
     return b;

@@ -46,7 +46,8 @@ template <typename T, bool REDUCE>
 __global__ void __launch_bounds__(STEP_THREADS, REDUCE ? 2 : (sizeof(T) == 4 ? 5 : 3))
 step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
             typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
-            const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags)
+            const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags,
+            typename Vec4<T>::type* __restrict__ snapshot)
 {
     typedef typename Vec4<T>::type V4;
     pdl_launch_dependents();
@@ -81,7 +82,7 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
                 const V4 a = acc[i];
                 apx = a.x; apy = a.y; apz = a.z;
             }
-            if (flags & (STEP_CLOSE | STEP_OPEN)) {
+            if (flags & (STEP_CLOSE | STEP_OPEN | STEP_SNAPSHOT)) {
                 T ex, ey, ez;
                 ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
                 const T tx = apx + ex, ty = apy + ey, tz = apz + ez;
@@ -89,6 +90,15 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
                 V4 v = vel[i];
                 if (flags & STEP_CLOSE) {
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
+                }
+                if (snapshot) {
+                    // tape of the reverse-mode derivative (odisseo_leapfrog_kdk_tape_*): the synchronised state
+                    // {x_k, v_k, pair-only a_k} between the closing kick of step k - 1 and the opening kick of step k
+                    V4 vs = v; vs.w = (T)0;
+                    V4 as; as.x = apx; as.y = apy; as.z = apz; as.w = (T)0;
+                    snapshot[i] = p;
+                    snapshot[plan.n + i] = vs;
+                    snapshot[2 * plan.n + i] = as;
                 }
                 if (flags & STEP_OPEN) {
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
@@ -175,28 +185,28 @@ inline unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
 
 cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
-                            cudaStream_t stream)
+                            float* snapshot, cudaStream_t stream)
 {
     const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
     typedef float4 V4;
     if (flags & STEP_FROM_PARTIALS)
         return launch_pdl(step_kernel<float, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
     return launch_pdl(step_kernel<float, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
 }
 
 cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
-                            cudaStream_t stream)
+                            double* snapshot, cudaStream_t stream)
 {
     const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
     typedef double4 V4;
     if (flags & STEP_FROM_PARTIALS)
         return launch_pdl(step_kernel<double, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
     return launch_pdl(step_kernel<double, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags);
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
 }
 
 cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,

@@ -148,7 +148,8 @@ enum : int {
     STEP_FROM_PARTIALS = 1,   // a_pair = G * fixed-order sum of partial rows (else read acc)
     STEP_CLOSE = 2,           // closing half kick  v += a dt/2  (end of a step)
     STEP_OPEN = 4,            // opening half kick + drift: v += a dt/2; x += v dt (start of next step)
-    STEP_PACK_ONLY = 8        // only (re)write the staged source array from posm
+    STEP_PACK_ONLY = 8,       // only (re)write the staged source array from posm
+    STEP_SNAPSHOT = 16        // no kick: only store the tape snapshot {x, v, pair-only a} (nsteps == 0 with a tape)
 };
 
 // ---------------------------------------------------------------------------------------
@@ -284,10 +285,10 @@ cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void
                             double eps, cudaStream_t stream);
 cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
-                            cudaStream_t stream);
+                            float* snapshot, cudaStream_t stream);
 cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
-                            cudaStream_t stream);
+                            double* snapshot, cudaStream_t stream);
 cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,
                            cudaStream_t stream);
 cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const PotParams<double>& pot, int accumulate,
@@ -313,19 +314,22 @@ cudaError_t launch_diag_terms_f64(const PairPlan& plan, const double* posm, cons
                                   double* phi_out, cudaStream_t stream);
 cudaError_t launch_diag_final(const double* block_sums, int nblocks, double* out, cudaStream_t stream);
 // adjoint.cu
-void vjp_plan(int64_t n, int num_sms, int* nsplit, int64_t* chunk);
-size_t vjp_workspace_bytes(int64_t n, int is_f64, int num_sms);
-void vjp_carve(void* ws, int64_t n, int num_sms, double** dt_sums, void** cot);
-cudaError_t launch_accel_vjp_f32(const float* posm, const float* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 float* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
-                                 void* ws, int num_sms, cudaStream_t stream);
-cudaError_t launch_accel_vjp_f64(const double* posm, const double* cot, int64_t n, double G, double eps, const PotParams<double>& pot,
-                                 double* gx, double* gm, double* gparams, const double* dt_sums, int accumulate, int with_eps_G,
-                                 void* ws, int num_sms, cudaStream_t stream);
-cudaError_t launch_vjp_pre_f32(const float* tape_k, const float* tape_k1, int64_t n, const PotParams<float>& pot, float dt, float w,
-                               int first, const float* lx, float* lv, float* cot, double* dt_sums, cudaStream_t stream);
-cudaError_t launch_vjp_pre_f64(const double* tape_k, const double* tape_k1, int64_t n, const PotParams<double>& pot, double dt,
-                               double w, int first, const double* lx, double* lv, double* cot, double* dt_sums, cudaStream_t stream);
+void vjp_geometry(int is_f64, int* ipt, int* cthreads, int* tile, int* minb);
+PairPlan make_vjp_plan(int64_t n, int is_f64, int num_sms);          // api.cu
+size_t vjp_workspace_bytes(const PairPlan& plan, int is_f64);
+cudaError_t launch_accel_vjp_f32(const PairPlan& plan, const float* posm, const float* cot, double G, double eps,
+                                 const PotParams<double>& pot, float* gx, double* gm, double* gparams, int with_eps_G, void* ws,
+                                 cudaStream_t stream);
+cudaError_t launch_accel_vjp_f64(const PairPlan& plan, const double* posm, const double* cot, double G, double eps,
+                                 const PotParams<double>& pot, double* gx, double* gm, double* gparams, int with_eps_G, void* ws,
+                                 cudaStream_t stream);
+cudaError_t launch_leapfrog_vjp_f32(const PairPlan& plan, const float* tape, int64_t nsteps, double G, double eps, float dt,
+                                    const PotParams<double>& pot64, const PotParams<float>& pot, int with_eps_G, float* lx, float* lv,
+                                    double* gm, double* gparams, void* ws, int64_t* launches, cudaStream_t stream);
+cudaError_t launch_leapfrog_vjp_f64(const PairPlan& plan, const double* tape, int64_t nsteps, double G, double eps, double dt,
+                                    const PotParams<double>& pot64, const PotParams<double>& pot, int with_eps_G, double* lx, double* lv,
+                                    double* gm, double* gparams, void* ws, int64_t* launches, cudaStream_t stream);
+cudaError_t configure_vjp();
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
                                 int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream);
 cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
