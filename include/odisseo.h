@@ -103,6 +103,37 @@ odisseo_status odisseo_pair_accel_cross_f64(const double *d_targets, int64_t nt,
                                             double *d_acc, double G, double eps,
                                             void *d_workspace, size_t workspace_bytes, void *stream);
 
+/* Sharded form: one simulation spread over R ranks by TARGET slices (section 2.1, Fig. 1 -- the paper's
+ * only performance experiment).  Rank r owns the particles [lo_r, lo_r + count_r), holds
+ * the staged source records of ALL n particles in its workspace, and per KDK step calls
+ *     odisseo_kick_drift_slice_*   (moves its slice, re-stages the slice's records at their global index)
+ *     <exchange>                   (in-place all-gather of the record array, by the caller: NCCL / torch.distributed)
+ *     odisseo_pair_accel_staged_*  (its targets against the staged sources; no re-packing of the n sources)
+ * after one odisseo_stage_sources_* (records, padding and the equal-mass flags, which never change: masses are
+ * constant).  The summation order of a target depends on n only (chunk and tile boundaries are functions of n),
+ * so every rank count -- 1 included -- gives results BIT-IDENTICAL to odisseo_leapfrog_kdk_* on one GPU.
+ *   odisseo_staged_sources_layout: out = {byte offset of record 0 in the workspace, bytes per record, records the
+ *     array has room for (8 ceil(n/8) + 1,024: room for equal 8-aligned slices of up to 128 ranks)}.  Host arithmetic.
+ *     fp32 records are {x,x,y,y},{z,z,m,m}; fp64 records {x,y,z,m}; both 32 bytes.
+ *   odisseo_stage_sources_*: d_posm [n][4].  Workspace >= odisseo_cross_workspace_bytes(nt, n, is_f64).
+ *   odisseo_pair_accel_staged_*: d_targets [nt][4] (positions; lane 3 ignored), d_acc [nt][4] out (pair-only).
+ *   odisseo_kick_drift_slice_*: d_posm, d_vel, d_acc address the slice's count records (d_posm may point into the
+ *     array of all particles); mode as odisseo_kick_drift_*.  The rank whose slice ends at n also writes the padding
+ *     records; an empty slice with lo == n still does.  lo + count > n -> ERR_ARG. */
+odisseo_status odisseo_staged_sources_layout(int64_t n, int is_f64, int64_t out[3]);
+odisseo_status odisseo_stage_sources_f32(const float *d_posm, int64_t n, void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_stage_sources_f64(const double *d_posm, int64_t n, void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_pair_accel_staged_f32(const float *d_targets, int64_t nt, int64_t n, float *d_acc, float G, float eps,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_pair_accel_staged_f64(const double *d_targets, int64_t nt, int64_t n, double *d_acc, double G, double eps,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+odisseo_status odisseo_kick_drift_slice_f32(float *d_posm, float *d_vel, const float *d_acc, int64_t n, int64_t lo, int64_t count,
+                                            float G, float dt, const odisseo_potential *pot, int mode, void *d_workspace,
+                                            size_t workspace_bytes, void *stream);
+odisseo_status odisseo_kick_drift_slice_f64(double *d_posm, double *d_vel, const double *d_acc, int64_t n, int64_t lo, int64_t count,
+                                            double G, double dt, const odisseo_potential *pot, int mode, void *d_workspace,
+                                            size_t workspace_bytes, void *stream);
+
 /* Structure-of-arrays face of the fp32 pair call: seven length-n float arrays (4-byte
  * aligned).  Packs into the workspace, runs the same kernel, unpacks.  Workspace must be
  * odisseo_workspace_bytes(n, 0) + 32 * n + 512 bytes, 256-byte aligned. */
@@ -262,7 +293,9 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float *d_posm, float *d_vel, in
  *   odisseo_ensemble_leapfrog_kdk_vjp_f32: d_lx, d_lv [nsim][n][4] hold dL/dx_N, dL/dv_N of every simulation on
  *     entry and dL/dx_0, dL/dv_0 on exit; d_gm [nsim][n] double = dL/dm_i; d_gparams [nsim][8] double =
  *     dL/d(M_s, r_s, M_d, a, b, G, eps, dt) of each simulation.  h_params as in the forward call (the same
- *     records).  One CTA per simulation, the whole backward time loop in one kernel. */
+ *     records).  accumulate != 0: d_gm and d_gparams are added to instead of overwritten (a backward pass cut
+ *     into segments, the later segment first: no gradient arithmetic is left to the caller).
+ *     One CTA per simulation, the whole backward time loop in one kernel. */
 size_t odisseo_ensemble_tape_bytes(int64_t n, int64_t nsim, int64_t nsteps);
 odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float *d_posm, float *d_vel, int64_t n, int64_t nsim,
                                                       const odisseo_sim_params *h_params, int64_t nparams,
@@ -270,9 +303,9 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float *d_posm, float *d_ve
                                                       void *d_workspace, size_t workspace_bytes, void *stream);
 odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float *d_tape, int64_t n, int64_t nsim,
                                                      const odisseo_sim_params *h_params, int64_t nparams,
-                                                     int64_t nsteps, int with_eps_G, float *d_lx, float *d_lv, double *d_gm,
-                                                     double *d_gparams, void *d_workspace, size_t workspace_bytes,
-                                                     void *stream);
+                                                     int64_t nsteps, int with_eps_G, int accumulate, float *d_lx, float *d_lv,
+                                                     double *d_gm, double *d_gparams, void *d_workspace,
+                                                     size_t workspace_bytes, void *stream);
 
 /* Instrumentation (bench.py's gpu_launches and roofline legs).
  *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA

@@ -112,10 +112,9 @@ class _EnsembleLeapfrogKDK(torch.autograd.Function):
         g_mass_final = lx[:, :, 3].clone()
         lx[:, :, 3] = 0
         lv[:, :, 3] = 0
-        gm_tot = torch.zeros(nsim, n, dtype=torch.float64, device=lx.device)
-        gp_tot = torch.zeros(nsim, 8, dtype=torch.float64, device=lx.device)
-        gm = torch.empty_like(gm_tot)
-        gp = torch.empty_like(gp_tot)
+        # the C ABI accumulates the segment gradients itself (accumulate flag): no gradient arithmetic here
+        gm_tot = torch.empty(nsim, n, dtype=torch.float64, device=lx.device)
+        gp_tot = torch.empty(nsim, 8, dtype=torch.float64, device=lx.device)
         for s in range(len(segments) - 1, -1, -1):
             k = segments[s]
             if starts:                                                    # recompute this segment with a tape
@@ -124,9 +123,7 @@ class _EnsembleLeapfrogKDK(torch.autograd.Function):
                 B.ensemble_leapfrog_kdk_tape(p, v, params, k, seg_tape, ws)
             else:
                 seg_tape = tape
-            B.ensemble_leapfrog_kdk_vjp(seg_tape, params, k, lx, lv, gm, gp, ws)
-            gm_tot += gm
-            gp_tot += gp
+            B.ensemble_leapfrog_kdk_vjp(seg_tape, params, k, lx, lv, gm_tot, gp_tot, ws, accumulate=s < len(segments) - 1)
         lx[:, :, 3] = gm_tot.to(lx.dtype) + g_mass_final
         return (lx, lv, gp_tot[:, :5].to(theta.dtype).to(theta.device), gp_tot[:, 7].to(dt.dtype).to(dt.device),
                 None, None, None, None)

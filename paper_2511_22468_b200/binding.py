@@ -32,7 +32,9 @@ EXPORTS = [
     "odisseo_leapfrog_kdk_tape_f32", "odisseo_leapfrog_kdk_tape_f64", "odisseo_leapfrog_kdk_vjp_f32",
     "odisseo_leapfrog_kdk_vjp_f64", "odisseo_ensemble_tape_bytes", "odisseo_ensemble_leapfrog_kdk_tape_f32",
     "odisseo_ensemble_leapfrog_kdk_vjp_f32", "odisseo_cross_workspace_bytes", "odisseo_pair_accel_cross_f32",
-    "odisseo_pair_accel_cross_f64", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
+    "odisseo_pair_accel_cross_f64", "odisseo_staged_sources_layout", "odisseo_stage_sources_f32", "odisseo_stage_sources_f64",
+    "odisseo_pair_accel_staged_f32", "odisseo_pair_accel_staged_f64", "odisseo_kick_drift_slice_f32",
+    "odisseo_kick_drift_slice_f64", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
 ]
 
 
@@ -98,6 +100,10 @@ def lib():
             getattr(L, "odisseo_diagnostics_" + suffix).argtypes = [vp, vp, i64, sc, sc, vp, vp, vp, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_" + suffix).argtypes = [vp, vp, vp, i64, sc, sc, vp, ci, vp, sz, vp]
             getattr(L, "odisseo_leapfrog_kdk_host_" + suffix).argtypes = [vp, vp, vp, ci, i64, sc, sc, sc, i64, vp, vp, sz, vp]
+            getattr(L, "odisseo_stage_sources_" + suffix).argtypes = [vp, i64, vp, sz, vp]
+            getattr(L, "odisseo_pair_accel_staged_" + suffix).argtypes = [vp, i64, i64, vp, sc, sc, vp, sz, vp]
+            getattr(L, "odisseo_kick_drift_slice_" + suffix).argtypes = [vp, vp, vp, i64, i64, i64, sc, sc, vp, ci, vp, sz, vp]
+        L.odisseo_staged_sources_layout.argtypes = [i64, ci, vp]
         L.odisseo_cross_workspace_bytes.restype = sz
         L.odisseo_cross_workspace_bytes.argtypes = [i64, i64, ci]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
@@ -117,7 +123,7 @@ def lib():
         L.odisseo_ensemble_tape_bytes.restype = sz
         L.odisseo_ensemble_tape_bytes.argtypes = [i64, i64, i64]
         L.odisseo_ensemble_leapfrog_kdk_tape_f32.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, sz, vp, sz, vp]
-        L.odisseo_ensemble_leapfrog_kdk_vjp_f32.argtypes = [vp, i64, i64, vp, i64, i64, ci, vp, vp, vp, vp, vp, sz, vp]
+        L.odisseo_ensemble_leapfrog_kdk_vjp_f32.argtypes = [vp, i64, i64, vp, i64, i64, ci, ci, vp, vp, vp, vp, vp, sz, vp]
         L.odisseo_launch_count.restype = i64
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
@@ -431,9 +437,9 @@ def ensemble_leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, params, ns
 
 def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch.Tensor, lv: torch.Tensor,
                               gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor,
-                              with_eps_G: bool = False, stream=None):
+                              with_eps_G: bool = False, accumulate: bool = False, stream=None):
     """Gradients of every simulation of a batch from its tape: lx, lv [nsim, n, 4] in/out; gm float64 [nsim, n];
-    gparams float64 [nsim, 8] (GRADIENT_FIELDS)."""
+    gparams float64 [nsim, 8] (GRADIENT_FIELDS); accumulate adds to gm and gparams instead of overwriting them."""
     nsim, n = _ens_state(lx, lv, "lx and lv")
     _f64vec(gm, "gm", nsim * n)
     _f64vec(gparams, "gparams", nsim * 8)
@@ -441,9 +447,9 @@ def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch
         raise ValueError("tape does not hold nsteps + 1 snapshots of every simulation")
     arr = _sim_params(params)
     _check(lib().odisseo_ensemble_leapfrog_kdk_vjp_f32(tape.data_ptr(), n, nsim, ctypes.cast(arr, ctypes.c_void_p),
-                                                       len(params), int(nsteps), int(bool(with_eps_G)), lx.data_ptr(),
-                                                       lv.data_ptr(), gm.data_ptr(), gparams.data_ptr(), workspace.data_ptr(),
-                                                       workspace.numel(), _stream(stream)),
+                                                       len(params), int(nsteps), int(bool(with_eps_G)), int(bool(accumulate)),
+                                                       lx.data_ptr(), lv.data_ptr(), gm.data_ptr(), gparams.data_ptr(),
+                                                       workspace.data_ptr(), workspace.numel(), _stream(stream)),
            "ensemble_leapfrog_kdk_vjp_f32")
 
 
@@ -484,6 +490,42 @@ def profile_end():
     ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
     _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
     return float(ms.value), int(nl.value), int(nd.value)
+
+
+def staged_sources_layout(n: int, is_f64: bool = False):
+    """(byte offset of record 0 in a workspace, bytes per record, records the array has room for)."""
+    out = (ctypes.c_int64 * 3)()
+    _check(lib().odisseo_staged_sources_layout(int(n), int(bool(is_f64)), out), "staged_sources_layout")
+    return int(out[0]), int(out[1]), int(out[2])
+
+
+def stage_sources(posm: torch.Tensor, workspace: torch.Tensor, stream=None):
+    """Stage all n sources (records, padding, equal-mass flags) into the workspace (odisseo_stage_sources_*)."""
+    n = _rec(posm, "posm")
+    sfx = _suffix(posm)
+    _check(getattr(lib(), "odisseo_stage_sources_" + sfx)(posm.data_ptr(), n, workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "stage_sources_" + sfx)
+
+
+def pair_accel_staged(targets: torch.Tensor, n: int, acc: torch.Tensor, G: float, eps: float, workspace: torch.Tensor, stream=None):
+    """acc[nt,4] = pair acceleration at targets[nt,4] due to the n sources already staged in the workspace."""
+    nt = _rec(targets, "targets")
+    _rec(acc, "acc", nt)
+    sfx = _suffix(targets)
+    _check(getattr(lib(), "odisseo_pair_accel_staged_" + sfx)(targets.data_ptr(), nt, int(n), acc.data_ptr(), G, eps, workspace.data_ptr(),
+                                                             workspace.numel(), _stream(stream)), "pair_accel_staged_" + sfx)
+
+
+def kick_drift_slice(posm_slice: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, n: int, lo: int, G: float, dt: float,
+                     pot: Optional[Potential], mode: int, workspace: torch.Tensor, stream=None):
+    """odisseo_kick_drift_slice_*: kick/drift the slice [lo, lo + count) of n particles and re-stage its records."""
+    count = _rec(posm_slice, "posm_slice")
+    _rec(vel, "vel", count)
+    _rec(acc, "acc", count)
+    sfx = _suffix(posm_slice)
+    _check(getattr(lib(), "odisseo_kick_drift_slice_" + sfx)(posm_slice.data_ptr(), vel.data_ptr(), acc.data_ptr(), int(n), int(lo), count,
+                                                            G, dt, _pot(pot), int(mode), workspace.data_ptr(), workspace.numel(),
+                                                            _stream(stream)), "kick_drift_slice_" + sfx)
 
 
 def ubench_kinds():

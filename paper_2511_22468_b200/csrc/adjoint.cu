@@ -462,7 +462,7 @@ static VjpCarve vjp_carve_all(void* ws, const PairPlan& plan)
 {
     unsigned char* base = static_cast<unsigned char*>(ws);
     VjpCarve c;
-    c.jsrc = base;
+    c.jsrc = plan_records(base, plan);
     c.rows = reinterpret_cast<double*>(base + plan_jsrc_bytes(plan));
     c.block_sums = reinterpret_cast<double*>(base + plan_jsrc_bytes(plan) + vjp_rows_bytes(plan));
     c.cot = base + plan_jsrc_bytes(plan) + vjp_rows_bytes(plan) + vjp_blocks_bytes(plan);

@@ -218,11 +218,13 @@ cudaError_t launch_pair(const PairPlan& p, const T* x, const void* j, double* pa
     return e;
 }
 inline cudaError_t launch_step(const PairPlan& p, float* x, float* v, float* a, void* j, const double* part, float G,
-                               const PotParams<float>& pot, float dt, int flags, cudaStream_t s, float* snap = nullptr)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, snap, s); }
+                               const PotParams<float>& pot, float dt, int flags, cudaStream_t s, float* snap = nullptr,
+                               int64_t lo = 0, int64_t count = -1)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f32(p, x, v, a, j, part, G, pot, dt, flags, snap, lo, count < 0 ? p.n : count, s); }
 inline cudaError_t launch_step(const PairPlan& p, double* x, double* v, double* a, void* j, const double* part, double G,
-                               const PotParams<double>& pot, double dt, int flags, cudaStream_t s, double* snap = nullptr)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, snap, s); }
+                               const PotParams<double>& pot, double dt, int flags, cudaStream_t s, double* snap = nullptr,
+                               int64_t lo = 0, int64_t count = -1)
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, snap, lo, count < 0 ? p.n : count, s); }
 
 inline cudaError_t launch_ext(const float* x, float* a, int64_t n, const PotParams<float>& pot, int accumulate, cudaStream_t s)
 { g_launches.fetch_add(1, std::memory_order_relaxed); return launch_ext_f32(x, a, n, pot, accumulate, s); }
@@ -237,7 +239,7 @@ odisseo_status carve(const PairPlan& plan, void* ws, size_t ws_bytes, Carve& out
     if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
     const size_t need = plan_jsrc_bytes(plan) + plan_partial_bytes(plan);
     if (ws_bytes < need) return ODISSEO_ERR_WORKSPACE;
-    out.jsrc = ws;
+    out.jsrc = plan_records(ws, plan);
     out.partials = reinterpret_cast<double*>(static_cast<unsigned char*>(ws) + plan_jsrc_bytes(plan));
     return ODISSEO_OK;
 }
@@ -312,6 +314,93 @@ odisseo_status pair_cross_impl(const T* targets, int64_t nt, const T* sources, i
     e = launch_pair(plan, targets, cv.jsrc, cv.partials, eps, s);
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_reduce_rows(plan, cv.partials, cv.jsrc, G, acc, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+// ---- sharded form: the three calls of one rank's KDK step on a slice ----------------
+// The staged source array in the workspace is kept across calls: stage_sources writes all of it (records, padding,
+// equal-mass flags), kick_drift_slice re-stages the records of the slice it moves, the caller's exchange fills in the
+// other ranks' records (an in-place all-gather of the record array), pair_accel_staged evaluates targets against it.
+template <typename T>
+odisseo_status stage_sources_impl(const T* posm, int64_t n, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0) return ODISSEO_ERR_ARG;
+    if (n == 0) return ODISSEO_OK;
+    if (!posm || !ws) return ODISSEO_ERR_NULL;
+    if (misaligned(posm, 4 * sizeof(T)) || misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    if (ws_bytes < plan_jsrc_bytes(plan)) return ODISSEO_ERR_WORKSPACE;
+    PotParams<T> nopot;
+    memset(&nopot, 0, sizeof(nopot));
+    cudaError_t e = launch_step(plan, const_cast<T*>(posm), (T*)nullptr, (T*)nullptr, plan_records(ws, plan), nullptr, (T)0, nopot,
+                                (T)0, STEP_PACK_ONLY, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? ODISSEO_OK : cuda_fail(e);
+}
+
+template <typename T>
+odisseo_status pair_staged_impl(const T* targets, int64_t nt, int64_t n, T* acc, T G, T eps, void* ws, size_t ws_bytes,
+                                void* stream)
+{
+    if (n < 0 || nt < 0) return ODISSEO_ERR_ARG;
+    if (nt == 0) return ODISSEO_OK;
+    if (!targets || !acc || !ws) return ODISSEO_ERR_NULL;
+    const size_t rec = 4 * sizeof(T);
+    if (misaligned(targets, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+    if (overlap(targets, nt * rec, acc, nt * rec)) return ODISSEO_ERR_ARG;
+    odisseo_status st = check_pair_scalars<T>(G, eps);
+    if (st != ODISSEO_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (n == 0) {
+        cudaError_t e0 = cudaMemsetAsync(acc, 0, (size_t)nt * rec, s);
+        return e0 == cudaSuccess ? ODISSEO_OK : cuda_fail(e0);
+    }
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_cross_plan(nt, n, sizeof(T) == 8, dev.sms);
+    Carve cv;
+    st = carve(plan, ws, ws_bytes, cv);
+    if (st != ODISSEO_OK) return st;
+    cudaError_t e = launch_pair(plan, targets, cv.jsrc, cv.partials, eps, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = launch_reduce_rows(plan, cv.partials, cv.jsrc, G, acc, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+template <typename T>
+odisseo_status kick_drift_slice_impl(T* posm, T* vel, const T* acc, int64_t n, int64_t lo, int64_t count, T G, T dt,
+                                     const odisseo_potential* pot, int mode, void* ws, size_t ws_bytes, void* stream)
+{
+    if (n < 0 || lo < 0 || count < 0 || lo + count > n || mode < 1 || mode > 3) return ODISSEO_ERR_ARG;
+    if (!ws) return ODISSEO_ERR_NULL;
+    if (misaligned(ws, 256)) return ODISSEO_ERR_ALIGN;
+    if (n == 0) return ODISSEO_OK;
+    const size_t rec = 4 * sizeof(T);
+    if (count > 0) {
+        if (!posm || !vel || !acc) return ODISSEO_ERR_NULL;
+        if (misaligned(posm, rec) || misaligned(vel, rec) || misaligned(acc, rec)) return ODISSEO_ERR_ALIGN;
+        if (overlap(posm, count * rec, acc, count * rec) || overlap(posm, count * rec, vel, count * rec) ||
+            overlap(vel, count * rec, acc, count * rec))
+            return ODISSEO_ERR_ARG;
+    }
+    if (!isfinite((double)G) || !isfinite((double)dt)) return ODISSEO_ERR_ARG;
+    PotParams<T> pp;
+    odisseo_status st = make_pot<T>(G, pot, pp);
+    if (st != ODISSEO_OK) return st;
+    DeviceInfo dev;
+    st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    if (ws_bytes < plan_jsrc_bytes(plan)) return ODISSEO_ERR_WORKSPACE;
+    if (count == 0 && lo != n) return ODISSEO_OK;          // an empty slice that does not own the padding
+    const int flags = ((mode & 1) ? STEP_CLOSE : 0) | ((mode & 2) ? STEP_OPEN : 0) | STEP_SLICE;
+    cudaError_t e = launch_step(plan, posm, vel, const_cast<T*>(acc), plan_records(ws, plan), nullptr, G, pp, dt, flags,
+                                static_cast<cudaStream_t>(stream), nullptr, lo, count);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -1036,8 +1125,8 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_tape_f32(float* d_posm, float* d_ve
 
 odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_t n, int64_t nsim,
                                                      const odisseo_sim_params* h_params, int64_t nparams, int64_t nsteps,
-                                                     int with_eps_G, float* d_lx, float* d_lv, double* d_gm, double* d_gparams,
-                                                     void* d_workspace, size_t workspace_bytes, void* stream)
+                                                     int with_eps_G, int accumulate, float* d_lx, float* d_lv, double* d_gm,
+                                                     double* d_gparams, void* d_workspace, size_t workspace_bytes, void* stream)
 {
     if (n < 0 || nsim < 0 || nsteps < 0 || n > ENSEMBLE_MAX_N || nsim > 0x7fffffff) return ODISSEO_ERR_ARG;
     if (n == 0 || nsim == 0) return ODISSEO_OK;
@@ -1058,7 +1147,7 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_
     if (st != ODISSEO_OK) return st;
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = launch_ensemble_vjp_f32(d_tape, d64, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps, with_eps_G != 0, d_lx, d_lv, d_gm,
-                                            d_gparams, s);
+                                            d_gparams, accumulate != 0, s);
     if (e != cudaSuccess) return cuda_fail(e);
     return ODISSEO_OK;
 }
@@ -1082,5 +1171,37 @@ odisseo_status odisseo_leapfrog_kdk_host_f64(double* h_posm, double* h_vel, doub
                                              double eps, double dt, int64_t nsteps, const odisseo_potential* pot,
                                              void* d_workspace, size_t workspace_bytes, void* stream)
 { return leapfrog_host_impl<double>(h_posm, h_vel, h_acc, acc_valid, n, G, eps, dt, nsteps, pot, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_staged_sources_layout(int64_t n, int is_f64, int64_t out[3])
+{
+    if (!out) return ODISSEO_ERR_NULL;
+    if (n <= 0) return ODISSEO_ERR_ARG;
+    const PairPlan p = make_plan(n, is_f64, 148);          // the layout depends on n only
+    out[0] = (int64_t)plan_flag_bytes(p);
+    out[1] = p.rec_bytes;
+    out[2] = plan_npad(p) + STAGED_SLACK;
+    return ODISSEO_OK;
+}
+
+odisseo_status odisseo_stage_sources_f32(const float* d_posm, int64_t n, void* d_workspace, size_t workspace_bytes, void* stream)
+{ return stage_sources_impl<float>(d_posm, n, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_stage_sources_f64(const double* d_posm, int64_t n, void* d_workspace, size_t workspace_bytes, void* stream)
+{ return stage_sources_impl<double>(d_posm, n, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_pair_accel_staged_f32(const float* d_targets, int64_t nt, int64_t n, float* d_acc, float G, float eps,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return pair_staged_impl<float>(d_targets, nt, n, d_acc, G, eps, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_pair_accel_staged_f64(const double* d_targets, int64_t nt, int64_t n, double* d_acc, double G, double eps,
+                                             void* d_workspace, size_t workspace_bytes, void* stream)
+{ return pair_staged_impl<double>(d_targets, nt, n, d_acc, G, eps, d_workspace, workspace_bytes, stream); }
+
+odisseo_status odisseo_kick_drift_slice_f32(float* d_posm, float* d_vel, const float* d_acc, int64_t n, int64_t lo, int64_t count,
+                                            float G, float dt, const odisseo_potential* pot, int mode, void* d_workspace,
+                                            size_t workspace_bytes, void* stream)
+{ return kick_drift_slice_impl<float>(d_posm, d_vel, d_acc, n, lo, count, G, dt, pot, mode, d_workspace, workspace_bytes, stream); }
+odisseo_status odisseo_kick_drift_slice_f64(double* d_posm, double* d_vel, const double* d_acc, int64_t n, int64_t lo, int64_t count,
+                                            double G, double dt, const odisseo_potential* pot, int mode, void* d_workspace,
+                                            size_t workspace_bytes, void* stream)
+{ return kick_drift_slice_impl<double>(d_posm, d_vel, d_acc, n, lo, count, G, dt, pot, mode, d_workspace, workspace_bytes, stream); }
 
 }  // extern "C"

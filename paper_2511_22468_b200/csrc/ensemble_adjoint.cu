@@ -23,7 +23,7 @@ template <int NQ, bool EG>
 __global__ void __launch_bounds__(VJP_THREADS, NQ <= 2 ? 2 : 1)
 ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __restrict__ params, const int shared_params,
                     const int n, const int64_t nsteps, float4* __restrict__ lx, float4* __restrict__ lv,
-                    double* __restrict__ gm_out, double* __restrict__ gparams)
+                    double* __restrict__ gm_out, double* __restrict__ gparams, const int accumulate)
 {
     extern __shared__ __align__(16) unsigned char evjp_smem[];
     constexpr int n_pad = NQ * VJP_THREADS;
@@ -183,26 +183,26 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
         if (i < n) {
             LX[i] = make_float4(Lx[q][0], Lx[q][1], Lx[q][2], 0.f);
             LV[i] = make_float4(Lv[q][0], Lv[q][1], Lv[q][2], 0.f);
-            gm_out[sim * n + i] = gm[q];
+            gm_out[sim * n + i] = accumulate ? gm_out[sim * n + i] + gm[q] : gm[q];
         }
     }
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         const double tot = vjp_block_sum(gp[k], warp_scratch);
-        if (tid == 0) gparams[sim * 8 + k] = tot;
+        if (tid == 0) gparams[sim * 8 + k] = accumulate ? gparams[sim * 8 + k] + tot : tot;
     }
 }
 
 template <int NQ, bool EG>
 cudaError_t launch_evjp(const float* tape, const EnsembleParams64* params, int shared_params, int n, int64_t nsim,
-                        int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, cudaStream_t stream)
+                        int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, int accumulate, cudaStream_t stream)
 {
     const size_t smem = (size_t)NQ * VJP_THREADS * (32 + 24);
     cudaError_t e = cudaFuncSetAttribute(ensemble_vjp_kernel<NQ, EG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     ensemble_vjp_kernel<NQ, EG><<<(unsigned)nsim, VJP_THREADS, smem, stream>>>(
         reinterpret_cast<const float4*>(tape), params, shared_params, n, nsteps, reinterpret_cast<float4*>(lx),
-        reinterpret_cast<float4*>(lv), gm, gparams);
+        reinterpret_cast<float4*>(lv), gm, gparams, accumulate);
     return cudaGetLastError();
 }
 
@@ -210,26 +210,26 @@ cudaError_t launch_evjp(const float* tape, const EnsembleParams64* params, int s
 
 template <bool EG>
 static cudaError_t dispatch_evjp(const float* tape, const EnsembleParams64* params, int shared_params, int n, int64_t nsim,
-                                 int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, cudaStream_t stream)
+                                 int64_t nsteps, float* lx, float* lv, double* gm, double* gparams, int accumulate, cudaStream_t stream)
 {
     switch ((n + VJP_THREADS - 1) / VJP_THREADS) {
-        case 1: return launch_evjp<1, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 2: return launch_evjp<2, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 3: return launch_evjp<3, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 4: return launch_evjp<4, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 5: return launch_evjp<5, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 6: return launch_evjp<6, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        case 7: return launch_evjp<7, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-        default: return launch_evjp<8, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+        case 1: return launch_evjp<1, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 2: return launch_evjp<2, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 3: return launch_evjp<3, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 4: return launch_evjp<4, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 5: return launch_evjp<5, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 6: return launch_evjp<6, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        case 7: return launch_evjp<7, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+        default: return launch_evjp<8, EG>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
     }
 }
 
 cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
                                     int64_t nsim, int64_t nsteps, int with_eps_G, float* lx, float* lv, double* gm,
-                                    double* gparams, cudaStream_t stream)
+                                    double* gparams, int accumulate, cudaStream_t stream)
 {
-    if (with_eps_G) return dispatch_evjp<true>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
-    return dispatch_evjp<false>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, stream);
+    if (with_eps_G) return dispatch_evjp<true>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
+    return dispatch_evjp<false>(tape, params, shared_params, n, nsim, nsteps, lx, lv, gm, gparams, accumulate, stream);
 }
 
 }  // namespace odisseo

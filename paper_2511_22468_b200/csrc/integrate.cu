@@ -47,24 +47,27 @@ __global__ void __launch_bounds__(STEP_THREADS, REDUCE ? 2 : (sizeof(T) == 4 ? 5
 step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
             typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
             const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags,
-            typename Vec4<T>::type* __restrict__ snapshot)
+            typename Vec4<T>::type* __restrict__ snapshot, const int64_t lo, const int64_t count)
 {
+    // posm, vel, acc address the particles [lo, lo + count) of the plan's n (the whole set: lo = 0, count = n; a
+    // rank's slice in the sharded form, STEP_SLICE); staged records are written at their global index.
     typedef typename Vec4<T>::type V4;
     pdl_launch_dependents();
     pdl_wait();                                      // the pair kernel's rows (or the caller's state) are complete
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
+    const bool flagging = staging && !(flags & STEP_SLICE);             // masses never change: a slice keeps the flags
     int mass_differs = 0;
     int* const block_flag = const_cast<int*>(plan_flags(jsrc, plan)) + blockIdx.x;
-    if (staging) {                                   // uniform branch: flags is a kernel argument
+    if (flagging) {                                  // uniform branch: flags is a kernel argument
         if (threadIdx.x == 0) *block_flag = 0;
         __syncthreads();                             // before any load is in flight: costs nothing
     }
-    if (i < plan.n) {
+    if (i < count) {
         const T mass0 = reinterpret_cast<const T*>(posm)[3];            // masses are never modified
         V4 p = posm[i];
         if (flags & STEP_PACK_ONLY) {
-            stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+            stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
         } else {
             T apx, apy, apz;
             if (REDUCE) {
@@ -104,18 +107,18 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
                     p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
                     posm[i] = p;
-                    stage_record(jsrc, i, p.x, p.y, p.z, p.w);
+                    stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
                 }
                 v.w = (T)0;
                 vel[i] = v;
             }
         }
-        if (staging) mass_differs = !(p.w == mass0);                // NaN counts as different
-    } else if (staging && i < plan_npad(plan)) {
-        const T far = pad_pos((T)0);
-        stage_record(jsrc, i, far, far, far, (T)0);
+        if (flagging) mass_differs = !(p.w == mass0);               // NaN counts as different
+    } else if (staging && lo + count == plan.n && lo + i < plan_npad(plan)) {
+        const T far = pad_pos((T)0);                                    // whoever holds the last particle pads the tail
+        stage_record(jsrc, lo + i, far, far, far, (T)0);
     }
-    if (staging) {
+    if (flagging) {
         // same-value plain stores after the block's own zeroing: no atomics, no closing barrier
         const unsigned any = __ballot_sync(0xffffffffu, mass_differs);
         if (any != 0u && (threadIdx.x & 31) == 0) *block_flag = 1;
@@ -185,28 +188,28 @@ inline unsigned grid_for(int64_t n) { return (unsigned)((n + 255) / 256); }
 
 cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
-                            float* snapshot, cudaStream_t stream)
+                            float* snapshot, int64_t lo, int64_t count, cudaStream_t stream)
 {
-    const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
+    const dim3 grid(grid_for(count + (plan_npad(plan) - plan.n))), block(STEP_THREADS);
     typedef float4 V4;
     if (flags & STEP_FROM_PARTIALS)
         return launch_pdl(step_kernel<float, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot), lo, count);
     return launch_pdl(step_kernel<float, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot), lo, count);
 }
 
 cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
-                            double* snapshot, cudaStream_t stream)
+                            double* snapshot, int64_t lo, int64_t count, cudaStream_t stream)
 {
-    const dim3 grid(grid_for(plan_npad(plan))), block(STEP_THREADS);
+    const dim3 grid(grid_for(count + (plan_npad(plan) - plan.n))), block(STEP_THREADS);
     typedef double4 V4;
     if (flags & STEP_FROM_PARTIALS)
         return launch_pdl(step_kernel<double, true>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
+                          reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot), lo, count);
     return launch_pdl(step_kernel<double, false>, grid, block, 0, stream, reinterpret_cast<V4*>(posm), reinterpret_cast<V4*>(vel),
-                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot));
+                      reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot), lo, count);
 }
 
 cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,

@@ -64,12 +64,23 @@ constexpr int STEP_THREADS = 256;
 __host__ __device__ __forceinline__ int32_t plan_nflags(const PairPlan& p) {
     return (int32_t)((plan_npad(p) + STEP_THREADS - 1) / STEP_THREADS);
 }
+// Workspace layout of the staged sources: [flags + decision word, rounded to 256 B][records].  `jsrc` always points
+// at the first RECORD; the flags sit in front of it, so that the record array can be longer than 8 * n8 records:
+// STAGED_SLACK extra records leave room for an in-place all-gather of equal, 8-aligned slices of up to 128 ranks
+// (sharded form).  The kernels never read a record past 8 * n8.
+constexpr int64_t STAGED_SLACK = 1024;
+__host__ __device__ __forceinline__ size_t plan_flag_bytes(const PairPlan& p) {
+    return (((size_t)plan_nflags(p) + 1) * sizeof(int) + 255) & ~(size_t)255;
+}
 __host__ __device__ __forceinline__ size_t plan_jsrc_bytes(const PairPlan& p) {
-    size_t b = (size_t)plan_npad(p) * p.rec_bytes + ((size_t)plan_nflags(p) + 1) * sizeof(int);
+    const size_t b = plan_flag_bytes(p) + (size_t)(plan_npad(p) + STAGED_SLACK) * p.rec_bytes;
     return (b + 255) & ~(size_t)255;
 }
+__host__ __device__ __forceinline__ void* plan_records(void* ws, const PairPlan& p) {
+    return static_cast<unsigned char*>(ws) + plan_flag_bytes(p);
+}
 __host__ __device__ __forceinline__ const int* plan_flags(const void* jsrc, const PairPlan& p) {
-    return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) + (size_t)plan_npad(p) * p.rec_bytes);
+    return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) - plan_flag_bytes(p));
 }
 __host__ __device__ __forceinline__ const int* plan_eqm_word(const void* jsrc, const PairPlan& p) {
     return plan_flags(jsrc, p) + plan_nflags(p);
@@ -149,7 +160,8 @@ enum : int {
     STEP_CLOSE = 2,           // closing half kick  v += a dt/2  (end of a step)
     STEP_OPEN = 4,            // opening half kick + drift: v += a dt/2; x += v dt (start of next step)
     STEP_PACK_ONLY = 8,       // only (re)write the staged source array from posm
-    STEP_SNAPSHOT = 16        // no kick: only store the tape snapshot {x, v, pair-only a} (nsteps == 0 with a tape)
+    STEP_SNAPSHOT = 16,       // no kick: only store the tape snapshot {x, v, pair-only a} (nsteps == 0 with a tape)
+    STEP_SLICE = 32           // the arrays address a slice [lo, lo + count) of the plan's particles (sharded form)
 };
 
 // ---------------------------------------------------------------------------------------
@@ -285,10 +297,10 @@ cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void
                             double eps, cudaStream_t stream);
 cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
-                            float* snapshot, cudaStream_t stream);
+                            float* snapshot, int64_t lo, int64_t count, cudaStream_t stream);
 cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc,
                             const double* partials, double G, const PotParams<double>& pot, double dt, int flags,
-                            double* snapshot, cudaStream_t stream);
+                            double* snapshot, int64_t lo, int64_t count, cudaStream_t stream);
 cudaError_t launch_ext_f32(const float* posm, float* acc, int64_t n, const PotParams<float>& pot, int accumulate,
                            cudaStream_t stream);
 cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const PotParams<double>& pot, int accumulate,
@@ -334,7 +346,7 @@ cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* p
                                 int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream);
 cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
                                     int64_t nsim, int64_t nsteps, int with_eps_G, float* lx, float* lv, double* gm,
-                                    double* gparams, cudaStream_t stream);
+                                    double* gparams, int accumulate, cudaStream_t stream);
 cudaError_t configure_pair_f32();
 cudaError_t configure_pair_f64();
 

@@ -15,28 +15,39 @@ NFW, MN, G, EPS, DT = (1.0e12, 16.0), (6.8e10, 3.0, 0.28), 4.4985e-12, 0.001, 0.
 
 
 class OracleCompute:
-    """Test stand-in for CudaCompute: the same two calls, evaluated by the fp64 oracle on numpy views of torch CPU
-    tensors (tests may import the oracle; the product module does not)."""
+    """Test stand-in for CudaCompute: the same calls, evaluated by the fp64 oracle on numpy views of torch CPU
+    tensors (tests may import the oracle; the product module does not).  Its "staged records" are plain {x, y, z, m}
+    rows in an array padded to world * L rows, which is what the exchange all-gathers."""
 
-    def __init__(self):
+    def __init__(self, n, world):
         from oracle import oracle as O
-        self.O, self.pot = O, O.Potential.make(nfw=NFW, mn=MN)
+        self.O, self.pot, self.n = O, O.Potential.make(nfw=NFW, mn=MN), n
+        L, _ = S.aligned_slices(n, world)
+        self.rec = torch.zeros(world * L, 4, dtype=torch.float64)
 
-    def cross(self, targets, sources, acc):
-        nt = targets.shape[0]
-        both = np.concatenate([sources.numpy(), targets.numpy()], axis=0).copy()
-        both[sources.shape[0]:, 3] = 0.0                                  # targets act as massless tracers
-        a, _ = self.O.pair_accel(both, G, EPS, targets=np.arange(sources.shape[0], sources.shape[0] + nt))
+    def stage_all(self, posm_all):
+        self.rec[:self.n] = posm_all
+
+    def records(self):
+        return self.rec
+
+    def accel(self, targets, acc):
+        nt, n = targets.shape[0], self.n
+        both = np.concatenate([self.rec[:n].numpy(), targets.numpy()], axis=0).copy()
+        both[n:, 3] = 0.0                                                 # targets act as massless tracers
+        a, _ = self.O.pair_accel(both, G, EPS, targets=np.arange(n, n + nt))
         acc[:, :3] = torch.from_numpy(a)
         acc[:, 3] = 0
 
-    def kick_drift(self, posm, vel, acc, mode):
+    def kick_drift(self, posm_all, vel, acc, lo, hi, mode):
+        posm = posm_all[lo:hi]
         a = acc[:, :3].numpy() + self.O.ext_accel(posm.numpy(), G, self.pot)
         if mode & 1:
             vel[:, :3] += torch.from_numpy(0.5 * DT * a)
         if mode & 2:
             vel[:, :3] += torch.from_numpy(0.5 * DT * a)
             posm[:, :3] += DT * vel[:, :3]
+            self.rec[lo:hi] = posm
 
 
 def _state(n):
@@ -54,12 +65,14 @@ def _worker(rank, world, port, n, nsteps, out):
     dist.init_process_group(backend="gloo")
     try:
         posm, vel = _state(n)
-        bounds = S.slice_bounds(n, world)
+        _, bounds = S.aligned_slices(n, world)
         lo, hi = bounds[rank]
         posm_all = torch.from_numpy(posm.copy())
         vel_slice = torch.from_numpy(vel[lo:hi].copy())
         acc_slice = torch.zeros(hi - lo, 4, dtype=torch.float64)
-        S.sharded_leapfrog_kdk(OracleCompute(), S.DistExchange(dist, bounds), posm_all, vel_slice, acc_slice, lo, hi, nsteps)
+        ex = S.DistExchange(dist, n, world, rank)
+        S.sharded_leapfrog_kdk(OracleCompute(n, world), ex, posm_all, vel_slice, acc_slice, lo, hi, nsteps)
+        ex.positions(posm_all)
         out.put((rank, lo, hi, posm_all.numpy().copy(), vel_slice.numpy().copy(), acc_slice.numpy().copy()))
     finally:
         dist.destroy_process_group()
@@ -75,9 +88,20 @@ def test_slice_bounds_cover_every_particle_once():
             assert max(sizes) - min(sizes) <= 1
 
 
+def test_aligned_slices_put_every_record_at_its_global_index():
+    for n in (0, 1, 7, 8, 9, 1000, 1001, 262144):
+        for world in (1, 2, 3, 5, 8):
+            L, b = S.aligned_slices(n, world)
+            assert L % 8 == 0 and L > 0 and world * L >= n and len(b) == world
+            assert b[0][0] == 0 and b[-1][1] == n
+            for r, (lo, hi) in enumerate(b):
+                assert lo == min(r * L, n) and hi == min((r + 1) * L, n) and 0 <= hi - lo <= L
+            assert world * L - n < 8 * world + 8                          # fits the staged array's 1,024-record slack
+
+
 def test_two_ranks_reproduce_the_single_process_oracle_trajectory():
     from oracle import oracle as O
-    n, nsteps = 101, 4                                                    # odd n: slices of 51 and 50
+    n, nsteps = 101, 4                                                    # odd n: slices of 56 and 45
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = 29600 + os.getpid() % 2000
