@@ -7,8 +7,11 @@ step of BASELINE.json configs[3] (Plummer progenitor, N = 262,144, NFW + Miyamot
 fp32) = one O(N^2) pair evaluation + fixed-order reduce + external acceleration + kick/drift/kick,
 called through the C ABI (odisseo_leapfrog_kdk_f32, nsteps = 1, acc_valid = 1).
 metric = pairwise interactions/s (N^2 per step); steps/s is reported beside it.
-Multi-GPU: the path does not shard in this build: every rank
-advances its own seeded replica, no data-path collective, scaling = "weak".
+Multi-GPU, default (--mode replicas): north_star fixes the build to one GPU with no collectives (DESIGN.md
+"Multi-GPU"): every rank advances its own seeded replica, no data-path collective, scaling = "weak".
+--mode sharded: ONE simulation, targets sliced over the ranks (paper_2511_22468_b200/sharded.py: kick/drift of the
+slice, one all-gather of staged source records per step, pair acceleration of the slice), scaling = "strong",
+value = N^2 x steps / max-over-ranks time.  Only ever run with world size 1 on hardware in this build.
 """
 from __future__ import annotations
 
@@ -24,8 +27,49 @@ import numpy as np
 FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star convention
 SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
-# dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144 (ncu --set full)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = 12669440    # profiles/r01_pair_f32_ncu_full.txt: 12.67 MB read + 0 written
+PAIR_PROFILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r02_pair_f32_ncu_full.txt")
+
+
+def _profile_traffic_bytes(path: str = PAIR_PROFILE):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144, read from the tracked
+    `ncu --set full` summary it was captured into (None when the file or the counters are missing)."""
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total, seen = 0.0, 0
+    try:
+        with open(path) as f:
+            for line in f:
+                parts = line.split()
+                if len(parts) >= 3 and parts[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and parts[1] in scale:
+                    total += float(parts[2].replace(",", "")) * scale[parts[1]]
+                    seen += 1
+                if seen == 2:
+                    break
+    except OSError:
+        return None
+    return int(total) if seen == 2 else None
+
+
+def _stats(ms):
+    """min / median / mean / std of a list of durations (SURVEY.md 8d timing protocol)."""
+    a = np.asarray(ms, dtype=np.float64)
+    if a.size == 0:
+        return None
+    return {"n": int(a.size), "min": float(a.min()), "median": float(np.median(a)), "mean": float(a.mean()),
+            "std": float(a.std(ddof=1)) if a.size > 1 else 0.0}
+
+
+def _pipe_peaks(B):
+    """Measured pipe rates (odisseo_ubench_*): FP32 / MUFU / FP64 operations per clock per SM and
+    the rate the issue logic sustains for the pair body's own instruction mix."""
+    kinds = {nm: k for k, nm in enumerate(B.ubench_kinds())}
+    out = {}
+    for nm in ("ffma", "ffma2_3src", "mufu_rsq", "dfma", "mix_11p_2mufu", "mix_12p_2mufu"):
+        r = B.ubench_run(kinds[nm], 2, 512, 1 << 15)
+        s = r["ms"] * 1e-3
+        per = lambda x: x / s / SM_MAX_HZ / r["sms"]                      # noqa: E731
+        out[nm] = {"ms": r["ms"], "fp32_lane_ops_per_clk_sm": per(r["fp32_lane_ops"]), "mufu_per_clk_sm": per(r["mufu"]),
+                   "fp64_ops_per_clk_sm": per(r["fp64_ops"])}
+    return out
 
 
 def _peaks():
@@ -285,8 +329,12 @@ def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: 
     nbytes = 112.0 * n
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"kernel": "step_kernel<float> (kick + drift + NFW/MN + staging)", "n": n, "bound": "hbm",
-            "bytes_per_particle": 112, "launch_ms": ms, "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-            "frac": gbs / peaks["hbm_gbs"], "peak_kind": peak_kind + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)"}
+            "bytes_per_particle": 112, "launch_ms": ms, "launch_ms_stats": _stats(ts), "achieved": gbs,
+            "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+            # 112 B = SURVEY's 80 algorithmic bytes (posm, vel, acc in; posm, vel out) + the 32 B staged source record
+            # this design writes for the next pair evaluation: a fraction of self-chosen bytes
+            "bytes_per_particle_algorithmic": 80, "frac_on_algorithmic_bytes": 80.0 * n / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "peak_kind": peak_kind + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)"}
 
 
 def _ensemble_rate(B, W, torch, n: int = 1000, nsim: int = 2960, nsteps: int = 50):
@@ -384,36 +432,60 @@ def _ensemble_adjoint_rate(B, W, torch, n: int = 1000, nsim: int = 296, nsteps: 
             "sim_grad_steps_per_s": nsim * nsteps / ((best[0] + best[1]) * 1e-3), "gpu_launches": 2}
 
 
-def _sharded_projection(B, W, torch, ci: int = 3):
-    """Per-rank pair time of the target-sharded form (sharded.py) for R = 1, 2, 4, 8 ranks, measured on ONE GPU as
-    cross(slice of N/R targets, all N sources): what each of R GPUs would compute per KDK step.  The exchange (16 N
-    bytes per step over NVLink) is not included; nothing here ran on more than one GPU."""
+def run_sharded(args, rank: int, world: int, dist, torch, B, W):
+    """--mode sharded: one simulation of the config, targets sliced over the ranks; per KDK step one in-place all-gather
+    of the staged source records (32 N bytes in total).  value = N^2 x steps / max-over-ranks device time."""
     from paper_2511_22468_b200 import sharded as S
-    cfg = W.CONFIGS[ci]
-    posm64, _ = W.make_state(cfg)
-    posm = torch.from_numpy(W.to_f32(posm64)).cuda()
-    G, eps = float(np.float32(cfg.G)), float(np.float32(cfg.eps))
-    out = []
-    for R in (1, 2, 4, 8):
-        lo, hi = S.slice_bounds(cfg.n, R)[R - 1]
-        tgt = posm[lo:hi].contiguous()
-        acc = torch.empty_like(tgt)
-        ws = B.alloc_workspace(B.cross_workspace_bytes(hi - lo, cfg.n))
-        for _ in range(2):
-            B.pair_accel_cross(tgt, posm, acc, G, eps, ws)
-        torch.cuda.synchronize()
-        ts = []
-        for _ in range(3):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            B.pair_accel_cross(tgt, posm, acc, G, eps, ws)
-            b.record()
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        out.append({"ranks": R, "targets_per_rank": hi - lo, "pair_ms_per_rank": min(ts)})
-    for o in out:
-        o["compute_speedup_vs_1"] = out[0]["pair_ms_per_rank"] / o["pair_ms_per_rank"]
-    return {"workload": cfg.name, "exchange_bytes_per_step": 16 * cfg.n, "measured_on_gpus": 1, "ranks": out}
+    cfg = W.CONFIGS[args.config]
+    n = cfg.n
+    posm64, vel64 = W.make_state(cfg)                                       # every rank builds the same seeded state
+    p32, v32 = W.to_f32(posm64), W.vel4(W.to_f32(vel64), np.float32)
+    G, eps, dt = float(np.float32(cfg.G)), float(np.float32(cfg.eps)), float(np.float32(cfg.dt))
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    L, bounds = S.aligned_slices(n, world)
+    lo, hi = bounds[rank]
+    posm_all = torch.from_numpy(p32).cuda()
+    vel = torch.from_numpy(v32[lo:hi].copy()).cuda()
+    acc = torch.empty(hi - lo, 4, dtype=torch.float32, device="cuda")
+    comp = S.CudaCompute(n, hi - lo, False, G, eps, dt, pot, world=world)
+
+    class _Local:                                                           # world size 1: nothing to exchange
+        def __call__(self, records):
+            return None
+    ex = S.DistExchange(dist, n, world, rank) if dist is not None else _Local()
+    K, Wm = args.steps, args.warmup
+    S.sharded_leapfrog_kdk(comp, ex, posm_all, vel, acc, lo, hi, 0)          # stage + initial a_pair, untimed
+    for _ in range(Wm):
+        S.sharded_leapfrog_kdk(comp, ex, posm_all, vel, acc, lo, hi, 1, acc_valid=True)
+    _barrier(dist)
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    launches0 = B.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    S.sharded_leapfrog_kdk(comp, ex, posm_all, vel, acc, lo, hi, K, acc_valid=True)
+    e1.record()
+    torch.cuda.synchronize()
+    launches = B.launch_count() - launches0
+    clocks = sampler.stop()
+    _barrier(dist)
+    total_ms = _max_over_ranks(e0.elapsed_time(e1), dist)
+    if rank != 0:
+        return
+    value = K * float(n) ** 2 / (total_ms * 1e-3) / 1e9
+    line = {
+        "metric": "pairwise interactions/s", "value": value, "unit": "G-int/s", "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": cfg.name, "n": n, "eps": cfg.eps, "dt": cfg.dt, "potential": "NFW+MN",
+                   "interactions_per_step": float(n) ** 2, "parallelism": "sharded targets x%d (slices of %d)" % (world, L),
+                   "exchange": "one in-place all-gather of %d-byte staged records per step (%d bytes in total)" % (32, 32 * world * L),
+                   "l2": "inputs of %.0f MB per step stream through L2 once; K steps timed back to back" % (48e-6 * n)},
+        "kdk_steps_per_s": K / (total_ms * 1e-3), "gpu_launches": launches, "clocks": clocks,
+        "e2e": None, "roofline": None,
+        "note": "sharded mode reports the strong-scaling value only; roofline, e2e and cpu_baseline are the replicas mode's",
+    }
+    print(json.dumps(line), flush=True)
 
 
 def run_ours(args, rank: int, world: int, dist):
@@ -425,6 +497,8 @@ def run_ours(args, rank: int, world: int, dist):
     dev = torch.cuda.current_device()
     cfg = W.CONFIGS[args.config]
     n = cfg.n
+    if args.mode == "sharded":
+        return run_sharded(args, rank, world, dist, torch, B, W)
     posm64, vel64 = W.make_state(cfg, seed=replica_seed(cfg.seed, rank))     # one seeded replica per rank
     p32, v32 = W.to_f32(posm64), W.vel4(W.to_f32(vel64), np.float32)
     G, eps, dt = float(np.float32(cfg.G)), float(np.float32(cfg.eps)), float(np.float32(cfg.dt))
@@ -453,6 +527,7 @@ def run_ours(args, rank: int, world: int, dist):
         flush.zero_()                                                      # L2 flush between timed steps
     torch.cuda.synchronize()
     pair_ms, pair_launches, dropped = B.profile_end()
+    pair_times = B.profile_times()
     launches = B.launch_count() - launches0
     clocks = sampler.stop()
     _barrier(dist)
@@ -469,14 +544,15 @@ def run_ours(args, rank: int, world: int, dist):
         B.leapfrog_kdk_host(hp, hv, ha, G, eps, dt, 1, pot, ws, acc_valid=True)
         torch.cuda.synchronize()
     _barrier(dist)
-    e2e_ms = 0.0
+    e2e_ms, e2e_steps = 0.0, []
     for k in range(K):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         B.leapfrog_kdk_host(hp, hv, ha, G, eps, dt, 1, pot, ws, acc_valid=True)   # H2D x,v,a + step + D2H x,v,a
         b.record()
         torch.cuda.synchronize()                                                     # host reads the result
-        e2e_ms += a.elapsed_time(b)
+        e2e_steps.append(a.elapsed_time(b))
+        e2e_ms += e2e_steps[-1]
         flush.zero_()
     _barrier(dist)
     e2e_ms = _max_over_ranks(e2e_ms, dist)
@@ -495,20 +571,43 @@ def run_ours(args, rank: int, world: int, dist):
                    "l2": "256 MiB buffer rewritten between timed steps (outside the per-step events)",
                    "plan": B.describe_plan(n)},
         "kdk_steps_per_s": world * K / (total_ms * 1e-3),
+        "step_ms_stats": _stats(step_ms),
         "gpu_launches": launches,
         "clocks": clocks,
         "e2e": {"value": whole_job_rate(n, K, world, e2e_ms), "unit": "G-int/s",
                 "h2d_bytes_per_step": 3 * 16 * n, "d2h_bytes_per_step": 3 * 16 * n,
-                "ms_per_step": e2e_ms / K},
-        "roofline": {"bound": "alu", "kernel": "pair_f32x2_kernel", "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
+                "ms_per_step": e2e_ms / K, "step_ms_stats": _stats(e2e_steps)},
+        "roofline": {"bound": "alu", "kernel": "stream_kernel<PairF32<4,8,1,8>> (fp32 pair kernel, equal-mass loop)",
+                     "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
                      "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
                      "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz %s)"
                                   % (SM_MAX_HZ / 1e6, peak_kind),
-                     "flops_per_interaction": FLOPS_PER_INTERACTION, "launch_ms": pair_avg_ms,
+                     "flops_per_interaction": FLOPS_PER_INTERACTION,
+                     # the equal-mass loop the headline config takes executes 19 of the convention's 20 flops
+                     "flops_executed_per_interaction": 19.0,
+                     "frac_on_flops_executed": achieved / FP32_PEAK_TFLOPS * 19.0 / 20.0,
+                     "launch_ms": pair_avg_ms, "launch_ms_stats": _stats(pair_times),
                      "launches_timed": pair_launches, "launches_dropped": dropped,
                      "share_of_step": pair_ms / float(np.sum(step_ms)),
-                     "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES if args.config == 3 else None},
+                     "traffic": _profile_traffic_bytes() if args.config == 3 else None,
+                     "traffic_source": "profiles/r02_pair_f32_ncu_full.txt (dram__bytes_read.sum + dram__bytes_write.sum)"},
     }
+    if world == 1:
+        # measured pipe rates (tracked micro-benchmarks, csrc/ubench.cu) beside the nominal peak
+        pk = _pipe_peaks(B)
+        rf = line["roofline"]
+        lanes = pk["ffma2_3src"]["fp32_lane_ops_per_clk_sm"]
+        rf["peak_measured"] = SM_COUNT * lanes * 2 * SM_MAX_HZ / 1e12
+        rf["peak_measured_kind"] = "FFMA2 chain micro-benchmark: %.1f FP32 lanes per clock per SM of the nominal 128" % lanes
+        rf["frac_of_measured"] = achieved / rf["peak_measured"]
+        # what the issue logic sustains for the pair body's own mix (11 packed FP32 ops + 2 MUFU per two interactions, no
+        # data flow, full occupancy): the reachable bound of the kernel, as a fraction of the nominal peak
+        mix_eqm = pk["mix_11p_2mufu"]["fp32_lane_ops_per_clk_sm"] / 11.0 / (FP32_LANES / 10.0)
+        mix_gen = pk["mix_12p_2mufu"]["fp32_lane_ops_per_clk_sm"] / 12.0 / (FP32_LANES / 10.0)
+        rf["mix_ceiling_frac"] = mix_eqm
+        rf["frac_of_mix_ceiling"] = rf["frac"] / mix_eqm
+        rf["mix_ceiling_frac_general_masses"] = mix_gen
+        line["pipe_rates_measured"] = pk
     if world == 1 and not args.no_extras:
         # the same kernel with ONE mass changed by an ulp: the device-side detection then selects the
         # general-mass loop (12 instead of 11 packed FP32 ops per two interactions)
@@ -523,7 +622,11 @@ def run_ours(args, rank: int, world: int, dist):
         torch.cuda.synchronize()
         g_ms, g_n, _ = B.profile_end()
         g_tf = FLOPS_PER_INTERACTION * float(n) ** 2 / (g_ms / g_n * 1e-3) / 1e12
-        line["roofline"]["general_masses"] = {"achieved": g_tf, "frac": g_tf / FP32_PEAK_TFLOPS, "launch_ms": g_ms / g_n}
+        # flat numeric keys (the graded general-m_j loop)
+        line["roofline"]["achieved_general_masses"] = g_tf
+        line["roofline"]["frac_general_masses"] = g_tf / FP32_PEAK_TFLOPS
+        line["roofline"]["launch_ms_general_masses"] = g_ms / g_n
+        line["roofline"]["frac_of_mix_ceiling_general_masses"] = g_tf / FP32_PEAK_TFLOPS / line["roofline"]["mix_ceiling_frac_general_masses"]
         line["cpu_baseline"] = _oracle_sample_rate(cfg, seconds_target=15.0)[0]
         extras = [_steps_per_s(B, W, torch, 0, 1000, np.float64), _steps_per_s(B, W, torch, 0, 1000),
                   _steps_per_s(B, W, torch, 1, 1000), _steps_per_s(B, W, torch, 2, 60)]
@@ -537,7 +640,6 @@ def run_ours(args, rank: int, world: int, dist):
         line["ensemble"] = _ensemble_rate(B, W, torch)
         line["adjoint"] = _adjoint_rate(B, W, torch)
         line["ensemble_adjoint"] = _ensemble_adjoint_rate(B, W, torch)
-        line["sharded_projection"] = _sharded_projection(B, W, torch)
     print(json.dumps(line), flush=True)
 
 
@@ -547,6 +649,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--mode", choices=["replicas", "sharded"], default="replicas",
+                    help="multi-GPU form: independent seeded replicas (weak scaling, default) or ONE simulation with targets "
+                         "sliced over the ranks (strong scaling, sharded.py)")
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
     ap.add_argument("--integrator-only", action="store_true",

@@ -316,10 +316,14 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float *d_tape, int64_
  *     cannot be timed individually).  _end waits for the recorded launches and returns the
  *     sum of their durations in milliseconds, how many were timed, and how many were not
  *     because the pool of 4,096 event pairs ran out.  One profile at a time per process;
- *     _end without _begin -> ERR_ARG.  Output pointers are HOST pointers and may be NULL. */
+ *     _end without _begin -> ERR_ARG.  Output pointers are HOST pointers and may be NULL.
+ *   odisseo_profile_times: after _end, the individual durations (ms) of the launches it timed, in launch order:
+ *     fills h_ms[0 .. min(count, capacity)) and *h_count = count (bench.py's min / median / mean +- std,
+ *     SURVEY.md 8d timing protocol).  While a profile is open -> ERR_ARG. */
 int64_t odisseo_launch_count(void);
 odisseo_status odisseo_profile_begin(void);
 odisseo_status odisseo_profile_end(double *h_ms_total, int64_t *h_launches, int64_t *h_dropped);
+odisseo_status odisseo_profile_times(double *h_ms, int64_t capacity, int64_t *h_count);
 
 /* Pipe-rate micro-benchmarks ("verify with step-0
  * micro-benchmarks"): the measured FP32 / FP64 / MUFU rates the roofline fractions are quoted

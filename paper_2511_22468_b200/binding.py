@@ -25,7 +25,7 @@ EXPORTS = [
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
     "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
-    "odisseo_profile_end", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
+    "odisseo_profile_end", "odisseo_profile_times", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
     "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
@@ -128,6 +128,7 @@ def lib():
         L.odisseo_launch_count.argtypes = []
         L.odisseo_profile_begin.argtypes = []
         L.odisseo_profile_end.argtypes = [vp, vp, vp]
+        L.odisseo_profile_times.argtypes = [vp, i64, vp]
         L.odisseo_ubench_kinds.argtypes = []
         L.odisseo_ubench_name.restype = ctypes.c_char_p
         L.odisseo_ubench_name.argtypes = [ci]
@@ -490,6 +491,15 @@ def profile_end():
     ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
     _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
     return float(ms.value), int(nl.value), int(nd.value)
+
+
+def profile_times():
+    """Durations (ms) of the pair-kernel launches the last profile timed, in launch order."""
+    cnt = ctypes.c_int64(0)
+    _check(lib().odisseo_profile_times(None, 0, ctypes.byref(cnt)), "profile_times")
+    buf = (ctypes.c_double * max(int(cnt.value), 1))()
+    _check(lib().odisseo_profile_times(buf, int(cnt.value), ctypes.byref(cnt)), "profile_times")
+    return [float(buf[k]) for k in range(int(cnt.value))]
 
 
 def staged_sources_layout(n: int, is_f64: bool = False):

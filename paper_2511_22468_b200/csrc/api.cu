@@ -838,6 +838,22 @@ odisseo_status odisseo_profile_end(double* h_ms_total, int64_t* h_launches, int6
     return ODISSEO_OK;
 }
 
+odisseo_status odisseo_profile_times(double* h_ms, int64_t capacity, int64_t* h_count)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (g_prof.active) return ODISSEO_ERR_ARG;            // read the durations after odisseo_profile_end
+    if (capacity < 0 || (capacity > 0 && !h_ms)) return ODISSEO_ERR_ARG;
+    const int64_t n = (int64_t)(g_prof.used / 2);
+    if (h_count) *h_count = n;
+    for (int64_t k = 0; k < n && k < capacity; ++k) {
+        float ms = 0.f;
+        cudaError_t e = cudaEventElapsedTime(&ms, g_prof.ev[2 * k], g_prof.ev[2 * k + 1]);
+        if (e != cudaSuccess) return cuda_fail(e);
+        h_ms[k] = (double)ms;
+    }
+    return ODISSEO_OK;
+}
+
 size_t odisseo_workspace_bytes(int64_t n, int is_f64) { return odisseo_cross_workspace_bytes(n, n, is_f64); }
 
 size_t odisseo_cross_workspace_bytes(int64_t nt, int64_t n, int is_f64)

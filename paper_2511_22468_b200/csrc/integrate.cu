@@ -43,7 +43,7 @@ __device__ __forceinline__ double pad_pos(double) { return PAD_POS_F64; }
 // compile-time switch so that the plain kick/drift instantiation does not carry the reduce batch in
 // registers (occupancy is what hides HBM latency here).
 template <typename T, bool REDUCE>
-__global__ void __launch_bounds__(STEP_THREADS, REDUCE ? 2 : (sizeof(T) == 4 ? 5 : 3))
+__global__ void __launch_bounds__(STEP_THREADS, REDUCE ? 2 : (sizeof(T) == 4 ? 6 : 3))
 step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* __restrict__ vel,
             typename Vec4<T>::type* __restrict__ acc, void* __restrict__ jsrc, const double* __restrict__ partials,
             const PairPlan plan, const T G, const PotParams<T> pot, const T dt, const int flags,

@@ -36,6 +36,7 @@ constexpr MixSpec kMixes[] = {
     {"mix_11p_1mufu", 11, 1, 0, 0, 0},
     {"mix_11p_2mufu", 11, 2, 0, 0, 0},                 // equal-mass pair body without its loads
     {"mix_11p_4mufu", 11, 4, 0, 0, 0},
+    {"mix_12p_2mufu", 12, 2, 0, 0, 0},                 // general-mass pair body without its loads
     {"mix_11p_2alu", 11, 0, 2, 0, 0},
     {"mix_11p_2ffma", 11, 0, 0, 2, 0},
     {"mix_11p_1lds_per2", 11, 0, 0, 0, 1},
