@@ -307,6 +307,26 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float *d_tape, int64_
                                                      double *d_gm, double *d_gparams, void *d_workspace,
                                                      size_t workspace_bytes, void *stream);
 
+/* Maximum Mean Discrepancy loss between simulated and observed streams, and its gradient (Fig. 2 step 4:
+ * "The resulting simulated stream is compared to the observed stream using the Maximum Mean Discrepancy (MMD), and the
+ * gradient of the loss is computed"; L39 "full 6D phase-space information"; L47).  The paper prints
+ * neither kernel nor estimator (reading R20): Gaussian kernel, one scale per coordinate, biased V-statistic,
+ *   k(u, v) = exp(-1/2 sum_d ((u_d - v_d) / sigma_d)^2),  d = x, y, z, vx, vy, vz,
+ *   MMD^2 = 1/n^2 sum_ii' k(x_i, x_i') + 1/m^2 sum_jj' k(y_j, y_j') - 2/(n m) sum_ij k(x_i, y_j).
+ * Batched like the ensemble calls: d_xpos, d_xvel [nsim][n][4] float (the final state of odisseo_ensemble_leapfrog_kdk_f32;
+ * lane 3 ignored) are the simulated clouds, d_ypos, d_yvel the observed one(s): [m][4] shared by every simulation
+ * (shared_y != 0) or [nsim][m][4].  h_sigma: 6 HOST doubles > 0 (ERR_ARG otherwise).  d_mmd2 [nsim] double out.
+ * d_gpos, d_gvel (both or neither; [nsim][n][4] float out, lane 3 = 0): d_grad_scale[sim] * dMMD^2/d(position, velocity)
+ * of every simulated point -- the layout of d_lx, d_lv of odisseo_ensemble_leapfrog_kdk_vjp_f32, so loss -> gradient ->
+ * pull-back stays on the device; d_grad_scale [nsim] double or NULL (= 1).  n, m >= 1 (ERR_ARG for an empty cloud),
+ * nsim <= 65,535; nsim == 0 -> OK no-op.  Sums: fp32 inside 256-point tiles, fp64 across tiles and blocks in fixed
+ * order (bit-reproducible).  Workspace: odisseo_mmd_workspace_bytes(n, m, nsim), 256-byte aligned. */
+size_t odisseo_mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim);
+odisseo_status odisseo_mmd2_f32(const float *d_xpos, const float *d_xvel, int64_t n, const float *d_ypos, const float *d_yvel,
+                                int64_t m, int64_t nsim, int shared_y, const double *h_sigma, const double *d_grad_scale,
+                                double *d_mmd2, float *d_gpos, float *d_gvel, void *d_workspace, size_t workspace_bytes,
+                                void *stream);
+
 /* Instrumentation (bench.py's gpu_launches and roofline legs).
  *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA
  *     graph replay counts its kernel nodes).  Host counter, no GPU work.

@@ -135,3 +135,39 @@ def ensemble_leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.
     dt [nsim].  Returns (posm_final, vel_final); gradients flow to posm0 (lane 3 = masses), vel0, theta and dt.
     checkpoint_every = K keeps a K-step tape instead of the whole trajectory (one extra forward pass in backward)."""
     return _EnsembleLeapfrogKDK.apply(posm0, vel0, theta, dt, G, eps, nsteps, checkpoint_every)
+
+
+class _MMD2(torch.autograd.Function):
+    """MMD^2 between simulated clouds and an observed one (odisseo_mmd2_f32).  forward: the value; backward: the same
+    kernel again with the upstream gradient as its per-simulation scale, so the cotangents of (posm, vel) come out of
+    the C ABI ready for the ensemble pull-back -- no gradient arithmetic in Python."""
+
+    @staticmethod
+    def forward(ctx, posm, vel, yposm, yvel, sigma):
+        x, v = posm.detach().contiguous(), vel.detach().contiguous()
+        single = x.dim() == 2
+        nsim, n = (1, x.shape[0]) if single else x.shape[:2]
+        m = yposm.shape[-2]
+        out = torch.empty(nsim, dtype=torch.float64, device=x.device)
+        ws = B.alloc_workspace(B.mmd_workspace_bytes(n, m, nsim))
+        B.mmd2(x, v, yposm.detach().contiguous(), yvel.detach().contiguous(), sigma, out, ws)
+        ctx.save_for_backward(x, v, yposm.detach().contiguous(), yvel.detach().contiguous())
+        ctx.meta = (tuple(float(s) for s in sigma), ws, single)
+        return out[0] if single else out
+
+    @staticmethod
+    def backward(ctx, g_out):
+        x, v, y, yv = ctx.saved_tensors
+        sigma, ws, single = ctx.meta
+        scale = g_out.detach().to(torch.float64).reshape(-1).contiguous()
+        out = torch.empty_like(scale)
+        gp, gv = torch.empty_like(x), torch.empty_like(v)
+        B.mmd2(x, v, y, yv, sigma, out, ws, gp, gv, scale)
+        return gp, gv, None, None, None
+
+
+def mmd2(posm: torch.Tensor, vel: torch.Tensor, yposm: torch.Tensor, yvel: torch.Tensor, sigma):
+    """Differentiable MMD^2 loss (Fig. 2 step 4): posm, vel float32 CUDA [nsim, n, 4] (or [n, 4]) simulated
+    clouds, yposm, yvel [m, 4] (shared) or [nsim, m, 4] observed; sigma: 6 kernel scales (x, y, z, vx, vy, vz).  Returns
+    [nsim] float64 (or a 0-d tensor); gradients flow to posm and vel."""
+    return _MMD2.apply(posm, vel, yposm, yvel, tuple(float(s) for s in sigma))

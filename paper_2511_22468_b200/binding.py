@@ -34,7 +34,7 @@ EXPORTS = [
     "odisseo_ensemble_leapfrog_kdk_vjp_f32", "odisseo_cross_workspace_bytes", "odisseo_pair_accel_cross_f32",
     "odisseo_pair_accel_cross_f64", "odisseo_staged_sources_layout", "odisseo_stage_sources_f32", "odisseo_stage_sources_f64",
     "odisseo_pair_accel_staged_f32", "odisseo_pair_accel_staged_f64", "odisseo_kick_drift_slice_f32",
-    "odisseo_kick_drift_slice_f64", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
+    "odisseo_kick_drift_slice_f64", "odisseo_mmd_workspace_bytes", "odisseo_mmd2_f32", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
 ]
 
 
@@ -104,6 +104,9 @@ def lib():
             getattr(L, "odisseo_pair_accel_staged_" + suffix).argtypes = [vp, i64, i64, vp, sc, sc, vp, sz, vp]
             getattr(L, "odisseo_kick_drift_slice_" + suffix).argtypes = [vp, vp, vp, i64, i64, i64, sc, sc, vp, ci, vp, sz, vp]
         L.odisseo_staged_sources_layout.argtypes = [i64, ci, vp]
+        L.odisseo_mmd_workspace_bytes.restype = sz
+        L.odisseo_mmd_workspace_bytes.argtypes = [i64, i64, i64]
+        L.odisseo_mmd2_f32.argtypes = [vp, vp, i64, vp, vp, i64, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
         L.odisseo_cross_workspace_bytes.restype = sz
         L.odisseo_cross_workspace_bytes.argtypes = [i64, i64, ci]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
@@ -491,6 +494,46 @@ def profile_end():
     ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
     _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
     return float(ms.value), int(nl.value), int(nd.value)
+
+
+def mmd_workspace_bytes(n: int, m: int, nsim: int = 1) -> int:
+    return int(lib().odisseo_mmd_workspace_bytes(int(n), int(m), int(nsim)))
+
+
+def mmd2(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch.Tensor, sigma: Sequence[float], out: torch.Tensor,
+         workspace: torch.Tensor, gpos: Optional[torch.Tensor] = None, gvel: Optional[torch.Tensor] = None,
+         grad_scale: Optional[torch.Tensor] = None, stream=None):
+    """MMD^2 between simulated clouds xpos/xvel [nsim, n, 4] (or [n, 4]) and observed ypos/yvel ([m, 4] shared, or
+    [nsim, m, 4]) into out [nsim] float64; with gpos/gvel also grad_scale * dMMD^2/d(xpos, xvel) (odisseo_mmd2_f32)."""
+    if xpos.dim() == 2:
+        xpos, xvel = xpos.unsqueeze(0), xvel.unsqueeze(0)
+        if gpos is not None:
+            gpos, gvel = gpos.unsqueeze(0), gvel.unsqueeze(0)
+    nsim, n = _ens_state(xpos, xvel, "xpos and xvel")
+    shared = ypos.dim() == 2
+    if shared:
+        m = _rec(ypos, "ypos")
+        _rec(yvel, "yvel", m)
+        if ypos.dtype != torch.float32 or yvel.dtype != torch.float32:
+            raise TypeError("mmd2 is float32")
+    else:
+        ns2, m = _ens_state(ypos, yvel, "ypos and yvel")
+        if ns2 != nsim:
+            raise ValueError("ypos holds %d clouds, expected 1 shared or %d" % (ns2, nsim))
+    _f64vec(out, "out", nsim)
+    if (gpos is None) != (gvel is None):
+        raise ValueError("gpos and gvel go together")
+    if gpos is not None:
+        ng, nn = _ens_state(gpos, gvel, "gpos and gvel")
+        if (ng, nn) != (nsim, n):
+            raise ValueError("gpos/gvel must match xpos/xvel")
+    if grad_scale is not None:
+        _f64vec(grad_scale, "grad_scale", nsim)
+    sig = (ctypes.c_double * 6)(*[float(v) for v in sigma])
+    _check(lib().odisseo_mmd2_f32(xpos.data_ptr(), xvel.data_ptr(), n, ypos.data_ptr(), yvel.data_ptr(), m, nsim, int(shared), sig,
+                                  grad_scale.data_ptr() if grad_scale is not None else None, out.data_ptr(),
+                                  gpos.data_ptr() if gpos is not None else None, gvel.data_ptr() if gvel is not None else None,
+                                  workspace.data_ptr(), workspace.numel(), _stream(stream)), "mmd2_f32")
 
 
 def profile_times():

@@ -1220,4 +1220,40 @@ odisseo_status odisseo_kick_drift_slice_f64(double* d_posm, double* d_vel, const
                                             size_t workspace_bytes, void* stream)
 { return kick_drift_slice_impl<double>(d_posm, d_vel, d_acc, n, lo, count, G, dt, pot, mode, d_workspace, workspace_bytes, stream); }
 
+size_t odisseo_mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim)
+{
+    if (n <= 0 || m <= 0 || nsim <= 0) return 0;
+    return mmd_workspace_bytes(n, m, nsim);
+}
+
+odisseo_status odisseo_mmd2_f32(const float* d_xpos, const float* d_xvel, int64_t n, const float* d_ypos, const float* d_yvel,
+                                int64_t m, int64_t nsim, int shared_y, const double* h_sigma, const double* d_grad_scale,
+                                double* d_mmd2, float* d_gpos, float* d_gvel, void* d_workspace, size_t workspace_bytes,
+                                void* stream)
+{
+    if (n < 0 || m < 0 || nsim < 0 || n > 0x7fffffff || m > 0x7fffffff || nsim > 65535) return ODISSEO_ERR_ARG;
+    if (nsim == 0) return ODISSEO_OK;
+    if (n == 0 || m == 0) return ODISSEO_ERR_ARG;          // the estimator divides by n and m
+    if (!d_xpos || !d_xvel || !d_ypos || !d_yvel || !h_sigma || !d_mmd2 || !d_workspace) return ODISSEO_ERR_NULL;
+    if ((d_gpos == nullptr) != (d_gvel == nullptr)) return ODISSEO_ERR_NULL;
+    if (misaligned(d_xpos, 16) || misaligned(d_xvel, 16) || misaligned(d_ypos, 16) || misaligned(d_yvel, 16) ||
+        misaligned(d_mmd2, 8) || misaligned(d_workspace, 256) || (d_gpos && (misaligned(d_gpos, 16) || misaligned(d_gvel, 16))) ||
+        (d_grad_scale && misaligned(d_grad_scale, 8)))
+        return ODISSEO_ERR_ALIGN;
+    double inv[6];
+    for (int c = 0; c < 6; ++c) {
+        if (!(h_sigma[c] > 0.0) || !isfinite(h_sigma[c])) return ODISSEO_ERR_ARG;
+        inv[c] = 1.0 / h_sigma[c];
+    }
+    if (workspace_bytes < mmd_workspace_bytes(n, m, nsim)) return ODISSEO_ERR_WORKSPACE;
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    cudaError_t e = launch_mmd_f32(d_xpos, d_xvel, n, d_ypos, d_yvel, m, shared_y != 0, inv, nsim, d_grad_scale, d_mmd2, d_gpos,
+                                   d_gvel, d_workspace, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
 }  // extern "C"

@@ -1,0 +1,207 @@
+// Maximum Mean Discrepancy between simulated and observed 6-D point clouds and its gradient with respect to the
+// simulated cloud (Fig. 2 step 4 "compared to the observed stream using the Maximum Mean Discrepancy
+// (MMD), and the gradient of the loss is computed"; L39 "full 6D phase-space information"; L47).
+// The paper prints neither kernel nor estimator; reading R20: Gaussian kernel with one scale per
+// coordinate, biased V-statistic,
+//
+//   k(u, v)     = exp(-1/2 sum_d ((u_d - v_d)/sigma_d)^2),  d = x, y, z, vx, vy, vz
+//   MMD^2(X, Y) = 1/n^2 sum_ii' k(x_i, x_i') + 1/m^2 sum_jj' k(y_j, y_j') - 2/(n m) sum_ij k(x_i, y_j)
+//   dMMD^2/dx_i = -2/(n^2 sigma^2) sum_i' k(x_i, x_i') (x_i - x_i') + 2/(n m sigma^2) sum_j k(x_i, y_j) (x_i - y_j)
+//
+// Batched like the ensemble kernels (the paper's grid search and gradient steps run thousands of N = 1,000 simulations
+// against one observed stream, L47): grid = (target blocks, simulations).  All-pairs tiling as in the pair kernels:
+// a thread keeps its target's six scaled coordinates u = x s_d, s_d = sqrt(log2(e)/2)/sigma_d, in registers, so that
+// k = ex2(-|u - u'|^2) is 6 FADD + 6 FFMA + 1 MUFU.EX2; source tiles of 256 points are staged scaled in shared memory
+// (structure of arrays, broadcast reads); sums are fp32 inside a tile and fp64 across tiles; per-block sums are added
+// in block order by a second kernel (fixed order, no atomics: bit-reproducible).  The gradient lands in the layout of
+// the pull-back's cotangents (float4 {d/dx, d/dy, d/dz, 0}), so loss -> gradient never leaves the device.
+#include "odisseo_common.cuh"
+
+namespace odisseo {
+
+namespace {
+
+constexpr int MMD_THREADS = 256;
+constexpr int MMD_TILE = 256;
+
+struct MmdScales { float s[6]; float back[6]; };    // u = x s_d;  back_d = 4 s_d ln 2 (below)
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+__device__ __forceinline__ double mmd_block_sum(double v, double* warp_scratch)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) warp_scratch[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < MMD_THREADS / 32; ++w) s += warp_scratch[w];
+    return s;
+}
+
+// One pass of the targets of block (blockIdx.x, sim) over a source cloud: returns sum_j k and, when GRAD, adds
+// sum_j k (u_src - u_tgt)_d into acc[0..5].
+template <bool GRAD>
+__device__ __forceinline__ double mmd_pass(const float4* __restrict__ spos, const float4* __restrict__ svel, const int ns,
+                                           const MmdScales& sc, const float (&u)[6], float (*tile)[MMD_TILE], double (&acc)[6])
+{
+    double total = 0.0;
+    for (int j0 = 0; j0 < ns; j0 += MMD_TILE) {
+        __syncthreads();                                     // the previous tile is consumed
+        const int j = j0 + threadIdx.x;
+        if (threadIdx.x < MMD_TILE) {
+            float4 p = make_float4(0.f, 0.f, 0.f, 0.f), v = p;
+            if (j < ns) { p = spos[j]; v = svel[j]; }
+            tile[0][threadIdx.x] = p.x * sc.s[0]; tile[1][threadIdx.x] = p.y * sc.s[1]; tile[2][threadIdx.x] = p.z * sc.s[2];
+            tile[3][threadIdx.x] = v.x * sc.s[3]; tile[4][threadIdx.x] = v.y * sc.s[4]; tile[5][threadIdx.x] = v.z * sc.s[5];
+        }
+        __syncthreads();
+        const int len = ns - j0 < MMD_TILE ? ns - j0 : MMD_TILE;
+        float ksum = 0.f, g[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll 4
+        for (int t = 0; t < len; ++t) {
+            float d[6], q = 0.f;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) { d[c] = tile[c][t] - u[c]; q = fmaf(d[c], d[c], q); }
+            const float k = ex2_approx(-q);
+            ksum += k;
+            if (GRAD) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) g[c] = fmaf(k, d[c], g[c]);
+            }
+        }
+        total += (double)ksum;                               // second summation level, as in the pair kernels
+        if (GRAD) {
+#pragma unroll
+            for (int c = 0; c < 6; ++c) acc[c] += (double)g[c];
+        }
+    }
+    return total;
+}
+
+// grid = (ceil(max(n, m) / 256), nsim).  Thread t of block b handles simulated point i = b*256 + t (xx and xy sums,
+// gradient) and observed point j = b*256 + t (yy sum).  block_sums[sim][block][3] = {sum k_xx, sum k_xy, sum k_yy}.
+template <bool GRAD>
+__global__ void __launch_bounds__(MMD_THREADS)
+mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, const int n, const float4* __restrict__ ypos,
+           const float4* __restrict__ yvel, const int m, const int shared_y, const MmdScales sc,
+           const double* __restrict__ grad_scale, float4* __restrict__ gpos, float4* __restrict__ gvel,
+           double* __restrict__ block_sums)
+{
+    __shared__ float tile[6][MMD_TILE];
+    __shared__ double warp_scratch[MMD_THREADS / 32];
+    const int64_t sim = blockIdx.y;
+    const float4* const XP = xpos + sim * n;
+    const float4* const XV = xvel + sim * n;
+    const float4* const YP = ypos + (shared_y ? 0 : sim * m);
+    const float4* const YV = yvel + (shared_y ? 0 : sim * m);
+    const int i = blockIdx.x * MMD_THREADS + threadIdx.x;
+
+    // ---- simulated point i against X and against Y ----------------------------------------------------------
+    float u[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (i < n) {
+        const float4 p = XP[i], v = XV[i];
+        u[0] = p.x * sc.s[0]; u[1] = p.y * sc.s[1]; u[2] = p.z * sc.s[2];
+        u[3] = v.x * sc.s[3]; u[4] = v.y * sc.s[4]; u[5] = v.z * sc.s[5];
+    }
+    double axx[6] = {0, 0, 0, 0, 0, 0}, axy[6] = {0, 0, 0, 0, 0, 0};
+    double sxx = 0.0, sxy = 0.0, syy = 0.0;
+    if (blockIdx.x * MMD_THREADS < n) {                       // block-uniform: the barriers inside are safe
+        sxx = mmd_pass<GRAD>(XP, XV, n, sc, u, tile, axx);
+        sxy = mmd_pass<GRAD>(YP, YV, m, sc, u, tile, axy);
+        if (i >= n) sxx = sxy = 0.0;
+        if (GRAD && i < n) {
+            // with k = ex2(-|u - u'|^2): dk/dx_d = -2 ln2 s_d k (u - u')_d, and the symmetric double sum doubles the xx
+            // term: dMMD^2/dx_{i,d} = 4 ln2 s_d [ sum_i' k (u_i' - u_i)_d / n^2 - sum_j k (u_j - u_i)_d / (n m) ];
+            // the accumulators hold exactly those two sums
+            const double gs = grad_scale ? grad_scale[sim] : 1.0;
+            const double cxx = gs / ((double)n * n), cxy = -gs / ((double)n * m);
+            float o[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) o[c] = (float)((cxx * axx[c] + cxy * axy[c]) * (double)sc.back[c]);
+            gpos[sim * n + i] = make_float4(o[0], o[1], o[2], 0.f);
+            gvel[sim * n + i] = make_float4(o[3], o[4], o[5], 0.f);
+        }
+    }
+    // ---- observed point j = i against Y (value only) ----------------------------------------------------------
+    if (blockIdx.x * MMD_THREADS < m) {
+        float w[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (i < m) {
+            const float4 p = YP[i], v = YV[i];
+            w[0] = p.x * sc.s[0]; w[1] = p.y * sc.s[1]; w[2] = p.z * sc.s[2];
+            w[3] = v.x * sc.s[3]; w[4] = v.y * sc.s[4]; w[5] = v.z * sc.s[5];
+        }
+        double unused[6] = {0, 0, 0, 0, 0, 0};
+        syy = mmd_pass<false>(YP, YV, m, sc, w, tile, unused);
+        if (i >= m) syy = 0.0;
+    }
+    const double bxx = mmd_block_sum(sxx, warp_scratch);
+    const double bxy = mmd_block_sum(sxy, warp_scratch);
+    const double byy = mmd_block_sum(syy, warp_scratch);
+    if (threadIdx.x == 0) {
+        double* o = block_sums + ((size_t)sim * gridDim.x + blockIdx.x) * 3;
+        o[0] = bxx; o[1] = bxy; o[2] = byy;
+    }
+}
+
+// mmd2[sim] = sum_blocks xx / n^2 + sum_blocks yy / m^2 - 2 sum_blocks xy / (n m), blocks in order.
+__global__ void __launch_bounds__(32)
+mmd_final_kernel(const double* __restrict__ block_sums, const int nblocks, const int64_t nsim, const int n, const int m,
+                 double* __restrict__ out)
+{
+    const int64_t sim = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (sim >= nsim) return;
+    double xx = 0.0, xy = 0.0, yy = 0.0;
+    for (int b = 0; b < nblocks; ++b) {
+        const double* o = block_sums + ((size_t)sim * nblocks + b) * 3;
+        xx += o[0]; xy += o[1]; yy += o[2];
+    }
+    out[sim] = xx / ((double)n * n) + yy / ((double)m * m) - 2.0 * xy / ((double)n * m);
+}
+
+}  // namespace
+
+size_t mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim)
+{
+    const int64_t big = n > m ? n : m;
+    const size_t blocks = (size_t)((big + MMD_THREADS - 1) / MMD_THREADS);
+    return ((size_t)nsim * blocks * 3 * sizeof(double) + 255) & ~(size_t)255;
+}
+
+cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel, int64_t m,
+                           int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale, double* mmd2,
+                           float* gpos, float* gvel, void* ws, cudaStream_t stream)
+{
+    MmdScales sc;
+    for (int c = 0; c < 6; ++c) {
+        const double s = inv_sigma[c] * 0.84932180028801904272;      // sqrt(log2(e) / 2)
+        sc.s[c] = (float)s;
+        sc.back[c] = (float)(4.0 * s * 0.69314718055994530942);      // 4 ln2 s_d
+    }
+    const int64_t big = n > m ? n : m;
+    const dim3 grid((unsigned)((big + MMD_THREADS - 1) / MMD_THREADS), (unsigned)nsim);
+    double* block_sums = static_cast<double*>(ws);
+    const float4* xp = reinterpret_cast<const float4*>(xpos);
+    const float4* xv = reinterpret_cast<const float4*>(xvel);
+    const float4* yp = reinterpret_cast<const float4*>(ypos);
+    const float4* yv = reinterpret_cast<const float4*>(yvel);
+    if (gpos)
+        mmd_kernel<true><<<grid, MMD_THREADS, 0, stream>>>(xp, xv, (int)n, yp, yv, (int)m, shared_y, sc, grad_scale,
+                                                           reinterpret_cast<float4*>(gpos), reinterpret_cast<float4*>(gvel), block_sums);
+    else
+        mmd_kernel<false><<<grid, MMD_THREADS, 0, stream>>>(xp, xv, (int)n, yp, yv, (int)m, shared_y, sc, nullptr, nullptr, nullptr,
+                                                            block_sums);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    mmd_final_kernel<<<(unsigned)((nsim + 31) / 32), 32, 0, stream>>>(block_sums, (int)grid.x, nsim, (int)n, (int)m, mmd2);
+    return cudaGetLastError();
+}
+
+}  // namespace odisseo

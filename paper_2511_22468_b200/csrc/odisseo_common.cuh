@@ -347,6 +347,11 @@ cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* p
 cudaError_t launch_ensemble_vjp_f32(const float* tape, const EnsembleParams64* params, int shared_params, int n,
                                     int64_t nsim, int64_t nsteps, int with_eps_G, float* lx, float* lv, double* gm,
                                     double* gparams, int accumulate, cudaStream_t stream);
+// mmd.cu
+size_t mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim);
+cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel, int64_t m,
+                           int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale, double* mmd2,
+                           float* gpos, float* gvel, void* ws, cudaStream_t stream);
 cudaError_t configure_pair_f32();
 cudaError_t configure_pair_f64();
 
