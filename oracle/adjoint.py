@@ -32,6 +32,7 @@ from __future__ import annotations
 import numpy as np
 
 PARAM_NAMES = ("M_s", "r_s", "M_d", "a", "b")
+BULGE_PARAM_NAMES = ("M_b", "r_c")                        # alpha (the shape) is not differentiated
 
 
 def pair_accel_vjp(posm, c, G, eps):
@@ -68,13 +69,30 @@ def _nfw_parts(x, G, Ms, rs):
     return r, cc, mu, F, dF_dr
 
 
-def ext_accel_vjp(posm, c, G, nfw=None, mn=None):
-    """(gx [n,3], gparams {M_s, r_s, M_d, a, b}, gG): cotangent c pulled back through a_NFW + a_MN."""
+def ext_accel_vjp(posm, c, G, nfw=None, mn=None, bulge=None):
+    """(gx [n,3], gparams {M_s, r_s, M_d, a, b, M_b, r_c}, gG): cotangent c pulled back through a_NFW + a_MN + a_bulge."""
     x = np.asarray(posm, dtype=np.float64)[:, :3]
     c = np.asarray(c, dtype=np.float64)
     gx = np.zeros_like(x)
-    gp = dict.fromkeys(PARAM_NAMES, 0.0)
+    gp = dict.fromkeys(PARAM_NAMES + BULGE_PARAM_NAMES, 0.0)
     gG = 0.0
+    if bulge is not None and bulge[0] > 0:
+        # a = -G M_b F(r) x,  F = P(s, t)/r^3,  t = (r/r_c)^2,  dP/dt = t^(s-1) e^-t / Gamma(s)
+        from scipy import special
+        Mb, alpha, rc = bulge
+        s_ = 0.5 * (3.0 - alpha)
+        r = np.linalg.norm(x, axis=1)
+        t = (r / rc) ** 2
+        P = special.gammainc(s_, t)
+        dP_dt = np.exp((s_ - 1.0) * np.log(t) - t - special.gammaln(s_))
+        F = P / r ** 3
+        dF_dr = dP_dt * (2.0 * r / rc ** 2) / r ** 3 - 3.0 * P / r ** 4
+        xc = np.einsum("ik,ik->i", x, c)
+        gx += -G * Mb * (F[:, None] * c + (dF_dr / r * xc)[:, None] * x)
+        a = -G * Mb * F[:, None] * x
+        gp["M_b"] += float(np.sum(a * c)) / Mb
+        gG += float(np.sum(a * c)) / G
+        gp["r_c"] += float(np.sum(-G * Mb * (dP_dt * (-2.0 * t / rc)) / r ** 3 * xc))
     if nfw is not None and nfw[0] > 0:
         Ms, rs = nfw
         r, cc, mu, F, dF_dr = _nfw_parts(x, G, Ms, rs)
@@ -111,47 +129,47 @@ def ext_accel_vjp(posm, c, G, nfw=None, mn=None):
     return gx, gp, gG
 
 
-def _total_accel(posm, G, eps, nfw, mn):
+def _total_accel(posm, G, eps, nfw, mn, bulge=None):
     from oracle import oracle as O
-    pot = O.Potential.make(nfw=nfw, mn=mn) if (nfw is not None or mn is not None) else None
+    pot = O.Potential.make(nfw=nfw, mn=mn, bulge=bulge) if (nfw is not None or mn is not None or bulge is not None) else None
     acc, _ = O.pair_accel(posm, G, eps)
     if pot is not None:
         acc = acc + O.ext_accel(posm, G, pot)
     return acc
 
 
-def accel_vjp(posm, c, G, eps, nfw=None, mn=None):
+def accel_vjp(posm, c, G, eps, nfw=None, mn=None, bulge=None):
     """Cotangent c pulled back through a = a_pair + a_ext: (gx, gm, gparams, gG, geps)."""
     gx, gm, gG, geps = pair_accel_vjp(posm, c, G, eps)
-    ex, gp, eG = ext_accel_vjp(posm, c, G, nfw, mn)
+    ex, gp, eG = ext_accel_vjp(posm, c, G, nfw, mn, bulge)
     return gx + ex, gm, gp, gG + eG, geps
 
 
-def leapfrog_kdk_vjp(posm, vel, G, eps, dt, nsteps, lam_x, lam_v, nfw=None, mn=None):
+def leapfrog_kdk_vjp(posm, vel, G, eps, dt, nsteps, lam_x, lam_v, nfw=None, mn=None, bulge=None):
     """Reverse-mode derivative of nsteps KDK steps (oracle.leapfrog_kdk) of a loss with final-state cotangents
     lam_x = dL/dx_N, lam_v = dL/dv_N.  Returns a dict: x0, v0 [n,3]; m [n]; M_s, r_s, M_d, a, b, dt, G, eps."""
     posm = np.array(posm, dtype=np.float64)
     v = np.array(vel, dtype=np.float64)
-    xs, vs, accs = [posm.copy()], [v.copy()], [_total_accel(posm, G, eps, nfw, mn)]
+    xs, vs, accs = [posm.copy()], [v.copy()], [_total_accel(posm, G, eps, nfw, mn, bulge)]
     for _ in range(nsteps):                               # forward, textbook order, taping (x_k, v_k, a_k)
         vh = vs[-1] + 0.5 * dt * accs[-1]
         p = xs[-1].copy()
         p[:, :3] += dt * vh
-        a = _total_accel(p, G, eps, nfw, mn)
+        a = _total_accel(p, G, eps, nfw, mn, bulge)
         xs.append(p)
         vs.append(vh + 0.5 * dt * a)
         accs.append(a)
     Lv = np.array(lam_v, dtype=np.float64)
     Lx = np.array(lam_x, dtype=np.float64)
     out = {"m": np.zeros(posm.shape[0]), "dt": 0.0, "G": 0.0, "eps": 0.0}
-    out.update(dict.fromkeys(PARAM_NAMES, 0.0))
+    out.update(dict.fromkeys(PARAM_NAMES + BULGE_PARAM_NAMES, 0.0))
 
     def pull(k, w):
-        gx, gm, gp, gG, geps = accel_vjp(xs[k], w * Lv, G, eps, nfw, mn)
+        gx, gm, gp, gG, geps = accel_vjp(xs[k], w * Lv, G, eps, nfw, mn, bulge)
         out["m"] += gm
         out["G"] += gG
         out["eps"] += geps
-        for name in PARAM_NAMES:
+        for name in PARAM_NAMES + BULGE_PARAM_NAMES:
             out[name] += gp[name]
         return gx
 

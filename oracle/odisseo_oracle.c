@@ -31,7 +31,9 @@
  * force, Newton's third law, translation/permutation invariance, MN(a=0,b=eps)
  * == softened point mass, finite differences of the potentials, Poisson
  * equation, NFW circular speed, two-body circular and Kepler orbits, leapfrog
- * order / energy / reversibility / L_z, Plummer W = -3 pi G M^2 / (32 a).
+ * order / energy / reversibility / L_z, Plummer W = -3 pi G M^2 / (32 a); bulge:
+ * enclosed mass against 40-digit quadrature of rho, Poisson, finite differences,
+ * point-mass and power-law limits, scipy's incomplete gamma (tests/test_oracle_bulge.py).
  * No function here is "parity unpinned".
  *
  * Layouts: posm = n records of 4 doubles {x, y, z, m}; vel, acc = n records of
@@ -47,7 +49,8 @@
 
 typedef struct { double M_s, r_s; } oracle_nfw;    /* M_s <= 0 disables the term */
 typedef struct { double M, a, b; } oracle_mn;      /* M   <= 0 disables the term */
-typedef struct { oracle_nfw nfw; oracle_mn mn; } oracle_potential;
+typedef struct { double M_b, alpha, r_c; } oracle_bulge;   /* M_b <= 0 disables the term */
+typedef struct { oracle_nfw nfw; oracle_mn mn; oracle_bulge bulge; } oracle_potential;
 
 int oracle_num_threads(void)
 {
@@ -176,7 +179,52 @@ static void mn_acc(double G, const oracle_mn *p, double x, double y, double z, d
     a[0] = f * x; a[1] = f * y; a[2] = f * z * (s / B);
 }
 
-/* External acceleration a_NFW + a_MN per particle; pot == NULL -> zeros. acc: n x 3. */
+/*
+ * Bulge of galpy's MWPotential2014 ("we adopt the MWPotential2014 model from galpy"; DESIGN.md reading
+ * R21): a spherical power law with an exponential cut-off,
+ *   rho(r) = A r^-alpha exp(-(r/r_c)^2),   total mass M_b = 2 pi A r_c^(3-alpha) Gamma(s),  s = (3 - alpha)/2,
+ *   M(<r)  = M_b P(s, t),  t = (r/r_c)^2,  P = regularised lower incomplete gamma function,
+ *   a(x)   = -G M(<r) x / r^3,
+ *   Phi(r) = -G M(<r)/r - 4 pi G int_r^inf rho r' dr' = -G M_b [ P(s, t)/r + Gamma(s - 1/2, t) / (r_c Gamma(s)) ]
+ * (alpha < 2 so that Phi(0) = -G M_b Gamma(s - 1/2)/(r_c Gamma(s)) is finite; MWPotential2014: alpha = 1.8, r_c = 1.9 kpc).
+ * P(s, t) is evaluated by its all-positive Kummer series  t^s e^-t / Gamma(s+1) * sum_k t^k / ((s+1)...(s+k)),
+ * which converges for every t (no cancellation; up to ~t + 60 terms); for t > 60, 1 - P < 1e-26: P = 1 to rounding.
+ */
+static double gamma_p(double s, double t)
+{
+    if (t <= 0.0) return 0.0;
+    if (t > 60.0) return 1.0;
+    double term = 1.0, sum = 1.0;
+    for (int k = 1; k < 4000; ++k) {
+        term *= t / (s + k);
+        sum += term;
+        if (term < 1e-18 * sum) break;
+    }
+    const double p = exp(s * log(t) - t - lgamma(s + 1.0)) * sum;
+    return p < 1.0 ? p : 1.0;
+}
+
+static double bulge_phi(double G, const oracle_bulge *p, double x, double y, double z)
+{
+    const double s = 0.5 * (3.0 - p->alpha);
+    const double r = sqrt(x * x + y * y + z * z);
+    const double t = (r / p->r_c) * (r / p->r_c);
+    const double outer = tgamma(s - 0.5) * (1.0 - gamma_p(s - 0.5, t)) / (p->r_c * tgamma(s));
+    if (r == 0.0) return -G * p->M_b * outer;
+    return -G * p->M_b * (gamma_p(s, t) / r + outer);
+}
+
+static void bulge_acc(double G, const oracle_bulge *p, double x, double y, double z, double a[3])
+{
+    const double s = 0.5 * (3.0 - p->alpha);
+    const double r = sqrt(x * x + y * y + z * z);
+    if (r == 0.0) { a[0] = a[1] = a[2] = 0.0; return; }
+    const double t = (r / p->r_c) * (r / p->r_c);
+    const double f = -G * p->M_b * gamma_p(s, t) / (r * r * r);
+    a[0] = f * x; a[1] = f * y; a[2] = f * z;
+}
+
+/* External acceleration a_NFW + a_MN + a_bulge per particle; pot == NULL -> zeros. acc: n x 3. */
 void oracle_ext_accel(int64_t n, const double *posm, double G,
                       const oracle_potential *pot, double *acc)
 {
@@ -190,11 +238,15 @@ void oracle_ext_accel(int64_t n, const double *posm, double G,
             mn_acc(G, &pot->mn, posm[4 * i], posm[4 * i + 1], posm[4 * i + 2], t);
             a[0] += t[0]; a[1] += t[1]; a[2] += t[2];
         }
+        if (pot && pot->bulge.M_b > 0.0) {
+            bulge_acc(G, &pot->bulge, posm[4 * i], posm[4 * i + 1], posm[4 * i + 2], t);
+            a[0] += t[0]; a[1] += t[1]; a[2] += t[2];
+        }
         acc[3 * i] = a[0]; acc[3 * i + 1] = a[1]; acc[3 * i + 2] = a[2];
     }
 }
 
-/* External potential Phi_NFW + Phi_MN per particle (per unit mass). phi: n. */
+/* External potential Phi_NFW + Phi_MN + Phi_bulge per particle (per unit mass). phi: n. */
 void oracle_ext_potential(int64_t n, const double *posm, double G,
                           const oracle_potential *pot, double *phi)
 {
@@ -204,6 +256,8 @@ void oracle_ext_potential(int64_t n, const double *posm, double G,
             p += nfw_phi(G, &pot->nfw, posm[4 * i], posm[4 * i + 1], posm[4 * i + 2]);
         if (pot && pot->mn.M > 0.0)
             p += mn_phi(G, &pot->mn, posm[4 * i], posm[4 * i + 1], posm[4 * i + 2]);
+        if (pot && pot->bulge.M_b > 0.0)
+            p += bulge_phi(G, &pot->bulge, posm[4 * i], posm[4 * i + 1], posm[4 * i + 2]);
         phi[i] = p;
     }
 }

@@ -41,15 +41,20 @@ class MN(ctypes.Structure):
     _fields_ = [("M", ctypes.c_double), ("a", ctypes.c_double), ("b", ctypes.c_double)]
 
 
+class Bulge(ctypes.Structure):
+    _fields_ = [("M_b", ctypes.c_double), ("alpha", ctypes.c_double), ("r_c", ctypes.c_double)]
+
+
 class Potential(ctypes.Structure):
-    """NFW{M_s, r_s} + MN{M, a, b}; a mass <= 0 disables that term."""
-    _fields_ = [("nfw", NFW), ("mn", MN)]
+    """NFW{M_s, r_s} + MN{M, a, b} + bulge{M_b, alpha, r_c}; a mass <= 0 disables that term."""
+    _fields_ = [("nfw", NFW), ("mn", MN), ("bulge", Bulge)]
 
     @classmethod
-    def make(cls, nfw=None, mn=None):
+    def make(cls, nfw=None, mn=None, bulge=None):
         p = cls()
         p.nfw = NFW(*(nfw if nfw else (0.0, 1.0)))
         p.mn = MN(*(mn if mn else (0.0, 1.0, 1.0)))
+        p.bulge = Bulge(*(bulge if bulge else (0.0, 1.8, 1.0)))
         return p
 
 
