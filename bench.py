@@ -376,7 +376,7 @@ def _adjoint_rate(B, W, torch, n: int = 16384, nsteps: int = 20):
     ws = B.alloc_workspace(max(B.workspace_bytes(n), B.vjp_workspace_bytes(n)))
     tape = torch.empty(B.tape_bytes(n, nsteps) // 4, dtype=torch.float32, device="cuda")
     gm = torch.empty(n, dtype=torch.float64, device="cuda")
-    gp = torch.empty(8, dtype=torch.float64, device="cuda")
+    gp = torch.empty(B.NGRAD, dtype=torch.float64, device="cuda")
     times = []
     for rep in range(3):
         posm, vel = posm0.clone(), vel0.clone()
@@ -410,7 +410,7 @@ def _ensemble_adjoint_rate(B, W, torch, n: int = 1000, nsim: int = 296, nsteps: 
                              mn=(cfg.mn[0] * rng.uniform(0.5, 2.0), cfg.mn[1], cfg.mn[2]))) for _ in range(nsim)]
     tape = torch.empty(B.ensemble_tape_bytes(n, nsim, nsteps) // 4, dtype=torch.float32, device="cuda")
     gm = torch.empty(nsim, n, dtype=torch.float64, device="cuda")
-    gp = torch.empty(nsim, 8, dtype=torch.float64, device="cuda")
+    gp = torch.empty(nsim, B.NGRAD, dtype=torch.float64, device="cuda")
     best = None
     for _ in range(2):
         p, v = posm.clone(), vel.clone()

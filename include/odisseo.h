@@ -61,8 +61,13 @@ typedef enum {
 typedef struct { double M_s, r_s; } odisseo_nfw;
 /* Miyamoto-Nagai: Phi = -G M / sqrt(R^2 + (a + sqrt(z^2 + b^2))^2).  M <= 0 disables; b > 0. */
 typedef struct { double M, a, b; } odisseo_mn;
+/* Bulge of galpy's MWPotential2014 (reading R21): spherical power law with exponential cut-off,
+ * rho = A r^-alpha exp(-(r/r_c)^2), total mass M_b = 2 pi A r_c^(3-alpha) Gamma((3-alpha)/2);  a = -G M_b P(s, t) x / r^3 with
+ * s = (3-alpha)/2, t = (r/r_c)^2 and P the regularised lower incomplete gamma function.  M_b <= 0 disables; 0 <= alpha < 2,
+ * r_c > 0 required when enabled (MWPotential2014: alpha = 1.8, r_c = 1.9 kpc, M_b = 4.5e9 Msun).  a(0) := 0. */
+typedef struct { double M_b, alpha, r_c; } odisseo_bulge;
 /* A NULL odisseo_potential pointer means "no external potential" (config 0). HOST struct. */
-typedef struct { odisseo_nfw nfw; odisseo_mn mn; } odisseo_potential;
+typedef struct { odisseo_nfw nfw; odisseo_mn mn; odisseo_bulge bulge; } odisseo_potential;
 
 /* Library version string, e.g. "odisseo-b200 0.1 (sm_100a)". Never NULL. */
 const char *odisseo_version(void);
@@ -229,13 +234,13 @@ odisseo_status odisseo_diagnostics_f64(const double *d_posm, const double *d_vel
  *   a(x) = a_pair(x; m, G, eps) + a_NFW(x) + a_MN(x):
  *     d_gx [n][4]      (da/dx)^T c                      (pad lane 0)
  *     d_gm [n] double  d(c.a)/dm_i
- *     d_gparams [8] double, DEVICE: d(c.a)/d(M_s, r_s, M_d, a, b, G, eps), slot 7 = 0
+ *     d_gparams [10] double, DEVICE: d(c.a)/d(M_s, r_s, M_d, a, b, G, eps), slot 7 = 0, slots 8, 9 = d/d(M_b, r_c)
  * odisseo_leapfrog_kdk_tape_*: odisseo_leapfrog_kdk_* (acc_valid = 0) that also records the nsteps + 1
  *   snapshots {posm, vel, pair-only acc} k = 0..nsteps into d_tape (odisseo_tape_bytes(n, nsteps, is_f64)
  *   bytes: snapshot k at byte offset k * 3 * n * record size).  Final state bit-identical to the plain call.
  * odisseo_leapfrog_kdk_vjp_*: given the tape and the cotangents of the final state, d_lx = dL/dx_N and
  *   d_lv = dL/dv_N ([n][4], in/out), returns in place dL/dx_0 and dL/dv_0, and
- *     d_gm [n] double  dL/dm_i        d_gparams [8] double: dL/d(M_s, r_s, M_d, a, b, G, eps, dt)
+ *     d_gm [n] double  dL/dm_i        d_gparams [10] double: dL/d(M_s, r_s, M_d, a, b, G, eps, dt, M_b, r_c)
  *   (dt at fixed nsteps, i.e. t_end / nsteps; M_s, r_s, M_d, a, b as in odisseo_potential, disabled terms give 0).
  * with_eps_G == 0 leaves the G and eps slots 0 and skips their terms in the O(N^2) loop (neither is in the
  * paper's parameter vectors; ~15 % of the pull-back's instructions).
@@ -291,8 +296,8 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_f32(float *d_posm, float *d_vel, in
  *     k = 0..nsteps, {posm, vel, TOTAL acceleration} ([nsim][nsteps+1][3][n][4] float,
  *     odisseo_ensemble_tape_bytes(n, nsim, nsteps) bytes).  Final state identical to the plain call.
  *   odisseo_ensemble_leapfrog_kdk_vjp_f32: d_lx, d_lv [nsim][n][4] hold dL/dx_N, dL/dv_N of every simulation on
- *     entry and dL/dx_0, dL/dv_0 on exit; d_gm [nsim][n] double = dL/dm_i; d_gparams [nsim][8] double =
- *     dL/d(M_s, r_s, M_d, a, b, G, eps, dt) of each simulation.  h_params as in the forward call (the same
+ *     entry and dL/dx_0, dL/dv_0 on exit; d_gm [nsim][n] double = dL/dm_i; d_gparams [nsim][10] double =
+ *     dL/d(M_s, r_s, M_d, a, b, G, eps, dt, M_b, r_c) of each simulation.  h_params as in the forward call (the same
  *     records).  accumulate != 0: d_gm and d_gparams are added to instead of overwritten (a backward pass cut
  *     into segments, the later segment first: no gradient arithmetic is left to the caller).
  *     One CTA per simulation, the whole backward time loop in one kernel. */

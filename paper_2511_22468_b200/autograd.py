@@ -20,8 +20,18 @@ from . import binding as B
 
 
 def _potential(theta) -> B.Potential:
+    """theta = (M_s, r_s, M_d, a, b) or, with the bulge of MWPotential2014, (M_s, r_s, M_d, a, b, M_b, alpha, r_c)."""
     t = [float(x) for x in theta.detach().cpu().tolist()]
-    return B.Potential.make(nfw=(t[0], t[1]), mn=(t[2], t[3], t[4]))
+    return B.Potential.make(nfw=(t[0], t[1]), mn=(t[2], t[3], t[4]), bulge=(t[5], t[6], t[7]) if len(t) == 8 else None)
+
+
+def _theta_grad(gp, theta):
+    """Gradient slots of the C ABI (binding.GRADIENT_FIELDS) re-ordered like theta; the bulge shape alpha gets 0."""
+    idx = [0, 1, 2, 3, 4] if theta.shape[-1] == 5 else [0, 1, 2, 3, 4, 8, 8, 9]
+    g = gp[..., idx].clone()
+    if theta.shape[-1] == 8:
+        g[..., 6] = 0
+    return g.to(theta.dtype).to(theta.device)
 
 
 class _LeapfrogKDK(torch.autograd.Function):
@@ -49,11 +59,11 @@ class _LeapfrogKDK(torch.autograd.Function):
         lx[:, 3] = 0
         lv[:, 3] = 0
         gm = torch.empty(n, dtype=torch.float64, device=lx.device)
-        gp = torch.empty(8, dtype=torch.float64, device=lx.device)
+        gp = torch.empty(B.NGRAD, dtype=torch.float64, device=lx.device)
         B.leapfrog_kdk_vjp(tape, n, G, eps, float(dt), nsteps, _potential(theta), lx, lv, gm, gp, ws)
         g_posm0 = lx
         g_posm0[:, 3] = gm.to(lx.dtype) + g_mass_final
-        g_theta = gp[:5].to(theta.dtype).to(theta.device)
+        g_theta = _theta_grad(gp, theta)
         g_dt = gp[7].to(dt.dtype).to(dt.device).reshape(dt.shape)
         return g_posm0, lv, g_theta, g_dt, None, None, None
 
@@ -68,9 +78,8 @@ def leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.Tensor, d
 
 
 def _ens_params(theta, dt, G, eps):
-    th, dts = theta.detach().cpu().tolist(), dt.detach().cpu().tolist()
-    return [(float(G), float(eps), float(dts[k]), B.Potential.make(nfw=(th[k][0], th[k][1]), mn=(th[k][2], th[k][3], th[k][4])))
-            for k in range(len(dts))]
+    dts = dt.detach().cpu().tolist()
+    return [(float(G), float(eps), float(dts[k]), _potential(theta[k])) for k in range(len(dts))]
 
 
 class _EnsembleLeapfrogKDK(torch.autograd.Function):
@@ -114,7 +123,7 @@ class _EnsembleLeapfrogKDK(torch.autograd.Function):
         lv[:, :, 3] = 0
         # the C ABI accumulates the segment gradients itself (accumulate flag): no gradient arithmetic here
         gm_tot = torch.empty(nsim, n, dtype=torch.float64, device=lx.device)
-        gp_tot = torch.empty(nsim, 8, dtype=torch.float64, device=lx.device)
+        gp_tot = torch.empty(nsim, B.NGRAD, dtype=torch.float64, device=lx.device)
         for s in range(len(segments) - 1, -1, -1):
             k = segments[s]
             if starts:                                                    # recompute this segment with a tape
@@ -125,7 +134,7 @@ class _EnsembleLeapfrogKDK(torch.autograd.Function):
                 seg_tape = tape
             B.ensemble_leapfrog_kdk_vjp(seg_tape, params, k, lx, lv, gm_tot, gp_tot, ws, accumulate=s < len(segments) - 1)
         lx[:, :, 3] = gm_tot.to(lx.dtype) + g_mass_final
-        return (lx, lv, gp_tot[:, :5].to(theta.dtype).to(theta.device), gp_tot[:, 7].to(dt.dtype).to(dt.device),
+        return (lx, lv, _theta_grad(gp_tot, theta), gp_tot[:, 7].to(dt.dtype).to(dt.device),
                 None, None, None, None)
 
 

@@ -56,15 +56,21 @@ class _MN(ctypes.Structure):
     _fields_ = [("M", ctypes.c_double), ("a", ctypes.c_double), ("b", ctypes.c_double)]
 
 
+class _Bulge(ctypes.Structure):
+    _fields_ = [("M_b", ctypes.c_double), ("alpha", ctypes.c_double), ("r_c", ctypes.c_double)]
+
+
 class Potential(ctypes.Structure):
-    """odisseo_potential: NFW{M_s, r_s} + MN{M, a, b}; a mass <= 0 disables the term."""
-    _fields_ = [("nfw", _NFW), ("mn", _MN)]
+    """odisseo_potential: NFW{M_s, r_s} + MN{M, a, b} + bulge{M_b, alpha, r_c}; a mass <= 0 disables the term."""
+    _fields_ = [("nfw", _NFW), ("mn", _MN), ("bulge", _Bulge)]
 
     @classmethod
-    def make(cls, nfw: Optional[Sequence[float]] = None, mn: Optional[Sequence[float]] = None):
+    def make(cls, nfw: Optional[Sequence[float]] = None, mn: Optional[Sequence[float]] = None,
+             bulge: Optional[Sequence[float]] = None):
         p = cls()
         p.nfw = _NFW(*(nfw if nfw else (0.0, 1.0)))
         p.mn = _MN(*(mn if mn else (0.0, 1.0, 1.0)))
+        p.bulge = _Bulge(*(bulge if bulge else (0.0, 1.8, 1.0)))
         return p
 
 
@@ -309,7 +315,8 @@ def leapfrog_kdk_host(posm: torch.Tensor, vel: torch.Tensor, acc: Optional[torch
            "leapfrog_kdk_host_" + sfx)
 
 
-GRADIENT_FIELDS = ("M_s", "r_s", "M_d", "a", "b", "G", "eps", "dt")
+GRADIENT_FIELDS = ("M_s", "r_s", "M_d", "a", "b", "G", "eps", "dt", "M_b", "r_c")
+NGRAD = len(GRADIENT_FIELDS)
 
 
 def vjp_workspace_bytes(n: int, is_f64: bool = False) -> int:
@@ -332,7 +339,7 @@ def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: 
     _rec(cot, "cot", n)
     _rec(gx, "gx", n)
     _f64vec(gm, "gm", n)
-    _f64vec(gparams, "gparams", 8)
+    _f64vec(gparams, "gparams", NGRAD)
     sfx = _suffix(posm)
     fn = getattr(lib(), "odisseo_accel_vjp_" + sfx)
     _check(fn(posm.data_ptr(), cot.data_ptr(), n, G, eps, _pot(pot), int(bool(with_eps_G)), gx.data_ptr(), gm.data_ptr(),
@@ -360,11 +367,11 @@ def leapfrog_kdk_vjp(tape: torch.Tensor, n: int, G: float, eps: float, dt: float
                      lx: torch.Tensor, lv: torch.Tensor, gm: torch.Tensor, gparams: torch.Tensor,
                      workspace: torch.Tensor, with_eps_G: bool = False, stream=None):
     """Reverse-mode derivative of nsteps KDK steps from the tape: lx, lv [n,4] hold dL/dx_N, dL/dv_N on entry and
-    dL/dx_0, dL/dv_0 on exit; gm [n] and gparams [8] (GRADIENT_FIELDS) are float64 outputs."""
+    dL/dx_0, dL/dv_0 on exit; gm [n] and gparams [10] (GRADIENT_FIELDS) are float64 outputs."""
     _rec(lx, "lx", n)
     _rec(lv, "lv", n)
     _f64vec(gm, "gm", n)
-    _f64vec(gparams, "gparams", 8)
+    _f64vec(gparams, "gparams", NGRAD)
     sfx = _suffix(lx)
     if tape.dtype != lx.dtype or not tape.is_cuda or tape.numel() < 12 * n * (nsteps + 1):
         raise ValueError("tape does not hold nsteps + 1 snapshots of the state's dtype")
@@ -443,10 +450,10 @@ def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch
                               gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor,
                               with_eps_G: bool = False, accumulate: bool = False, stream=None):
     """Gradients of every simulation of a batch from its tape: lx, lv [nsim, n, 4] in/out; gm float64 [nsim, n];
-    gparams float64 [nsim, 8] (GRADIENT_FIELDS); accumulate adds to gm and gparams instead of overwriting them."""
+    gparams float64 [nsim, 10] (GRADIENT_FIELDS); accumulate adds to gm and gparams instead of overwriting them."""
     nsim, n = _ens_state(lx, lv, "lx and lv")
     _f64vec(gm, "gm", nsim * n)
-    _f64vec(gparams, "gparams", nsim * 8)
+    _f64vec(gparams, "gparams", nsim * NGRAD)
     if tape.dtype != torch.float32 or not tape.is_cuda or tape.numel() * 4 < ensemble_tape_bytes(n, nsim, nsteps):
         raise ValueError("tape does not hold nsteps + 1 snapshots of every simulation")
     arr = _sim_params(params)

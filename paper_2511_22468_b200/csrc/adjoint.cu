@@ -331,7 +331,8 @@ __device__ __forceinline__ double vjp_pre_step(const VjpPreArgs<T>& a, const Pai
 }
 
 // Row reduce (fixed unit order) + external part + accumulation:  gx_out (+)= G [m] rows + h,  gm_out (+)= -G row,
-// block_sums[block][0..6] (+)= this block's terms of d/d(M_s, r_s, M_d, a, b, G, eps); slot 7 (+)= its dt terms.
+// block_sums[block][0..6] (+)= this block's terms of d/d(M_s, r_s, M_d, a, b, G, eps); slot 7 (+)= its dt terms;
+// slots 8, 9 (+)= d/d(M_b, r_c).
 // REDUCE = false skips the reduce (the step k = N, before any pull-back); PRE = true appends the backward KDK step
 // of snapshot k - 1 for the same particle (everything it needs is this particle's own Lx, Lv): one O(N) launch per
 // backward step instead of three.  Block sums accumulate over the steps of a backward pass in fixed step order;
@@ -350,9 +351,9 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
     pdl_launch_dependents();
     pdl_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    double term[8];
+    double term[VJP_NOUT];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) term[k] = 0.0;
+    for (int k = 0; k < VJP_NOUT; ++k) term[k] = 0.0;
     V4 o; o.x = o.y = o.z = o.w = (T)0;
     if (REDUCE && i < plan.n) {
         double r[COMPS];
@@ -360,7 +361,7 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
         // the equal-mass loop left the common mass out of the x, y, z (and eps, G) sums
         const double mu = __ldcg(plan_eqm_word(jsrc, plan)) != 0 ? (double)posm[0].w : 1.0;
         const V4 p = posm[i], c = cot[i];
-        double h[3], t[6];
+        double h[3], t[8];
         ext_vjp(pot, G, (double)p.x, (double)p.y, (double)p.z, (double)c.x, (double)c.y, (double)c.z, h, t);
         const double Gm = G * mu;
         double gx = fma(Gm, r[0], h[0]), gy = fma(Gm, r[1], h[1]), gz = fma(Gm, r[2], h[2]);
@@ -375,6 +376,8 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
         gm_out[i] = gm;
 #pragma unroll
         for (int k = 0; k < 5; ++k) term[k] = t[k];
+        term[8] = t[6];
+        term[9] = t[7];
         if (EG) {
             term[5] = t[5] + mu * r[COMPS - 1];                         // d/dG: external + pair (sum_j m_j f d.c_i)
             term[6] = eps * Gm * r[COMPS - 2];
@@ -388,25 +391,25 @@ vjp_finish_kernel(const typename AVec4<T>::type* __restrict__ posm, const typena
     }
     if ((int64_t)blockIdx.x * blockDim.x < plan.n) {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
+        for (int k = 0; k < VJP_NOUT; ++k) {
             const double sum = vjp_block_sum(term[k], warp_scratch);
             if (threadIdx.x == 0) {
-                double* slot = block_sums + (size_t)blockIdx.x * 8 + k;
+                double* slot = block_sums + (size_t)blockIdx.x * VJP_NOUT + k;
                 *slot = accumulate ? *slot + sum : sum;
             }
         }
     }
 }
 
-// out[0..7] (+)= sum over blocks, in block order, of block_sums.
+// out[0..9] (+)= sum over blocks, in block order, of block_sums.
 __global__ void __launch_bounds__(VJP_THREADS)
 vjp_final_kernel(const double* __restrict__ block_sums, const int nblocks, double* __restrict__ out, const int accumulate)
 {
     __shared__ double warp_scratch[VJP_THREADS / 32];
     pdl_wait();
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < VJP_NOUT; ++k) {
         double v = 0.0;
-        for (int b = threadIdx.x; b < nblocks; b += VJP_THREADS) v += block_sums[(size_t)b * 8 + k];
+        for (int b = threadIdx.x; b < nblocks; b += VJP_THREADS) v += block_sums[(size_t)b * VJP_NOUT + k];
         const double tot = vjp_block_sum(v, warp_scratch);
         if (threadIdx.x == 0) out[k] = accumulate ? out[k] + tot : tot;
     }
@@ -448,7 +451,7 @@ void vjp_geometry(int is_f64, int* ipt, int* cthreads, int* tile, int* minb)
 static size_t vjp_rows_bytes(const PairPlan& plan) { return ((size_t)plan.U * 6 * plan.IB * sizeof(double) + 255) & ~(size_t)255; }
 static size_t vjp_blocks_bytes(const PairPlan& plan)
 {
-    return ((size_t)((plan_npad(plan) + VJP_THREADS - 1) / VJP_THREADS) * 8 * sizeof(double) + 255) & ~(size_t)255;
+    return ((size_t)((plan_npad(plan) + VJP_THREADS - 1) / VJP_THREADS) * VJP_NOUT * sizeof(double) + 255) & ~(size_t)255;
 }
 
 size_t vjp_workspace_bytes(const PairPlan& plan, int is_f64)

@@ -105,14 +105,14 @@ __device__ __forceinline__ double vjp_block_sum(double v, double* warp_scratch)
 }
 
 // Cotangent c pulled back through a_NFW + a_MN at x, in fp64: h = (da/dx)^T c, and the terms of the
-// parameter sums t[0..5] = d(c.a)/d(M_s, r_s, M_d, a, b, G).
+// parameter sums t[0..7] = d(c.a)/d(M_s, r_s, M_d, a, b, G, M_b, r_c).
 __device__ __forceinline__ void ext_vjp(const PotParams<double>& pot, const double G, const double x, const double y,
                                         const double z, const double cx, const double cy, const double cz,
-                                        double (&h)[3], double (&t)[6])
+                                        double (&h)[3], double (&t)[8])
 {
     h[0] = h[1] = h[2] = 0.0;
 #pragma unroll
-    for (int k = 0; k < 6; ++k) t[k] = 0.0;
+    for (int k = 0; k < 8; ++k) t[k] = 0.0;
     const double invG = G != 0.0 ? 1.0 / G : 0.0;
     if (pot.GMs != 0.0) {
         const double r2 = fma(x, x, fma(y, y, z * z));
@@ -152,6 +152,25 @@ __device__ __forceinline__ void ext_vjp(const PotParams<double>& pot, const doub
         t[5] += ca * invG;
         t[3] += -pot.GMd * fma(q, s, cz * z * iB * iD3);
         t[4] += -pot.GMd * fma(q, s * b * iB, cz * z * (-pot.a * b * iB * iB * iB) * iD3);
+    }
+    if (pot.GMb != 0.0) {
+        // a = -G M_b F(r) x,  F = P(s, tt)/r^3,  tt = (r/r_c)^2,  dP/dtt = tt^(s-1) e^-tt / Gamma(s)
+        const double r2 = fma(x, x, fma(y, y, z * z));
+        if (r2 > 0.0) {
+            const double r = sqrt(r2), ir = 1.0 / r, ir3 = ir * ir * ir;
+            const double tt = r2 * pot.inv_rc * pot.inv_rc;
+            double dP;
+            const double P = gamma_p(pot.bs, tt, pot.lgam_s, &dP);
+            const double F = P * ir3;
+            const double dF_over_r = (dP * 2.0 * pot.inv_rc * pot.inv_rc * ir3 * r - 3.0 * P * ir3 * ir) * ir;
+            const double xc = fma(x, cx, fma(y, cy, z * cz));
+            const double k1 = -pot.GMb * F, k2 = -pot.GMb * dF_over_r * xc;
+            h[0] += fma(k1, cx, k2 * x); h[1] += fma(k1, cy, k2 * y); h[2] += fma(k1, cz, k2 * z);
+            const double ca = k1 * xc;                                   // c . a_bulge
+            t[6] += ca * (G * (1.0 / pot.GMb));                          // / M_b
+            t[5] += ca * invG;
+            t[7] += -pot.GMb * (dP * (-2.0 * tt * pot.inv_rc)) * ir3 * xc;   // dP/dr_c = dP/dtt (-2 tt / r_c)
+        }
     }
 }
 

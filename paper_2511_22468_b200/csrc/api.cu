@@ -189,6 +189,18 @@ template <typename T> odisseo_status make_pot(T G, const odisseo_potential* pot,
         out.a = (T)pot->mn.a;
         out.b2 = (T)(pot->mn.b * pot->mn.b);
     }
+    if (pot->bulge.M_b > 0.0) {
+        const odisseo_bulge& b = pot->bulge;
+        if (!(b.r_c > 0.0) || !(b.alpha >= 0.0) || !(b.alpha < 2.0) || !isfinite(b.M_b) || !isfinite(b.r_c)) return ODISSEO_ERR_ARG;
+        const double s = 0.5 * (3.0 - b.alpha);
+        out.GMb = (T)((double)G * b.M_b);
+        out.inv_rc = (T)(1.0 / b.r_c);
+        out.bs = (T)s;
+        out.lgam_s = (T)lgamma(s);
+        out.bs_half = (T)(s - 0.5);
+        out.lgam_s_half = (T)lgamma(s - 0.5);
+        out.phi_outer = (T)(tgamma(s - 0.5) / (b.r_c * tgamma(s)));
+    }
     return ODISSEO_OK;
 }
 
@@ -665,7 +677,7 @@ odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps
     if (!gparams) return ODISSEO_ERR_NULL;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     if (n == 0) {
-        cudaError_t e0 = cudaMemsetAsync(gparams, 0, 8 * sizeof(double), s);
+        cudaError_t e0 = cudaMemsetAsync(gparams, 0, VJP_NOUT * sizeof(double), s);
         return e0 == cudaSuccess ? ODISSEO_OK : cuda_fail(e0);
     }
     if (!posm || !cot || !gx || !gm || !ws) return ODISSEO_ERR_NULL;
@@ -711,7 +723,7 @@ odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int
     if (n < 0 || nsteps < 0) return ODISSEO_ERR_ARG;
     if (!gparams) return ODISSEO_ERR_NULL;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    cudaError_t e = cudaMemsetAsync(gparams, 0, 8 * sizeof(double), s);
+    cudaError_t e = cudaMemsetAsync(gparams, 0, VJP_NOUT * sizeof(double), s);
     if (e != cudaSuccess) return cuda_fail(e);
     if (n == 0) return ODISSEO_OK;
     if (!tape || !lx || !lv || !gm || !ws) return ODISSEO_ERR_NULL;

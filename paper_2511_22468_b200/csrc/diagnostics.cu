@@ -11,6 +11,7 @@
 //   final   : one block adds the block sums in index order -> 16 doubles
 // Every reduction has a fixed order: results are bit-reproducible run to run.
 #include "odisseo_common.cuh"
+#include "ext_potential.cuh"
 
 namespace odisseo {
 
@@ -51,6 +52,13 @@ __device__ __forceinline__ double ext_potential(const PotParams<double>& pot, do
     if (pot.GMd != 0.0) {
         const double sB = pot.a + sqrt(fma(z, z, pot.b2));
         phi += -pot.GMd / sqrt(fma(x, x, fma(y, y, sB * sB)));
+    }
+    if (pot.GMb != 0.0) {
+        // Phi = -G M_b [ P(s, t)/r + Gamma(s - 1/2, t) / (r_c Gamma(s)) ],  Gamma(a, t) = Gamma(a) (1 - P(a, t))
+        const double r = sqrt(fma(x, x, fma(y, y, z * z)));
+        const double t = (r * pot.inv_rc) * (r * pot.inv_rc);
+        const double outer = pot.phi_outer * (1.0 - gamma_p(pot.bs_half, t, pot.lgam_s_half));
+        phi += -pot.GMb * ((r > 0.0 ? gamma_p(pot.bs, t, pot.lgam_s) / r : 0.0) + outer);
     }
     return phi;
 }

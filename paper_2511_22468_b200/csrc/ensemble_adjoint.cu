@@ -41,7 +41,7 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
     const float hdt = 0.5f * dt;
 
     float Lx[NQ][3], Lv[NQ][3], an[NQ][3];                              // an = a_{k+1} of the previous iteration
-    double gm[NQ], gp[8];
+    double gm[NQ], gp[VJP_NOUT];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
         const int i = q * VJP_THREADS + tid;
@@ -53,7 +53,7 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
         gm[q] = 0.0;
     }
 #pragma unroll
-    for (int k = 0; k < 8; ++k) gp[k] = 0.0;
+    for (int k = 0; k < VJP_NOUT; ++k) gp[k] = 0.0;
 
     // equal masses (checked once on snapshot 0; masses never change): the mass leaves the pair loop
     int differs = 0;
@@ -159,7 +159,7 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             if (q * VJP_THREADS + tid < n) {
-                double h[3], t6[6];
+                double h[3], t6[8];
                 ext_vjp(prm.pot, prm.G, (double)xs[q][0], (double)xs[q][1], (double)xs[q][2], (double)cs[q][0], (double)cs[q][1],
                         (double)cs[q][2], h, t6);
                 const double gscale = (eqm && !EG) ? prm.G * (double)mass0 : prm.G;   // the equal-mass loop left m out
@@ -169,6 +169,8 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
                 gm[q] += -prm.G * (double)o[q][3];
 #pragma unroll
                 for (int c = 0; c < 5; ++c) gp[c] += t6[c];
+                gp[8] += t6[6];
+                gp[9] += t6[7];
                 if (EG) {
                     gp[5] += t6[5] + (double)o[q][5];
                     gp[6] += prm.eps * prm.G * (double)o[q][4];
@@ -187,9 +189,9 @@ ensemble_vjp_kernel(const float4* __restrict__ tape, const EnsembleParams64* __r
         }
     }
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < VJP_NOUT; ++k) {
         const double tot = vjp_block_sum(gp[k], warp_scratch);
-        if (tid == 0) gparams[sim * 8 + k] = accumulate ? gparams[sim * 8 + k] + tot : tot;
+        if (tid == 0) gparams[sim * VJP_NOUT + k] = accumulate ? gparams[sim * VJP_NOUT + k] + tot : tot;
     }
 }
 

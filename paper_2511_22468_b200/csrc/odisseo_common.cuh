@@ -140,7 +140,11 @@ PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms);   // n
 template <typename T> struct PotParams {
     T GMs, inv_rs;   // NFW: G*M_s, 1/r_s   (GMs == 0 disables)
     T GMd, a, b2;    // MN:  G*M, a, b^2    (GMd == 0 disables)
+    // bulge (GMb == 0 disables): G*M_b, 1/r_c, s = (3 - alpha)/2, ln Gamma(s), and for the potential
+    // s - 1/2, ln Gamma(s - 1/2) and Gamma(s - 1/2) / (r_c Gamma(s))
+    T GMb, inv_rc, bs, lgam_s, bs_half, lgam_s_half, phi_outer;
 };
+constexpr int VJP_NOUT = 10;      // gradient slots: M_s, r_s, M_d, a, b, G, eps, dt, M_b, r_c
 
 // Per-simulation parameters of the ensemble kernel (ensemble.cu), device layout, 32 bytes.
 struct EnsembleParams {

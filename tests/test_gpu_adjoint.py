@@ -28,7 +28,7 @@ def gpu_accel_vjp(posm, c, G, eps, pot, dtype, with_eps_G=True):
     n = posm.shape[0]
     gx = torch.full((n, 4), float("nan"), dtype=torch.float32 if dtype == np.float32 else torch.float64, device="cuda")
     gm = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
-    gp = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
+    gp = torch.full((B.NGRAD,), float("nan"), dtype=torch.float64, device="cuda")
     ws = B.alloc_workspace(B.vjp_workspace_bytes(n, dtype == np.float64))
     B.accel_vjp(dev(posm, dtype), dev(pad4(c, dtype), dtype), G, eps, pot, gx, gm, gp, ws, with_eps_G=with_eps_G)
     torch.cuda.synchronize()
@@ -110,7 +110,7 @@ def gpu_leapfrog_vjp(p, v, G, eps, dt, nsteps, pot, lx, lv, dtype):
     B.leapfrog_kdk_tape(posm, vel, acc, G, eps, dt, nsteps, pot, tape, ws)
     dlx, dlv = dev(pad4(lx, dtype), dtype), dev(pad4(lv, dtype), dtype)
     gm = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
-    gp = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
+    gp = torch.full((B.NGRAD,), float("nan"), dtype=torch.float64, device="cuda")
     B.leapfrog_kdk_vjp(tape, n, G, eps, dt, nsteps, pot, dlx, dlv, gm, gp, ws, with_eps_G=True)
     torch.cuda.synchronize()
     final = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())

@@ -186,7 +186,7 @@ def test_degenerate_sizes_are_ok_noops_or_zeros():
     B.kick_drift(e4, e4.clone(), e4.clone(), 1.0, 0.1, pot, 3, ws)
     out = torch.full((16,), 7.0, dtype=torch.float64, device="cuda")
     B.diagnostics(e4, e4.clone(), 1.0, 0.1, pot, out, ws)
-    gp = torch.full((8,), 7.0, dtype=torch.float64, device="cuda")
+    gp = torch.full((B.NGRAD,), 7.0, dtype=torch.float64, device="cuda")
     B.accel_vjp(e4, e4.clone(), 1.0, 0.1, pot, e4.clone(), torch.zeros(0, dtype=torch.float64, device="cuda"), gp, ws)
     torch.cuda.synchronize()
     assert torch.all(out == 0) and torch.all(gp == 0)

@@ -138,7 +138,7 @@ def _run_vjp(posm, vel, bparams, nsteps, lx, lv, with_eps_G=False):
     B.ensemble_leapfrog_kdk_tape(dp, dv, bparams, nsteps, tape, ws)
     dlx, dlv = torch.from_numpy(lx.copy()).cuda(), torch.from_numpy(lv.copy()).cuda()
     gm = torch.full((nsim, n), float("nan"), dtype=torch.float64, device="cuda")
-    gp = torch.full((nsim, 8), float("nan"), dtype=torch.float64, device="cuda")
+    gp = torch.full((nsim, B.NGRAD), float("nan"), dtype=torch.float64, device="cuda")
     B.ensemble_leapfrog_kdk_vjp(tape, bparams, nsteps, dlx, dlv, gm, gp, ws, with_eps_G=with_eps_G)
     torch.cuda.synchronize()
     return dp.cpu().numpy(), dv.cpu().numpy(), dlx.cpu().numpy(), dlv.cpu().numpy(), gm.cpu().numpy(), gp.cpu().numpy()
