@@ -26,9 +26,13 @@
  *   - posm and acc (and vel) must not alias or overlap: ODISSEO_ERR_ARG.
  *   - Errors are return codes, never exceptions or aborts: NULL pointer -> ERR_NULL,
  *     misaligned pointer -> ERR_ALIGN, n < 0, nsteps < 0, eps <= 0 (the kernels include the
- *     self term, which is exactly 0 only when eps > 0), non-finite scalar, enabled MN term
- *     with b <= 0 or enabled NFW term with r_s <= 0 -> ERR_ARG, workspace too small ->
- *     ERR_WORKSPACE, device is not compute capability 10.x -> ERR_ARCH, CUDA failure ->
+ *     self term, which is exactly 0 only when eps > 0) or eps so small that the self term
+ *     overflows in the precision of the call (eps^-3 in the forward calls: fp32 needs
+ *     eps >= 1e-12, fp64 eps^2 >= 1e-30; 3 eps^-5 in the fp32 reverse-mode and ensemble-gradient
+ *     calls: eps >= 1e-7), eps^2 > 1e30, non-finite scalar, enabled MN term with b <= 0,
+ *     enabled NFW term with r_s <= 0, enabled bulge with r_c <= 0 or alpha outside [0, 2)
+ *     -> ERR_ARG, workspace too small -> ERR_WORKSPACE, device is not compute capability
+ *     10.0 (the library holds sm_100a code only, no PTX fallback) -> ERR_ARCH, CUDA failure ->
  *     ERR_CUDA (code in odisseo_last_cuda_error()).  n == 0 or nsteps == 0 is an OK no-op
  *     (nsteps == 0 with acc_valid == 0 still evaluates acc).  Inputs are not screened for
  *     NaN/Inf particles; they propagate.
@@ -74,6 +78,13 @@ const char *odisseo_version(void);
 const char *odisseo_status_string(odisseo_status s);
 /* cudaError_t value of the most recent ODISSEO_ERR_CUDA on this thread (0 if none). */
 int odisseo_last_cuda_error(void);
+
+/* Releases what the library keeps between calls: the cached CUDA-graph executables of odisseo_leapfrog_kdk_* and the
+ * CUDA events of odisseo_profile_*.  Call with no library work in flight on other host threads; every entry point may
+ * be used again afterwards (the caches refill).  ERR_ARG while a profile is open.  The library's other globals are a
+ * launch counter and per-device attribute records; calls from several host threads are safe (the graph cache is
+ * looked up, filled, evicted and launched under one lock). */
+odisseo_status odisseo_shutdown(void);
 
 /* Upper bound, in bytes, of the device scratch any pair/leapfrog call on n particles
  * needs (staged source records + one row of fixed-order partial sums per work unit).

@@ -25,7 +25,7 @@ EXPORTS = [
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
     "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
-    "odisseo_profile_end", "odisseo_profile_times", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
+    "odisseo_profile_end", "odisseo_profile_times", "odisseo_shutdown", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
     "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
@@ -138,12 +138,31 @@ def lib():
         L.odisseo_profile_begin.argtypes = []
         L.odisseo_profile_end.argtypes = [vp, vp, vp]
         L.odisseo_profile_times.argtypes = [vp, i64, vp]
+        L.odisseo_shutdown.argtypes = []
         L.odisseo_ubench_kinds.argtypes = []
         L.odisseo_ubench_name.restype = ctypes.c_char_p
         L.odisseo_ubench_name.argtypes = [ci]
         L.odisseo_ubench_run.argtypes = [ci, ci, ci, i64, vp, vp]
         _lib = L
     return _lib
+
+
+def _on_device(fn):
+    """The C library works on the CURRENT CUDA device and the stream passed in.  Every CUDA tensor argument must live
+    on one device; that device is made current for the call (so tensors on cuda:1 never launch on GPU 0) and the
+    default stream argument resolves to ITS current stream."""
+    import functools
+
+    @functools.wraps(fn)
+    def wrapper(*args, **kwargs):
+        devs = {t.device for t in list(args) + list(kwargs.values()) if isinstance(t, torch.Tensor) and t.is_cuda}
+        if len(devs) > 1:
+            raise ValueError("%s: tensors live on different devices %s" % (fn.__name__, sorted(str(d) for d in devs)))
+        if not devs:
+            return fn(*args, **kwargs)
+        with torch.cuda.device(next(iter(devs))):
+            return fn(*args, **kwargs)
+    return wrapper
 
 
 def _check(status: int, where: str):
@@ -219,6 +238,7 @@ def plan_probe(n: int, is_f64: bool, num_sms: int, u: int, c: int, nt: Optional[
     return tuple(int(v) for v in out)
 
 
+@_on_device
 def pair_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, eps: float, workspace: torch.Tensor, stream=None):
     """acc[n,4] = pair acceleration of posm[n,4] (odisseo_pair_accel_f32/_f64)."""
     n = _rec(posm, "posm")
@@ -236,6 +256,7 @@ def cross_workspace_bytes(nt: int, n: int, is_f64: bool = False) -> int:
     return int(lib().odisseo_cross_workspace_bytes(int(nt), int(n), int(bool(is_f64))))
 
 
+@_on_device
 def pair_accel_cross(targets: torch.Tensor, sources: torch.Tensor, acc: torch.Tensor, G: float, eps: float,
                      workspace: torch.Tensor, stream=None):
     """acc[nt,4] = acceleration at targets[nt,4] due to sources[n,4] (odisseo_pair_accel_cross_f32/_f64)."""
@@ -251,6 +272,7 @@ def pair_accel_cross(targets: torch.Tensor, sources: torch.Tensor, acc: torch.Te
     return acc
 
 
+@_on_device
 def pair_accel_soa(x, y, z, m, ax, ay, az, G: float, eps: float, workspace: torch.Tensor, stream=None):
     n = x.numel()
     for t in (x, y, z, m, ax, ay, az):
@@ -261,6 +283,7 @@ def pair_accel_soa(x, y, z, m, ax, ay, az, G: float, eps: float, workspace: torc
                                             workspace.numel(), _stream(stream)), "pair_accel_soa_f32")
 
 
+@_on_device
 def ext_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, pot: Optional[Potential], accumulate: bool = False,
               stream=None):
     n = _rec(posm, "posm")
@@ -272,6 +295,7 @@ def ext_accel(posm: torch.Tensor, acc: torch.Tensor, G: float, pot: Optional[Pot
     return acc
 
 
+@_on_device
 def leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, eps: float, dt: float,
                  nsteps: int, pot: Optional[Potential], workspace: torch.Tensor, acc_valid: bool = False, stream=None):
     """nsteps KDK steps in place on device tensors (odisseo_leapfrog_kdk_f32/_f64)."""
@@ -284,6 +308,7 @@ def leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: fl
               _pot(pot), workspace.data_ptr(), workspace.numel(), _stream(stream)), "leapfrog_kdk_" + sfx)
 
 
+@_on_device
 def kick_drift(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, dt: float,
                pot: Optional[Potential], mode: int, workspace: torch.Tensor, stream=None):
     """The O(N) integrator kernel alone (odisseo_kick_drift_f32/_f64): mode 1 = closing half kick,
@@ -332,6 +357,7 @@ def _f64vec(t: torch.Tensor, name: str, numel: int):
         raise ValueError("%s must be a contiguous float64 CUDA tensor of %d values" % (name, numel))
 
 
+@_on_device
 def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: Optional[Potential], gx: torch.Tensor,
               gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor, with_eps_G: bool = False, stream=None):
     """Cotangent cot [n,4] pulled back through a = a_pair + a_ext (odisseo_accel_vjp_f32/_f64)."""
@@ -347,6 +373,7 @@ def accel_vjp(posm: torch.Tensor, cot: torch.Tensor, G: float, eps: float, pot: 
               workspace.data_ptr(), workspace.numel(), _stream(stream)), "accel_vjp_" + sfx)
 
 
+@_on_device
 def leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, G: float, eps: float, dt: float,
                       nsteps: int, pot: Optional[Potential], tape: torch.Tensor, workspace: torch.Tensor, stream=None):
     """leapfrog_kdk that also records the nsteps + 1 snapshots {posm, vel, pair-only acc} into tape
@@ -363,6 +390,7 @@ def leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, 
            "leapfrog_kdk_tape_" + sfx)
 
 
+@_on_device
 def leapfrog_kdk_vjp(tape: torch.Tensor, n: int, G: float, eps: float, dt: float, nsteps: int, pot: Optional[Potential],
                      lx: torch.Tensor, lv: torch.Tensor, gm: torch.Tensor, gparams: torch.Tensor,
                      workspace: torch.Tensor, with_eps_G: bool = False, stream=None):
@@ -389,6 +417,7 @@ def diagnostics_workspace_bytes(n: int) -> int:
     return int(lib().odisseo_diagnostics_workspace_bytes(int(n)))
 
 
+@_on_device
 def diagnostics(posm: torch.Tensor, vel: torch.Tensor, G: float, eps: float, pot: Optional[Potential],
                 out: torch.Tensor, workspace: torch.Tensor, phi: Optional[torch.Tensor] = None, stream=None):
     """Energies, momenta and centre of mass of a state in fp64 (odisseo_diagnostics_f32/_f64).
@@ -432,6 +461,7 @@ def ensemble_tape_bytes(n: int, nsim: int, nsteps: int) -> int:
     return int(lib().odisseo_ensemble_tape_bytes(int(n), int(nsim), int(nsteps)))
 
 
+@_on_device
 def ensemble_leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, params, nsteps: int, tape: torch.Tensor,
                                workspace: torch.Tensor, stream=None):
     """ensemble_leapfrog_kdk that also records {posm, vel, total acc} per simulation and step into tape (float32)."""
@@ -446,6 +476,7 @@ def ensemble_leapfrog_kdk_tape(posm: torch.Tensor, vel: torch.Tensor, params, ns
            "ensemble_leapfrog_kdk_tape_f32")
 
 
+@_on_device
 def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch.Tensor, lv: torch.Tensor,
                               gm: torch.Tensor, gparams: torch.Tensor, workspace: torch.Tensor,
                               with_eps_G: bool = False, accumulate: bool = False, stream=None):
@@ -464,6 +495,7 @@ def ensemble_leapfrog_kdk_vjp(tape: torch.Tensor, params, nsteps: int, lx: torch
            "ensemble_leapfrog_kdk_vjp_f32")
 
 
+@_on_device
 def ensemble_leapfrog_kdk(posm: torch.Tensor, vel: torch.Tensor, params, nsteps: int, workspace: torch.Tensor,
                           stream=None):
     """nsim independent small-N simulations in one launch (odisseo_ensemble_leapfrog_kdk_f32).
@@ -507,6 +539,7 @@ def mmd_workspace_bytes(n: int, m: int, nsim: int = 1) -> int:
     return int(lib().odisseo_mmd_workspace_bytes(int(n), int(m), int(nsim)))
 
 
+@_on_device
 def mmd2(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch.Tensor, sigma: Sequence[float], out: torch.Tensor,
          workspace: torch.Tensor, gpos: Optional[torch.Tensor] = None, gvel: Optional[torch.Tensor] = None,
          grad_scale: Optional[torch.Tensor] = None, stream=None):
@@ -543,6 +576,11 @@ def mmd2(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch
                                   workspace.data_ptr(), workspace.numel(), _stream(stream)), "mmd2_f32")
 
 
+def shutdown():
+    """Release the cached graph executables and profile events (odisseo_shutdown)."""
+    _check(lib().odisseo_shutdown(), "shutdown")
+
+
 def profile_times():
     """Durations (ms) of the pair-kernel launches the last profile timed, in launch order."""
     cnt = ctypes.c_int64(0)
@@ -559,6 +597,7 @@ def staged_sources_layout(n: int, is_f64: bool = False):
     return int(out[0]), int(out[1]), int(out[2])
 
 
+@_on_device
 def stage_sources(posm: torch.Tensor, workspace: torch.Tensor, stream=None):
     """Stage all n sources (records, padding, equal-mass flags) into the workspace (odisseo_stage_sources_*)."""
     n = _rec(posm, "posm")
@@ -567,6 +606,7 @@ def stage_sources(posm: torch.Tensor, workspace: torch.Tensor, stream=None):
            "stage_sources_" + sfx)
 
 
+@_on_device
 def pair_accel_staged(targets: torch.Tensor, n: int, acc: torch.Tensor, G: float, eps: float, workspace: torch.Tensor, stream=None):
     """acc[nt,4] = pair acceleration at targets[nt,4] due to the n sources already staged in the workspace."""
     nt = _rec(targets, "targets")
@@ -576,6 +616,7 @@ def pair_accel_staged(targets: torch.Tensor, n: int, acc: torch.Tensor, G: float
                                                              workspace.numel(), _stream(stream)), "pair_accel_staged_" + sfx)
 
 
+@_on_device
 def kick_drift_slice(posm_slice: torch.Tensor, vel: torch.Tensor, acc: torch.Tensor, n: int, lo: int, G: float, dt: float,
                      pot: Optional[Potential], mode: int, workspace: torch.Tensor, stream=None):
     """odisseo_kick_drift_slice_*: kick/drift the slice [lo, lo + count) of n particles and re-stage its records."""

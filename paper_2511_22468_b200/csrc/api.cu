@@ -112,7 +112,7 @@ thread_local int g_last_cuda_error = 0;
 // ---- instrumentation (include/odisseo.h "Instrumentation") --------------------------------
 std::atomic<int64_t> g_launches{0};
 struct Profile {
-    bool active = false;
+    std::atomic<bool> active{false};     // read without the lock on the launch path
     std::vector<cudaEvent_t> ev;     // pairs (start, stop) around pair-kernel launches
     size_t used = 0;                 // events used so far
     int64_t dropped = 0;             // launches seen after the pool ran out
@@ -127,7 +127,7 @@ odisseo_status cuda_fail(cudaError_t e)
     return ODISSEO_ERR_CUDA;
 }
 
-struct DeviceInfo { int device; int sms; int major; bool configured; };
+struct DeviceInfo { int device; int sms; int major; int minor; bool configured; };
 std::mutex g_mutex;
 std::vector<DeviceInfo> g_devices;
 
@@ -138,13 +138,16 @@ odisseo_status device_info(DeviceInfo& out)
     if (e != cudaSuccess) return cuda_fail(e);
     std::lock_guard<std::mutex> lock(g_mutex);
     for (const DeviceInfo& d : g_devices)
-        if (d.device == dev) { out = d; return d.major == 10 ? ODISSEO_OK : ODISSEO_ERR_ARCH; }
-    DeviceInfo d{dev, 0, 0, false};
+        if (d.device == dev) { out = d; return (d.major == 10 && d.minor == 0) ? ODISSEO_OK : ODISSEO_ERR_ARCH; }
+    DeviceInfo d{dev, 0, 0, 0, false};
     e = cudaDeviceGetAttribute(&d.major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaDeviceGetAttribute(&d.minor, cudaDevAttrComputeCapabilityMinor, dev);
     if (e != cudaSuccess) return cuda_fail(e);
     e = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return cuda_fail(e);
-    if (d.major != 10) { g_devices.push_back(d); out = d; return ODISSEO_ERR_ARCH; }
+    // the library holds sm_100a code only (architecture-specific, no PTX fallback): any other part, 10.x included, is ERR_ARCH
+    if (d.major != 10 || d.minor != 0) { g_devices.push_back(d); out = d; return ODISSEO_ERR_ARCH; }
     e = configure_pair_f32();
     if (e != cudaSuccess) return cuda_fail(e);
     e = configure_pair_f64();
@@ -164,11 +167,15 @@ inline bool overlap(const void* a, size_t na, const void* b, size_t nb)
     return x < y + nb && y < x + na;
 }
 
-template <typename T> odisseo_status check_pair_scalars(T G, T eps)
+// eps > 0 (reading R2) and inside the range where the unbranched self term stays finite in the precision of
+// the call: the forward kernels form eps^-3 (fp32: eps >= 1e-12; fp64 seeds its rsqrt in fp32 range: eps^2 >= 1e-30), the
+// pull-back kernels form 3 eps^-5 (fp32: eps >= 1e-7), so that inf * 0 = NaN cannot arise from an accepted eps.
+template <typename T> odisseo_status check_pair_scalars(T G, T eps, bool pullback = false)
 {
     if (!isfinite((double)G) || !isfinite((double)eps) || !(eps > (T)0)) return ODISSEO_ERR_ARG;
-    const double e2 = (double)eps * (double)eps;
-    if (e2 < 1e-30 || e2 > 1e30) return ODISSEO_ERR_ARG;   // keeps eps^2 and r2 inside the fp32 normal range
+    const double e = (double)eps;
+    if (e * e < 1e-30 || e * e > 1e30) return ODISSEO_ERR_ARG;
+    if (sizeof(T) == 4 && e < (pullback ? 1e-7 : 1e-12)) return ODISSEO_ERR_ARG;
     return ODISSEO_OK;
 }
 
@@ -454,6 +461,7 @@ struct GraphKey {
 };
 struct GraphEntry { GraphKey key; cudaGraphExec_t exec; uint64_t stamp; };
 std::vector<GraphEntry> g_graphs;
+std::mutex g_graph_mutex;
 uint64_t g_stamp = 0;
 constexpr size_t GRAPH_CACHE = 8;
 
@@ -516,12 +524,12 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
         key.G = (double)G; key.eps = (double)eps; key.dt = (double)dt; key.has_pot = pot != nullptr;
         if (pot) key.pot = *pot;
         key.block = block; key.device = dev.device;
+        // The cache is shared by every host thread: an executable is looked up, created, evicted AND launched under
+        // g_graph_mutex, so no thread can destroy an executable another one is about to launch.
+        std::lock_guard<std::mutex> graph_lock(g_graph_mutex);
         cudaGraphExec_t exec = nullptr;
-        {
-            std::lock_guard<std::mutex> lock(g_mutex);
-            for (GraphEntry& ge : g_graphs)
-                if (ge.key == key) { exec = ge.exec; ge.stamp = ++g_stamp; break; }
-        }
+        for (GraphEntry& ge : g_graphs)
+            if (ge.key == key) { exec = ge.exec; ge.stamp = ++g_stamp; break; }
         if (!exec) {
             cudaGraph_t graph = nullptr;
             ODISSEO_TRY(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
@@ -540,7 +548,6 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
             e = cudaGraphInstantiate(&exec, graph, 0);
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) return cuda_fail(e);
-            std::lock_guard<std::mutex> lock(g_mutex);
             if (g_graphs.size() >= GRAPH_CACHE) {
                 size_t victim = 0;
                 for (size_t k = 1; k < g_graphs.size(); ++k)
@@ -686,7 +693,7 @@ odisseo_status accel_vjp_impl(const T* posm, const T* cot, int64_t n, T G, T eps
         misaligned(ws, 256))
         return ODISSEO_ERR_ALIGN;
     if (overlap(posm, n * rec, gx, n * rec) || overlap(cot, n * rec, gx, n * rec)) return ODISSEO_ERR_ARG;
-    odisseo_status st = check_pair_scalars<T>(G, eps);
+    odisseo_status st = check_pair_scalars<T>(G, eps, true);
     if (st != ODISSEO_OK) return st;
     PotParams<double> pp;
     st = make_pot<double>((double)G, pot, pp);
@@ -732,7 +739,7 @@ odisseo_status leapfrog_vjp_impl(const T* tape, int64_t n, T G, T eps, T dt, int
         misaligned(ws, 256))
         return ODISSEO_ERR_ALIGN;
     if (overlap(lx, n * rec, lv, n * rec)) return ODISSEO_ERR_ARG;
-    odisseo_status st = check_pair_scalars<T>(G, eps);
+    odisseo_status st = check_pair_scalars<T>(G, eps, true);
     if (st != ODISSEO_OK) return st;
     if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
     PotParams<double> pd;
@@ -811,6 +818,22 @@ const char* odisseo_status_string(odisseo_status s)
 int odisseo_last_cuda_error(void) { return g_last_cuda_error; }
 
 int64_t odisseo_launch_count(void) { return g_launches.load(); }
+
+odisseo_status odisseo_shutdown(void)
+{
+    {
+        std::lock_guard<std::mutex> graph_lock(g_graph_mutex);
+        for (GraphEntry& ge : g_graphs) cudaGraphExecDestroy(ge.exec);
+        g_graphs.clear();
+    }
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (g_prof.active.load()) return ODISSEO_ERR_ARG;     // a profile is open: close it first
+    for (cudaEvent_t ev : g_prof.ev) cudaEventDestroy(ev);
+    g_prof.ev.clear();
+    g_prof.used = 0;
+    (void)cudaGetLastError();
+    return ODISSEO_OK;
+}
 
 odisseo_status odisseo_profile_begin(void)
 {
@@ -1078,7 +1101,8 @@ namespace {
 
 // Validates the host records and uploads them: float records at ws, double records behind them.
 odisseo_status ensemble_upload_params(const odisseo_sim_params* h_params, int64_t nparams, void* ws, size_t ws_bytes,
-                                      cudaStream_t s, const EnsembleParams** d32, const EnsembleParams64** d64)
+                                      cudaStream_t s, const EnsembleParams** d32, const EnsembleParams64** d64,
+                                      bool pullback = false)
 {
     const size_t off64 = (((size_t)nparams * sizeof(EnsembleParams)) + 255) & ~(size_t)255;
     if (ws_bytes < off64 + (size_t)nparams * sizeof(EnsembleParams64)) return ODISSEO_ERR_WORKSPACE;
@@ -1087,7 +1111,7 @@ odisseo_status ensemble_upload_params(const odisseo_sim_params* h_params, int64_
     for (int64_t k = 0; k < nparams; ++k) {
         const odisseo_sim_params& hp = h_params[k];
         const float G = (float)hp.G, eps = (float)hp.eps, dt = (float)hp.dt;
-        odisseo_status st = check_pair_scalars<float>(G, eps);
+        odisseo_status st = check_pair_scalars<float>(G, eps, pullback);
         if (st != ODISSEO_OK) return st;
         if (!isfinite((double)dt)) return ODISSEO_ERR_ARG;
         EnsembleParams& d = p32[(size_t)k];
@@ -1171,7 +1195,7 @@ odisseo_status odisseo_ensemble_leapfrog_kdk_vjp_f32(const float* d_tape, int64_
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const EnsembleParams* d32;
     const EnsembleParams64* d64;
-    st = ensemble_upload_params(h_params, nparams, d_workspace, workspace_bytes, s, &d32, &d64);
+    st = ensemble_upload_params(h_params, nparams, d_workspace, workspace_bytes, s, &d32, &d64, true);
     if (st != ODISSEO_OK) return st;
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = launch_ensemble_vjp_f32(d_tape, d64, nparams == 1 ? 1 : 0, (int)n, nsim, nsteps, with_eps_G != 0, d_lx, d_lv, d_gm,

@@ -132,6 +132,12 @@ def test_argument_validation_happens_before_any_device_work(lib):
     assert f(addr16 + 4, addr16 + 128, 4, 1.0, 0.1, ws, 1 << 20, None) == 2     # misaligned
     assert f(addr16, addr16 + 16, 4, 1.0, 0.1, ws, 1 << 20, None) == 3          # overlap
     assert f(addr16, addr16 + 128, 4, 1.0, 0.0, ws, 1 << 20, None) == 3         # eps <= 0
+    assert f(addr16, addr16 + 128, 4, 1.0, 1e-13, ws, 1 << 20, None) == 3       # fp32: eps^-3 would overflow
+    v = lib.odisseo_accel_vjp_f32
+    dbl = (ctypes.c_double * 64)()
+    a8 = ctypes.addressof(dbl)
+    # fp32 pull-back forms 3 eps^-5: eps = 1e-8 is refused before any device work, eps = 1e-6 passes validation
+    assert v(addr16, addr16 + 64, 4, 1.0, 1e-8, None, 0, addr16 + 128, a8, a8 + 256, ws, 1 << 20, None) == 3
     assert f(addr16, addr16 + 128, 4, float("nan"), 0.1, ws, 1 << 20, None) == 3
     g = lib.odisseo_leapfrog_kdk_f32
     assert g(addr16, addr16 + 64, addr16 + 128, 0, 4, 1.0, 0.1, 0.1, -1, None, ws, 1 << 20, None) == 3
