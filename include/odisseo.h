@@ -79,6 +79,13 @@ const char *odisseo_status_string(odisseo_status s);
 /* cudaError_t value of the most recent ODISSEO_ERR_CUDA on this thread (0 if none). */
 int odisseo_last_cuda_error(void);
 
+/* odisseo_leapfrog_kdk_* can run a whole call as ONE cooperative launch: a persistent kernel with the time loop inside
+ * and a grid barrier between the pair and the integrate phase, bit-identical to the per-step launch sequence.  By
+ * default only fp64 calls on n <= 4,096 take it (measured: the two barriers per step cost what the launch edges cost;
+ * see csrc/api.cu).  This sets the largest n served that way for both precisions (clamped to [0, 16384]; 0 = always
+ * launch per step) and returns the previous fp64 value: a tuning and test knob, process-wide. */
+int64_t odisseo_set_fused_max_n(int64_t n);
+
 /* Releases what the library keeps between calls: the cached CUDA-graph executables of odisseo_leapfrog_kdk_* and the
  * CUDA events of odisseo_profile_*.  Call with no library work in flight on other host threads; every entry point may
  * be used again afterwards (the caches refill).  ERR_ARG while a profile is open.  The library's other globals are a

@@ -107,6 +107,15 @@ PairPlan make_vjp_plan(int64_t n, int is_f64, int num_sms)
 
 namespace {
 
+// Largest n the whole-loop kernel (fused_step.cuh) serves, per precision {fp32, fp64}; odisseo_set_fused_max_n sets
+// both (0 = never).  Measured on B200, us per KDK step, whole-loop kernel / per-step launches (graph + programmatic
+// dependent launch):   fp32  N = 1,024 10.2 / 8.3   2,048 12.5 / 12.6   4,096 23.8 / 20.2   16,384 112.7 / 108.9
+//                      fp64  N = 1,024 12.6 / 12.0  2,048 16.3 / 19.8   4,096 31.5 / 36.1   16,384 285 / 261
+// Two grid barriers per step (arrive atomic + release flag, ~2.5 us each with the fences around them) cost as much as
+// the two launch edges they replace, so the whole-loop form only pays where the per-step kernels are slowest to start:
+// fp64 up to 4,096.  fp32 keeps the per-step launches by default.
+std::atomic<int64_t> g_fused_max_n[2] = {{0}, {4096}};
+
 thread_local int g_last_cuda_error = 0;
 
 // ---- instrumentation (include/odisseo.h "Instrumentation") --------------------------------
@@ -148,9 +157,9 @@ odisseo_status device_info(DeviceInfo& out)
     if (e != cudaSuccess) return cuda_fail(e);
     // the library holds sm_100a code only (architecture-specific, no PTX fallback): any other part, 10.x included, is ERR_ARCH
     if (d.major != 10 || d.minor != 0) { g_devices.push_back(d); out = d; return ODISSEO_ERR_ARCH; }
-    e = configure_pair_f32();
+    e = configure_pair_f32(d.sms);
     if (e != cudaSuccess) return cuda_fail(e);
-    e = configure_pair_f64();
+    e = configure_pair_f64(d.sms);
     if (e != cudaSuccess) return cuda_fail(e);
     e = configure_vjp();
     if (e != cudaSuccess) return cuda_fail(e);
@@ -244,6 +253,15 @@ inline cudaError_t launch_step(const PairPlan& p, double* x, double* v, double* 
                                const PotParams<double>& pot, double dt, int flags, cudaStream_t s, double* snap = nullptr,
                                int64_t lo = 0, int64_t count = -1)
 { g_launches.fetch_add(1, std::memory_order_relaxed); return launch_step_f64(p, x, v, a, j, part, G, pot, dt, flags, snap, lo, count < 0 ? p.n : count, s); }
+
+inline cudaError_t launch_fused(const PairPlan& p, float* x, float* v, float* a, void* j, double* part, float G, float eps, float dt,
+                                const PotParams<float>& pot, int64_t nsteps, int acc_valid, unsigned* bar, cudaStream_t s)
+{ return launch_fused_f32(p, x, v, a, j, part, G, eps, dt, pot, nsteps, acc_valid, bar, s); }
+inline cudaError_t launch_fused(const PairPlan& p, double* x, double* v, double* a, void* j, double* part, double G, double eps, double dt,
+                                const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* bar, cudaStream_t s)
+{ return launch_fused_f64(p, x, v, a, j, part, G, eps, dt, pot, nsteps, acc_valid, bar, s); }
+inline int fused_max_ctas(float, int variant) { return fused_max_ctas_f32(variant); }
+inline int fused_max_ctas(double, int variant) { return fused_max_ctas_f64(variant); }
 
 inline cudaError_t launch_ext(const float* x, float* a, int64_t n, const PotParams<float>& pot, int accumulate, cudaStream_t s)
 { g_launches.fetch_add(1, std::memory_order_relaxed); return launch_ext_f32(x, a, n, pot, accumulate, s); }
@@ -495,6 +513,23 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     cudaError_t e;
 
 #define ODISSEO_TRY(call) do { e = (call); if (e != cudaSuccess) return cuda_fail(e); } while (0)
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
+    // Small and mid N: the whole call in ONE cooperative launch (fused_step.cuh) -- same plan, same code per phase, hence
+    // bit-identical to the two-kernel sequence below.  Not inside a caller's capture, with a tape, or while a profile
+    // is open (its event pairs bracket pair-kernel launches).
+    if (n <= g_fused_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && nsteps >= 1 && !tape && cap == cudaStreamCaptureStatusNone && !g_prof.active) {
+        PairPlan fplan = plan;
+        const int cap_ctas = fused_max_ctas(T(), plan.variant);
+        if (cap_ctas >= 1) {
+            if (fplan.P > cap_ctas) fplan.P = cap_ctas;          // P only deals the units out: the sums do not depend on it
+            unsigned* bar = plan_barrier_block(cv.jsrc, plan);
+            ODISSEO_TRY(cudaMemsetAsync(bar, 0, 256, s));
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            ODISSEO_TRY(launch_fused(fplan, posm, vel, acc, cv.jsrc, cv.partials, G, eps, dt, pp, nsteps, acc_valid, bar, s));
+            return ODISSEO_OK;
+        }
+    }
     // tape != nullptr (odisseo_leapfrog_kdk_tape_*): every step kernel also stores the synchronised snapshot
     // {x_k, v_k, pair-only a_k} it holds in registers at the moment between two steps -- no copies, no extra launch
     const size_t snap = (size_t)n * 12;
@@ -511,8 +546,6 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN, s, tape));
 
     int64_t mid = nsteps - 1;     // full steps: pair + (close, open)
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
     // no graph on the legacy stream, inside a caller's capture, or while a profile is open
     // (event pairs around the pair kernels cannot be read back from graph nodes)
     const bool use_graph = (s != nullptr) && cap == cudaStreamCaptureStatusNone && mid >= 2 && !g_prof.active && !tape;
@@ -818,6 +851,14 @@ const char* odisseo_status_string(odisseo_status s)
 int odisseo_last_cuda_error(void) { return g_last_cuda_error; }
 
 int64_t odisseo_launch_count(void) { return g_launches.load(); }
+
+int64_t odisseo_set_fused_max_n(int64_t n)
+{
+    if (n < 0) n = 0;
+    if (n > 16384) n = 16384;
+    g_fused_max_n[0].store(n);
+    return g_fused_max_n[1].exchange(n);
+}
 
 odisseo_status odisseo_shutdown(void)
 {

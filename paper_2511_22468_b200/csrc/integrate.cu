@@ -11,33 +11,11 @@
 // The two half kicks are two separate FMAs, so a step split across two calls is bit-identical to
 // the fused one (PAPER.md:L47 Velocity-Verlet; chaining contract in include/odisseo.h).
 // Memory-bound: one 16 B (32 B) record load per array, coalesced 128-bit accesses.
-#include "odisseo_common.cuh"
-#include "ext_potential.cuh"
+#include "step_body.cuh"
 
 namespace odisseo {
 
 namespace {
-
-template <typename T> struct Vec4;
-template <> struct Vec4<float> { typedef float4 type; };
-template <> struct Vec4<double> { typedef double4 type; };
-
-// Staged source record writers.  fp32: {x,x,y,y},{z,z,m,m} (pre-duplicated packed operands);
-// fp64: plain {x,y,z,m}.  Records [n, n_pad) are massless padding parked far away
-// (odisseo_common.cuh PAD_POS_*).
-__device__ __forceinline__ void stage_record(void* jsrc, int64_t i, float x, float y, float z, float m)
-{
-    float4* out = reinterpret_cast<float4*>(jsrc) + 2 * i;
-    out[0] = make_float4(x, x, y, y);
-    out[1] = make_float4(z, z, m, m);
-}
-__device__ __forceinline__ void stage_record(void* jsrc, int64_t i, double x, double y, double z, double m)
-{
-    reinterpret_cast<double4*>(jsrc)[i] = make_double4(x, y, z, m);
-}
-
-__device__ __forceinline__ float pad_pos(float) { return PAD_POS_F32; }
-__device__ __forceinline__ double pad_pos(double) { return PAD_POS_F64; }
 
 // REDUCE = the launch starts from the pair kernel's partial rows (flags & STEP_FROM_PARTIALS); a
 // compile-time switch so that the plain kick/drift instantiation does not carry the reduce batch in
@@ -57,67 +35,12 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
     const bool flagging = staging && !(flags & STEP_SLICE);             // masses never change: a slice keeps the flags
-    int mass_differs = 0;
     int* const block_flag = const_cast<int*>(plan_flags(jsrc, plan)) + blockIdx.x;
     if (flagging) {                                  // uniform branch: flags is a kernel argument
         if (threadIdx.x == 0) *block_flag = 0;
         __syncthreads();                             // before any load is in flight: costs nothing
     }
-    if (i < count) {
-        const T mass0 = reinterpret_cast<const T*>(posm)[3];            // masses are never modified
-        V4 p = posm[i];
-        if (flags & STEP_PACK_ONLY) {
-            stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
-        } else {
-            T apx, apy, apz;
-            if (REDUCE) {
-                // fixed order: the S rows of this i-block in increasing s, then the factors left out of the rows
-                double sum[3];
-                reduce_unit_rows<3>(partials, plan, i, sum);
-                const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
-                const double sx = sum[0], sy = sum[1], sz = sum[2];
-                apx = (T)(gm * sx);
-                apy = (T)(gm * sy);
-                apz = (T)(gm * sz);
-                V4 a; a.x = apx; a.y = apy; a.z = apz; a.w = (T)0;
-                acc[i] = a;
-            } else {
-                const V4 a = acc[i];
-                apx = a.x; apy = a.y; apz = a.z;
-            }
-            if (flags & (STEP_CLOSE | STEP_OPEN | STEP_SNAPSHOT)) {
-                T ex, ey, ez;
-                ext_accel<T>(pot, p.x, p.y, p.z, ex, ey, ez);
-                const T tx = apx + ex, ty = apy + ey, tz = apz + ez;
-                const T h = (T)0.5 * dt;
-                V4 v = vel[i];
-                if (flags & STEP_CLOSE) {
-                    v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
-                }
-                if (snapshot) {
-                    // tape of the reverse-mode derivative (odisseo_leapfrog_kdk_tape_*): the synchronised state
-                    // {x_k, v_k, pair-only a_k} between the closing kick of step k - 1 and the opening kick of step k
-                    V4 vs = v; vs.w = (T)0;
-                    V4 as; as.x = apx; as.y = apy; as.z = apz; as.w = (T)0;
-                    snapshot[i] = p;
-                    snapshot[plan.n + i] = vs;
-                    snapshot[2 * plan.n + i] = as;
-                }
-                if (flags & STEP_OPEN) {
-                    v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
-                    p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
-                    posm[i] = p;
-                    stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
-                }
-                v.w = (T)0;
-                vel[i] = v;
-            }
-        }
-        if (flagging) mass_differs = !(p.w == mass0);               // NaN counts as different
-    } else if (staging && lo + count == plan.n && lo + i < plan_npad(plan)) {
-        const T far = pad_pos((T)0);                                    // whoever holds the last particle pads the tail
-        stage_record(jsrc, lo + i, far, far, far, (T)0);
-    }
+    const int mass_differs = step_particle<T, REDUCE>(posm, vel, acc, jsrc, partials, plan, G, pot, dt, flags, snapshot, lo, count, i);
     if (flagging) {
         // same-value plain stores after the block's own zeroing: no atomics, no closing barrier
         const unsigned any = __ballot_sync(0xffffffffu, mass_differs);
@@ -134,9 +57,9 @@ reduce_rows_kernel(const double* __restrict__ partials, const void* __restrict__
     pdl_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= plan.nt) return;
+    const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
     double sum[3];
     reduce_unit_rows<3>(partials, plan, i, sum);
-    const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
     typename Vec4<T>::type a;
     a.x = (T)(gm * sum[0]); a.y = (T)(gm * sum[1]); a.z = (T)(gm * sum[2]); a.w = (T)0;
     acc[i] = a;

@@ -70,7 +70,8 @@ __host__ __device__ __forceinline__ int32_t plan_nflags(const PairPlan& p) {
 // (sharded form).  The kernels never read a record past 8 * n8.
 constexpr int64_t STAGED_SLACK = 1024;
 __host__ __device__ __forceinline__ size_t plan_flag_bytes(const PairPlan& p) {
-    return (((size_t)plan_nflags(p) + 1) * sizeof(int) + 255) & ~(size_t)255;
+    // [256 B grid-barrier block: arrival counter | release flag, 128 B apart][flags, decision word], rounded to 256 B
+    return 256 + ((((size_t)plan_nflags(p) + 1) * sizeof(int) + 255) & ~(size_t)255);
 }
 __host__ __device__ __forceinline__ size_t plan_jsrc_bytes(const PairPlan& p) {
     const size_t b = plan_flag_bytes(p) + (size_t)(plan_npad(p) + STAGED_SLACK) * p.rec_bytes;
@@ -80,10 +81,15 @@ __host__ __device__ __forceinline__ void* plan_records(void* ws, const PairPlan&
     return static_cast<unsigned char*>(ws) + plan_flag_bytes(p);
 }
 __host__ __device__ __forceinline__ const int* plan_flags(const void* jsrc, const PairPlan& p) {
-    return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) - plan_flag_bytes(p));
+    return reinterpret_cast<const int*>(static_cast<const unsigned char*>(jsrc) - plan_flag_bytes(p) + 256);
 }
 __host__ __device__ __forceinline__ const int* plan_eqm_word(const void* jsrc, const PairPlan& p) {
     return plan_flags(jsrc, p) + plan_nflags(p);
+}
+// 256-byte block of the whole-loop kernel's grid barrier (fused_step.cuh), zeroed by the host before each launch:
+// word 0 = arrival counter, word 32 (another 128-byte line) = release flag.
+__host__ __device__ __forceinline__ unsigned* plan_barrier_block(void* jsrc, const PairPlan& p) {
+    return reinterpret_cast<unsigned*>(static_cast<unsigned char*>(jsrc) - plan_flag_bytes(p));
 }
 // Padding records of the staged source array: zero mass, parked so far away that the softened
 // inverse cube underflows to exactly 0 (ftz) -- they contribute 0 with or without the mass factor.
@@ -127,9 +133,11 @@ __device__ __forceinline__ void reduce_unit_rows(const double* __restrict__ part
 template <typename T>
 __device__ __forceinline__ double plan_row_mass(const void* __restrict__ jsrc, const PairPlan& plan)
 {
-    if (__ldcg(plan_eqm_word(jsrc, plan)) == 0) return 1.0;
+    // both loads are issued unconditionally (no dependent round trip: at small N the reduce is latency-bound)
+    const int eqm = __ldcg(plan_eqm_word(jsrc, plan));
     // mass of staged record 0: fp32 records are {x,x,y,y},{z,z,m,m}; fp64 records {x,y,z,m}
-    return sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 6) : __ldcg(static_cast<const double*>(jsrc) + 3);
+    const double m0 = sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 6) : __ldcg(static_cast<const double*>(jsrc) + 3);
+    return eqm != 0 ? m0 : 1.0;
 }
 #endif
 
@@ -356,7 +364,15 @@ size_t mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim);
 cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel, int64_t m,
                            int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale, double* mmd2,
                            float* gpos, float* gvel, void* ws, cudaStream_t stream);
-cudaError_t configure_pair_f32();
-cudaError_t configure_pair_f64();
+cudaError_t configure_pair_f32(int num_sms);
+cudaError_t configure_pair_f64(int num_sms);
+// whole-loop kernels (fused_step.cuh)
+int fused_max_ctas_f32(int variant);
+int fused_max_ctas_f64(int variant);
+cudaError_t launch_fused_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc, double* partials, float G, float eps,
+                             float dt, const PotParams<float>& pot, int64_t nsteps, int acc_valid, unsigned* barrier, cudaStream_t stream);
+cudaError_t launch_fused_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc, double* partials, double G,
+                             double eps, double dt, const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* barrier,
+                             cudaStream_t stream);
 
 }  // namespace odisseo

@@ -20,7 +20,7 @@
 //     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2, and the
 //     reduce step multiplies by the mass once;
 //   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
-#include "pair_stream.cuh"
+#include "fused_step.cuh"
 
 namespace odisseo {
 
@@ -129,14 +129,36 @@ struct PairF32 {
 
 typedef PairF32<4, 8, 1, 8> LargeF32;    // 2,048 targets per CTA, one CTA per SM
 typedef PairF32<1, 2, 8, 4> SmallF32;    // 128 targets per CTA, up to 8 CTAs per SM (n <= 4,096)
+typedef PairF32<1, 2, 4, 4> SmallF32Fused;   // the same loop inside the whole-loop kernel, which also holds the reduce batch
+
+int g_fused_max_ctas[2] = {0, 0};        // co-resident CTAs of the whole-loop kernel, [variant]
 
 }  // namespace
 
-cudaError_t configure_pair_f32()
+cudaError_t configure_pair_f32(int num_sms)
 {
     cudaError_t e = configure_stream<LargeF32>(512);
-    if (e != cudaSuccess) return e;
-    return configure_stream<SmallF32>(256);
+    if (e == cudaSuccess) e = configure_stream<SmallF32>(256);
+    if (e == cudaSuccess) e = configure_fused<LargeF32, float>(512, num_sms, &g_fused_max_ctas[0]);
+    if (e == cudaSuccess) e = configure_fused<SmallF32Fused, float>(256, num_sms, &g_fused_max_ctas[1]);
+    return e;
+}
+
+// Whole-loop kernel (fused_step.cuh): all nsteps KDK steps of odisseo_leapfrog_kdk_f32 in one cooperative launch.
+int fused_max_ctas_f32(int variant) { return g_fused_max_ctas[variant ? 1 : 0]; }
+
+cudaError_t launch_fused_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc, double* partials, float G, float eps,
+                             float dt, const PotParams<float>& pot, int64_t nsteps, int acc_valid, unsigned* barrier, cudaStream_t stream)
+{
+    FusedArgs<float> fa;
+    fa.posm = reinterpret_cast<float4*>(posm); fa.vel = reinterpret_cast<float4*>(vel); fa.acc = reinterpret_cast<float4*>(acc);
+    fa.G = G; fa.dt = dt; fa.pot = pot; fa.nsteps = nsteps; fa.acc_valid = acc_valid; fa.barrier = barrier;
+    if (plan.variant == 0) {
+        const LargeF32::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
+        return launch_fused<LargeF32, float>(plan, prm, jsrc, partials, fa, stream);
+    }
+    const SmallF32Fused::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
+    return launch_fused<SmallF32Fused, float>(plan, prm, jsrc, partials, fa, stream);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,

@@ -11,7 +11,7 @@
 // seed cost as much as the arithmetic they feed.
 // Summation: fp64 inside a tile, tile sums added in tile order inside a unit, one row per unit -- the
 // same fixed grouping as the fp32 kernel.
-#include "pair_stream.cuh"
+#include "fused_step.cuh"
 
 namespace odisseo {
 
@@ -119,16 +119,38 @@ typedef PairF64<4, 8, 1, 4, false> LargeF64;
 typedef PairF64<2, 2, 8, 2, false> SmallF64;
 typedef PairF64<4, 8, 1, 4, true> LargePot;
 typedef PairF64<2, 2, 8, 2, true> SmallPot;
+typedef PairF64<2, 2, 4, 2, false> SmallF64Fused;
+
+int g_fused_max_ctas64[2] = {0, 0};
 
 }  // namespace
 
-cudaError_t configure_pair_f64()
+cudaError_t configure_pair_f64(int num_sms)
 {
     cudaError_t e = configure_stream<LargeF64>(256);
     if (e == cudaSuccess) e = configure_stream<SmallF64>(256);
     if (e == cudaSuccess) e = configure_stream<LargePot>(256);
     if (e == cudaSuccess) e = configure_stream<SmallPot>(256);
+    if (e == cudaSuccess) e = configure_fused<LargeF64, double>(256, num_sms, &g_fused_max_ctas64[0]);
+    if (e == cudaSuccess) e = configure_fused<SmallF64Fused, double>(256, num_sms, &g_fused_max_ctas64[1]);
     return e;
+}
+
+int fused_max_ctas_f64(int variant) { return g_fused_max_ctas64[variant ? 1 : 0]; }
+
+cudaError_t launch_fused_f64(const PairPlan& plan, double* posm, double* vel, double* acc, void* jsrc, double* partials, double G,
+                             double eps, double dt, const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* barrier,
+                             cudaStream_t stream)
+{
+    FusedArgs<double> fa;
+    fa.posm = reinterpret_cast<double4*>(posm); fa.vel = reinterpret_cast<double4*>(vel); fa.acc = reinterpret_cast<double4*>(acc);
+    fa.G = G; fa.dt = dt; fa.pot = pot; fa.nsteps = nsteps; fa.acc_valid = acc_valid; fa.barrier = barrier;
+    if (plan.variant == 0) {
+        const LargeF64::Params prm{reinterpret_cast<const double4*>(posm), eps * eps};
+        return launch_fused<LargeF64, double>(plan, prm, jsrc, partials, fa, stream);
+    }
+    const SmallF64Fused::Params prm{reinterpret_cast<const double4*>(posm), eps * eps};
+    return launch_fused<SmallF64Fused, double>(plan, prm, jsrc, partials, fa, stream);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,

@@ -64,16 +64,15 @@ struct TileWalk {
 template <class C, bool EQM>
 __device__ __forceinline__ void consume_units(const typename C::Params& prm, double* __restrict__ rows, const PairPlan& plan,
                                               unsigned char* smem_raw, uint64_t* full_bar, uint64_t* empty_bar,
-                                              const int64_t u0, const int64_t u1)
+                                              const int64_t u0, const int64_t u1, int& s, uint32_t& ph)
 {
+    // s, ph: the ring position, kept by the caller so that a persistent kernel can walk its units again and again
     const uint32_t stage_bytes = (uint32_t)plan.T * C::REC;
     typename C::template State<EQM> st(prm, plan, smem_raw + (size_t)STAGES * stage_bytes);
     const int lane = threadIdx.x & 31;
     TileWalk w(plan, u0, u1);
     int32_t b_cur = -1;
     bool fresh = true;
-    int s = 0;
-    uint32_t ph = 0;
     while (w.valid()) {
         if (w.b != b_cur) { st.load_targets(w.b); b_cur = w.b; }
         if (fresh) { st.zero_outer(); fresh = false; }
@@ -160,10 +159,12 @@ stream_kernel(const typename C::Params prm, const unsigned char* __restrict__ js
         return;
     }
 
+    int cs = 0;
+    uint32_t cph = 0;
     if (eqm)
-        consume_units<C, true>(prm, rows, plan, smem_raw, full_bar, empty_bar, u0, u1);
+        consume_units<C, true>(prm, rows, plan, smem_raw, full_bar, empty_bar, u0, u1, cs, cph);
     else
-        consume_units<C, false>(prm, rows, plan, smem_raw, full_bar, empty_bar, u0, u1);
+        consume_units<C, false>(prm, rows, plan, smem_raw, full_bar, empty_bar, u0, u1, cs, cph);
 }
 
 template <class C> size_t stream_smem_bytes(const PairPlan& plan) { return (size_t)STAGES * plan.T * C::REC + C::outer_bytes(); }

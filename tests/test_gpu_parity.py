@@ -360,7 +360,7 @@ def test_launch_count_and_pair_kernel_profile():
     """Instrumentation used by bench.py: the launch counter counts graph-replayed kernels, and a
     profile brackets exactly the pair-kernel launches without changing results."""
     cfg = W.CONFIGS[1]
-    posm64, vel64 = W.make_state(cfg, n=2048)
+    posm64, vel64 = W.make_state(cfg, n=6000)                                     # above the whole-loop kernel's range
     p32, v32 = W.to_f32(posm64), W.to_f32(vel64)
     pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
     c0 = B.launch_count()
@@ -377,6 +377,40 @@ def test_launch_count_and_pair_kernel_profile():
         assert x.tobytes() == y.tobytes()
     with pytest.raises(B.OdisseoError):
         B.profile_end()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n,ci", [(1, 1), (2, 0), (129, 1), (1000, 0), (1024, 0), (3000, 1), (4096, 1), (5000, 1), (16384, 1)])
+def test_whole_loop_kernel_is_bit_identical_to_the_per_step_launches(n, ci, dtype):
+    """Small and mid N run all steps in ONE cooperative launch (csrc/fused_step.cuh: pair phase, grid barrier, integrate
+    phase, grid barrier); it executes the same code on the same plan as the {pair, step} launch sequence, so state
+    and acc must agree bit for bit -- with and without acc_valid, and chained."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg, n=n)
+    if n == 129:
+        posm64[7, 3] *= 1.5                                                      # general-mass loop
+    p, v = posm64.astype(dtype), vel64.astype(dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    old = B.set_fused_max_n(16384)
+    try:
+        fused = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, 7, pot, dtype)
+        c0 = B.launch_count()
+        gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, 7, pot, dtype)
+        assert B.launch_count() - c0 == 1                                         # one launch for the whole call
+        # chained: 3 steps, then 4 more with acc_valid
+        posm, vel = dev(p, dtype), dev(W.vel4(v, dtype), dtype)
+        acc = torch.empty_like(posm)
+        ws = B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64))
+        B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, 3, pot, ws)
+        B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, 4, pot, ws, acc_valid=True)
+        torch.cuda.synchronize()
+        chained = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
+        B.set_fused_max_n(0)
+        plain = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, 7, pot, dtype)
+    finally:
+        B.set_fused_max_n(old)
+    for a, b, c in zip(fused, plain, chained):
+        assert a.tobytes() == b.tobytes() and a.tobytes() == c.tobytes()
 
 
 def test_leapfrog_conserves_lz_and_tracks_single_particle_orbit_f32():
