@@ -58,17 +58,21 @@ def _stats(ms):
             "std": float(a.std(ddof=1)) if a.size > 1 else 0.0}
 
 
-def _pipe_peaks(B):
+def _pipe_peaks(B, all_kinds: bool = False, ctas_per_sm: int = 2, threads: int = 512):
     """Measured pipe rates (odisseo_ubench_*): FP32 / MUFU / FP64 operations per clock per SM and
     the rate the issue logic sustains for the pair body's own instruction mix."""
     kinds = {nm: k for k, nm in enumerate(B.ubench_kinds())}
     out = {}
-    for nm in ("ffma", "ffma2_3src", "mufu_rsq", "dfma", "mix_11p_2mufu", "mix_12p_2mufu"):
-        r = B.ubench_run(kinds[nm], 2, 512, 1 << 15)
+    names = list(kinds) if all_kinds else ["ffma", "ffma2_3src", "mufu_rsq", "dfma", "mix_11p_2mufu", "mix_12p_2mufu"]
+    for nm in names:
+        r = B.ubench_run(kinds[nm], ctas_per_sm, threads, 1 << 15)
         s = r["ms"] * 1e-3
         per = lambda x: x / s / SM_MAX_HZ / r["sms"]                      # noqa: E731
+        warps_per_smsp = ctas_per_sm * threads / 32 / 4
         out[nm] = {"ms": r["ms"], "fp32_lane_ops_per_clk_sm": per(r["fp32_lane_ops"]), "mufu_per_clk_sm": per(r["mufu"]),
-                   "fp64_ops_per_clk_sm": per(r["fp64_ops"])}
+                   "fp64_ops_per_clk_sm": per(r["fp64_ops"]), "lds_per_clk_sm": per(r["lds"]),
+                   # scheduler cycles one warp's loop iteration occupies (time x clock / iterations / warps per scheduler)
+                   "cycles_per_iteration_per_warp": s * SM_MAX_HZ / (1 << 15) / warps_per_smsp}
     return out
 
 
@@ -432,6 +436,39 @@ def _ensemble_adjoint_rate(B, W, torch, n: int = 1000, nsim: int = 296, nsteps: 
             "sim_grad_steps_per_s": nsim * nsteps / ((best[0] + best[1]) * 1e-3), "gpu_launches": 2}
 
 
+def _mmd_rate(B, W, torch, n: int = 1000, m: int = 1000, nsim: int = 2960):
+    """MMD^2 loss + gradient of a batch of simulated clouds against one observed cloud (PAPER.md:L43 step 4): the loss of
+    the paper's grid search (10^4 simulations of N = 1,000) in one launch pair; 3 n m kernel evaluations per simulation
+    (xx, xy with gradient, yy)."""
+    cfg = W.CONFIGS[1]
+    p64, v64 = W.make_state(cfg, n=n)
+    rng = np.random.Generator(np.random.PCG64(8))
+    xp = torch.from_numpy(np.repeat(W.to_f32(p64)[None], nsim, axis=0)).cuda()
+    xv = torch.from_numpy(np.repeat(W.vel4(W.to_f32(v64), np.float32)[None], nsim, axis=0)).cuda()
+    xp[:, :, :3] += torch.from_numpy(rng.normal(0, 0.005, (nsim, 1, 3)).astype(np.float32)).cuda()
+    y64, w64 = W.make_state(cfg, n=m, seed=77)
+    yp, yv = torch.from_numpy(W.to_f32(y64)).cuda(), torch.from_numpy(W.vel4(W.to_f32(w64), np.float32)).cuda()
+    out = torch.empty(nsim, dtype=torch.float64, device="cuda")
+    gp, gv = torch.empty_like(xp), torch.empty_like(xv)
+    ws = B.alloc_workspace(B.mmd_workspace_bytes(n, m, nsim))
+    sigma = [0.02, 0.02, 0.02, 0.004, 0.004, 0.004]
+    B.mmd2(xp, xv, yp, yv, sigma, out, ws, gp, gv)
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(5):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        B.mmd2(xp, xv, yp, yv, sigma, out, ws, gp, gv)
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    ms = min(ts)
+    pairs = nsim * (n * n + n * m + m * m)
+    return {"workload": "MMD^2 + gradient of %d clouds of %d points against one of %d" % (nsim, n, m), "ms": ms,
+            "ms_stats": _stats(ts), "G_kernel_evals_per_s": pairs / (ms * 1e-3) / 1e9, "losses_per_s": nsim / (ms * 1e-3),
+            "mmd2_first": float(out[0].item()), "gpu_launches": 2}
+
+
 def run_sharded(args, rank: int, world: int, dist, torch, B, W):
     """--mode sharded: one simulation of the config, targets sliced over the ranks; per KDK step one in-place all-gather
     of the staged source records (32 N bytes in total).  value = N^2 x steps / max-over-ranks device time."""
@@ -640,6 +677,7 @@ def run_ours(args, rank: int, world: int, dist):
         line["ensemble"] = _ensemble_rate(B, W, torch)
         line["adjoint"] = _adjoint_rate(B, W, torch)
         line["ensemble_adjoint"] = _ensemble_adjoint_rate(B, W, torch)
+        line["mmd"] = _mmd_rate(B, W, torch)
     print(json.dumps(line), flush=True)
 
 
@@ -654,6 +692,8 @@ def main():
                          "sliced over the ranks (strong scaling, sharded.py)")
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
+    ap.add_argument("--leg", choices=["pair_f64", "adjoint", "ensemble", "ensemble_adjoint", "mmd", "pipe_rates"], default=None,
+                    help="run one of the side legs alone and print its JSON (what the ncu captures under profiles/ run)")
     ap.add_argument("--integrator-only", action="store_true",
                     help="run only the O(N) integrator kernel's HBM roofline leg (N = 2^24) and print it")
     ap.add_argument("--cpu-pieces", action="store_true",
@@ -664,6 +704,19 @@ def main():
         return 0
     if args.impl == "reference":
         run_reference(args, int(os.environ.get("RANK", "0")))
+        return 0
+    if args.leg:
+        import torch
+        from paper_2511_22468_b200 import binding as B
+        from paper_2511_22468_b200 import workloads as W
+        legs = {"pair_f64": lambda: _steps_per_s(B, W, torch, 3, 3, np.float64),
+                "adjoint": lambda: _adjoint_rate(B, W, torch, n=65536, nsteps=4),
+                "ensemble": lambda: _ensemble_rate(B, W, torch),
+                "ensemble_adjoint": lambda: _ensemble_adjoint_rate(B, W, torch),
+                "mmd": lambda: _mmd_rate(B, W, torch),
+                "pipe_rates": lambda: {"2 warps per scheduler (1 CTA x 256)": _pipe_peaks(B, True, 1, 256),
+                                       "8 warps per scheduler (2 CTAs x 512)": _pipe_peaks(B, True, 2, 512)}}
+        print(json.dumps({args.leg: legs[args.leg]()}), flush=True)
         return 0
     if args.integrator_only:
         import torch
