@@ -81,10 +81,21 @@ int odisseo_last_cuda_error(void);
 
 /* odisseo_leapfrog_kdk_* can run a whole call as ONE cooperative launch: a persistent kernel with the time loop inside
  * and a grid barrier between the pair and the integrate phase, bit-identical to the per-step launch sequence.  By
- * default only fp64 calls on n <= 4,096 take it (measured: the two barriers per step cost what the launch edges cost;
- * see csrc/api.cu).  This sets the largest n served that way for both precisions (clamped to [0, 16384]; 0 = always
- * launch per step) and returns the previous fp64 value: a tuning and test knob, process-wide. */
+ * default only fp64 calls on 1,280 <= n <= 4,096 take it (measured: the two barriers per step cost what the launch edges
+ * cost; see csrc/api.cu).  This sets the largest n served that way for both precisions, with no lower bound (clamped
+ * to 16384; 0 = always launch per step; negative = restore the defaults) and returns the previous fp64 value: a
+ * tuning and test knob, process-wide. */
 int64_t odisseo_set_fused_max_n(int64_t n);
+
+/* Small simulations (the inference runs N = 1,000 particles for 1,000 steps) take a third form of
+ * odisseo_leapfrog_kdk_*: ONE launch of one thread-block cluster (16 CTAs) that keeps every position in the shared
+ * memory of each CTA, exchanges the moved records through distributed shared memory and synchronises with one
+ * hardware cluster barrier per step; same summation order, bit-identical to the other two forms.  Default bounds:
+ * n <= 1,024 (fp32) / 512 (fp64).  This sets the largest n served that way for both precisions (clamped to 4,096;
+ * the shared memory of a CTA bounds it further; 0 = never; negative = restore the defaults) and returns the previous
+ * fp32 value: a tuning and test knob, process-wide.  Not used with a tape, inside a stream capture or while a
+ * profile is open. */
+int64_t odisseo_set_cluster_max_n(int64_t n);
 
 /* Releases what the library keeps between calls: the cached CUDA-graph executables of odisseo_leapfrog_kdk_* and the
  * CUDA events of odisseo_profile_*.  Call with no library work in flight on other host threads; every entry point may

@@ -14,8 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libodisseo_b200.so")
 SOURCES = ["api.cu", "pair_f32.cu", "pair_f64.cu", "integrate.cu", "ensemble.cu", "diagnostics.cu", "adjoint.cu", "ensemble_adjoint.cu", "ubench.cu", "mmd.cu"]
-HEADERS = [os.path.join(CSRC, "odisseo_common.cuh"), os.path.join(CSRC, "ext_potential.cuh"), os.path.join(CSRC, "adjoint_terms.cuh"),
-           os.path.join(os.path.dirname(HERE), "include", "odisseo.h")]
+HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")) + [os.path.join(os.path.dirname(HERE), "include", "odisseo.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"] + os.environ.get("ODISSEO_NVCC_EXTRA", "").split()
 

@@ -114,7 +114,16 @@ namespace {
 // Two grid barriers per step (arrive atomic + release flag, ~2.5 us each with the fences around them) cost as much as
 // the two launch edges they replace, so the whole-loop form only pays where the per-step kernels are slowest to start:
 // fp64 up to 4,096.  fp32 keeps the per-step launches by default.
-std::atomic<int64_t> g_fused_max_n[2] = {{0}, {4096}};
+// Below n ~ 1,280 the per-step launches are faster again in fp64 (10.8 against 12.0 us at N = 1,024), hence a lower bound.
+constexpr int64_t FUSED_DEFAULT_MAX_N[2] = {0, 4096}, FUSED_DEFAULT_MIN_N[2] = {0, 1280};
+std::atomic<int64_t> g_fused_max_n[2] = {{FUSED_DEFAULT_MAX_N[0]}, {FUSED_DEFAULT_MAX_N[1]}};
+std::atomic<int64_t> g_fused_min_n[2] = {{FUSED_DEFAULT_MIN_N[0]}, {FUSED_DEFAULT_MIN_N[1]}};
+
+// Largest n the cluster kernel (cluster_kdk.cuh) serves, per precision {fp32, fp64}: the whole simulation in the shared
+// memory of one cluster of 16 CTAs, one hardware cluster barrier per step.  It uses 16 of the 148 SMs, so it wins while a
+// step on all SMs is latency-bound; odisseo_set_cluster_max_n changes the bounds (measurements at CLUSTER_DEFAULT_MAX_N).
+constexpr int64_t CLUSTER_DEFAULT_MAX_N[2] = {1024, 512};
+std::atomic<int64_t> g_cluster_max_n[2] = {{CLUSTER_DEFAULT_MAX_N[0]}, {CLUSTER_DEFAULT_MAX_N[1]}};
 
 thread_local int g_last_cuda_error = 0;
 
@@ -260,6 +269,14 @@ inline cudaError_t launch_fused(const PairPlan& p, float* x, float* v, float* a,
 inline cudaError_t launch_fused(const PairPlan& p, double* x, double* v, double* a, void* j, double* part, double G, double eps, double dt,
                                 const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* bar, cudaStream_t s)
 { return launch_fused_f64(p, x, v, a, j, part, G, eps, dt, pot, nsteps, acc_valid, bar, s); }
+inline bool cluster_fits(float, const PairPlan& p) { return cluster_fits_f32(p); }
+inline bool cluster_fits(double, const PairPlan& p) { return cluster_fits_f64(p); }
+inline cudaError_t launch_cluster(const PairPlan& p, float* x, float* v, float* a, float G, float eps, float dt, const PotParams<float>& pot,
+                                  int64_t nsteps, int acc_valid, cudaStream_t s)
+{ return launch_cluster_f32(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, s); }
+inline cudaError_t launch_cluster(const PairPlan& p, double* x, double* v, double* a, double G, double eps, double dt, const PotParams<double>& pot,
+                                  int64_t nsteps, int acc_valid, cudaStream_t s)
+{ return launch_cluster_f64(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, s); }
 inline int fused_max_ctas(float, int variant) { return fused_max_ctas_f32(variant); }
 inline int fused_max_ctas(double, int variant) { return fused_max_ctas_f64(variant); }
 
@@ -515,10 +532,19 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
 #define ODISSEO_TRY(call) do { e = (call); if (e != cudaSuccess) return cuda_fail(e); } while (0)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (s != nullptr) ODISSEO_TRY(cudaStreamIsCapturing(s, &cap));
+    // Small N: the whole call on ONE thread-block cluster (cluster_kdk.cuh): state in distributed shared memory, one
+    // cluster barrier per step, the canonical summation order -- bit-identical to the sequences below.
+    const bool one_launch_ok = nsteps >= 1 && !tape && cap == cudaStreamCaptureStatusNone && !g_prof.active;
+    if (one_launch_ok && n <= g_cluster_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && cluster_fits(T(), plan)) {
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        ODISSEO_TRY(launch_cluster(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, s));
+        return ODISSEO_OK;
+    }
     // Small and mid N: the whole call in ONE cooperative launch (fused_step.cuh) -- same plan, same code per phase, hence
     // bit-identical to the two-kernel sequence below.  Not inside a caller's capture, with a tape, or while a profile
     // is open (its event pairs bracket pair-kernel launches).
-    if (n <= g_fused_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && nsteps >= 1 && !tape && cap == cudaStreamCaptureStatusNone && !g_prof.active) {
+    if (one_launch_ok && n <= g_fused_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) &&
+        n >= g_fused_min_n[sizeof(T) == 8].load(std::memory_order_relaxed)) {
         PairPlan fplan = plan;
         const int cap_ctas = fused_max_ctas(T(), plan.variant);
         if (cap_ctas >= 1) {
@@ -854,10 +880,17 @@ int64_t odisseo_launch_count(void) { return g_launches.load(); }
 
 int64_t odisseo_set_fused_max_n(int64_t n)
 {
-    if (n < 0) n = 0;
     if (n > 16384) n = 16384;
-    g_fused_max_n[0].store(n);
-    return g_fused_max_n[1].exchange(n);
+    for (int k = 0; k < 2; ++k) g_fused_min_n[k].store(n < 0 ? FUSED_DEFAULT_MIN_N[k] : 0);
+    g_fused_max_n[0].store(n < 0 ? FUSED_DEFAULT_MAX_N[0] : n);
+    return g_fused_max_n[1].exchange(n < 0 ? FUSED_DEFAULT_MAX_N[1] : n);
+}
+
+int64_t odisseo_set_cluster_max_n(int64_t n)
+{
+    if (n > CLUSTER_MAX_N) n = CLUSTER_MAX_N;
+    g_cluster_max_n[1].store(n < 0 ? CLUSTER_DEFAULT_MAX_N[1] : n);
+    return g_cluster_max_n[0].exchange(n < 0 ? CLUSTER_DEFAULT_MAX_N[0] : n);
 }
 
 odisseo_status odisseo_shutdown(void)

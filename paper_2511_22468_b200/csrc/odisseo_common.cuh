@@ -375,4 +375,13 @@ cudaError_t launch_fused_f64(const PairPlan& plan, double* posm, double* vel, do
                              double eps, double dt, const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* barrier,
                              cudaStream_t stream);
 
+// cluster kernels (cluster_kdk.cuh): the whole KDK loop of a small simulation on one thread-block cluster
+constexpr int CLUSTER_MAX_N = 4096;               // upper bound of the knob; shared memory bounds it further
+bool cluster_fits_f32(const PairPlan& plan);
+bool cluster_fits_f64(const PairPlan& plan);
+cudaError_t launch_cluster_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
+                               const PotParams<float>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream);
+cudaError_t launch_cluster_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
+                               const PotParams<double>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream);
+
 }  // namespace odisseo

@@ -21,6 +21,7 @@
 //     reduce step multiplies by the mass once;
 //   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
 #include "fused_step.cuh"
+#include "cluster_kdk.cuh"
 
 namespace odisseo {
 
@@ -114,6 +115,24 @@ struct PairF32 {
                 ax[p] = ay[p] = az[p] = 0ull;
             }
         }
+        // cluster kernel (cluster_kdk.cuh): two targets handed over as records; tile sums promoted into six doubles
+        __device__ __forceinline__ void set_target_pair(const float4 p0, const float4 p1)
+        {
+            static_assert(NPAIR >= 1, "one packed pair");
+            const f32x2 nz = pk(-0.0f, -0.0f);
+            xi[0] = add2(pk(p0.x, p1.x), nz);
+            yi[0] = add2(pk(p0.y, p1.y), nz);
+            zi[0] = add2(pk(p0.z, p1.z), nz);
+            ax[0] = ay[0] = az[0] = 0ull;
+        }
+        __device__ __forceinline__ void take_sums(double (&s)[6])
+        {
+            float lo, hi;
+            unpk(ax[0], lo, hi); s[0] += (double)lo; s[3] += (double)hi;
+            unpk(ay[0], lo, hi); s[1] += (double)lo; s[4] += (double)hi;
+            unpk(az[0], lo, hi); s[2] += (double)lo; s[5] += (double)hi;
+            ax[0] = ay[0] = az[0] = 0ull;
+        }
         __device__ __forceinline__ void write_row(double* __restrict__ row)
         {
 #pragma unroll
@@ -131,7 +150,10 @@ typedef PairF32<4, 8, 1, 8> LargeF32;    // 2,048 targets per CTA, one CTA per S
 typedef PairF32<1, 2, 8, 4> SmallF32;    // 128 targets per CTA, up to 8 CTAs per SM (n <= 4,096)
 typedef PairF32<1, 2, 4, 4> SmallF32Fused;   // the same loop inside the whole-loop kernel, which also holds the reduce batch
 
+typedef PairF32<1, 2, 1, 4> ClusterF32;      // the same loop, two targets per lane, inside the cluster kernel (cluster_kdk.cuh)
+
 int g_fused_max_ctas[2] = {0, 0};        // co-resident CTAs of the whole-loop kernel, [variant]
+int g_cluster_size = 0;                  // CTAs per cluster the device schedules for the cluster kernel (0 = none)
 
 }  // namespace
 
@@ -141,6 +163,7 @@ cudaError_t configure_pair_f32(int num_sms)
     if (e == cudaSuccess) e = configure_stream<SmallF32>(256);
     if (e == cudaSuccess) e = configure_fused<LargeF32, float>(512, num_sms, &g_fused_max_ctas[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF32Fused, float>(256, num_sms, &g_fused_max_ctas[1]);
+    if (e == cudaSuccess) e = configure_cluster<ClusterF32, float>(&g_cluster_size);
     return e;
 }
 
@@ -159,6 +182,24 @@ cudaError_t launch_fused_f32(const PairPlan& plan, float* posm, float* vel, floa
     }
     const SmallF32Fused::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
     return launch_fused<SmallF32Fused, float>(plan, prm, jsrc, partials, fa, stream);
+}
+
+// Cluster kernel (cluster_kdk.cuh): does this call fit the shared memory of one cluster?
+bool cluster_fits_f32(const PairPlan& plan)
+{
+    int32_t tpc;
+    return g_cluster_size > 0 && plan.n <= CLUSTER_MAX_N && cluster_geometry<float>(plan, g_cluster_size, &tpc) != 0;
+}
+
+cudaError_t launch_cluster_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
+                               const PotParams<float>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream)
+{
+    ClusterArgs<float> ca;
+    ca.posm = reinterpret_cast<float4*>(posm); ca.vel = reinterpret_cast<float4*>(vel); ca.acc = reinterpret_cast<float4*>(acc);
+    ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
+    ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
+    const size_t smem = cluster_geometry<float>(plan, g_cluster_size, &ca.tpc);
+    return launch_cluster<ClusterF32, float>(ca, g_cluster_size, smem, stream);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,

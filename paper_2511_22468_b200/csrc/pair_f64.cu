@@ -12,6 +12,7 @@
 // Summation: fp64 inside a tile, tile sums added in tile order inside a unit, one row per unit -- the
 // same fixed grouping as the fp32 kernel.
 #include "fused_step.cuh"
+#include "cluster_kdk.cuh"
 
 namespace odisseo {
 
@@ -100,6 +101,20 @@ struct PairF64 {
                 ax[k] = ay[k] = az[k] = 0.0;
             }
         }
+        // cluster kernel (cluster_kdk.cuh): two targets handed over as records; tile sums added into six doubles
+        __device__ __forceinline__ void set_target_pair(const double4 p0, const double4 p1)
+        {
+            static_assert(IPT >= 2, "two targets per thread");
+            xi[0] = p0.x; yi[0] = p0.y; zi[0] = p0.z;
+            xi[1] = p1.x; yi[1] = p1.y; zi[1] = p1.z;
+            ax[0] = ay[0] = az[0] = ax[1] = ay[1] = az[1] = 0.0;
+        }
+        __device__ __forceinline__ void take_sums(double (&s)[6])
+        {
+            s[0] += ax[0]; s[1] += ay[0]; s[2] += az[0];
+            s[3] += ax[1]; s[4] += ay[1]; s[5] += az[1];
+            ax[0] = ay[0] = az[0] = ax[1] = ay[1] = az[1] = 0.0;
+        }
         __device__ __forceinline__ void write_row(double* __restrict__ row)
         {
 #pragma unroll
@@ -121,7 +136,10 @@ typedef PairF64<4, 8, 1, 4, true> LargePot;
 typedef PairF64<2, 2, 8, 2, true> SmallPot;
 typedef PairF64<2, 2, 4, 2, false> SmallF64Fused;
 
+typedef PairF64<2, 2, 1, 2, false> ClusterF64;   // the same loop inside the cluster kernel (cluster_kdk.cuh)
+
 int g_fused_max_ctas64[2] = {0, 0};
+int g_cluster_size64 = 0;
 
 }  // namespace
 
@@ -133,6 +151,7 @@ cudaError_t configure_pair_f64(int num_sms)
     if (e == cudaSuccess) e = configure_stream<SmallPot>(256);
     if (e == cudaSuccess) e = configure_fused<LargeF64, double>(256, num_sms, &g_fused_max_ctas64[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF64Fused, double>(256, num_sms, &g_fused_max_ctas64[1]);
+    if (e == cudaSuccess) e = configure_cluster<ClusterF64, double>(&g_cluster_size64);
     return e;
 }
 
@@ -151,6 +170,23 @@ cudaError_t launch_fused_f64(const PairPlan& plan, double* posm, double* vel, do
     }
     const SmallF64Fused::Params prm{reinterpret_cast<const double4*>(posm), eps * eps};
     return launch_fused<SmallF64Fused, double>(plan, prm, jsrc, partials, fa, stream);
+}
+
+bool cluster_fits_f64(const PairPlan& plan)
+{
+    int32_t tpc;
+    return g_cluster_size64 > 0 && plan.n <= CLUSTER_MAX_N && cluster_geometry<double>(plan, g_cluster_size64, &tpc) != 0;
+}
+
+cudaError_t launch_cluster_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
+                               const PotParams<double>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream)
+{
+    ClusterArgs<double> ca;
+    ca.posm = reinterpret_cast<double4*>(posm); ca.vel = reinterpret_cast<double4*>(vel); ca.acc = reinterpret_cast<double4*>(acc);
+    ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
+    ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
+    const size_t smem = cluster_geometry<double>(plan, g_cluster_size64, &ca.tpc);
+    return launch_cluster<ClusterF64, double>(ca, g_cluster_size64, smem, stream);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
