@@ -59,6 +59,29 @@ def pair_accel_vjp(posm, c, G, eps):
     return gx, gm, gG, geps
 
 
+def pair_accel_vjp_scale(posm, c, G, eps):
+    """Per-particle sums of the MAGNITUDES of the terms pair_accel_vjp adds, the denominators of the per-element
+    gradient tolerance (the analogue of S_i = sum_j |a_ij| of the forward tolerance, reading R6):
+      Sx_i = G sum_j (f |u| + |g| |d| |d.u|),   Sm_i = G sum_j f |d.c_j|.
+    By the triangle inequality |gx_i| <= Sx_i and |gm_i| <= Sm_i, with equality when a particle has one partner
+    and u is parallel to d (tests/test_oracle_adjoint.py)."""
+    posm = np.asarray(posm, dtype=np.float64)
+    c = np.asarray(c, dtype=np.float64)
+    x, m = posm[:, :3], posm[:, 3]
+    d = x[None, :, :] - x[:, None, :]
+    s = np.einsum("ijk,ijk->ij", d, d) + eps * eps
+    with np.errstate(divide="ignore"):
+        f = s ** -1.5
+        g = 3.0 * s ** -2.5
+    np.fill_diagonal(f, 0.0)
+    np.fill_diagonal(g, 0.0)
+    u = m[:, None, None] * c[None, :, :] - m[None, :, None] * c[:, None, :]
+    du = np.abs(np.einsum("ijk,ijk->ij", d, u))
+    Sx = G * np.sum(f * np.linalg.norm(u, axis=2) + g * np.linalg.norm(d, axis=2) * du, axis=1)
+    Sm = G * np.sum(f * np.abs(np.einsum("ijk,jk->ij", d, c)), axis=1)
+    return Sx, Sm
+
+
 def _nfw_parts(x, G, Ms, rs):
     r = np.linalg.norm(x, axis=1)
     cc = r / rs

@@ -536,9 +536,12 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     // cluster barrier per step, the canonical summation order -- bit-identical to the sequences below.
     const bool one_launch_ok = nsteps >= 1 && !tape && cap == cudaStreamCaptureStatusNone && !g_prof.active;
     if (one_launch_ok && n <= g_cluster_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && cluster_fits(T(), plan)) {
-        g_launches.fetch_add(1, std::memory_order_relaxed);
-        ODISSEO_TRY(launch_cluster(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, s));
-        return ODISSEO_OK;
+        // a device that cannot place the cluster right now (partitioned or shared GPU) takes the sequences below
+        if (launch_cluster(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, s) == cudaSuccess) {
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            return ODISSEO_OK;
+        }
+        (void)cudaGetLastError();
     }
     // Small and mid N: the whole call in ONE cooperative launch (fused_step.cuh) -- same plan, same code per phase, hence
     // bit-identical to the two-kernel sequence below.  Not inside a caller's capture, with a tape, or while a profile

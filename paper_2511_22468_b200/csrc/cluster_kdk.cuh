@@ -9,9 +9,16 @@
 //     shared-memory broadcasts, the Consumer's very inner loop (State::tile of pair_f32.cu / pair_f64.cu);
 //   * reduce + integrate: the owner thread of a particle adds its S chunk sums in increasing s (fp64), applies G [m],
 //     the external acceleration and the kicks / drift (the arithmetic of step_body.cuh), and PUSHES the new record into
-//     the shared memory of every CTA of the cluster (st.shared::cluster, distributed shared memory);
-//   * one hardware cluster barrier per step (barrier.cluster arrive.release / wait.acquire, ~0.2 us) instead of two
-//     grid barriers or two launch edges; positions, velocities and accelerations never leave the SMs inside the loop.
+//     the shared memory of every CTA of the cluster with asynchronous distributed-shared-memory stores whose bytes are
+//     counted on an mbarrier of the destination CTA (st.async ... mbarrier::complete_tx::bytes);
+//   * a CTA starts the next step when its own "inbox" barrier has counted the n records of this step: no cluster-wide
+//     barrier, no grid barrier, no launch edge inside the loop; positions, velocities and accelerations never leave
+//     the SMs.  Two record buffers and two inbox barriers alternate, which is enough: a CTA pushes step k + 1 only
+//     after it has received every push of step k, and a CTA pushes step k only after it has read buffer k.
+// Measured (B200, us per KDK step, this kernel / per-step launches): fp32 N = 128 2.4 / 4.8, 256 2.9 / 5.4, 512 4.1 / 6.2,
+// 1,024 7.0 / 7.8; fp64 256 6.1 / 7.4, 512 7.8 / 8.3, 1,024 13.8 / 10.8.  It runs on 16 of the 148 SMs, so above N ~ 1,000
+// the pair phase (N^2 / 16 per SM; 9.3 k of the 13.5 k cycles of a step at N = 1,024) costs more than the latency it saves;
+// the sequential fp64 sum of the S chunk rows (1.9 k cycles at S = 22) is the price of the canonical order.
 //
 // Summation order: chunk and tile boundaries are the launch plan's (functions of n alone), tile sums in the Consumer's
 // precision, promoted to fp64 per tile, chunk sums added in increasing s, factor G [m] applied once in fp64 -- the
@@ -145,14 +152,7 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
         __syncthreads();
     };
     // chunk sums of the owned targets: item = (group of 64 targets, chunk s) per warp, two targets per lane
-#ifdef ODISSEO_CLUSTER_TIMING
-    long long tq[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tmark = clock64();
-#define CLUSTER_MARK(k) do { const long long now_ = clock64(); tq[k] += now_ - tmark; tmark = now_; } while (0)
-#else
-#define CLUSTER_MARK(k) do { } while (0)
-#endif
     auto pair_phase = [&]() {
-        CLUSTER_MARK(4);
         typename C::template State<EQM> st(prm, fake, nullptr);
         const V4* rec = records(cb);
         const unsigned char* src = staged(cb);
@@ -177,7 +177,6 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
             }
         }
         __syncthreads();
-        CLUSTER_MARK(0);
     };
     // the per-particle body of step_body.cuh on the owner thread; OPEN pushes the moved record to every CTA
     auto integrate = [&](const bool reduce, const bool close, const bool open) {
@@ -205,7 +204,6 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
                 }
                 a.x = (T)(gm * sx); a.y = (T)(gm * sy); a.z = (T)(gm * sz); a.w = (T)0;
                 sacc[tid] = a;
-                CLUSTER_MARK(5);
             } else {
                 a = sacc[tid];
             }
@@ -232,20 +230,14 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
                 v.w = (T)0;
                 svel[tid] = v;
             }
-            CLUSTER_MARK(6);
         }
         if (open) {
             const int nb = cb ^ 1;
-            CLUSTER_MARK(1);
             mbar_wait(&inbox[nb], inbox_phase[nb]);                  // every other CTA's records of this step have landed
             inbox_phase[nb] ^= 1u;
             if (tid == 0) mbar_arrive_expect_tx(&inbox[nb], incoming);   // arm the next use of this buffer (two steps on)
-            CLUSTER_MARK(2);
             cb = nb;
             expand();
-            CLUSTER_MARK(3);
-        } else {
-            CLUSTER_MARK(1);
         }
     };
 
@@ -272,9 +264,6 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
         ca.vel[me] = svel[tid];
         ca.acc[me] = sacc[tid];
     }
-#ifdef ODISSEO_CLUSTER_TIMING
-    if (rank == 0 && tid < 8) reinterpret_cast<T*>(ca.acc + tid)[3] = (T)((double)tq[tid] / (double)ca.nsteps);
-#endif
 }
 
 template <class C, typename T>

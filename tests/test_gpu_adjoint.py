@@ -90,6 +90,22 @@ def test_accel_vjp_equal_masses_take_the_tile_wise_equal_mass_loop(n, dtype, tol
         assert np.abs(gm2 - rm2).max() <= tol * np.abs(rm2).max()
 
 
+@pytest.mark.parametrize("n", [2, 129, 1000, 3001])
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-12), (np.float32, 1e-5)])
+@pytest.mark.parametrize("unequal", [True, False])
+def test_accel_vjp_per_element_bound(n, dtype, tol, unequal):
+    """Every particle's gradient against the sum of the magnitudes of ITS OWN terms (not the largest component of the
+    whole array): |gx_i - ref_i| <= tol * G sum_j (f |u| + |g| |d| |d.u|), |gm_i - ref_i| <= tol * G sum_j f |d.c_j| --
+    the forward tolerance's form (north_star: |a_gpu,i - a_ref,i| / sum_j |a_ij|) carried to the pull-back."""
+    cfg, p, _, c, G, eps = _inputs(n, 900 + n, dtype, unequal=unequal)
+    gx, gm, _ = gpu_accel_vjp(p, c, G, eps, None, dtype, with_eps_G=False)
+    p64, c64 = p.astype(np.float64), c.astype(np.float64)
+    rx, rm, _, _ = A.pair_accel_vjp(p64, c64, G, eps)
+    Sx, Sm = A.pair_accel_vjp_scale(p64, c64, G, eps)
+    assert np.all(np.linalg.norm(gx[:, :3] - rx, axis=1) <= tol * Sx)
+    assert np.all(np.abs(gm - rm) <= tol * Sm)
+
+
 def test_accel_vjp_without_potential_and_reproducible():
     cfg, p, _, c, G, eps = _inputs(2000, 77, np.float64)
     a = gpu_accel_vjp(p, c, G, eps, None, np.float64)

@@ -116,3 +116,26 @@ def test_leapfrog_vjp_matches_finite_differences_of_the_forward_leapfrog(nsteps)
     for name, ref in refs.items():
         # the loss is O(100) and d loss / d eps O(1e-4): the difference quotient carries ~1e-5 of rounding noise
         assert abs(g[name] - ref) <= (1e-4 if name == "eps" else 2e-6) * abs(ref) + 1e-12 * abs(g["dt"]), name
+
+
+def test_pair_vjp_scale_bounds_the_gradient_and_is_tight_for_one_aligned_partner():
+    """The per-element tolerance denominators: triangle inequality on random inputs, equality for two particles
+    whose u = m_0 c_1 - m_1 c_0 is parallel to their separation (closed form: G (f |u| + |g| |d|^2 |u|))."""
+    rng = np.random.default_rng(5)
+    posm = np.concatenate([rng.normal(size=(17, 3)), rng.uniform(0.5, 2.0, size=(17, 1))], axis=1)
+    c = rng.normal(size=(17, 3))
+    gx, gm, _, _ = A.pair_accel_vjp(posm, c, 1.3, 0.2)
+    Sx, Sm = A.pair_accel_vjp_scale(posm, c, 1.3, 0.2)
+    assert np.all(np.linalg.norm(gx, axis=1) <= Sx * (1 + 1e-12)) and np.all(np.abs(gm) <= Sm * (1 + 1e-12))
+    assert np.all(Sx > 0) and np.all(Sm > 0)
+    two = np.array([[0.0, 0.0, 0.0, 2.0], [3.0, 0.0, 0.0, 5.0]])
+    c2 = np.array([[1.0, 0.0, 0.0], [-0.5, 0.0, 0.0]])                  # u_01 = 2 (-0.5) - 5 (1) = -6 along x = along d
+    G, eps = 0.7, 4.0
+    s = 9.0 + 16.0
+    expect = G * (s ** -1.5 * 6.0 + 3.0 * s ** -2.5 * 3.0 * 18.0)
+    Sx2, Sm2 = A.pair_accel_vjp_scale(two, c2, G, eps)
+    gx2, gm2, _, _ = A.pair_accel_vjp(two, c2, G, eps)
+    assert abs(Sx2[0] - expect) <= 1e-15 * expect and abs(Sx2[1] - expect) <= 1e-15 * expect
+    # f u and g d (d.u) have opposite signs here, so the gradient is strictly smaller than the scale
+    assert abs(gx2[0, 0]) < Sx2[0] and abs(abs(gx2[0, 0]) - G * abs(s ** -1.5 * 6.0 - 3.0 * s ** -2.5 * 54.0)) <= 1e-15
+    assert abs(Sm2[0] - G * s ** -1.5 * 1.5) <= 1e-16 and abs(abs(gm2[0]) - Sm2[0]) <= 1e-16
