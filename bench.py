@@ -302,6 +302,42 @@ def _steps_per_s(B, W, torch, ci: int, nsteps: int, dtype=np.float32):
             "steps_per_s": nsteps / (ms * 1e-3), "G_int_per_s": nsteps * float(cfg.n) ** 2 / (ms * 1e-3) / 1e9}
 
 
+def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048), nsteps: int = 2000):
+    """us per KDK step of config-0-shaped simulations under the three launch forms of odisseo_leapfrog_kdk_*: the
+    thread-block-cluster kernel (csrc/cluster_kdk.cuh), the per-step launches (CUDA graph + programmatic dependent
+    launch) and the cooperative whole-loop kernel (csrc/fused_step.cuh).  All three give bit-identical results."""
+    cfg = W.CONFIGS[0]
+    out = []
+    try:
+        for dtype in (np.float32, np.float64):
+            for n in sizes:
+                posm64, vel64 = W.make_state(cfg, n=n)
+                row = {"n": n, "dtype": "f32" if dtype == np.float32 else "f64"}
+                for form, (cluster, fused) in {"cluster": (4096, 0), "per_step": (0, 0), "cooperative": (0, 16384)}.items():
+                    B.set_cluster_max_n(cluster)
+                    B.set_fused_max_n(fused)
+                    posm = torch.from_numpy(np.ascontiguousarray(posm64, dtype=dtype)).cuda()
+                    vel = torch.from_numpy(W.vel4(vel64.astype(dtype), dtype)).cuda()
+                    acc = torch.empty_like(posm)
+                    ws = B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64))
+                    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, 40, None, ws)
+                    torch.cuda.synchronize()
+                    best = float("inf")
+                    for _ in range(3):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, None, ws, acc_valid=True)
+                        e1.record()
+                        torch.cuda.synchronize()
+                        best = min(best, e0.elapsed_time(e1))
+                    row[form + "_us_per_step"] = best * 1e3 / nsteps
+                out.append(row)
+    finally:
+        B.set_cluster_max_n(-1)
+        B.set_fused_max_n(-1)
+    return out
+
+
 def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: int = 10):
     """HBM roofline of the O(N) integrator kernel (reduce-free form: reads posm, vel, acc; writes posm, vel and
     the staged sources = 112 B per particle in fp32) through odisseo_kick_drift_f32 at N = 2^24: 1.9 GB per
@@ -532,6 +568,8 @@ def run_ours(args, rank: int, world: int, dist):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a B200: the hot path has no CPU fallback")
     dev = torch.cuda.current_device()
+    # everything runs on one non-default stream: the library replays its CUDA graphs only off the legacy stream
+    torch.cuda.set_stream(torch.cuda.Stream())
     cfg = W.CONFIGS[args.config]
     n = cfg.n
     if args.mode == "sharded":
@@ -678,6 +716,7 @@ def run_ours(args, rank: int, world: int, dist):
         line["adjoint"] = _adjoint_rate(B, W, torch)
         line["ensemble_adjoint"] = _ensemble_adjoint_rate(B, W, torch)
         line["mmd"] = _mmd_rate(B, W, torch)
+        line["small_n_launch_forms"] = _small_n_forms(B, W, torch, sizes=(256, 1024), nsteps=1000)
     print(json.dumps(line), flush=True)
 
 
@@ -692,7 +731,7 @@ def main():
                          "sliced over the ranks (strong scaling, sharded.py)")
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the other-config lines")
-    ap.add_argument("--leg", choices=["pair_f64", "adjoint", "ensemble", "ensemble_adjoint", "mmd", "pipe_rates"], default=None,
+    ap.add_argument("--leg", choices=["pair_f64", "adjoint", "ensemble", "ensemble_adjoint", "mmd", "pipe_rates", "small_n"], default=None,
                     help="run one of the side legs alone and print its JSON (what the ncu captures under profiles/ run)")
     ap.add_argument("--integrator-only", action="store_true",
                     help="run only the O(N) integrator kernel's HBM roofline leg (N = 2^24) and print it")
@@ -709,11 +748,13 @@ def main():
         import torch
         from paper_2511_22468_b200 import binding as B
         from paper_2511_22468_b200 import workloads as W
+        torch.cuda.set_stream(torch.cuda.Stream())
         legs = {"pair_f64": lambda: _steps_per_s(B, W, torch, 3, 3, np.float64),
                 "adjoint": lambda: _adjoint_rate(B, W, torch, n=65536, nsteps=4),
                 "ensemble": lambda: _ensemble_rate(B, W, torch),
                 "ensemble_adjoint": lambda: _ensemble_adjoint_rate(B, W, torch),
                 "mmd": lambda: _mmd_rate(B, W, torch),
+                "small_n": lambda: _small_n_forms(B, W, torch),
                 "pipe_rates": lambda: {"2 warps per scheduler (1 CTA x 256)": _pipe_peaks(B, True, 1, 256),
                                        "8 warps per scheduler (2 CTAs x 512)": _pipe_peaks(B, True, 2, 512)}}
         print(json.dumps({args.leg: legs[args.leg]()}), flush=True)
