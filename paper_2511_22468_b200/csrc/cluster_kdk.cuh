@@ -17,8 +17,10 @@
 //     after it has received every push of step k, and a CTA pushes step k only after it has read buffer k.
 // Measured (B200, us per KDK step, this kernel / per-step launches): fp32 N = 128 2.4 / 4.8, 256 2.9 / 5.4, 512 4.1 / 6.2,
 // 1,024 7.0 / 7.8; fp64 256 6.1 / 7.4, 512 7.8 / 8.3, 1,024 13.8 / 10.8.  It runs on 16 of the 148 SMs, so above N ~ 1,000
-// the pair phase (N^2 / 16 per SM; 9.3 k of the 13.5 k cycles of a step at N = 1,024) costs more than the latency it saves;
-// the sequential fp64 sum of the S chunk rows (1.9 k cycles at S = 22) is the price of the canonical order.
+// the pair phase (N^2 / 16 per SM; 9.3 k of the 13.5 k cycles of a step at N = 1,024) costs more than the latency it saves.
+// The rest of a step at N = 1,024: the owners' row reduce 1.9 k cycles (a balanced-tree grouping was tried: no faster),
+// kicks + drift + 16 pushes 0.65 k, waiting for the other CTAs' records 0.9 k, re-expansion 0.6 k
+// (profiles/r02_cluster_kdk_ncu_full.txt).
 //
 // Summation order: chunk and tile boundaries are the launch plan's (functions of n alone), tile sums in the Consumer's
 // precision, promoted to fp64 per tile, chunk sums added in increasing s, factor G [m] applied once in fp64 -- the
