@@ -302,10 +302,11 @@ def _steps_per_s(B, W, torch, ci: int, nsteps: int, dtype=np.float32):
             "steps_per_s": nsteps / (ms * 1e-3), "G_int_per_s": nsteps * float(cfg.n) ** 2 / (ms * 1e-3) / 1e9}
 
 
-def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048), nsteps: int = 2000):
-    """us per KDK step of config-0-shaped simulations under the three launch forms of odisseo_leapfrog_kdk_*: the
-    thread-block-cluster kernel (csrc/cluster_kdk.cuh), the per-step launches (CUDA graph + programmatic dependent
-    launch) and the cooperative whole-loop kernel (csrc/fused_step.cuh).  All three give bit-identical results."""
+def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048, 4096), nsteps: int = 2000):
+    """us per KDK step of config-0-shaped simulations under the four launch forms of odisseo_leapfrog_kdk_*: the
+    owner-computes kernel with the flag-in-data exchange (csrc/ll_kdk.cuh), the thread-block-cluster kernel
+    (csrc/cluster_kdk.cuh), the per-step launches (CUDA graph + programmatic dependent launch) and the cooperative
+    whole-loop kernel (csrc/fused_step.cuh).  All four give bit-identical results."""
     cfg = W.CONFIGS[0]
     out = []
     try:
@@ -313,7 +314,9 @@ def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048), nsteps: int = 2000
             for n in sizes:
                 posm64, vel64 = W.make_state(cfg, n=n)
                 row = {"n": n, "dtype": "f32" if dtype == np.float32 else "f64"}
-                for form, (cluster, fused) in {"cluster": (4096, 0), "per_step": (0, 0), "cooperative": (0, 16384)}.items():
+                for form, (ll, cluster, fused) in {"flag_in_data": (6144, 0, 0), "cluster": (0, 4096, 0), "per_step": (0, 0, 0),
+                                                   "cooperative": (0, 0, 16384)}.items():
+                    B.set_ll_max_n(ll)
                     B.set_cluster_max_n(cluster)
                     B.set_fused_max_n(fused)
                     posm = torch.from_numpy(np.ascontiguousarray(posm64, dtype=dtype)).cuda()
@@ -333,6 +336,7 @@ def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048), nsteps: int = 2000
                     row[form + "_us_per_step"] = best * 1e3 / nsteps
                 out.append(row)
     finally:
+        B.set_ll_max_n(-1)
         B.set_cluster_max_n(-1)
         B.set_fused_max_n(-1)
     return out

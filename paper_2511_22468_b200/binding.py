@@ -25,7 +25,7 @@ EXPORTS = [
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
     "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
-    "odisseo_profile_end", "odisseo_profile_times", "odisseo_shutdown", "odisseo_set_fused_max_n", "odisseo_set_cluster_max_n", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
+    "odisseo_profile_end", "odisseo_profile_times", "odisseo_shutdown", "odisseo_set_fused_max_n", "odisseo_set_cluster_max_n", "odisseo_set_ll_max_n", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
     "odisseo_vjp_workspace_bytes", "odisseo_tape_bytes", "odisseo_accel_vjp_f32", "odisseo_accel_vjp_f64",
@@ -143,6 +143,8 @@ def lib():
         L.odisseo_set_fused_max_n.argtypes = [i64]
         L.odisseo_set_cluster_max_n.restype = i64
         L.odisseo_set_cluster_max_n.argtypes = [i64]
+        L.odisseo_set_ll_max_n.restype = i64
+        L.odisseo_set_ll_max_n.argtypes = [i64]
         L.odisseo_ubench_kinds.argtypes = []
         L.odisseo_ubench_name.restype = ctypes.c_char_p
         L.odisseo_ubench_name.argtypes = [ci]
@@ -583,6 +585,12 @@ def mmd2(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch
 def set_fused_max_n(n: int) -> int:
     """Largest n leapfrog_kdk runs as one cooperative whole-loop launch (0 = never); returns the previous value."""
     return int(lib().odisseo_set_fused_max_n(int(n)))
+
+
+def set_ll_max_n(n: int) -> int:
+    """Largest n leapfrog_kdk runs as the owner-computes whole-loop kernel with the flag-in-data exchange (0 = never,
+    negative = defaults); returns the previous fp32 value."""
+    return int(lib().odisseo_set_ll_max_n(int(n)))
 
 
 def set_cluster_max_n(n: int) -> int:

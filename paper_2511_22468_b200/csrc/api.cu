@@ -122,6 +122,10 @@ std::atomic<int64_t> g_fused_min_n[2] = {{FUSED_DEFAULT_MIN_N[0]}, {FUSED_DEFAUL
 // Largest n the cluster kernel (cluster_kdk.cuh) serves, per precision {fp32, fp64}: the whole simulation in the shared
 // memory of one cluster of 16 CTAs, one hardware cluster barrier per step.  It uses 16 of the 148 SMs, so it wins while a
 // step on all SMs is latency-bound; odisseo_set_cluster_max_n changes the bounds (measurements at CLUSTER_DEFAULT_MAX_N).
+// Largest n the flag-in-data whole-loop kernel (ll_kdk.cuh) serves, per precision {fp32, fp64}: owner-computes on all SMs,
+// the moved positions exchanged as {value, step tag} words through L2 -- one round trip per step.  Tried first.
+constexpr int64_t LL_DEFAULT_MAX_N[2] = {4096, 2048};
+std::atomic<int64_t> g_ll_max_n[2] = {{LL_DEFAULT_MAX_N[0]}, {LL_DEFAULT_MAX_N[1]}};
 constexpr int64_t CLUSTER_DEFAULT_MAX_N[2] = {1024, 512};
 std::atomic<int64_t> g_cluster_max_n[2] = {{CLUSTER_DEFAULT_MAX_N[0]}, {CLUSTER_DEFAULT_MAX_N[1]}};
 
@@ -269,6 +273,14 @@ inline cudaError_t launch_fused(const PairPlan& p, float* x, float* v, float* a,
 inline cudaError_t launch_fused(const PairPlan& p, double* x, double* v, double* a, void* j, double* part, double G, double eps, double dt,
                                 const PotParams<double>& pot, int64_t nsteps, int acc_valid, unsigned* bar, cudaStream_t s)
 { return launch_fused_f64(p, x, v, a, j, part, G, eps, dt, pot, nsteps, acc_valid, bar, s); }
+inline size_t ll_fits(float, const PairPlan& p) { return ll_fits_f32(p); }
+inline size_t ll_fits(double, const PairPlan& p) { return ll_fits_f64(p); }
+inline cudaError_t launch_ll(const PairPlan& p, float* x, float* v, float* a, float G, float eps, float dt, const PotParams<float>& pot,
+                             int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t s)
+{ return launch_ll_f32(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, s); }
+inline cudaError_t launch_ll(const PairPlan& p, double* x, double* v, double* a, double G, double eps, double dt, const PotParams<double>& pot,
+                             int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t s)
+{ return launch_ll_f64(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, s); }
 inline bool cluster_fits(float, const PairPlan& p) { return cluster_fits_f32(p); }
 inline bool cluster_fits(double, const PairPlan& p) { return cluster_fits_f64(p); }
 inline cudaError_t launch_cluster(const PairPlan& p, float* x, float* v, float* a, float G, float eps, float dt, const PotParams<float>& pot,
@@ -535,6 +547,19 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     // Small N: the whole call on ONE thread-block cluster (cluster_kdk.cuh): state in distributed shared memory, one
     // cluster barrier per step, the canonical summation order -- bit-identical to the sequences below.
     const bool one_launch_ok = nsteps >= 1 && !tape && cap == cudaStreamCaptureStatusNone && !g_prof.active;
+    // Small N, first choice: the whole call as ONE cooperative launch of the owner-computes kernel (ll_kdk.cuh): every CTA
+    // holds all sources in shared memory and integrates its own few targets; the moved positions travel as {value, step
+    // tag} words through the (otherwise unused) partial-row area of the workspace -- one L2 round trip per step.
+    if (one_launch_ok && n <= g_ll_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && nsteps < (int64_t)0x7fffffff) {
+        const size_t xbytes = ll_fits(T(), plan);
+        if (xbytes != 0 && xbytes <= plan_partial_bytes(plan)) {
+            if (launch_ll(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, cv.partials, s) == cudaSuccess) {
+                g_launches.fetch_add(1, std::memory_order_relaxed);
+                return ODISSEO_OK;
+            }
+            (void)cudaGetLastError();          // the device cannot hold the grid right now: the forms below do not need that
+        }
+    }
     if (one_launch_ok && n <= g_cluster_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && cluster_fits(T(), plan)) {
         // a device that cannot place the cluster right now (partitioned or shared GPU) takes the sequences below
         if (launch_cluster(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, s) == cudaSuccess) {
@@ -887,6 +912,13 @@ int64_t odisseo_set_fused_max_n(int64_t n)
     for (int k = 0; k < 2; ++k) g_fused_min_n[k].store(n < 0 ? FUSED_DEFAULT_MIN_N[k] : 0);
     g_fused_max_n[0].store(n < 0 ? FUSED_DEFAULT_MAX_N[0] : n);
     return g_fused_max_n[1].exchange(n < 0 ? FUSED_DEFAULT_MAX_N[1] : n);
+}
+
+int64_t odisseo_set_ll_max_n(int64_t n)
+{
+    if (n > LL_MAX_N) n = LL_MAX_N;
+    g_ll_max_n[1].store(n < 0 ? LL_DEFAULT_MAX_N[1] : n);
+    return g_ll_max_n[0].exchange(n < 0 ? LL_DEFAULT_MAX_N[0] : n);
 }
 
 int64_t odisseo_set_cluster_max_n(int64_t n)

@@ -95,8 +95,13 @@ __host__ __device__ __forceinline__ unsigned* plan_barrier_block(void* jsrc, con
 // inverse cube underflows to exactly 0 (ftz) -- they contribute 0 with or without the mass factor.
 constexpr float PAD_POS_F32 = 3.0e18f;
 constexpr double PAD_POS_F64 = 1.0e150;
+// The area of the unit rows also serves the flag-in-data whole-loop kernels (ll_kdk.cuh), which need no rows but two
+// buffers of tagged exchange words: at most 2 x 6 x 8 bytes per particle (fp64), for n up to LL_MAX_N.
+constexpr int LL_MAX_N = 6144;                    // upper bound of odisseo_set_ll_max_n; shared memory bounds it further
 __host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p) {
-    return (size_t)p.U * p.comps * p.IB * sizeof(double);
+    const size_t rows = (size_t)p.U * p.comps * p.IB * sizeof(double);
+    const size_t exchange = p.n <= LL_MAX_N ? (size_t)p.n * 96 : 0;
+    return rows > exchange ? rows : exchange;
 }
 
 #if defined(__CUDACC__)
@@ -383,5 +388,12 @@ cudaError_t launch_cluster_f32(const PairPlan& plan, float* posm, float* vel, fl
                                const PotParams<float>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream);
 cudaError_t launch_cluster_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
                                const PotParams<double>& pot, int64_t nsteps, int acc_valid, cudaStream_t stream);
+// flag-in-data whole-loop kernels (ll_kdk.cuh): owner-computes on all SMs, one L2 round trip per step
+size_t ll_fits_f32(const PairPlan& plan);         // bytes of exchange buffer needed, 0 = the call does not fit
+size_t ll_fits_f64(const PairPlan& plan);
+cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
+                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream);
+cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
+                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream);
 
 }  // namespace odisseo

@@ -22,6 +22,7 @@
 //   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
 #include "fused_step.cuh"
 #include "cluster_kdk.cuh"
+#include "ll_kdk.cuh"
 
 namespace odisseo {
 
@@ -154,6 +155,7 @@ typedef PairF32<1, 2, 1, 4> ClusterF32;      // the same loop, two targets per l
 
 int g_fused_max_ctas[2] = {0, 0};        // co-resident CTAs of the whole-loop kernel, [variant]
 int g_cluster_size = 0;                  // CTAs per cluster the device schedules for the cluster kernel (0 = none)
+int g_ll_max_ctas = 0;                   // co-resident CTAs of the flag-in-data whole-loop kernel (ll_kdk.cuh)
 
 }  // namespace
 
@@ -164,6 +166,7 @@ cudaError_t configure_pair_f32(int num_sms)
     if (e == cudaSuccess) e = configure_fused<LargeF32, float>(512, num_sms, &g_fused_max_ctas[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF32Fused, float>(256, num_sms, &g_fused_max_ctas[1]);
     if (e == cudaSuccess) e = configure_cluster<ClusterF32, float>(&g_cluster_size);
+    if (e == cudaSuccess) e = configure_ll<ClusterF32, float>(num_sms, &g_ll_max_ctas);
     return e;
 }
 
@@ -200,6 +203,30 @@ cudaError_t launch_cluster_f32(const PairPlan& plan, float* posm, float* vel, fl
     ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
     const size_t smem = cluster_geometry<float>(plan, g_cluster_size, &ca.tpc);
     return launch_cluster<ClusterF32, float>(ca, g_cluster_size, smem, stream);
+}
+
+// Flag-in-data whole-loop kernel (ll_kdk.cuh): bytes of the exchange buffer the call needs, 0 = the call does not fit.
+size_t ll_fits_f32(const PairPlan& plan)
+{
+    int32_t tpc, ctas;
+    size_t xbytes = 0;
+    return ll_geometry<float>(plan, g_ll_max_ctas, &tpc, &ctas, &xbytes) != 0 ? xbytes : 0;
+}
+
+cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
+                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream)
+{
+    LLArgs<float> ca;
+    ca.posm = reinterpret_cast<float4*>(posm); ca.vel = reinterpret_cast<float4*>(vel); ca.acc = reinterpret_cast<float4*>(acc);
+    ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
+    ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
+    ca.xbuf = static_cast<unsigned long long*>(xbuf);
+    int32_t ctas;
+    size_t xbytes;
+    const size_t smem = ll_geometry<float>(plan, g_ll_max_ctas, &ca.tpc, &ctas, &xbytes);
+    cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
+    if (e != cudaSuccess) return e;
+    return launch_ll<ClusterF32, float>(ca, ctas, smem, stream);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,

@@ -13,6 +13,7 @@
 // same fixed grouping as the fp32 kernel.
 #include "fused_step.cuh"
 #include "cluster_kdk.cuh"
+#include "ll_kdk.cuh"
 
 namespace odisseo {
 
@@ -140,6 +141,7 @@ typedef PairF64<2, 2, 1, 2, false> ClusterF64;   // the same loop inside the clu
 
 int g_fused_max_ctas64[2] = {0, 0};
 int g_cluster_size64 = 0;
+int g_ll_max_ctas64 = 0;
 
 }  // namespace
 
@@ -152,6 +154,7 @@ cudaError_t configure_pair_f64(int num_sms)
     if (e == cudaSuccess) e = configure_fused<LargeF64, double>(256, num_sms, &g_fused_max_ctas64[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF64Fused, double>(256, num_sms, &g_fused_max_ctas64[1]);
     if (e == cudaSuccess) e = configure_cluster<ClusterF64, double>(&g_cluster_size64);
+    if (e == cudaSuccess) e = configure_ll<ClusterF64, double>(num_sms, &g_ll_max_ctas64);
     return e;
 }
 
@@ -187,6 +190,29 @@ cudaError_t launch_cluster_f64(const PairPlan& plan, double* posm, double* vel, 
     ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
     const size_t smem = cluster_geometry<double>(plan, g_cluster_size64, &ca.tpc);
     return launch_cluster<ClusterF64, double>(ca, g_cluster_size64, smem, stream);
+}
+
+size_t ll_fits_f64(const PairPlan& plan)
+{
+    int32_t tpc, ctas;
+    size_t xbytes = 0;
+    return ll_geometry<double>(plan, g_ll_max_ctas64, &tpc, &ctas, &xbytes) != 0 ? xbytes : 0;
+}
+
+cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
+                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream)
+{
+    LLArgs<double> ca;
+    ca.posm = reinterpret_cast<double4*>(posm); ca.vel = reinterpret_cast<double4*>(vel); ca.acc = reinterpret_cast<double4*>(acc);
+    ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
+    ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
+    ca.xbuf = static_cast<unsigned long long*>(xbuf);
+    int32_t ctas;
+    size_t xbytes;
+    const size_t smem = ll_geometry<double>(plan, g_ll_max_ctas64, &ca.tpc, &ctas, &xbytes);
+    cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
+    if (e != cudaSuccess) return e;
+    return launch_ll<ClusterF64, double>(ca, ctas, smem, stream);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,

@@ -392,7 +392,8 @@ def test_whole_loop_kernel_is_bit_identical_to_the_per_step_launches(n, ci, dtyp
     p, v = posm64.astype(dtype), vel64.astype(dtype)
     pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
     old = B.set_fused_max_n(16384)
-    B.set_cluster_max_n(0)                                                        # the cluster kernel has its own test
+    B.set_cluster_max_n(0)                                                        # the other whole-loop kernels have their own tests
+    B.set_ll_max_n(0)
     try:
         fused = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, 7, pot, dtype)
         c0 = B.launch_count()
@@ -411,6 +412,7 @@ def test_whole_loop_kernel_is_bit_identical_to_the_per_step_launches(n, ci, dtyp
     finally:
         B.set_fused_max_n(-1)
         B.set_cluster_max_n(-1)
+        B.set_ll_max_n(-1)
     for a, b, c in zip(fused, plain, chained):
         assert a.tobytes() == b.tobytes() and a.tobytes() == c.tobytes()
 
@@ -430,6 +432,7 @@ def test_cluster_kernel_is_bit_identical_to_the_per_step_launches(n, ci, nsteps,
     p, v = posm64.astype(dtype), vel64.astype(dtype)
     pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
     B.set_fused_max_n(0)
+    B.set_ll_max_n(0)
     B.set_cluster_max_n(4096)
     try:
         clustered = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype)
@@ -451,7 +454,51 @@ def test_cluster_kernel_is_bit_identical_to_the_per_step_launches(n, ci, nsteps,
     finally:
         B.set_cluster_max_n(-1)
         B.set_fused_max_n(-1)
+        B.set_ll_max_n(-1)
     for a, b, c in zip(clustered, plain, chained):
+        assert a.tobytes() == b.tobytes() and a.tobytes() == c.tobytes()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n,ci,nsteps", [(1, 1, 3), (2, 0, 3), (3, 1, 1), (63, 0, 5), (65, 1, 5), (129, 1, 7), (1000, 0, 7), (1024, 0, 10),
+                                         (1025, 1, 4), (2047, 0, 3), (4096, 1, 3)])
+def test_flag_in_data_kernel_is_bit_identical_to_the_per_step_launches(n, ci, nsteps, dtype):
+    """Small N runs the whole call as one cooperative launch of the owner-computes kernel (csrc/ll_kdk.cuh: every CTA holds
+    all sources in shared memory and owns a few targets; moved positions are exchanged as {value, step tag} words that
+    every CTA polls).  It follows the canonical summation order, so state and acc must agree bit for bit with the
+    {pair, step} launch sequence -- with and without acc_valid, chained, equal and general masses, with and without
+    the external potential."""
+    cfg = W.CONFIGS[ci]
+    posm64, vel64 = W.make_state(cfg, n=n)
+    if n == 129:
+        posm64[7, 3] *= 1.5                                                      # general-mass loop
+    p, v = posm64.astype(dtype), vel64.astype(dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+    B.set_fused_max_n(0)
+    B.set_cluster_max_n(0)
+    B.set_ll_max_n(6144)
+    try:
+        ll = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype)
+        c0 = B.launch_count()
+        gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype)
+        assert B.launch_count() - c0 == 1                                         # one launch for the whole call
+        posm, vel = dev(p, dtype), dev(W.vel4(v, dtype), dtype)
+        acc = torch.empty_like(posm)
+        ws = B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64))
+        k1 = max(1, nsteps // 2)
+        B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, k1, pot, ws)
+        if nsteps > k1:
+            B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps - k1, pot, ws, acc_valid=True)
+        torch.cuda.synchronize()
+        chained = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
+        B.set_ll_max_n(0)
+        plain = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype)
+        assert B.launch_count() - c0 > 3
+    finally:
+        B.set_cluster_max_n(-1)
+        B.set_fused_max_n(-1)
+        B.set_ll_max_n(-1)
+    for a, b, c in zip(ll, plain, chained):
         assert a.tobytes() == b.tobytes() and a.tobytes() == c.tobytes()
 
 
