@@ -36,6 +36,10 @@ namespace odisseo {
 constexpr int LL_WARPS = ODISSEO_LL_WARPS;        // threads per CTA / 32, one CTA per SM
 constexpr int LL_THREADS = LL_WARPS * 32;
 constexpr int LL_SMEM_MAX = 226 * 1024;
+#ifndef ODISSEO_LL_LANES
+#define ODISSEO_LL_LANES 128
+#endif
+constexpr int LL_LANES = ODISSEO_LL_LANES;        // lanes of pair-phase work a CTA takes before the grid grows
 
 template <typename T> struct LLArgs {
     typename Vec4<T>::type *posm, *vel, *acc;
@@ -45,7 +49,7 @@ template <typename T> struct LLArgs {
     int32_t acc_valid;
     int32_t n, n8, S, Ttile;                      // the plan's source split (chunks of octets, tile length)
     int32_t tpc;                                  // targets owned per CTA (even)
-    unsigned long long* xbuf;                     // [2][n][LLWords<T>] tagged words, zeroed by the host before the launch
+    unsigned long long* xbuf;                     // [2][n rounded up to even][LLWords<T>] tagged words, zeroed by the host before the launch
 };
 
 template <typename T> struct LLWords { static constexpr int value = sizeof(T) == 4 ? 3 : 6; };
@@ -175,31 +179,37 @@ __device__ __forceinline__ void ll_fetch(const unsigned long long* rec, uint32_t
     z = __longlong_as_double((long long)((w[4] & 0xffffffffull) | (w[5] << 32)));
 }
 
-// two records at once: all loads of a round are issued before any tag is looked at
+__device__ __forceinline__ void ll_ld16(const unsigned long long* p, unsigned long long& a, unsigned long long& b)
+{
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+// Two consecutive records (2 W words, 16-byte aligned) polled with 16-byte loads: half the requests at the L2 lines
+// that every CTA polls.  Each 8-byte word still validates itself by its own tag, so it does not matter whether the
+// hardware performs a 16-byte access as one transaction.  second = false: only the first record exists.
 template <typename T>
-__device__ __forceinline__ void ll_fetch2(const unsigned long long* ra, const unsigned long long* rb, uint32_t tag, T& x, T& y, T& z,
-                                          T& x2, T& y2, T& z2)
+__device__ __forceinline__ void ll_fetch_pair(const unsigned long long* rec, const bool second, uint32_t tag, T& x, T& y, T& z, T& x2,
+                                              T& y2, T& z2)
 {
     constexpr int W = LLWords<T>::value;
-    unsigned long long a[W], b[W];
+    unsigned long long w[2 * W];
     bool ok;
     do {
 #pragma unroll
-        for (int k = 0; k < W; ++k) { a[k] = ll_ld(ra + k); b[k] = ll_ld(rb + k); }
+        for (int k = 0; k < W; ++k) ll_ld16(rec + 2 * k, w[2 * k], w[2 * k + 1]);
         ok = true;
 #pragma unroll
-        for (int k = 0; k < W; ++k) ok = ok && (uint32_t)(a[k] >> 32) == tag && (uint32_t)(b[k] >> 32) == tag;
+        for (int k = 0; k < 2 * W; ++k) ok = ok && ((uint32_t)(w[k] >> 32) == tag || (k >= W && !second));
     } while (!ok);
     if (sizeof(T) == 4) {
-        x = (T)__uint_as_float((uint32_t)a[0]); y = (T)__uint_as_float((uint32_t)a[1]); z = (T)__uint_as_float((uint32_t)a[2]);
-        x2 = (T)__uint_as_float((uint32_t)b[0]); y2 = (T)__uint_as_float((uint32_t)b[1]); z2 = (T)__uint_as_float((uint32_t)b[2]);
+        x = (T)__uint_as_float((uint32_t)w[0]); y = (T)__uint_as_float((uint32_t)w[1]); z = (T)__uint_as_float((uint32_t)w[2]);
+        x2 = (T)__uint_as_float((uint32_t)w[W]); y2 = (T)__uint_as_float((uint32_t)w[W + 1]); z2 = (T)__uint_as_float((uint32_t)w[W + 2]);
     } else {
-        x = (T)__longlong_as_double((long long)((a[0] & 0xffffffffull) | (a[1 % W] << 32)));
-        y = (T)__longlong_as_double((long long)((a[2] & 0xffffffffull) | (a[3 % W] << 32)));
-        z = (T)__longlong_as_double((long long)((a[4 % W] & 0xffffffffull) | (a[5 % W] << 32)));
-        x2 = (T)__longlong_as_double((long long)((b[0] & 0xffffffffull) | (b[1 % W] << 32)));
-        y2 = (T)__longlong_as_double((long long)((b[2] & 0xffffffffull) | (b[3 % W] << 32)));
-        z2 = (T)__longlong_as_double((long long)((b[4 % W] & 0xffffffffull) | (b[5 % W] << 32)));
+        x = (T)__longlong_as_double((long long)((w[0] & 0xffffffffull) | (w[1] << 32)));
+        y = (T)__longlong_as_double((long long)((w[2] & 0xffffffffull) | (w[3] << 32)));
+        z = (T)__longlong_as_double((long long)((w[4 % (2 * W)] & 0xffffffffull) | (w[5 % (2 * W)] << 32)));
+        x2 = (T)__longlong_as_double((long long)((w[W] & 0xffffffffull) | (w[W + 1] << 32)));
+        y2 = (T)__longlong_as_double((long long)((w[(W + 2) % (2 * W)] & 0xffffffffull) | (w[(W + 3) % (2 * W)] << 32)));
+        z2 = (T)__longlong_as_double((long long)((w[(W + 4) % (2 * W)] & 0xffffffffull) | (w[(W + 5) % (2 * W)] << 32)));
     }
 }
 
@@ -228,6 +238,7 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
     const double gm = (double)ca.G * (EQM ? m0 : 1.0);               // plan_row_mass(): the factor left out of the sums
     const T h = (T)0.5 * ca.dt;
     uint32_t pushes = 0;                                             // tag of the latest exchange
+    const size_t nbuf = ((size_t)n + 1) & ~(size_t)1;                // records per exchange buffer (16-byte aligned buffers)
 
     PairPlan fake;                                                   // State's constructor reads nt and IB only
     fake.nt = n; fake.IB = 2;
@@ -336,7 +347,7 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
                 if (open) {
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
                     p.x = fma(v.x, ca.dt, p.x); p.y = fma(v.y, ca.dt, p.y); p.z = fma(v.z, ca.dt, p.z);
-                    ll_publish(ca.xbuf + ((size_t)((pushes + 1) & 1u) * n + me) * WORDS, pushes + 1, p.x, p.y, p.z);
+                    ll_publish(ca.xbuf + ((size_t)((pushes + 1) & 1u) * nbuf + me) * WORDS, pushes + 1, p.x, p.y, p.z);
                 }
                 v.w = (T)0;
                 svel[tid] = v;
@@ -347,15 +358,13 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
             ++pushes;
             __syncthreads();                                         // the owners have read their old records
             LL_MARK(4);
-            const unsigned long long* buf = ca.xbuf + (size_t)(pushes & 1u) * n * WORDS;
-            // two records per thread in flight: their polls overlap (one L2 round trip, not two)
-            for (int32_t j = tid; j < n; j += 2 * LL_THREADS) {
-                const int32_t j2 = j + LL_THREADS;
-                T x, y, z, x2 = (T)0, y2 = (T)0, z2 = (T)0;
-                if (j2 < n) ll_fetch2(buf + (size_t)j * WORDS, buf + (size_t)j2 * WORDS, pushes, x, y, z, x2, y2, z2);
-                else ll_fetch(buf + (size_t)j * WORDS, pushes, x, y, z);
+            const unsigned long long* buf = ca.xbuf + (size_t)(pushes & 1u) * nbuf * WORDS;
+            for (int32_t j = 2 * tid; j < n; j += 2 * LL_THREADS) {   // two consecutive records per thread
+                const bool second = j + 1 < n;
+                T x, y, z, x2, y2, z2;
+                ll_fetch_pair(buf + (size_t)j * WORDS, second, pushes, x, y, z, x2, y2, z2);
                 ll_put_position(cur, j, chunk_of[j], x, y, z);
-                if (j2 < n) ll_put_position(cur, j2, chunk_of[j2], x2, y2, z2);
+                if (second) ll_put_position(cur, j + 1, chunk_of[j + 1], x2, y2, z2);
             }
             LL_MARK(5);
             __syncthreads();
@@ -442,10 +451,16 @@ template <class C, typename T> cudaError_t configure_ll(int num_sms, int* max_ct
 template <typename T> size_t ll_geometry(const PairPlan& plan, int max_ctas, int32_t* tpc, int32_t* ctas, size_t* xbuf_bytes)
 {
     if (max_ctas < 1) return 0;
+    // Few CTAs are better than many as long as a CTA's pair phase stays one warp per scheduler deep (its length is the
+    // chunk length either way): every CTA polls every record, and the polls of all CTAs queue at the same L2 lines.
     const int64_t pairs = (plan.n + 1) / 2;
-    *tpc = (int32_t)(2 * ((pairs + max_ctas - 1) / max_ctas));
+    int64_t per_cta = (pairs + max_ctas - 1) / max_ctas;             // what the co-resident grid forces
+    int64_t comfy = 1;                                               // largest power of two of pairs whose (pair, chunk)
+    while (2 * comfy * plan.S <= LL_LANES) comfy *= 2;               // lanes fit LL_LANES lanes (groups are powers of two)
+    if (per_cta < comfy) per_cta = comfy;
+    *tpc = (int32_t)(2 * per_cta);
     *ctas = (int32_t)((plan.n + *tpc - 1) / *tpc);
-    *xbuf_bytes = (size_t)2 * plan.n * LLWords<T>::value * sizeof(unsigned long long);
+    *xbuf_bytes = (size_t)2 * (((size_t)plan.n + 1) & ~(size_t)1) * LLWords<T>::value * sizeof(unsigned long long);
     if (*tpc > LL_THREADS) return 0;                                 // one owner thread per particle
     const LLSmem<T> L((int32_t)plan.n8, plan.S, *tpc);
     return L.total <= (size_t)LL_SMEM_MAX ? L.total : 0;

@@ -100,7 +100,7 @@ constexpr double PAD_POS_F64 = 1.0e150;
 constexpr int LL_MAX_N = 6144;                    // upper bound of odisseo_set_ll_max_n; shared memory bounds it further
 __host__ __device__ __forceinline__ size_t plan_partial_bytes(const PairPlan& p) {
     const size_t rows = (size_t)p.U * p.comps * p.IB * sizeof(double);
-    const size_t exchange = p.n <= LL_MAX_N ? (size_t)p.n * 96 : 0;
+    const size_t exchange = p.n <= LL_MAX_N ? (size_t)(p.n + 1) * 96 : 0;
     return rows > exchange ? rows : exchange;
 }
 

@@ -152,6 +152,7 @@ typedef PairF32<1, 2, 8, 4> SmallF32;    // 128 targets per CTA, up to 8 CTAs pe
 typedef PairF32<1, 2, 4, 4> SmallF32Fused;   // the same loop inside the whole-loop kernel, which also holds the reduce batch
 
 typedef PairF32<1, 2, 1, 4> ClusterF32;      // the same loop, two targets per lane, inside the cluster kernel (cluster_kdk.cuh)
+typedef PairF32<1, 2, 1, 8> LLF32;           // ... and inside the flag-in-data kernel (ll_kdk.cuh): one warp deep, so unrolled further
 
 int g_fused_max_ctas[2] = {0, 0};        // co-resident CTAs of the whole-loop kernel, [variant]
 int g_cluster_size = 0;                  // CTAs per cluster the device schedules for the cluster kernel (0 = none)
@@ -166,7 +167,7 @@ cudaError_t configure_pair_f32(int num_sms)
     if (e == cudaSuccess) e = configure_fused<LargeF32, float>(512, num_sms, &g_fused_max_ctas[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF32Fused, float>(256, num_sms, &g_fused_max_ctas[1]);
     if (e == cudaSuccess) e = configure_cluster<ClusterF32, float>(&g_cluster_size);
-    if (e == cudaSuccess) e = configure_ll<ClusterF32, float>(num_sms, &g_ll_max_ctas);
+    if (e == cudaSuccess) e = configure_ll<LLF32, float>(num_sms, &g_ll_max_ctas);
     return e;
 }
 
@@ -226,7 +227,7 @@ cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* 
     const size_t smem = ll_geometry<float>(plan, g_ll_max_ctas, &ca.tpc, &ctas, &xbytes);
     cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
     if (e != cudaSuccess) return e;
-    return launch_ll<ClusterF32, float>(ca, ctas, smem, stream);
+    return launch_ll<LLF32, float>(ca, ctas, smem, stream);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,

@@ -138,6 +138,7 @@ typedef PairF64<2, 2, 8, 2, true> SmallPot;
 typedef PairF64<2, 2, 4, 2, false> SmallF64Fused;
 
 typedef PairF64<2, 2, 1, 2, false> ClusterF64;   // the same loop inside the cluster kernel (cluster_kdk.cuh)
+typedef PairF64<2, 2, 1, 4, false> LLF64;        // ... and inside the flag-in-data kernel (ll_kdk.cuh)
 
 int g_fused_max_ctas64[2] = {0, 0};
 int g_cluster_size64 = 0;
@@ -154,7 +155,7 @@ cudaError_t configure_pair_f64(int num_sms)
     if (e == cudaSuccess) e = configure_fused<LargeF64, double>(256, num_sms, &g_fused_max_ctas64[0]);
     if (e == cudaSuccess) e = configure_fused<SmallF64Fused, double>(256, num_sms, &g_fused_max_ctas64[1]);
     if (e == cudaSuccess) e = configure_cluster<ClusterF64, double>(&g_cluster_size64);
-    if (e == cudaSuccess) e = configure_ll<ClusterF64, double>(num_sms, &g_ll_max_ctas64);
+    if (e == cudaSuccess) e = configure_ll<LLF64, double>(num_sms, &g_ll_max_ctas64);
     return e;
 }
 
@@ -212,7 +213,7 @@ cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, doubl
     const size_t smem = ll_geometry<double>(plan, g_ll_max_ctas64, &ca.tpc, &ctas, &xbytes);
     cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
     if (e != cudaSuccess) return e;
-    return launch_ll<ClusterF64, double>(ca, ctas, smem, stream);
+    return launch_ll<LLF64, double>(ca, ctas, smem, stream);
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
