@@ -103,9 +103,9 @@ int64_t odisseo_set_cluster_max_n(int64_t n);
  * polls (the flag travels with the data: no grid barrier, no fence, one L2 round trip per step).  Same summation
  * order, bit-identical to the other forms.  Default bounds: n <= 4,096 (fp32) / 2,048 (fp64).  This sets the largest n
  * served that way for both precisions (clamped to 6,144; the shared memory of a CTA bounds it further; 0 = never;
- * negative = restore the defaults) and returns the previous fp32 value: a tuning and test knob, process-wide.  Not
- * used with a tape, inside a stream capture or while a profile is open; when the device cannot hold the grid the
- * call falls back to the other forms. */
+ * negative = restore the defaults) and returns the previous fp32 value: a tuning and test knob, process-wide.  It
+ * also serves odisseo_leapfrog_kdk_tape_* (the owner threads store the snapshots).  Not used inside a stream capture
+ * or while a profile is open; when the device cannot hold the grid the call falls back to the other forms. */
 int64_t odisseo_set_ll_max_n(int64_t n);
 
 /* Releases what the library keeps between calls: the cached CUDA-graph executables of odisseo_leapfrog_kdk_* and the

@@ -276,11 +276,11 @@ inline cudaError_t launch_fused(const PairPlan& p, double* x, double* v, double*
 inline size_t ll_fits(float, const PairPlan& p) { return ll_fits_f32(p); }
 inline size_t ll_fits(double, const PairPlan& p) { return ll_fits_f64(p); }
 inline cudaError_t launch_ll(const PairPlan& p, float* x, float* v, float* a, float G, float eps, float dt, const PotParams<float>& pot,
-                             int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t s)
-{ return launch_ll_f32(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, s); }
+                             int64_t nsteps, int acc_valid, void* xbuf, float* tape, cudaStream_t s)
+{ return launch_ll_f32(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, tape, s); }
 inline cudaError_t launch_ll(const PairPlan& p, double* x, double* v, double* a, double G, double eps, double dt, const PotParams<double>& pot,
-                             int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t s)
-{ return launch_ll_f64(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, s); }
+                             int64_t nsteps, int acc_valid, void* xbuf, double* tape, cudaStream_t s)
+{ return launch_ll_f64(p, x, v, a, G, eps, dt, pot, nsteps, acc_valid, xbuf, tape, s); }
 inline bool cluster_fits(float, const PairPlan& p) { return cluster_fits_f32(p); }
 inline bool cluster_fits(double, const PairPlan& p) { return cluster_fits_f64(p); }
 inline cudaError_t launch_cluster(const PairPlan& p, float* x, float* v, float* a, float G, float eps, float dt, const PotParams<float>& pot,
@@ -550,10 +550,12 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     // Small N, first choice: the whole call as ONE cooperative launch of the owner-computes kernel (ll_kdk.cuh): every CTA
     // holds all sources in shared memory and integrates its own few targets; the moved positions travel as {value, step
     // tag} words through the (otherwise unused) partial-row area of the workspace -- one L2 round trip per step.
-    if (one_launch_ok && n <= g_ll_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && nsteps < (int64_t)0x7fffffff) {
+    // (it also writes the reverse mode's tape: the owner threads store the snapshots)
+    if ((one_launch_ok || (tape && nsteps >= 1 && cap == cudaStreamCaptureStatusNone && !g_prof.active)) &&
+        n <= g_ll_max_n[sizeof(T) == 8].load(std::memory_order_relaxed) && nsteps < (int64_t)0x7fffffff) {
         const size_t xbytes = ll_fits(T(), plan);
         if (xbytes != 0 && xbytes <= plan_partial_bytes(plan)) {
-            if (launch_ll(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, cv.partials, s) == cudaSuccess) {
+            if (launch_ll(plan, posm, vel, acc, G, eps, dt, pp, nsteps, acc_valid, cv.partials, tape, s) == cudaSuccess) {
                 g_launches.fetch_add(1, std::memory_order_relaxed);
                 return ODISSEO_OK;
             }

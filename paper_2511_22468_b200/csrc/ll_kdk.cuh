@@ -50,6 +50,7 @@ template <typename T> struct LLArgs {
     int32_t n, n8, S, Ttile;                      // the plan's source split (chunks of octets, tile length)
     int32_t tpc;                                  // targets owned per CTA (even)
     unsigned long long* xbuf;                     // [2][n rounded up to even][LLWords<T>] tagged words, zeroed by the host before the launch
+    typename Vec4<T>::type* tape;                 // reverse mode's tape of nsteps + 1 snapshots {x_k, v_k, pair-only a_k}, or null
 };
 
 template <typename T> struct LLWords { static constexpr int value = sizeof(T) == 4 ? 3 : 6; };
@@ -344,6 +345,15 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
                 const T tx = a.x + ex, ty = a.y + ey, tz = a.z + ez;
                 V4 v = svel[tid];
                 if (close) { v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z); }
+                if (ca.tape) {
+                    // the synchronised state between the closing kick of step k - 1 and the opening kick of step k
+                    // (step_body.cuh's snapshot); k = pushes: one snapshot per integrate call
+                    V4* snap = ca.tape + (size_t)pushes * 3 * n;
+                    V4 vs = v; vs.w = (T)0;
+                    snap[me] = p;
+                    snap[n + me] = vs;
+                    snap[2 * (size_t)n + me] = a;
+                }
                 if (open) {
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
                     p.x = fma(v.x, ca.dt, p.x); p.y = fma(v.y, ca.dt, p.y); p.z = fma(v.z, ca.dt, p.z);

@@ -392,8 +392,8 @@ cudaError_t launch_cluster_f64(const PairPlan& plan, double* posm, double* vel, 
 size_t ll_fits_f32(const PairPlan& plan);         // bytes of exchange buffer needed, 0 = the call does not fit
 size_t ll_fits_f64(const PairPlan& plan);
 cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
-                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream);
+                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, float* tape, cudaStream_t stream);
 cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
-                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream);
+                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, double* tape, cudaStream_t stream);
 
 }  // namespace odisseo

@@ -215,13 +215,14 @@ size_t ll_fits_f32(const PairPlan& plan)
 }
 
 cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* acc, float G, float eps, float dt,
-                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream)
+                          const PotParams<float>& pot, int64_t nsteps, int acc_valid, void* xbuf, float* tape, cudaStream_t stream)
 {
     LLArgs<float> ca;
     ca.posm = reinterpret_cast<float4*>(posm); ca.vel = reinterpret_cast<float4*>(vel); ca.acc = reinterpret_cast<float4*>(acc);
     ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
     ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
     ca.xbuf = static_cast<unsigned long long*>(xbuf);
+    ca.tape = reinterpret_cast<float4*>(tape);
     int32_t ctas;
     size_t xbytes;
     const size_t smem = ll_geometry<float>(plan, g_ll_max_ctas, &ca.tpc, &ctas, &xbytes);

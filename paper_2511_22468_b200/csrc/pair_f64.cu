@@ -201,13 +201,14 @@ size_t ll_fits_f64(const PairPlan& plan)
 }
 
 cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, double* acc, double G, double eps, double dt,
-                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, cudaStream_t stream)
+                          const PotParams<double>& pot, int64_t nsteps, int acc_valid, void* xbuf, double* tape, cudaStream_t stream)
 {
     LLArgs<double> ca;
     ca.posm = reinterpret_cast<double4*>(posm); ca.vel = reinterpret_cast<double4*>(vel); ca.acc = reinterpret_cast<double4*>(acc);
     ca.G = G; ca.eps2 = eps * eps; ca.dt = dt; ca.pot = pot; ca.nsteps = nsteps; ca.acc_valid = acc_valid;
     ca.n = (int32_t)plan.n; ca.n8 = (int32_t)plan.n8; ca.S = plan.S; ca.Ttile = plan.T;
     ca.xbuf = static_cast<unsigned long long*>(xbuf);
+    ca.tape = reinterpret_cast<double4*>(tape);
     int32_t ctas;
     size_t xbytes;
     const size_t smem = ll_geometry<double>(plan, g_ll_max_ctas64, &ca.tpc, &ctas, &xbytes);

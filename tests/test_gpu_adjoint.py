@@ -117,6 +117,33 @@ def test_accel_vjp_without_potential_and_reproducible():
     assert np.all(a[2][:5] == 0)
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n,nsteps,unequal", [(1, 2, False), (129, 4, True), (1000, 6, False), (2048, 3, False)])
+def test_tape_of_the_flag_in_data_kernel_equals_the_per_step_tape(n, nsteps, unequal, dtype):
+    """At small n the forward pass with a tape is ONE launch of the owner-computes kernel (csrc/ll_kdk.cuh), whose owner
+    threads store the snapshots {x_k, v_k, pair-only a_k}; tape and final state must equal the per-step launches' bit for bit."""
+    cfg, p, v, _, G, eps = _inputs(n, 40 + n, dtype, unequal=unequal)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    dt = float(np.float32(cfg.dt)) if dtype == np.float32 else cfg.dt
+    out = []
+    try:
+        for ll in (6144, 0):
+            B.set_ll_max_n(ll)
+            posm, vel = dev(p, dtype), dev(W.vel4(v, dtype), dtype)
+            acc = torch.empty_like(posm)
+            ws = B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64))
+            tape = torch.full((B.tape_bytes(n, nsteps, dtype == np.float64) // posm.element_size(),), float("nan"), dtype=posm.dtype, device="cuda")
+            c0 = B.launch_count()
+            B.leapfrog_kdk_tape(posm, vel, acc, G, eps, dt, nsteps, pot, tape, ws)
+            torch.cuda.synchronize()
+            assert (B.launch_count() - c0 == 1) == (ll != 0)
+            out.append((tape.cpu().numpy(), posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy()))
+    finally:
+        B.set_ll_max_n(-1)
+    for a, b in zip(*out):
+        assert a.tobytes() == b.tobytes()
+
+
 def gpu_leapfrog_vjp(p, v, G, eps, dt, nsteps, pot, lx, lv, dtype):
     n = p.shape[0]
     posm, vel = dev(p, dtype), dev(W.vel4(v, dtype), dtype)
