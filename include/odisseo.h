@@ -116,7 +116,8 @@ int64_t odisseo_set_ll_max_n(int64_t n);
 odisseo_status odisseo_shutdown(void);
 
 /* Upper bound, in bytes, of the device scratch any pair/leapfrog call on n particles
- * needs (staged source records + one row of fixed-order partial sums per work unit).
+ * needs (staged source records + one row of fixed-order partial sums per work unit; for n <= 6,144 the row area
+ * is at least 96 (n + 1) bytes, the exchange words of the small-n whole-loop kernel).
  * is_f64 != 0 for the fp64 calls.  Returns 0 for n <= 0.  With a current CUDA device the
  * bound is the one for that device's SM count; without one (no GPU) it is the maximum over
  * devices with 64..192 SMs.  Host arithmetic only. */
