@@ -600,3 +600,36 @@ def test_kick_drift_composes_to_the_leapfrog_bitwise(dtype):
         assert got.cpu().numpy().tobytes() == want.tobytes()
     with pytest.raises(B.OdisseoError, match="ERR_ARG"):
         B.kick_drift(posm, vel, acc, cfg.G, cfg.dt, pot, 0, ws)
+
+
+def test_flag_in_data_kernel_random_sizes_steps_and_splits():
+    """Sixty seeded random cases (n = 1 ... 4,096, 1 ... 40 steps, both precisions, with / without the potential, an odd
+    mass now and then, the call cut in two at a random step): the one-launch form and the per-step launches agree bit for
+    bit.  Guards the two-buffer exchange of csrc/ll_kdk.cuh (a CTA that runs ahead must never overwrite a record another
+    CTA still waits for)."""
+    rng = np.random.default_rng(2511)
+    try:
+        for _ in range(60):
+            dtype = np.float32 if rng.random() < 0.6 else np.float64
+            top = 4097 if dtype == np.float32 else 2049
+            n = int(rng.choice([rng.integers(1, 64), rng.integers(64, 1100), rng.integers(1100, top)]))
+            nsteps = int(rng.integers(1, 41))
+            cfg = W.CONFIGS[int(rng.integers(0, 2))]
+            posm64, vel64 = W.make_state(cfg, n=n, seed=int(rng.integers(1, 10 ** 6)))
+            if n > 3 and rng.random() < 0.3:
+                posm64[int(rng.integers(0, n)), 3] *= 1.7
+            p, v = posm64.astype(dtype), vel64.astype(dtype)
+            pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn) if cfg.nfw else None
+            k1 = int(rng.integers(1, nsteps + 1))
+            B.set_fused_max_n(0)
+            B.set_cluster_max_n(0)
+            B.set_ll_max_n(6144)
+            one = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype, chunks=[k1] + ([nsteps - k1] if nsteps > k1 else []))
+            B.set_ll_max_n(0)
+            ref = gpu_leapfrog(p, v, cfg.G, cfg.eps, cfg.dt, nsteps, pot, dtype)
+            for a, b in zip(one, ref):
+                assert a.tobytes() == b.tobytes(), (dtype.__name__, n, nsteps, k1)
+    finally:
+        B.set_ll_max_n(-1)
+        B.set_cluster_max_n(-1)
+        B.set_fused_max_n(-1)
