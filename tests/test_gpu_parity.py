@@ -133,6 +133,20 @@ def test_pair_f64_config0_full():
     assert pair_ratio(acc, posm64, cfg.G, cfg.eps) <= TOL_F64
 
 
+def test_pair_beyond_the_baseline_sizes_ragged_two_million():
+    """Twice the largest BASELINE size plus a ragged tail (N = 2^21 + 5, config 4's shape, fp32): 4.4e12 interactions in
+    one evaluation, checked on 1,024 seeded targets against all sources (index arithmetic and workspace sizes past 2^31
+    bytes of rows and 2^42 interactions)."""
+    cfg = W.CONFIGS[4]
+    n = (1 << 21) + 5
+    posm64, _ = W.make_state(cfg, n=n)
+    p, p64, G, eps = f32_inputs(posm64, cfg.G, cfg.eps)
+    acc = gpu_pair(p, G, eps, np.float32)
+    assert np.all(np.isfinite(acc))
+    idx = W.target_subset(n, size=1024)
+    assert pair_ratio(acc, p64, G, eps, targets=idx) <= TOL_F32
+
+
 @pytest.mark.parametrize("ci,dtype", [(2, np.float32), (3, np.float32), (3, np.float64), (4, np.float32)])
 def test_pair_full_size_on_seeded_target_subset(ci, dtype):
     """BASELINE.json full sizes in the launch configuration bench.py times; the oracle
