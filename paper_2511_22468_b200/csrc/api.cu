@@ -67,7 +67,7 @@ PairPlan make_cross_plan(int64_t nt, int64_t n, int is_f64, int num_sms)
     const VariantGeom g = variant_geom(p.variant, is_f64);
     p.ipt = g.ipt;
     p.cthreads = g.cthreads;
-    p.rec_bytes = 32;
+    p.rec_bytes = is_f64 ? 32 : 16;                       // staged records are plain {x, y, z, m}
     p.comps = 3;
     p.IB = p.ipt * p.cthreads;
     p.nb = (int32_t)((nt + p.IB - 1) / p.IB);

@@ -49,22 +49,21 @@ template <typename T> struct ClusterArgs {
 };
 
 // Shared-memory carve (bytes), identical on the host and on the device.
-//   fp32: cur = 8 n8 expanded records {x,x,y,y},{z,z,m,m}; raw[2] = n float4 {x,y,z,m} each (the pushed form)
-//   fp64: cur[2] = 8 n8 double4 records each (pushed as they are)
-//   part  = (tpc / 64) S items x 3 planes x 64 doubles;  svel, sacc = tpc records each
+//   cur[2] = 8 n8 staged records {x, y, z, m} each (pushed as they are; fp32 16 B, fp64 32 B per record)
+//   part   = (tpc / 64) S items x 3 planes x 64 doubles;  svel, sacc = tpc records each
 template <typename T> struct ClusterSmem {
-    size_t cur, raw, part, svel, sacc, total;
+    size_t cur, part, svel, sacc, total;
     __host__ __device__ ClusterSmem(int32_t n, int32_t n8, int32_t S, int32_t tpc)
     {
         const size_t npad = (size_t)8 * n8;
-        const size_t nrec = ((size_t)n + 7) & ~(size_t)7;
         size_t off = 0;
-        cur = off; off += sizeof(T) == 4 ? npad * 32 : 2 * npad * 32;
-        raw = off; off += sizeof(T) == 4 ? 2 * nrec * 16 : 0;
+        cur = off; off += 2 * npad * 4 * sizeof(T);
+        off = (off + 127) & ~(size_t)127;
         part = off; off += (size_t)(tpc / CLUSTER_GROUP) * S * 3 * CLUSTER_GROUP * sizeof(double);
         svel = off; off += (size_t)tpc * 4 * sizeof(T);
         sacc = off; off += (size_t)tpc * 4 * sizeof(T);
         total = off;
+        (void)n;
     }
 };
 
@@ -113,16 +112,13 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int32_t n = ca.n, S = ca.S;
     const ClusterSmem<T> L(n, ca.n8, S, ca.tpc);
-    const size_t npad = (size_t)8 * ca.n8, nrec = ((size_t)n + 7) & ~(size_t)7;
+    const size_t npad = (size_t)8 * ca.n8;
     double* const part = reinterpret_cast<double*>(smem + L.part);
     V4* const svel = reinterpret_cast<V4*>(smem + L.svel);
     V4* const sacc = reinterpret_cast<V4*>(smem + L.sacc);
-    // the {x, y, z, m} records of buffer b (fp32: the pushed form; fp64: the staged records themselves)
-    auto records = [&](int b) -> V4* {
-        return reinterpret_cast<V4*>(smem + (sizeof(T) == 4 ? L.raw + (size_t)b * nrec * 16 : L.cur + (size_t)b * npad * 32));
-    };
-    // what the pair loop reads in buffer b
-    auto staged = [&](int b) -> const unsigned char* { return smem + L.cur + (sizeof(T) == 4 ? 0 : (size_t)b * npad * 32); };
+    // the staged {x, y, z, m} records of buffer b: what the pair loop reads and what the owners push
+    auto records = [&](int b) -> V4* { return reinterpret_cast<V4*>(smem + L.cur) + (size_t)b * npad; };
+    auto staged = [&](int b) -> const unsigned char* { return reinterpret_cast<const unsigned char*>(records(b)); };
 
     const int32_t lo = (int32_t)rank * ca.tpc;                       // this CTA owns the particles [lo, lo + owned)
     const int32_t owned = lo >= n ? 0 : (n - lo < ca.tpc ? n - lo : ca.tpc);
@@ -140,19 +136,6 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
     fake.nt = n; fake.IB = CLUSTER_GROUP;
     const typename C::Params prm{nullptr, ca.eps2};
 
-    // fp32: raw[cb] -> the expanded records the packed loop reads ({x,x,y,y},{z,z,m,m}); fp64 reads the records as pushed
-    auto expand = [&]() {
-        if (sizeof(T) == 4) {
-            const float4* src = reinterpret_cast<const float4*>(records(cb));
-            float4* dst = reinterpret_cast<float4*>(smem + L.cur);
-            // one 16-byte word per thread: neighbouring lanes write neighbouring words (no bank conflicts)
-            for (int32_t w = tid; w < 2 * n; w += CLUSTER_THREADS) {
-                const float4 r = src[w >> 1];
-                dst[w] = (w & 1) ? make_float4(r.z, r.z, r.w, r.w) : make_float4(r.x, r.x, r.y, r.y);
-            }
-        }
-        __syncthreads();
-    };
     // chunk sums of the owned targets: item = (group of 64 targets, chunk s) per warp, two targets per lane
     auto pair_phase = [&]() {
         typename C::template State<EQM> st(prm, fake, nullptr);
@@ -168,7 +151,7 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
             double sum[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             for (int64_t j = 8 * (((int64_t)s * ca.n8) / S); j < j1; j += ca.Ttile) {
                 const int64_t left = j1 - j;
-                st.tile(src + (size_t)j * 32, (int)(left < ca.Ttile ? left : ca.Ttile));
+                st.tile(src + (size_t)j * sizeof(V4), (int)(left < ca.Ttile ? left : ca.Ttile));
                 st.take_sums(sum);                                   // second level: tile sums promoted to fp64
             }
             double* out = part + (size_t)item * 3 * CLUSTER_GROUP + lane;
@@ -239,7 +222,7 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
             inbox_phase[nb] ^= 1u;
             if (tid == 0) mbar_arrive_expect_tx(&inbox[nb], incoming);   // arm the next use of this buffer (two steps on)
             cb = nb;
-            expand();
+            __syncthreads();
         }
     };
 
@@ -251,7 +234,7 @@ __device__ __forceinline__ void cluster_kdk_loop(const ClusterArgs<T>& ca, unsig
         mbar_arrive_expect_tx(&inbox[0], incoming);
         mbar_arrive_expect_tx(&inbox[1], incoming);
     }
-    expand();                                                        // buffer 0 was filled from global memory by the caller
+    __syncthreads();                                                 // buffer 0 was filled from global memory by the caller
     // ---- the KDK loop of odisseo_leapfrog_kdk_* (api.cu leapfrog_impl), nsteps >= 1 ------------------------------------
     if (!ca.acc_valid) pair_phase();
     integrate(!ca.acc_valid, false, true);
@@ -285,11 +268,11 @@ cluster_kdk_kernel(const ClusterArgs<T> ca)
     const ClusterSmem<T> L(ca.n, ca.n8, ca.S, ca.tpc);
     const size_t npad = (size_t)8 * ca.n8;
 
-    // every CTA reads all n records from global memory into buffer 0, pads the staged tails (both fp64 buffers) and
+    // every CTA reads all n records from global memory into buffer 0, pads the staged tails (both buffers) and
     // decides "all masses equal" for itself (the same answer everywhere)
     const T mass0 = reinterpret_cast<const T*>(ca.posm)[3];
     int differs = 0;
-    V4* rec0 = reinterpret_cast<V4*>(smem_raw + (sizeof(T) == 4 ? L.raw : L.cur));
+    V4* rec0 = reinterpret_cast<V4*>(smem_raw + L.cur);
     for (int32_t j = tid; j < ca.n; j += CLUSTER_THREADS) {
         const V4 p = ca.posm[j];
         differs |= !(p.w == mass0);                                  // NaN counts as different
@@ -297,14 +280,8 @@ cluster_kdk_kernel(const ClusterArgs<T> ca)
     }
     const T far = pad_pos((T)0);
     for (size_t j = (size_t)ca.n + tid; j < npad; j += CLUSTER_THREADS) {
-        if (sizeof(T) == 4) {
-            float4* dst = reinterpret_cast<float4*>(smem_raw + L.cur);
-            dst[2 * j] = make_float4((float)far, (float)far, (float)far, (float)far);
-            dst[2 * j + 1] = make_float4((float)far, (float)far, 0.0f, 0.0f);
-        } else {
-            double4* dst = reinterpret_cast<double4*>(smem_raw + L.cur);
-            dst[j] = dst[npad + j] = make_double4((double)far, (double)far, (double)far, 0.0);
-        }
+        V4 pad; pad.x = far; pad.y = far; pad.z = far; pad.w = (T)0;
+        rec0[j] = rec0[npad + j] = pad;
     }
     const bool eqm = __syncthreads_or(differs) == 0;
     cluster_barrier();                         // every CTA is running and its inbox barriers are initialised: pushes may start

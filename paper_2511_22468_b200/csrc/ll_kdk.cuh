@@ -62,7 +62,7 @@ template <typename T> struct LLSmem {
     __host__ __device__ LLSmem(int32_t n8, int32_t S, int32_t tpc)
     {
         size_t off = 0;
-        cur = off; off += (size_t)8 * n8 * 32 + (size_t)LLSkew<T>::value * S;
+        cur = off; off += (size_t)8 * n8 * 4 * sizeof(T) + (size_t)LLSkew<T>::value * S;
         chunk = off; off += (size_t)8 * n8 * sizeof(uint16_t);          // chunk index of every staged record
         off = (off + 127) & ~(size_t)127;
         part = off; off += (size_t)(tpc / 2) * S * 6 * sizeof(double);
@@ -89,12 +89,10 @@ __device__ __forceinline__ int32_t ll_chunk_of(int32_t j, int32_t n8, int32_t S)
     const int32_t s = (int32_t)((((int64_t)oct + 1) * S + n8 - 1) / n8) - 1;
     return s < S - 1 ? s : S - 1;
 }
-// staged record j of chunk s in the skewed array -> {x, y, z, m}
+// staged record j of chunk s in the skewed array ({x, y, z, m}; fp32 16 B, fp64 32 B per record)
 __device__ __forceinline__ float4 ll_record(const unsigned char* cur, int32_t j, int32_t s, float)
 {
-    const float4* w = reinterpret_cast<const float4*>(cur + (size_t)32 * j + (size_t)16 * s);
-    const float4 A = w[0], B = w[1];
-    return make_float4(A.x, A.z, B.x, B.z);
+    return *reinterpret_cast<const float4*>(cur + (size_t)16 * j + (size_t)16 * s);
 }
 __device__ __forceinline__ double4 ll_record(const unsigned char* cur, int32_t j, int32_t s, double)
 {
@@ -102,24 +100,19 @@ __device__ __forceinline__ double4 ll_record(const unsigned char* cur, int32_t j
     const double2 A = w[0], B = w[1];
     return make_double4(A.x, A.y, B.x, B.y);
 }
-__device__ __forceinline__ float4 ll_record_at(const unsigned char* rec, float)
-{
-    const float4* w = reinterpret_cast<const float4*>(rec);
-    const float4 A = w[0], B = w[1];
-    return make_float4(A.x, A.z, B.x, B.z);
-}
+__device__ __forceinline__ float4 ll_record_at(const unsigned char* rec, float) { return *reinterpret_cast<const float4*>(rec); }
 __device__ __forceinline__ double4 ll_record_at(const unsigned char* rec, double)
 {
     const double2* w = reinterpret_cast<const double2*>(rec);
     const double2 A = w[0], B = w[1];
     return make_double4(A.x, A.y, B.x, B.y);
 }
-// (re)write the position of staged record j; the mass words stay
+// (re)write the position of staged record j; the mass word stays
 __device__ __forceinline__ void ll_put_position(unsigned char* cur, int32_t j, int32_t s, float x, float y, float z)
 {
-    float4* w = reinterpret_cast<float4*>(cur + (size_t)32 * j + (size_t)16 * s);
-    w[0] = make_float4(x, x, y, y);
-    *reinterpret_cast<float2*>(w + 1) = make_float2(z, z);
+    float* w = reinterpret_cast<float*>(cur + (size_t)16 * j + (size_t)16 * s);
+    *reinterpret_cast<float2*>(w) = make_float2(x, y);
+    w[2] = z;
 }
 __device__ __forceinline__ void ll_put_position(unsigned char* cur, int32_t j, int32_t s, double x, double y, double z)
 {
@@ -129,7 +122,7 @@ __device__ __forceinline__ void ll_put_position(unsigned char* cur, int32_t j, i
 }
 __device__ __forceinline__ void ll_put_mass(unsigned char* cur, int32_t j, int32_t s, float m)
 {
-    reinterpret_cast<float2*>(cur + (size_t)32 * j + (size_t)16 * s)[3] = make_float2(m, m);
+    reinterpret_cast<float*>(cur + (size_t)16 * j + (size_t)16 * s)[3] = m;
 }
 __device__ __forceinline__ void ll_put_mass(unsigned char* cur, int32_t j, int32_t s, double m)
 {
@@ -222,6 +215,7 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
     typedef typename Vec4<T>::type V4;
     constexpr int WORDS = LLWords<T>::value;
     constexpr int SKEW = LLSkew<T>::value;
+    constexpr int REC = 4 * (int)sizeof(T);                          // bytes per staged record {x, y, z, m}
     const int tid = threadIdx.x;
     const int32_t n = ca.n, n8 = ca.n8, S = ca.S;
     const LLSmem<T> L(n8, S, ca.tpc);
@@ -274,11 +268,11 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
         if (sc >= S || p >= npairs) return it;
         int32_t i0 = lo + 2 * p, i1 = i0 + 1;
         i1 = i1 < n ? i1 : n - 1;                                    // an odd tail pairs the last target with itself
-        it.t0 = 32 * i0 + SKEW * (int32_t)chunk_of[i0];
-        it.t1 = 32 * i1 + SKEW * (int32_t)chunk_of[i1];
+        it.t0 = REC * i0 + SKEW * (int32_t)chunk_of[i0];
+        it.t1 = REC * i1 + SKEW * (int32_t)chunk_of[i1];
         const int32_t j0 = 8 * (int32_t)(((uint32_t)sc * (uint32_t)n8) / (uint32_t)S);
         const int32_t j1 = 8 * (int32_t)(((uint32_t)(sc + 1) * (uint32_t)n8) / (uint32_t)S);
-        it.src = 32 * j0 + SKEW * sc;
+        it.src = REC * j0 + SKEW * sc;
         it.len = j1 - j0;
         it.out = (p * S + sc) * 6;
         return it;
@@ -295,7 +289,7 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
                 double sum[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
                 for (int32_t j = 0; j < it.len; j += ca.Ttile) {
                     const int32_t left = it.len - j;
-                    st.tile(cur + it.src + (size_t)32 * j, left < ca.Ttile ? left : ca.Ttile);
+                    st.tile(cur + it.src + (size_t)REC * j, left < ca.Ttile ? left : ca.Ttile);
                     st.take_sums(sum);                               // second level: tile sums promoted to fp64
                 }
                 double* out = part + it.out;

@@ -140,8 +140,8 @@ __device__ __forceinline__ double plan_row_mass(const void* __restrict__ jsrc, c
 {
     // both loads are issued unconditionally (no dependent round trip: at small N the reduce is latency-bound)
     const int eqm = __ldcg(plan_eqm_word(jsrc, plan));
-    // mass of staged record 0: fp32 records are {x,x,y,y},{z,z,m,m}; fp64 records {x,y,z,m}
-    const double m0 = sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 6) : __ldcg(static_cast<const double*>(jsrc) + 3);
+    // mass of staged record 0 ({x, y, z, m} in both precisions)
+    const double m0 = sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 3) : __ldcg(static_cast<const double*>(jsrc) + 3);
     return eqm != 0 ? m0 : 1.0;
 }
 #endif

@@ -30,7 +30,7 @@ namespace {
 
 template <int NPAIR, int CWARPS_, int MINB_, int JUNROLL>
 struct PairF32 {
-    static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 32, COMPS = 3;
+    static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 16, COMPS = 3;
     static constexpr int CTHREADS = CWARPS * 32;
     struct Params { const float4* posm; float eps2; };
     static size_t outer_bytes() { return (size_t)6 * NPAIR * CTHREADS * sizeof(double); }
@@ -80,16 +80,18 @@ struct PairF32 {
         }
         __device__ __forceinline__ void tile(const unsigned char* tile_raw, const int len)
         {
-            const ulonglong2* __restrict__ t = reinterpret_cast<const ulonglong2*>(tile_raw);
+            const float4* __restrict__ t = reinterpret_cast<const float4*>(tile_raw);
 #pragma unroll JUNROLL
             for (int j = 0; j < len; ++j) {
-                const ulonglong2 A = t[2 * j];        // {x,x},{y,y}
-                const ulonglong2 B = t[2 * j + 1];    // {z,z},{m,m}
+                // one LDS.128 per source; the splats below cost nothing: ptxas feeds the scalar register to the packed
+                // instruction as a broadcast operand (FADD2 R, Rj.F32, -Ri.F32x2) -- no MOV, no pre-duplicated staging
+                const float4 q = t[j];
+                const f32x2 qx = pk(q.x, q.x), qy = pk(q.y, q.y), qz = pk(q.z, q.z), qm = pk(q.w, q.w);
 #pragma unroll
                 for (int p = 0; p < NPAIR; ++p) {
-                    const f32x2 dx = sub2(A.x, xi[p]);
-                    const f32x2 dy = sub2(A.y, yi[p]);
-                    const f32x2 dz = sub2(B.x, zi[p]);
+                    const f32x2 dx = sub2(qx, xi[p]);
+                    const f32x2 dy = sub2(qy, yi[p]);
+                    const f32x2 dz = sub2(qz, zi[p]);
                     f32x2 r2 = fma2(dx, dx, e2);
                     r2 = fma2(dy, dy, r2);
                     r2 = fma2(dz, dz, r2);
@@ -97,7 +99,7 @@ struct PairF32 {
                     unpk(r2, r2l, r2h);
                     const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
                     const f32x2 ri2 = mul2(ri, ri);
-                    const f32x2 w = mul2(ri2, EQM ? ri : mul2(B.y, ri));
+                    const f32x2 w = mul2(ri2, EQM ? ri : mul2(qm, ri));
                     ax[p] = fma2(w, dx, ax[p]);
                     ay[p] = fma2(w, dy, ay[p]);
                     az[p] = fma2(w, dz, az[p]);

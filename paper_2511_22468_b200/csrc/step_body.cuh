@@ -20,14 +20,12 @@ template <typename T> struct Vec4;
 template <> struct Vec4<float> { typedef float4 type; };
 template <> struct Vec4<double> { typedef double4 type; };
 
-// Staged source record writers.  fp32: {x,x,y,y},{z,z,m,m} (pre-duplicated packed operands);
-// fp64: plain {x,y,z,m}.  Records [n, n_pad) are massless padding parked far away
-// (odisseo_common.cuh PAD_POS_*).
+// Staged source record writers: plain {x, y, z, m} in both precisions (fp32 16 B, fp64 32 B).  The packed fp32 loops
+// take the source coordinate as a scalar operand broadcast to both halves (SASS FADD2 R, Rj.F32, -Ri.F32x2), so nothing
+// is pre-duplicated.  Records [n, n_pad) are massless padding parked far away (odisseo_common.cuh PAD_POS_*).
 __device__ __forceinline__ void stage_record(void* jsrc, int64_t i, float x, float y, float z, float m)
 {
-    float4* out = reinterpret_cast<float4*>(jsrc) + 2 * i;
-    out[0] = make_float4(x, x, y, y);
-    out[1] = make_float4(z, z, m, m);
+    reinterpret_cast<float4*>(jsrc)[i] = make_float4(x, y, z, m);
 }
 __device__ __forceinline__ void stage_record(void* jsrc, int64_t i, double x, double y, double z, double m)
 {

@@ -47,7 +47,8 @@ def test_workspace_bytes_is_monotone_and_bounds_every_plan(lib):
                 p = B.describe_plan(n, f64, sms)
                 ib = p["i_bodies_per_thread"] * (p["threads_per_cta"] - 32)
                 npad = 8 * -(-n // 8)
-                need = (((-(-npad // 256) + 1) * 4 + 255) // 256) * 256 + (npad + 1024) * 32 + p["partial_rows"] * 3 * ib * 8
+                rec = 32 if f64 else 16                                      # staged records are plain {x, y, z, m}
+                need = (((-(-npad // 256) + 1) * 4 + 255) // 256) * 256 + (npad + 1024) * rec + p["partial_rows"] * 3 * ib * 8
                 assert need <= w, (n, f64, sms)
         assert B.workspace_bytes(n) >= prev
         prev = B.workspace_bytes(n)
