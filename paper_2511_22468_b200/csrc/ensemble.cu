@@ -9,9 +9,9 @@
 //   * positions, velocities and masses of a thread's targets live in registers as packed f32x2 pairs
 //     (thread t owns particles (2p+h)*256 + t);
 //   * after every drift each thread re-stages its own particles into the CTA's shared-memory source
-//     array in the pre-duplicated layout {x,x,y,y},{z,z,m,m} of pair_f32.cu, so the inner loop is the
-//     same 3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per two interactions (2 FMUL2 for equal masses,
-//     detected per simulation);
+//     array as plain {x, y, z, m} records (the layout of pair_f32.cu: one LDS.128 per source, the coordinate a
+//     scalar broadcast operand of the packed instructions), so the inner loop is the same 3 FADD2 + 6 FFMA2 +
+//     3 FMUL2 + 2 MUFU.RSQ per two interactions (2 FMUL2 for equal masses, detected per simulation);
 //   * two __syncthreads per step (sources staged / sources consumed), no global traffic in the loop;
 //   * two-level fp32 summation: 512-source tiles, tile sums added in tile order (n <= 2,048, so the
 //     single-accumulator stagnation of SURVEY.md section 0 cannot occur).
@@ -28,19 +28,20 @@ constexpr int ENS_TILE = 512;
 
 // One pass of a thread's NPAIR target pairs over sources [j0, j0 + ENS_TILE) of the staged array.
 template <int NPAIR, bool EQM>
-__device__ __forceinline__ void ens_tile(const ulonglong2* __restrict__ src, const int j0, const f32x2 e2,
+__device__ __forceinline__ void ens_tile(const float4* __restrict__ src, const int j0, const f32x2 e2,
                                          const f32x2 (&xi)[NPAIR], const f32x2 (&yi)[NPAIR], const f32x2 (&zi)[NPAIR],
                                          f32x2 (&ax)[NPAIR], f32x2 (&ay)[NPAIR], f32x2 (&az)[NPAIR])
 {
 #pragma unroll 8
     for (int j = j0; j < j0 + ENS_TILE; ++j) {
-        const ulonglong2 A = src[2 * j];          // {x,x},{y,y}
-        const ulonglong2 B = src[2 * j + 1];      // {z,z},{m,m}
+        // one LDS.128 per source {x, y, z, m}; the splats are scalar broadcast operands of the packed ops (pair_f32.cu)
+        const float4 q = src[j];
+        const f32x2 qx = pk(q.x, q.x), qy = pk(q.y, q.y), qz = pk(q.z, q.z), qm = pk(q.w, q.w);
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
-            const f32x2 dx = sub2(A.x, xi[p]);
-            const f32x2 dy = sub2(A.y, yi[p]);
-            const f32x2 dz = sub2(B.x, zi[p]);
+            const f32x2 dx = sub2(qx, xi[p]);
+            const f32x2 dy = sub2(qy, yi[p]);
+            const f32x2 dz = sub2(qz, zi[p]);
             f32x2 r2 = fma2(dx, dx, e2);
             r2 = fma2(dy, dy, r2);
             r2 = fma2(dz, dz, r2);
@@ -48,7 +49,7 @@ __device__ __forceinline__ void ens_tile(const ulonglong2* __restrict__ src, con
             unpk(r2, r2l, r2h);
             const f32x2 ri = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
             const f32x2 ri2 = mul2(ri, ri);
-            const f32x2 w = mul2(ri2, EQM ? ri : mul2(B.y, ri));
+            const f32x2 w = mul2(ri2, EQM ? ri : mul2(qm, ri));
             ax[p] = fma2(w, dx, ax[p]);
             ay[p] = fma2(w, dy, ay[p]);
             az[p] = fma2(w, dz, az[p]);
@@ -58,7 +59,7 @@ __device__ __forceinline__ void ens_tile(const ulonglong2* __restrict__ src, con
 
 // a_pair of the thread's targets from the staged sources: G * (m0 *) sum over tiles, tile order.
 template <int NPAIR, bool EQM>
-__device__ __forceinline__ void ens_pair(const ulonglong2* __restrict__ src, const int n_pad, const float eps2,
+__device__ __forceinline__ void ens_pair(const float4* __restrict__ src, const int n_pad, const float eps2,
                                          const float scale, const f32x2 (&xi)[NPAIR], const f32x2 (&yi)[NPAIR],
                                          const f32x2 (&zi)[NPAIR], f32x2 (&gx)[NPAIR], f32x2 (&gy)[NPAIR],
                                          f32x2 (&gz)[NPAIR])
@@ -89,15 +90,16 @@ __device__ __forceinline__ void ens_pair(const ulonglong2* __restrict__ src, con
     }
 }
 
-template <int NPAIR>
-__global__ void __launch_bounds__(ENS_THREADS, NPAIR <= 2 ? 2 : 1)
+// THREADS x 2 NPAIR target slots per simulation.
+template <int NPAIR, int THREADS>
+__global__ void __launch_bounds__(THREADS, NPAIR <= 2 ? 2 : 1)
 ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const EnsembleParams* __restrict__ params,
                     const int shared_params, const int n, const int64_t nsteps, float4* __restrict__ tape)
 {
     extern __shared__ __align__(16) unsigned char ens_smem[];
     float4* const stage4 = reinterpret_cast<float4*>(ens_smem);
-    const ulonglong2* const src = reinterpret_cast<const ulonglong2*>(ens_smem);
-    constexpr int n_pad = NPAIR * ENS_TILE;
+    const float4* const src = reinterpret_cast<const float4*>(ens_smem);
+    constexpr int n_pad = 2 * NPAIR * THREADS;
     const int tid = threadIdx.x;
     const int64_t sim = blockIdx.x;
     const EnsembleParams prm = params[shared_params ? 0 : sim];
@@ -113,7 +115,7 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
         float4 q[2], w[2];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const int i = (2 * p + h) * ENS_THREADS + tid;
+            const int i = (2 * p + h) * THREADS + tid;
             if (i < n) {
                 q[h] = P[i];
                 w[h] = V[i];
@@ -141,11 +143,9 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
         for (int p = 0; p < NPAIR; ++p) {
             float x0, x1, y0, y1, z0, z1, m0, m1;
             unpk(xi[p], x0, x1); unpk(yi[p], y0, y1); unpk(zi[p], z0, z1); unpk(mi[p], m0, m1);
-            const int i0 = (2 * p) * ENS_THREADS + tid, i1 = i0 + ENS_THREADS;
-            stage4[2 * i0] = make_float4(x0, x0, y0, y0);
-            stage4[2 * i0 + 1] = make_float4(z0, z0, m0, m0);
-            stage4[2 * i1] = make_float4(x1, x1, y1, y1);
-            stage4[2 * i1 + 1] = make_float4(z1, z1, m1, m1);
+            const int i0 = (2 * p) * THREADS + tid, i1 = i0 + THREADS;
+            stage4[i0] = make_float4(x0, y0, z0, m0);
+            stage4[i1] = make_float4(x1, y1, z1, m1);
         }
         __syncthreads();                                   // sources staged
         if (n == 1) {
@@ -164,11 +164,11 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
                 unpk(xi[p], x0, x1); unpk(yi[p], y0, y1); unpk(zi[p], z0, z1);
                 unpk(gx[p], a0, a1); unpk(gy[p], b0, b1); unpk(gz[p], c0, c1);
                 float ex, ey, ez;
-                if ((2 * p) * ENS_THREADS + tid < n) {
+                if ((2 * p) * THREADS + tid < n) {
                     ext_accel<float>(prm.pot, x0, y0, z0, ex, ey, ez);
                     a0 += ex; b0 += ey; c0 += ez;
                 }
-                if ((2 * p + 1) * ENS_THREADS + tid < n) {
+                if ((2 * p + 1) * THREADS + tid < n) {
                     ext_accel<float>(prm.pot, x1, y1, z1, ex, ey, ez);
                     a1 += ex; b1 += ey; c1 += ez;
                 }
@@ -191,7 +191,7 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
             unpk(gx[p], ga[0], ga[1]); unpk(gy[p], gb[0], gb[1]); unpk(gz[p], gc[0], gc[1]);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const int i = (2 * p + h) * ENS_THREADS + tid;
+                const int i = (2 * p + h) * THREADS + tid;
                 if (i < n) {
                     S[i] = make_float4(x[h], y[h], z[h], m[h]);
                     S[n + i] = make_float4(a[h], b[h], c[h], 0.0f);
@@ -227,7 +227,7 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
         unpk(vx[p], a[0], a[1]); unpk(vy[p], b[0], b[1]); unpk(vz[p], c[0], c[1]);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const int i = (2 * p + h) * ENS_THREADS + tid;
+            const int i = (2 * p + h) * THREADS + tid;
             if (i < n) {
                 P[i] = make_float4(x[h], y[h], z[h], m[h]);
                 V[i] = make_float4(a[h], b[h], c[h], 0.0f);
@@ -236,14 +236,15 @@ ensemble_kdk_kernel(float4* __restrict__ posm, float4* __restrict__ vel, const E
     }
 }
 
-template <int NPAIR>
+template <int NPAIR, int THREADS>
 cudaError_t launch_ens(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n, int64_t nsim,
                        int64_t nsteps, float* tape, cudaStream_t stream)
 {
-    const size_t smem = (size_t)NPAIR * ENS_TILE * 32;
-    cudaError_t e = cudaFuncSetAttribute(ensemble_kdk_kernel<NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static_assert((2 * NPAIR * THREADS) % ENS_TILE == 0, "whole source tiles");
+    const size_t smem = (size_t)2 * NPAIR * THREADS * 16;
+    cudaError_t e = cudaFuncSetAttribute(ensemble_kdk_kernel<NPAIR, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ensemble_kdk_kernel<NPAIR><<<(unsigned)nsim, ENS_THREADS, smem, stream>>>(
+    ensemble_kdk_kernel<NPAIR, THREADS><<<(unsigned)nsim, THREADS, smem, stream>>>(
         reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vel), params, shared_params, n, nsteps,
         reinterpret_cast<float4*>(tape));
     return cudaGetLastError();
@@ -254,10 +255,11 @@ cudaError_t launch_ens(float* posm, float* vel, const EnsembleParams* params, in
 cudaError_t launch_ensemble_f32(float* posm, float* vel, const EnsembleParams* params, int shared_params, int n,
                                 int64_t nsim, int64_t nsteps, float* tape, cudaStream_t stream)
 {
-    if (n <= 1 * ENS_TILE) return launch_ens<1>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
-    if (n <= 2 * ENS_TILE) return launch_ens<2>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
-    if (n <= 3 * ENS_TILE) return launch_ens<3>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
-    return launch_ens<4>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    // (128 threads x 8 targets, the pair kernel's register tile, measured no faster: 2.45-2.49 against 2.51 M simulation-steps/s)
+    if (n <= 1 * ENS_TILE) return launch_ens<1, 256>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    if (n <= 2 * ENS_TILE) return launch_ens<2, 256>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    if (n <= 3 * ENS_TILE) return launch_ens<3, 256>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
+    return launch_ens<4, 256>(posm, vel, params, shared_params, n, nsim, nsteps, tape, stream);
 }
 
 }  // namespace odisseo
