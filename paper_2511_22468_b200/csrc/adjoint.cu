@@ -16,8 +16,8 @@
 // ranges, {position, cotangent} source records through the TMA ring, one row of fp64 sums per unit, rows added
 // in fixed order by vjp_finish_kernel (bit-reproducible, no atomics).  fp32: every loop form (equal or general
 // masses, with or without the eps / G terms) runs on packed f32x2 pairs, two targets per instruction, sources
-// staged pre-duplicated {x,x,y,y},{z,z,cx,cx},{cy,cy,cz,cz},{m,m,0,0}: 26 packed ops + 2 MUFU per two pairs in the
-// equal-mass form.  fp64: the scalar term of adjoint_terms.cuh.  Per-tile sums in the state's precision, promoted
+// staged as plain {x,y,z,m},{cx,cy,cz,0} records (two LDS.128 per source, scalar broadcast operands): 26 packed ops + 2 MUFU
+// per two pairs in the equal-mass form.  fp64: the scalar term of adjoint_terms.cuh.  Per-tile sums in the state's precision, promoted
 // to fp64 between tiles.  The O(N) parts (external potential, parameter sums) are evaluated in fp64 whatever the
 // state precision.
 #include "adjoint_terms.cuh"
@@ -34,7 +34,7 @@ template <> struct AVec4<double> { typedef double4 type; };
 // ---- fp32 consumer: 2*NPAIR targets per thread as packed pairs -------------------------------------------------
 template <int NPAIR, bool EG, int CWARPS_, int MINB_, int JUNROLL>
 struct VjpF32 {
-    static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 64, COMPS = EG ? 6 : 4;
+    static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 32, COMPS = EG ? 6 : 4;
     static constexpr int CTHREADS = CWARPS * 32;
     struct Params { const float4* posm; const float4* cot; float eps2; };
     static size_t outer_bytes() { return (size_t)2 * NPAIR * COMPS * CTHREADS * sizeof(double); }
@@ -83,14 +83,17 @@ struct VjpF32 {
         }
         __device__ __forceinline__ void tile(const unsigned char* tile_raw, const int len)
         {
-            const ulonglong2* __restrict__ t = reinterpret_cast<const ulonglong2*>(tile_raw);
+            const float4* __restrict__ t = reinterpret_cast<const float4*>(tile_raw);
 #pragma unroll JUNROLL
             for (int j = 0; j < len; ++j) {
-                const ulonglong2 A = t[4 * j];            // {x,x},{y,y}
-                const ulonglong2 B = t[4 * j + 1];        // {z,z},{cx,cx}
-                const ulonglong2 C = t[4 * j + 2];        // {cy,cy},{cz,cz}
+                // two LDS.128 per source: {x, y, z, m}, {cx, cy, cz, 0}; the splats are scalar broadcast operands of the
+                // packed instructions (pair_f32.cu), nothing is pre-duplicated
+                const float4 q = t[2 * j], c = t[2 * j + 1];
+                struct { f32x2 x, y; } A, B, C;
+                A.x = pk(q.x, q.x); A.y = pk(q.y, q.y); B.x = pk(q.z, q.z);
+                B.y = pk(c.x, c.x); C.x = pk(c.y, c.y); C.y = pk(c.z, c.z);
                 f32x2 mj = 0ull;
-                if (!EQM) mj = t[4 * j + 3].x;            // {m,m}
+                if (!EQM) mj = pk(q.w, q.w);
 #pragma unroll
                 for (int p = 0; p < NPAIR; ++p) {
                     const f32x2 dx = sub2(A.x, xi[p]), dy = sub2(A.y, yi[p]), dz = sub2(B.x, zi[p]);
@@ -231,14 +234,13 @@ struct VjpF64 {
 constexpr int VJP_NPAIR = 3, VJP_CW = 8, VJP_MINB = 1, VJP_JU = 4;
 constexpr int VJP_IPT64 = 2, VJP_T32 = 256, VJP_T64 = 128;
 
-// Staged source record of the pull-back (64 B), padding records massless, parked far away, zero cotangent.
+// Staged source record of the pull-back: {x, y, z, m}, {cx, cy, cz, 0} (fp32 32 B, fp64 64 B); padding records massless,
+// parked far away, zero cotangent.
 __device__ __forceinline__ void vjp_stage_record(void* jsrc, int64_t i, float x, float y, float z, float m, float cx, float cy, float cz)
 {
-    float4* out = reinterpret_cast<float4*>(jsrc) + 4 * i;
-    out[0] = make_float4(x, x, y, y);
-    out[1] = make_float4(z, z, cx, cx);
-    out[2] = make_float4(cy, cy, cz, cz);
-    out[3] = make_float4(m, m, 0.f, 0.f);
+    float4* out = reinterpret_cast<float4*>(jsrc) + 2 * i;
+    out[0] = make_float4(x, y, z, m);
+    out[1] = make_float4(cx, cy, cz, 0.f);
 }
 __device__ __forceinline__ void vjp_stage_record(void* jsrc, int64_t i, double x, double y, double z, double m, double cx, double cy,
                                                  double cz)

@@ -94,7 +94,7 @@ PairPlan make_vjp_plan(int64_t n, int is_f64, int num_sms)
     p.IB = ipt * cthreads;
     p.S = source_split(n, p.T, p.IB, (int64_t)num_sms * minb);
     p.variant = 0;
-    p.rec_bytes = 64;
+    p.rec_bytes = is_f64 ? 64 : 32;                       // {x, y, z, m}, {cx, cy, cz, 0}
     p.comps = 6;
     p.nb = (int32_t)((n + p.IB - 1) / p.IB);
     p.U = (int64_t)p.nb * p.S;
