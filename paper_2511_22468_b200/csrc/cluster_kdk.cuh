@@ -15,12 +15,13 @@
 //     barrier, no grid barrier, no launch edge inside the loop; positions, velocities and accelerations never leave
 //     the SMs.  Two record buffers and two inbox barriers alternate, which is enough: a CTA pushes step k + 1 only
 //     after it has received every push of step k, and a CTA pushes step k only after it has read buffer k.
-// Measured (B200, us per KDK step, this kernel / per-step launches): fp32 N = 128 2.4 / 4.8, 256 2.9 / 5.4, 512 4.1 / 6.2,
-// 1,024 7.0 / 7.8; fp64 256 6.1 / 7.4, 512 7.8 / 8.3, 1,024 13.8 / 10.8.  It runs on 16 of the 148 SMs, so above N ~ 1,000
-// the pair phase (N^2 / 16 per SM; 9.3 k of the 13.5 k cycles of a step at N = 1,024) costs more than the latency it saves.
-// The rest of a step at N = 1,024: the owners' row reduce 1.9 k cycles (a balanced-tree grouping was tried: no faster),
-// kicks + drift + 16 pushes 0.65 k, waiting for the other CTAs' records 0.9 k, re-expansion 0.6 k
-// (profiles/r02_cluster_kdk_ncu_full.txt).
+// Measured (B200, us per KDK step, this kernel / per-step launches): fp32 N = 256 2.5 / 5.2, 512 4.1 / 6.2, 1,024 6.1 / 7.7;
+// fp64 256 6.1 / 7.4, 512 7.8 / 8.3, 1,024 13.8 / 10.8.  It runs on 16 of the 148 SMs, so above N ~ 1,000 the pair phase
+// (N^2 / 16 per SM; two thirds of a step at N = 1,024) costs more than the latency it saves; the rest of a step is the
+// owners' row reduce, kicks + drift + 16 pushes, and the wait for the other CTAs' records
+// (profiles/r02_cluster_kdk_ncu_full.txt, captured while the records were still staged pre-duplicated).  The
+// flag-in-data kernel (ll_kdk.cuh: all SMs, one L2 round trip per step) is tried first; this form serves when that
+// cooperative grid cannot be placed.
 //
 // Summation order: chunk and tile boundaries are the launch plan's (functions of n alone), tile sums in the Consumer's
 // precision, promoted to fp64 per tile, chunk sums added in increasing s, factor G [m] applied once in fp64 -- the
