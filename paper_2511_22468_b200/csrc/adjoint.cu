@@ -231,7 +231,7 @@ struct VjpF64 {
 
 // 6 targets per thread as 3 packed pairs, 8 compute warps, one CTA per SM, j loop unrolled 4: the best of the
 // measured geometries (2-4 pairs x 8/12/16 warps x 1-2 CTAs: 1,080-1,180 G-pairs/s at N = 262,144).
-constexpr int VJP_NPAIR = 3, VJP_CW = 8, VJP_MINB = 1, VJP_JU = 4;
+constexpr int VJP_NPAIR = 3, VJP_CW = 8, VJP_MINB = 1, VJP_JU = 8;
 constexpr int VJP_IPT64 = 2, VJP_T32 = 256, VJP_T64 = 128;
 
 // Staged source record of the pull-back: {x, y, z, m}, {cx, cy, cz, 0} (fp32 32 B, fp64 64 B); padding records massless,

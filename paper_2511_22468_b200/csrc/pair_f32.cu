@@ -28,7 +28,10 @@ namespace odisseo {
 
 namespace {
 
-template <int NPAIR, int CWARPS_, int MINB_, int JUNROLL>
+// JUNROLL / JUNROLL_G: unroll of the j loop on the equal-mass / general-mass path (the general body holds one more
+// packed value per source).  Measured at N = 262,144: equal-mass loop 24.43 ms at 8, 24.21 at 16 and 32; the general loop is
+// within 1 % for 2 ... 16 (25.9-26.2 ms; 25.8 when the equal-mass loop is unrolled 8: the two paths share one register budget).
+template <int NPAIR, int CWARPS_, int MINB_, int JUNROLL, int JUNROLL_G = JUNROLL>
 struct PairF32 {
     static constexpr int CWARPS = CWARPS_, MINB = MINB_, REC = 16, COMPS = 3;
     static constexpr int CTHREADS = CWARPS * 32;
@@ -81,7 +84,7 @@ struct PairF32 {
         __device__ __forceinline__ void tile(const unsigned char* tile_raw, const int len)
         {
             const float4* __restrict__ t = reinterpret_cast<const float4*>(tile_raw);
-#pragma unroll JUNROLL
+#pragma unroll (EQM ? JUNROLL : JUNROLL_G)
             for (int j = 0; j < len; ++j) {
                 // one LDS.128 per source; the splats below cost nothing: ptxas feeds the scalar register to the packed
                 // instruction as a broadcast operand (FADD2 R, Rj.F32, -Ri.F32x2) -- no MOV, no pre-duplicated staging
@@ -149,7 +152,7 @@ struct PairF32 {
     };
 };
 
-typedef PairF32<4, 8, 1, 8> LargeF32;    // 2,048 targets per CTA, one CTA per SM
+typedef PairF32<4, 8, 1, 16, 8> LargeF32;  // 2,048 targets per CTA, one CTA per SM
 typedef PairF32<1, 2, 8, 4> SmallF32;    // 128 targets per CTA, up to 8 CTAs per SM (n <= 4,096)
 typedef PairF32<1, 2, 4, 4> SmallF32Fused;   // the same loop inside the whole-loop kernel, which also holds the reduce batch
 
