@@ -209,7 +209,7 @@ __device__ __forceinline__ void ll_fetch_pair(const unsigned long long* rec, con
 
 // C: a pair Consumer with two targets per thread (PairF32<1, ...> / PairF64<2, ...>); its State<EQM> supplies
 // set_target_pair(), tile() and take_sums().
-template <class C, typename T, bool EQM>
+template <class C, typename T, bool EQM, bool TAPE>
 __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* smem, const double m0)
 {
     typedef typename Vec4<T>::type V4;
@@ -339,7 +339,7 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
                 const T tx = a.x + ex, ty = a.y + ey, tz = a.z + ez;
                 V4 v = svel[tid];
                 if (close) { v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z); }
-                if (ca.tape) {
+                if (TAPE && ca.tape) {
                     // the synchronised state between the closing kick of step k - 1 and the opening kick of step k
                     // (step_body.cuh's snapshot); k = pushes: one snapshot per integrate call
                     V4* snap = ca.tape + (size_t)pushes * 3 * n;
@@ -402,7 +402,8 @@ __device__ __forceinline__ void ll_kdk_loop(const LLArgs<T>& ca, unsigned char* 
 #endif
 }
 
-template <class C, typename T>
+// TAPE: the instantiation that can store the reverse mode's snapshots (it also runs with a null tape).
+template <class C, typename T, bool TAPE>
 __global__ void __launch_bounds__(LL_THREADS, 1)
 ll_kdk_kernel(const LLArgs<T> ca)
 {
@@ -433,21 +434,23 @@ ll_kdk_kernel(const LLArgs<T> ca)
     }
     const bool eqm = __syncthreads_or(differs) == 0;
     if (eqm)
-        ll_kdk_loop<C, T, true>(ca, smem_raw, (double)mass0);
+        ll_kdk_loop<C, T, true, TAPE>(ca, smem_raw, (double)mass0);
     else
-        ll_kdk_loop<C, T, false>(ca, smem_raw, (double)mass0);
+        ll_kdk_loop<C, T, false, TAPE>(ca, smem_raw, (double)mass0);
 }
 
 // Host side.  Co-resident CTAs of the kernel on this device (cooperative launch bound).
 template <class C, typename T> cudaError_t configure_ll(int num_sms, int* max_ctas)
 {
     *max_ctas = 0;
-    cudaError_t e = cudaFuncSetAttribute(ll_kdk_kernel<C, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, LL_SMEM_MAX);
+    cudaError_t e = cudaFuncSetAttribute(ll_kdk_kernel<C, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, LL_SMEM_MAX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(ll_kdk_kernel<C, T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, LL_SMEM_MAX);
     if (e != cudaSuccess) return e;
-    int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ll_kdk_kernel<C, T>, LL_THREADS, (size_t)LL_SMEM_MAX);
+    int per_sm = 0, per_sm2 = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ll_kdk_kernel<C, T, true>, LL_THREADS, (size_t)LL_SMEM_MAX);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, ll_kdk_kernel<C, T, false>, LL_THREADS, (size_t)LL_SMEM_MAX);
     if (e != cudaSuccess) return e;
-    *max_ctas = per_sm * num_sms;
+    *max_ctas = (per_sm < per_sm2 ? per_sm : per_sm2) * num_sms;
     return cudaSuccess;
 }
 
@@ -470,12 +473,14 @@ template <typename T> size_t ll_geometry(const PairPlan& plan, int max_ctas, int
     return L.total <= (size_t)LL_SMEM_MAX ? L.total : 0;
 }
 
+// tape_code: launch the instantiation that carries the snapshot stores (required when ca.tape is set).
 template <class C, typename T>
-cudaError_t launch_ll(const LLArgs<T>& ca, int ctas, size_t smem, cudaStream_t stream)
+cudaError_t launch_ll(const LLArgs<T>& ca, int ctas, size_t smem, bool tape_code, cudaStream_t stream)
 {
     LLArgs<T> a = ca;
     void* args[] = {&a};
-    return cudaLaunchCooperativeKernel(reinterpret_cast<void*>(ll_kdk_kernel<C, T>), dim3(ctas), dim3(LL_THREADS), args, smem, stream);
+    void* kernel = tape_code || ca.tape ? reinterpret_cast<void*>(ll_kdk_kernel<C, T, true>) : reinterpret_cast<void*>(ll_kdk_kernel<C, T, false>);
+    return cudaLaunchCooperativeKernel(kernel, dim3(ctas), dim3(LL_THREADS), args, smem, stream);
 }
 
 }  // namespace odisseo

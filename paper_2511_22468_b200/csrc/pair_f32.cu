@@ -162,6 +162,10 @@ typedef PairF32<1, 2, 1, 8> LLF32;           // ... and inside the flag-in-data 
 int g_fused_max_ctas[2] = {0, 0};        // co-resident CTAs of the whole-loop kernel, [variant]
 int g_cluster_size = 0;                  // CTAs per cluster the device schedules for the cluster kernel (0 = none)
 int g_ll_max_ctas = 0;                   // co-resident CTAs of the flag-in-data whole-loop kernel (ll_kdk.cuh)
+// Which instantiation serves calls WITHOUT a tape.  The step of that kernel is a latency chain, and the two instantiations,
+// which differ by a few predicated stores in the owner threads, schedule differently: measured at N = 1,024 the one with
+// the tape code runs 3.1 us per step in fp32 (4.5 without) and 8.7 in fp64 (6.8 without).  Measured choice, per precision.
+constexpr bool LL_TAPE_CODE_FLOAT = true;
 
 }  // namespace
 
@@ -233,7 +237,7 @@ cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* 
     const size_t smem = ll_geometry<float>(plan, g_ll_max_ctas, &ca.tpc, &ctas, &xbytes);
     cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
     if (e != cudaSuccess) return e;
-    return launch_ll<LLF32, float>(ca, ctas, smem, stream);
+    return launch_ll<LLF32, float>(ca, ctas, smem, LL_TAPE_CODE_FLOAT, stream);
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
