@@ -511,7 +511,7 @@ def _mmd_rate(B, W, torch, n: int = 1000, m: int = 1000, nsim: int = 2960):
 
 def run_sharded(args, rank: int, world: int, dist, torch, B, W):
     """--mode sharded: one simulation of the config, targets sliced over the ranks; per KDK step one in-place all-gather
-    of the staged source records (32 N bytes in total).  value = N^2 x steps / max-over-ranks device time."""
+    of the staged source records (16 N bytes in total).  value = N^2 x steps / max-over-ranks device time."""
     from paper_2511_22468_b200 import sharded as S
     cfg = W.CONFIGS[args.config]
     n = cfg.n

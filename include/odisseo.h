@@ -160,7 +160,7 @@ odisseo_status odisseo_pair_accel_cross_f64(const double *d_targets, int64_t nt,
  * so every rank count -- 1 included -- gives results BIT-IDENTICAL to odisseo_leapfrog_kdk_* on one GPU.
  *   odisseo_staged_sources_layout: out = {byte offset of record 0 in the workspace, bytes per record, records the
  *     array has room for (8 ceil(n/8) + 1,024: room for equal 8-aligned slices of up to 128 ranks)}.  Host arithmetic.
- *     fp32 records are {x,x,y,y},{z,z,m,m}; fp64 records {x,y,z,m}; both 32 bytes.
+ *     Records are plain {x,y,z,m} in both precisions: 16 bytes (fp32) / 32 bytes (fp64).
  *   odisseo_stage_sources_*: d_posm [n][4].  Workspace >= odisseo_cross_workspace_bytes(nt, n, is_f64).
  *   odisseo_pair_accel_staged_*: d_targets [nt][4] (positions; lane 3 ignored), d_acc [nt][4] out (pair-only).
  *   odisseo_kick_drift_slice_*: d_posm, d_vel, d_acc address the slice's count records (d_posm may point into the

@@ -6,13 +6,13 @@ shards naturally over TARGETS: rank r owns the contiguous slice [lo_r, hi_r) of 
 records of ALL particles, and per KDK step
 
     kick + drift its slice            odisseo_kick_drift_slice: also re-stages the slice's records in place
-    exchange                          ONE in-place all-gather of the record array (32 N bytes in total per step)
+    exchange                          ONE in-place all-gather of the record array (16 N bytes in total per step in fp32, 32 N in fp64)
     a_pair(slice) from all sources    odisseo_pair_accel_staged: no re-packing of the N sources
 
 Slices are equal and 8-aligned (the last one shorter), so rank r's records sit at [r L, (r+1) L) of the record array
 and the all-gather lands every rank's records at their global index.  The order in which a target's partial sums
 are added depends on N only (include/odisseo.h), so any number of ranks -- 1 included -- is BIT-IDENTICAL to
-odisseo_leapfrog_kdk on one GPU.  Compute per rank is N^2 / R, traffic 32 N bytes per step: at N = 262,144 on 8 GPUs
+odisseo_leapfrog_kdk on one GPU.  Compute per rank is N^2 / R, traffic 16 N bytes per step (fp32): at N = 262,144 on 8 GPUs
 ~3 ms of arithmetic against microseconds on NVLink, the near-linear behaviour the paper reports.
 
 north_star fixes this build to ONE GPU, and nothing in this run can execute more than one: `bench.py --mode sharded`
