@@ -157,3 +157,14 @@ def test_product_path_fails_loudly_without_gpu_or_library(monkeypatch):
     monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/libodisseo_b200.so")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         B.lib()
+
+
+def test_staged_sources_layout_plain_records(lib):
+    """The staged source array of the sharded form holds plain {x, y, z, m} records (16 B fp32, 32 B fp64) behind the
+    flag block, with room for the 8-aligned padding plus 1,024 records of slack for the in-place all-gather."""
+    for n in (1, 7, 8, 1000, 262144):
+        for f64, rec in ((False, 16), (True, 32)):
+            off, rec_bytes, cap = B.staged_sources_layout(n, f64)
+            assert rec_bytes == rec and off % 256 == 0 and off >= 256
+            assert cap == 8 * -(-n // 8) + 1024
+            assert off + cap * rec_bytes <= B.workspace_bytes(n, f64)
