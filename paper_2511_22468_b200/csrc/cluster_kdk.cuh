@@ -19,7 +19,7 @@
 // fp64 256 6.1 / 7.4, 512 7.8 / 8.3, 1,024 13.8 / 10.8.  It runs on 16 of the 148 SMs, so above N ~ 1,000 the pair phase
 // (N^2 / 16 per SM; two thirds of a step at N = 1,024) costs more than the latency it saves; the rest of a step is the
 // owners' row reduce, kicks + drift + 16 pushes, and the wait for the other CTAs' records
-// (profiles/r02_cluster_kdk_ncu_full.txt, captured while the records were still staged pre-duplicated).  The
+// (profiles/r02_cluster_kdk_ncu_full.txt).  The
 // flag-in-data kernel (ll_kdk.cuh: all SMs, one L2 round trip per step) is tried first; this form serves when that
 // cooperative grid cannot be placed.
 //
