@@ -10,9 +10,10 @@
 //
 // Batched like the ensemble kernels (the paper's grid search and gradient steps run thousands of N = 1,000 simulations
 // against one observed stream, L47): grid = (target blocks, simulations).  All-pairs tiling as in the pair kernels:
-// a thread keeps its target's six scaled coordinates u = x s_d, s_d = sqrt(log2(e)/2)/sigma_d, in registers, so that
-// k = ex2(-|u - u'|^2) is 6 FADD + 6 FFMA + 1 MUFU.EX2; source tiles of 256 points are staged scaled in shared memory
-// (structure of arrays, broadcast reads); sums are fp32 inside a tile and fp64 across tiles; per-block sums are added
+// a thread keeps the six scaled coordinates u = x s_d, s_d = sqrt(log2(e)/2)/sigma_d, of TWO targets in registers as packed
+// f32x2 pairs, so that two evaluations k = ex2(-|u - u'|^2) cost 6 FADD2 + 6 FFMA2 + 2 MUFU.EX2; source tiles of 256 points
+// are staged scaled in shared memory ({x,y,z,vx},{vy,vz}: two broadcast loads per source, each coordinate a scalar
+// broadcast operand of the packed instructions); sums are fp32 inside a tile and fp64 across tiles; per-block sums are added
 // in block order by a second kernel (fixed order, no atomics: bit-reproducible).  The gradient lands in the layout of
 // the pull-back's cotangents (float4 {d/dx, d/dy, d/dz, 0}), so loss -> gradient never leaves the device.
 #include "odisseo_common.cuh"
@@ -23,6 +24,7 @@ namespace {
 
 constexpr int MMD_THREADS = 256;
 constexpr int MMD_TILE = 256;
+constexpr int MMD_PER_BLOCK = 2 * MMD_THREADS;      // two target slots per thread
 
 struct MmdScales { float s[6]; float back[6]; };    // u = x s_d;  back_d = 4 s_d ln 2 (below)
 
@@ -46,48 +48,60 @@ __device__ __forceinline__ double mmd_block_sum(double v, double* warp_scratch)
     return s;
 }
 
-// One pass of the targets of block (blockIdx.x, sim) over a source cloud: returns sum_j k and, when GRAD, adds
-// sum_j k (u_src - u_tgt)_d into acc[0..5].
+// One pass of the block's targets over a source cloud.  A thread holds TWO targets as packed f32x2 pairs (slots t and
+// t + 256 of the block's 512); a source arrives as {x,y,z,vx},{vy,vz} (LDS.128 + LDS.64 broadcasts) and each coordinate
+// enters the packed instructions as a scalar operand broadcast to both halves (pair_f32.cu): per source and thread
+// 7 FADD2 + 12 FFMA2 + 2 MUFU.EX2 for two kernel evaluations with their gradient terms.  Returns sum_j k per target and,
+// when GRAD, adds sum_j k (u_src - u_tgt)_d into acc0 / acc1.
 template <bool GRAD>
-__device__ __forceinline__ double mmd_pass(const float4* __restrict__ spos, const float4* __restrict__ svel, const int ns,
-                                           const MmdScales& sc, const float (&u)[6], float (*tile)[MMD_TILE], double (&acc)[6])
+__device__ __forceinline__ void mmd_pass(const float4* __restrict__ spos, const float4* __restrict__ svel, const int ns,
+                                         const MmdScales& sc, const f32x2 (&u)[6], float4* tileA, float2* tileB, double (&acc0)[6],
+                                         double (&acc1)[6], double& total0, double& total1)
 {
-    double total = 0.0;
+    total0 = total1 = 0.0;
     for (int j0 = 0; j0 < ns; j0 += MMD_TILE) {
         __syncthreads();                                     // the previous tile is consumed
         const int j = j0 + threadIdx.x;
         if (threadIdx.x < MMD_TILE) {
             float4 p = make_float4(0.f, 0.f, 0.f, 0.f), v = p;
             if (j < ns) { p = spos[j]; v = svel[j]; }
-            tile[0][threadIdx.x] = p.x * sc.s[0]; tile[1][threadIdx.x] = p.y * sc.s[1]; tile[2][threadIdx.x] = p.z * sc.s[2];
-            tile[3][threadIdx.x] = v.x * sc.s[3]; tile[4][threadIdx.x] = v.y * sc.s[4]; tile[5][threadIdx.x] = v.z * sc.s[5];
+            tileA[threadIdx.x] = make_float4(p.x * sc.s[0], p.y * sc.s[1], p.z * sc.s[2], v.x * sc.s[3]);
+            tileB[threadIdx.x] = make_float2(v.y * sc.s[4], v.z * sc.s[5]);
         }
         __syncthreads();
         const int len = ns - j0 < MMD_TILE ? ns - j0 : MMD_TILE;
-        float ksum = 0.f, g[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        f32x2 ksum = 0ull, g[6] = {0ull, 0ull, 0ull, 0ull, 0ull, 0ull};
 #pragma unroll 4
         for (int t = 0; t < len; ++t) {
-            float d[6], q = 0.f;
+            const float4 A = tileA[t];
+            const float2 Bv = tileB[t];
+            const float s6[6] = {A.x, A.y, A.z, A.w, Bv.x, Bv.y};
+            f32x2 d[6], q = 0ull;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) { d[c] = tile[c][t] - u[c]; q = fmaf(d[c], d[c], q); }
-            const float k = ex2_approx(-q);
-            ksum += k;
+            for (int c = 0; c < 6; ++c) { d[c] = sub2(pk(s6[c], s6[c]), u[c]); q = fma2(d[c], d[c], q); }
+            float ql, qh;
+            unpk(q, ql, qh);
+            const f32x2 k = pk(ex2_approx(-ql), ex2_approx(-qh));
+            ksum = add2(ksum, k);
             if (GRAD) {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) g[c] = fmaf(k, d[c], g[c]);
+                for (int c = 0; c < 6; ++c) g[c] = fma2(k, d[c], g[c]);
             }
         }
-        total += (double)ksum;                               // second summation level, as in the pair kernels
+        float lo, hi;
+        unpk(ksum, lo, hi);
+        total0 += (double)lo;                                // second summation level, as in the pair kernels
+        total1 += (double)hi;
         if (GRAD) {
 #pragma unroll
-            for (int c = 0; c < 6; ++c) acc[c] += (double)g[c];
+            for (int c = 0; c < 6; ++c) { unpk(g[c], lo, hi); acc0[c] += (double)lo; acc1[c] += (double)hi; }
         }
     }
-    return total;
 }
 
-// grid = (ceil(max(n, m) / 256), nsim).  Thread t of block b handles simulated point i = b*256 + t (xx and xy sums,
-// gradient) and observed point j = b*256 + t (yy sum).  block_sums[sim][block][3] = {sum k_xx, sum k_xy, sum k_yy}.
+// grid = (ceil(max(n, m) / 512), nsim).  Thread t of block b handles simulated points i0 = b*512 + t and i1 = i0 + 256
+// (xx and xy sums, gradient) and the observed points with the same indices (yy sum).
+// block_sums[sim][block][3] = {sum k_xx, sum k_xy, sum k_yy}.
 template <bool GRAD>
 __global__ void __launch_bounds__(MMD_THREADS)
 mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, const int n, const float4* __restrict__ ypos,
@@ -95,52 +109,73 @@ mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, con
            const double* __restrict__ grad_scale, float4* __restrict__ gpos, float4* __restrict__ gvel,
            double* __restrict__ block_sums)
 {
-    __shared__ float tile[6][MMD_TILE];
+    __shared__ float4 tileA[MMD_TILE];
+    __shared__ float2 tileB[MMD_TILE];
     __shared__ double warp_scratch[MMD_THREADS / 32];
     const int64_t sim = blockIdx.y;
     const float4* const XP = xpos + sim * n;
     const float4* const XV = xvel + sim * n;
     const float4* const YP = ypos + (shared_y ? 0 : sim * m);
     const float4* const YV = yvel + (shared_y ? 0 : sim * m);
-    const int i = blockIdx.x * MMD_THREADS + threadIdx.x;
+    const int base = blockIdx.x * MMD_PER_BLOCK;
+    const int i0 = base + threadIdx.x, i1 = i0 + MMD_THREADS;
+    const f32x2 nz = pk(-0.0f, -0.0f);
 
-    // ---- simulated point i against X and against Y ----------------------------------------------------------
-    float u[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (i < n) {
-        const float4 p = XP[i], v = XV[i];
-        u[0] = p.x * sc.s[0]; u[1] = p.y * sc.s[1]; u[2] = p.z * sc.s[2];
-        u[3] = v.x * sc.s[3]; u[4] = v.y * sc.s[4]; u[5] = v.z * sc.s[5];
-    }
-    double axx[6] = {0, 0, 0, 0, 0, 0}, axy[6] = {0, 0, 0, 0, 0, 0};
+    // scaled coordinates of two points of a cloud as packed pairs (slots beyond the cloud: zeros, their sums are dropped)
+    auto load_pair = [&](const float4* P, const float4* V, const int cnt, f32x2 (&u)[6]) {
+        float a[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, b[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (i0 < cnt) {
+            const float4 p = P[i0], v = V[i0];
+            a[0] = p.x * sc.s[0]; a[1] = p.y * sc.s[1]; a[2] = p.z * sc.s[2]; a[3] = v.x * sc.s[3]; a[4] = v.y * sc.s[4]; a[5] = v.z * sc.s[5];
+        }
+        if (i1 < cnt) {
+            const float4 p = P[i1], v = V[i1];
+            b[0] = p.x * sc.s[0]; b[1] = p.y * sc.s[1]; b[2] = p.z * sc.s[2]; b[3] = v.x * sc.s[3]; b[4] = v.y * sc.s[4]; b[5] = v.z * sc.s[5];
+        }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) u[c] = add2(pk(a[c], b[c]), nz);
+    };
+
+    // ---- simulated points against X and against Y ---------------------------------------------------------------
     double sxx = 0.0, sxy = 0.0, syy = 0.0;
-    if (blockIdx.x * MMD_THREADS < n) {                       // block-uniform: the barriers inside are safe
-        sxx = mmd_pass<GRAD>(XP, XV, n, sc, u, tile, axx);
-        sxy = mmd_pass<GRAD>(YP, YV, m, sc, u, tile, axy);
-        if (i >= n) sxx = sxy = 0.0;
-        if (GRAD && i < n) {
+    if (base < n) {                                           // block-uniform: the barriers inside are safe
+        f32x2 u[6];
+        load_pair(XP, XV, n, u);
+        double axx0[6] = {0, 0, 0, 0, 0, 0}, axx1[6] = {0, 0, 0, 0, 0, 0}, axy0[6] = {0, 0, 0, 0, 0, 0}, axy1[6] = {0, 0, 0, 0, 0, 0};
+        double xx0, xx1, xy0, xy1;
+        mmd_pass<GRAD>(XP, XV, n, sc, u, tileA, tileB, axx0, axx1, xx0, xx1);
+        mmd_pass<GRAD>(YP, YV, m, sc, u, tileA, tileB, axy0, axy1, xy0, xy1);
+        sxx = (i0 < n ? xx0 : 0.0) + (i1 < n ? xx1 : 0.0);
+        sxy = (i0 < n ? xy0 : 0.0) + (i1 < n ? xy1 : 0.0);
+        if (GRAD) {
             // with k = ex2(-|u - u'|^2): dk/dx_d = -2 ln2 s_d k (u - u')_d, and the symmetric double sum doubles the xx
             // term: dMMD^2/dx_{i,d} = 4 ln2 s_d [ sum_i' k (u_i' - u_i)_d / n^2 - sum_j k (u_j - u_i)_d / (n m) ];
             // the accumulators hold exactly those two sums
             const double gs = grad_scale ? grad_scale[sim] : 1.0;
             const double cxx = gs / ((double)n * n), cxy = -gs / ((double)n * m);
-            float o[6];
+            if (i0 < n) {
+                float o[6];
 #pragma unroll
-            for (int c = 0; c < 6; ++c) o[c] = (float)((cxx * axx[c] + cxy * axy[c]) * (double)sc.back[c]);
-            gpos[sim * n + i] = make_float4(o[0], o[1], o[2], 0.f);
-            gvel[sim * n + i] = make_float4(o[3], o[4], o[5], 0.f);
+                for (int c = 0; c < 6; ++c) o[c] = (float)((cxx * axx0[c] + cxy * axy0[c]) * (double)sc.back[c]);
+                gpos[sim * n + i0] = make_float4(o[0], o[1], o[2], 0.f);
+                gvel[sim * n + i0] = make_float4(o[3], o[4], o[5], 0.f);
+            }
+            if (i1 < n) {
+                float o[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) o[c] = (float)((cxx * axx1[c] + cxy * axy1[c]) * (double)sc.back[c]);
+                gpos[sim * n + i1] = make_float4(o[0], o[1], o[2], 0.f);
+                gvel[sim * n + i1] = make_float4(o[3], o[4], o[5], 0.f);
+            }
         }
     }
-    // ---- observed point j = i against Y (value only) ----------------------------------------------------------
-    if (blockIdx.x * MMD_THREADS < m) {
-        float w[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        if (i < m) {
-            const float4 p = YP[i], v = YV[i];
-            w[0] = p.x * sc.s[0]; w[1] = p.y * sc.s[1]; w[2] = p.z * sc.s[2];
-            w[3] = v.x * sc.s[3]; w[4] = v.y * sc.s[4]; w[5] = v.z * sc.s[5];
-        }
-        double unused[6] = {0, 0, 0, 0, 0, 0};
-        syy = mmd_pass<false>(YP, YV, m, sc, w, tile, unused);
-        if (i >= m) syy = 0.0;
+    // ---- observed points against Y (value only) -------------------------------------------------------------------
+    if (base < m) {
+        f32x2 w[6];
+        load_pair(YP, YV, m, w);
+        double unused0[6] = {0, 0, 0, 0, 0, 0}, unused1[6] = {0, 0, 0, 0, 0, 0}, yy0, yy1;
+        mmd_pass<false>(YP, YV, m, sc, w, tileA, tileB, unused0, unused1, yy0, yy1);
+        syy = (i0 < m ? yy0 : 0.0) + (i1 < m ? yy1 : 0.0);
     }
     const double bxx = mmd_block_sum(sxx, warp_scratch);
     const double bxy = mmd_block_sum(sxy, warp_scratch);
@@ -171,7 +206,7 @@ mmd_final_kernel(const double* __restrict__ block_sums, const int nblocks, const
 size_t mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim)
 {
     const int64_t big = n > m ? n : m;
-    const size_t blocks = (size_t)((big + MMD_THREADS - 1) / MMD_THREADS);
+    const size_t blocks = (size_t)((big + MMD_PER_BLOCK - 1) / MMD_PER_BLOCK);
     return ((size_t)nsim * blocks * 3 * sizeof(double) + 255) & ~(size_t)255;
 }
 
@@ -186,7 +221,7 @@ cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, cons
         sc.back[c] = (float)(4.0 * s * 0.69314718055994530942);      // 4 ln2 s_d
     }
     const int64_t big = n > m ? n : m;
-    const dim3 grid((unsigned)((big + MMD_THREADS - 1) / MMD_THREADS), (unsigned)nsim);
+    const dim3 grid((unsigned)((big + MMD_PER_BLOCK - 1) / MMD_PER_BLOCK), (unsigned)nsim);
     double* block_sums = static_cast<double*>(ws);
     const float4* xp = reinterpret_cast<const float4*>(xpos);
     const float4* xv = reinterpret_cast<const float4*>(xvel);
