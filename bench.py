@@ -344,7 +344,7 @@ def _small_n_forms(B, W, torch, sizes=(256, 512, 1024, 2048, 4096), nsteps: int 
 
 def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: int = 10):
     """HBM roofline of the O(N) integrator kernel (reduce-free form: reads posm, vel, acc; writes posm, vel and
-    the staged sources = 96 B per particle in fp32) through odisseo_kick_drift_f32 at N = 2^24: 1.9 GB per
+    no staged copy = the 80 algorithmic B per particle in fp32) through odisseo_kick_drift_f32 at N = 2^24: 1.3 GB per
     launch, far larger than the 126 MB L2."""
     cfg = W.CONFIGS[3]
     g = torch.Generator(device="cuda").manual_seed(1234)
@@ -370,12 +370,12 @@ def _integrator_roofline(B, W, torch, peaks, peak_kind, n: int = 1 << 24, reps: 
         torch.cuda.synchronize()
         ts.append(a.elapsed_time(b))
     ms = float(np.mean(ts))
-    nbytes = 96.0 * n
+    nbytes = 80.0 * n
     gbs = nbytes / (ms * 1e-3) / 1e9
-    return {"kernel": "step_kernel<float> (kick + drift + NFW/MN + staging)", "n": n, "bound": "hbm",
-            "bytes_per_particle": 96, "launch_ms": ms, "launch_ms_stats": _stats(ts), "achieved": gbs,
+    return {"kernel": "step_kernel<float> (kick + drift + NFW/MN)", "n": n, "bound": "hbm",
+            "bytes_per_particle": 80, "launch_ms": ms, "launch_ms_stats": _stats(ts), "achieved": gbs,
             "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
-            # 96 B = SURVEY's 80 algorithmic bytes (posm, vel, acc in; posm, vel out) + the 16 B staged source record
+            # 80 B = SURVEY's algorithmic bytes (posm, vel, acc in; posm, vel out): the pair kernel reads posm itself, nothing is staged
             # this design writes for the next pair evaluation: a fraction of self-chosen bytes
             "bytes_per_particle_algorithmic": 80, "frac_on_algorithmic_bytes": 80.0 * n / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
             "peak_kind": peak_kind + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)"}

@@ -497,10 +497,10 @@ static cudaError_t pair_vjp_launch(const PairPlan& plan, const VjpCarve& cv, con
     const V4* c4 = reinterpret_cast<const V4*>(cot);
     if (with_eps_G) {
         const typename WithEG::Params prm{p4, c4, (T)(eps * eps)};
-        return launch_stream<WithEG>(plan, prm, cv.jsrc, cv.rows, stream);
+        return launch_stream<WithEG>(plan, prm, cv.jsrc, cv.jsrc, cv.rows, stream);
     }
     const typename Plain::Params prm{p4, c4, (T)(eps * eps)};
-    return launch_stream<Plain>(plan, prm, cv.jsrc, cv.rows, stream);
+    return launch_stream<Plain>(plan, prm, cv.jsrc, cv.jsrc, cv.rows, stream);
 }
 
 // Cotangent cot pulled back through a = a_pair + a_ext at posm (odisseo_accel_vjp_*): stage, O(N^2) pass, finish, final.

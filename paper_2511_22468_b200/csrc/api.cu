@@ -234,10 +234,12 @@ template <typename T> odisseo_status make_pot(T G, const odisseo_potential* pot,
 }
 
 // ---- typed launch shims ----------------------------------------------------------------
+// j: the workspace's staged array (flags in front of it); the tiles are copied from the targets' own array x when the plan
+// says so (plan.direct: no staged copy exists), else from j.
 inline cudaError_t launch_pair_raw(const PairPlan& p, const float* x, const void* j, double* part, float eps, cudaStream_t s)
-{ return launch_pair_f32(p, x, j, part, eps, s); }
+{ return launch_pair_f32(p, x, j, p.direct ? (const void*)x : j, part, eps, s); }
 inline cudaError_t launch_pair_raw(const PairPlan& p, const double* x, const void* j, double* part, double eps, cudaStream_t s)
-{ return launch_pair_f64(p, x, j, part, eps, s); }
+{ return launch_pair_f64(p, x, j, p.direct ? (const void*)x : j, part, eps, s); }
 // Pair-kernel launch; while a profile is open (and the stream is not capturing) it is bracketed
 // by a pair of CUDA events on the launching stream.
 template <typename T>
@@ -324,7 +326,8 @@ odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, voi
     DeviceInfo dev;
     st = device_info(dev);
     if (st != ODISSEO_OK) return st;
-    const PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    PairPlan plan = make_plan(n, sizeof(T) == 8, dev.sms);
+    plan.direct = 1;                               // the sources are the targets' own records: no staged copy, only the flags
     Carve cv;
     st = carve(plan, ws, ws_bytes, cv);
     if (st != ODISSEO_OK) return st;
@@ -332,7 +335,7 @@ odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, voi
     PotParams<T> nopot;
     memset(&nopot, 0, sizeof(nopot));
     cudaError_t e = launch_step(plan, const_cast<T*>(posm), (T*)nullptr, acc, cv.jsrc, cv.partials, G, nopot, (T)0,
-                                STEP_PACK_ONLY, s);
+                                STEP_PACK_ONLY | STEP_NO_STAGE, s);
     if (e != cudaSuccess) return cuda_fail(e);
     e = launch_pair(plan, posm, cv.jsrc, cv.partials, eps, s);
     if (e != cudaSuccess) return cuda_fail(e);
@@ -343,9 +346,9 @@ odisseo_status pair_accel_impl(const T* posm, T* acc, int64_t n, T G, T eps, voi
 }
 
 inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, const void* j, float G, float* a, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f32(p, part, j, G, a, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f32(p, part, j, j, G, a, s); }
 inline cudaError_t launch_reduce_rows(const PairPlan& p, const double* part, const void* j, double G, double* a, cudaStream_t s)
-{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f64(p, part, j, G, a, s); }
+{ g_launches.fetch_add(1, std::memory_order_relaxed); return launch_reduce_rows_f64(p, part, j, j, G, a, s); }
 
 // Acceleration at nt target positions due to n sources (targets need not be sources; their masses are ignored).
 template <typename T>
@@ -588,18 +591,23 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
     }
     // tape != nullptr (odisseo_leapfrog_kdk_tape_*): every step kernel also stores the synchronised snapshot
     // {x_k, v_k, pair-only a_k} it holds in registers at the moment between two steps -- no copies, no extra launch
+    // The per-step launches keep no staged copy of the sources: the pair kernel's TMA reads the particles' own records
+    // (plan.direct), and the step kernel writes posm, vel, acc and the equal-mass flags only (80 bytes per particle in fp32).
+    PairPlan dplan = plan;
+    dplan.direct = 1;
+    const int NS = STEP_NO_STAGE;
     const size_t snap = (size_t)n * 12;
     int first = 0;
     if (!acc_valid) {
-        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_PACK_ONLY, s));
-        ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
+        ODISSEO_TRY(launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_PACK_ONLY | NS, s));
+        ODISSEO_TRY(launch_pair(dplan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
         first = STEP_FROM_PARTIALS;
     }
     if (nsteps == 0) {
-        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | (tape ? STEP_SNAPSHOT : 0), s, tape));
+        ODISSEO_TRY(launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | (tape ? STEP_SNAPSHOT : 0) | NS, s, tape));
         return ODISSEO_OK;
     }
-    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN, s, tape));
+    ODISSEO_TRY(launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, first | STEP_OPEN | NS, s, tape));
 
     int64_t mid = nsteps - 1;     // full steps: pair + (close, open)
     // no graph on the legacy stream, inside a caller's capture, or while a profile is open
@@ -625,10 +633,10 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
             const int64_t counted = g_launches.load();   // captured launches run at replay, not now
             cudaError_t ce = cudaSuccess;
             for (int k = 0; k < block && ce == cudaSuccess; ++k) {
-                ce = launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s, true);
+                ce = launch_pair(dplan, (const T*)posm, cv.jsrc, cv.partials, eps, s, true);
                 if (ce == cudaSuccess)
-                    ce = launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
-                                     STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s);
+                    ce = launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
+                                     STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN | NS, s);
             }
             e = cudaStreamEndCapture(s, &graph);
             g_launches.store(counted);
@@ -653,12 +661,12 @@ odisseo_status leapfrog_impl(T* posm, T* vel, T* acc, int acc_valid, int64_t n, 
         }
     }
     for (; mid > 0; --mid) {
-        ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
-        ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
-                                STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN, s, tape ? tape + (size_t)(nsteps - mid) * snap : nullptr));
+        ODISSEO_TRY(launch_pair(dplan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
+        ODISSEO_TRY(launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt,
+                                STEP_FROM_PARTIALS | STEP_CLOSE | STEP_OPEN | NS, s, tape ? tape + (size_t)(nsteps - mid) * snap : nullptr));
     }
-    ODISSEO_TRY(launch_pair(plan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
-    ODISSEO_TRY(launch_step(plan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE, s,
+    ODISSEO_TRY(launch_pair(dplan, (const T*)posm, cv.jsrc, cv.partials, eps, s));
+    ODISSEO_TRY(launch_step(dplan, posm, vel, acc, cv.jsrc, cv.partials, G, pp, dt, STEP_FROM_PARTIALS | STEP_CLOSE | NS, s,
                             tape ? tape + (size_t)nsteps * snap : nullptr));
     return ODISSEO_OK;
 }
@@ -686,7 +694,8 @@ odisseo_status kick_drift_impl(T* posm, T* vel, const T* acc, int64_t n, T G, T 
     Carve cv;
     st = carve(plan, ws, ws_bytes, cv);
     if (st != ODISSEO_OK) return st;
-    const int flags = ((mode & 1) ? STEP_CLOSE : 0) | ((mode & 2) ? STEP_OPEN : 0);
+    // no staged copy: odisseo_pair_accel_* reads the particles' own records (the equal-mass flags are still refreshed)
+    const int flags = ((mode & 1) ? STEP_CLOSE : 0) | ((mode & 2) ? STEP_OPEN : 0) | STEP_NO_STAGE;
     cudaError_t e = launch_step(plan, posm, vel, const_cast<T*>(acc), cv.jsrc, cv.partials, G, pp, dt, flags,
                                 static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e);

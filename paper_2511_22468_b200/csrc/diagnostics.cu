@@ -95,7 +95,7 @@ diag_terms_kernel(const typename DVec4<T>::type* __restrict__ posm, const typena
         const double x = p.x, y = p.y, z = p.z, m = p.w, vx = w.x, vy = w.y, vz = w.z;
         double rows[1];
         reduce_unit_rows<1>(partials, plan, i, rows);                    // increasing j, fixed grouping
-        const double sum = plan_row_mass<double>(jsrc, plan) * rows[0];
+        const double sum = plan_row_mass<double>(jsrc, plan, jsrc) * rows[0];
         const double phi = -G * (sum - m / eps);       // the kernel's self term is m_i (0 + eps^2)^-1/2
         if (phi_out) phi_out[i] = phi;
         val[0] = 0.5 * m * fma(vx, vx, fma(vy, vy, vz * vz));

@@ -51,13 +51,13 @@ step_kernel(typename Vec4<T>::type* __restrict__ posm, typename Vec4<T>::type* _
 // Fixed-order row reduce alone (cross call: the targets are not the staged sources): acc_i = G * sum of rows.
 template <typename T>
 __global__ void __launch_bounds__(STEP_THREADS)
-reduce_rows_kernel(const double* __restrict__ partials, const void* __restrict__ jsrc, const PairPlan plan, const T G,
-                   typename Vec4<T>::type* __restrict__ acc)
+reduce_rows_kernel(const double* __restrict__ partials, const void* __restrict__ jsrc, const void* __restrict__ records,
+                   const PairPlan plan, const T G, typename Vec4<T>::type* __restrict__ acc)
 {
     pdl_wait();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= plan.nt) return;
-    const double gm = (double)G * plan_row_mass<T>(jsrc, plan);
+    const double gm = (double)G * plan_row_mass<T>(jsrc, plan, records);
     double sum[3];
     reduce_unit_rows<3>(partials, plan, i, sum);
     typename Vec4<T>::type a;
@@ -135,16 +135,16 @@ cudaError_t launch_step_f64(const PairPlan& plan, double* posm, double* vel, dou
                       reinterpret_cast<V4*>(acc), jsrc, partials, plan, G, pot, dt, flags, reinterpret_cast<V4*>(snapshot), lo, count);
 }
 
-cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,
-                                   cudaStream_t stream)
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, const void* records, float G,
+                                   float* acc, cudaStream_t stream)
 {
-    return launch_pdl(reduce_rows_kernel<float>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, plan, G,
+    return launch_pdl(reduce_rows_kernel<float>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, records, plan, G,
                       reinterpret_cast<float4*>(acc));
 }
-cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, double G, double* acc,
-                                   cudaStream_t stream)
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, const void* records, double G,
+                                   double* acc, cudaStream_t stream)
 {
-    return launch_pdl(reduce_rows_kernel<double>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, plan, G,
+    return launch_pdl(reduce_rows_kernel<double>, dim3(grid_for(plan.nt)), dim3(STEP_THREADS), 0, stream, partials, jsrc, records, plan, G,
                       reinterpret_cast<double4*>(acc));
 }
 

@@ -40,6 +40,7 @@ struct PairPlan {
     int32_t variant;  // 0 = large (8 compute warps), 1 = small (2 compute warps)
     int32_t rec_bytes;// bytes per staged source record
     int32_t comps;    // planes of IB doubles per row (3: x, y, z sums)
+    int32_t direct;   // 1: the sources are read from the caller's posm array itself (n records, no padding): the last tile ends at n
 };
 
 __host__ __device__ __forceinline__ int64_t plan_start(const PairPlan& p, int64_t c) {
@@ -135,13 +136,14 @@ __device__ __forceinline__ void reduce_unit_rows(const double* __restrict__ part
     }
 }
 // Factor the pair kernel left out of the rows: the common mass when it took the equal-mass loop, else 1.
+// records: the array the pair kernel read its sources from (the staged array, or posm itself when plan.direct).
 template <typename T>
-__device__ __forceinline__ double plan_row_mass(const void* __restrict__ jsrc, const PairPlan& plan)
+__device__ __forceinline__ double plan_row_mass(const void* __restrict__ jsrc, const PairPlan& plan, const void* __restrict__ records)
 {
     // both loads are issued unconditionally (no dependent round trip: at small N the reduce is latency-bound)
     const int eqm = __ldcg(plan_eqm_word(jsrc, plan));
-    // mass of staged record 0 ({x, y, z, m} in both precisions)
-    const double m0 = sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(jsrc) + 3) : __ldcg(static_cast<const double*>(jsrc) + 3);
+    // mass of source record 0 ({x, y, z, m} in both precisions)
+    const double m0 = sizeof(T) == 4 ? (double)__ldcg(static_cast<const float*>(records) + 3) : __ldcg(static_cast<const double*>(records) + 3);
     return eqm != 0 ? m0 : 1.0;
 }
 #endif
@@ -178,7 +180,8 @@ enum : int {
     STEP_OPEN = 4,            // opening half kick + drift: v += a dt/2; x += v dt (start of next step)
     STEP_PACK_ONLY = 8,       // only (re)write the staged source array from posm
     STEP_SNAPSHOT = 16,       // no kick: only store the tape snapshot {x, v, pair-only a} (nsteps == 0 with a tape)
-    STEP_SLICE = 32           // the arrays address a slice [lo, lo + count) of the plan's particles (sharded form)
+    STEP_SLICE = 32,          // the arrays address a slice [lo, lo + count) of the plan's particles (sharded form)
+    STEP_NO_STAGE = 64        // write the equal-mass flags but no staged records: the pair kernel reads posm itself (plan.direct)
 };
 
 // ---------------------------------------------------------------------------------------
@@ -308,9 +311,9 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 #endif
 
 // launchers (defined in pair_f32.cu / pair_f64.cu / integrate.cu)
-cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials,
+cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, const void* src, double* partials,
                             float eps, cudaStream_t stream);
-cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials,
+cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, const void* src, double* partials,
                             double eps, cudaStream_t stream);
 cudaError_t launch_step_f32(const PairPlan& plan, float* posm, float* vel, float* acc, void* jsrc,
                             const double* partials, float G, const PotParams<float>& pot, float dt, int flags,
@@ -325,10 +328,10 @@ cudaError_t launch_ext_f64(const double* posm, double* acc, int64_t n, const Pot
 cudaError_t launch_soa_pack_f32(const float* x, const float* y, const float* z, const float* m, float* posm,
                                 int64_t n, cudaStream_t stream);
 cudaError_t launch_soa_unpack_f32(const float* acc, float* ax, float* ay, float* az, int64_t n, cudaStream_t stream);
-cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, float G, float* acc,
-                                   cudaStream_t stream);
-cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, double G, double* acc,
-                                   cudaStream_t stream);
+cudaError_t launch_reduce_rows_f32(const PairPlan& plan, const double* partials, const void* jsrc, const void* records, float G,
+                                   float* acc, cudaStream_t stream);
+cudaError_t launch_reduce_rows_f64(const PairPlan& plan, const double* partials, const void* jsrc, const void* records, double G,
+                                   double* acc, cudaStream_t stream);
 cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double* partials, double eps,
                                  cudaStream_t stream);
 // diagnostics.cu: stage (promote to double) / per-particle terms + block sums / final fixed-order sum

@@ -240,15 +240,15 @@ cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* 
     return launch_ll<LLF32, float>(ca, ctas, smem, LL_TAPE_CODE_FLOAT, stream);
 }
 
-cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, double* partials, float eps,
+cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, const void* src, double* partials, float eps,
                             cudaStream_t stream)
 {
     if (plan.variant == 0) {
         const LargeF32::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
-        return launch_stream<LargeF32>(plan, prm, jsrc, partials, stream);
+        return launch_stream<LargeF32>(plan, prm, jsrc, src, partials, stream);
     }
     const SmallF32::Params prm{reinterpret_cast<const float4*>(posm), eps * eps};
-    return launch_stream<SmallF32>(plan, prm, jsrc, partials, stream);
+    return launch_stream<SmallF32>(plan, prm, jsrc, src, partials, stream);
 }
 
 }  // namespace odisseo

@@ -218,12 +218,12 @@ cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, doubl
     return launch_ll<LLF64, double>(ca, ctas, smem, LL_TAPE_CODE_DOUBLE, stream);
 }
 
-cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, double* partials, double eps,
+cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, const void* src, double* partials, double eps,
                             cudaStream_t stream)
 {
     const LargeF64::Params prm{reinterpret_cast<const double4*>(posm), eps * eps};
-    if (plan.variant == 0) return launch_stream<LargeF64>(plan, prm, jsrc, partials, stream);
-    return launch_stream<SmallF64>(plan, SmallF64::Params{prm.posm, prm.eps2}, jsrc, partials, stream);
+    if (plan.variant == 0) return launch_stream<LargeF64>(plan, prm, jsrc, src, partials, stream);
+    return launch_stream<SmallF64>(plan, SmallF64::Params{prm.posm, prm.eps2}, jsrc, src, partials, stream);
 }
 
 // Softened potential sums phi'_i = sum_j m_j (r_ij^2 + eps^2)^-1/2 (self term included) into the x-plane of
@@ -232,8 +232,8 @@ cudaError_t launch_potential_f64(const PairPlan& plan, const void* jsrc, double*
                                  cudaStream_t stream)
 {
     const double4* targets = static_cast<const double4*>(jsrc);
-    if (plan.variant == 0) return launch_stream<LargePot>(plan, LargePot::Params{targets, eps * eps}, jsrc, partials, stream);
-    return launch_stream<SmallPot>(plan, SmallPot::Params{targets, eps * eps}, jsrc, partials, stream);
+    if (plan.variant == 0) return launch_stream<LargePot>(plan, LargePot::Params{targets, eps * eps}, jsrc, jsrc, partials, stream);
+    return launch_stream<SmallPot>(plan, SmallPot::Params{targets, eps * eps}, jsrc, jsrc, partials, stream);
 }
 
 }  // namespace odisseo

@@ -34,7 +34,7 @@ constexpr int STAGES = 4;
 // The tile sequence of one CTA: units [u0, u1); unit u = chunk s = u % S of i-block b = u / S; the chunk's
 // records [lo, hi) are cut into tiles of at most T records.  Producer and consumers run the same walk.
 struct TileWalk {
-    int64_t u, u1, j, hi, n8;
+    int64_t u, u1, j, hi, n8, nlim;
     int32_t T, S, b, s;
     __device__ __forceinline__ void set_unit()
     {
@@ -42,9 +42,10 @@ struct TileWalk {
         s = (int32_t)(u - (int64_t)b * S);
         j = 8 * (((int64_t)s * n8) / S);
         hi = 8 * (((int64_t)(s + 1) * n8) / S);
+        hi = hi < nlim ? hi : nlim;                       // sources read from posm itself end at n, not at the padding
     }
     __device__ __forceinline__ TileWalk(const PairPlan& p, int64_t u0_, int64_t u1_)
-        : u(u0_), u1(u1_), j(0), hi(0), n8(p.n8), T(p.T), S(p.S), b(0), s(0)
+        : u(u0_), u1(u1_), j(0), hi(0), n8(p.n8), nlim(p.direct ? p.n : 8 * p.n8), T(p.T), S(p.S), b(0), s(0)
     {
         if (u < u1) set_unit();
     }
@@ -92,7 +93,8 @@ __device__ __forceinline__ void consume_units(const typename C::Params& prm, dou
 
 template <class C>
 __global__ void __launch_bounds__((C::CWARPS + 1) * 32, C::MINB)
-stream_kernel(const typename C::Params prm, const unsigned char* __restrict__ jsrc, double* __restrict__ rows, const PairPlan plan)
+stream_kernel(const typename C::Params prm, const unsigned char* __restrict__ jsrc, const unsigned char* __restrict__ src,
+              double* __restrict__ rows, const PairPlan plan)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t full_bar[STAGES];
@@ -129,7 +131,7 @@ stream_kernel(const typename C::Params prm, const unsigned char* __restrict__ js
         for (; prefetch < STAGES && pw.valid(); ++prefetch) {
             const uint32_t bytes = (uint32_t)pw.len() * C::REC;
             mbar_arrive_expect_tx(&full_bar[prefetch], bytes);
-            tma_load_1d(smem_raw + (size_t)prefetch * stage_bytes, jsrc + (size_t)pw.j * C::REC, bytes, &full_bar[prefetch]);
+            tma_load_1d(smem_raw + (size_t)prefetch * stage_bytes, src + (size_t)pw.j * C::REC, bytes, &full_bar[prefetch]);
             pw.next();
         }
     }
@@ -152,7 +154,7 @@ stream_kernel(const typename C::Params prm, const unsigned char* __restrict__ js
                 mbar_wait_backoff(&empty_bar[s], ph ^ 1u);
                 const uint32_t bytes = (uint32_t)pw.len() * C::REC;
                 mbar_arrive_expect_tx(&full_bar[s], bytes);
-                tma_load_1d(smem_raw + (size_t)s * stage_bytes, jsrc + (size_t)pw.j * C::REC, bytes, &full_bar[s]);
+                tma_load_1d(smem_raw + (size_t)s * stage_bytes, src + (size_t)pw.j * C::REC, bytes, &full_bar[s]);
                 if (++s == STAGES) { s = 0; ph ^= 1u; }
             }
         }
@@ -176,10 +178,13 @@ template <class C> cudaError_t configure_stream(int max_tile)
 }
 
 template <class C>
-cudaError_t launch_stream(const PairPlan& plan, const typename C::Params& prm, const void* jsrc, double* rows, cudaStream_t stream)
+// jsrc: the workspace's staged array (the flags sit in front of it); src: the records the tiles are copied from (jsrc, or
+// the caller's posm array when plan.direct).
+cudaError_t launch_stream(const PairPlan& plan, const typename C::Params& prm, const void* jsrc, const void* src, double* rows,
+                          cudaStream_t stream)
 {
     return launch_pdl(stream_kernel<C>, dim3(plan.P), dim3((C::CWARPS + 1) * 32), stream_smem_bytes<C>(plan), stream, prm,
-                      static_cast<const unsigned char*>(jsrc), rows, plan);
+                      static_cast<const unsigned char*>(jsrc), static_cast<const unsigned char*>(src), rows, plan);
 }
 
 }  // namespace odisseo

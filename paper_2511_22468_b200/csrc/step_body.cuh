@@ -48,17 +48,18 @@ __device__ __forceinline__ int step_particle(typename Vec4<T>::type* __restrict_
     typedef typename Vec4<T>::type V4;
     const bool staging = (flags & (STEP_OPEN | STEP_PACK_ONLY)) != 0;
     const bool flagging = staging && !(flags & STEP_SLICE);
+    const bool records = !(flags & STEP_NO_STAGE);                      // the pair kernel reads posm itself otherwise (plan.direct)
     int mass_differs = 0;
     if (i < count) {
         const T mass0 = reinterpret_cast<const T*>(posm)[3];            // masses are never modified
         V4 p = posm[i];
         if (flags & STEP_PACK_ONLY) {
-            stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
+            if (records) stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
         } else {
             T apx, apy, apz;
             if (REDUCE) {
                 // fixed order: the S rows of this i-block in increasing s, then the factors left out of the rows
-                const double gm = (double)G * plan_row_mass<T>(jsrc, plan);       // loads in flight with the rows'
+                const double gm = (double)G * plan_row_mass<T>(jsrc, plan, plan.direct ? (const void*)posm : (const void*)jsrc);   // loads in flight with the rows'
                 double sum[3];
                 reduce_unit_rows<3>(partials, plan, i, sum);
                 const double sx = sum[0], sy = sum[1], sz = sum[2];
@@ -93,14 +94,14 @@ __device__ __forceinline__ int step_particle(typename Vec4<T>::type* __restrict_
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
                     p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
                     posm[i] = p;
-                    stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
+                    if (records) stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
                 }
                 v.w = (T)0;
                 vel[i] = v;
             }
         }
         if (flagging) mass_differs = !(p.w == mass0);               // NaN counts as different
-    } else if (staging && lo + count == plan.n && lo + i < plan_npad(plan)) {
+    } else if (staging && records && lo + count == plan.n && lo + i < plan_npad(plan)) {
         const T far = pad_pos((T)0);                                    // whoever holds the last particle pads the tail
         stage_record(jsrc, lo + i, far, far, far, (T)0);
     }
