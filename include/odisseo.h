@@ -116,7 +116,8 @@ int64_t odisseo_set_ll_max_n(int64_t n);
 odisseo_status odisseo_shutdown(void);
 
 /* Upper bound, in bytes, of the device scratch any pair/leapfrog call on n particles
- * needs (staged source records + one row of fixed-order partial sums per work unit; for n <= 6,144 the row area
+ * needs (room for staged source records -- used by the cross, sharded and cooperative forms only; the default path
+ * reads the particles' own records -- + one row of fixed-order partial sums per work unit; for n <= 6,144 the row area
  * is at least 96 (n + 1) bytes, the exchange words of the small-n whole-loop kernel).
  * is_f64 != 0 for the fp64 calls.  Returns 0 for n <= 0.  With a current CUDA device the
  * bound is the one for that device's SM count; without one (no GPU) it is the maximum over
@@ -218,8 +219,9 @@ odisseo_status odisseo_leapfrog_kdk_f64(double *d_posm, double *d_vel, double *d
 /* The O(N) integrator kernel on its own (SURVEY.md 8a rows a2 + a3): given the
  * pair-only acceleration in d_acc (input, unchanged), with a = d_acc + a_NFW(x) + a_MN(x):
  *   mode & 1: closing half kick          v += a dt/2
- *   mode & 2: opening half kick + drift  v += a dt/2 ; x += v dt   (a evaluated BEFORE the drift),
- *             and the moved sources are staged into the workspace for the next pair evaluation.
+ *   mode & 2: opening half kick + drift  v += a dt/2 ; x += v dt   (a evaluated BEFORE the drift).
+ * Nothing is staged: odisseo_pair_accel_* and the leapfrog read the particles' own {x,y,z,m} records (the
+ * workspace only receives the equal-mass flags), so the launch moves the 80 algorithmic bytes per particle in fp32.
  * mode 3 = the kernel a full leapfrog step launches between two pair evaluations.  This is the launch
  * bench.py times for the integrator's HBM roofline; it is also the building block for callers that
  * obtain pair accelerations elsewhere.  Workspace as for odisseo_pair_accel_*.  mode outside 1..3 ->
