@@ -57,7 +57,8 @@ typedef enum {
     ODISSEO_ERR_ARG = 3,
     ODISSEO_ERR_WORKSPACE = 4,
     ODISSEO_ERR_ARCH = 5,
-    ODISSEO_ERR_CUDA = 6
+    ODISSEO_ERR_CUDA = 6,
+    ODISSEO_ERR_STATIC_LIMIT = 7   /* the problem needs more scratch than odisseo_mmd2_static_scratch_bytes() */
 } odisseo_status;
 
 /* NFW: Phi = -G M_s ln(1 + r/r_s) / r, i.e. M_s = 4 pi rho_0 r_s^3 (reading R10).
@@ -374,6 +375,30 @@ odisseo_status odisseo_mmd2_f32(const float *d_xpos, const float *d_xvel, int64_
                                 int64_t m, int64_t nsim, int shared_y, const double *h_sigma, const double *d_grad_scale,
                                 double *d_mmd2, float *d_gpos, float *d_gvel, void *d_workspace, size_t workspace_bytes,
                                 void *stream);
+
+/* odisseo_mmd2_f32 for callers that cannot allocate device memory (same operation and passages: Fig. 2
+ * step 4, L47; reading R20).  odisseo_mmd2_f32 needs a workspace for its per-block sums, and somebody has to
+ * cudaMalloc it.  Two kinds of caller cannot: code living inside a host program whose own memory pool took the whole
+ * HBM at start-up (a loss called from a JAX or PyTorch process is the usual case here, and a cudaMalloc next to such a
+ * pool can simply fail), and code in a region where allocation is ruled out because cudaMalloc / cudaFree stall every
+ * stream of the device (an optimisation loop that must not hiccup, a plug-in whose host forbids it).  This entry
+ * point takes inputs and outputs only and calls no cudaMalloc, cudaFree or allocating library routine: the block sums
+ * go to a fixed array of odisseo_mmd2_static_scratch_bytes() = 1 MiB that is part of the library image (every GPU
+ * that loads the library holds it until the process exits).
+ *   Arguments, layouts, validation, results: exactly those of odisseo_mmd2_f32 without d_workspace / workspace_bytes;
+ *     the same two kernels run, so the outputs are bit-identical to odisseo_mmd2_f32's.
+ *   Limit: odisseo_mmd_workspace_bytes(n, m, nsim) = 24 * nsim * ceil(max(n, m) / 512) bytes (rounded up to 256)
+ *     must not exceed odisseo_mmd2_static_scratch_bytes(); otherwise ODISSEO_ERR_STATIC_LIMIT and nothing is
+ *     launched (2,960 clouds of 1,000 points need 139 KiB; 43,690 cloud-blocks fit).  Use odisseo_mmd2_f32 beyond it.
+ *   First call on each device: looks up the array's device address (with that device current) and keeps it; make
+ *     this first call before any stream capture begins.  Later calls only launch.
+ *   Sharing: every call on a device uses the same array.  Nothing in it has to be cleared -- each call overwrites the
+ *     sums it later reads -- but two calls that overlap on the GPU (different streams, or threads, without an
+ *     ordering between them) race on it and corrupt each other's d_mmd2.  Calls on one stream are safe. */
+size_t odisseo_mmd2_static_scratch_bytes(void);
+odisseo_status odisseo_mmd2_static_f32(const float *d_xpos, const float *d_xvel, int64_t n, const float *d_ypos,
+                                       const float *d_yvel, int64_t m, int64_t nsim, int shared_y, const double *h_sigma,
+                                       const double *d_grad_scale, double *d_mmd2, float *d_gpos, float *d_gvel, void *stream);
 
 /* Instrumentation (bench.py's gpu_launches and roofline legs).
  *   odisseo_launch_count: kernels this library has launched in this process so far (a CUDA

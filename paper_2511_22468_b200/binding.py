@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libodisseo_b200.so")
 _lib = None
 
-STATUS = {0: "OK", 1: "ERR_NULL", 2: "ERR_ALIGN", 3: "ERR_ARG", 4: "ERR_WORKSPACE", 5: "ERR_ARCH", 6: "ERR_CUDA"}
+STATUS = {0: "OK", 1: "ERR_NULL", 2: "ERR_ALIGN", 3: "ERR_ARG", 4: "ERR_WORKSPACE", 5: "ERR_ARCH", 6: "ERR_CUDA",
+          7: "ERR_STATIC_LIMIT"}
 
 EXPORTS = [
     "odisseo_version", "odisseo_status_string", "odisseo_last_cuda_error", "odisseo_workspace_bytes",
@@ -34,7 +35,8 @@ EXPORTS = [
     "odisseo_ensemble_leapfrog_kdk_vjp_f32", "odisseo_cross_workspace_bytes", "odisseo_pair_accel_cross_f32",
     "odisseo_pair_accel_cross_f64", "odisseo_staged_sources_layout", "odisseo_stage_sources_f32", "odisseo_stage_sources_f64",
     "odisseo_pair_accel_staged_f32", "odisseo_pair_accel_staged_f64", "odisseo_kick_drift_slice_f32",
-    "odisseo_kick_drift_slice_f64", "odisseo_mmd_workspace_bytes", "odisseo_mmd2_f32", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
+    "odisseo_kick_drift_slice_f64", "odisseo_mmd_workspace_bytes", "odisseo_mmd2_f32",
+    "odisseo_mmd2_static_scratch_bytes", "odisseo_mmd2_static_f32", "odisseo_ubench_kinds", "odisseo_ubench_name", "odisseo_ubench_run",
 ]
 
 
@@ -113,6 +115,9 @@ def lib():
         L.odisseo_mmd_workspace_bytes.restype = sz
         L.odisseo_mmd_workspace_bytes.argtypes = [i64, i64, i64]
         L.odisseo_mmd2_f32.argtypes = [vp, vp, i64, vp, vp, i64, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.odisseo_mmd2_static_scratch_bytes.restype = sz
+        L.odisseo_mmd2_static_scratch_bytes.argtypes = []
+        L.odisseo_mmd2_static_f32.argtypes = [vp, vp, i64, vp, vp, i64, i64, ci, vp, vp, vp, vp, vp, vp]
         L.odisseo_cross_workspace_bytes.restype = sz
         L.odisseo_cross_workspace_bytes.argtypes = [i64, i64, ci]
         L.odisseo_pair_accel_soa_f32.argtypes = [vp] * 7 + [i64, f, f, vp, sz, vp]
@@ -580,6 +585,54 @@ def mmd2(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch
                                   grad_scale.data_ptr() if grad_scale is not None else None, out.data_ptr(),
                                   gpos.data_ptr() if gpos is not None else None, gvel.data_ptr() if gvel is not None else None,
                                   workspace.data_ptr(), workspace.numel(), _stream(stream)), "mmd2_f32")
+
+
+def mmd2_static_scratch_bytes() -> int:
+    """Size of the library's built-in scratch array; mmd2_static refuses calls whose mmd_workspace_bytes exceed it."""
+    return int(lib().odisseo_mmd2_static_scratch_bytes())
+
+
+@_on_device
+def mmd2_static(xpos: torch.Tensor, xvel: torch.Tensor, ypos: torch.Tensor, yvel: torch.Tensor, sigma: Sequence[float],
+                out: torch.Tensor, gpos: Optional[torch.Tensor] = None, gvel: Optional[torch.Tensor] = None,
+                grad_scale: Optional[torch.Tensor] = None, stream=None):
+    """mmd2 without a workspace tensor (odisseo_mmd2_static_f32), for callers that must not allocate device memory:
+    a loss evaluated inside a process whose memory pool already owns the HBM, or inside a loop where the stall of a
+    cudaMalloc is not acceptable.  You pass inputs and outputs you already hold; the per-block sums go to a 1 MiB
+    array built into the library, and neither this wrapper nor the call under it allocates on the device.  Same
+    arguments and bit-identical results as mmd2.  Raises OdisseoError (ERR_STATIC_LIMIT) when
+    mmd_workspace_bytes(n, m, nsim) > mmd2_static_scratch_bytes().  The first call on a device also looks up the
+    array's address: make it before any stream capture.  All calls on a device share the array, so calls that
+    overlap on the GPU (two streams with no ordering between them) corrupt each other; calls on one stream are fine."""
+    if xpos.dim() == 2:
+        xpos, xvel = xpos.unsqueeze(0), xvel.unsqueeze(0)
+        if gpos is not None:
+            gpos, gvel = gpos.unsqueeze(0), gvel.unsqueeze(0)
+    nsim, n = _ens_state(xpos, xvel, "xpos and xvel")
+    shared = ypos.dim() == 2
+    if shared:
+        m = _rec(ypos, "ypos")
+        _rec(yvel, "yvel", m)
+        if ypos.dtype != torch.float32 or yvel.dtype != torch.float32:
+            raise TypeError("mmd2_static is float32")
+    else:
+        ns2, m = _ens_state(ypos, yvel, "ypos and yvel")
+        if ns2 != nsim:
+            raise ValueError("ypos holds %d clouds, expected 1 shared or %d" % (ns2, nsim))
+    _f64vec(out, "out", nsim)
+    if (gpos is None) != (gvel is None):
+        raise ValueError("gpos and gvel go together")
+    if gpos is not None:
+        ng, nn = _ens_state(gpos, gvel, "gpos and gvel")
+        if (ng, nn) != (nsim, n):
+            raise ValueError("gpos/gvel must match xpos/xvel")
+    if grad_scale is not None:
+        _f64vec(grad_scale, "grad_scale", nsim)
+    sig = (ctypes.c_double * 6)(*[float(v) for v in sigma])
+    _check(lib().odisseo_mmd2_static_f32(xpos.data_ptr(), xvel.data_ptr(), n, ypos.data_ptr(), yvel.data_ptr(), m, nsim,
+                                         int(shared), sig, grad_scale.data_ptr() if grad_scale is not None else None,
+                                         out.data_ptr(), gpos.data_ptr() if gpos is not None else None,
+                                         gvel.data_ptr() if gvel is not None else None, _stream(stream)), "mmd2_static_f32")
 
 
 def set_fused_max_n(n: int) -> int:

@@ -909,6 +909,9 @@ const char* odisseo_status_string(odisseo_status s)
         case ODISSEO_ERR_WORKSPACE: return "workspace too small";
         case ODISSEO_ERR_ARCH: return "device is not compute capability 10.x (B200)";
         case ODISSEO_ERR_CUDA: return "CUDA error (see odisseo_last_cuda_error)";
+        case ODISSEO_ERR_STATIC_LIMIT:
+            return "problem too large for the library's built-in scratch array (odisseo_mmd2_static_scratch_bytes); "
+                   "use the call that takes a workspace";
     }
     return "unknown status";
 }
@@ -1409,6 +1412,39 @@ odisseo_status odisseo_mmd2_f32(const float* d_xpos, const float* d_xvel, int64_
     cudaError_t e = launch_mmd_f32(d_xpos, d_xvel, n, d_ypos, d_yvel, m, shared_y != 0, inv, nsim, d_grad_scale, d_mmd2, d_gpos,
                                    d_gvel, d_workspace, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return cuda_fail(e);
+    return ODISSEO_OK;
+}
+
+size_t odisseo_mmd2_static_scratch_bytes(void) { return mmd_static_scratch_bytes(); }
+
+// odisseo_mmd2_f32 without a workspace argument (include/odisseo.h): for callers that cannot cudaMalloc one.  The
+// checks are those of odisseo_mmd2_f32; the size test is against the built-in array instead of the caller's bytes.
+odisseo_status odisseo_mmd2_static_f32(const float* d_xpos, const float* d_xvel, int64_t n, const float* d_ypos,
+                                       const float* d_yvel, int64_t m, int64_t nsim, int shared_y, const double* h_sigma,
+                                       const double* d_grad_scale, double* d_mmd2, float* d_gpos, float* d_gvel, void* stream)
+{
+    if (n < 0 || m < 0 || nsim < 0 || n > 0x7fffffff || m > 0x7fffffff || nsim > 65535) return ODISSEO_ERR_ARG;
+    if (nsim == 0) return ODISSEO_OK;
+    if (n == 0 || m == 0) return ODISSEO_ERR_ARG;
+    if (!d_xpos || !d_xvel || !d_ypos || !d_yvel || !h_sigma || !d_mmd2) return ODISSEO_ERR_NULL;
+    if ((d_gpos == nullptr) != (d_gvel == nullptr)) return ODISSEO_ERR_NULL;
+    if (misaligned(d_xpos, 16) || misaligned(d_xvel, 16) || misaligned(d_ypos, 16) || misaligned(d_yvel, 16) ||
+        misaligned(d_mmd2, 8) || (d_gpos && (misaligned(d_gpos, 16) || misaligned(d_gvel, 16))) ||
+        (d_grad_scale && misaligned(d_grad_scale, 8)))
+        return ODISSEO_ERR_ALIGN;
+    double inv[6];
+    for (int c = 0; c < 6; ++c) {
+        if (!(h_sigma[c] > 0.0) || !isfinite(h_sigma[c])) return ODISSEO_ERR_ARG;
+        inv[c] = 1.0 / h_sigma[c];
+    }
+    if (mmd_workspace_bytes(n, m, nsim) > mmd_static_scratch_bytes()) return ODISSEO_ERR_STATIC_LIMIT;
+    DeviceInfo dev;
+    odisseo_status st = device_info(dev);
+    if (st != ODISSEO_OK) return st;
+    cudaError_t e = launch_mmd_f32_static(d_xpos, d_xvel, n, d_ypos, d_yvel, m, shared_y != 0, inv, nsim, d_grad_scale, d_mmd2,
+                                          d_gpos, d_gvel, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(e);
+    g_launches.fetch_add(2, std::memory_order_relaxed);
     return ODISSEO_OK;
 }
 

@@ -16,6 +16,8 @@
 // broadcast operand of the packed instructions); sums are fp32 inside a tile and fp64 across tiles; per-block sums are added
 // in block order by a second kernel (fixed order, no atomics: bit-reproducible).  The gradient lands in the layout of
 // the pull-back's cotangents (float4 {d/dx, d/dy, d/dz, 0}), so loss -> gradient never leaves the device.
+#include <mutex>
+
 #include "odisseo_common.cuh"
 
 namespace odisseo {
@@ -237,6 +239,61 @@ cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, cons
     if (e != cudaSuccess) return e;
     mmd_final_kernel<<<(unsigned)((nsim + 31) / 32), 32, 0, stream>>>(block_sums, (int)grid.x, nsim, (int)n, (int)m, mmd2);
     return cudaGetLastError();
+}
+
+// ---- MMD^2 with the library's own scratch (odisseo_mmd2_static_f32) ------------------------------------------------------
+// The per-block sums of mmd_kernel normally live in a workspace the caller allocates.  Some callers have no way to do
+// that: a loss evaluated from inside a host program whose own memory pool already holds the whole HBM (an ML
+// framework that reserves the device at start-up is the usual case for this library's users), or from a code region
+// whose rules forbid cudaMalloc because it stalls every stream of the device.  For them the same two kernels run on
+// this array instead.  It is part of the library image: every GPU that loads the library holds these bytes until the
+// process exits, which is why the size is kept small; problems that need more are refused, not truncated.
+constexpr size_t MMD_STATIC_BYTES = (size_t)1 << 20;
+static __device__ __align__(256) unsigned char g_mmd_static_scratch[MMD_STATIC_BYTES];
+
+namespace {
+
+// In host code the name g_mmd_static_scratch is only the handle the runtime looks the array up by -- it is NOT the
+// address the GPU sees, and must never be handed to a kernel.  The device address is asked for once per device, with
+// that device current, and remembered here.
+constexpr int MMD_STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+void* g_static_ptr[MMD_STATIC_MAX_DEVICES] = {};
+
+cudaError_t mmd_static_scratch(void** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);                     // the device the caller made current owns the launch
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MMD_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[dev] == nullptr) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_mmd_static_scratch);  // this device's copy of the array
+        if (e != cudaSuccess) return e;
+        if (p == nullptr) return cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+size_t mmd_static_scratch_bytes() { return MMD_STATIC_BYTES; }
+
+// Same launches as launch_mmd_f32 on the array above; the caller has checked mmd_workspace_bytes(n, m, nsim) against
+// mmd_static_scratch_bytes().  Nothing in the array has to start at zero: every block of mmd_kernel stores its three
+// sums before mmd_final_kernel (same stream, later) reads exactly those, so what an earlier call left behind is
+// never read.  No cudaMalloc / cudaFree here or below.
+cudaError_t launch_mmd_f32_static(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel,
+                                  int64_t m, int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale,
+                                  double* mmd2, float* gpos, float* gvel, cudaStream_t stream)
+{
+    void* scratch = nullptr;
+    const cudaError_t e = mmd_static_scratch(&scratch);
+    if (e != cudaSuccess) return e;
+    return launch_mmd_f32(xpos, xvel, n, ypos, yvel, m, shared_y, inv_sigma, nsim, grad_scale, mmd2, gpos, gvel, scratch, stream);
 }
 
 }  // namespace odisseo

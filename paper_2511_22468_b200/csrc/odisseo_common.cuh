@@ -372,6 +372,10 @@ size_t mmd_workspace_bytes(int64_t n, int64_t m, int64_t nsim);
 cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel, int64_t m,
                            int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale, double* mmd2,
                            float* gpos, float* gvel, void* ws, cudaStream_t stream);
+size_t mmd_static_scratch_bytes();
+cudaError_t launch_mmd_f32_static(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel,
+                                  int64_t m, int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale,
+                                  double* mmd2, float* gpos, float* gvel, cudaStream_t stream);
 cudaError_t configure_pair_f32(int num_sms);
 cudaError_t configure_pair_f64(int num_sms);
 // whole-loop kernels (fused_step.cuh)

@@ -32,7 +32,7 @@ def test_exports_every_declared_symbol(lib):
 
 
 def test_status_strings(lib):
-    for code in range(7):
+    for code in range(8):
         assert lib.odisseo_status_string(code)
     assert lib.odisseo_last_cuda_error() == 0
 
