@@ -35,10 +35,36 @@ PARAM_NAMES = ("M_s", "r_s", "M_d", "a", "b")
 BULGE_PARAM_NAMES = ("M_b", "r_c")                        # alpha (the shape) is not differentiated
 
 
-def pair_accel_vjp(posm, c, G, eps):
-    """(gx [n,3], gm [n], gG, geps) = cotangent c [n,3] pulled back through a_pair(x, m, G, eps)."""
+def pair_accel_vjp(posm, c, G, eps, targets=None):
+    """(gx [n,3], gm [n], gG, geps) = cotangent c [n,3] pulled back through a_pair(x, m, G, eps).
+
+    targets = index array: only the rows gx[targets], gm[targets] are evaluated, one particle at a time with O(n)
+    memory (the dense form below holds [n, n, 3] arrays and stops near n = 3,000); the return value is
+    (gx [len(targets), 3], gm [len(targets)], gG, geps) with gG and geps summed over the target rows i only (the
+    totals when targets = every particle).  Same formula, term for term; pinned by targets = all particles
+    against the dense form and by finite differences of the forward oracle (tests/test_oracle_adjoint.py)."""
     posm = np.asarray(posm, dtype=np.float64)
     c = np.asarray(c, dtype=np.float64)
+    if targets is not None:
+        x, m = posm[:, :3], posm[:, 3]
+        gx = np.zeros((len(targets), 3))
+        gm = np.zeros(len(targets))
+        gG = geps = 0.0
+        for row, i in enumerate(targets):
+            d = x - x[i]                                      # d[j] = x_j - x_i
+            s = np.einsum("jk,jk->j", d, d) + eps * eps
+            with np.errstate(divide="ignore"):
+                f = s ** -1.5
+                g = -3.0 * s ** -2.5
+            f[i] = 0.0                                        # the pair sum skips j == i
+            g[i] = 0.0
+            u = m[i] * c - m[:, None] * c[i]                  # u[j] = m_i c_j - m_j c_i
+            du = np.einsum("jk,jk->j", d, u)
+            gx[row] = G * (np.einsum("j,jk->k", f, u) + np.einsum("j,jk->k", g * du, d))
+            gm[row] = -G * np.sum(f * np.einsum("jk,jk->j", d, c))
+            gG += float(np.dot(c[i], np.einsum("j,jk->k", f * m, d)))             # c_i . a_i / G
+            geps += float(eps * G * np.sum(m * g * (d @ c[i])))
+        return gx, gm, gG, geps
     x, m = posm[:, :3], posm[:, 3]
     d = x[None, :, :] - x[:, None, :]                     # d[i, j] = x_j - x_i
     s = np.einsum("ijk,ijk->ij", d, d) + eps * eps
@@ -59,14 +85,32 @@ def pair_accel_vjp(posm, c, G, eps):
     return gx, gm, gG, geps
 
 
-def pair_accel_vjp_scale(posm, c, G, eps):
+def pair_accel_vjp_scale(posm, c, G, eps, targets=None):
     """Per-particle sums of the MAGNITUDES of the terms pair_accel_vjp adds, the denominators of the per-element
     gradient tolerance (the analogue of S_i = sum_j |a_ij| of the forward tolerance, reading R6):
       Sx_i = G sum_j (f |u| + |g| |d| |d.u|),   Sm_i = G sum_j f |d.c_j|.
     By the triangle inequality |gx_i| <= Sx_i and |gm_i| <= Sm_i, with equality when a particle has one partner
-    and u is parallel to d (tests/test_oracle_adjoint.py)."""
+    and u is parallel to d (tests/test_oracle_adjoint.py).  targets = index array: those rows only, one particle at a
+    time with O(n) memory (as in pair_accel_vjp)."""
     posm = np.asarray(posm, dtype=np.float64)
     c = np.asarray(c, dtype=np.float64)
+    if targets is not None:
+        x, m = posm[:, :3], posm[:, 3]
+        Sx = np.zeros(len(targets))
+        Sm = np.zeros(len(targets))
+        for row, i in enumerate(targets):
+            d = x - x[i]
+            s = np.einsum("jk,jk->j", d, d) + eps * eps
+            with np.errstate(divide="ignore"):
+                f = s ** -1.5
+                g = 3.0 * s ** -2.5
+            f[i] = 0.0
+            g[i] = 0.0
+            u = m[i] * c - m[:, None] * c[i]
+            du = np.abs(np.einsum("jk,jk->j", d, u))
+            Sx[row] = G * np.sum(f * np.linalg.norm(u, axis=1) + g * np.linalg.norm(d, axis=1) * du)
+            Sm[row] = G * np.sum(f * np.abs(np.einsum("jk,jk->j", d, c)))
+        return Sx, Sm
     x, m = posm[:, :3], posm[:, 3]
     d = x[None, :, :] - x[:, None, :]
     s = np.einsum("ijk,ijk->ij", d, d) + eps * eps
@@ -161,16 +205,18 @@ def _total_accel(posm, G, eps, nfw, mn, bulge=None):
     return acc
 
 
-def accel_vjp(posm, c, G, eps, nfw=None, mn=None, bulge=None):
-    """Cotangent c pulled back through a = a_pair + a_ext: (gx, gm, gparams, gG, geps)."""
-    gx, gm, gG, geps = pair_accel_vjp(posm, c, G, eps)
+def accel_vjp(posm, c, G, eps, nfw=None, mn=None, bulge=None, rowwise=False):
+    """Cotangent c pulled back through a = a_pair + a_ext: (gx, gm, gparams, gG, geps).  rowwise: the pair part
+    particle by particle (pair_accel_vjp with targets = every particle) for n beyond the dense form's memory."""
+    gx, gm, gG, geps = pair_accel_vjp(posm, c, G, eps, np.arange(np.asarray(posm).shape[0]) if rowwise else None)
     ex, gp, eG = ext_accel_vjp(posm, c, G, nfw, mn, bulge)
     return gx + ex, gm, gp, gG + eG, geps
 
 
-def leapfrog_kdk_vjp(posm, vel, G, eps, dt, nsteps, lam_x, lam_v, nfw=None, mn=None, bulge=None):
+def leapfrog_kdk_vjp(posm, vel, G, eps, dt, nsteps, lam_x, lam_v, nfw=None, mn=None, bulge=None, rowwise=False):
     """Reverse-mode derivative of nsteps KDK steps (oracle.leapfrog_kdk) of a loss with final-state cotangents
-    lam_x = dL/dx_N, lam_v = dL/dv_N.  Returns a dict: x0, v0 [n,3]; m [n]; M_s, r_s, M_d, a, b, dt, G, eps."""
+    lam_x = dL/dx_N, lam_v = dL/dv_N.  Returns a dict: x0, v0 [n,3]; m [n]; M_s, r_s, M_d, a, b, dt, G, eps.
+    rowwise: every pair pull-back particle by particle (accel_vjp), same arithmetic, O(n) memory."""
     posm = np.array(posm, dtype=np.float64)
     v = np.array(vel, dtype=np.float64)
     xs, vs, accs = [posm.copy()], [v.copy()], [_total_accel(posm, G, eps, nfw, mn, bulge)]
@@ -188,7 +234,7 @@ def leapfrog_kdk_vjp(posm, vel, G, eps, dt, nsteps, lam_x, lam_v, nfw=None, mn=N
     out.update(dict.fromkeys(PARAM_NAMES + BULGE_PARAM_NAMES, 0.0))
 
     def pull(k, w):
-        gx, gm, gp, gG, geps = accel_vjp(xs[k], w * Lv, G, eps, nfw, mn, bulge)
+        gx, gm, gp, gG, geps = accel_vjp(xs[k], w * Lv, G, eps, nfw, mn, bulge, rowwise)
         out["m"] += gm
         out["G"] += gG
         out["eps"] += geps

@@ -65,8 +65,10 @@ struct PairF32 {
                 int64_t i1 = i0 + CTHREADS;
                 i0 = i0 < nt ? i0 : nt - 1;               // clamped rows are computed and never read back
                 i1 = i1 < nt ? i1 : nt - 1;
-                const float4 p0 = __ldg(posm + i0);
-                const float4 p1 = __ldg(posm + i1);
+                // coherent (L2) loads: this consumer also runs inside the whole-loop kernels (fused_step.cuh), where
+                // posm is rewritten between pair phases of ONE launch; a non-coherent ld.global.nc would be undefined there
+                const float4 p0 = __ldcg(posm + i0);
+                const float4 p1 = __ldcg(posm + i1);
                 // x + (-0) == x exactly; routing the pack through FADD2 makes the pair a native 64-bit
                 // register value, so ptxas does not re-assemble it with MOVs inside the j loop
                 const f32x2 nz = pk(-0.0f, -0.0f);

@@ -49,8 +49,10 @@ struct PairF64 {
             for (int k = 0; k < IPT; ++k) {
                 int64_t i = (int64_t)b * IB + (int64_t)k * CTHREADS + threadIdx.x;
                 i = i < nt ? i : nt - 1;
-                const double4 p = posm[i];
-                xi[k] = p.x; yi[k] = p.y; zi[k] = p.z;
+                // coherent (L2) loads: posm is rewritten between pair phases inside the whole-loop kernels
+                const double2 pxy = __ldcg(reinterpret_cast<const double2*>(posm + i));
+                const double pz = __ldcg(reinterpret_cast<const double*>(posm + i) + 2);
+                xi[k] = pxy.x; yi[k] = pxy.y; zi[k] = pz;
                 ax[k] = ay[k] = az[k] = 0.0;
             }
         }

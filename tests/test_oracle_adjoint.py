@@ -41,6 +41,51 @@ def test_pair_vjp_matches_finite_differences_of_the_forward_oracle():
     assert abs(geps - _fd(lambda t: loss(posm, e_=t), eps, 1e-7)) <= 1e-6 * abs(geps)
 
 
+@pytest.mark.parametrize("n,eps", [(2, 0.0), (7, 0.02), (200, 0.003)])
+def test_pair_vjp_row_form_equals_the_dense_form_and_finite_differences(n, eps):
+    """pair_accel_vjp(targets=...) and pair_accel_vjp_scale(targets=...) evaluate one particle at a time (what lets the
+    GPU parity tests reach N = 65,536): all rows == the dense form to rounding, a subset == those rows, the rows'
+    gG / geps == the dense totals, and on n = 7 the rows also meet central differences of the forward oracle directly."""
+    posm, _ = _cloud(n, 21 + n)
+    G = 1.3
+    c = np.random.Generator(np.random.PCG64(22 + n)).normal(size=(n, 3))
+    gx, gm, gG, geps = A.pair_accel_vjp(posm, c, G, eps)
+    rx, rm, rG, reps = A.pair_accel_vjp(posm, c, G, eps, targets=np.arange(n))
+    assert np.abs(rx - gx).max() <= 1e-13 * np.abs(gx).max() and np.abs(rm - gm).max() <= 1e-13 * np.abs(gm).max()
+    assert abs(rG - gG) <= 1e-12 * np.abs(c).max() * np.abs(O.pair_accel(posm, 1.0, eps)[0]).sum()
+    assert abs(reps - geps) <= 1e-12 * max(abs(geps), 1e-300) + (0 if eps else 1e-300)
+    sub = np.array([n - 1, 0, n // 2])
+    sx, sm, _, _ = A.pair_accel_vjp(posm, c, G, eps, targets=sub)
+    assert np.array_equal(sx, rx[sub]) and np.array_equal(sm, rm[sub])
+    Sx, Sm = A.pair_accel_vjp_scale(posm, c, G, eps)
+    Tx, Tm = A.pair_accel_vjp_scale(posm, c, G, eps, targets=sub)
+    assert np.abs(Tx - Sx[sub]).max() <= 1e-13 * Sx.max() and np.abs(Tm - Sm[sub]).max() <= 1e-13 * Sm.max()
+    assert np.all(np.linalg.norm(sx, axis=1) <= Tx * (1 + 1e-12)) and np.all(np.abs(sm) <= Tm * (1 + 1e-12))
+    if n == 7:
+        loss = lambda p: float(np.sum(c * O.pair_accel(p, G, eps)[0]))                  # noqa: E731
+        for row, i in enumerate(sub):
+            for k in range(4):
+                def f(t, i=i, k=k):
+                    p = posm.copy(); p[i, k] = t
+                    return loss(p)
+                ref = _fd(f, posm[i, k], 1e-6 if k < 3 else 1e-2)
+                got = sx[row, k] if k < 3 else sm[row]
+                assert abs(got - ref) <= 1e-7 * max(abs(ref), np.abs(gx).max() if k < 3 else np.abs(gm).max())
+
+
+def test_leapfrog_vjp_row_form_equals_the_dense_form():
+    n, nsteps = 60, 4
+    posm, vel = _cloud(n, 31, scale=0.02)
+    rng = np.random.Generator(np.random.PCG64(32))
+    lx, lv = rng.normal(size=(n, 3)), rng.normal(size=(n, 3)) * 10.0
+    a = A.leapfrog_kdk_vjp(posm, vel, G_KPC, 0.003, 0.7, nsteps, lx, lv, NFW, MN)
+    b = A.leapfrog_kdk_vjp(posm, vel, G_KPC, 0.003, 0.7, nsteps, lx, lv, NFW, MN, rowwise=True)
+    for key in a:
+        scale = np.abs(a[key]).max() if key != "eps" else max(abs(a["eps"]), 1e-300)
+        tol = 1e-12 if key not in ("G", "eps") else 1e-9       # totals that cancel between particles
+        assert np.abs(np.asarray(a[key]) - np.asarray(b[key])).max() <= tol * scale, key
+
+
 def test_pair_vjp_invariants_and_two_body_closed_form():
     posm, _ = _cloud(40, 3)
     c = np.tile(np.array([[0.3, -1.0, 2.0]]), (40, 1))
