@@ -106,6 +106,54 @@ def test_accel_vjp_per_element_bound(n, dtype, tol, unequal):
     assert np.all(np.abs(gm - rm) <= tol * Sm)
 
 
+@pytest.mark.parametrize("n,ntargets,variant", [(16384, 1024, "unequal"), (16384, 1024, "equal"), (16384, 1024, "odd_late"),
+                                                (65536, 256, "unequal"), (65536, 256, "odd_late")])
+def test_accel_vjp_at_the_benchmarked_sizes_on_seeded_targets(n, ntargets, variant):
+    """The pull-back on the path the sizes bench.py times take (cfg1 / cfg2 shape): several tiles per unit (fp64 sums
+    across tiles in flush_tile), the 4-stage ring wrapping around, CTAs that walk several units and cross i-blocks
+    (N = 65,536: 7 / 13 units per CTA in fp32 / fp64), and -- "odd_late" -- one different mass in a LATE tile of an
+    otherwise equal-mass cloud, so that the tile-wise equal-mass decision flips in the middle of a unit.  Oracle: the row
+    form of oracle/adjoint.py (O(n) memory) on seeded targets, which always include the particle with the odd mass,
+    the first and the last; per-element bound of test_accel_vjp_per_element_bound, fp32 and fp64 on the same
+    fp32-rounded inputs."""
+    cfg, p32, _, c32, G, eps = _inputs(n, 1200 + n, np.float32, unequal=(variant == "unequal"))
+    odd = (7 * n) // 8 + 3
+    if variant == "odd_late":
+        p32[odd, 3] *= 3
+    rng = np.random.Generator(np.random.PCG64(n + 5))
+    targets = np.unique(np.concatenate([rng.choice(n, ntargets - 3, replace=False), [0, odd, n - 1]]))
+    p64, c64 = p32.astype(np.float64), c32.astype(np.float64)
+    rx, rm, _, _ = A.pair_accel_vjp(p64, c64, G, eps, targets=targets)
+    Sx, Sm = A.pair_accel_vjp_scale(p64, c64, G, eps, targets=targets)
+    assert np.all(Sx > 0) and np.all(Sm > 0)
+    for dtype, tol in ((np.float32, 1e-5), (np.float64, 1e-12)):
+        gx, gm, _ = gpu_accel_vjp(p32.astype(dtype), c32.astype(dtype), G, eps, None, dtype, with_eps_G=False)
+        ex = np.linalg.norm(gx[targets, :3] - rx, axis=1) / Sx
+        em = np.abs(gm[targets] - rm) / Sm
+        print("n %d %s %s: max err / scale  gx %.2e gm %.2e" % (n, variant, dtype.__name__, ex.max(), em.max()))
+        assert ex.max() <= tol and em.max() <= tol
+        assert np.all(gx[:, 3] == 0) and np.all(np.isfinite(gx)) and np.all(np.isfinite(gm))
+
+
+def test_leapfrog_vjp_f64_with_several_tiles_per_unit_matches_the_row_wise_oracle():
+    """n = 6,000 x 3 steps in fp64: the pull-back plan gives 12 chunks of 504 records = 4 tiles of 128 per unit (the
+    n <= 3,001 cases above are one tile per unit), through the whole tape / KDK reverse loop.  Oracle: leapfrog_kdk_vjp
+    with rowwise=True (the dense form would need [n, n, 3] arrays)."""
+    n, nsteps = 6000, 3
+    cfg, p, v, _, G, eps = _inputs(n, 1300, np.float64)
+    v = v * 0.02 + np.asarray(cfg.velocity)
+    rng = np.random.Generator(np.random.PCG64(12))
+    lx, lv = rng.normal(size=(n, 3)), rng.normal(size=(n, 3)) * 10.0
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    gx0, gv0, gm, gp, _ = gpu_leapfrog_vjp(p, v, G, eps, cfg.dt, nsteps, pot, lx, lv, np.float64)
+    ref = A.leapfrog_kdk_vjp(p, v, G, eps, cfg.dt, nsteps, lx, lv, cfg.nfw, cfg.mn, rowwise=True)
+    assert np.abs(gx0[:, :3] - ref["x0"]).max() <= 1e-9 * np.abs(ref["x0"]).max()
+    assert np.abs(gv0[:, :3] - ref["v0"]).max() <= 1e-9 * np.abs(ref["v0"]).max()
+    assert np.abs(gm - ref["m"]).max() <= 1e-9 * np.abs(ref["m"]).max()
+    for k, name in enumerate(NAMES):
+        assert abs(gp[k] - ref[name]) <= 1e-8 * abs(ref[name]) + 1e-13 * abs(ref["dt"]), name
+
+
 def test_accel_vjp_without_potential_and_reproducible():
     cfg, p, _, c, G, eps = _inputs(2000, 77, np.float64)
     a = gpu_accel_vjp(p, c, G, eps, None, np.float64)

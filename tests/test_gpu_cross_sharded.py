@@ -105,23 +105,8 @@ class _ThreadExchange:
         return exchange
 
 
-@pytest.mark.parametrize("world", [1, 2, 3, 8])
-@pytest.mark.parametrize("dtype", [np.float32, np.float64])
-@pytest.mark.parametrize("n", [3000, 5000])
-def test_sharded_driver_with_emulated_ranks_is_bit_identical_to_the_single_gpu_leapfrog(world, dtype, n):
-    """SURVEY 8f NEXT-1: "result bit-identical to 1 GPU (same fixed reduction order per i)".  n = 3,000 takes the small
-    kernel variant, n = 5,000 the large one; 3 and 8 ranks give ragged, 8-aligned slices."""
-    cfg = W.CONFIGS[1]
-    nsteps = 6
-    posm64, vel64 = W.make_state(cfg, n=n)
-    p0, v0 = posm64.astype(dtype), W.vel4(vel64.astype(dtype), dtype)
-    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
-    posm, vel = dev(p0, dtype), dev(v0, dtype)
-    acc = torch.empty_like(posm)
-    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64)))
-    torch.cuda.synchronize()
-    want = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
-
+def _run_emulated_ranks(p0, v0, n, world, dtype, cfg, pot, nsteps):
+    """The sharded driver on `world` emulated ranks (threads) of one GPU; returns the gathered (posm, vel, acc)."""
     ex = _ThreadExchange(n, world)
     bounds = ex.bounds
     bufs = [dev(p0, dtype) for _ in range(world)]
@@ -147,6 +132,27 @@ def test_sharded_driver_with_emulated_ranks_is_bit_identical_to_the_single_gpu_l
     got_p = np.concatenate([bufs[r][lo:hi].cpu().numpy() for r, (lo, hi) in enumerate(bounds)])
     got_v = np.concatenate([v.cpu().numpy() for v in vels])
     got_a = np.concatenate([a.cpu().numpy() for a in accs])
+    return got_p, got_v, got_a
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 8])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n", [3000, 5000])
+def test_sharded_driver_with_emulated_ranks_is_bit_identical_to_the_single_gpu_leapfrog(world, dtype, n):
+    """SURVEY 8f NEXT-1: "result bit-identical to 1 GPU (same fixed reduction order per i)".  n = 3,000 takes the small
+    kernel variant, n = 5,000 the large one; 3 and 8 ranks give ragged, 8-aligned slices."""
+    cfg = W.CONFIGS[1]
+    nsteps = 6
+    posm64, vel64 = W.make_state(cfg, n=n)
+    p0, v0 = posm64.astype(dtype), W.vel4(vel64.astype(dtype), dtype)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    posm, vel = dev(p0, dtype), dev(v0, dtype)
+    acc = torch.empty_like(posm)
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, B.alloc_workspace(B.workspace_bytes(n, dtype == np.float64)))
+    torch.cuda.synchronize()
+    want = (posm.cpu().numpy(), vel.cpu().numpy(), acc.cpu().numpy())
+
+    got_p, got_v, got_a = _run_emulated_ranks(p0, v0, n, world, dtype, cfg, pot, nsteps)
     assert got_p.tobytes() == want[0].tobytes() and got_v.tobytes() == want[1].tobytes() and got_a.tobytes() == want[2].tobytes()
 
 
@@ -195,3 +201,24 @@ def test_degenerate_sizes_are_ok_noops_or_zeros():
     e30 = torch.zeros(4, 0, 4, device="cuda")
     B.ensemble_leapfrog_kdk(e30, e30.clone(), [(cfg.G, cfg.eps, cfg.dt, pot)], 3, ws)       # no particles
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("n,world", [(3000, 3), (5000, 2)])
+def test_sharded_driver_matches_the_oracle_leapfrog(n, world):
+    """The staged trio (stage_sources, kick_drift_slice, pair_accel_staged) against the ORACLE, not against the GPU:
+    fp64, cfg1-shaped cloud, 6 KDK steps on emulated ranks with ragged slices, positions and velocities within 1e-10
+    relative of oracle.leapfrog_kdk (north_star's fp64 trajectory tolerance), accelerations within 1e-12 S_i."""
+    cfg = W.CONFIGS[1]
+    nsteps = 6
+    posm64, vel64 = W.make_state(cfg, n=n)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    got_p, got_v, got_a = _run_emulated_ranks(posm64, W.vel4(vel64, np.float64), n, world, np.float64, cfg, pot, nsteps)
+    opot = O.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    pr, vr, ar = O.leapfrog_kdk(posm64, vel64, cfg.G, cfg.eps, cfg.dt, nsteps, opot)
+    assert np.abs(got_p[:, :3] - pr[:, :3]).max() <= 1e-10 * np.abs(pr[:, :3]).max()
+    assert np.abs(got_v[:, :3] - vr).max() <= 1e-10 * np.abs(vr).max()
+    assert np.array_equal(got_p[:, 3], posm64[:, 3])
+    # acc holds the PAIR-ONLY acceleration of the final positions (include/odisseo.h); x differs from the oracle's by
+    # ~1e-16 relative, which the tidal tensor of close neighbours turns into more than 1e-12 S_i: compare at the GPU's x
+    pair_only, Sn = O.pair_accel(got_p, cfg.G, cfg.eps)
+    assert (np.linalg.norm(got_a[:, :3] - pair_only, axis=1) / Sn).max() <= 1e-12
