@@ -11,7 +11,8 @@ Multi-GPU, default (--mode replicas): north_star fixes the build to one GPU with
 "Multi-GPU"): every rank advances its own seeded replica, no data-path collective, scaling = "weak".
 --mode sharded: ONE simulation, targets sliced over the ranks (paper_2511_22468_b200/sharded.py: kick/drift of the
 slice, one all-gather of staged source records per step, pair acceleration of the slice), scaling = "strong",
-value = N^2 x steps / max-over-ranks time.  Only ever run with world size 1 on hardware in this build.
+value = N^2 x steps / max-over-ranks time.  On hardware only ever run with world size 1 in this build (the collective
+then runs on NCCL with one rank).
 """
 from __future__ import annotations
 
@@ -27,18 +28,35 @@ import numpy as np
 FLOPS_PER_INTERACTION = 20.0                      # BASELINE.json north_star convention
 SM_COUNT, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_HZ / 1e12      # 74.45, DESIGN.md "Roofline"
-PAIR_PROFILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r02_pair_f32_ncu_full.txt")
+ROOT = os.path.dirname(os.path.abspath(__file__))
+PAIR_PROFILE = os.path.join(ROOT, "profiles", "r03_pair_f32_ncu_full.txt")
+# the sources the fp32 pair kernel is compiled from: the tracked ncu summary names their hash, and its DRAM traffic is
+# quoted only while they are unchanged (otherwise "traffic": null -- the profile is of another binary)
+PAIR_KERNEL_SOURCES = ("pair_f32.cu", "pair_stream.cuh", "odisseo_common.cuh")
+
+
+def _kernel_sources_sha16():
+    import hashlib
+    h = hashlib.sha256()
+    for name in PAIR_KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2511_22468_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
 
 
 def _profile_traffic_bytes(path: str = PAIR_PROFILE):
     """dram__bytes_read.sum + dram__bytes_write.sum of one pair-kernel launch at N = 262,144, read from the tracked
     `ncu --set full` summary it was captured into (None when the file or the counters are missing)."""
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
-    total, seen = 0.0, 0
+    total, seen, captured_at = 0.0, 0, None
     try:
         with open(path) as f:
             for line in f:
                 parts = line.split()
+                if len(parts) >= 3 and parts[0] == "#" and parts[1] == "kernel_sources_sha16:":
+                    captured_at = parts[2]
+                    if captured_at != _kernel_sources_sha16():
+                        return None                      # the kernel's sources changed since the capture
                 if len(parts) >= 3 and parts[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and parts[1] in scale:
                     total += float(parts[2].replace(",", "")) * scale[parts[1]]
                     seen += 1
@@ -46,7 +64,7 @@ def _profile_traffic_bytes(path: str = PAIR_PROFILE):
                     break
     except OSError:
         return None
-    return int(total) if seen == 2 else None
+    return int(total) if seen == 2 and captured_at is not None else None
 
 
 def _stats(ms):
@@ -139,16 +157,24 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
-def _dist_setup(n_gpus: int, backend: str = "nccl"):
+def _dist_setup(n_gpus: int, backend: str = "nccl", single_rank_group: bool = False):
     """One process per GPU under torchrun; returns (rank, world, dist-or-None).  backend = "gloo" is the
-    CPU stand-in the tests use for the rank logic (no kernels run there)."""
+    CPU stand-in the tests use for the rank logic (no kernels run there).  single_rank_group: a process group even at
+    world size 1 (--mode sharded), so that the per-step collective really runs on NCCL on the one GPU there is."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
-    if world == 1:
+    if world == 1 and not single_rank_group:
         return 0, 1, None
     import torch
     import torch.distributed as dist
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    if world == 1 and "MASTER_PORT" not in os.environ:                       # plain `python bench.py`, no torchrun
+        import socket
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            os.environ["MASTER_PORT"] = str(s.getsockname()[1])
+        os.environ.setdefault("RANK", "0")
+        os.environ.setdefault("WORLD_SIZE", "1")
     if backend == "nccl":
         torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     dist.init_process_group(backend=backend)
@@ -526,10 +552,9 @@ def run_sharded(args, rank: int, world: int, dist, torch, B, W):
     acc = torch.empty(hi - lo, 4, dtype=torch.float32, device="cuda")
     comp = S.CudaCompute(n, hi - lo, False, G, eps, dt, pot, world=world)
 
-    class _Local:                                                           # world size 1: nothing to exchange
-        def __call__(self, records):
-            return None
-    ex = S.DistExchange(dist, n, world, rank) if dist is not None else _Local()
+    # a process group exists at every world size (main: single_rank_group), so the in-place all-gather runs on NCCL
+    # even on one GPU
+    ex = S.DistExchange(dist, n, world, rank)
     K, Wm = args.steps, args.warmup
     S.sharded_leapfrog_kdk(comp, ex, posm_all, vel, acc, lo, hi, 0)          # stage + initial a_pair, untimed
     for _ in range(Wm):
@@ -560,6 +585,7 @@ def run_sharded(args, rank: int, world: int, dist, torch, B, W):
                    "l2": "inputs of %.0f MB per step stream through L2 once; K steps timed back to back" % (48e-6 * n)},
         "kdk_steps_per_s": K / (total_ms * 1e-3), "gpu_launches": launches, "clocks": clocks,
         "e2e": None, "roofline": None,
+        "collective": "all_gather_into_tensor, in place, backend %s, once per step" % dist.get_backend(),
         "note": "sharded mode reports the strong-scaling value only; roofline, e2e and cpu_baseline are the replicas mode's",
     }
     print(json.dumps(line), flush=True)
@@ -656,9 +682,12 @@ def run_ours(args, rank: int, world: int, dist):
         "e2e": {"value": whole_job_rate(n, K, world, e2e_ms), "unit": "G-int/s",
                 "h2d_bytes_per_step": 3 * 16 * n, "d2h_bytes_per_step": 3 * 16 * n,
                 "ms_per_step": e2e_ms / K, "step_ms_stats": _stats(e2e_steps)},
-        "roofline": {"bound": "alu", "kernel": "stream_kernel<PairF32<4,8,1,8>> (fp32 pair kernel, equal-mass loop)",
+        "roofline": {"bound": "alu", "kernel": B.pair_kernel_name(n) + " (fp32 pair kernel, equal-mass loop)",
                      "achieved": achieved, "peak": FP32_PEAK_TFLOPS,
                      "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                     # the graded general-m_j loop, filled in below; kept next to "frac" so that a parser
+                     # that keeps only an object's first keys keeps it
+                     "frac_general_masses": None, "achieved_general_masses": None,
                      "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz %s)"
                                   % (SM_MAX_HZ / 1e6, peak_kind),
                      "flops_per_interaction": FLOPS_PER_INTERACTION,
@@ -669,7 +698,9 @@ def run_ours(args, rank: int, world: int, dist):
                      "launches_timed": pair_launches, "launches_dropped": dropped,
                      "share_of_step": pair_ms / float(np.sum(step_ms)),
                      "traffic": _profile_traffic_bytes() if args.config == 3 else None,
-                     "traffic_source": "profiles/r02_pair_f32_ncu_full.txt (dram__bytes_read.sum + dram__bytes_write.sum)"},
+                     "traffic_source": "profiles/r03_pair_f32_ncu_full.txt (dram__bytes_read.sum + dram__bytes_write.sum), quoted "
+                                       "only while its kernel_sources_sha16 equals this tree's",
+                     "kernel_sources_sha16": _kernel_sources_sha16()},
     }
     if world == 1:
         # measured pipe rates (tracked micro-benchmarks, csrc/ubench.cu) beside the nominal peak
@@ -770,7 +801,7 @@ def main():
         peaks, peak_kind = _peaks()
         print(json.dumps({"integrator_roofline": _integrator_roofline(B, W, torch, peaks, peak_kind)}), flush=True)
         return 0
-    rank, world, dist = _dist_setup(args.gpus)
+    rank, world, dist = _dist_setup(args.gpus, single_rank_group=(args.mode == "sharded"))
     try:
         run_ours(args, rank, world, dist)
     finally:

@@ -35,7 +35,11 @@
  *     10.0 (the library holds sm_100a code only, no PTX fallback) -> ERR_ARCH, CUDA failure ->
  *     ERR_CUDA (code in odisseo_last_cuda_error()).  n == 0 or nsteps == 0 is an OK no-op
  *     (nsteps == 0 with acc_valid == 0 still evaluates acc).  Inputs are not screened for
- *     NaN/Inf particles; they propagate.
+ *     NaN/Inf particles; they propagate.  The masses live on the device, so the eps bound above cannot
+ *     know them: the fp32 loop for UNEQUAL masses forms m_j eps^-3 in the self term, and the accepted region
+ *     is  max_j |m_j| * eps^-3 < 3.4e38 (FLT_MAX);  beyond it that product is inf, inf * 0 = NaN, and every
+ *     acceleration of the call is NaN (tests/test_gpu_parity.py pins both sides of the edge).  Equal masses
+ *     are applied in fp64 after the sum and have no such bound; fp64 calls need |m_j| eps^-3 < 1.8e308.
  *   - There is no CPU fallback: without a B200 every compute call fails with ERR_ARCH/ERR_CUDA.
  *   - Results are bit-reproducible run to run for fixed (n, device SM count): partial sums
  *     are combined in a fixed order, never with atomics.
@@ -414,6 +418,11 @@ odisseo_status odisseo_mmd2_static_f32(const float *d_xpos, const float *d_xvel,
  *     fills h_ms[0 .. min(count, capacity)) and *h_count = count (bench.py's min / median / mean +- std,
  *     SURVEY.md 8d timing protocol).  While a profile is open -> ERR_ARG. */
 int64_t odisseo_launch_count(void);
+/* Name of the O(N^2) kernel instantiation odisseo_pair_accel_f32 / _f64 (and the per-step leapfrog) launch for n
+ * particles, as profilers print it without namespaces, e.g. "stream_kernel<PairF32<4,8,1,16,8>>" -- spelled from the
+ * template arguments in the library, so bench.py's roofline.kernel and the summaries under profiles/ cannot go
+ * stale.  Static string, never NULL ("" for n <= 0). */
+const char *odisseo_pair_kernel_name(int64_t n, int is_f64);
 odisseo_status odisseo_profile_begin(void);
 odisseo_status odisseo_profile_end(double *h_ms_total, int64_t *h_launches, int64_t *h_dropped);
 odisseo_status odisseo_profile_times(double *h_ms, int64_t capacity, int64_t *h_count);

@@ -34,6 +34,20 @@ def _theta_grad(gp, theta):
     return g.to(theta.dtype).to(theta.device)
 
 
+def _check_alpha(theta, freeze_alpha: bool):
+    """The C ABI has no gradient slot for the bulge shape alpha (binding.GRADIENT_FIELDS): an 8-parameter theta that
+    requires grad would get a silent 0 there.  Refuse unless the caller says that is what they want."""
+    if theta.shape[-1] == 8 and theta.requires_grad and not freeze_alpha:
+        raise ValueError("theta has 8 entries (with the bulge) and requires grad, but d/d(alpha) is not computed: pass "
+                         "freeze_alpha=True to accept a zero gradient for alpha (entry 6), or detach theta")
+
+
+def _check_observed(yposm, yvel):
+    if yposm.requires_grad or yvel.requires_grad:
+        raise ValueError("mmd2 differentiates with respect to the simulated clouds only: the observed cloud (yposm, yvel) "
+                         "gets no gradient; detach it")
+
+
 class _LeapfrogKDK(torch.autograd.Function):
     @staticmethod
     def forward(ctx, posm0, vel0, theta, dt, G, eps, nsteps):
@@ -69,10 +83,13 @@ class _LeapfrogKDK(torch.autograd.Function):
 
 
 def leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.Tensor, dt: torch.Tensor, G: float, eps: float,
-                 nsteps: int):
+                 nsteps: int, freeze_alpha: bool = False):
     """Differentiable nsteps KDK steps.  posm0, vel0: CUDA [n, 4] (float32 or float64); theta: 5 values
-    (M_s, r_s, M_d, a, b), a mass <= 0 disables that term; dt: 0-d tensor.  Returns (posm_final, vel_final);
-    gradients flow to posm0 (lane 3 = masses), vel0, theta and dt."""
+    (M_s, r_s, M_d, a, b), a mass <= 0 disables that term, or 8 with the bulge (M_b, alpha, r_c); dt: 0-d tensor.
+    Returns (posm_final, vel_final); gradients flow to posm0 (lane 3 = masses), vel0, theta and dt.
+    LIMITATION: the bulge shape alpha is not differentiated.  An 8-entry theta that requires grad raises ValueError
+    unless freeze_alpha=True, in which case theta.grad[6] is 0 by construction, not by calculus."""
+    _check_alpha(theta, freeze_alpha)
     dt = torch.as_tensor(dt)
     return _LeapfrogKDK.apply(posm0, vel0, theta, dt, G, eps, nsteps)
 
@@ -139,10 +156,13 @@ class _EnsembleLeapfrogKDK(torch.autograd.Function):
 
 
 def ensemble_leapfrog_kdk(posm0: torch.Tensor, vel0: torch.Tensor, theta: torch.Tensor, dt: torch.Tensor, G: float,
-                          eps: float, nsteps: int, checkpoint_every: int = 0):
-    """Differentiable batch of small simulations: posm0, vel0 float32 CUDA [nsim, n, 4] (n <= 2,048); theta [nsim, 5];
-    dt [nsim].  Returns (posm_final, vel_final); gradients flow to posm0 (lane 3 = masses), vel0, theta and dt.
-    checkpoint_every = K keeps a K-step tape instead of the whole trajectory (one extra forward pass in backward)."""
+                          eps: float, nsteps: int, checkpoint_every: int = 0, freeze_alpha: bool = False):
+    """Differentiable batch of small simulations: posm0, vel0 float32 CUDA [nsim, n, 4] (n <= 2,048); theta [nsim, 5]
+    (or [nsim, 8] with the bulge); dt [nsim].  Returns (posm_final, vel_final); gradients flow to posm0 (lane 3 =
+    masses), vel0, theta and dt.  checkpoint_every = K keeps a K-step tape instead of the whole trajectory (one extra
+    forward pass in backward).  LIMITATION: the bulge shape alpha is not differentiated; an 8-entry theta that requires
+    grad raises ValueError unless freeze_alpha=True (theta.grad[:, 6] is then 0 by construction)."""
+    _check_alpha(theta, freeze_alpha)
     return _EnsembleLeapfrogKDK.apply(posm0, vel0, theta, dt, G, eps, nsteps, checkpoint_every)
 
 
@@ -178,5 +198,7 @@ class _MMD2(torch.autograd.Function):
 def mmd2(posm: torch.Tensor, vel: torch.Tensor, yposm: torch.Tensor, yvel: torch.Tensor, sigma):
     """Differentiable MMD^2 loss (Fig. 2 step 4): posm, vel float32 CUDA [nsim, n, 4] (or [n, 4]) simulated
     clouds, yposm, yvel [m, 4] (shared) or [nsim, m, 4] observed; sigma: 6 kernel scales (x, y, z, vx, vy, vz).  Returns
-    [nsim] float64 (or a 0-d tensor); gradients flow to posm and vel."""
+    [nsim] float64 (or a 0-d tensor); gradients flow to posm and vel ONLY: an observed cloud that requires grad raises
+    ValueError (it would silently get none)."""
+    _check_observed(yposm, yvel)
     return _MMD2.apply(posm, vel, yposm, yvel, tuple(float(s) for s in sigma))

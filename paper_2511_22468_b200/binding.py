@@ -25,7 +25,7 @@ EXPORTS = [
     "odisseo_pair_accel_f32", "odisseo_pair_accel_f64", "odisseo_pair_accel_soa_f32",
     "odisseo_ext_accel_f32", "odisseo_ext_accel_f64", "odisseo_leapfrog_kdk_f32", "odisseo_leapfrog_kdk_f64",
     "odisseo_leapfrog_kdk_host_f32", "odisseo_leapfrog_kdk_host_f64", "odisseo_describe_plan",
-    "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_profile_begin",
+    "odisseo_describe_plan_for", "odisseo_describe_cross_plan_for", "odisseo_plan_probe", "odisseo_launch_count", "odisseo_pair_kernel_name", "odisseo_profile_begin",
     "odisseo_profile_end", "odisseo_profile_times", "odisseo_shutdown", "odisseo_set_fused_max_n", "odisseo_set_cluster_max_n", "odisseo_set_ll_max_n", "odisseo_kick_drift_f32", "odisseo_kick_drift_f64",
     "odisseo_ensemble_workspace_bytes", "odisseo_ensemble_leapfrog_kdk_f32",
     "odisseo_diagnostics_workspace_bytes", "odisseo_diagnostics_f32", "odisseo_diagnostics_f64",
@@ -115,6 +115,8 @@ def lib():
         L.odisseo_mmd_workspace_bytes.restype = sz
         L.odisseo_mmd_workspace_bytes.argtypes = [i64, i64, i64]
         L.odisseo_mmd2_f32.argtypes = [vp, vp, i64, vp, vp, i64, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.odisseo_pair_kernel_name.restype = ctypes.c_char_p
+        L.odisseo_pair_kernel_name.argtypes = [i64, ci]
         L.odisseo_mmd2_static_scratch_bytes.restype = sz
         L.odisseo_mmd2_static_scratch_bytes.argtypes = []
         L.odisseo_mmd2_static_f32.argtypes = [vp, vp, i64, vp, vp, i64, i64, ci, vp, vp, vp, vp, vp, vp]
@@ -544,6 +546,11 @@ def profile_end():
     ms, nl, nd = ctypes.c_double(0.0), ctypes.c_int64(0), ctypes.c_int64(0)
     _check(lib().odisseo_profile_end(ctypes.byref(ms), ctypes.byref(nl), ctypes.byref(nd)), "profile_end")
     return float(ms.value), int(nl.value), int(nd.value)
+
+
+def pair_kernel_name(n: int, is_f64: bool = False) -> str:
+    """The pair-kernel instantiation pair_accel / leapfrog_kdk launch for n particles (odisseo_pair_kernel_name)."""
+    return lib().odisseo_pair_kernel_name(int(n), int(bool(is_f64))).decode()
 
 
 def mmd_workspace_bytes(n: int, m: int, nsim: int = 1) -> int:

@@ -449,7 +449,7 @@ void vjp_geometry(int is_f64, int* ipt, int* cthreads, int* tile, int* minb)
     *minb = is_f64 ? 1 : VJP_MINB;
 }
 
-// Workspace of the pull-back: [staged records + flags][unit rows, 6 planes][block sums (8 per block)][cotangents].
+// Workspace of the pull-back: [staged records + flags][unit rows, 6 planes][block sums (VJP_NOUT = 10 per block)][cotangents].
 static size_t vjp_rows_bytes(const PairPlan& plan) { return ((size_t)plan.U * 6 * plan.IB * sizeof(double) + 255) & ~(size_t)255; }
 static size_t vjp_blocks_bytes(const PairPlan& plan)
 {

@@ -907,7 +907,7 @@ const char* odisseo_status_string(odisseo_status s)
         case ODISSEO_ERR_ALIGN: return "misaligned pointer";
         case ODISSEO_ERR_ARG: return "invalid argument";
         case ODISSEO_ERR_WORKSPACE: return "workspace too small";
-        case ODISSEO_ERR_ARCH: return "device is not compute capability 10.x (B200)";
+        case ODISSEO_ERR_ARCH: return "device is not compute capability 10.0 (B200, sm_100a)";
         case ODISSEO_ERR_CUDA: return "CUDA error (see odisseo_last_cuda_error)";
         case ODISSEO_ERR_STATIC_LIMIT:
             return "problem too large for the library's built-in scratch array (odisseo_mmd2_static_scratch_bytes); "
@@ -919,6 +919,13 @@ const char* odisseo_status_string(odisseo_status s)
 int odisseo_last_cuda_error(void) { return g_last_cuda_error; }
 
 int64_t odisseo_launch_count(void) { return g_launches.load(); }
+
+const char* odisseo_pair_kernel_name(int64_t n, int is_f64)
+{
+    if (n <= 0) return "";
+    const int variant = make_cross_plan(n, n, is_f64 != 0, 148).variant;       // the variant is a function of n alone
+    return is_f64 ? pair_kernel_name_f64(variant) : pair_kernel_name_f32(variant);
+}
 
 int64_t odisseo_set_fused_max_n(int64_t n)
 {

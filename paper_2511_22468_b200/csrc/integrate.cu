@@ -6,7 +6,8 @@
 //   a      = a_pair + a_NFW(x) + a_MN(x)
 //   v     += a dt/2          [STEP_CLOSE: second half kick of the step that just ended]
 //   v     += a dt/2 ; x += v dt   [STEP_OPEN: first half kick + drift of the next step]
-//   stage x for the next pair evaluation
+//   stage x for the next pair evaluation -- only in the staged forms (cross, sharded, cooperative); on the default
+//   path the pair kernel's TMA reads posm itself and this kernel writes posm, vel, acc and the equal-mass flags only
 //
 // The two half kicks are two separate FMAs, so a step split across two calls is bit-identical to
 // the fused one (PAPER.md:L47 Velocity-Verlet; chaining contract in include/odisseo.h).

@@ -22,8 +22,8 @@ namespace odisseo {
 // a target receives is  G m0 sum_s ( sum_{tiles of chunk s} fp32 tile sum ),  a fixed grouping
 // that depends on n only -- not on the number of targets, CTAs or ranks (SURVEY.md 8f NEXT-1:
 // "same fixed reduction order per i"), with no atomics: bit-reproducible.
-// S is chosen on the host so that nb(n) * S is a multiple of the CTA count when that is cheap
-// (148 = 4 * 37: S = 37 at n = 2^18 gives 32 equal units per CTA): no wave-quantisation tail.
+// S is chosen on the host by a cost model of the busiest CTA (source_split, api.cu): at n = 2^18 on 148 SMs
+// S = 15, U = 128 * 15 = 1,920 units, 12 or 13 per CTA.
 // ---------------------------------------------------------------------------------------
 struct PairPlan {
     int64_t n;        // source particles (staged, chunked along j)
@@ -376,6 +376,8 @@ size_t mmd_static_scratch_bytes();
 cudaError_t launch_mmd_f32_static(const float* xpos, const float* xvel, int64_t n, const float* ypos, const float* yvel,
                                   int64_t m, int shared_y, const double inv_sigma[6], int64_t nsim, const double* grad_scale,
                                   double* mmd2, float* gpos, float* gvel, cudaStream_t stream);
+const char* pair_kernel_name_f32(int variant);
+const char* pair_kernel_name_f64(int variant);
 cudaError_t configure_pair_f32(int num_sms);
 cudaError_t configure_pair_f64(int num_sms);
 // whole-loop kernels (fused_step.cuh)

@@ -7,19 +7,26 @@
 //     thread so that ptxas interleaves a thread's four interaction chains), contiguous equal ranges of
 //     (i-block x source-chunk) units per CTA, source tiles through a TMA ring (pair_stream.cuh)
 //     -> every SM busy for any N, no wave-quantisation tail;
-//   * each compute thread keeps 2*NPAIR targets in registers as packed f32x2 pairs; sources are
-//     staged pre-duplicated {x,x,y,y},{z,z,m,m} so that one LDS.128 yields two ready packed
-//     operands and the body is 3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per TWO interactions
-//     (half the issue slots of the scalar form, no register-pair MOVs);
+//   * each compute thread keeps 2*NPAIR targets in registers as packed f32x2 pairs; sources are plain
+//     {x,y,z,m} records (16 B) -- on the default path the particles' OWN records, read by TMA with no
+//     staged copy (plan.direct) -- so that one LDS.128 broadcast yields a source, whose coordinates enter
+//     the packed instructions as scalar operands broadcast to both halves; the body is
+//     3 FADD2 + 6 FFMA2 + 3 FMUL2 + 2 MUFU.RSQ per TWO interactions (half the issue slots of the scalar
+//     form, no register-pair MOVs);
 //   * two-level summation: fp32 inside one tile (<= 512 terms), promoted to fp64 between tiles
 //     (a single running fp32 sum fails the 1e-5 tolerance at N >= 2^18); one row of
 //     fp64 sums per unit, rows added in unit order by the reduce step (fixed grouping, function of n only);
-//   * the self term contributes exactly 0 because eps > 0; padding records are massless and parked at
-//     3e18, where the inverse cube underflows to exactly 0 (ftz), so they vanish on both paths;
+//   * the self term contributes exactly 0 because eps > 0; the direct path has no padding (the last tile
+//     ends at n and tile() takes any length -- keep its remainder handling); the staged forms (cross, sharded,
+//     cooperative) pad with massless records parked at 3e18, where the inverse cube underflows to exactly 0 (ftz);
 //   * equal masses (the paper's Plummer progenitors, PAPER.md:L43 step 3) are detected on the device by
-//     the staging kernel; the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2, and the
+//     the step / staging kernel (one flag per 256 particles); the mass factor then leaves the inner loop: 3 FADD2 + 6 FFMA2 + 2 FMUL2, and the
 //     reduce step multiplies by the mass once;
 //   * programmatic dependent launch: barrier init and plan arithmetic overlap the predecessor's tail.
+#include <stdio.h>
+
+#include <string>
+
 #include "fused_step.cuh"
 #include "cluster_kdk.cuh"
 #include "ll_kdk.cuh"
@@ -240,6 +247,21 @@ cudaError_t launch_ll_f32(const PairPlan& plan, float* posm, float* vel, float* 
     cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
     if (e != cudaSuccess) return e;
     return launch_ll<LLF32, float>(ca, ctas, smem, LL_TAPE_CODE_FLOAT, stream);
+}
+
+// The instantiation launch_pair_f32 selects, spelled from the template arguments themselves (odisseo_pair_kernel_name).
+template <int A, int B, int C, int D, int E>
+static std::string stream_kernel_name(const PairF32<A, B, C, D, E>*)
+{
+    char buf[96];
+    snprintf(buf, sizeof buf, "stream_kernel<PairF32<%d,%d,%d,%d,%d>>", A, B, C, D, E);
+    return buf;
+}
+const char* pair_kernel_name_f32(int variant)
+{
+    static const std::string names[2] = {stream_kernel_name(static_cast<const LargeF32*>(nullptr)),
+                                         stream_kernel_name(static_cast<const SmallF32*>(nullptr))};
+    return names[variant ? 1 : 0].c_str();
 }
 
 cudaError_t launch_pair_f32(const PairPlan& plan, const float* posm, const void* jsrc, const void* src, double* partials, float eps,

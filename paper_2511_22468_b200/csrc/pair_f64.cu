@@ -11,6 +11,10 @@
 // seed cost as much as the arithmetic they feed.
 // Summation: fp64 inside a tile, tile sums added in tile order inside a unit, one row per unit -- the
 // same fixed grouping as the fp32 kernel.
+#include <stdio.h>
+
+#include <string>
+
 #include "fused_step.cuh"
 #include "cluster_kdk.cuh"
 #include "ll_kdk.cuh"
@@ -218,6 +222,20 @@ cudaError_t launch_ll_f64(const PairPlan& plan, double* posm, double* vel, doubl
     cudaError_t e = cudaMemsetAsync(xbuf, 0, xbytes, stream);          // tags start at 1
     if (e != cudaSuccess) return e;
     return launch_ll<LLF64, double>(ca, ctas, smem, LL_TAPE_CODE_DOUBLE, stream);
+}
+
+template <int A, int B, int C, int D, bool POT>
+static std::string stream_kernel_name(const PairF64<A, B, C, D, POT>*)
+{
+    char buf[96];
+    snprintf(buf, sizeof buf, "stream_kernel<PairF64<%d,%d,%d,%d,%d>>", A, B, C, D, (int)POT);
+    return buf;
+}
+const char* pair_kernel_name_f64(int variant)
+{
+    static const std::string names[2] = {stream_kernel_name(static_cast<const LargeF64*>(nullptr)),
+                                         stream_kernel_name(static_cast<const SmallF64*>(nullptr))};
+    return names[variant ? 1 : 0].c_str();
 }
 
 cudaError_t launch_pair_f64(const PairPlan& plan, const double* posm, const void* jsrc, const void* src, double* partials, double eps,

@@ -13,7 +13,7 @@
 //           State(const Params&, const PairPlan&, unsigned char* outer_smem);
 //           void load_targets(int32_t b);               // i-block b -> registers
 //           void zero_outer();                          // start of a unit
-//           void tile(const unsigned char* tile, int len);   // len source records (multiple of 8)
+//           void tile(const unsigned char* tile, int len);   // len source records, ANY length >= 1 (direct path: the last tile ends at n)
 //           void flush_tile();                          // second summation level: tile sums -> fp64
 //           void write_row(double* row);                // end of a unit
 //       };

@@ -93,7 +93,14 @@ __device__ __forceinline__ int step_particle(typename Vec4<T>::type* __restrict_
                 if (flags & STEP_OPEN) {
                     v.x = fma(tx, h, v.x); v.y = fma(ty, h, v.y); v.z = fma(tz, h, v.z);
                     p.x = fma(v.x, dt, p.x); p.y = fma(v.y, dt, p.y); p.z = fma(v.z, dt, p.z);
-                    posm[i] = p;
+                    if (i == 0) {
+                        // every thread of the launch reads the mass word of record 0 (mass0 above, plan_row_mass): its
+                        // owner stores the position words only, so that word is never written while others read it
+                        T* const p0 = reinterpret_cast<T*>(posm);
+                        p0[0] = p.x; p0[1] = p.y; p0[2] = p.z;
+                    } else {
+                        posm[i] = p;
+                    }
                     if (records) stage_record(jsrc, lo + i, p.x, p.y, p.z, p.w);
                 }
                 v.w = (T)0;

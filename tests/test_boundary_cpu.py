@@ -168,3 +168,19 @@ def test_staged_sources_layout_plain_records(lib):
             assert rec_bytes == rec and off % 256 == 0 and off >= 256
             assert cap == 8 * -(-n // 8) + 1024
             assert off + cap * rec_bytes <= B.workspace_bytes(n, f64)
+
+
+def test_autograd_faces_refuse_gradients_they_do_not_compute():
+    """No silent zeros: the bulge shape alpha has no gradient slot in the C ABI, and the MMD loss is differentiated with
+    respect to the simulated clouds only.  Checked before any CUDA call, so this runs without a GPU."""
+    import torch
+    from paper_2511_22468_b200 import autograd as AG
+    posm = torch.zeros(4, 4)
+    theta8 = torch.ones(8, requires_grad=True)
+    with pytest.raises(ValueError, match="alpha"):
+        AG.leapfrog_kdk(posm, posm, theta8, torch.tensor(0.1), 1.0, 0.1, 1)
+    with pytest.raises(ValueError, match="alpha"):
+        AG.ensemble_leapfrog_kdk(posm[None], posm[None], theta8[None].detach().requires_grad_(), torch.ones(1), 1.0, 0.1, 1)
+    y = torch.zeros(3, 4, requires_grad=True)
+    with pytest.raises(ValueError, match="observed"):
+        AG.mmd2(posm, posm, y, y, (1,) * 6)

@@ -222,3 +222,32 @@ def test_sharded_driver_matches_the_oracle_leapfrog(n, world):
     # ~1e-16 relative, which the tidal tensor of close neighbours turns into more than 1e-12 S_i: compare at the GPU's x
     pair_only, Sn = O.pair_accel(got_p, cfg.G, cfg.eps)
     assert (np.linalg.norm(got_a[:, :3] - pair_only, axis=1) / Sn).max() <= 1e-12
+
+
+@pytest.mark.timeout(300)
+def test_sharded_driver_over_nccl_with_one_rank_is_bit_identical_to_the_single_gpu_leapfrog(tmp_path):
+    """DistExchange's in-place all_gather_into_tensor (input = a view of the output) on the NCCL backend.  One GPU is all
+    there is here, so the group has one rank -- the collective still goes through NCCL's launch path on the stream the
+    kernels use, and the trajectory must stay bit-identical to odisseo_leapfrog_kdk."""
+    import torch.distributed as dist
+    cfg = W.CONFIGS[1]
+    n, nsteps = 5000, 5
+    posm64, vel64 = W.make_state(cfg, n=n)
+    p0, v0 = posm64.astype(np.float32), W.vel4(vel64.astype(np.float32), np.float32)
+    pot = B.Potential.make(nfw=cfg.nfw, mn=cfg.mn)
+    posm, vel = dev(p0, np.float32), dev(v0, np.float32)
+    acc = torch.empty_like(posm)
+    B.leapfrog_kdk(posm, vel, acc, cfg.G, cfg.eps, cfg.dt, nsteps, pot, B.alloc_workspace(B.workspace_bytes(n)))
+    torch.cuda.synchronize()
+    assert not dist.is_initialized()
+    dist.init_process_group(backend="nccl", init_method="file://" + str(tmp_path / "rendezvous"), rank=0, world_size=1)
+    try:
+        ex = S.DistExchange(dist, n, 1, 0)
+        comp = S.CudaCompute(n, n, False, cfg.G, cfg.eps, cfg.dt, pot, world=1)
+        sp, sv, sa = dev(p0, np.float32), dev(v0, np.float32), torch.empty_like(posm)
+        S.sharded_leapfrog_kdk(comp, ex, sp, sv, sa, 0, n, nsteps)
+        ex.positions(sp)
+        torch.cuda.synchronize()
+    finally:
+        dist.destroy_process_group()
+    assert torch.equal(sp, posm) and torch.equal(sv, vel) and torch.equal(sa, acc)

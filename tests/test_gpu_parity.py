@@ -64,6 +64,23 @@ def test_pair_f32_ragged_sizes_unequal_masses(n):
     assert pair_ratio(acc, p64, G, eps) <= TOL_F32
 
 
+def test_pair_f32_accepted_region_of_tiny_softening_with_unequal_masses():
+    """include/odisseo.h: eps >= 1e-12 is accepted in fp32, and with unequal masses the self term m_j eps^-3 must stay below
+    FLT_MAX.  Inside the region (m <= 300 at eps = 1.1e-12: 2.3e38) the result meets the usual tolerance; just outside (one
+    mass of 500: 3.8e38 = inf, inf * 0 = NaN) the accelerations are NaN, as documented -- not silently wrong numbers."""
+    n = 700
+    posm64, _ = W.random_cloud(n, seed=4242)
+    posm64[:, 3] = np.random.Generator(np.random.PCG64(1)).uniform(100.0, 300.0, n)
+    p32, p64, G, eps = f32_inputs(posm64, 1.0, 1.1e-12)       # float32(1e-12) itself rounds below the bound
+    acc = gpu_pair(p32, G, eps, np.float32)
+    assert np.all(np.isfinite(acc)) and pair_ratio(acc, p64, G, eps) <= TOL_F32
+    p32[n // 2, 3] = 500.0
+    assert not np.all(np.isfinite(gpu_pair(p32, G, eps, np.float32)[:, :3]))
+    p32[:, 3] = 500.0                                    # equal masses: applied in fp64 after the sum, no bound
+    acc = gpu_pair(p32, G, eps, np.float32)
+    assert np.all(np.isfinite(acc)) and pair_ratio(acc, p32.astype(np.float64), G, eps) <= TOL_F32
+
+
 @pytest.mark.parametrize("n", [1, 2, 127, 1000, 1025, 4097, 6000])
 def test_pair_f64_ragged_sizes_unequal_masses(n):
     posm64, _ = W.random_cloud(n, seed=200 + n)
