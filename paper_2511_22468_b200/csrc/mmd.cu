@@ -103,7 +103,7 @@ __device__ __forceinline__ void mmd_pass(const float4* __restrict__ spos, const 
 
 // grid = (ceil(max(n, m) / 512), nsim).  Thread t of block b handles simulated points i0 = b*512 + t and i1 = i0 + 256
 // (xx and xy sums, gradient) and the observed points with the same indices (yy sum).
-// block_sums[sim][block][3] = {sum k_xx, sum k_xy, sum k_yy}.
+// block_sums[sim][block][3] = {sum k_xx, sum k_xy, sum k_yy}  (with a shared observed cloud sum k_yy is formed by sim 0 only).
 template <bool GRAD>
 __global__ void __launch_bounds__(MMD_THREADS)
 mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, const int n, const float4* __restrict__ ypos,
@@ -172,7 +172,10 @@ mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, con
         }
     }
     // ---- observed points against Y (value only) -------------------------------------------------------------------
-    if (base < m) {
+    // One observed cloud shared by every simulation (the paper's case: thousands of simulated streams against one observed
+    // stream): sum k_yy is the same number for all of them, so only simulation 0 forms it and
+    // mmd_final_kernel reads it from there -- a third of the kernel's pair work otherwise.
+    if (base < m && (!shared_y || sim == 0)) {
         f32x2 w[6];
         load_pair(YP, YV, m, w);
         double unused0[6] = {0, 0, 0, 0, 0, 0}, unused1[6] = {0, 0, 0, 0, 0, 0}, yy0, yy1;
@@ -191,14 +194,15 @@ mmd_kernel(const float4* __restrict__ xpos, const float4* __restrict__ xvel, con
 // mmd2[sim] = sum_blocks xx / n^2 + sum_blocks yy / m^2 - 2 sum_blocks xy / (n m), blocks in order.
 __global__ void __launch_bounds__(32)
 mmd_final_kernel(const double* __restrict__ block_sums, const int nblocks, const int64_t nsim, const int n, const int m,
-                 double* __restrict__ out)
+                 const int shared_y, double* __restrict__ out)
 {
     const int64_t sim = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (sim >= nsim) return;
     double xx = 0.0, xy = 0.0, yy = 0.0;
     for (int b = 0; b < nblocks; ++b) {
         const double* o = block_sums + ((size_t)sim * nblocks + b) * 3;
-        xx += o[0]; xy += o[1]; yy += o[2];
+        xx += o[0]; xy += o[1];
+        yy += shared_y ? block_sums[(size_t)b * 3 + 2] : o[2];      // shared observed cloud: simulation 0 holds sum k_yy
     }
     out[sim] = xx / ((double)n * n) + yy / ((double)m * m) - 2.0 * xy / ((double)n * m);
 }
@@ -237,7 +241,7 @@ cudaError_t launch_mmd_f32(const float* xpos, const float* xvel, int64_t n, cons
                                                             block_sums);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    mmd_final_kernel<<<(unsigned)((nsim + 31) / 32), 32, 0, stream>>>(block_sums, (int)grid.x, nsim, (int)n, (int)m, mmd2);
+    mmd_final_kernel<<<(unsigned)((nsim + 31) / 32), 32, 0, stream>>>(block_sums, (int)grid.x, nsim, (int)n, (int)m, shared_y, mmd2);
     return cudaGetLastError();
 }
 
